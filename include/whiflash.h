@@ -1,0 +1,161 @@
+/* whiflash.h — C ABI of the B200-native (sm_100a) verify-and-switch hot path of WhiFlash
+ * (arxiv/paper_2606_07710).  Citations are lines of /root/reference/PAPER.md and readings
+ * C1..C25 of DESIGN.md.
+ *
+ * Conventions
+ *  - Every call returns int: WF_OK (0) or a negative wf_status.  Nothing throws or aborts.
+ *    wf_last_error(ctx) returns a static/ctx-owned message for the last failing call.
+ *  - Pointers are DEVICE pointers unless the name ends in _host.  Tensor bases and row strides are
+ *    16-byte aligned.  bf16 tensors are passed as void* (raw bf16 bits, little endian).
+ *  - Hot calls are asynchronous on the caller's CUDA stream (a cudaStream_t passed as void*; NULL =
+ *    the legacy default stream) and never synchronise the host.  Conditions only the device can
+ *    see (page exhaustion, backlog overflow) set a sticky device status word read by
+ *    wf_poll_status.
+ *  - Ownership: the caller allocates and owns every tensor (pools, block tables, lengths, weights,
+ *    backlog, workspaces).  Handles (wf_ctx, wf_paged_kv, wf_drafter) are opaque, created and
+ *    destroyed here; they borrow the caller's pointers and own only small bookkeeping buffers
+ *    (free-page ring, pages-held counters, RoPE table, tensor maps, row plans).
+ *  - Every step of every call runs in this library's own CUDA kernels; there is no CPU path.
+ */
+#ifndef WHIFLASH_H_
+#define WHIFLASH_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  WF_OK = 0,
+  WF_ERR_INVALID_ARG = -1,
+  WF_ERR_UNSUPPORTED_SHAPE = -2,
+  WF_ERR_OUT_OF_PAGES = -3,     /* device status: a reserve could not be served; nothing was allocated */
+  WF_ERR_QUEUE_OVERFLOW = -4,   /* device status: one round's rows alone exceed backlog_cap */
+  WF_ERR_CUDA = -5
+} wf_status;
+
+#define WF_ROUTE_DIFFUSION 0
+#define WF_ROUTE_AR 1
+
+typedef struct wf_ctx wf_ctx;
+typedef struct wf_paged_kv wf_paged_kv;
+typedef struct wf_drafter wf_drafter;
+
+/* ---- lifecycle ------------------------------------------------------------------------------ */
+int wf_ctx_create(wf_ctx** out, int device_ordinal);
+int wf_ctx_destroy(wf_ctx* ctx);
+const char* wf_last_error(const wf_ctx* ctx);
+/* Copies the sticky device status word to *status_host (synchronises `stream`) and clears it. */
+int wf_poll_status(wf_ctx* ctx, void* stream, int* status_host);
+/* Number of kernels this library has launched through ctx since creation (host counter). */
+int64_t wf_launch_count(const wf_ctx* ctx);
+
+/* ---- paged KV cache + block table (BASELINE.json north_star "plus a paged-KV block table";
+ *      the paper itself uses the HF cache).  The target cache and every drafter
+ *      cache are instances.
+ * Pools: bf16 [n_layers][num_pages][n_kv_heads][page_size][head_dim], K and V separate.
+ * block_table int32 [max_seqs][max_pages_per_seq] (-1 = no page); seq_len int32 [max_seqs] =
+ * tokens that are final in the cache.  Both are caller-owned and may be written by the caller
+ * between calls (e.g. to set the initial context after a reserve).
+ * Allocation order (reading C24): the free list is an explicit ordered ring initialised from
+ * free_pages_host; one reserve call serves sequences in ascending index, each taking consecutive
+ * ring entries from the head; released pages go to the tail in block-table order. */
+typedef struct {
+  int n_layers, n_kv_heads, head_dim, page_size, num_pages, max_seqs, max_pages_per_seq;
+} wf_kv_shape;
+
+int wf_kv_create(wf_ctx* ctx, const wf_kv_shape* shape, void* k_pool, void* v_pool,
+                 int32_t* block_table, int32_t* seq_len,
+                 const int32_t* free_pages_host, int n_free, wf_paged_kv** out);
+int wf_kv_destroy(wf_paged_kv* kv);
+/* Grow block tables so that sequence b in [0,B) can hold seq_len[b] + add_tokens[b] tokens.
+ * If the ring cannot serve the whole call, nothing is allocated and the device status becomes
+ * WF_ERR_OUT_OF_PAGES.  seq_len is not changed. */
+int wf_kv_reserve(wf_paged_kv* kv, const int32_t* add_tokens, int B, void* stream);
+/* Return all pages of sequence `seq` to the ring tail; seq_len[seq] = 0. */
+int wf_kv_release_seq(wf_paged_kv* kv, int seq, void* stream);
+/* Device pointer to the int32 [max_seqs] pages-held counters (library-owned; for inspection). */
+const int32_t* wf_kv_pages_held(const wf_paged_kv* kv);
+
+/* ---- (a) verification attention for ONE target layer -------------------------------------------
+ * PAPER.md:65 (§3.2 "returned to the target model for parallel verification"); north_star (a).
+ * For sequence b with ctx_b = target_kv.seq_len[b], rows i in [0, q_b), q_b = q_indptr[b+1] -
+ * q_indptr[b] <= max_q_len, query head h, kv head g = h / (n_q_heads / n_kv_heads) (C11):
+ *     s_j = <Q[i,h,:], K[b,j,g,:]> * sm_scale, j = 0 .. ctx_b + i      (causal within block, C10)
+ *     O[i,h,:] = sum_j softmax(s)_j V[b,j,g,:]                          (fp32 accumulate, C13)
+ * The block's own K/V must already be in the cache at positions ctx_b .. ctx_b+q_b-1 (C10).
+ * q, out: bf16 [sum_q][n_q_heads][head_dim].  workspace: >= wf_verify_attn_workspace_bytes.
+ * Supported: head_dim 64 or 128; page_size 16; q_b * group <= 64 (group = n_q_heads/n_kv_heads). */
+int wf_verify_attn(wf_ctx* ctx, const wf_paged_kv* target_kv, int layer,
+                   const void* q, const int32_t* q_indptr, int B, int n_q_heads, int max_q_len,
+                   float sm_scale, void* out, void* workspace, size_t workspace_bytes, void* stream);
+size_t wf_verify_attn_workspace_bytes(const wf_kv_shape* shape, int B, int n_q_heads, int max_q_len);
+
+/* ---- (b) accept + bonus + entropy + route -------------------------------------------------------
+ * PAPER.md:65, 75-81 (§3.3.1), 135; readings C1-C9.  Per sequence b (block rows r0..r0+gamma):
+ *     g_i = argmax_v logits[r0+i][v] (lowest id on ties);  a = longest prefix with
+ *     draft_tokens[r0+j] == g_{j-1}, j = 1..a;  bonus = g_a;  n_commit = a+1;
+ *     H = Shannon entropy (nats) of softmax(logits[r0+a]);  route = AR(1) if H > tau else 0.
+ * If target_kv != NULL, target_kv.seq_len[b] += n_commit[b].
+ * tau: device fp32 [B], or [1] if tau_is_scalar.  logits rows must be finite or -inf (C23).
+ * max_q_len: host upper bound on q_b (<= 64) that sizes the grid.
+ * workspace: >= wf_accept_workspace_bytes(B * max_q_len, V); contents need no initialisation. */
+int wf_accept_entropy_route(wf_ctx* ctx, const float* logits, int V, const int32_t* draft_tokens,
+                            const int32_t* q_indptr, int B, int max_q_len, const float* tau,
+                            int tau_is_scalar, int32_t* accept_len, int32_t* bonus_token,
+                            float* entropy, int32_t* route, int32_t* n_commit,
+                            wf_paged_kv* target_kv, void* workspace, size_t workspace_bytes,
+                            void* stream);
+size_t wf_accept_workspace_bytes(int sum_q, int V);
+
+/* ---- drafter descriptor -------------------------------------------------------------------------
+ * PAPER.md:119; readings C14-C18: every layer l projects the same hidden rows X with its own
+ * W_K[l], W_V[l]: bf16 [hidden][n_kv_heads*head_dim] (K = X W; column c -> head c / D, lane c % D).
+ * w_k_host_ptrs / w_v_host_ptrs: HOST arrays of n_layers DEVICE pointers.
+ * backlog: bf16 [max_seqs][backlog_cap][hidden]; backlog_len: int32 [max_seqs] (caller-owned,
+ * zero-initialised by the caller).  RoPE: rotate-half pairs (r, r + D/2), angle pos * theta^(-2r/D),
+ * cos/sin table [max_pos][D/2] built in fp64 on the host at creation (C17). */
+typedef struct {
+  int n_layers, hidden, n_kv_heads, head_dim;
+  float rope_theta;
+  int max_pos;
+  int backlog_cap;
+} wf_drafter_shape;
+
+int wf_drafter_create(wf_ctx* ctx, const wf_drafter_shape* shape,
+                      const void* const* w_k_host_ptrs, const void* const* w_v_host_ptrs,
+                      wf_paged_kv* drafter_kv, void* backlog, int32_t* backlog_len,
+                      wf_drafter** out);
+int wf_drafter_destroy(wf_drafter* d);
+
+/* ---- (c) KV-only prefill (eager) ----------------------------------------------------------------
+ * PAPER.md:119 (§3.4 "KV-only Prefill"), :206.  For each b in [0,B): rows t = 0..n_rows[b]-1 of the
+ * block (hidden[q_indptr[b]+t]) are projected by every layer's W_K (+RoPE at position
+ * p0+t, p0 = drafter_kv.seq_len[seq_ids[b]]) and W_V, rounded to bf16 (RNE) and written at logical
+ * positions p0+t through the drafter's block table (pages reserved first, C24);
+ * drafter_kv.seq_len[seq] += n_rows[b].  No attention, MLP or LM head runs.
+ * seq_ids may be NULL (= identity).  n_rows[b] <= max_rows (host upper bound that sizes grids). */
+int wf_kv_only_prefill(wf_ctx* ctx, wf_drafter* d, const void* hidden, const int32_t* q_indptr,
+                       const int32_t* n_rows, const int32_t* seq_ids, int B, int max_rows,
+                       void* stream);
+
+/* ---- (d) Lazy Catch-up --------------------------------------------------------------------------
+ * PAPER.md:117 (§3.4 "Lazy Catch-up"), :204.  enqueue: for each b with idle_mask[b] != 0 append rows
+ * 0..n_rows[b]-1 of the block to the FIFO backlog of sequence seq_ids[b]; no projection work is
+ * done.  If the rows would not fit (len + n > backlog_cap) that sequence's backlog is flushed first
+ * (one batched prefill for all such sequences of the call), then the rows are enqueued: rows are
+ * never dropped or reordered (C20).  n > backlog_cap sets WF_ERR_QUEUE_OVERFLOW and skips the rows.
+ * flush: one batched KV-only prefill (same device code as (c)) over the whole backlog of every
+ * sequence b in [0,B) with flush_mask[b] != 0 (NULL = all); backlog_len <- 0 for those.
+ * Postcondition: the drafter cache is bit-identical to eager per-round appends. */
+int wf_lazy_catchup_enqueue(wf_ctx* ctx, wf_drafter* d, const void* hidden, const int32_t* q_indptr,
+                            const int32_t* n_rows, const int32_t* seq_ids, const int32_t* idle_mask,
+                            int B, int max_rows, void* stream);
+int wf_lazy_catchup_flush(wf_ctx* ctx, wf_drafter* d, const int32_t* flush_mask, int B, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* WHIFLASH_H_ */

@@ -1,0 +1,241 @@
+// (b) accept + bonus + entropy + route: ONE vectorised sweep over the block's target logits.
+// PAPER.md:65, 75-81 (§3.3.1), 135; readings C1-C9, C23.
+//
+// Grid (n_chunks, max_q_len, B).  A CTA owns one ACC_CHUNK-float slice of one logits row: it loads
+// the slice with 16-byte loads into registers, block-reduces (max, lowest argmax), then, relative
+// to the slice max, Z_c = sum e^{z-m_c} and S_c = sum e^{z-m_c}(z-m_c), and writes a 16-byte
+// partial.  The last CTA of a sequence (self-resetting counter) combines the partials per row
+// (argmax g_i), walks the draft tokens for the accepted prefix a, combines row a's (m_c,Z_c,S_c)
+// in fp64 into H = ln Z - S/Z, thresholds it, and advances the target cache length.
+#include "wf_internal.cuh"
+
+namespace {
+
+constexpr int ACC_THREADS = 256;
+constexpr int ACC_VEC_PER_THREAD = 8;                              // 8 x float4 in flight per thread
+constexpr int ACC_CHUNK = ACC_THREADS * ACC_VEC_PER_THREAD * 4;    // 8192 floats = 32 KB per CTA
+constexpr int ACC_MAX_Q = 64;
+
+struct __align__(16) AccPartial {
+  float m;      // slice max (-inf if the slice carries no mass)
+  int idx;      // lowest index attaining m
+  float Z;      // sum e^{z-m}
+  float S;      // sum e^{z-m} (z-m)
+};
+
+__device__ __forceinline__ float4 ld_stream(const float4* p) {
+  float4 r;
+  asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0,%1,%2,%3}, [%4];"
+               : "=f"(r.x), "=f"(r.y), "=f"(r.z), "=f"(r.w) : "l"(p));
+  return r;
+}
+
+__device__ __forceinline__ void argmax_merge(float& m, int& i, float om, int oi) {
+  if (om > m || (om == m && oi < i)) { m = om; i = oi; }
+}
+
+template <bool VEC>
+__global__ void __launch_bounds__(ACC_THREADS)
+wf_accept_kernel(const float* __restrict__ logits, int V, int n_chunks, const int32_t* __restrict__ draft_tokens,
+                 const int32_t* __restrict__ q_indptr, const float* __restrict__ tau, int tau_is_scalar,
+                 int32_t* __restrict__ accept_len, int32_t* __restrict__ bonus_token, float* __restrict__ entropy,
+                 int32_t* __restrict__ route, int32_t* __restrict__ n_commit, int32_t* __restrict__ kv_seq_len,
+                 AccPartial* __restrict__ partials, unsigned int* __restrict__ counters) {
+  const int b = blockIdx.z, i = blockIdx.y, chunk = blockIdx.x;
+  const int r0 = q_indptr[b];
+  const int q_b = q_indptr[b + 1] - r0;
+  if (q_b == 0 && i == 0 && blockIdx.x == 0 && threadIdx.x == 0) {
+    // empty block: nothing verified, nothing committed
+    accept_len[b] = 0; bonus_token[b] = 0; entropy[b] = 0.f; route[b] = 0; n_commit[b] = 0;
+  }
+  if (i >= q_b) return;                                   // whole CTA exits together
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+  const float* row = logits + (size_t)(r0 + i) * V;
+  const int c0 = chunk * ACC_CHUNK;
+  const int n_here = min(ACC_CHUNK, V - c0);
+
+  float v[ACC_VEC_PER_THREAD * 4];
+  if (VEC) {
+    const float4* p = reinterpret_cast<const float4*>(row + c0);
+#pragma unroll
+    for (int k = 0; k < ACC_VEC_PER_THREAD; ++k) {
+      const int e = (k * ACC_THREADS + tid) * 4;
+      float4 x = make_float4(-INFINITY, -INFINITY, -INFINITY, -INFINITY);
+      if (e < n_here) x = ld_stream(p + k * ACC_THREADS + tid);     // V % 4 == 0: all or nothing
+      v[4 * k + 0] = x.x; v[4 * k + 1] = x.y; v[4 * k + 2] = x.z; v[4 * k + 3] = x.w;
+    }
+  } else {
+#pragma unroll
+    for (int k = 0; k < ACC_VEC_PER_THREAD; ++k)
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        const int e = (k * ACC_THREADS + tid) * 4 + j;
+        v[4 * k + j] = e < n_here ? __ldg(row + c0 + e) : -INFINITY;
+      }
+  }
+
+  // thread-local max; indices ascend with (k, j), strict > keeps the lowest index on ties (C7)
+  float m = -INFINITY;
+  int mi = 0x7fffffff;
+#pragma unroll
+  for (int k = 0; k < ACC_VEC_PER_THREAD; ++k)
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      const int e = c0 + (k * ACC_THREADS + tid) * 4 + j;
+      if (v[4 * k + j] > m) { m = v[4 * k + j]; mi = e; }
+    }
+#pragma unroll
+  for (int d = 16; d > 0; d >>= 1) {
+    float om = __shfl_xor_sync(0xffffffffu, m, d);
+    int oi = __shfl_xor_sync(0xffffffffu, mi, d);
+    argmax_merge(m, mi, om, oi);
+  }
+  __shared__ float s_m[ACC_THREADS / 32];
+  __shared__ int s_i[ACC_THREADS / 32];
+  __shared__ float s_z[ACC_THREADS / 32], s_s[ACC_THREADS / 32];
+  if (lane == 0) { s_m[wid] = m; s_i[wid] = mi; }
+  __syncthreads();
+  m = s_m[0]; mi = s_i[0];
+#pragma unroll
+  for (int w = 1; w < ACC_THREADS / 32; ++w) argmax_merge(m, mi, s_m[w], s_i[w]);
+
+  // Z_c, S_c relative to the slice max; -inf entries contribute 0 (0 * ln 0 := 0, C23)
+  float Z = 0.f, S = 0.f;
+  if (m > -INFINITY) {
+    constexpr float LOG2E = 1.4426950408889634f;
+#pragma unroll
+    for (int k = 0; k < ACC_VEC_PER_THREAD * 4; ++k) {
+      const float d = v[k] - m;
+      const float e = exp2f(d * LOG2E);
+      Z += e;
+      S += (v[k] > -INFINITY) ? e * d : 0.f;
+    }
+  }
+#pragma unroll
+  for (int d = 16; d > 0; d >>= 1) {
+    Z += __shfl_xor_sync(0xffffffffu, Z, d);
+    S += __shfl_xor_sync(0xffffffffu, S, d);
+  }
+  if (lane == 0) { s_z[wid] = Z; s_s[wid] = S; }
+  __syncthreads();
+
+  __shared__ bool s_last;
+  if (tid == 0) {
+    float Zt = 0.f, St = 0.f;
+#pragma unroll
+    for (int w = 0; w < ACC_THREADS / 32; ++w) { Zt += s_z[w]; St += s_s[w]; }
+    AccPartial p; p.m = m; p.idx = mi; p.Z = Zt; p.S = St;
+    partials[(size_t)(r0 + i) * n_chunks + chunk] = p;
+    __threadfence();
+    const unsigned int total = (unsigned int)(q_b * n_chunks);
+    const unsigned int old = atomicAdd(&counters[b], 1u);
+    s_last = (old == total - 1);
+    if (s_last) counters[b] = 0;                          // self-reset for the next call
+  }
+  __syncthreads();
+  if (!s_last) return;
+  __threadfence();
+
+  // ---- finalise sequence b (one CTA) ----
+  __shared__ int s_g[ACC_MAX_Q];
+  __shared__ int s_a;
+  for (int r = wid; r < q_b; r += ACC_THREADS / 32) {     // one warp per row: argmax over slices
+    float rm = -INFINITY;
+    int ri = 0x7fffffff;
+    for (int c = lane; c < n_chunks; c += 32) {
+      const AccPartial* pp = &partials[(size_t)(r0 + r) * n_chunks + c];
+      const float pm = __ldcg(&pp->m);
+      const int pi = __ldcg(&pp->idx);
+      argmax_merge(rm, ri, pm, pi);
+    }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) {
+      float om = __shfl_xor_sync(0xffffffffu, rm, d);
+      int oi = __shfl_xor_sync(0xffffffffu, ri, d);
+      argmax_merge(rm, ri, om, oi);
+    }
+    if (lane == 0) s_g[r] = ri;
+  }
+  __syncthreads();
+  if (tid == 0) {                                          // longest accepted prefix (C6)
+    const int gamma = q_b - 1;
+    int a = 0;
+    while (a < gamma && draft_tokens[r0 + a + 1] == s_g[a]) ++a;
+    s_a = a;
+  }
+  __syncthreads();
+  if (wid == 0) {                                          // entropy of row a, fp64 combine (C3, C4)
+    const int a = s_a;
+    const AccPartial* pr = &partials[(size_t)(r0 + a) * n_chunks];
+    float gm = -INFINITY;
+    for (int c = lane; c < n_chunks; c += 32) gm = fmaxf(gm, __ldcg(&pr[c].m));
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) gm = fmaxf(gm, __shfl_xor_sync(0xffffffffu, gm, d));
+    double Zd = 0.0, Sd = 0.0;
+    for (int c = lane; c < n_chunks; c += 32) {
+      const float pm = __ldcg(&pr[c].m);
+      if (pm > -INFINITY) {
+        const double dm = (double)pm - (double)gm;
+        const double w = exp(dm);
+        const double Zc = (double)__ldcg(&pr[c].Z), Sc = (double)__ldcg(&pr[c].S);
+        Zd += Zc * w;
+        Sd += w * (Sc + dm * Zc);
+      }
+    }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) {
+      Zd += __shfl_xor_sync(0xffffffffu, Zd, d);
+      Sd += __shfl_xor_sync(0xffffffffu, Sd, d);
+    }
+    if (lane == 0) {
+      const float H = (float)(log(Zd) - Sd / Zd);
+      const float t = tau_is_scalar ? tau[0] : tau[b];
+      accept_len[b] = a;
+      bonus_token[b] = s_g[a];
+      n_commit[b] = a + 1;
+      entropy[b] = H;
+      route[b] = (H > t) ? WF_ROUTE_AR : WF_ROUTE_DIFFUSION;     // C1, C2
+      if (kv_seq_len) kv_seq_len[b] += a + 1;
+    }
+  }
+}
+
+}  // namespace
+
+extern "C" size_t wf_accept_workspace_bytes(int sum_q, int V) {
+  if (sum_q <= 0 || V <= 0) return 16;
+  const size_t n_chunks = ((size_t)V + ACC_CHUNK - 1) / ACC_CHUNK;
+  return (size_t)sum_q * n_chunks * sizeof(AccPartial);
+}
+
+extern "C" int wf_accept_entropy_route(wf_ctx* ctx, const float* logits, int V, const int32_t* draft_tokens,
+                                       const int32_t* q_indptr, int B, int max_q_len, const float* tau,
+                                       int tau_is_scalar, int32_t* accept_len, int32_t* bonus_token,
+                                       float* entropy, int32_t* route, int32_t* n_commit,
+                                       wf_paged_kv* target_kv, void* workspace, size_t workspace_bytes,
+                                       void* stream) {
+  if (!ctx) return WF_ERR_INVALID_ARG;
+  WF_REQUIRE(ctx, logits && draft_tokens && q_indptr && tau && accept_len && bonus_token && entropy && route &&
+                 n_commit && workspace, WF_ERR_INVALID_ARG, "wf_accept_entropy_route: null argument");
+  WF_REQUIRE(ctx, V > 0 && B >= 0 && B <= ctx->n_counters && B <= 65535, WF_ERR_INVALID_ARG,
+             "wf_accept_entropy_route: bad V or B");
+  WF_REQUIRE(ctx, max_q_len >= 0 && max_q_len <= ACC_MAX_Q, WF_ERR_UNSUPPORTED_SHAPE,
+             "wf_accept_entropy_route: max_q_len must be <= %d", ACC_MAX_Q);
+  WF_REQUIRE(ctx, !target_kv || B <= target_kv->s.max_seqs, WF_ERR_INVALID_ARG,
+             "wf_accept_entropy_route: B exceeds the cache's max_seqs");
+  if (B == 0) return WF_OK;
+  cudaStream_t st = (cudaStream_t)stream;
+  if (max_q_len == 0) max_q_len = 1;                       // still launch: empty blocks get zeroed outputs
+  const int n_chunks = (V + ACC_CHUNK - 1) / ACC_CHUNK;
+  WF_REQUIRE(ctx, workspace_bytes >= wf_accept_workspace_bytes(B * max_q_len, V), WF_ERR_INVALID_ARG, "wf_accept_entropy_route: workspace too small");
+  dim3 grid(n_chunks, max_q_len, B);
+  int32_t* kv_len = target_kv ? target_kv->seq_len : nullptr;
+  const bool vec = (V % 4 == 0) && ((uintptr_t)logits % 16 == 0);
+  if (vec)
+    wf_accept_kernel<true><<<grid, ACC_THREADS, 0, st>>>(logits, V, n_chunks, draft_tokens, q_indptr, tau,
+        tau_is_scalar, accept_len, bonus_token, entropy, route, n_commit, kv_len, (AccPartial*)workspace, ctx->d_counters);
+  else
+    wf_accept_kernel<false><<<grid, ACC_THREADS, 0, st>>>(logits, V, n_chunks, draft_tokens, q_indptr, tau,
+        tau_is_scalar, accept_len, bonus_token, entropy, route, n_commit, kv_len, (AccPartial*)workspace, ctx->d_counters);
+  return wf_check_launch(ctx, "wf_accept_kernel");
+}

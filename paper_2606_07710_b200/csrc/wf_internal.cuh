@@ -1,0 +1,148 @@
+// Internal definitions shared by the CUDA translation units of libwhiflash (product path only;
+// nothing under oracle/ includes or links this).
+#pragma once
+
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+
+#include "whiflash.h"
+
+struct wf_ctx {
+  int device;
+  int sm_count;
+  int* d_status;               // sticky device status word (0 = ok, else a negative wf_status)
+  unsigned int* d_counters;    // self-resetting "blocks done" counters for the accept sweep
+  unsigned int* d_counters_attn; // same, per (sequence, kv head), for the split-KV combine
+  int n_counters;
+  int64_t launches;            // kernels launched through this ctx (host counter)
+  char err[256];
+};
+
+struct wf_paged_kv {
+  wf_ctx* ctx;
+  wf_kv_shape s;
+  __nv_bfloat16* k_pool;
+  __nv_bfloat16* v_pool;
+  int32_t* block_table;        // caller-owned [max_seqs][max_pages_per_seq]
+  int32_t* seq_len;            // caller-owned [max_seqs]
+  int32_t* pages_held;         // library-owned [max_seqs]
+  int32_t* free_ring;          // library-owned [num_pages]
+  int32_t* ring_state;         // library-owned [2]: head, count
+  int32_t* scratch;            // library-owned [2*max_seqs]: need, offset
+};
+
+// Device-side view of a paged KV cache passed by value to kernels.
+struct KvView {
+  __nv_bfloat16* k_pool;
+  __nv_bfloat16* v_pool;
+  int32_t* block_table;
+  int32_t* seq_len;
+  int32_t* pages_held;
+  int32_t* free_ring;
+  int32_t* ring_state;
+  int32_t* scratch;
+  int n_layers, n_kv_heads, head_dim, page_size, num_pages, max_seqs, max_pages_per_seq;
+};
+
+static inline KvView kv_view(const wf_paged_kv* kv) {
+  KvView v;
+  v.k_pool = kv->k_pool; v.v_pool = kv->v_pool;
+  v.block_table = kv->block_table; v.seq_len = kv->seq_len;
+  v.pages_held = kv->pages_held; v.free_ring = kv->free_ring;
+  v.ring_state = kv->ring_state; v.scratch = kv->scratch;
+  v.n_layers = kv->s.n_layers; v.n_kv_heads = kv->s.n_kv_heads; v.head_dim = kv->s.head_dim;
+  v.page_size = kv->s.page_size; v.num_pages = kv->s.num_pages; v.max_seqs = kv->s.max_seqs;
+  v.max_pages_per_seq = kv->s.max_pages_per_seq;
+  return v;
+}
+
+int wf_set_error(wf_ctx* ctx, int code, const char* fmt, ...);
+int wf_check_launch(wf_ctx* ctx, const char* what);   // cudaGetLastError -> WF_ERR_CUDA; counts the launch
+
+#define WF_REQUIRE(ctx, cond, code, ...)                         \
+  do {                                                           \
+    if (!(cond)) return wf_set_error((ctx), (code), __VA_ARGS__); \
+  } while (0)
+
+#define WF_CUDA(ctx, expr)                                                                   \
+  do {                                                                                       \
+    cudaError_t e__ = (expr);                                                                \
+    if (e__ != cudaSuccess)                                                                  \
+      return wf_set_error((ctx), WF_ERR_CUDA, "%s: %s", #expr, cudaGetErrorString(e__));     \
+  } while (0)
+
+// ---------------------------------------------------------------------------------------------
+// Block-wide page reservation (reading C24), callable from any kernel that runs as ONE block.
+// add(b) gives the tokens sequence slot `seq(b)` must additionally hold, b in [0,B).
+// Sequences are served in ascending b; each takes consecutive ring entries from the head.
+// If the ring cannot serve the whole call (or a sequence would exceed max_pages_per_seq), nothing
+// is allocated, *status becomes WF_ERR_OUT_OF_PAGES and false is returned (block-uniform).
+// Requires blockDim.x a multiple of 32, <= 1024.
+// ---------------------------------------------------------------------------------------------
+template <typename AddFn, typename SeqFn>
+__device__ inline bool kv_reserve_block(const KvView& kv, int B, AddFn add, SeqFn seq, int* status) {
+  __shared__ int s_warp[32];
+  __shared__ int s_carry;
+  __shared__ int s_bad;
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5, nw = blockDim.x >> 5;
+  if (tid == 0) { s_carry = 0; s_bad = 0; }
+  __syncthreads();
+  int* need = kv.scratch;
+  int* off = kv.scratch + kv.max_seqs;
+  for (int base = 0; base < B; base += blockDim.x) {
+    const int b = base + tid;
+    int n = 0;
+    if (b < B) {
+      const int s = seq(b);
+      const int want = (kv.seq_len[s] + add(b) + kv.page_size - 1) / kv.page_size;
+      if (want > kv.max_pages_per_seq) s_bad = 1;
+      n = max(0, want - kv.pages_held[s]);
+    }
+    int x = n;                                   // inclusive warp scan
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+      int y = __shfl_up_sync(0xffffffffu, x, d);
+      if (lane >= d) x += y;
+    }
+    if (lane == 31) s_warp[wid] = x;
+    __syncthreads();
+    if (wid == 0) {
+      int w = lane < nw ? s_warp[lane] : 0;
+#pragma unroll
+      for (int d = 1; d < 32; d <<= 1) {
+        int y = __shfl_up_sync(0xffffffffu, w, d);
+        if (lane >= d) w += y;
+      }
+      s_warp[lane] = w;                          // inclusive scan of warp totals
+    }
+    __syncthreads();
+    const int warp_excl = wid == 0 ? 0 : s_warp[wid - 1];
+    if (b < B) { need[b] = n; off[b] = s_carry + warp_excl + x - n; }
+    __syncthreads();
+    if (tid == 0) s_carry += s_warp[nw - 1];
+    __syncthreads();
+  }
+  const int total = s_carry;
+  const int head = kv.ring_state[0], count = kv.ring_state[1];
+  if (s_bad || total > count) {
+    if (tid == 0) *status = WF_ERR_OUT_OF_PAGES;
+    return false;
+  }
+  for (int b = wid; b < B; b += nw) {            // one warp per sequence copies its ring entries
+    const int s = seq(b);
+    const int n = need[b], o = off[b], held = kv.pages_held[s];
+    for (int i = lane; i < n; i += 32)
+      kv.block_table[(size_t)s * kv.max_pages_per_seq + held + i] = kv.free_ring[(head + o + i) % kv.num_pages];
+    __syncwarp();
+    if (lane == 0 && n > 0) kv.pages_held[s] = held + n;
+  }
+  __syncthreads();
+  if (tid == 0) {
+    kv.ring_state[0] = (head + total) % kv.num_pages;
+    kv.ring_state[1] = count - total;
+  }
+  __syncthreads();
+  return true;
+}

@@ -1,0 +1,234 @@
+"""GPU parity (through the C-ABI) for the paged-KV block table, (b) accept/entropy/route and
+(a) verification attention, element by element against oracle/ on the same seeded inputs.
+
+Tolerances (BASELINE.json north_star): integers bit-exact (route exempt only when |H - tau| < 1e-4,
+counted separately); entropy 1e-3 absolute; attention max-abs 2e-2 and relative L2 5e-3.
+"""
+
+import math
+
+import numpy as np
+import pytest
+
+from oracle import accept_route, verify_attn
+from paper_2606_07710_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+ATTN_MAX_ABS = 2e-2
+ATTN_REL_L2 = 5e-3
+ENTROPY_ABS = 1e-3
+ROUTE_BAND = 1e-4
+
+
+@pytest.fixture(scope="module")
+def wf():
+    import torch
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device"
+    from paper_2606_07710_b200 import binding
+    ctx = binding.Ctx(0)
+    yield binding, ctx
+    ctx.close()
+
+
+# ------------------------------------------------------------------------------------ block table
+def test_block_table_matches_oracle(wf):
+    import torch
+    from tests import gpu_harness as H
+    binding, ctx = wf
+    g = synth.rng(7, 1)
+    P, S = 300, 6
+    free = synth.draw_free_list(P, g, True)
+    pair = H.KvPair(ctx, 1, 2, 64, P, S, 40, free)
+    pair.reserve([100, 0, 17, 16, 1, 250])
+    pair.assert_tables_equal()
+    pair.set_seq_len([100, 0, 17, 16, 1, 250])
+    pair.reserve([5, 3, 0, 1, 15, 16])                     # grows only where a page boundary is crossed
+    pair.assert_tables_equal()
+    # release and reuse: pages go to the ring tail in block-table order (C24)
+    pair.oracle.release_seq(0)
+    pair.gpu.release_seq(0)
+    pair.oracle.release_seq(5)
+    pair.gpu.release_seq(5)
+    pair.assert_tables_equal()
+    pair.reserve([300, 10, 0, 0, 0, 40])
+    pair.assert_tables_equal()
+    assert ctx.poll_status() == 0
+    # exhaustion: nothing allocated, sticky status (oracle raises)
+    before = pair.block_table.clone()
+    pair.gpu.reserve(H.i32([16 * 39] * 6), 6)              # 6 x 39 pages > 300 pages in the pool
+    torch.cuda.synchronize()
+    assert torch.equal(before, pair.block_table)
+    st = ctx.poll_status()
+    assert st == binding.WF_ERR_OUT_OF_PAGES
+    assert ctx.poll_status() == 0
+    pair.close()
+
+
+# ------------------------------------------------------------------------------ accept / route
+def _run_accept(binding, ctx, logits, drafts, q_indptr, tau, max_q):
+    import torch
+    from tests import gpu_harness as H
+    B = len(q_indptr) - 1
+    V = logits.shape[1]
+    d_logits = H.f32(logits)
+    outs = {k: torch.full((B,), -7, dtype=torch.int32, device="cuda") for k in ("accept_len", "bonus_token", "route", "n_commit")}
+    ent = torch.full((B,), -7.0, dtype=torch.float32, device="cuda")
+    tau_arr = np.atleast_1d(np.asarray(tau, dtype=np.float32))
+    ws = torch.empty(binding.wf_accept_workspace_bytes(B * max_q, V), dtype=torch.uint8, device="cuda")
+    binding.wf_accept_entropy_route(ctx, d_logits, V, H.i32(drafts), H.i32(q_indptr), B, max_q, H.f32(tau_arr),
+                                    len(tau_arr) == 1, outs["accept_len"], outs["bonus_token"], ent, outs["route"],
+                                    outs["n_commit"], None, ws)
+    torch.cuda.synchronize()
+    res = {k: v.cpu().numpy() for k, v in outs.items()}
+    res["entropy"] = ent.cpu().numpy()
+    return res
+
+
+def _check_accept(res, want, tau):
+    B = len(want["accept_len"])
+    tau = np.broadcast_to(np.asarray(tau, dtype=np.float64), (B,))
+    for k in ("accept_len", "bonus_token", "n_commit"):
+        np.testing.assert_array_equal(res[k], want[k], err_msg=k)
+    assert np.abs(res["entropy"].astype(np.float64) - want["entropy"]).max() <= ENTROPY_ABS
+    near = np.abs(want["entropy"] - tau) < ROUTE_BAND
+    np.testing.assert_array_equal(res["route"][~near], want["route"][~near])
+    return int(near.sum())
+
+
+@pytest.mark.parametrize("seed", range(16))
+def test_accept_cfg1_tiny(wf, seed):
+    """configs[0]: vocab 4096, gamma 7, planted prefix uniform 0..7, spike puts H on both sides of tau."""
+    binding, ctx = wf
+    wl = synth.WORKLOADS[0]
+    g = synth.rng(wl.seed, 1000 + seed)
+    u = synth.draw_accept_prefix(g, [7])
+    spike = g.uniform(0.0, 10.0, size=1)
+    logits, drafts, q_indptr, _ = synth.make_logits_block(g, [8], wl.shapes.vocab, wl.shapes.logit_sigma, u, spike)
+    want = accept_route.accept_entropy_route(logits, drafts, q_indptr, wl.shapes.tau)
+    assert want["accept_len"][0] == u[0]
+    res = _run_accept(binding, ctx, logits, drafts, q_indptr, wl.shapes.tau, 8)
+    _check_accept(res, want, wl.shapes.tau)
+
+
+def test_accept_8b_vocab_mixed_gamma(wf):
+    """vocab 151936 (19 slices, ragged last slice), mixed gamma 7/15, an empty block, per-sequence tau."""
+    binding, ctx = wf
+    g = synth.rng(synth.SEED_BASE + 1, 77)
+    q_lens = [16, 8, 0, 16, 8, 1]
+    u = [15, 3, 0, 0, 7, 0]
+    spike = [6.0, 0.0, 0.0, 9.0, 4.5, 5.0]
+    logits, drafts, q_indptr, _ = synth.make_logits_block(g, q_lens, 151936, 3.0, u, spike)
+    tau = np.array([2.0, 2.0, 2.0, 1.0, 7.0, 2.0], dtype=np.float32)
+    want = accept_route.accept_entropy_route(logits, drafts, q_indptr, tau)
+    res = _run_accept(binding, ctx, logits, drafts, q_indptr, tau, 16)
+    _check_accept(res, want, tau)
+    assert set(want["route"].tolist()) == {0, 1}, "the case must exercise both routes"
+    assert res["n_commit"][2] == 0 and res["accept_len"][2] == 0
+
+
+def test_accept_edge_rows(wf):
+    """-inf (masked vocabulary), exact ties (lowest id wins), V % 4 != 0 (scalar path), closed forms."""
+    binding, ctx = wf
+    V = 1003
+    logits = np.full((4, V), -np.inf, dtype=np.float32)
+    logits[0, [5, 900]] = 1.5                      # two equal maxima, rest -inf: H = ln 2, argmax = 5
+    logits[1, :] = 0.25                            # constant row: H = ln V, argmax = 0
+    logits[2, 77] = 3.0                            # one-hot: H = 0
+    logits[3, :] = np.linspace(-3, 3, V, dtype=np.float32)
+    drafts = np.array([0, 5, 0, 77], dtype=np.int32)   # row1 draft = g_0 = 5, row2 draft 0 = g_1, row3 draft 77 = g_2
+    q_indptr = np.array([0, 4], dtype=np.int32)
+    want = accept_route.accept_entropy_route(logits, drafts, q_indptr, 2.0)
+    assert want["accept_len"][0] == 3
+    res = _run_accept(binding, ctx, logits, drafts, q_indptr, 2.0, 4)
+    _check_accept(res, want, 2.0)
+    for rows, H_want in (([0], math.log(2.0)), ([1], math.log(V)), ([2], 0.0)):
+        r = _run_accept(binding, ctx, logits[rows], np.zeros(1, np.int32), np.array([0, 1], np.int32), 2.0, 1)
+        assert abs(float(r["entropy"][0]) - H_want) <= ENTROPY_ABS
+
+
+def test_accept_advances_target_len(wf):
+    import torch
+    from tests import gpu_harness as H
+    binding, ctx = wf
+    pair = H.make_kv_pair(ctx, [100, 37], [8, 8], 1, 2, 64, seed=5, fill=False)
+    g = synth.rng(11, 3)
+    logits, drafts, q_indptr, _ = synth.make_logits_block(g, [8, 8], 4096, 2.0, [4, 7], [0.0, 8.0])
+    want = accept_route.accept_entropy_route(logits, drafts, q_indptr, 2.0, kv=pair.oracle)
+    B, V = 2, 4096
+    o = [torch.zeros(B, dtype=torch.int32, device="cuda") for _ in range(4)]
+    ent = torch.zeros(B, dtype=torch.float32, device="cuda")
+    ws = torch.empty(binding.wf_accept_workspace_bytes(16, V), dtype=torch.uint8, device="cuda")
+    for _ in range(2):                                  # second call checks the self-resetting counters
+        pair.set_seq_len([100, 37])
+        binding.wf_accept_entropy_route(ctx, H.f32(logits), V, H.i32(drafts), H.i32(q_indptr), B, 8, H.f32([2.0]), True,
+                                        o[0], o[1], ent, o[2], o[3], pair.gpu, ws)
+        torch.cuda.synchronize()
+        np.testing.assert_array_equal(pair.seq_len.cpu().numpy()[:2], [100 + 5, 37 + 8])
+        np.testing.assert_array_equal(o[0].cpu().numpy(), want["accept_len"])
+    pair.close()
+
+
+# ------------------------------------------------------------------------------------ attention
+def _run_attn(binding, ctx, pair, layer, Q_bits, q_indptr, Hq, max_q, scale):
+    import torch
+    from tests import gpu_harness as H
+    B = len(q_indptr) - 1
+    q = H.bits_to_bf16_tensor(Q_bits)
+    out = torch.zeros_like(q)
+    ws = torch.empty(binding.wf_verify_attn_workspace_bytes(pair.shape, B, Hq, max_q), dtype=torch.uint8, device="cuda")
+    binding.wf_verify_attn(ctx, pair.gpu, layer, q, H.i32(q_indptr), B, Hq, max_q, scale, out, ws)
+    torch.cuda.synchronize()
+    return H.bf16_tensor_to_bits(out)
+
+
+def _attn_case(wf, ctx_lens, q_lens, Hq, Hkv, D, seed, n_layers=1, layer=0, q_std=1.0, kv_std=None, poison=False):
+    from tests import gpu_harness as H
+    binding, ctx = wf
+    pair = H.make_kv_pair(ctx, ctx_lens, q_lens, n_layers, Hkv, D, seed, kv_std=kv_std)
+    if poison:   # NaN in every slot at or beyond ctx+q of each sequence and in unreferenced pages (pin O1.vi)
+        ref = np.zeros(pair.oracle.k_pool.shape[1:], dtype=bool)       # [page][head][slot][d] referenced?
+        for b, (c, qn) in enumerate(zip(ctx_lens, q_lens)):
+            for j in range(c + qn):
+                pg, slot = pair.oracle.locate(b, j)
+                ref[pg, :, slot, :] = True
+        pair.oracle.k_pool[:, ~ref] = 0x7FC0
+        pair.oracle.v_pool[:, ~ref] = 0x7FC0
+        pair.upload_pools()
+    g = synth.rng(seed, 202)
+    q_indptr = np.zeros(len(q_lens) + 1, dtype=np.int32)
+    q_indptr[1:] = np.cumsum(q_lens)
+    Q = synth.normal_bf16(g, (int(q_indptr[-1]), Hq, D), q_std)
+    scale = 1.0 / math.sqrt(D)
+    want = verify_attn.verify_attn(pair.oracle, layer, Q, q_indptr, Hq, scale)
+    got = _run_attn(binding, ctx, pair, layer, Q, q_indptr, Hq, max(q_lens), scale)
+    pair.close()
+    assert not np.isnan(H.attn_errors(got, want)[0])
+    return H.attn_errors(got, want)
+
+
+def test_attn_cfg1_tiny(wf):
+    """configs[0]: 4 q / 2 kv heads, D 64, ctx 512, gamma 7."""
+    for seed in range(4):
+        max_abs, rel = _attn_case(wf, [512], [8], 4, 2, 64, seed=synth.SEED_BASE + seed)
+        assert max_abs <= ATTN_MAX_ABS and rel <= ATTN_REL_L2, (max_abs, rel)
+
+
+def test_attn_8b_shapes_ragged_split(wf):
+    """8B-class heads (32/8, D 128), ragged contexts spanning several split chunks and a ragged tail,
+    mixed gamma 7/15, an empty block, shuffled pages, layer 1 of 2, NaN beyond the visible range."""
+    max_abs, rel = _attn_case(wf, [3000, 17, 1, 1500, 640, 255], [16, 8, 16, 0, 8, 16], 32, 8, 128, seed=9,
+                              n_layers=2, layer=1, poison=True)
+    assert max_abs <= ATTN_MAX_ABS and rel <= ATTN_REL_L2, (max_abs, rel)
+
+
+def test_attn_peaked_scores(wf):
+    """Stress the online-softmax rescaling: Q scaled so that the score std is about 4."""
+    max_abs, rel = _attn_case(wf, [2100, 300], [16, 8], 32, 8, 128, seed=10, q_std=4.0, kv_std=1.0)
+    assert max_abs <= ATTN_MAX_ABS and rel <= 2 * ATTN_REL_L2, (max_abs, rel)
+
+
+def test_attn_single_query_and_zero_context(wf):
+    """q = 1 (plain decode) and ctx = 0 (the block is the whole sequence)."""
+    max_abs, rel = _attn_case(wf, [0, 0, 700], [16, 1, 1], 8, 2, 64, seed=12)
+    assert max_abs <= ATTN_MAX_ABS and rel <= ATTN_REL_L2, (max_abs, rel)
