@@ -34,7 +34,7 @@ def wf():
 # ------------------------------------------------------------------------------------ block table
 def test_block_table_matches_oracle(wf):
     import torch
-    from tests import gpu_harness as H
+    import gpu_harness as H
     binding, ctx = wf
     g = synth.rng(7, 1)
     P, S = 300, 6
@@ -68,7 +68,7 @@ def test_block_table_matches_oracle(wf):
 # ------------------------------------------------------------------------------ accept / route
 def _run_accept(binding, ctx, logits, drafts, q_indptr, tau, max_q):
     import torch
-    from tests import gpu_harness as H
+    import gpu_harness as H
     B = len(q_indptr) - 1
     V = logits.shape[1]
     d_logits = H.f32(logits)
@@ -149,7 +149,7 @@ def test_accept_edge_rows(wf):
 
 def test_accept_advances_target_len(wf):
     import torch
-    from tests import gpu_harness as H
+    import gpu_harness as H
     binding, ctx = wf
     pair = H.make_kv_pair(ctx, [100, 37], [8, 8], 1, 2, 64, seed=5, fill=False)
     g = synth.rng(11, 3)
@@ -172,7 +172,7 @@ def test_accept_advances_target_len(wf):
 # ------------------------------------------------------------------------------------ attention
 def _run_attn(binding, ctx, pair, layer, Q_bits, q_indptr, Hq, max_q, scale):
     import torch
-    from tests import gpu_harness as H
+    import gpu_harness as H
     B = len(q_indptr) - 1
     q = H.bits_to_bf16_tensor(Q_bits)
     out = torch.zeros_like(q)
@@ -183,7 +183,7 @@ def _run_attn(binding, ctx, pair, layer, Q_bits, q_indptr, Hq, max_q, scale):
 
 
 def _attn_case(wf, ctx_lens, q_lens, Hq, Hkv, D, seed, n_layers=1, layer=0, q_std=1.0, kv_std=None, poison=False):
-    from tests import gpu_harness as H
+    import gpu_harness as H
     binding, ctx = wf
     pair = H.make_kv_pair(ctx, ctx_lens, q_lens, n_layers, Hkv, D, seed, kv_std=kv_std)
     if poison:   # NaN in every slot at or beyond ctx+q of each sequence and in unreferenced pages (pin O1.vi)
