@@ -74,11 +74,9 @@ wf_verify_attn_kernel(const AttnParams p) {
   constexpr int NT_O = D / 8;                    // output n-tiles per warp
   constexpr int LD_ITERS = AT_BN * CPR / AT_THREADS;
 
-  extern __shared__ __align__(1024) uint8_t smem[];
+  extern __shared__ __align__(128) uint8_t smem[];
   uint8_t* q_s = smem;                                          // R_PAD x D bf16
   uint8_t* kv_s = smem + R_PAD * D * 2;                         // AT_STAGES x (K tile, V tile)
-  __shared__ int s_len[AT_MAX_B];                               // len_b, then n_split_b
-  __shared__ int s_pref[AT_MAX_B + 1];                          // item prefix over b
   __shared__ int s_red[AT_THREADS / 32];
   __shared__ int s_chunk;
   __shared__ bool s_last;
@@ -88,13 +86,11 @@ wf_verify_attn_kernel(const AttnParams p) {
   const KvView& kv = p.kv;
   const int Hkv = kv.n_kv_heads;
 
-  // ---- work list from the device-resident lengths (identical in every CTA) ----
+  // ---- split size from the device-resident lengths (identical in every CTA, no host sync) ----
   int part = 0;
   for (int b = tid; b < p.B; b += AT_THREADS) {
     const int qb = p.q_indptr[b + 1] - p.q_indptr[b];
-    const int len = qb > 0 ? kv.seq_len[b] + qb : 0;
-    s_len[b] = len;
-    part += len;
+    part += qb > 0 ? kv.seq_len[b] + qb : 0;
   }
 #pragma unroll
   for (int d = 16; d > 0; d >>= 1) part += __shfl_xor_sync(0xffffffffu, part, d);
@@ -109,50 +105,36 @@ wf_verify_attn_kernel(const AttnParams p) {
   }
   __syncthreads();
   const int chunk_target = s_chunk;
-  for (int b = tid; b < p.B; b += AT_THREADS) {
-    const int len = s_len[b];
-    int ns = 0;
-    if (len > 0) {
-      const int pages = (len + 15) >> 4;
-      const int ns0 = (len + chunk_target - 1) / chunk_target;
-      const int pps = (pages + ns0 - 1) / ns0;
-      ns = (pages + pps - 1) / pps;
-    }
-    s_len[b] = ns;                                             // now: n_split_b (len is re-read below)
-  }
-  __syncthreads();
-  if (warp == 0) {                                             // exclusive scan of n_split * Hkv
-    int carry = 0;
-    for (int base = 0; base < p.B; base += 32) {
-      const int b = base + lane;
-      const int n = b < p.B ? s_len[b] * Hkv : 0;
-      int x = n;
-#pragma unroll
-      for (int d = 1; d < 32; d <<= 1) {
-        const int y = __shfl_up_sync(0xffffffffu, x, d);
-        if (lane >= d) x += y;
-      }
-      if (b < p.B) s_pref[b] = carry + x - n;
-      carry += __shfl_sync(0xffffffffu, x, 31);
-    }
-    if (lane == 0) s_pref[p.B] = carry;
-  }
-  __syncthreads();
-  const int n_items = s_pref[p.B];
+  // n_split of a sequence of `len` keys: page-aligned equal parts of about chunk_target keys
+  auto splits_of = [&](int len) {
+    if (len <= 0) return 0;
+    const int pages = (len + 15) >> 4;
+    const int ns0 = (len + chunk_target - 1) / chunk_target;
+    const int pps = (pages + ns0 - 1) / ns0;
+    return (pages + pps - 1) / pps;
+  };
+  auto len_of = [&](int b) {
+    const int qb = p.q_indptr[b + 1] - p.q_indptr[b];
+    return qb > 0 ? kv.seq_len[b] + qb : 0;
+  };
+  // Items are numbered b-major: item = pref_b + split * Hkv + g.  A CTA visits its items in
+  // ascending order, so it walks (b_cur, pref_cur) forward instead of keeping a table.
+  int b_cur = 0, pref_cur = 0;
+  int ns_cur = p.B > 0 ? splits_of(len_of(0)) : 0;
 
   float o[MT][NT_O][4];
   float s[MT][4][4];
 
-  for (int item = blockIdx.x; item < n_items; item += gridDim.x) {
-    // ---- decode item -> (b, split, g) ----
-    int lo = 0, hi = p.B - 1;
-    while (lo < hi) {                                          // last b with s_pref[b] <= item
-      const int mid = (lo + hi + 1) >> 1;
-      if (s_pref[mid] <= item) lo = mid; else hi = mid - 1;
+  for (int item = blockIdx.x;; item += gridDim.x) {
+    while (b_cur < p.B && item >= pref_cur + ns_cur * Hkv) {   // uniform across the CTA
+      pref_cur += ns_cur * Hkv;
+      ++b_cur;
+      ns_cur = b_cur < p.B ? splits_of(len_of(b_cur)) : 0;
     }
-    const int b = lo;
-    const int n_split = s_len[b];
-    const int local = item - s_pref[b];
+    if (b_cur >= p.B) break;
+    const int b = b_cur;
+    const int n_split = ns_cur;
+    const int local = item - pref_cur;
     const int split = local / Hkv, g = local % Hkv;
     const int r0 = p.q_indptr[b];
     const int q_b = p.q_indptr[b + 1] - r0;
@@ -396,27 +378,50 @@ wf_verify_attn_kernel(const AttnParams p) {
     __syncthreads();
     if (!s_last) continue;
     __threadfence();
-    const int item0 = s_pref[b] + g;                           // split s of (b,g) is item0 + s*Hkv
-    for (int r = warp; r < R; r += AT_THREADS / 32) {          // one warp per row; lanes over D
+    const int item0 = pref_cur + g;                            // split s of (b,g) is item0 + s*Hkv
+    // (1) normalised weight of every (split, row): w = 2^(m_s - m) / sum_s l_s 2^(m_s - m)  -> smem
+    float* wgt = reinterpret_cast<float*>(kv_s);               // [n_split][R_PAD]; stages are idle here
+    for (int r = tid; r < R; r += AT_THREADS) {
       float m = -INFINITY;
       for (int sp = 0; sp < n_split; ++sp) m = fmaxf(m, __ldcg(&p.ws_ml[(size_t)(item0 + sp * Hkv) * R_PAD + r].x));
-      float acc[D / 32];
-#pragma unroll
-      for (int c = 0; c < D / 32; ++c) acc[c] = 0.f;
       float l = 0.f;
       for (int sp = 0; sp < n_split; ++sp) {
-        const size_t it = (size_t)(item0 + sp * Hkv) * R_PAD + r;
-        const float2 ml = __ldcg(&p.ws_ml[it]);
+        const float2 ml = __ldcg(&p.ws_ml[(size_t)(item0 + sp * Hkv) * R_PAD + r]);
         const float w = exp2f(ml.x - m);                       // -inf partials get weight 0
+        wgt[sp * R_PAD + r] = w;
         l += ml.y * w;
-#pragma unroll
-        for (int c = 0; c < D / 32; ++c) acc[c] += w * __ldcg(p.ws_o + it * D + c * 32 + lane);
       }
       const float inv = 1.f / l;
+      for (int sp = 0; sp < n_split; ++sp) wgt[sp * R_PAD + r] *= inv;
+    }
+    __syncthreads();
+    // (2) out[r][:] = sum_s w[s][r] O_s[r][:]; one warp per row, 16-byte loads, 4 splits in flight
+    constexpr int C4 = D / 4;                                  // float4 per row
+    for (int r = warp; r < R; r += AT_THREADS / 32) {
       const int i = r / p.group, hg = r % p.group;
       __nv_bfloat16* dst = p.out + ((size_t)(r0 + i) * p.n_q_heads + g * p.group + hg) * D;
+      for (int c = lane; c < C4; c += 32) {
+        float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+        int sp = 0;
+        for (; sp + 4 <= n_split; sp += 4) {
+          float4 x[4];
 #pragma unroll
-      for (int c = 0; c < D / 32; ++c) dst[c * 32 + lane] = __float2bfloat16_rn(acc[c] * inv);
+          for (int u = 0; u < 4; ++u)
+            x[u] = __ldcg(reinterpret_cast<const float4*>(p.ws_o + ((size_t)(item0 + (sp + u) * Hkv) * R_PAD + r) * D) + c);
+#pragma unroll
+          for (int u = 0; u < 4; ++u) {
+            const float w = wgt[(sp + u) * R_PAD + r];
+            acc.x += w * x[u].x; acc.y += w * x[u].y; acc.z += w * x[u].z; acc.w += w * x[u].w;
+          }
+        }
+        for (; sp < n_split; ++sp) {
+          const float4 x = __ldcg(reinterpret_cast<const float4*>(p.ws_o + ((size_t)(item0 + sp * Hkv) * R_PAD + r) * D) + c);
+          const float w = wgt[sp * R_PAD + r];
+          acc.x += w * x.x; acc.y += w * x.y; acc.z += w * x.z; acc.w += w * x.w;
+        }
+        uint2 pk = make_uint2(pack_bf16(acc.x, acc.y), pack_bf16(acc.z, acc.w));
+        *reinterpret_cast<uint2*>(dst + c * 4) = pk;
+      }
     }
   }
 }
