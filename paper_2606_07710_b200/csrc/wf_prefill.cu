@@ -1,13 +1,654 @@
-// (c) KV-only prefill and (d) Lazy Catch-up.  TEMPORARY placeholder while the tcgen05 GEMM is written.
+// (c) KV-only Prefill and (d) Lazy Catch-up.
+// PAPER.md:117-119 (§3.4), :204-206; readings C14-C22.
+//
+// One device path serves eager prefill, flush and the forced flush inside enqueue (bit-identity of
+// lazy vs eager):
+//   plan kernel (1 CTA)  : which rows go where.  Compacts the rows of the call into a row table
+//                          (source pointer, RoPE position, physical page*16+slot), reserves pages in
+//                          the drafter's block table (C24) and advances seq_len / backlog_len.
+//   projection kernel    : out[M, D] tile per (layer, K|V, kv head) = X[M, hidden] . W[hidden, D-slice]
+//                          on tcgen05 (UMMA 128 x D x 16, bf16 in, fp32 accumulators in TMEM).
+//                          W streams through a TMA + mbarrier ring (MN-major, 128B swizzle); the
+//                          gathered X rows are staged with 16-byte cp.async into the K-major 128B
+//                          swizzle layout.  Epilogue: tcgen05.ld, RoPE (fp32, host-built fp64 table)
+//                          on K tiles, bf16 RNE, 16-byte stores straight into the paged pool.
+// A row's bits do not depend on M, on its tile position or on the call that carries it: one code
+// path, a fixed K order, no split-K.
+#include <cuda.h>
+#include <math.h>
+
+#include <new>
+#include <vector>
+
 #include "wf_internal.cuh"
-extern "C" int wf_drafter_create(wf_ctx* ctx, const wf_drafter_shape*, const void* const*, const void* const*,
-                                 wf_paged_kv*, void*, int32_t*, wf_drafter** out) {
-  if (out) *out = nullptr;
-  return wf_set_error(ctx, WF_ERR_UNSUPPORTED_SHAPE, "not built yet");
+
+namespace {
+
+constexpr int PF_BLOCK_M = 128;         // UMMA M
+constexpr int PF_BLOCK_K = 64;          // one 128-byte swizzle row of bf16
+constexpr int PF_MAX_MT = 2;            // m-tiles per pass (TMEM columns = PF_MAX_MT * D)
+constexpr int PF_THREADS = 192;         // warp 0: TMA, warp 1: MMA, warps 2-5: X gather + epilogue
+constexpr int PF_SMEM_BUDGET = 200 * 1024;
+constexpr int PF_GATHER_LAG = 2;        // cp.async groups kept in flight per gather thread
+
+struct RowEntry {
+  const __nv_bfloat16* src;             // hidden row
+  int32_t pos;                          // absolute position (RoPE)
+  int32_t page_slot;                    // physical page * 16 + slot in the drafter cache
+};
+
+// ---- PTX wrappers -------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
 }
-extern "C" int wf_drafter_destroy(wf_drafter*) { return WF_ERR_INVALID_ARG; }
-extern "C" int wf_kv_only_prefill(wf_ctx* ctx, wf_drafter*, const void*, const int32_t*, const int32_t*,
-                                  const int32_t*, int, int, void*) { return wf_set_error(ctx, WF_ERR_UNSUPPORTED_SHAPE, "not built yet"); }
-extern "C" int wf_lazy_catchup_enqueue(wf_ctx* ctx, wf_drafter*, const void*, const int32_t*, const int32_t*,
-                                       const int32_t*, const int32_t*, int, int, void*) { return wf_set_error(ctx, WF_ERR_UNSUPPORTED_SHAPE, "not built yet"); }
-extern "C" int wf_lazy_catchup_flush(wf_ctx* ctx, wf_drafter*, const int32_t*, int, void*) { return wf_set_error(ctx, WF_ERR_UNSUPPORTED_SHAPE, "not built yet"); }
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  uint32_t done = 0;
+  for (uint32_t spins = 0; !done; ++spins) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+    if (spins > (1u << 26)) __trap();   // a lost arrival becomes an error, never a hang
+  }
+}
+__device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const void* tmap, int c0, int c1, uint32_t bar) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+      ::"r"(dst), "l"(tmap), "r"(c0), "r"(c1), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+__device__ __forceinline__ void tmem_alloc(uint32_t dst_smem, uint32_t ncols) {
+  asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(dst_smem), "r"(ncols) : "memory");
+  asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_dealloc(uint32_t taddr, uint32_t ncols) {
+  asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(ncols) : "memory");
+}
+// D[tmem] (+)= A[smem desc] . B[smem desc], issued by one thread for the whole CTA
+__device__ __forceinline__ void umma_bf16(uint32_t tmem_d, uint64_t desc_a, uint64_t desc_b, uint32_t idesc, uint32_t acc) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
+      ::"r"(tmem_d), "l"(desc_a), "l"(desc_b), "r"(idesc), "r"(acc) : "memory");
+}
+// arrive on an mbarrier once every previously issued tcgen05.mma of this thread has completed
+__device__ __forceinline__ void umma_commit(uint32_t bar) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+// 32 lanes x 32 consecutive fp32 columns: thread t of the warp receives row (lane base + t)
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+      "{%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,"
+      "%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];"
+      : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+        "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]),
+        "=r"(v[16]), "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]),
+        "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+      : "r"(taddr) : "memory");
+}
+__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+
+// UMMA shared-memory descriptor, 128-byte swizzle (layout type 2), Blackwell version bit set.
+// K-major operand  : rows of 128 B, 8-row atoms 1024 B apart -> SBO = 1024 (LBO unused, 1).
+// MN-major operand : 128 B of MN per k-row, 8-k-row atoms SBO = 1024 apart, next 64 MN elements LBO apart.
+__device__ __forceinline__ uint64_t umma_desc(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
+  uint64_t d = 0;
+  d |= (uint64_t)((saddr & 0x3FFFF) >> 4);
+  d |= (uint64_t)((lbo_bytes >> 4) & 0x3FFF) << 16;
+  d |= (uint64_t)((sbo_bytes >> 4) & 0x3FFF) << 32;
+  d |= (uint64_t)1 << 46;
+  d |= (uint64_t)2 << 61;
+  return d;
+}
+// instruction descriptor: D fp32, A/B bf16, A K-major, B MN-major, M x N
+__device__ __forceinline__ uint32_t umma_idesc(int M, int N) {
+  return (1u << 4) | (1u << 7) | (1u << 10) | (0u << 15) | (1u << 16) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
+}
+
+__device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
+  __nv_bfloat162 v = __floats2bfloat162_rn(lo, hi);
+  return *reinterpret_cast<uint32_t*>(&v);
+}
+
+// ---- the plan kernel -------------------------------------------------------------------------
+enum PlanMode { PLAN_EAGER = 0, PLAN_FLUSH = 1, PLAN_FORCED = 2 };
+
+struct PlanParams {
+  int mode, B, hidden, cap, max_pos, row_cap;
+  const __nv_bfloat16* hidden_rows;     // EAGER: block hidden states [sum_q][hidden]
+  const int32_t* q_indptr;              // EAGER / FORCED
+  const int32_t* n_rows;                // EAGER / FORCED
+  const int32_t* seq_ids;               // EAGER / FORCED (NULL = identity)
+  const int32_t* mask;                  // FLUSH: flush_mask (NULL = all); FORCED: idle_mask
+  const __nv_bfloat16* backlog;         // [max_seqs][cap][hidden]
+  int32_t* backlog_len;
+  KvView kv;
+  RowEntry* rows;
+  int32_t* m_total;
+  int32_t* plan_n;                      // [max_seqs] rows of sequence b in this call
+  int32_t* plan_off;                    // [max_seqs] first compact row of sequence b
+  int* status;
+};
+
+__global__ void __launch_bounds__(1024) wf_prefill_plan_kernel(const PlanParams p) {
+  __shared__ int s_warp[32];
+  __shared__ int s_carry;
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5, nw = blockDim.x >> 5;
+  auto seq_of = [&](int b) { return (p.mode != PLAN_FLUSH && p.seq_ids) ? p.seq_ids[b] : b; };
+  // rows each sequence contributes to this call
+  for (int b = tid; b < p.B; b += blockDim.x) {
+    const int sq = seq_of(b);
+    int n;
+    if (p.mode == PLAN_EAGER) {
+      n = p.n_rows[b];
+    } else if (p.mode == PLAN_FLUSH) {
+      n = (!p.mask || p.mask[b]) ? p.backlog_len[sq] : 0;
+    } else {                                                   // forced flush before an enqueue (C20)
+      const int add = p.n_rows[b];
+      if (p.mask[b] && add > p.cap) *p.status = WF_ERR_QUEUE_OVERFLOW;
+      n = (p.mask[b] && add <= p.cap && p.backlog_len[sq] + add > p.cap) ? p.backlog_len[sq] : 0;
+    }
+    p.plan_n[b] = n;
+  }
+  if (tid == 0) s_carry = 0;
+  __syncthreads();
+  // pages first (C24: ascending b, consecutive ring entries); nothing is written if they do not fit
+  const bool ok = kv_reserve_block(p.kv, p.B, [&](int b) { return p.plan_n[b]; }, seq_of, p.status);
+  if (!ok) {
+    if (tid == 0) *p.m_total = 0;
+    return;
+  }
+  // exclusive scan of plan_n -> plan_off
+  for (int base = 0; base < p.B; base += blockDim.x) {
+    const int b = base + tid;
+    const int n = b < p.B ? p.plan_n[b] : 0;
+    int x = n;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+      const int y = __shfl_up_sync(0xffffffffu, x, d);
+      if (lane >= d) x += y;
+    }
+    if (lane == 31) s_warp[wid] = x;
+    __syncthreads();
+    if (wid == 0) {
+      int w = lane < nw ? s_warp[lane] : 0;
+#pragma unroll
+      for (int d = 1; d < 32; d <<= 1) {
+        const int y = __shfl_up_sync(0xffffffffu, w, d);
+        if (lane >= d) w += y;
+      }
+      s_warp[lane] = w;
+    }
+    __syncthreads();
+    if (b < p.B) p.plan_off[b] = s_carry + (wid ? s_warp[wid - 1] : 0) + x - n;
+    __syncthreads();
+    if (tid == 0) s_carry += s_warp[nw - 1];
+    __syncthreads();
+  }
+  const int total = s_carry;
+  if (total > p.row_cap) {                                     // host bounds make this unreachable
+    if (tid == 0) { *p.status = WF_ERR_INVALID_ARG; *p.m_total = 0; }
+    return;
+  }
+  // row table: one warp per sequence
+  for (int b = wid; b < p.B; b += nw) {
+    const int sq = seq_of(b);
+    const int n = p.plan_n[b], off = p.plan_off[b];
+    const int p0 = p.kv.seq_len[sq];
+    const __nv_bfloat16* base = p.mode == PLAN_EAGER
+        ? p.hidden_rows + (size_t)p.q_indptr[b] * p.hidden
+        : p.backlog + (size_t)sq * p.cap * p.hidden;
+    for (int t = lane; t < n; t += 32) {
+      const int pos = p0 + t;
+      if (pos >= p.max_pos) *p.status = WF_ERR_INVALID_ARG;
+      const int page = p.kv.block_table[(size_t)sq * p.kv.max_pages_per_seq + (pos >> 4)];
+      RowEntry e;
+      e.src = base + (size_t)t * p.hidden;
+      e.pos = min(pos, p.max_pos - 1);
+      e.page_slot = page * 16 + (pos & 15);
+      p.rows[off + t] = e;
+    }
+    __syncwarp();
+    if (lane == 0 && n > 0) {
+      p.kv.seq_len[sq] = p0 + n;
+      if (p.mode != PLAN_EAGER) p.backlog_len[sq] = 0;
+    }
+  }
+  if (tid == 0) *p.m_total = total;
+}
+
+// ---- the projection kernel ------------------------------------------------------------------
+constexpr int PF_MAX_STAGES = 12;
+
+struct GemmParams {
+  const CUtensorMap* tmaps;             // [n_layers * 2] (W_K[l], W_V[l]): dims {Hkv*D, hidden}, box {64, 64}, SW128
+  const RowEntry* rows;
+  const int32_t* m_total;
+  const float2* rope;                   // [max_pos][D/2] (cos, sin)
+  __nv_bfloat16* k_pool;
+  __nv_bfloat16* v_pool;
+  int hidden, n_kv_heads, num_pages;
+};
+
+template <int D>
+__global__ void __launch_bounds__(PF_THREADS, 1) wf_prefill_gemm_kernel(const GemmParams p) {
+  constexpr int B_BYTES = PF_BLOCK_K * D * 2;          // W stage: D/64 boxes of [64 k][128 B]
+  constexpr int A_TILE = PF_BLOCK_M * PF_BLOCK_K * 2;  // 16 KB: 128 rows x 128 B
+  constexpr uint32_t TMEM_COLS = PF_MAX_MT * D;        // 256 or 128: a power of two >= 32
+  extern __shared__ __align__(1024) uint8_t smem[];
+  __shared__ __align__(8) uint64_t s_full[PF_MAX_STAGES], s_empty[PF_MAX_STAGES], s_acc_full, s_acc_empty;
+  __shared__ uint32_t s_tmem;
+
+  const int M = *p.m_total;
+  if (M == 0) return;                                  // nothing queued for this call
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int tile = blockIdx.x;                         // (layer, K|V, kv head)
+  const int layer = tile / (2 * p.n_kv_heads);
+  const int is_v = (tile / p.n_kv_heads) & 1;
+  const int head = tile % p.n_kv_heads;
+  const int n_kb = p.hidden / PF_BLOCK_K;
+  const int n_pass = (M + PF_MAX_MT * PF_BLOCK_M - 1) / (PF_MAX_MT * PF_BLOCK_M);
+
+  // A stage holds only the rows that exist (8-row swizzle atoms); UMMA reads 128 rows from its start,
+  // the surplus lands in later stages / the W ring and feeds accumulator rows nobody reads.
+  const int m_first = min(M, PF_MAX_MT * PF_BLOCK_M);
+  const int a_bytes = ((m_first + 7) / 8) * 1024;
+  const int n_stages = min(PF_MAX_STAGES, PF_SMEM_BUDGET / (a_bytes + B_BYTES));
+  uint8_t* a_base = smem;
+  uint8_t* b_base = smem + (size_t)n_stages * a_bytes;      // 1024-aligned: a_bytes is a multiple of 1024
+
+  if (tid == 0) {
+    for (int i = 0; i < n_stages; ++i) { mbar_init(smem_u32(&s_full[i]), 1 + 128); mbar_init(smem_u32(&s_empty[i]), 1); }
+    mbar_init(smem_u32(&s_acc_full), 1);
+    mbar_init(smem_u32(&s_acc_empty), 128);
+    fence_barrier_init();
+  }
+  if (warp == 1) tmem_alloc(smem_u32(&s_tmem), TMEM_COLS);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = s_tmem;
+
+  if (warp == 0) {
+    // ===== TMA producer: stream this tile's W slab, one [64 k][D] block per stage =====
+    if (lane == 0) {
+      const CUtensorMap* tm = p.tmaps + layer * 2 + is_v;
+      int it = 0;
+      for (int pass = 0; pass < n_pass; ++pass)
+        for (int kb = 0; kb < n_kb; ++kb, ++it) {
+          const int s = it % n_stages;
+          mbar_wait(smem_u32(&s_empty[s]), ((it / n_stages) & 1) ^ 1);
+          mbar_arrive_expect_tx(smem_u32(&s_full[s]), B_BYTES);
+#pragma unroll
+          for (int j = 0; j < D / 64; ++j)
+            tma_load_2d(smem_u32(b_base + (size_t)s * B_BYTES + j * 8192), tm, head * D + j * 64, kb * PF_BLOCK_K,
+                        smem_u32(&s_full[s]));
+        }
+    }
+  } else if (warp == 1) {
+    // ===== MMA issuer: one thread drives the tensor core for the CTA =====
+    if (lane == 0) {
+      const uint32_t idesc = umma_idesc(PF_BLOCK_M, D);
+      int it = 0;
+      for (int pass = 0; pass < n_pass; ++pass) {
+        const int rows_here = min(M - pass * PF_MAX_MT * PF_BLOCK_M, PF_MAX_MT * PF_BLOCK_M);
+        const int n_mt = (rows_here + PF_BLOCK_M - 1) / PF_BLOCK_M;
+        if (pass > 0) { mbar_wait(smem_u32(&s_acc_empty), (pass - 1) & 1); tc_fence_after(); }
+        for (int kb = 0; kb < n_kb; ++kb, ++it) {
+          const int s = it % n_stages;
+          mbar_wait(smem_u32(&s_full[s]), (it / n_stages) & 1);
+          tc_fence_after();
+          const uint32_t a_s = smem_u32(a_base + (size_t)s * a_bytes);
+          const uint32_t b_s = smem_u32(b_base + (size_t)s * B_BYTES);
+          for (int mt = 0; mt < n_mt; ++mt)
+#pragma unroll
+            for (int k16 = 0; k16 < PF_BLOCK_K / 16; ++k16) {
+              const uint64_t da = umma_desc(a_s + mt * A_TILE + k16 * 32, 16, 1024);        // K-major
+              const uint64_t db = umma_desc(b_s + k16 * 2048, 8192, 1024);                 // MN-major
+              umma_bf16(tmem_base + mt * D, da, db, idesc, (kb | k16) != 0);
+            }
+          umma_commit(smem_u32(&s_empty[s]));            // frees the stage when these MMAs retire
+        }
+        umma_commit(smem_u32(&s_acc_full));
+      }
+    }
+  } else {
+    // ===== warps 2-5: gather X rows into the swizzled A stages, then run the epilogue =====
+    const int gt = tid - 64;                             // 0..127: row inside an m-tile
+    const int quarter = warp & 3;                        // TMEM lane quarter this warp may read
+    int it = 0;
+    for (int pass = 0; pass < n_pass; ++pass) {
+      const int m_base = pass * PF_MAX_MT * PF_BLOCK_M;
+      const int rows_here = min(M - m_base, PF_MAX_MT * PF_BLOCK_M);
+      const int n_mt = (rows_here + PF_BLOCK_M - 1) / PF_BLOCK_M;
+      const __nv_bfloat16* src[PF_MAX_MT];
+#pragma unroll
+      for (int mt = 0; mt < PF_MAX_MT; ++mt) {
+        const int m = m_base + mt * PF_BLOCK_M + gt;
+        src[mt] = m < M ? p.rows[m].src : nullptr;
+      }
+      const int it0 = it;
+      for (int kb = 0; kb < n_kb; ++kb, ++it) {
+        const int s = it % n_stages;
+        mbar_wait(smem_u32(&s_empty[s]), ((it / n_stages) & 1) ^ 1);
+        const uint32_t a_s = smem_u32(a_base + (size_t)s * a_bytes);
+#pragma unroll
+        for (int mt = 0; mt < PF_MAX_MT; ++mt)
+          if (src[mt]) {
+            const uint32_t row_s = a_s + mt * A_TILE + gt * 128;
+#pragma unroll
+            for (int c = 0; c < 8; ++c)
+              cp_async16(row_s + ((c ^ (gt & 7)) << 4), src[mt] + kb * PF_BLOCK_K + c * 8);
+          }
+        cp_async_commit();
+        if (it - it0 >= PF_GATHER_LAG) {                 // publish the stage filled LAG iterations ago
+          cp_async_wait<PF_GATHER_LAG>();
+          fence_proxy_async();                           // generic-proxy writes -> visible to the tensor core
+          mbar_arrive(smem_u32(&s_full[(it - PF_GATHER_LAG) % n_stages]));
+        }
+      }
+      cp_async_wait<0>();
+      fence_proxy_async();
+      for (int j = max(it0, it - PF_GATHER_LAG); j < it; ++j) mbar_arrive(smem_u32(&s_full[j % n_stages]));
+
+      // ---- epilogue: TMEM -> registers -> (RoPE) -> bf16 -> paged pool ----
+      mbar_wait(smem_u32(&s_acc_full), pass & 1);
+      tc_fence_after();
+      for (int mt = 0; mt < n_mt; ++mt) {
+        const int m = m_base + mt * PF_BLOCK_M + quarter * 32 + lane;
+        const bool valid = m < M;
+        RowEntry e;
+        e.src = nullptr; e.pos = 0; e.page_slot = 0;
+        if (valid) e = p.rows[m];
+        __nv_bfloat16* dst = (is_v ? p.v_pool : p.k_pool) +
+            ((((size_t)layer * p.num_pages + (e.page_slot >> 4)) * p.n_kv_heads + head) * 16 + (e.page_slot & 15)) * D;
+        const uint32_t t_row = tmem_base + ((uint32_t)(quarter * 32) << 16) + mt * D;
+        if (!is_v) {
+          const float2* cs = p.rope + (size_t)e.pos * (D / 2);
+#pragma unroll
+          for (int j = 0; j < D / 64; ++j) {             // 32 rotation pairs (r, r + D/2) per step
+            uint32_t lo[32], hi[32];
+            tmem_ld32(t_row + j * 32, lo);
+            tmem_ld32(t_row + D / 2 + j * 32, hi);
+            tmem_ld_wait();
+            if (valid) {
+              uint32_t olo[16], ohi[16];
+#pragma unroll
+              for (int i = 0; i < 32; i += 2) {
+                const float4 c2 = *reinterpret_cast<const float4*>(cs + j * 32 + i);   // (cos,sin) x 2
+                const float a0 = __uint_as_float(lo[i]), b0 = __uint_as_float(hi[i]);
+                const float a1 = __uint_as_float(lo[i + 1]), b1 = __uint_as_float(hi[i + 1]);
+                olo[i / 2] = pack_bf16(a0 * c2.x - b0 * c2.y, a1 * c2.z - b1 * c2.w);
+                ohi[i / 2] = pack_bf16(b0 * c2.x + a0 * c2.y, b1 * c2.z + a1 * c2.w);
+              }
+#pragma unroll
+              for (int q4 = 0; q4 < 4; ++q4) {
+                *reinterpret_cast<uint4*>(dst + j * 32 + q4 * 8) = make_uint4(olo[q4 * 4], olo[q4 * 4 + 1], olo[q4 * 4 + 2], olo[q4 * 4 + 3]);
+                *reinterpret_cast<uint4*>(dst + D / 2 + j * 32 + q4 * 8) = make_uint4(ohi[q4 * 4], ohi[q4 * 4 + 1], ohi[q4 * 4 + 2], ohi[q4 * 4 + 3]);
+              }
+            }
+          }
+        } else {
+#pragma unroll
+          for (int j = 0; j < D / 32; ++j) {
+            uint32_t v[32];
+            tmem_ld32(t_row + j * 32, v);
+            tmem_ld_wait();
+            if (valid) {
+#pragma unroll
+              for (int q4 = 0; q4 < 4; ++q4) {
+                uint4 o;
+                o.x = pack_bf16(__uint_as_float(v[q4 * 8 + 0]), __uint_as_float(v[q4 * 8 + 1]));
+                o.y = pack_bf16(__uint_as_float(v[q4 * 8 + 2]), __uint_as_float(v[q4 * 8 + 3]));
+                o.z = pack_bf16(__uint_as_float(v[q4 * 8 + 4]), __uint_as_float(v[q4 * 8 + 5]));
+                o.w = pack_bf16(__uint_as_float(v[q4 * 8 + 6]), __uint_as_float(v[q4 * 8 + 7]));
+                *reinterpret_cast<uint4*>(dst + j * 32 + q4 * 8) = o;
+              }
+            }
+          }
+        }
+      }
+      tc_fence_before();
+      mbar_arrive(smem_u32(&s_acc_empty));               // TMEM may be overwritten by the next pass
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) tmem_dealloc(tmem_base, TMEM_COLS);
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------------
+// host side
+// ------------------------------------------------------------------------------------------------
+struct wf_drafter {
+  wf_ctx* ctx;
+  wf_drafter_shape s;
+  wf_paged_kv* kv;
+  const __nv_bfloat16* backlog;
+  int32_t* backlog_len;
+  CUtensorMap* d_tmaps;        // [n_layers * 2]
+  float2* d_rope;              // [max_pos][D/2]
+  RowEntry* d_rows;
+  int row_cap;
+  int32_t* d_m_total;
+  int32_t* d_plan;             // [2 * max_seqs]: plan_n, plan_off
+};
+
+namespace {
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn get_encode_tiled() {
+  static EncodeTiledFn fn = [] {
+    void* f = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &f, cudaEnableDefault, &q) != cudaSuccess ||
+        q != cudaDriverEntryPointSuccess)
+      f = nullptr;
+    return (EncodeTiledFn)f;
+  }();
+  return fn;
+}
+
+template <int D>
+int launch_gemm(wf_drafter* d, cudaStream_t st) {
+  wf_ctx* ctx = d->ctx;
+  static bool configured = false;
+  if (!configured) {
+    WF_CUDA(ctx, cudaFuncSetAttribute(wf_prefill_gemm_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, PF_SMEM_BUDGET));
+    configured = true;
+  }
+  GemmParams g;
+  g.tmaps = d->d_tmaps; g.rows = d->d_rows; g.m_total = d->d_m_total; g.rope = d->d_rope;
+  g.k_pool = d->kv->k_pool; g.v_pool = d->kv->v_pool;
+  g.hidden = d->s.hidden; g.n_kv_heads = d->s.n_kv_heads; g.num_pages = d->kv->s.num_pages;
+  const int grid = d->s.n_layers * 2 * d->s.n_kv_heads;
+  wf_prefill_gemm_kernel<D><<<grid, PF_THREADS, PF_SMEM_BUDGET, st>>>(g);
+  return wf_check_launch(ctx, "wf_prefill_gemm_kernel");
+}
+
+// plan + projection: the one device path behind eager prefill, flush and forced flush
+int run_prefill(wf_drafter* d, PlanParams& pp, cudaStream_t st) {
+  wf_ctx* ctx = d->ctx;
+  pp.hidden = d->s.hidden; pp.cap = d->s.backlog_cap; pp.max_pos = d->s.max_pos; pp.row_cap = d->row_cap;
+  pp.backlog = d->backlog; pp.backlog_len = d->backlog_len;
+  pp.kv = kv_view(d->kv);
+  pp.rows = d->d_rows; pp.m_total = d->d_m_total;
+  pp.plan_n = d->d_plan; pp.plan_off = d->d_plan + d->kv->s.max_seqs;
+  pp.status = ctx->d_status;
+  wf_prefill_plan_kernel<<<1, 1024, 0, st>>>(pp);
+  int rc = wf_check_launch(ctx, "wf_prefill_plan_kernel");
+  if (rc != WF_OK) return rc;
+  return d->s.head_dim == 128 ? launch_gemm<128>(d, st) : launch_gemm<64>(d, st);
+}
+
+}  // namespace
+
+extern "C" int wf_drafter_create(wf_ctx* ctx, const wf_drafter_shape* s, const void* const* w_k_host_ptrs,
+                                 const void* const* w_v_host_ptrs, wf_paged_kv* kv, void* backlog,
+                                 int32_t* backlog_len, wf_drafter** out) {
+  if (!ctx || !out) return WF_ERR_INVALID_ARG;
+  *out = nullptr;
+  WF_REQUIRE(ctx, s && w_k_host_ptrs && w_v_host_ptrs && kv, WF_ERR_INVALID_ARG, "wf_drafter_create: null argument");
+  WF_REQUIRE(ctx, s->n_layers == kv->s.n_layers && s->n_kv_heads == kv->s.n_kv_heads && s->head_dim == kv->s.head_dim,
+             WF_ERR_INVALID_ARG, "wf_drafter_create: drafter shape does not match its KV cache");
+  WF_REQUIRE(ctx, s->head_dim == 64 || s->head_dim == 128, WF_ERR_UNSUPPORTED_SHAPE, "wf_drafter_create: head_dim must be 64 or 128");
+  WF_REQUIRE(ctx, s->hidden > 0 && s->hidden % PF_BLOCK_K == 0, WF_ERR_UNSUPPORTED_SHAPE,
+             "wf_drafter_create: hidden must be a positive multiple of %d", PF_BLOCK_K);
+  WF_REQUIRE(ctx, s->max_pos > 0 && s->rope_theta > 0.f && s->backlog_cap >= 0, WF_ERR_INVALID_ARG, "wf_drafter_create: bad max_pos/theta/cap");
+  WF_REQUIRE(ctx, s->backlog_cap == 0 || (backlog && backlog_len), WF_ERR_INVALID_ARG, "wf_drafter_create: backlog buffers missing");
+  EncodeTiledFn encode = get_encode_tiled();
+  WF_REQUIRE(ctx, encode, WF_ERR_CUDA, "wf_drafter_create: cuTensorMapEncodeTiled unavailable");
+
+  const int L = s->n_layers, D = s->head_dim, N = s->n_kv_heads * D;
+  std::vector<CUtensorMap> maps(L * 2);
+  for (int l = 0; l < L; ++l)
+    for (int v = 0; v < 2; ++v) {
+      const void* w = v ? w_v_host_ptrs[l] : w_k_host_ptrs[l];
+      WF_REQUIRE(ctx, w && (uintptr_t)w % 16 == 0, WF_ERR_INVALID_ARG, "wf_drafter_create: weight pointer null or unaligned");
+      cuuint64_t dims[2] = {(cuuint64_t)N, (cuuint64_t)s->hidden};
+      cuuint64_t strides[1] = {(cuuint64_t)N * 2};
+      cuuint32_t box[2] = {64, (cuuint32_t)PF_BLOCK_K};
+      cuuint32_t estr[2] = {1, 1};
+      CUresult r = encode(&maps[l * 2 + v], CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(w), dims, strides, box,
+                          estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                          CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+      WF_REQUIRE(ctx, r == CUDA_SUCCESS, WF_ERR_CUDA, "wf_drafter_create: cuTensorMapEncodeTiled failed (%d)", (int)r);
+    }
+  // RoPE table in fp64 on the host (C17): angle = pos * theta^(-2r/D)
+  const int half = D / 2;
+  std::vector<float2> rope((size_t)s->max_pos * half);
+  std::vector<double> inv_freq(half);
+  for (int r = 0; r < half; ++r) inv_freq[r] = pow((double)s->rope_theta, -2.0 * r / D);
+  for (int pos = 0; pos < s->max_pos; ++pos)
+    for (int r = 0; r < half; ++r) {
+      const double a = (double)pos * inv_freq[r];
+      rope[(size_t)pos * half + r] = make_float2((float)cos(a), (float)sin(a));
+    }
+
+  wf_drafter* d = new (std::nothrow) wf_drafter();
+  if (!d) return wf_set_error(ctx, WF_ERR_INVALID_ARG, "wf_drafter_create: host allocation failed");
+  d->ctx = ctx; d->s = *s; d->kv = kv;
+  d->backlog = (const __nv_bfloat16*)backlog; d->backlog_len = backlog_len;
+  d->d_tmaps = nullptr; d->d_rope = nullptr; d->d_rows = nullptr; d->d_m_total = nullptr; d->d_plan = nullptr;
+  d->row_cap = kv->s.max_seqs * (s->backlog_cap > 64 ? s->backlog_cap : 64);
+  cudaError_t e = cudaMalloc(&d->d_tmaps, sizeof(CUtensorMap) * maps.size());
+  if (e == cudaSuccess) e = cudaMalloc(&d->d_rope, sizeof(float2) * rope.size());
+  if (e == cudaSuccess) e = cudaMalloc(&d->d_rows, sizeof(RowEntry) * d->row_cap);
+  if (e == cudaSuccess) e = cudaMalloc(&d->d_m_total, sizeof(int32_t));
+  if (e == cudaSuccess) e = cudaMalloc(&d->d_plan, sizeof(int32_t) * 2 * kv->s.max_seqs);
+  if (e == cudaSuccess) e = cudaMemcpy(d->d_tmaps, maps.data(), sizeof(CUtensorMap) * maps.size(), cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) e = cudaMemcpy(d->d_rope, rope.data(), sizeof(float2) * rope.size(), cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) e = cudaMemset(d->d_m_total, 0, sizeof(int32_t));
+  if (e != cudaSuccess) {
+    wf_drafter_destroy(d);
+    return wf_set_error(ctx, WF_ERR_CUDA, "wf_drafter_create: %s", cudaGetErrorString(e));
+  }
+  *out = d;
+  return WF_OK;
+}
+
+extern "C" int wf_drafter_destroy(wf_drafter* d) {
+  if (!d) return WF_ERR_INVALID_ARG;
+  cudaFree(d->d_tmaps); cudaFree(d->d_rope); cudaFree(d->d_rows); cudaFree(d->d_m_total); cudaFree(d->d_plan);
+  delete d;
+  return WF_OK;
+}
+
+extern "C" int wf_kv_only_prefill(wf_ctx* ctx, wf_drafter* d, const void* hidden, const int32_t* q_indptr,
+                                  const int32_t* n_rows, const int32_t* seq_ids, int B, int max_rows, void* stream) {
+  if (!ctx || !d) return WF_ERR_INVALID_ARG;
+  WF_REQUIRE(ctx, hidden && q_indptr && n_rows, WF_ERR_INVALID_ARG, "wf_kv_only_prefill: null argument");
+  WF_REQUIRE(ctx, B >= 0 && B <= d->kv->s.max_seqs && max_rows >= 0 && (long long)B * max_rows <= d->row_cap,
+             WF_ERR_INVALID_ARG, "wf_kv_only_prefill: B * max_rows exceeds the row table (%d)", d->row_cap);
+  WF_REQUIRE(ctx, (uintptr_t)hidden % 16 == 0, WF_ERR_INVALID_ARG, "wf_kv_only_prefill: hidden must be 16-byte aligned");
+  if (B == 0 || max_rows == 0) return WF_OK;
+  PlanParams pp{};
+  pp.mode = PLAN_EAGER; pp.B = B;
+  pp.hidden_rows = (const __nv_bfloat16*)hidden; pp.q_indptr = q_indptr; pp.n_rows = n_rows; pp.seq_ids = seq_ids;
+  pp.mask = nullptr;
+  return run_prefill(d, pp, (cudaStream_t)stream);
+}
+
+extern "C" int wf_lazy_catchup_flush(wf_ctx* ctx, wf_drafter* d, const int32_t* flush_mask, int B, void* stream) {
+  if (!ctx || !d) return WF_ERR_INVALID_ARG;
+  WF_REQUIRE(ctx, B >= 0 && B <= d->kv->s.max_seqs, WF_ERR_INVALID_ARG, "wf_lazy_catchup_flush: bad B");
+  WF_REQUIRE(ctx, d->s.backlog_cap > 0, WF_ERR_INVALID_ARG, "wf_lazy_catchup_flush: drafter has no backlog");
+  if (B == 0) return WF_OK;
+  PlanParams pp{};
+  pp.mode = PLAN_FLUSH; pp.B = B; pp.mask = flush_mask;
+  return run_prefill(d, pp, (cudaStream_t)stream);
+}
+
+namespace {
+// copy rows 0..n_rows[b]-1 of each idle sequence's block to the tail of its backlog (FIFO)
+__global__ void wf_enqueue_kernel(const __nv_bfloat16* __restrict__ hidden, const int32_t* __restrict__ q_indptr,
+                                  const int32_t* __restrict__ n_rows, const int32_t* __restrict__ seq_ids,
+                                  const int32_t* __restrict__ idle_mask, __nv_bfloat16* __restrict__ backlog,
+                                  const int32_t* __restrict__ backlog_len, int hidden_dim, int cap) {
+  const int b = blockIdx.y, t = blockIdx.x;
+  if (!idle_mask[b]) return;
+  const int n = n_rows[b];
+  if (t >= n || n > cap) return;
+  const int sq = seq_ids ? seq_ids[b] : b;
+  const uint4* src = reinterpret_cast<const uint4*>(hidden + (size_t)(q_indptr[b] + t) * hidden_dim);
+  uint4* dst = reinterpret_cast<uint4*>(backlog + ((size_t)sq * cap + backlog_len[sq] + t) * hidden_dim);
+  for (int i = threadIdx.x; i < hidden_dim / 8; i += blockDim.x) dst[i] = src[i];
+}
+__global__ void wf_enqueue_len_kernel(const int32_t* __restrict__ n_rows, const int32_t* __restrict__ seq_ids,
+                                      const int32_t* __restrict__ idle_mask, int32_t* __restrict__ backlog_len, int B, int cap) {
+  const int b = blockIdx.x * blockDim.x + threadIdx.x;
+  if (b < B && idle_mask[b] && n_rows[b] <= cap) backlog_len[seq_ids ? seq_ids[b] : b] += n_rows[b];
+}
+}  // namespace
+
+extern "C" int wf_lazy_catchup_enqueue(wf_ctx* ctx, wf_drafter* d, const void* hidden, const int32_t* q_indptr,
+                                       const int32_t* n_rows, const int32_t* seq_ids, const int32_t* idle_mask,
+                                       int B, int max_rows, void* stream) {
+  if (!ctx || !d) return WF_ERR_INVALID_ARG;
+  WF_REQUIRE(ctx, hidden && q_indptr && n_rows && idle_mask, WF_ERR_INVALID_ARG, "wf_lazy_catchup_enqueue: null argument");
+  WF_REQUIRE(ctx, B >= 0 && B <= d->kv->s.max_seqs && max_rows >= 0, WF_ERR_INVALID_ARG, "wf_lazy_catchup_enqueue: bad B");
+  WF_REQUIRE(ctx, d->s.backlog_cap > 0 && max_rows <= d->s.backlog_cap, WF_ERR_INVALID_ARG,
+             "wf_lazy_catchup_enqueue: max_rows exceeds backlog_cap");
+  if (B == 0 || max_rows == 0) return WF_OK;
+  cudaStream_t st = (cudaStream_t)stream;
+  // (1) forced flush of the sequences whose backlog would overflow (C20): same device path as flush
+  PlanParams pp{};
+  pp.mode = PLAN_FORCED; pp.B = B;
+  pp.q_indptr = q_indptr; pp.n_rows = n_rows; pp.seq_ids = seq_ids; pp.mask = idle_mask;
+  int rc = run_prefill(d, pp, st);
+  if (rc != WF_OK) return rc;
+  // (2) append the rows, (3) advance the lengths
+  wf_enqueue_kernel<<<dim3(max_rows, B), 128, 0, st>>>((const __nv_bfloat16*)hidden, q_indptr, n_rows, seq_ids, idle_mask,
+                                                      const_cast<__nv_bfloat16*>(d->backlog), d->backlog_len, d->s.hidden, d->s.backlog_cap);
+  rc = wf_check_launch(ctx, "wf_enqueue_kernel");
+  if (rc != WF_OK) return rc;
+  wf_enqueue_len_kernel<<<(B + 255) / 256, 256, 0, st>>>(n_rows, seq_ids, idle_mask, d->backlog_len, B, d->s.backlog_cap);
+  return wf_check_launch(ctx, "wf_enqueue_len_kernel");
+}

@@ -109,3 +109,54 @@ def attn_errors(got_bits, want_f64):
     max_abs = float(np.abs(diff).max()) if diff.size else 0.0
     rel_l2 = float(np.sqrt((diff ** 2).sum() / max((want_f64 ** 2).sum(), 1e-300)))
     return max_abs, rel_l2
+
+
+class DrafterPair:
+    """An oracle drafter (+ LazyCatchup) and its GPU twin with identical weights and free list."""
+
+    def __init__(self, ctx, n_layers, hidden, n_kv_heads, head_dim, num_pages, max_seqs, max_pages_per_seq,
+                 free_pages, seed, backlog_cap=32, theta=1e6, max_pos=40000, w_std=0.02, weights=None):
+        from oracle.kv_prefill import Drafter as OracleDrafter
+        from oracle.lazy_catchup import LazyCatchup
+        from paper_2606_07710_b200 import binding
+        torch = torch_mod()
+        self.kvp = KvPair(ctx, n_layers, n_kv_heads, head_dim, num_pages, max_seqs, max_pages_per_seq, free_pages)
+        N = n_kv_heads * head_dim
+        if weights is None:
+            g = synth.rng(seed, 303)
+            weights = ([synth.normal_bf16(g, (hidden, N), w_std) for _ in range(n_layers)],
+                       [synth.normal_bf16(g, (hidden, N), w_std) for _ in range(n_layers)])
+        self.weights = weights
+        self.oracle = OracleDrafter(weights[0], weights[1], self.kvp.oracle, theta)
+        self.oracle_lazy = LazyCatchup(self.oracle, backlog_cap)
+        self.w_k = [bits_to_bf16_tensor(w) for w in weights[0]]
+        self.w_v = [bits_to_bf16_tensor(w) for w in weights[1]]
+        self.backlog = torch.zeros((max_seqs, max(backlog_cap, 1), hidden), dtype=torch.bfloat16, device="cuda")
+        self.backlog_len = torch.zeros(max_seqs, dtype=torch.int32, device="cuda")
+        self.shape = binding.DrafterShape(n_layers, hidden, n_kv_heads, head_dim, theta, max_pos, backlog_cap)
+        self.gpu = binding.Drafter(ctx, self.shape, self.w_k, self.w_v, self.kvp.gpu, self.backlog, self.backlog_len)
+        self.ctx = ctx
+
+    def gather_gpu(self, layer, b, n):
+        """Logical (K, V) bits [n][Hkv][D] of sequence b read back from the GPU pools through its block table."""
+        kv = self.kvp
+        if n == 0:
+            z = np.empty((0, kv.oracle.Hkv, kv.oracle.D), dtype=np.uint16)
+            return z, z.copy()
+        pages = kv.block_table[b, : -(-n // 16)].long()
+        K = bf16_tensor_to_bits(kv.k_pool[layer][pages].permute(0, 2, 1, 3).reshape(-1, kv.oracle.Hkv, kv.oracle.D)[:n])
+        V = bf16_tensor_to_bits(kv.v_pool[layer][pages].permute(0, 2, 1, 3).reshape(-1, kv.oracle.Hkv, kv.oracle.D)[:n])
+        return K, V
+
+    def close(self):
+        self.gpu.close()
+        self.kvp.close()
+
+
+def rel_l2(got_bits, want_f64):
+    got = (np.asarray(got_bits, dtype=np.uint16).astype(np.uint32) << 16).view(np.float32).astype(np.float64)
+    return float(np.sqrt(((got - want_f64) ** 2).sum() / max((want_f64 ** 2).sum(), 1e-300)))
+
+
+def bf16_f64(bits):
+    return (np.asarray(bits, dtype=np.uint16).astype(np.uint32) << 16).view(np.float32).astype(np.float64)
