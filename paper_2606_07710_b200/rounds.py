@@ -1,0 +1,243 @@
+"""Round driver: one verify-and-switch round of the hot path on synthetic, device-resident inputs.
+
+    reserve target pages -> 36 x wf_verify_attn -> wf_accept_entropy_route
+      -> active drafter: wf_kv_only_prefill (stands in for its own forward, reading C22)
+      -> idle drafter:   wf_lazy_catchup_enqueue
+      -> switching sequences: wf_lazy_catchup_flush of the incoming drafter (C21)
+
+Everything is launched on one stream with no host synchronisation inside the round.
+The route trace is seeded and planted in the logits (spike on the row of the last accepted token),
+so the host knows every round's block lengths in advance; the device still computes every output and
+`check_plan` compares them with the plan afterwards.  This module holds no method arithmetic: it
+only builds inputs (synth) and calls the C-ABI binding.  It never imports oracle/.
+"""
+
+import math
+
+import numpy as np
+
+from . import binding as wf
+from . import synth
+
+SPIKE_LOW_ENTROPY = 9.0      # added to the planted winner: H well below tau = 2.0 -> diffusion
+SPIKE_HIGH_ENTROPY = 0.0     # Gaussian row: H ~ ln V - sigma^2/2 (about 7.4 nats at V = 151936) -> AR
+
+
+def _i32(a, device):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a, dtype=np.int32)).to(device)
+
+
+class Slot:
+    """Inputs and plan of one round of the cyclic schedule."""
+    pass
+
+
+class RoundState:
+    def __init__(self, ctx, wl: synth.Workload, n_slots=4, n_rounds_max=64, device="cuda", layers=None,
+                 host_copies=False):
+        import torch
+        self.torch, self.ctx, self.wl, self.device = torch, ctx, wl, device
+        sh = wl.shapes
+        self.sh = sh
+        self.L = layers if layers is not None else sh.n_layers
+        self.B = B = wl.batch
+        g = synth.rng(wl.seed, 1)
+        self.gmax = max(wl.gammas)
+        self.qmax = self.gmax + 1
+        # ---- target cache: contexts, pages for n_rounds_max rounds of growth, shuffled or not ----
+        self.ctx0 = synth.draw_contexts(wl, g)
+        grow = n_rounds_max * self.qmax + self.qmax
+        self.max_pages_per_seq = int(-(-(int(self.ctx0.max()) + grow) // sh.page_size)) + 1
+        num_pages = int(sum(-(-(int(c) + grow) // sh.page_size) for c in self.ctx0)) + 8
+        free = synth.draw_free_list(num_pages, g, wl.shuffled_pages)
+        self.kv_shape = wf.KvShape(self.L, sh.n_kv_heads, sh.head_dim, sh.page_size, num_pages, B, self.max_pages_per_seq)
+        pool = (self.L, num_pages, sh.n_kv_heads, sh.page_size, sh.head_dim)
+        kv_std = 1.0 / math.sqrt(sh.head_dim)
+        # The block's own K/V (reading C10) are whatever the pool already holds at those slots: every
+        # page is pre-filled with N(0, 1/sqrt(D)) values, which is what the target's QKV projection
+        # would have written there.
+        self.k_pool = synth.device_normal_bf16(pool, kv_std, wl.seed, 11, device)
+        self.v_pool = synth.device_normal_bf16(pool, kv_std, wl.seed, 12, device)
+        self.block_table = torch.full((B, self.max_pages_per_seq), -1, dtype=torch.int32, device=device)
+        self.seq_len = torch.zeros(B, dtype=torch.int32, device=device)
+        self.target_kv = wf.PagedKV(ctx, self.kv_shape, self.k_pool, self.v_pool, self.block_table, self.seq_len, free)
+        self.target_kv.reserve(_i32(self.ctx0, device), B)
+        self.seq_len.copy_(_i32(self.ctx0, device))
+        # ---- drafters: A = autoregressive (1 layer), D = diffusion (5 layers, configs[1]) ----
+        self.drafters = {}
+        for name, n_layers in zip(("A", "D"), sh.drafter_layers if len(sh.drafter_layers) == 2 else (sh.drafter_layers[0],) * 2):
+            self.drafters[name] = self._make_drafter(name, n_layers, grow, g)
+        # ---- cyclic schedule of n_slots rounds ----
+        self.n_slots = n_slots
+        route = (g.random((n_slots, B)) < 0.5).astype(np.int32)            # planned route OUTPUT of slot k (1 = AR)
+        if len(wl.gammas) == 1:
+            gam_of = lambda r: wl.gammas[0]
+        else:
+            gam_of = lambda r: wl.gammas[0] if r == wf.ROUTE_AR else wl.gammas[-1]
+        self.slots = []
+        for k in range(n_slots):
+            s = Slot()
+            s.cur = route[(k - 1) % n_slots]                                 # drafter that drafted slot k's block
+            s.next = route[k]
+            s.q_lens = np.array([gam_of(r) + 1 for r in s.cur], dtype=np.int64)
+            s.u = synth.draw_accept_prefix(g, s.q_lens - 1, wl.mean_accept)
+            s.spike = np.where(s.next == wf.ROUTE_AR, SPIKE_HIGH_ENTROPY, SPIKE_LOW_ENTROPY)
+            self._make_slot_inputs(s, k, host_copies)
+            self.slots.append(s)
+        self.tau = torch.full((1,), sh.tau, dtype=torch.float32, device=device)
+        self.out = {n: torch.zeros(B, dtype=torch.int32, device=device) for n in ("accept_len", "bonus_token", "route", "n_commit")}
+        self.entropy = torch.zeros(B, dtype=torch.float32, device=device)
+        self.attn_ws = torch.empty(wf.wf_verify_attn_workspace_bytes(self.kv_shape, B, sh.n_q_heads, self.qmax),
+                                   dtype=torch.uint8, device=device)
+        self.acc_ws = torch.empty(wf.wf_accept_workspace_bytes(B * self.qmax, sh.vocab), dtype=torch.uint8, device=device)
+        self.sm_scale = 1.0 / math.sqrt(sh.head_dim)
+        self.rounds_done = 0
+        torch.cuda.synchronize()
+
+    # ------------------------------------------------------------------------------------------
+    def _make_drafter(self, name, n_layers, grow, g):
+        torch, sh, B, wl = self.torch, self.sh, self.B, self.wl
+        N = sh.n_kv_heads * sh.head_dim
+        per_seq = int(-(-(int(self.ctx0.max()) + grow) // sh.page_size)) + 1
+        # drafter caches start EMPTY of history the bench never reads: positions continue from ctx0
+        num_pages = int(sum(-(-(int(c) + grow) // sh.page_size) for c in self.ctx0)) + 8
+        free = synth.draw_free_list(num_pages, g, wl.shuffled_pages)
+        shape = wf.KvShape(n_layers, sh.n_kv_heads, sh.head_dim, sh.page_size, num_pages, B, per_seq)
+        pool = (n_layers, num_pages, sh.n_kv_heads, sh.page_size, sh.head_dim)
+        d = Slot()
+        d.k_pool = torch.zeros(pool, dtype=torch.bfloat16, device=self.device)
+        d.v_pool = torch.zeros(pool, dtype=torch.bfloat16, device=self.device)
+        d.block_table = torch.full((B, per_seq), -1, dtype=torch.int32, device=self.device)
+        d.seq_len = torch.zeros(B, dtype=torch.int32, device=self.device)
+        d.kv = wf.PagedKV(self.ctx, shape, d.k_pool, d.v_pool, d.block_table, d.seq_len, free)
+        d.kv.reserve(_i32(self.ctx0, self.device), B)
+        d.seq_len.copy_(_i32(self.ctx0, self.device))
+        sid = 20 if name == "A" else 40
+        d.w_k = [synth.device_normal_bf16((sh.hidden, N), 0.02, wl.seed, sid + 2 * l, self.device) for l in range(n_layers)]
+        d.w_v = [synth.device_normal_bf16((sh.hidden, N), 0.02, wl.seed, sid + 2 * l + 1, self.device) for l in range(n_layers)]
+        cap = max(wl.backlog_cap, self.qmax)
+        d.backlog = torch.zeros((B, cap, sh.hidden), dtype=torch.bfloat16, device=self.device)
+        d.backlog_len = torch.zeros(B, dtype=torch.int32, device=self.device)
+        max_pos = int(self.ctx0.max()) + grow + 64
+        d.shape = wf.DrafterShape(n_layers, sh.hidden, sh.n_kv_heads, sh.head_dim, sh.rope_theta, max_pos, cap)
+        d.handle = wf.Drafter(self.ctx, d.shape, d.w_k, d.w_v, d.kv, d.backlog, d.backlog_len)
+        d.cap = cap
+        return d
+
+    def _make_slot_inputs(self, s, k, host_copies):
+        """Device-resident inputs of slot k: Q, hidden rows, logits with planted winners, draft tokens, masks."""
+        torch, sh, wl, dev = self.torch, self.sh, self.wl, self.device
+        B = self.B
+        s.q_indptr_host = np.zeros(B + 1, dtype=np.int32)
+        s.q_indptr_host[1:] = np.cumsum(s.q_lens)
+        n = int(s.q_indptr_host[-1])
+        s.sum_q = n
+        s.q = synth.device_normal_bf16((n, sh.n_q_heads, sh.head_dim), 1.0, wl.seed, 1000 + 10 * k, dev)
+        s.attn_out = torch.zeros_like(s.q)
+        s.hidden = synth.device_normal_bf16((n, sh.hidden), 1.0, wl.seed, 1001 + 10 * k, dev)
+        s.logits = synth.device_normal_f32((n, sh.vocab), sh.logit_sigma, wl.seed, 1002 + 10 * k, dev)
+        g = synth.rng(wl.seed, 2000 + k)
+        winners = g.integers(0, sh.vocab, size=n).astype(np.int64)
+        gaps = g.uniform(0.05, 1.0, size=n).astype(np.float32)
+        spike_rows = np.zeros(n, dtype=np.float32)
+        drafts = g.integers(0, sh.vocab, size=n).astype(np.int32)
+        for b in range(B):
+            r0, gamma = int(s.q_indptr_host[b]), int(s.q_lens[b]) - 1
+            u = int(s.u[b])
+            for j in range(1, u + 1):
+                drafts[r0 + j] = winners[r0 + j - 1]
+            if u < gamma and drafts[r0 + u + 1] == winners[r0 + u]:
+                drafts[r0 + u + 1] = (drafts[r0 + u + 1] + 1) % sh.vocab
+            spike_rows[r0 + u] = s.spike[b]
+        # planted unique winner per row: logits[row, w] = (largest other entry) + gap (+ spike on row u_b)
+        rows = torch.arange(n, device=dev)
+        w_t = torch.from_numpy(winners).to(dev)
+        s.logits[rows, w_t] = -float("inf")
+        s.logits[rows, w_t] = s.logits.amax(dim=1) + torch.from_numpy(gaps + spike_rows).to(dev)
+        s.winners = winners
+        s.drafts = _i32(drafts, dev)
+        s.q_indptr = _i32(s.q_indptr_host, dev)
+        s.add_tokens = _i32(s.q_lens, dev)
+        # per-drafter masks (host-planned): who is active, idle, and who switches in after this round
+        s.masks = {}
+        for name, code in (("A", wf.ROUTE_AR), ("D", wf.ROUTE_DIFFUSION)):
+            active = (s.cur == code).astype(np.int32)
+            m = Slot()
+            m.active_host, m.idle_host = active, 1 - active
+            m.flush_host = ((s.next == code) & (s.cur != code)).astype(np.int32)
+            m.active, m.idle, m.flush = _i32(active, dev), _i32(1 - active, dev), _i32(m.flush_host, dev)
+            m.n_rows = torch.zeros(B, dtype=torch.int32, device=dev)
+            s.masks[name] = m
+        if host_copies:
+            s.host = {k2: getattr(s, k2).cpu().pin_memory() for k2 in ("q", "hidden", "logits", "drafts")}
+
+    # ------------------------------------------------------------------------------------------
+    def attn_bytes(self, slot, ctx_lens):
+        """Algorithmic KV bytes one attention launch reads: K and V once per kv head."""
+        sh = self.sh
+        return int(sum(int(c) + int(q) for c, q in zip(ctx_lens, slot.q_lens))) * sh.n_kv_heads * sh.head_dim * 2 * 2
+
+    def run_attention(self, s, stream=None):
+        sh = self.sh
+        for l in range(self.L):
+            wf.wf_verify_attn(self.ctx, self.target_kv, l, s.q, s.q_indptr, self.B, sh.n_q_heads, self.qmax,
+                              self.sm_scale, s.attn_out, self.attn_ws, stream)
+
+    def run_accept(self, s, stream=None):
+        o = self.out
+        wf.wf_accept_entropy_route(self.ctx, s.logits, self.sh.vocab, s.drafts, s.q_indptr, self.B, self.qmax, self.tau, True,
+                                   o["accept_len"], o["bonus_token"], self.entropy, o["route"], o["n_commit"],
+                                   self.target_kv, self.acc_ws, stream)
+
+    def run_catchup(self, s, stream=None, lazy=True):
+        """Drafter-cache maintenance after the accept: lazy (the paper's scheme) or eager (its baseline)."""
+        torch, B = self.torch, self.B
+        n_commit = self.out["n_commit"]
+        for name, d in self.drafters.items():
+            m = s.masks[name]
+            if lazy:
+                if m.active_host.any():
+                    torch.mul(n_commit, m.active, out=m.n_rows)            # argument marshalling, not the path
+                    wf.wf_kv_only_prefill(self.ctx, d.handle, s.hidden, s.q_indptr, m.n_rows, None, B, self.qmax, stream)
+                if m.idle_host.any():
+                    wf.wf_lazy_catchup_enqueue(self.ctx, d.handle, s.hidden, s.q_indptr, n_commit, None, m.idle, B, self.qmax, stream)
+                if m.flush_host.any():
+                    wf.wf_lazy_catchup_flush(self.ctx, d.handle, m.flush, B, stream)
+            else:
+                wf.wf_kv_only_prefill(self.ctx, d.handle, s.hidden, s.q_indptr, n_commit, None, B, self.qmax, stream)
+
+    def run_round(self, stream=None, lazy=True, events=None):
+        """One whole round.  events: optional dict of (start, end) CUDA event pairs to record around parts."""
+        s = self.slots[self.rounds_done % self.n_slots]
+        self.target_kv.reserve(s.add_tokens, self.B, stream)
+        if events:
+            events["attn"][0].record()
+        self.run_attention(s, stream)
+        if events:
+            events["attn"][1].record()
+        self.run_accept(s, stream)
+        if events:
+            events["catchup"][0].record()
+        self.run_catchup(s, stream, lazy)
+        if events:
+            events["catchup"][1].record()
+        self.rounds_done += 1
+        return s
+
+    def check_plan(self, s):
+        """After a sync: the device's outputs of the last round must equal the planted plan."""
+        self.torch.cuda.synchronize()
+        st = self.ctx.poll_status()
+        if st != 0:
+            raise RuntimeError(f"device status {st}")
+        a = self.out["accept_len"].cpu().numpy()
+        r = self.out["route"].cpu().numpy()
+        if not (np.array_equal(a, s.u) and np.array_equal(r, s.next)):
+            raise RuntimeError(f"device outputs differ from the planted plan: accept {a} vs {s.u}; route {r} vs {s.next}")
+
+    def close(self):
+        for d in self.drafters.values():
+            d.handle.close()
+            d.kv.close()
+        self.target_kv.close()
