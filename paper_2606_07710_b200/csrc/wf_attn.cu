@@ -1,52 +1,32 @@
 // (a) Target-model verification attention over the paged bf16 GQA KV cache.
 // PAPER.md:65 (§3.2 "parallel verification"); readings C10-C13.
 //
-// Split-KV, decode-style.  A work item is (sequence b, kv head g, key range [k0,k1)); its query
-// tile is all q_b rows of all `group` query heads that share kv head g (<= 64 rows), so K and V are
-// read from HBM once per kv head.  A persistent grid (2 CTAs per SM) strides over the item list,
-// which every CTA derives from the device-resident lengths (no host sync).  K/V pages are staged
-// through a 3-deep cp.async ring (16-byte coalesced copies, XOR-swizzled rows), QK^T and PV run on
-// bf16 tensor-core MMA with fp32 accumulators, the online softmax lives in registers with
-// warp-shuffle reductions, and the last CTA to finish a (b,g) pair merges the split partials.
+// Split-KV, decode-style, tcgen05.  A work item is (sequence b, kv head g, key range [k0,k1)); its
+// query tile is all q_b rows of the `group` query heads that share kv head g (<= 64 rows), so K and V
+// are read from HBM once per kv head.  One persistent CTA per SM walks the item list, which every CTA
+// derives from the device-resident lengths (no host sync).  Warp roles:
+//   warp 2    : TMA producer.  Per 128-key tile, lane p issues the 16-key page p of K and of V
+//               (cp.async.bulk.tensor.2d, 128-byte swizzle) into an mbarrier ring of stages.
+//   warp 3    : MMA issuer (one thread).  S = Q K^T (UMMA 128 x 128 x 16, both K-major) into TMEM,
+//               double buffered; O_t = P V (128 x D x 16, V MN-major) into TMEM, double buffered.
+//   warps 0,1,4,5 : softmax.  Thread = (query row = TMEM lane, half of the tile's keys).  S comes out
+//               of TMEM with tcgen05.ld, online softmax in the log2 domain, P goes to smem as the bf16
+//               A operand of the PV MMA, and the per-tile O_t is folded into fp32 registers with the
+//               running rescale.  QK^T of tile t+1 overlaps the softmax of tile t.
+// Split partials (fp32 O, m, l) are merged by the last CTA to finish a (b, g) pair.
 #include "wf_internal.cuh"
+#include "wf_sm100.cuh"
 
 namespace {
 
-constexpr int AT_THREADS = 128;        // 4 warps: (row group rg = warp & 1) x (key part kp = warp >> 1)
-constexpr int AT_BN = 64;              // keys per pipeline stage
-constexpr int AT_STAGES = 3;
+constexpr int AT_THREADS = 256;
+constexpr int AT_BN = 128;             // keys per tile
+constexpr int AT_ROWS = 64;            // query rows staged (UMMA M = 128; rows 64.. are never read back)
 constexpr int AT_MIN_CHUNK = 256;      // never split below this many keys
 constexpr int AT_ITEMS_PER_SM = 8;     // target number of work items per SM
 constexpr int AT_MAX_B = 1024;
+constexpr int AT_MAX_STAGES = 4;
 constexpr float LOG2E = 1.4426950408889634f;
-
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-
-__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src, bool valid) {
-  const int n = valid ? 16 : 0;        // src-size 0 -> 16 zero bytes
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(n) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-template <int N>
-__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
-
-__device__ __forceinline__ void ldsm_x4(uint32_t addr, uint32_t& r0, uint32_t& r1, uint32_t& r2, uint32_t& r3) {
-  asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0,%1,%2,%3}, [%4];"
-               : "=r"(r0), "=r"(r1), "=r"(r2), "=r"(r3) : "r"(addr));
-}
-__device__ __forceinline__ void ldsm_x4_t(uint32_t addr, uint32_t& r0, uint32_t& r1, uint32_t& r2, uint32_t& r3) {
-  asm volatile("ldmatrix.sync.aligned.m8n8.x4.trans.shared.b16 {%0,%1,%2,%3}, [%4];"
-               : "=r"(r0), "=r"(r1), "=r"(r2), "=r"(r3) : "r"(addr));
-}
-__device__ __forceinline__ void mma_bf16(float (&c)[4], const uint32_t (&a)[4], uint32_t b0, uint32_t b1) {
-  asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
-               : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
-               : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
-}
-__device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
-  __nv_bfloat162 v = __floats2bfloat162_rn(lo, hi);
-  return *reinterpret_cast<uint32_t*>(&v);
-}
 
 struct AttnParams {
   const __nv_bfloat16* q;
@@ -56,378 +36,423 @@ struct AttnParams {
   int layer, B, n_q_heads, group;
   float scale_log2;                    // sm_scale * log2(e)
   int target_items;
-  float* ws_o;                         // [items][R_PAD][D] fp32, unnormalised
-  float2* ws_ml;                       // [items][R_PAD] (m in log2 units, l)
+  float* ws_o;                         // [items][64][D] fp32, unnormalised
+  float2* ws_ml;                       // [items][64] (m in log2 units, l)
   unsigned int* counters;              // [B * Hkv], self-resetting
 };
 
-// swizzled byte offset of 16-byte chunk `ch` of row `row` (row pitch = D*2 bytes)
 template <int D>
-__device__ __forceinline__ uint32_t swz(int row, int ch) { return (uint32_t)(row * (D * 2) + ((ch ^ (row & 7)) << 4)); }
+struct AttnCfg {
+  static constexpr int NH = D / 64;                         // 64-element (128-byte) column halves of a K/V row
+  static constexpr int Q_BYTES = AT_ROWS * D * 2;           // NH halves x 64 rows x 128 B
+  static constexpr int P_BYTES = 2 * AT_ROWS * 128;         // 2 key halves x 64 rows x 128 B
+  static constexpr int KV_HALF = AT_BN * 128;               // one column half of a K (or V) tile: 16 KB
+  static constexpr int K_BYTES = NH * KV_HALF;
+  static constexpr int STAGE_BYTES = 2 * K_BYTES;
+  static constexpr int STAGES = D == 128 ? 3 : 4;
+  static constexpr int SMEM = Q_BYTES + P_BYTES + STAGES * STAGE_BYTES;
+  static constexpr uint32_t TM_S = 0, TM_O = 2 * AT_BN;     // TMEM columns: S0, S1, then O0, O1
+};
 
-template <int D, int MT>
-__global__ void __launch_bounds__(AT_THREADS, (D == 128 && MT == 2) ? 2 : 3)
-wf_verify_attn_kernel(const AttnParams p) {
-  constexpr int R_PAD = 32 * MT;                 // query rows per tile (2 row groups x MT x 16)
-  constexpr int CPR = D / 8;                     // 16-byte chunks per row
-  constexpr int TILE_BYTES = AT_BN * D * 2;      // one K (or V) stage
-  constexpr int NT_O = D / 8;                    // output n-tiles per warp
-  constexpr int LD_ITERS = AT_BN * CPR / AT_THREADS;
+struct ItemInfo {
+  int b, g, split, n_split, r0, q_b, ctx, k0, k1, n_tiles, item0;
+};
 
-  extern __shared__ __align__(128) uint8_t smem[];
-  uint8_t* q_s = smem;                                          // R_PAD x D bf16
-  uint8_t* kv_s = smem + R_PAD * D * 2;                         // AT_STAGES x (K tile, V tile)
-  __shared__ int s_red[AT_THREADS / 32];
-  __shared__ int s_chunk;
-  __shared__ bool s_last;
+// shared state of one CTA (static smem)
+struct AttnShared {
+  uint64_t kv_full[AT_MAX_STAGES], kv_empty[AT_MAX_STAGES];
+  uint64_t s_full[2], s_empty[2], o_empty[2], p_full, pv_done, q_ready;
+  float xmax[2][2][AT_ROWS];
+  float xl[2][AT_ROWS];
+  int red[AT_THREADS / 32];
+  int chunk;
+  uint32_t tmem;
+  int last;
+};
 
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int rg = warp & 1, kp = warp >> 1;
-  const KvView& kv = p.kv;
-  const int Hkv = kv.n_kv_heads;
-
-  // ---- split size from the device-resident lengths (identical in every CTA, no host sync) ----
-  int part = 0;
-  for (int b = tid; b < p.B; b += AT_THREADS) {
+// Walks the b-major item list (item = pref_b + split * Hkv + g); every role keeps its own walker.
+struct ItemWalker {
+  const AttnParams& p;
+  int chunk_target;
+  int b_cur = 0, pref_cur = 0, ns_cur = 0;
+  __device__ ItemWalker(const AttnParams& p_, int chunk) : p(p_), chunk_target(chunk) {
+    ns_cur = p.B > 0 ? splits_of(len_of(0)) : 0;
+  }
+  __device__ int len_of(int b) const {
     const int qb = p.q_indptr[b + 1] - p.q_indptr[b];
-    part += qb > 0 ? kv.seq_len[b] + qb : 0;
+    return qb > 0 ? p.kv.seq_len[b] + qb : 0;
   }
-#pragma unroll
-  for (int d = 16; d > 0; d >>= 1) part += __shfl_xor_sync(0xffffffffu, part, d);
-  if (lane == 0) s_red[warp] = part;
-  __syncthreads();
-  if (tid == 0) {
-    long long total = 0;
-    for (int w = 0; w < AT_THREADS / 32; ++w) total += s_red[w];
-    long long c = (total * Hkv + p.target_items - 1) / p.target_items;
-    c = (c + AT_BN - 1) / AT_BN * AT_BN;
-    s_chunk = (int)max((long long)AT_MIN_CHUNK, c);
-  }
-  __syncthreads();
-  const int chunk_target = s_chunk;
-  // n_split of a sequence of `len` keys: page-aligned equal parts of about chunk_target keys
-  auto splits_of = [&](int len) {
+  __device__ int splits_of(int len) const {     // page-aligned equal parts of about chunk_target keys
     if (len <= 0) return 0;
     const int pages = (len + 15) >> 4;
     const int ns0 = (len + chunk_target - 1) / chunk_target;
     const int pps = (pages + ns0 - 1) / ns0;
     return (pages + pps - 1) / pps;
-  };
-  auto len_of = [&](int b) {
-    const int qb = p.q_indptr[b + 1] - p.q_indptr[b];
-    return qb > 0 ? kv.seq_len[b] + qb : 0;
-  };
-  // Items are numbered b-major: item = pref_b + split * Hkv + g.  A CTA visits its items in
-  // ascending order, so it walks (b_cur, pref_cur) forward instead of keeping a table.
-  int b_cur = 0, pref_cur = 0;
-  int ns_cur = p.B > 0 ? splits_of(len_of(0)) : 0;
-
-  float o[MT][NT_O][4];
-  float s[MT][4][4];
-
-  for (int item = blockIdx.x;; item += gridDim.x) {
-    while (b_cur < p.B && item >= pref_cur + ns_cur * Hkv) {   // uniform across the CTA
+  }
+  __device__ bool next(int item, ItemInfo& it) {
+    const int Hkv = p.kv.n_kv_heads;
+    while (b_cur < p.B && item >= pref_cur + ns_cur * Hkv) {
       pref_cur += ns_cur * Hkv;
       ++b_cur;
       ns_cur = b_cur < p.B ? splits_of(len_of(b_cur)) : 0;
     }
-    if (b_cur >= p.B) break;
-    const int b = b_cur;
-    const int n_split = ns_cur;
+    if (b_cur >= p.B) return false;
+    it.b = b_cur; it.n_split = ns_cur;
     const int local = item - pref_cur;
-    const int split = local / Hkv, g = local % Hkv;
-    const int r0 = p.q_indptr[b];
-    const int q_b = p.q_indptr[b + 1] - r0;
-    const int ctx = kv.seq_len[b];
-    const int len = ctx + q_b;
+    it.split = local / Hkv; it.g = local % Hkv;
+    it.r0 = p.q_indptr[b_cur];
+    it.q_b = p.q_indptr[b_cur + 1] - it.r0;
+    it.ctx = p.kv.seq_len[b_cur];
+    const int len = it.ctx + it.q_b;
     const int pages = (len + 15) >> 4;
-    const int pps = (pages + n_split - 1) / n_split;
-    const int k0 = split * pps * 16;
-    const int k1 = min(len, k0 + pps * 16);
-    const int n_tiles = (k1 - k0 + AT_BN - 1) / AT_BN;
-    const int R = q_b * p.group;                               // valid query rows
-    const int32_t* bt = kv.block_table + (size_t)b * kv.max_pages_per_seq;
-    const size_t layer_off = (size_t)p.layer * kv.num_pages;
+    const int pps = (pages + ns_cur - 1) / ns_cur;
+    it.k0 = it.split * pps * 16;
+    it.k1 = min(len, it.k0 + pps * 16);
+    it.n_tiles = (it.k1 - it.k0 + AT_BN - 1) / AT_BN;
+    it.item0 = pref_cur + it.g;
+    return true;
+  }
+};
 
-    __syncthreads();                                           // previous item's smem fully consumed
-
-    // ---- Q tile -> smem (rows r = i*group + hg are contiguous in global memory per i) ----
-    for (int c = tid; c < R_PAD * CPR; c += AT_THREADS) {
-      const int r = c / CPR, ch = c % CPR;
-      const int i = r / p.group, hg = r % p.group;
-      const __nv_bfloat16* src = p.q + ((size_t)(r0 + i) * p.n_q_heads + g * p.group + hg) * D + ch * 8;
-      cp_async16(smem_u32(q_s) + swz<D>(r, ch), r < R ? src : p.q, r < R);
-    }
-    auto load_tile = [&](int t) {
-      if (t < n_tiles) {
-        uint8_t* ks = kv_s + (t % AT_STAGES) * 2 * TILE_BYTES;
-        uint8_t* vs = ks + TILE_BYTES;
-        const int tk0 = k0 + t * AT_BN;
+// ================= warp 2: TMA producer =================
+template <int D>
+__device__ __forceinline__ void attn_loader(const AttnParams& p, AttnShared& sh, uint8_t* kv_s, int chunk, int lane) {
+  using C = AttnCfg<D>;
+  const KvView& kv = p.kv;
+  ItemWalker walk(p, chunk);
+  ItemInfo it;
+  uint32_t gt = 0;
+  for (int item = blockIdx.x; walk.next(item, it); item += gridDim.x) {
+    const int32_t* bt = kv.block_table + (size_t)it.b * kv.max_pages_per_seq;
+    for (int t = 0; t < it.n_tiles; ++t, ++gt) {
+      const int st = gt % C::STAGES;
+      mbar_wait(smem_u32(&sh.kv_empty[st]), ((gt / C::STAGES) & 1) ^ 1);
+      const int tk0 = it.k0 + t * AT_BN;
+      const int npages = min(AT_BN / 16, (it.k1 - tk0 + 15) >> 4);
+      if (lane == 0) mbar_arrive_expect_tx(smem_u32(&sh.kv_full[st]), (uint32_t)npages * 2 * 16 * D * 2);
+      __syncwarp();
+      if (lane < npages) {
+        const int page = __ldg(bt + (tk0 >> 4) + lane);
+        const int row = (((p.layer * kv.num_pages + page) * kv.n_kv_heads) + it.g) * 16;
+        const uint32_t ks = smem_u32(kv_s + (size_t)st * C::STAGE_BYTES) + lane * 2048;
+        const uint32_t vs = ks + C::K_BYTES;
 #pragma unroll
-        for (int it = 0; it < LD_ITERS; ++it) {
-          const int c = it * AT_THREADS + tid;
-          const int key = c / CPR, ch = c % CPR;
-          const int pos = tk0 + key;
-          const bool valid = pos < k1;
-          const int page = valid ? __ldg(bt + (pos >> 4)) : 0;
-          const size_t off = (((layer_off + page) * Hkv + g) * 16 + (pos & 15)) * D + ch * 8;
-          const uint32_t so = swz<D>(key, ch);
-          cp_async16(smem_u32(ks) + so, kv.k_pool + (valid ? off : 0), valid);
-          cp_async16(smem_u32(vs) + so, kv.v_pool + (valid ? off : 0), valid);
+        for (int h = 0; h < C::NH; ++h) {
+          tma_load_2d(ks + h * C::KV_HALF, kv.tmaps + 0, h * 64, row, smem_u32(&sh.kv_full[st]));
+          tma_load_2d(vs + h * C::KV_HALF, kv.tmaps + 1, h * 64, row, smem_u32(&sh.kv_full[st]));
         }
-      }
-      cp_async_commit();
-    };
-#pragma unroll
-    for (int t = 0; t < AT_STAGES - 1; ++t) load_tile(t);      // group 0 also carries the Q tile
-
-    float m_run[MT][2], l_run[MT][2];
-#pragma unroll
-    for (int mt = 0; mt < MT; ++mt) {
-      m_run[mt][0] = m_run[mt][1] = -INFINITY;
-      l_run[mt][0] = l_run[mt][1] = 0.f;
-#pragma unroll
-      for (int nt = 0; nt < NT_O; ++nt) o[mt][nt][0] = o[mt][nt][1] = o[mt][nt][2] = o[mt][nt][3] = 0.f;
-    }
-    const int row_base = rg * 16 * MT;                         // this warp's first query row
-
-    for (int t = 0; t < n_tiles; ++t) {
-      cp_async_wait<AT_STAGES - 2>();
-      __syncthreads();
-      load_tile(t + AT_STAGES - 1);
-      const uint32_t ks = smem_u32(kv_s + (t % AT_STAGES) * 2 * TILE_BYTES);
-      const uint32_t vs = ks + TILE_BYTES;
-      const uint32_t qs = smem_u32(q_s);
-
-      // ---- S = Q K^T for this warp's 16*MT rows x 32 keys ----
-#pragma unroll
-      for (int mt = 0; mt < MT; ++mt)
-#pragma unroll
-        for (int nt = 0; nt < 4; ++nt) s[mt][nt][0] = s[mt][nt][1] = s[mt][nt][2] = s[mt][nt][3] = 0.f;
-#pragma unroll
-      for (int ks16 = 0; ks16 < D / 16; ++ks16) {
-        uint32_t a[MT][4];
-#pragma unroll
-        for (int mt = 0; mt < MT; ++mt) {
-          const int row = row_base + mt * 16 + (lane & 15);
-          ldsm_x4(qs + swz<D>(row, ks16 * 2 + (lane >> 4)), a[mt][0], a[mt][1], a[mt][2], a[mt][3]);
-        }
-#pragma unroll
-        for (int np = 0; np < 2; ++np) {
-          uint32_t b0, b1, b2, b3;
-          const int key = kp * 32 + np * 16 + (lane & 7) + ((lane >> 4) << 3);
-          ldsm_x4(ks + swz<D>(key, ks16 * 2 + ((lane >> 3) & 1)), b0, b1, b2, b3);
-#pragma unroll
-          for (int mt = 0; mt < MT; ++mt) {
-            mma_bf16(s[mt][np * 2 + 0], a[mt], b0, b1);
-            mma_bf16(s[mt][np * 2 + 1], a[mt], b2, b3);
-          }
-        }
-      }
-
-      // ---- causal / tail mask (only tiles that reach the block's own tokens or the item end) ----
-      const int tk0 = k0 + t * AT_BN + kp * 32;                // first key of this warp's slice
-      if (tk0 + 32 > min(ctx + 1, k1)) {
-#pragma unroll
-        for (int mt = 0; mt < MT; ++mt)
-#pragma unroll
-          for (int h = 0; h < 2; ++h) {
-            const int r = row_base + mt * 16 + (lane >> 2) + h * 8;
-            const int lim = min(k1, ctx + r / p.group + 1);    // keys j < lim are visible to row r
-#pragma unroll
-            for (int nt = 0; nt < 4; ++nt)
-#pragma unroll
-              for (int e = 0; e < 2; ++e) {
-                const int j = tk0 + nt * 8 + (lane & 3) * 2 + e;
-                if (j >= lim) s[mt][nt][h * 2 + e] = -INFINITY;
-              }
-          }
-      }
-
-      // ---- online softmax (log2 domain), P -> bf16 A fragments ----
-      uint32_t pa[MT][2][4];
-#pragma unroll
-      for (int mt = 0; mt < MT; ++mt)
-#pragma unroll
-        for (int h = 0; h < 2; ++h) {
-          float mx = -INFINITY;
-#pragma unroll
-          for (int nt = 0; nt < 4; ++nt) mx = fmaxf(mx, fmaxf(s[mt][nt][h * 2], s[mt][nt][h * 2 + 1]));
-          mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, 1));
-          mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, 2));
-          const float m_new = fmaxf(m_run[mt][h], mx * p.scale_log2);
-          const float m_use = m_new == -INFINITY ? 0.f : m_new;
-          const float alpha = exp2f(m_run[mt][h] - m_use);
-          m_run[mt][h] = m_new;
-          float rs = 0.f;
-#pragma unroll
-          for (int nt = 0; nt < 4; ++nt)
-#pragma unroll
-            for (int e = 0; e < 2; ++e) {
-              const float pv = exp2f(fmaf(s[mt][nt][h * 2 + e], p.scale_log2, -m_use));
-              s[mt][nt][h * 2 + e] = pv;
-              rs += pv;
-            }
-          l_run[mt][h] = l_run[mt][h] * alpha + rs;
-#pragma unroll
-          for (int nt = 0; nt < NT_O; ++nt) { o[mt][nt][h * 2] *= alpha; o[mt][nt][h * 2 + 1] *= alpha; }
-        }
-#pragma unroll
-      for (int mt = 0; mt < MT; ++mt)
-#pragma unroll
-        for (int kk = 0; kk < 2; ++kk) {
-          pa[mt][kk][0] = pack_bf16(s[mt][kk * 2][0], s[mt][kk * 2][1]);
-          pa[mt][kk][1] = pack_bf16(s[mt][kk * 2][2], s[mt][kk * 2][3]);
-          pa[mt][kk][2] = pack_bf16(s[mt][kk * 2 + 1][0], s[mt][kk * 2 + 1][1]);
-          pa[mt][kk][3] = pack_bf16(s[mt][kk * 2 + 1][2], s[mt][kk * 2 + 1][3]);
-        }
-
-      // ---- O += P V ----
-#pragma unroll
-      for (int kk = 0; kk < 2; ++kk) {
-        const int key = kp * 32 + kk * 16 + (lane & 7) + (((lane >> 3) & 1) << 3);
-#pragma unroll
-        for (int dp = 0; dp < NT_O / 2; ++dp) {
-          uint32_t b0, b1, b2, b3;
-          ldsm_x4_t(vs + swz<D>(key, dp * 2 + (lane >> 4)), b0, b1, b2, b3);
-#pragma unroll
-          for (int mt = 0; mt < MT; ++mt) {
-            mma_bf16(o[mt][dp * 2 + 0], pa[mt][kk], b0, b1);
-            mma_bf16(o[mt][dp * 2 + 1], pa[mt][kk], b2, b3);
-          }
-        }
-      }
-    }
-    cp_async_wait<0>();
-    __syncthreads();                                           // all stages idle: reuse them as scratch
-
-    // ---- merge the two key parts of each row group through smem ----
-#pragma unroll
-    for (int mt = 0; mt < MT; ++mt)
-#pragma unroll
-      for (int h = 0; h < 2; ++h) {
-        float l = l_run[mt][h];
-        l += __shfl_xor_sync(0xffffffffu, l, 1);
-        l += __shfl_xor_sync(0xffffffffu, l, 2);
-        l_run[mt][h] = l;
-      }
-    float* xo = reinterpret_cast<float*>(kv_s) + (size_t)rg * (16 * MT) * (D + 2);   // [16*MT rows][D+2]
-    if (kp == 1) {
-#pragma unroll
-      for (int mt = 0; mt < MT; ++mt)
-#pragma unroll
-        for (int h = 0; h < 2; ++h) {
-          float* rowp = xo + (mt * 16 + (lane >> 2) + h * 8) * (D + 2);
-#pragma unroll
-          for (int nt = 0; nt < NT_O; ++nt)
-            *reinterpret_cast<float2*>(rowp + nt * 8 + (lane & 3) * 2) = make_float2(o[mt][nt][h * 2], o[mt][nt][h * 2 + 1]);
-          if ((lane & 3) == 0) { rowp[D] = m_run[mt][h]; rowp[D + 1] = l_run[mt][h]; }
-        }
-    }
-    __syncthreads();
-    if (kp == 0) {
-#pragma unroll
-      for (int mt = 0; mt < MT; ++mt)
-#pragma unroll
-        for (int h = 0; h < 2; ++h) {
-          const int rl = mt * 16 + (lane >> 2) + h * 8;
-          const float* rowp = xo + rl * (D + 2);
-          const float m1 = rowp[D], l1 = rowp[D + 1];
-          const float m0 = m_run[mt][h];
-          const float m = fmaxf(m0, m1);
-          const float mu = m == -INFINITY ? 0.f : m;
-          const float e0 = exp2f(m0 - mu), e1 = exp2f(m1 - mu);
-          const float l = l_run[mt][h] * e0 + l1 * e1;
-          const int r = row_base + rl;
-          if (r < R) {
-            const int i = r / p.group, hg = r % p.group;
-            if (n_split == 1) {
-              const float inv = 1.f / l;                       // row r always sees key 0: l > 0
-              __nv_bfloat16* dst = p.out + ((size_t)(r0 + i) * p.n_q_heads + g * p.group + hg) * D;
-#pragma unroll
-              for (int nt = 0; nt < NT_O; ++nt) {
-                const int col = nt * 8 + (lane & 3) * 2;
-                const float2 x = *reinterpret_cast<const float2*>(rowp + col);
-                *reinterpret_cast<uint32_t*>(dst + col) =
-                    pack_bf16((o[mt][nt][h * 2] * e0 + x.x * e1) * inv, (o[mt][nt][h * 2 + 1] * e0 + x.y * e1) * inv);
-              }
-            } else {
-              float* dst = p.ws_o + ((size_t)item * R_PAD + r) * D;
-#pragma unroll
-              for (int nt = 0; nt < NT_O; ++nt) {
-                const int col = nt * 8 + (lane & 3) * 2;
-                const float2 x = *reinterpret_cast<const float2*>(rowp + col);
-                *reinterpret_cast<float2*>(dst + col) =
-                    make_float2(o[mt][nt][h * 2] * e0 + x.x * e1, o[mt][nt][h * 2 + 1] * e0 + x.y * e1);
-              }
-              if ((lane & 3) == 0) p.ws_ml[(size_t)item * R_PAD + r] = make_float2(m, l);
-            }
-          }
-        }
-    }
-    if (n_split == 1) continue;
-
-    // ---- split-KV combine by the last CTA to finish (b, g) ----
-    __threadfence();
-    __syncthreads();
-    if (tid == 0) {
-      const unsigned int old = atomicAdd(&p.counters[b * Hkv + g], 1u);
-      s_last = (old == (unsigned int)n_split - 1);
-      if (s_last) p.counters[b * Hkv + g] = 0;
-    }
-    __syncthreads();
-    if (!s_last) continue;
-    __threadfence();
-    const int item0 = pref_cur + g;                            // split s of (b,g) is item0 + s*Hkv
-    // (1) normalised weight of every (split, row): w = 2^(m_s - m) / sum_s l_s 2^(m_s - m)  -> smem
-    float* wgt = reinterpret_cast<float*>(kv_s);               // [n_split][R_PAD]; stages are idle here
-    for (int r = tid; r < R; r += AT_THREADS) {
-      float m = -INFINITY;
-      for (int sp = 0; sp < n_split; ++sp) m = fmaxf(m, __ldcg(&p.ws_ml[(size_t)(item0 + sp * Hkv) * R_PAD + r].x));
-      float l = 0.f;
-      for (int sp = 0; sp < n_split; ++sp) {
-        const float2 ml = __ldcg(&p.ws_ml[(size_t)(item0 + sp * Hkv) * R_PAD + r]);
-        const float w = exp2f(ml.x - m);                       // -inf partials get weight 0
-        wgt[sp * R_PAD + r] = w;
-        l += ml.y * w;
-      }
-      const float inv = 1.f / l;
-      for (int sp = 0; sp < n_split; ++sp) wgt[sp * R_PAD + r] *= inv;
-    }
-    __syncthreads();
-    // (2) out[r][:] = sum_s w[s][r] O_s[r][:]; one warp per row, 16-byte loads, 4 splits in flight
-    constexpr int C4 = D / 4;                                  // float4 per row
-    for (int r = warp; r < R; r += AT_THREADS / 32) {
-      const int i = r / p.group, hg = r % p.group;
-      __nv_bfloat16* dst = p.out + ((size_t)(r0 + i) * p.n_q_heads + g * p.group + hg) * D;
-      for (int c = lane; c < C4; c += 32) {
-        float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-        int sp = 0;
-        for (; sp + 4 <= n_split; sp += 4) {
-          float4 x[4];
-#pragma unroll
-          for (int u = 0; u < 4; ++u)
-            x[u] = __ldcg(reinterpret_cast<const float4*>(p.ws_o + ((size_t)(item0 + (sp + u) * Hkv) * R_PAD + r) * D) + c);
-#pragma unroll
-          for (int u = 0; u < 4; ++u) {
-            const float w = wgt[(sp + u) * R_PAD + r];
-            acc.x += w * x[u].x; acc.y += w * x[u].y; acc.z += w * x[u].z; acc.w += w * x[u].w;
-          }
-        }
-        for (; sp < n_split; ++sp) {
-          const float4 x = __ldcg(reinterpret_cast<const float4*>(p.ws_o + ((size_t)(item0 + sp * Hkv) * R_PAD + r) * D) + c);
-          const float w = wgt[sp * R_PAD + r];
-          acc.x += w * x.x; acc.y += w * x.y; acc.z += w * x.z; acc.w += w * x.w;
-        }
-        uint2 pk = make_uint2(pack_bf16(acc.x, acc.y), pack_bf16(acc.z, acc.w));
-        *reinterpret_cast<uint2*>(dst + c * 4) = pk;
       }
     }
   }
 }
 
-template <int D, int MT>
-size_t attn_smem_bytes() { return (size_t)(32 * MT) * D * 2 + (size_t)AT_STAGES * 2 * AT_BN * D * 2; }
+// ================= warp 3, one thread: MMA issuer =================
+template <int D>
+__device__ __forceinline__ void attn_mma(const AttnParams& p, AttnShared& sh, uint8_t* q_s, uint8_t* p_s, uint8_t* kv_s,
+                                         int chunk, uint32_t tmem_base) {
+  using C = AttnCfg<D>;
+  const uint32_t idesc_qk = umma_idesc_kk(128, AT_BN);
+  const uint32_t idesc_pv = umma_idesc(128, D);
+  ItemWalker walk(p, chunk);
+  ItemInfo it;
+  uint32_t gt = 0, n_item = 0;
+  auto issue_qk = [&](uint32_t g2) {
+    const int st = g2 % C::STAGES;
+    mbar_wait(smem_u32(&sh.kv_full[st]), (g2 / C::STAGES) & 1);
+    mbar_wait(smem_u32(&sh.s_empty[g2 & 1]), ((g2 >> 1) & 1) ^ 1);
+    tc_fence_after();
+    const uint32_t ks = smem_u32(kv_s + (size_t)st * C::STAGE_BYTES);
+    const uint32_t qs = smem_u32(q_s);
+#pragma unroll
+    for (int k16 = 0; k16 < D / 16; ++k16) {
+      const uint64_t da = umma_desc(qs + (k16 >> 2) * (AT_ROWS * 128) + (k16 & 3) * 32, 16, 1024);
+      const uint64_t db = umma_desc(ks + (k16 >> 2) * C::KV_HALF + (k16 & 3) * 32, 16, 1024);
+      umma_bf16(tmem_base + C::TM_S + (g2 & 1) * AT_BN, da, db, idesc_qk, k16 != 0);
+    }
+    umma_commit(smem_u32(&sh.s_full[g2 & 1]));
+  };
+  for (int item = blockIdx.x; walk.next(item, it); item += gridDim.x, ++n_item) {
+    mbar_wait(smem_u32(&sh.q_ready), n_item & 1);
+    tc_fence_after();
+    issue_qk(gt);
+    for (int t = 0; t < it.n_tiles; ++t, ++gt) {
+      if (t + 1 < it.n_tiles) issue_qk(gt + 1);
+      const int st = gt % C::STAGES;
+      mbar_wait(smem_u32(&sh.p_full), gt & 1);
+      mbar_wait(smem_u32(&sh.o_empty[gt & 1]), ((gt >> 1) & 1) ^ 1);
+      tc_fence_after();
+      const uint32_t vs = smem_u32(kv_s + (size_t)st * C::STAGE_BYTES) + C::K_BYTES;
+      const uint32_t ps = smem_u32(p_s);
+#pragma unroll
+      for (int k16 = 0; k16 < AT_BN / 16; ++k16) {
+        const uint64_t da = umma_desc(ps + (k16 >> 2) * (AT_ROWS * 128) + (k16 & 3) * 32, 16, 1024);
+        const uint64_t db = umma_desc(vs + k16 * 2048, C::KV_HALF, 1024);               // MN-major
+        umma_bf16(tmem_base + C::TM_O + (gt & 1) * D, da, db, idesc_pv, k16 != 0);
+      }
+      umma_commit(smem_u32(&sh.pv_done));
+      umma_commit(smem_u32(&sh.kv_empty[st]));
+    }
+  }
+}
+
+// ================= warps 0, 1, 4, 5: softmax, O accumulation, output, split combine =================
+template <int D>
+__device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared& sh, uint8_t* q_s, uint8_t* p_s, uint8_t* kv_s,
+                                             int chunk, uint32_t tmem_base, int warp, int lane) {
+  using C = AttnCfg<D>;
+  const int Hkv = p.kv.n_kv_heads;
+  const int quarter = warp & 3, ch = warp >> 2;
+  const int r = quarter * 32 + lane;                           // query row = TMEM lane
+  const int stid = ch * 64 + r;                                // 0..127 among the softmax threads
+  const uint32_t t_lane = tmem_base + ((uint32_t)(quarter * 32) << 16);
+  ItemWalker walk(p, chunk);
+  ItemInfo it;
+  uint32_t gt = 0;
+  for (int item = blockIdx.x; walk.next(item, it); item += gridDim.x) {
+    const int R = it.q_b * p.group;
+    const int qi = r / p.group, hg = r % p.group;
+    // ---- Q tile -> smem (K-major, 128-byte swizzle); rows >= R are zero.  All MMAs of the previous
+    //      item have retired: this thread waited for its last pv_done. ----
+    for (int c = stid; c < AT_ROWS * (D / 8); c += 128) {
+      const int rr = c / (D / 8), chn = c % (D / 8);
+      uint4 v = make_uint4(0, 0, 0, 0);
+      if (rr < R) {
+        const int i2 = rr / p.group, h2 = rr % p.group;
+        v = __ldg(reinterpret_cast<const uint4*>(p.q + ((size_t)(it.r0 + i2) * p.n_q_heads + it.g * p.group + h2) * D) + chn);
+      }
+      *reinterpret_cast<uint4*>(q_s + (chn >> 3) * (AT_ROWS * 128) + rr * 128 + (((chn & 7) ^ (rr & 7)) << 4)) = v;
+    }
+    fence_proxy_async();
+    mbar_arrive(smem_u32(&sh.q_ready));
+
+    float m_run = -INFINITY, l_run = 0.f, alpha_prev = 0.f;
+    float o[D / 2];
+#pragma unroll
+    for (int c = 0; c < D / 2; ++c) o[c] = 0.f;
+    const int lim_row = min(it.k1, it.ctx + qi + 1);           // keys j < lim_row are visible to this row
+
+    auto fold_o = [&](uint32_t g2, float alpha) {              // o = o * alpha + O_tile(g2)
+      const uint32_t ta = t_lane + C::TM_O + (g2 & 1) * D + ch * (D / 2);
+#pragma unroll
+      for (int c0 = 0; c0 < D / 2; c0 += 32) {
+        uint32_t v[32];
+        tmem_ld32(ta + c0, v);
+        tmem_ld_wait();
+#pragma unroll
+        for (int c = 0; c < 32; ++c) o[c0 + c] = fmaf(o[c0 + c], alpha, __uint_as_float(v[c]));
+      }
+      tc_fence_before();
+      mbar_arrive(smem_u32(&sh.o_empty[g2 & 1]));
+    };
+
+    for (int t = 0; t < it.n_tiles; ++t, ++gt) {
+      const int tk0 = it.k0 + t * AT_BN;
+      mbar_wait(smem_u32(&sh.s_full[gt & 1]), (gt >> 1) & 1);
+      tc_fence_after();
+      uint32_t sv[64];
+      {
+        uint32_t a0[32], a1[32];
+        const uint32_t ta = t_lane + C::TM_S + (gt & 1) * AT_BN + ch * 64;
+        tmem_ld32(ta, a0);
+        tmem_ld32(ta + 32, a1);
+        tmem_ld_wait();
+#pragma unroll
+        for (int c = 0; c < 32; ++c) { sv[c] = a0[c]; sv[32 + c] = a1[c]; }
+      }
+      tc_fence_before();
+      mbar_arrive(smem_u32(&sh.s_empty[gt & 1]));              // S buffer may be overwritten by QK(t+2)
+
+      const bool tail = tk0 + AT_BN > min(it.ctx + 1, it.k1);
+      float mx = -INFINITY;
+      if (tail) {
+        const int j0 = tk0 + ch * 64;
+#pragma unroll
+        for (int c = 0; c < 64; ++c) {
+          const float x = (j0 + c < lim_row) ? __uint_as_float(sv[c]) : -INFINITY;
+          sv[c] = __float_as_uint(x);
+          mx = fmaxf(mx, x);
+        }
+      } else {
+#pragma unroll
+        for (int c = 0; c < 64; ++c) mx = fmaxf(mx, __uint_as_float(sv[c]));
+      }
+      sh.xmax[gt & 1][ch][r] = mx;
+      named_bar_sync(1 + quarter, 64);
+      mx = fmaxf(mx, sh.xmax[gt & 1][ch ^ 1][r]);
+      const float m_new = fmaxf(m_run, mx * p.scale_log2);
+      const float m_use = m_new == -INFINITY ? 0.f : m_new;
+      const float alpha = exp2f(m_run - m_use);
+      m_run = m_new;
+      float rs = 0.f;
+      uint32_t pk[32];
+#pragma unroll
+      for (int c = 0; c < 64; c += 2) {
+        const float p0 = exp2f(fmaf(__uint_as_float(sv[c]), p.scale_log2, -m_use));
+        const float p1 = exp2f(fmaf(__uint_as_float(sv[c + 1]), p.scale_log2, -m_use));
+        rs += p0 + p1;
+        pk[c >> 1] = pack_bf16(p0, p1);
+      }
+      l_run = l_run * alpha + rs;
+
+      if (tk0 + AT_BN > it.k1) {
+        // Last tile of the sequence: keys >= k1 hold stale or never-written V bits.  Zero them so that
+        // 0 * garbage cannot produce NaN in the PV product (P is exactly 0 there).
+        mbar_wait(smem_u32(&sh.kv_full[gt % C::STAGES]), (gt / C::STAGES) & 1);
+        const int key = (it.k1 - tk0) + stid;
+        if (key < AT_BN) {
+          uint8_t* vrow = kv_s + (size_t)(gt % C::STAGES) * C::STAGE_BYTES + C::K_BYTES + key * 128;
+#pragma unroll
+          for (int h = 0; h < C::NH; ++h)
+#pragma unroll
+            for (int c = 0; c < 8; ++c) *reinterpret_cast<uint4*>(vrow + h * C::KV_HALF + c * 16) = make_uint4(0, 0, 0, 0);
+        }
+      }
+      if (t > 0) mbar_wait(smem_u32(&sh.pv_done), (gt - 1) & 1);          // PV(t-1) retired: P is free, O(t-1) is ready
+      {
+        uint8_t* prow = p_s + ch * (AT_ROWS * 128) + r * 128;
+#pragma unroll
+        for (int c = 0; c < 8; ++c)
+          *reinterpret_cast<uint4*>(prow + ((c ^ (r & 7)) << 4)) = make_uint4(pk[4 * c], pk[4 * c + 1], pk[4 * c + 2], pk[4 * c + 3]);
+      }
+      fence_proxy_async();
+      mbar_arrive(smem_u32(&sh.p_full));
+      if (t > 0) { tc_fence_after(); fold_o(gt - 1, alpha_prev); }
+      alpha_prev = alpha;
+    }
+    mbar_wait(smem_u32(&sh.pv_done), (gt - 1) & 1);
+    tc_fence_after();
+    fold_o(gt - 1, alpha_prev);
+
+    // ---- row sums of the two key halves; write the final rows or the split partial ----
+    sh.xl[ch][r] = l_run;
+    named_bar_sync(1 + quarter, 64);
+    const float l_tot = l_run + sh.xl[ch ^ 1][r];
+    if (r < R) {
+      if (it.n_split == 1) {
+        const float inv = 1.f / l_tot;                         // every row sees key 0: l > 0
+        __nv_bfloat16* dst = p.out + ((size_t)(it.r0 + qi) * p.n_q_heads + it.g * p.group + hg) * D + ch * (D / 2);
+#pragma unroll
+        for (int c = 0; c < D / 2; c += 8)
+          *reinterpret_cast<uint4*>(dst + c) = make_uint4(pack_bf16(o[c] * inv, o[c + 1] * inv), pack_bf16(o[c + 2] * inv, o[c + 3] * inv),
+                                                          pack_bf16(o[c + 4] * inv, o[c + 5] * inv), pack_bf16(o[c + 6] * inv, o[c + 7] * inv));
+      } else {
+        float* dst = p.ws_o + ((size_t)item * AT_ROWS + r) * D + ch * (D / 2);
+#pragma unroll
+        for (int c = 0; c < D / 2; c += 4) *reinterpret_cast<float4*>(dst + c) = make_float4(o[c], o[c + 1], o[c + 2], o[c + 3]);
+        if (ch == 0) p.ws_ml[(size_t)item * AT_ROWS + r] = make_float2(m_run, l_tot);
+      }
+    }
+    if (it.n_split == 1) continue;
+
+    // ---- split-KV combine by the last CTA to finish (b, g) ----
+    __threadfence();
+    named_bar_sync(3, 128);
+    if (stid == 0) {
+      const unsigned int old = atomicAdd(&p.counters[it.b * Hkv + it.g], 1u);
+      sh.last = (old == (unsigned int)it.n_split - 1);
+      if (sh.last) p.counters[it.b * Hkv + it.g] = 0;
+    }
+    named_bar_sync(3, 128);
+    const bool last = sh.last != 0;
+    named_bar_sync(3, 128);                                    // everyone has read the flag before it is reused
+    if (!last) continue;
+    __threadfence();
+    const int cw = stid >> 5;                                  // 4 combine warps, one row at a time each
+    for (int rr = cw; rr < R; rr += 4) {
+      float m = -INFINITY;
+      for (int sp = lane; sp < it.n_split; sp += 32)
+        m = fmaxf(m, __ldcg(&p.ws_ml[(size_t)(it.item0 + sp * Hkv) * AT_ROWS + rr].x));
+#pragma unroll
+      for (int d = 16; d > 0; d >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, d));
+      float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+      float l = 0.f;
+      for (int base = 0; base < it.n_split; base += 32) {
+        const int sp = base + lane;
+        float w = 0.f, lw = 0.f;
+        if (sp < it.n_split) {
+          const float2 ml = __ldcg(&p.ws_ml[(size_t)(it.item0 + sp * Hkv) * AT_ROWS + rr]);
+          w = exp2f(ml.x - m);                                 // -inf partials get weight 0
+          lw = ml.y * w;
+        }
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) lw += __shfl_xor_sync(0xffffffffu, lw, d);
+        l += lw;
+        const int cnt = min(32, it.n_split - base);
+#pragma unroll 4
+        for (int u = 0; u < cnt; ++u) {
+          const float wu = __shfl_sync(0xffffffffu, w, u);
+          if (lane < D / 4) {
+            const float4 x = __ldcg(reinterpret_cast<const float4*>(p.ws_o + ((size_t)(it.item0 + (base + u) * Hkv) * AT_ROWS + rr) * D) + lane);
+            acc.x = fmaf(wu, x.x, acc.x); acc.y = fmaf(wu, x.y, acc.y); acc.z = fmaf(wu, x.z, acc.z); acc.w = fmaf(wu, x.w, acc.w);
+          }
+        }
+      }
+      const float inv = 1.f / l;
+      const int i2 = rr / p.group, h2 = rr % p.group;
+      __nv_bfloat16* dst = p.out + ((size_t)(it.r0 + i2) * p.n_q_heads + it.g * p.group + h2) * D;
+      if (lane < D / 4)
+        *reinterpret_cast<uint2*>(dst + lane * 4) = make_uint2(pack_bf16(acc.x * inv, acc.y * inv), pack_bf16(acc.z * inv, acc.w * inv));
+    }
+  }
+}
+
+template <int D>
+__global__ void __launch_bounds__(AT_THREADS, 1) wf_verify_attn_kernel(const AttnParams p) {
+  using C = AttnCfg<D>;
+  extern __shared__ __align__(1024) uint8_t smem[];
+  __shared__ __align__(8) AttnShared sh;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  uint8_t* q_s = smem;
+  uint8_t* p_s = smem + C::Q_BYTES;
+  uint8_t* kv_s = p_s + C::P_BYTES;
+
+  // split size from the device-resident lengths (identical in every CTA, no host sync)
+  int part = 0;
+  for (int b = tid; b < p.B; b += AT_THREADS) {
+    const int qb = p.q_indptr[b + 1] - p.q_indptr[b];
+    part += qb > 0 ? p.kv.seq_len[b] + qb : 0;
+  }
+#pragma unroll
+  for (int d = 16; d > 0; d >>= 1) part += __shfl_xor_sync(0xffffffffu, part, d);
+  if (lane == 0) sh.red[warp] = part;
+  if (tid == 0) {
+    for (int i = 0; i < C::STAGES; ++i) { mbar_init(smem_u32(&sh.kv_full[i]), 1); mbar_init(smem_u32(&sh.kv_empty[i]), 1); }
+    for (int i = 0; i < 2; ++i) {
+      mbar_init(smem_u32(&sh.s_full[i]), 1);
+      mbar_init(smem_u32(&sh.s_empty[i]), 128);
+      mbar_init(smem_u32(&sh.o_empty[i]), 128);
+    }
+    mbar_init(smem_u32(&sh.p_full), 128);
+    mbar_init(smem_u32(&sh.pv_done), 1);
+    mbar_init(smem_u32(&sh.q_ready), 128);
+    fence_barrier_init();
+  }
+  if (warp == 3) tmem_alloc(smem_u32(&sh.tmem), 512);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = sh.tmem;
+  if (tid == 0) {
+    long long total = 0;
+    for (int w = 0; w < AT_THREADS / 32; ++w) total += sh.red[w];
+    long long c = (total * p.kv.n_kv_heads + p.target_items - 1) / p.target_items;
+    c = (c + AT_BN - 1) / AT_BN * AT_BN;
+    sh.chunk = (int)max((long long)AT_MIN_CHUNK, c);
+  }
+  __syncthreads();
+  const int chunk = sh.chunk;
+
+  if (warp == 2) {
+    attn_loader<D>(p, sh, kv_s, chunk, lane);
+  } else if (warp == 3) {
+    if (lane == 0) attn_mma<D>(p, sh, q_s, p_s, kv_s, chunk, tmem_base);
+  } else if ((warp & 3) < 2) {
+    attn_softmax<D>(p, sh, q_s, p_s, kv_s, chunk, tmem_base, warp, lane);
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 3) tmem_dealloc(tmem_base, 512);
+}
 
 }  // namespace
 
@@ -447,24 +472,16 @@ int attn_target_items() {
   return v;
 }
 
-template <int D, int MT>
+template <int D>
 int launch_attn(wf_ctx* ctx, const AttnParams& p, cudaStream_t st) {
-  static int grid = 0;
-  const size_t smem = attn_smem_bytes<D, MT>();
-  if (grid == 0) {
-    WF_CUDA(ctx, cudaFuncSetAttribute(wf_verify_attn_kernel<D, MT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    int occ = 0;
-    WF_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, wf_verify_attn_kernel<D, MT>, AT_THREADS, smem));
-    WF_REQUIRE(ctx, occ > 0, WF_ERR_CUDA, "wf_verify_attn: kernel does not fit on an SM");
-    grid = occ * ctx->sm_count;
+  static bool configured = false;
+  const size_t smem = AttnCfg<D>::SMEM;
+  if (!configured) {
+    WF_CUDA(ctx, cudaFuncSetAttribute(wf_verify_attn_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    configured = true;
   }
-  wf_verify_attn_kernel<D, MT><<<grid, AT_THREADS, smem, st>>>(p);
+  wf_verify_attn_kernel<D><<<ctx->sm_count, AT_THREADS, smem, st>>>(p);     // one persistent CTA per SM
   return wf_check_launch(ctx, "wf_verify_attn_kernel");
-}
-
-inline int attn_r_pad(int n_q_heads, int n_kv_heads, int max_q_len) {
-  const int rows = max_q_len * (n_q_heads / n_kv_heads);
-  return rows <= 32 ? 32 : 64;
 }
 
 }  // namespace
@@ -472,7 +489,7 @@ inline int attn_r_pad(int n_q_heads, int n_kv_heads, int max_q_len) {
 extern "C" size_t wf_verify_attn_workspace_bytes(const wf_kv_shape* s, int B, int n_q_heads, int max_q_len) {
   if (!s || B <= 0 || n_q_heads <= 0 || s->n_kv_heads <= 0) return 16;
   const size_t items = (size_t)AT_TARGET_ITEMS_MAX + (size_t)B * s->n_kv_heads;
-  const size_t r_pad = attn_r_pad(n_q_heads, s->n_kv_heads, max_q_len);
+  const size_t r_pad = AT_ROWS;
   return items * r_pad * ((size_t)s->head_dim * sizeof(float) + sizeof(float2));
 }
 
@@ -494,7 +511,7 @@ extern "C" int wf_verify_attn(wf_ctx* ctx, const wf_paged_kv* kv, int layer, con
   WF_REQUIRE(ctx, ((uintptr_t)q % 16 == 0) && ((uintptr_t)out % 16 == 0) && ((uintptr_t)workspace % 16 == 0),
              WF_ERR_INVALID_ARG, "wf_verify_attn: q/out/workspace must be 16-byte aligned");
   if (B == 0) return WF_OK;
-  const int r_pad = attn_r_pad(n_q_heads, kv->s.n_kv_heads, max_q_len);
+  const int r_pad = AT_ROWS;
   const size_t items = (size_t)AT_TARGET_ITEMS_MAX + (size_t)B * kv->s.n_kv_heads;
   AttnParams p;
   p.q = (const __nv_bfloat16*)q;
@@ -509,9 +526,7 @@ extern "C" int wf_verify_attn(wf_ctx* ctx, const wf_paged_kv* kv, int layer, con
   p.counters = ctx->d_counters_attn;
   cudaStream_t st = (cudaStream_t)stream;
   const int D = kv->s.head_dim;
-  if (D == 128 && r_pad == 64) return launch_attn<128, 2>(ctx, p, st);
-  if (D == 128 && r_pad == 32) return launch_attn<128, 1>(ctx, p, st);
-  if (D == 64 && r_pad == 64) return launch_attn<64, 2>(ctx, p, st);
-  if (D == 64 && r_pad == 32) return launch_attn<64, 1>(ctx, p, st);
+  if (D == 128) return launch_attn<128>(ctx, p, st);
+  if (D == 64) return launch_attn<64>(ctx, p, st);
   return wf_set_error(ctx, WF_ERR_UNSUPPORTED_SHAPE, "wf_verify_attn: head_dim %d unsupported", D);
 }

@@ -24,6 +24,33 @@ int wf_check_launch(wf_ctx* ctx, const char* what) {
   return WF_OK;
 }
 
+wf_encode_tiled_fn wf_get_encode_tiled() {
+  static wf_encode_tiled_fn fn = [] {
+    void* f = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &f, cudaEnableDefault, &q) != cudaSuccess ||
+        q != cudaDriverEntryPointSuccess)
+      f = nullptr;
+    return (wf_encode_tiled_fn)f;
+  }();
+  return fn;
+}
+
+int wf_make_tmap_2d(wf_ctx* ctx, CUtensorMap* out, const void* base, uint64_t rows, uint64_t cols, uint32_t box_cols,
+                    uint32_t box_rows) {
+  wf_encode_tiled_fn encode = wf_get_encode_tiled();
+  WF_REQUIRE(ctx, encode, WF_ERR_CUDA, "cuTensorMapEncodeTiled unavailable");
+  cuuint64_t dims[2] = {cols, rows};
+  cuuint64_t strides[1] = {cols * 2};
+  cuuint32_t box[2] = {box_cols, box_rows};
+  cuuint32_t estr[2] = {1, 1};
+  CUresult r = encode(out, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), dims, strides, box, estr,
+                      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                      CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  WF_REQUIRE(ctx, r == CUDA_SUCCESS, WF_ERR_CUDA, "cuTensorMapEncodeTiled failed (%d)", (int)r);
+  return WF_OK;
+}
+
 extern "C" int wf_ctx_create(wf_ctx** out, int device_ordinal) {
   if (!out) return WF_ERR_INVALID_ARG;
   *out = nullptr;
@@ -110,10 +137,20 @@ extern "C" int wf_kv_create(wf_ctx* ctx, const wf_kv_shape* s, void* k_pool, voi
   kv->block_table = block_table;
   kv->seq_len = seq_len;
   kv->pages_held = kv->free_ring = kv->ring_state = kv->scratch = nullptr;
+  kv->d_tmaps = nullptr;
+  CUtensorMap maps[2];
+  {
+    const uint64_t rows = (uint64_t)s->n_layers * s->num_pages * s->n_kv_heads * s->page_size;
+    int rc = wf_make_tmap_2d(ctx, &maps[0], k_pool, rows, s->head_dim, 64, 16);
+    if (rc == WF_OK) rc = wf_make_tmap_2d(ctx, &maps[1], v_pool, rows, s->head_dim, 64, 16);
+    if (rc != WF_OK) { delete kv; return rc; }
+  }
   cudaError_t e = cudaMalloc(&kv->pages_held, sizeof(int32_t) * s->max_seqs);
   if (e == cudaSuccess) e = cudaMalloc(&kv->free_ring, sizeof(int32_t) * s->num_pages);
   if (e == cudaSuccess) e = cudaMalloc(&kv->ring_state, sizeof(int32_t) * 2);
   if (e == cudaSuccess) e = cudaMalloc(&kv->scratch, sizeof(int32_t) * 2 * s->max_seqs);
+  if (e == cudaSuccess) e = cudaMalloc(&kv->d_tmaps, sizeof(maps));
+  if (e == cudaSuccess) e = cudaMemcpy(kv->d_tmaps, maps, sizeof(maps), cudaMemcpyHostToDevice);
   if (e == cudaSuccess) e = cudaMemset(kv->pages_held, 0, sizeof(int32_t) * s->max_seqs);
   if (e == cudaSuccess) e = cudaMemset(kv->free_ring, 0xff, sizeof(int32_t) * s->num_pages);
   if (e == cudaSuccess && n_free)
@@ -134,6 +171,7 @@ extern "C" int wf_kv_destroy(wf_paged_kv* kv) {
   cudaFree(kv->free_ring);
   cudaFree(kv->ring_state);
   cudaFree(kv->scratch);
+  cudaFree(kv->d_tmaps);
   delete kv;
   return WF_OK;
 }

@@ -2,6 +2,7 @@
 // nothing under oracle/ includes or links this).
 #pragma once
 
+#include <cuda.h>
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -31,6 +32,7 @@ struct wf_paged_kv {
   int32_t* free_ring;          // library-owned [num_pages]
   int32_t* ring_state;         // library-owned [2]: head, count
   int32_t* scratch;            // library-owned [2*max_seqs]: need, offset
+  CUtensorMap* d_tmaps;        // library-owned [2]: K pool, V pool as [rows][D], box {64, 16}, 128B swizzle
 };
 
 // Device-side view of a paged KV cache passed by value to kernels.
@@ -43,6 +45,7 @@ struct KvView {
   int32_t* free_ring;
   int32_t* ring_state;
   int32_t* scratch;
+  const CUtensorMap* tmaps;    // [0] = K pool, [1] = V pool
   int n_layers, n_kv_heads, head_dim, page_size, num_pages, max_seqs, max_pages_per_seq;
 };
 
@@ -52,6 +55,7 @@ static inline KvView kv_view(const wf_paged_kv* kv) {
   v.block_table = kv->block_table; v.seq_len = kv->seq_len;
   v.pages_held = kv->pages_held; v.free_ring = kv->free_ring;
   v.ring_state = kv->ring_state; v.scratch = kv->scratch;
+  v.tmaps = kv->d_tmaps;
   v.n_layers = kv->s.n_layers; v.n_kv_heads = kv->s.n_kv_heads; v.head_dim = kv->s.head_dim;
   v.page_size = kv->s.page_size; v.num_pages = kv->s.num_pages; v.max_seqs = kv->s.max_seqs;
   v.max_pages_per_seq = kv->s.max_pages_per_seq;
@@ -59,6 +63,14 @@ static inline KvView kv_view(const wf_paged_kv* kv) {
 }
 
 int wf_set_error(wf_ctx* ctx, int code, const char* fmt, ...);
+// cuTensorMapEncodeTiled through the runtime's driver entry point (no link-time libcuda dependency)
+typedef CUresult (*wf_encode_tiled_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                       const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                       CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+wf_encode_tiled_fn wf_get_encode_tiled();
+// 2-D bf16 tensor map, row-major [rows][cols], box {box_cols, box_rows}, 128-byte swizzle
+int wf_make_tmap_2d(wf_ctx* ctx, CUtensorMap* out, const void* base, uint64_t rows, uint64_t cols, uint32_t box_cols,
+                    uint32_t box_rows);
 int wf_check_launch(wf_ctx* ctx, const char* what);   // cudaGetLastError -> WF_ERR_CUDA; counts the launch
 
 #define WF_REQUIRE(ctx, cond, code, ...)                         \
