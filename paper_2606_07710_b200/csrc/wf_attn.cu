@@ -7,11 +7,11 @@
 // SM) owns the contiguous tile range [c*T/G, (c+1)*T/G) (stream-K), which every CTA derives from the
 // device-resident lengths (no host sync).  A range cuts at most two (b, g) pairs, so a CTA writes at
 // most two fp32 partials; the last CTA to finish a pair merges its few partials.  Warp roles:
-//   warp 4    : TMA producer.  Per tile, lane p issues the 16-key page p of K and of V
-//               (cp.async.bulk.tensor.2d, 128-byte swizzle) into an mbarrier ring of stages.
-//   warp 5    : MMA issuer (one thread).  S = Q K^T (UMMA 64 x 128 x 16, both K-major) into TMEM,
+//   warps 8,10: TMA producers (K ring, V ring).  Per tile, lane p issues the 16-key page p
+//               (cp.async.bulk.tensor.2d, 128-byte swizzle); a K tile is released when its QK^T retires.
+//   warp 9    : MMA issuer (one thread).  S = Q K^T (UMMA 64 x 128 x 16, both K-major) into TMEM,
 //               double buffered; O_t = P V (64 x D x 16, V MN-major) into TMEM, double buffered.
-//   warps 0-3 : softmax.  UMMA M = 64 puts rows 16w..16w+15 on TMEM lanes 32w..32w+15, so warp w owns
+//   warps 0-7 : softmax, two groups of 4 warps that ping-pong over the tiles.  UMMA M = 64 puts rows 16w..16w+15 on TMEM lanes 32w..32w+15, so warp w owns
 //               16 rows; tcgen05.ld.16x256b hands them out like an mma C fragment (a quad per row).
 //               Online softmax in the log2 domain with quad shuffles, P goes to smem as the bf16 A
 //               operand of the PV MMA, the per-tile O_t is folded into fp32 registers with the running
@@ -21,7 +21,7 @@
 
 namespace {
 
-constexpr int AT_THREADS = 192;
+constexpr int AT_THREADS = 384;           // 12 warps: 0-3 / 4-7 softmax groups, 8 K loader, 9 MMA, 10 V loader
 constexpr int AT_BN = 128;             // keys per tile
 constexpr int AT_ROWS = 64;            // query rows = UMMA M
 constexpr int AT_MAX_B = 1024;
@@ -49,17 +49,19 @@ struct AttnCfg {
   static constexpr int Q_BYTES = NH * Q_HALF;
   static constexpr int P_BYTES = 2 * Q_HALF;                // 2 key halves x 64 rows x 128 B
   static constexpr int KV_HALF = AT_BN * 128;               // one column half of a K (or V) tile: 16 KB
-  static constexpr int K_BYTES = NH * KV_HALF;
-  static constexpr int STAGE_BYTES = 2 * K_BYTES;
-  static constexpr int STAGES = D == 128 ? 3 : 4;
-  static constexpr int SMEM = Q_BYTES + P_BYTES + STAGES * STAGE_BYTES;
+  static constexpr int K_BYTES = NH * KV_HALF;               // one K (or V) tile
+  static constexpr int STAGES_K = D == 128 ? 3 : 4;          // K ring
+  static constexpr int STAGES_V = D == 128 ? 2 : 4;          // V ring
+  // smem map: P0 | Q | P1 | K ring | V ring   (Q + P1 double as the group-merge buffer)
+  static constexpr int SMEM = Q_BYTES + 2 * P_BYTES + (STAGES_K + STAGES_V) * K_BYTES;
   static constexpr uint32_t TM_S = 0, TM_O = 2 * AT_BN;     // TMEM columns: S0, S1, then O0, O1
 };
 
 // shared state of one CTA (static smem)
 struct AttnShared {
-  uint64_t kv_full[AT_MAX_STAGES], kv_empty[AT_MAX_STAGES];
-  uint64_t s_full[2], s_empty[2], o_empty[2], p_full, pv_done, q_ready;
+  uint64_t k_full[AT_MAX_STAGES], k_empty[AT_MAX_STAGES], v_full[AT_MAX_STAGES], v_empty[AT_MAX_STAGES];
+  uint64_t s_full[2], s_empty[2], o_empty[2], p_full[2], pv_done[2], q_ready;
+  float xm[2][128], xl[2][128];        // group-1 running max / row-sum partials for the group merge
   int red[2][AT_THREADS / 32];
   int total_tiles, g_eff;
   uint32_t tmem;
@@ -121,42 +123,43 @@ __device__ __forceinline__ int cta_of_tile(int x, int T, int G) {      // larges
   return c;
 }
 
-// ================= warp 4: TMA producer =================
+// ================= warps 8 (K) and 10 (V): TMA producers =================
+// K and V have separate rings so that a K tile is released as soon as its QK^T retires: more bytes in flight.
 template <int D>
-__device__ __forceinline__ void attn_loader(const AttnParams& p, AttnShared& sh, uint8_t* kv_s, int lane) {
+__device__ __forceinline__ void attn_loader(const AttnParams& p, AttnShared& sh, uint8_t* ring, int which, int lane) {
   using C = AttnCfg<D>;
   const KvView& kv = p.kv;
+  uint64_t* full = which ? sh.v_full : sh.k_full;
+  uint64_t* empty = which ? sh.v_empty : sh.k_empty;
   SegWalker walk(p, sh.total_tiles, sh.g_eff, blockIdx.x);
   Segment sg;
   uint32_t gt = 0;
   while (walk.next(sg)) {
     const int32_t* bt = kv.block_table + (size_t)sg.b * kv.max_pages_per_seq;
     for (int t = 0; t < sg.n_tiles; ++t, ++gt) {
-      const int st = gt % C::STAGES;
-      mbar_wait(smem_u32(&sh.kv_empty[st]), ((gt / C::STAGES) & 1) ^ 1);
+      const int n_st = which ? C::STAGES_V : C::STAGES_K;
+      const int st = gt % n_st;
+      mbar_wait(smem_u32(&empty[st]), ((gt / n_st) & 1) ^ 1);
       const int tk0 = sg.k0 + t * AT_BN;
       const int npages = min(AT_BN / 16, (sg.k1 - tk0 + 15) >> 4);
-      if (lane == 0) mbar_arrive_expect_tx(smem_u32(&sh.kv_full[st]), (uint32_t)npages * 2 * 16 * D * 2);
+      if (lane == 0) mbar_arrive_expect_tx(smem_u32(&full[st]), (uint32_t)npages * 16 * D * 2);
       __syncwarp();
       if (lane < npages) {
         const int page = __ldg(bt + (tk0 >> 4) + lane);
         const int row = (((p.layer * kv.num_pages + page) * kv.n_kv_heads) + sg.g) * 16;
-        const uint32_t ks = smem_u32(kv_s + (size_t)st * C::STAGE_BYTES) + lane * 2048;
-        const uint32_t vs = ks + C::K_BYTES;
+        const uint32_t dst = smem_u32(ring + (size_t)st * C::K_BYTES) + lane * 2048;
 #pragma unroll
-        for (int h = 0; h < C::NH; ++h) {
-          tma_load_2d(ks + h * C::KV_HALF, kv.tmaps + 0, h * 64, row, smem_u32(&sh.kv_full[st]));
-          tma_load_2d(vs + h * C::KV_HALF, kv.tmaps + 1, h * 64, row, smem_u32(&sh.kv_full[st]));
-        }
+        for (int h = 0; h < C::NH; ++h) tma_load_2d(dst + h * C::KV_HALF, kv.tmaps + which, h * 64, row, smem_u32(&full[st]));
       }
     }
   }
 }
 
-// ================= warp 5, one thread: MMA issuer =================
+// ================= warp 9, one thread: MMA issuer =================
+// Tile g2 (global tile counter) belongs to softmax group g2 & 1, which owns S[g2&1], P[g2&1], O[g2&1].
 template <int D>
-__device__ __forceinline__ void attn_mma(const AttnParams& p, AttnShared& sh, uint8_t* q_s, uint8_t* p_s, uint8_t* kv_s,
-                                         uint32_t tmem_base) {
+__device__ __forceinline__ void attn_mma(const AttnParams& p, AttnShared& sh, uint8_t* q_s, uint8_t* p0_s, uint8_t* p1_s,
+                                         uint8_t* k_s, uint8_t* v_s, uint32_t tmem_base) {
   using C = AttnCfg<D>;
   const uint32_t idesc_qk = umma_idesc_kk(AT_ROWS, AT_BN);
   const uint32_t idesc_pv = umma_idesc(AT_ROWS, D);
@@ -164,11 +167,11 @@ __device__ __forceinline__ void attn_mma(const AttnParams& p, AttnShared& sh, ui
   Segment sg;
   uint32_t gt = 0, n_seg = 0;
   auto issue_qk = [&](uint32_t g2) {
-    const int st = g2 % C::STAGES;
-    mbar_wait(smem_u32(&sh.kv_full[st]), (g2 / C::STAGES) & 1);
+    const int st = g2 % C::STAGES_K;
+    mbar_wait(smem_u32(&sh.k_full[st]), (g2 / C::STAGES_K) & 1);
     mbar_wait(smem_u32(&sh.s_empty[g2 & 1]), ((g2 >> 1) & 1) ^ 1);
     tc_fence_after();
-    const uint32_t ks = smem_u32(kv_s + (size_t)st * C::STAGE_BYTES);
+    const uint32_t ks = smem_u32(k_s + (size_t)st * C::K_BYTES);
     const uint32_t qs = smem_u32(q_s);
 #pragma unroll
     for (int k16 = 0; k16 < D / 16; ++k16) {
@@ -177,28 +180,31 @@ __device__ __forceinline__ void attn_mma(const AttnParams& p, AttnShared& sh, ui
       umma_bf16(tmem_base + C::TM_S + (g2 & 1) * AT_BN, da, db, idesc_qk, k16 != 0);
     }
     umma_commit(smem_u32(&sh.s_full[g2 & 1]));
+    umma_commit(smem_u32(&sh.k_empty[st]));                    // the K tile is free once QK^T has retired
   };
   while (walk.next(sg)) {
     mbar_wait(smem_u32(&sh.q_ready), n_seg & 1);
     ++n_seg;
     tc_fence_after();
     issue_qk(gt);
+    if (sg.n_tiles > 1) issue_qk(gt + 1);
     for (int t = 0; t < sg.n_tiles; ++t, ++gt) {
-      if (t + 1 < sg.n_tiles) issue_qk(gt + 1);
-      const int st = gt % C::STAGES;
-      mbar_wait(smem_u32(&sh.p_full), gt & 1);
-      mbar_wait(smem_u32(&sh.o_empty[gt & 1]), ((gt >> 1) & 1) ^ 1);
+      const int st = gt % C::STAGES_V, g = gt & 1;
+      mbar_wait(smem_u32(&sh.v_full[st]), (gt / C::STAGES_V) & 1);
+      mbar_wait(smem_u32(&sh.p_full[g]), (gt >> 1) & 1);
+      mbar_wait(smem_u32(&sh.o_empty[g]), ((gt >> 1) & 1) ^ 1);
       tc_fence_after();
-      const uint32_t vs = smem_u32(kv_s + (size_t)st * C::STAGE_BYTES) + C::K_BYTES;
-      const uint32_t ps = smem_u32(p_s);
+      const uint32_t vs = smem_u32(v_s + (size_t)st * C::K_BYTES);
+      const uint32_t ps = smem_u32(g ? p1_s : p0_s);
 #pragma unroll
       for (int k16 = 0; k16 < AT_BN / 16; ++k16) {
         const uint64_t da = umma_desc(ps + (k16 >> 2) * C::Q_HALF + (k16 & 3) * 32, 16, 1024);
         const uint64_t db = umma_desc(vs + k16 * 2048, C::KV_HALF, 1024);               // MN-major
-        umma_bf16(tmem_base + C::TM_O + (gt & 1) * D, da, db, idesc_pv, k16 != 0);
+        umma_bf16(tmem_base + C::TM_O + g * D, da, db, idesc_pv, k16 != 0);
       }
-      umma_commit(smem_u32(&sh.pv_done));
-      umma_commit(smem_u32(&sh.kv_empty[st]));
+      umma_commit(smem_u32(&sh.pv_done[g]));
+      umma_commit(smem_u32(&sh.v_empty[st]));
+      if (t + 2 < sg.n_tiles) issue_qk(gt + 2);
     }
   }
 }
@@ -209,26 +215,31 @@ __device__ __forceinline__ void tmem_ld_frag(uint32_t taddr, uint32_t (&v)[N]) {
   if constexpr (N == 64) tmem_ld_16x256b_x16(taddr, v); else tmem_ld_16x256b_x8(taddr, v);
 }
 
-// ================= warps 0-3: softmax, O accumulation, output, split merge =================
+// ================= warps 0-3 (group 0) and 4-7 (group 1): softmax, O accumulation, output, merges =================
+// The two groups ping-pong over the tiles: group g takes the tiles whose global counter has parity g and
+// keeps its own running (m, l, O); at the end of a segment group 1 hands its state to group 0 through smem.
 template <int D>
-__device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared& sh, uint8_t* q_s, uint8_t* p_s, uint8_t* kv_s,
-                                             uint32_t tmem_base, int warp, int lane) {
+__device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared& sh, uint8_t* q_s, uint8_t* p0_s, uint8_t* p1_s,
+                                             uint8_t* v_s, uint32_t tmem_base, int warp, int lane) {
   using C = AttnCfg<D>;
   constexpr int NO = D / 2;                                    // O registers per thread (2 rows x D/4 columns)
   const int Hkv = p.kv.n_kv_heads;
-  const int stid = warp * 32 + lane;                           // 0..127
-  const int rw = lane >> 2, cq = (lane & 3) * 2;               // row within the warp's 8-row group, first column of the pair
-  const int row_lo = warp * 16 + rw;                           // this thread's rows: row_lo and row_lo + 8
-  const uint32_t t_lane = tmem_base + ((uint32_t)(warp * 32) << 16);
+  const int grp = warp >> 2, qw = warp & 3;                    // group, TMEM lane quarter
+  const int stid = qw * 32 + lane;                             // 0..127 inside the group
+  const int rw = lane >> 2, cq = (lane & 3) * 2;               // row within the 8-row group, first column of the pair
+  const int row_lo = qw * 16 + rw;                             // this thread's rows: row_lo and row_lo + 8
+  const uint32_t t_lane = tmem_base + ((uint32_t)(qw * 32) << 16);
+  uint8_t* p_s = grp ? p1_s : p0_s;
+  float* xch = reinterpret_cast<float*>(q_s);                  // [NO][128] group-merge buffer (Q + P1 regions)
   const int T = sh.total_tiles, G = sh.g_eff;
   SegWalker walk(p, T, G, blockIdx.x);
   Segment sg;
-  uint32_t gt = 0;
+  uint32_t gt0 = 0;                                            // global tile counter at the start of the segment
   while (walk.next(sg)) {
     const int R = sg.q_b * p.group;
-    // ---- Q tile -> smem (K-major, 128-byte swizzle); rows >= R are zero.  All MMAs of the previous
-    //      segment have retired: this thread waited for its last pv_done. ----
-    for (int c = stid; c < AT_ROWS * (D / 8); c += 128) {
+    // ---- Q tile -> smem (K-major, 128-byte swizzle) by both groups; rows >= R are zero.  Every MMA of the
+    //      previous segment has retired (both groups waited for their last pv_done). ----
+    for (int c = grp * 128 + stid; c < AT_ROWS * (D / 8); c += 256) {
       const int rr = c / (D / 8), chn = c % (D / 8);
       uint4 v = make_uint4(0, 0, 0, 0);
       if (rr < R) {
@@ -248,25 +259,29 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared& sh
     lim[0] = min(sg.k1, sg.ctx + row_lo / p.group + 1);
     lim[1] = min(sg.k1, sg.ctx + (row_lo + 8) / p.group + 1);
 
-    auto fold_o = [&](uint32_t g2) {                           // o = o * alpha_prev + O_tile(g2)
+    auto fold_o = [&]() {                                      // o = o * alpha_prev + O_tile (this group's buffer)
       uint32_t v[NO];
-      tmem_ld_frag<NO>(t_lane + C::TM_O + (g2 & 1) * D, v);
+      tmem_ld_frag<NO>(t_lane + C::TM_O + grp * D, v);
       tmem_ld_wait();
       tc_fence_before();
-      mbar_arrive(smem_u32(&sh.o_empty[g2 & 1]));
+      mbar_arrive(smem_u32(&sh.o_empty[grp]));
 #pragma unroll
       for (int c = 0; c < NO; ++c) o[c] = fmaf(o[c], alpha_prev[(c >> 1) & 1], __uint_as_float(v[c]));
     };
 
-    for (int t = 0; t < sg.n_tiles; ++t, ++gt) {
+    bool pending = false;                                      // a PV of this group is in flight and not folded yet
+    uint32_t g_prev = 0;
+    const int t_first = ((gt0 & 1) == (uint32_t)grp) ? 0 : 1;
+    for (int t = t_first; t < sg.n_tiles; t += 2) {
+      const uint32_t g2 = gt0 + t;
       const int tk0 = sg.k0 + t * AT_BN;
-      mbar_wait(smem_u32(&sh.s_full[gt & 1]), (gt >> 1) & 1);
+      mbar_wait(smem_u32(&sh.s_full[grp]), (g2 >> 1) & 1);
       tc_fence_after();
       uint32_t sv[64];
-      tmem_ld_16x256b_x16(t_lane + C::TM_S + (gt & 1) * AT_BN, sv);
+      tmem_ld_16x256b_x16(t_lane + C::TM_S + grp * AT_BN, sv);
       tmem_ld_wait();
       tc_fence_before();
-      mbar_arrive(smem_u32(&sh.s_empty[gt & 1]));              // S buffer may be overwritten by QK(t+2)
+      mbar_arrive(smem_u32(&sh.s_empty[grp]));                 // S buffer may be overwritten by QK(g2 + 2)
 
       if (tk0 + AT_BN > min(sg.ctx + 1, sg.k1)) {              // causal / tail mask
 #pragma unroll
@@ -285,15 +300,15 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared& sh
         mx[h] = fmaxf(mx[h], __shfl_xor_sync(0xffffffffu, mx[h], 2));
         const float m_new = fmaxf(m_run[h], mx[h] * p.scale_log2);
         m_use[h] = m_new == -INFINITY ? 0.f : m_new;
-        alpha[h] = exp2f(m_run[h] - m_use[h]);
+        alpha[h] = fast_exp2(m_run[h] - m_use[h]);
         m_run[h] = m_new;
       }
       uint32_t pk[32];
 #pragma unroll
       for (int c = 0; c < 64; c += 2) {
         const int h = (c >> 1) & 1;
-        const float p0 = exp2f(fmaf(__uint_as_float(sv[c]), p.scale_log2, -m_use[h]));
-        const float p1 = exp2f(fmaf(__uint_as_float(sv[c + 1]), p.scale_log2, -m_use[h]));
+        const float p0 = fast_exp2(fmaf(__uint_as_float(sv[c]), p.scale_log2, -m_use[h]));
+        const float p1 = fast_exp2(fmaf(__uint_as_float(sv[c + 1]), p.scale_log2, -m_use[h]));
         rs[h] += p0 + p1;
         pk[c >> 1] = pack_bf16(p0, p1);
       }
@@ -303,17 +318,17 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared& sh
       if (tk0 + AT_BN > sg.k1) {
         // Last tile of the sequence: keys >= k1 hold stale or never-written V bits.  Zero them so that
         // 0 * garbage cannot produce NaN in the PV product (P is exactly 0 there).
-        mbar_wait(smem_u32(&sh.kv_full[gt % C::STAGES]), (gt / C::STAGES) & 1);
+        mbar_wait(smem_u32(&sh.v_full[g2 % C::STAGES_V]), (g2 / C::STAGES_V) & 1);
         const int key = (sg.k1 - tk0) + stid;
         if (key < AT_BN) {
-          uint8_t* vrow = kv_s + (size_t)(gt % C::STAGES) * C::STAGE_BYTES + C::K_BYTES + key * 128;
+          uint8_t* vrow = v_s + (size_t)(g2 % C::STAGES_V) * C::K_BYTES + key * 128;
 #pragma unroll
           for (int h = 0; h < C::NH; ++h)
 #pragma unroll
             for (int c = 0; c < 8; ++c) *reinterpret_cast<uint4*>(vrow + h * C::KV_HALF + c * 16) = make_uint4(0, 0, 0, 0);
         }
       }
-      if (t > 0) mbar_wait(smem_u32(&sh.pv_done), (gt - 1) & 1);          // PV(t-1) retired: P is free, O(t-1) is ready
+      if (pending) mbar_wait(smem_u32(&sh.pv_done[grp]), (g_prev >> 1) & 1);   // own PV retired: P is free, O is ready
 #pragma unroll
       for (int j = 0; j < 16; ++j) {                           // P -> smem, K-major 128-byte swizzle
         const uint32_t off = (j >> 3) * C::Q_HALF + (((j & 7) ^ (rw & 7)) << 4) + cq * 2;
@@ -321,14 +336,50 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared& sh
         *reinterpret_cast<uint32_t*>(p_s + off + (row_lo + 8) * 128) = pk[2 * j + 1];
       }
       fence_proxy_async();
-      mbar_arrive(smem_u32(&sh.p_full));
-      if (t > 0) { tc_fence_after(); fold_o(gt - 1); }
+      mbar_arrive(smem_u32(&sh.p_full[grp]));
+      if (pending) { tc_fence_after(); fold_o(); }
       alpha_prev[0] = alpha[0];
       alpha_prev[1] = alpha[1];
+      pending = true;
+      g_prev = g2;
     }
-    mbar_wait(smem_u32(&sh.pv_done), (gt - 1) & 1);
-    tc_fence_after();
-    fold_o(gt - 1);
+    if (pending) {
+      mbar_wait(smem_u32(&sh.pv_done[grp]), (g_prev >> 1) & 1);
+      tc_fence_after();
+      fold_o();
+    } else {
+      // one-tile segment owned by the other group: wait for its PV so that every MMA reading Q / P has retired
+      mbar_wait(smem_u32(&sh.pv_done[grp ^ 1]), (gt0 >> 1) & 1);
+    }
+    gt0 += sg.n_tiles;
+
+    // ---- group 1 hands (m, l, O) to group 0 through smem (Q and P1 are idle: every MMA has retired) ----
+    if (grp == 1) {
+#pragma unroll
+      for (int c = 0; c < NO; ++c) xch[c * 128 + stid] = o[c];
+      sh.xm[0][stid] = m_run[0]; sh.xm[1][stid] = m_run[1];
+      sh.xl[0][stid] = l_run[0]; sh.xl[1][stid] = l_run[1];
+      named_bar_sync(4, 256);
+      named_bar_sync(5, 256);                                  // group 0 has read the buffer: Q may be rewritten
+      continue;
+    }
+    named_bar_sync(4, 256);
+    {
+      float e0[2], e1[2];
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        const float m1 = sh.xm[h][stid], l1 = sh.xl[h][stid];
+        const float m = fmaxf(m_run[h], m1);
+        const float mu = m == -INFINITY ? 0.f : m;
+        e0[h] = fast_exp2(m_run[h] - mu);
+        e1[h] = fast_exp2(m1 - mu);
+        l_run[h] = l_run[h] * e0[h] + l1 * e1[h];
+        m_run[h] = m;
+      }
+#pragma unroll
+      for (int c = 0; c < NO; ++c) o[c] = o[c] * e0[(c >> 1) & 1] + xch[c * 128 + stid] * e1[(c >> 1) & 1];
+    }
+    named_bar_sync(5, 256);
 
     // ---- finish the rows: quad-reduce the row sums, write final rows or the partial ----
 #pragma unroll
@@ -356,7 +407,7 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared& sh
     }
     if (!sg.partial) continue;
 
-    // ---- merge by the last CTA to finish the (b, g) pair ----
+    // ---- merge by the last CTA to finish the (b, g) pair (group 0 only) ----
     const int c_first = cta_of_tile(sg.flat0, T, G), c_last = cta_of_tile(sg.flat0 + sg.nt - 1, T, G);
     const int n_seg = c_last - c_first + 1;
     __threadfence();
@@ -373,14 +424,14 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared& sh
     // the head partial of every CTA is slot 2c; only the first CTA can hold the pair as its tail (slot 2c+1)
     const int first_slot = 2 * c_first + ((int)((long long)c_first * T / G) < sg.flat0 ? 1 : 0);
     auto slot_of = [&](int s) { return s == 0 ? first_slot : 2 * (c_first + s); };
-    float (*wgt)[AT_MAX_SEG] = reinterpret_cast<float (*)[AT_MAX_SEG]>(p_s);   // P is idle: every PV has retired
+    float (*wgt)[AT_MAX_SEG] = reinterpret_cast<float (*)[AT_MAX_SEG]>(p0_s);   // P0 is idle: its last PV has retired
     if (stid < R) {                                            // weights: w_s = 2^(m_s - m) / sum_s l_s 2^(m_s - m)
       float m = -INFINITY;
       for (int s = 0; s < n_seg; ++s) m = fmaxf(m, __ldcg(&p.ws_ml[(size_t)slot_of(s) * AT_ROWS + stid].x));
       float l = 0.f;
       for (int s = 0; s < n_seg; ++s) {
         const float2 ml = __ldcg(&p.ws_ml[(size_t)slot_of(s) * AT_ROWS + stid]);
-        const float w = exp2f(ml.x - m);                       // -inf partials get weight 0
+        const float w = fast_exp2(ml.x - m);                       // -inf partials get weight 0
         wgt[stid][s] = w;
         l += ml.y * w;
       }
@@ -411,9 +462,11 @@ __global__ void __launch_bounds__(AT_THREADS, 1) wf_verify_attn_kernel(const Att
   extern __shared__ __align__(1024) uint8_t smem[];
   __shared__ __align__(8) AttnShared sh;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  uint8_t* q_s = smem;
-  uint8_t* p_s = smem + C::Q_BYTES;
-  uint8_t* kv_s = p_s + C::P_BYTES;
+  uint8_t* p0_s = smem;                                        // smem map: P0 | Q | P1 | K ring | V ring
+  uint8_t* q_s = p0_s + C::P_BYTES;
+  uint8_t* p1_s = q_s + C::Q_BYTES;
+  uint8_t* k_s = p1_s + C::P_BYTES;
+  uint8_t* v_s = k_s + C::STAGES_K * C::K_BYTES;
 
   // total tiles and the longest pair, from the device-resident lengths (identical in every CTA)
   int part = 0, longest = 0;
@@ -430,18 +483,21 @@ __global__ void __launch_bounds__(AT_THREADS, 1) wf_verify_attn_kernel(const Att
   }
   if (lane == 0) { sh.red[0][warp] = part; sh.red[1][warp] = longest; }
   if (tid == 0) {
-    for (int i = 0; i < C::STAGES; ++i) { mbar_init(smem_u32(&sh.kv_full[i]), 1); mbar_init(smem_u32(&sh.kv_empty[i]), 1); }
+    for (int i = 0; i < AT_MAX_STAGES; ++i) {
+      mbar_init(smem_u32(&sh.k_full[i]), 1); mbar_init(smem_u32(&sh.k_empty[i]), 1);
+      mbar_init(smem_u32(&sh.v_full[i]), 1); mbar_init(smem_u32(&sh.v_empty[i]), 1);
+    }
     for (int i = 0; i < 2; ++i) {
       mbar_init(smem_u32(&sh.s_full[i]), 1);
       mbar_init(smem_u32(&sh.s_empty[i]), 128);
       mbar_init(smem_u32(&sh.o_empty[i]), 128);
+      mbar_init(smem_u32(&sh.p_full[i]), 128);
+      mbar_init(smem_u32(&sh.pv_done[i]), 1);
     }
-    mbar_init(smem_u32(&sh.p_full), 128);
-    mbar_init(smem_u32(&sh.pv_done), 1);
-    mbar_init(smem_u32(&sh.q_ready), 128);
+    mbar_init(smem_u32(&sh.q_ready), 256);
     fence_barrier_init();
   }
-  if (warp == 5) tmem_alloc(smem_u32(&sh.tmem), 512);
+  if (warp == 9) tmem_alloc(smem_u32(&sh.tmem), 512);
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
@@ -458,17 +514,19 @@ __global__ void __launch_bounds__(AT_THREADS, 1) wf_verify_attn_kernel(const Att
   __syncthreads();
 
   if (sh.total_tiles > 0 && (int)blockIdx.x < sh.g_eff) {
-    if (warp == 4) {
-      attn_loader<D>(p, sh, kv_s, lane);
-    } else if (warp == 5) {
-      if (lane == 0) attn_mma<D>(p, sh, q_s, p_s, kv_s, tmem_base);
+    if (warp < 8) {
+      asm volatile("setmaxnreg.inc.sync.aligned.u32 216;");
+      attn_softmax<D>(p, sh, q_s, p0_s, p1_s, v_s, tmem_base, warp, lane);
     } else {
-      attn_softmax<D>(p, sh, q_s, p_s, kv_s, tmem_base, warp, lane);
+      asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
+      if (warp == 8) attn_loader<D>(p, sh, k_s, 0, lane);
+      else if (warp == 10) attn_loader<D>(p, sh, v_s, 1, lane);
+      else if (warp == 9 && lane == 0) attn_mma<D>(p, sh, q_s, p0_s, p1_s, k_s, v_s, tmem_base);
     }
   }
   tc_fence_before();
   __syncthreads();
-  if (warp == 5) tmem_dealloc(tmem_base, 512);
+  if (warp == 9) tmem_dealloc(tmem_base, 512);
 }
 
 }  // namespace

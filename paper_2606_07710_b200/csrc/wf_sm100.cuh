@@ -109,6 +109,12 @@ __device__ __forceinline__ void cp_async16_zfill(uint32_t dst, const void* src, 
   const int n = valid ? 16 : 0;
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(n) : "memory");
 }
+// 2^x on the SFU: one MUFU.EX2, flush-to-zero, ex2(-inf) = +0 (exp2f() adds range-scaling code around it)
+__device__ __forceinline__ float fast_exp2(float x) {
+  float y;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
 __device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
   asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
