@@ -155,14 +155,21 @@ __device__ __forceinline__ void attn_loader(const AttnParams& p, AttnShared& sh,
   }
 }
 
-// ================= warp 9, one thread: MMA issuer =================
+// ================= warp 9: MMA issuer =================
 // Tile g2 (global tile counter) belongs to softmax group g2 & 1, which owns S[g2&1], P[g2&1], O[g2&1].
+// The whole warp runs the loop so that addresses and descriptors stay warp-uniform; one elected lane
+// issues the tcgen05 instructions.  Descriptors are built once and advanced by constant offsets.
 template <int D>
 __device__ __forceinline__ void attn_mma(const AttnParams& p, AttnShared& sh, uint8_t* q_s, uint8_t* p0_s, uint8_t* p1_s,
                                          uint8_t* k_s, uint8_t* v_s, uint32_t tmem_base) {
   using C = AttnCfg<D>;
   const uint32_t idesc_qk = umma_idesc_kk(AT_ROWS, AT_BN);
   const uint32_t idesc_pv = umma_idesc(AT_ROWS, D);
+  const uint64_t dq0 = umma_desc(smem_u32(q_s), 16, 1024);                  // K-major
+  const uint64_t dk0 = umma_desc(smem_u32(k_s), 16, 1024);                  // K-major
+  const uint64_t dp0 = umma_desc(smem_u32(p0_s), 16, 1024);                 // K-major
+  const uint64_t dp1 = umma_desc(smem_u32(p1_s), 16, 1024);
+  const uint64_t dv0 = umma_desc(smem_u32(v_s), C::KV_HALF, 1024);          // MN-major
   SegWalker walk(p, sh.total_tiles, sh.g_eff, blockIdx.x);
   Segment sg;
   uint32_t gt = 0, n_seg = 0;
@@ -171,16 +178,17 @@ __device__ __forceinline__ void attn_mma(const AttnParams& p, AttnShared& sh, ui
     mbar_wait(smem_u32(&sh.k_full[st]), (g2 / C::STAGES_K) & 1);
     mbar_wait(smem_u32(&sh.s_empty[g2 & 1]), ((g2 >> 1) & 1) ^ 1);
     tc_fence_after();
-    const uint32_t ks = smem_u32(k_s + (size_t)st * C::K_BYTES);
-    const uint32_t qs = smem_u32(q_s);
+    if (elect_one()) {
+      const uint64_t dk = dk0 + (uint64_t)((st * C::K_BYTES) >> 4);
+      const uint32_t td = tmem_base + C::TM_S + (g2 & 1) * AT_BN;
 #pragma unroll
-    for (int k16 = 0; k16 < D / 16; ++k16) {
-      const uint64_t da = umma_desc(qs + (k16 >> 2) * C::Q_HALF + (k16 & 3) * 32, 16, 1024);
-      const uint64_t db = umma_desc(ks + (k16 >> 2) * C::KV_HALF + (k16 & 3) * 32, 16, 1024);
-      umma_bf16(tmem_base + C::TM_S + (g2 & 1) * AT_BN, da, db, idesc_qk, k16 != 0);
+      for (int k16 = 0; k16 < D / 16; ++k16)
+        umma_bf16(td, dq0 + (uint64_t)(((k16 >> 2) * C::Q_HALF + (k16 & 3) * 32) >> 4),
+                  dk + (uint64_t)(((k16 >> 2) * C::KV_HALF + (k16 & 3) * 32) >> 4), idesc_qk, k16 != 0);
+      umma_commit(smem_u32(&sh.s_full[g2 & 1]));
+      umma_commit(smem_u32(&sh.k_empty[st]));                  // the K tile is free once QK^T has retired
     }
-    umma_commit(smem_u32(&sh.s_full[g2 & 1]));
-    umma_commit(smem_u32(&sh.k_empty[st]));                    // the K tile is free once QK^T has retired
+    __syncwarp();
   };
   while (walk.next(sg)) {
     mbar_wait(smem_u32(&sh.q_ready), n_seg & 1);
@@ -194,16 +202,18 @@ __device__ __forceinline__ void attn_mma(const AttnParams& p, AttnShared& sh, ui
       mbar_wait(smem_u32(&sh.p_full[g]), (gt >> 1) & 1);
       mbar_wait(smem_u32(&sh.o_empty[g]), ((gt >> 1) & 1) ^ 1);
       tc_fence_after();
-      const uint32_t vs = smem_u32(v_s + (size_t)st * C::K_BYTES);
-      const uint32_t ps = smem_u32(g ? p1_s : p0_s);
+      if (elect_one()) {
+        const uint64_t dv = dv0 + (uint64_t)((st * C::K_BYTES) >> 4);
+        const uint64_t dp = g ? dp1 : dp0;
+        const uint32_t td = tmem_base + C::TM_O + g * D;
 #pragma unroll
-      for (int k16 = 0; k16 < AT_BN / 16; ++k16) {
-        const uint64_t da = umma_desc(ps + (k16 >> 2) * C::Q_HALF + (k16 & 3) * 32, 16, 1024);
-        const uint64_t db = umma_desc(vs + k16 * 2048, C::KV_HALF, 1024);               // MN-major
-        umma_bf16(tmem_base + C::TM_O + g * D, da, db, idesc_pv, k16 != 0);
+        for (int k16 = 0; k16 < AT_BN / 16; ++k16)
+          umma_bf16(td, dp + (uint64_t)(((k16 >> 2) * C::Q_HALF + (k16 & 3) * 32) >> 4), dv + (uint64_t)((k16 * 2048) >> 4),
+                    idesc_pv, k16 != 0);
+        umma_commit(smem_u32(&sh.pv_done[g]));
+        umma_commit(smem_u32(&sh.v_empty[st]));
       }
-      umma_commit(smem_u32(&sh.pv_done[g]));
-      umma_commit(smem_u32(&sh.v_empty[st]));
+      __syncwarp();
       if (t + 2 < sg.n_tiles) issue_qk(gt + 2);
     }
   }
@@ -521,7 +531,7 @@ __global__ void __launch_bounds__(AT_THREADS, 1) wf_verify_attn_kernel(const Att
       asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
       if (warp == 8) attn_loader<D>(p, sh, k_s, 0, lane);
       else if (warp == 10) attn_loader<D>(p, sh, v_s, 1, lane);
-      else if (warp == 9 && lane == 0) attn_mma<D>(p, sh, q_s, p0_s, p1_s, k_s, v_s, tmem_base);
+      else if (warp == 9) attn_mma<D>(p, sh, q_s, p0_s, p1_s, k_s, v_s, tmem_base);
     }
   }
   tc_fence_before();
