@@ -5,17 +5,20 @@
 // the `group` query heads that share kv head g (<= 64 rows), so K and V are read from HBM once per kv
 // head.  Work is the flattened list of 128-key tiles over all (b, g) pairs; persistent CTA c (one per
 // SM) owns the contiguous tile range [c*T/G, (c+1)*T/G) (stream-K), which every CTA derives from the
-// device-resident lengths (no host sync).  A range cuts at most two (b, g) pairs, so a CTA writes at
-// most two fp32 partials; the last CTA to finish a pair merges its few partials.  Warp roles:
-//   warps 8,10: TMA producers (K ring, V ring).  Per tile, lane p issues the 16-key page p
-//               (cp.async.bulk.tensor.2d, 128-byte swizzle); a K tile is released when its QK^T retires.
+// device-resident lengths (no host sync).  A range cuts at most two (b, g) pairs.  The last CTA to
+// arrive at a shared pair keeps its partial in registers and folds in the partials the others
+// published (fragment-order float4, coalesced); nobody re-reads its own partial.  Warp roles:
+//   warps 8,10: TMA producers (K ring, V ring).  One elected lane issues the 16 page boxes of a tile
+//               (cp.async.bulk.tensor.2d, 128-byte swizzle) in straight-line code; the page ids of the
+//               next tile are prefetched; a K tile is released when its QK^T retires.
 //   warp 9    : MMA issuer (one thread).  S = Q K^T (UMMA 64 x 128 x 16, both K-major) into TMEM,
 //               double buffered; O_t = P V (64 x D x 16, V MN-major) into TMEM, double buffered.
-//   warps 0-7 : softmax, two groups of 4 warps that ping-pong over the tiles.  UMMA M = 64 puts rows 16w..16w+15 on TMEM lanes 32w..32w+15, so warp w owns
-//               16 rows; tcgen05.ld.16x256b hands them out like an mma C fragment (a quad per row).
-//               Online softmax in the log2 domain with quad shuffles, P goes to smem as the bf16 A
-//               operand of the PV MMA, the per-tile O_t is folded into fp32 registers with the running
-//               rescale.  QK^T of tile t+1 and PV of tile t overlap the softmax of tile t+1.
+//               QK^T of tile t+2 is issued ahead of PV of tile t.
+//   warps 0-7 : softmax, two groups of 4 warps that ping-pong over the tiles.  UMMA M = 64 puts rows
+//               16w..16w+15 on TMEM lanes 32w..32w+15, so warp w owns 16 rows; tcgen05.ld.16x256b hands
+//               them out like an mma C fragment (a quad per row).  Online softmax in the log2 domain
+//               with quad shuffles, P goes to smem as the bf16 A operand of the PV MMA, the per-tile
+//               O_t is folded into fp32 registers with the running rescale.
 #include "wf_internal.cuh"
 #include "wf_sm100.cuh"
 
@@ -37,9 +40,9 @@ struct AttnParams {
   KvView kv;
   int layer, B, n_q_heads, group;
   float scale_log2;                    // sm_scale * log2(e)
-  float* ws_o;                         // [2 * CTAs][64][D] fp32, unnormalised
-  float2* ws_ml;                       // [2 * CTAs][64] (m in log2 units, l)
-  unsigned int* counters;              // [B * Hkv], self-resetting
+  float4* ws_o;                        // [2 * CTAs][D/8][128 threads] float4: unnormalised O in fragment order
+  float4* ws_ml;                       // [2 * CTAs][128 threads] (m, l) of the thread's two rows (m in log2 units)
+  unsigned int* counters;              // [B * Hkv][2] (arrived, published), self-resetting
 };
 
 template <int D>
@@ -134,23 +137,37 @@ __device__ __forceinline__ void attn_loader(const AttnParams& p, AttnShared& sh,
   SegWalker walk(p, sh.total_tiles, sh.g_eff, blockIdx.x);
   Segment sg;
   uint32_t gt = 0;
+  constexpr int PP = AT_BN / 16;                              // pages per tile
+  const void* tmap = kv.tmaps + which;
+  const uint32_t ring_s = smem_u32(ring);
   while (walk.next(sg)) {
-    const int32_t* bt = kv.block_table + (size_t)sg.b * kv.max_pages_per_seq;
+    const int32_t* bt = kv.block_table + (size_t)sg.b * kv.max_pages_per_seq + (sg.k0 >> 4);
+    const int pages_seg = (sg.k1 - sg.k0 + 15) >> 4;           // pages of this segment, tile t takes [8t, 8t+8)
+    // The page ids of tile t+1 are fetched while tile t is issued: the block-table latency is off the ring's
+    // critical path.  Lane q holds page q of the tile.
+    int page_next = lane < min(PP, pages_seg) ? __ldg(bt + lane) : 0;
     for (int t = 0; t < sg.n_tiles; ++t, ++gt) {
       const int n_st = which ? C::STAGES_V : C::STAGES_K;
       const int st = gt % n_st;
-      mbar_wait(smem_u32(&empty[st]), ((gt / n_st) & 1) ^ 1);
-      const int tk0 = sg.k0 + t * AT_BN;
-      const int npages = min(AT_BN / 16, (sg.k1 - tk0 + 15) >> 4);
-      if (lane == 0) mbar_arrive_expect_tx(smem_u32(&full[st]), (uint32_t)npages * 16 * D * 2);
-      __syncwarp();
-      if (lane < npages) {
-        const int page = __ldg(bt + (tk0 >> 4) + lane);
-        const int row = (((p.layer * kv.num_pages + page) * kv.n_kv_heads) + sg.g) * 16;
-        const uint32_t dst = smem_u32(ring + (size_t)st * C::K_BYTES) + lane * 2048;
+      const int npages = min(PP, pages_seg - t * PP);
+      const int row = (((p.layer * kv.num_pages + page_next) * kv.n_kv_heads) + sg.g) * 16;
+      if ((t + 1) * PP + lane < pages_seg && lane < PP) page_next = __ldg(bt + (t + 1) * PP + lane);
+      int rows[PP];
 #pragma unroll
-        for (int h = 0; h < C::NH; ++h) tma_load_2d(dst + h * C::KV_HALF, kv.tmaps + which, h * 64, row, smem_u32(&full[st]));
+      for (int q = 0; q < PP; ++q) rows[q] = __shfl_sync(0xffffffffu, row, q);
+      mbar_wait(smem_u32(&empty[st]), ((gt / n_st) & 1) ^ 1);
+      if (elect_one()) {                                       // one lane issues the whole tile: straight-line TMA issue
+        const uint32_t bar = smem_u32(&full[st]);
+        const uint32_t dst = ring_s + (uint32_t)st * C::K_BYTES;
+        mbar_arrive_expect_tx(bar, (uint32_t)npages * 16 * D * 2);
+#pragma unroll
+        for (int q = 0; q < PP; ++q)
+          if (q < npages) {
+#pragma unroll
+            for (int h = 0; h < C::NH; ++h) tma_load_2d(dst + q * 2048 + h * C::KV_HALF, tmap, h * 64, rows[q], bar);
+          }
       }
+      __syncwarp();
     }
   }
 }
@@ -197,6 +214,9 @@ __device__ __forceinline__ void attn_mma(const AttnParams& p, AttnShared& sh, ui
     issue_qk(gt);
     if (sg.n_tiles > 1) issue_qk(gt + 1);
     for (int t = 0; t < sg.n_tiles; ++t, ++gt) {
+      // QK^T of tile t+2 goes ahead of PV of tile t: its S buffer was released as soon as the softmax group
+      // had S(t) in registers, so S(t+2) is ready when the group comes back and the group never idles on it.
+      if (t + 2 < sg.n_tiles) issue_qk(gt + 2);
       const int st = gt % C::STAGES_V, g = gt & 1;
       mbar_wait(smem_u32(&sh.v_full[st]), (gt / C::STAGES_V) & 1);
       mbar_wait(smem_u32(&sh.p_full[g]), (gt >> 1) & 1);
@@ -214,7 +234,6 @@ __device__ __forceinline__ void attn_mma(const AttnParams& p, AttnShared& sh, ui
         umma_commit(smem_u32(&sh.v_empty[st]));
       }
       __syncwarp();
-      if (t + 2 < sg.n_tiles) issue_qk(gt + 2);
     }
   }
 }
@@ -397,72 +416,82 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared& sh
       l_run[h] += __shfl_xor_sync(0xffffffffu, l_run[h], 1);
       l_run[h] += __shfl_xor_sync(0xffffffffu, l_run[h], 2);
     }
+    auto write_rows = [&]() {                                  // normalise and store this thread's two rows
 #pragma unroll
-    for (int h = 0; h < 2; ++h) {
-      const int r = row_lo + 8 * h;
-      if (r >= R) continue;
-      if (!sg.partial) {
+      for (int h = 0; h < 2; ++h) {
+        const int r = row_lo + 8 * h;
+        if (r >= R) continue;
         const float inv = 1.f / l_run[h];                      // every row sees key 0: l > 0
         const int qi = r / p.group, hg = r % p.group;
         __nv_bfloat16* dst = p.out + ((size_t)(sg.r0 + qi) * p.n_q_heads + sg.g * p.group + hg) * D + cq;
 #pragma unroll
         for (int j = 0; j < D / 8; ++j)
           *reinterpret_cast<uint32_t*>(dst + 8 * j) = pack_bf16(o[4 * j + 2 * h] * inv, o[4 * j + 2 * h + 1] * inv);
-      } else {
-        float* dst = p.ws_o + ((size_t)sg.slot * AT_ROWS + r) * D + cq;
-#pragma unroll
-        for (int j = 0; j < D / 8; ++j) *reinterpret_cast<float2*>(dst + 8 * j) = make_float2(o[4 * j + 2 * h], o[4 * j + 2 * h + 1]);
-        if ((lane & 3) == 0) p.ws_ml[(size_t)sg.slot * AT_ROWS + r] = make_float2(m_run[h], l_run[h]);
       }
-    }
-    if (!sg.partial) continue;
+    };
+    if (!sg.partial) { write_rows(); continue; }
 
-    // ---- merge by the last CTA to finish the (b, g) pair (group 0 only) ----
+    // ---- the pair is shared with other CTAs (group 0 only from here).  The LAST CTA to arrive keeps its
+    //      partial in registers and folds the others' partials into it; every other CTA publishes its
+    //      partial in fragment order (thread-major float4: coalesced for writer and reader alike).
+    //      In steady state the last arriver is the CTA that holds the pair's head at the end of its range,
+    //      and the others published long ago. ----
     const int c_first = cta_of_tile(sg.flat0, T, G), c_last = cta_of_tile(sg.flat0 + sg.nt - 1, T, G);
     const int n_seg = c_last - c_first + 1;
-    __threadfence();
-    named_bar_sync(3, 128);
-    if (stid == 0) {
-      const unsigned int old = atomicAdd(&p.counters[sg.b * Hkv + sg.g], 1u);
-      sh.last = (old == (unsigned int)n_seg - 1);
-      if (sh.last) p.counters[sg.b * Hkv + sg.g] = 0;
-    }
+    unsigned int* cnt = p.counters + 2 * (sg.b * Hkv + sg.g);  // [0] arrived, [1] published
+    if (stid == 0) sh.last = (atomicAdd(&cnt[0], 1u) == (unsigned int)n_seg - 1);
     named_bar_sync(3, 128);
     const bool last = sh.last != 0;
-    if (!last) { named_bar_sync(3, 128); continue; }
-    __threadfence();
-    // the head partial of every CTA is slot 2c; only the first CTA can hold the pair as its tail (slot 2c+1)
-    const int first_slot = 2 * c_first + ((int)((long long)c_first * T / G) < sg.flat0 ? 1 : 0);
-    auto slot_of = [&](int s) { return s == 0 ? first_slot : 2 * (c_first + s); };
-    float (*wgt)[AT_MAX_SEG] = reinterpret_cast<float (*)[AT_MAX_SEG]>(p0_s);   // P0 is idle: its last PV has retired
-    if (stid < R) {                                            // weights: w_s = 2^(m_s - m) / sum_s l_s 2^(m_s - m)
-      float m = -INFINITY;
-      for (int s = 0; s < n_seg; ++s) m = fmaxf(m, __ldcg(&p.ws_ml[(size_t)slot_of(s) * AT_ROWS + stid].x));
-      float l = 0.f;
-      for (int s = 0; s < n_seg; ++s) {
-        const float2 ml = __ldcg(&p.ws_ml[(size_t)slot_of(s) * AT_ROWS + stid]);
-        const float w = fast_exp2(ml.x - m);                       // -inf partials get weight 0
-        wgt[stid][s] = w;
-        l += ml.y * w;
-      }
-      const float inv = 1.f / l;
-      for (int s = 0; s < n_seg; ++s) wgt[stid][s] *= inv;
+    if (!last) {
+      float4* dst = p.ws_o + (size_t)sg.slot * (NO / 4) * 128 + stid;
+#pragma unroll
+      for (int k = 0; k < NO / 4; ++k) dst[k * 128] = make_float4(o[4 * k], o[4 * k + 1], o[4 * k + 2], o[4 * k + 3]);
+      p.ws_ml[(size_t)sg.slot * 128 + stid] = make_float4(m_run[0], l_run[0], m_run[1], l_run[1]);
+      __threadfence();
+      named_bar_sync(3, 128);                                  // also: sh.last may be rewritten
+      if (stid == 0) atomicAdd(&cnt[1], 1u);
+      continue;
+    }
+    if (stid == 0) {                                           // the others have arrived, so they are running: bounded wait
+      for (uint32_t spins = 0; atomicAdd(&cnt[1], 0u) < (unsigned int)n_seg - 1; ++spins)
+        if (spins > (1u << 24)) __trap();
+      cnt[0] = 0; cnt[1] = 0;                                  // self-resetting for the next launch
+      __threadfence();
     }
     named_bar_sync(3, 128);
-    for (int idx = stid; idx < R * (D / 4); idx += 128) {      // out[r][4 columns] = sum_s w[r][s] O_s[r][4 columns]
-      const int rr = idx / (D / 4), c4 = idx % (D / 4);
-      float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-#pragma unroll 4
-      for (int s = 0; s < n_seg; ++s) {
-        const float4 x = __ldcg(reinterpret_cast<const float4*>(p.ws_o + ((size_t)slot_of(s) * AT_ROWS + rr) * D) + c4);
-        const float w = wgt[rr][s];
-        acc.x = fmaf(w, x.x, acc.x); acc.y = fmaf(w, x.y, acc.y); acc.z = fmaf(w, x.z, acc.z); acc.w = fmaf(w, x.w, acc.w);
+    // the head partial of every CTA is slot 2c; only the first CTA can hold the pair as its tail (slot 2c+1)
+    const int first_slot = 2 * c_first + ((int)((long long)c_first * T / G) < sg.flat0 ? 1 : 0);
+    const int s_own = (int)blockIdx.x - c_first;
+    for (int s2 = 0; s2 < n_seg; ++s2) {
+      if (s2 == s_own) continue;
+      const int slot = s2 == 0 ? first_slot : 2 * (c_first + s2);
+      const float4* src = p.ws_o + (size_t)slot * (NO / 4) * 128 + stid;
+      float4 x[NO / 4];
+#pragma unroll
+      for (int k = 0; k < NO / 4; ++k) x[k] = __ldcg(src + k * 128);
+      const float4 ml = __ldcg(&p.ws_ml[(size_t)slot * 128 + stid]);
+      float e0[2], e1[2];
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        const float m1 = h ? ml.z : ml.x, l1 = h ? ml.w : ml.y;
+        const float m = fmaxf(m_run[h], m1);
+        const float mu = m == -INFINITY ? 0.f : m;
+        e0[h] = fast_exp2(m_run[h] - mu);
+        e1[h] = fast_exp2(m1 - mu);
+        l_run[h] = l_run[h] * e0[h] + l1 * e1[h];
+        m_run[h] = m;
       }
-      const int i2 = rr / p.group, h2 = rr % p.group;
-      __nv_bfloat16* dst = p.out + ((size_t)(sg.r0 + i2) * p.n_q_heads + sg.g * p.group + h2) * D + c4 * 4;
-      *reinterpret_cast<uint2*>(dst) = make_uint2(pack_bf16(acc.x, acc.y), pack_bf16(acc.z, acc.w));
+#pragma unroll
+      for (int k = 0; k < NO / 4; ++k) {
+        const float xv[4] = {x[k].x, x[k].y, x[k].z, x[k].w};
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          const int c = 4 * k + u;
+          o[c] = o[c] * e0[(c >> 1) & 1] + xv[u] * e1[(c >> 1) & 1];
+        }
+      }
     }
-    named_bar_sync(3, 128);                                    // wgt / last are free for the next segment
+    write_rows();
   }
 }
 
@@ -565,7 +594,7 @@ extern "C" size_t wf_verify_attn_workspace_bytes(const wf_kv_shape* s, int B, in
   if (!s || B <= 0 || n_q_heads <= 0 || s->n_kv_heads <= 0) return 16;
   const size_t items = 2 * (size_t)AT_MAX_CTAS;            // a CTA writes at most a head and a tail partial
   const size_t r_pad = AT_ROWS;
-  return items * r_pad * ((size_t)s->head_dim * sizeof(float) + sizeof(float2));
+  return items * (r_pad * (size_t)s->head_dim * sizeof(float) + 128 * sizeof(float4));
 }
 
 extern "C" int wf_verify_attn(wf_ctx* ctx, const wf_paged_kv* kv, int layer, const void* q,
@@ -574,7 +603,7 @@ extern "C" int wf_verify_attn(wf_ctx* ctx, const wf_paged_kv* kv, int layer, con
   if (!ctx) return WF_ERR_INVALID_ARG;
   WF_REQUIRE(ctx, kv && q && q_indptr && out && workspace, WF_ERR_INVALID_ARG, "wf_verify_attn: null argument");
   WF_REQUIRE(ctx, layer >= 0 && layer < kv->s.n_layers, WF_ERR_INVALID_ARG, "wf_verify_attn: bad layer");
-  WF_REQUIRE(ctx, B >= 0 && B <= kv->s.max_seqs && B <= AT_MAX_B && B * kv->s.n_kv_heads <= ctx->n_counters,
+  WF_REQUIRE(ctx, B >= 0 && B <= kv->s.max_seqs && B <= AT_MAX_B && 2 * B * kv->s.n_kv_heads <= ctx->n_counters,
              WF_ERR_INVALID_ARG, "wf_verify_attn: bad B (max %d)", AT_MAX_B);
   WF_REQUIRE(ctx, n_q_heads > 0 && n_q_heads % kv->s.n_kv_heads == 0, WF_ERR_INVALID_ARG,
              "wf_verify_attn: n_q_heads must be a multiple of n_kv_heads");
@@ -595,8 +624,8 @@ extern "C" int wf_verify_attn(wf_ctx* ctx, const wf_paged_kv* kv, int layer, con
   p.kv = kv_view(kv);
   p.layer = layer; p.B = B; p.n_q_heads = n_q_heads; p.group = group;
   p.scale_log2 = sm_scale * LOG2E;
-  p.ws_o = (float*)workspace;
-  p.ws_ml = (float2*)((char*)workspace + items * r_pad * kv->s.head_dim * sizeof(float));
+  p.ws_o = (float4*)workspace;
+  p.ws_ml = (float4*)((char*)workspace + items * r_pad * kv->s.head_dim * sizeof(float));
   p.counters = ctx->d_counters_attn;
   cudaStream_t st = (cudaStream_t)stream;
   const int D = kv->s.head_dim;
