@@ -42,7 +42,7 @@ struct AttnParams {
   float scale_log2;                    // sm_scale * log2(e)
   float4* ws_o;                        // [2 * CTAs][D/8][128 threads] float4: unnormalised O in fragment order
   float4* ws_ml;                       // [2 * CTAs][128 threads] (m, l) of the thread's two rows (m in log2 units)
-  unsigned int* counters;              // [B * Hkv][2] (arrived, published), self-resetting
+  unsigned int* counters;              // [B * Hkv] arrived | published << 16, self-resetting
 };
 
 template <int D>
@@ -65,8 +65,10 @@ struct AttnShared {
   uint64_t k_full[AT_MAX_STAGES], k_empty[AT_MAX_STAGES], v_full[AT_MAX_STAGES], v_empty[AT_MAX_STAGES];
   uint64_t s_full[2], s_empty[2], o_empty[2], p_full[2], pv_done[2], q_ready;
   float xm[2][128], xl[2][128];        // group-1 running max / row-sum partials for the group merge
-  int red[2][AT_THREADS / 32];
-  int total_tiles, g_eff;
+  int pref[AT_MAX_B + 1];              // exclusive prefix of 128-key tiles per kv head over the sequences
+  int r0[AT_MAX_B + 1];                // q_indptr
+  int ctx[AT_MAX_B];                   // seq_len
+  int total_tiles, g_eff, B;
   uint32_t tmem;
   int last;
 };
@@ -79,36 +81,37 @@ struct Segment {
 };
 
 // Walks the tile range of one CTA over the flattened (b, g, tile) list; every role keeps its own walker.
+// The per-sequence table lives in shared memory (built once in the prologue), so a walk costs no global
+// round trips.
 struct SegWalker {
-  const AttnParams& p;
-  int T, G, c;
-  int lo, hi, x, b = 0, pref = 0;
-  __device__ SegWalker(const AttnParams& p_, int T_, int G_, int c_) : p(p_), T(T_), G(G_), c(c_) {
+  const AttnShared& sh;
+  int Hkv, c;
+  int lo, hi, x, b;
+  __device__ SegWalker(const AttnShared& sh_, int Hkv_, int c_) : sh(sh_), Hkv(Hkv_), c(c_) {
+    const int T = sh.total_tiles, G = sh.g_eff;
     lo = (int)((long long)c * T / G);
     hi = (int)((long long)(c + 1) * T / G);
     x = lo;
-  }
-  __device__ int len_of(int bb) const {
-    const int qb = p.q_indptr[bb + 1] - p.q_indptr[bb];
-    return qb > 0 ? p.kv.seq_len[bb] + qb : 0;
+    int l = 0, r = sh.B;                                       // largest b with Hkv * pref[b] <= lo
+    while (r - l > 1) {
+      const int mid = (l + r) >> 1;
+      if (Hkv * sh.pref[mid] <= lo) l = mid; else r = mid;
+    }
+    b = l;
   }
   __device__ bool next(Segment& s) {
     if (x >= hi) return false;
-    const int Hkv = p.kv.n_kv_heads;
-    int nt = (len_of(b) + AT_BN - 1) / AT_BN;
-    while (x >= pref + Hkv * nt) {
-      pref += Hkv * nt;
-      ++b;
-      nt = (len_of(b) + AT_BN - 1) / AT_BN;
-    }
+    while (x >= Hkv * sh.pref[b + 1]) ++b;                     // also skips empty sequences
+    const int nt = sh.pref[b + 1] - sh.pref[b];
+    const int pref = Hkv * sh.pref[b];
     const int local = x - pref;
     s.b = b; s.nt = nt;
     s.g = local / nt; s.t_lo = local % nt;
     s.t_hi = min(nt, s.t_lo + (hi - x));
     s.flat0 = pref + s.g * nt;
-    s.r0 = p.q_indptr[b];
-    s.q_b = p.q_indptr[b + 1] - s.r0;
-    s.ctx = p.kv.seq_len[b];
+    s.r0 = sh.r0[b];
+    s.q_b = sh.r0[b + 1] - s.r0;
+    s.ctx = sh.ctx[b];
     s.k0 = s.t_lo * AT_BN;
     s.k1 = min(s.ctx + s.q_b, s.t_hi * AT_BN);
     s.n_tiles = s.t_hi - s.t_lo;
@@ -134,7 +137,7 @@ __device__ __forceinline__ void attn_loader(const AttnParams& p, AttnShared& sh,
   const KvView& kv = p.kv;
   uint64_t* full = which ? sh.v_full : sh.k_full;
   uint64_t* empty = which ? sh.v_empty : sh.k_empty;
-  SegWalker walk(p, sh.total_tiles, sh.g_eff, blockIdx.x);
+  SegWalker walk(sh, p.kv.n_kv_heads, blockIdx.x);
   Segment sg;
   uint32_t gt = 0;
   constexpr int PP = AT_BN / 16;                              // pages per tile
@@ -187,7 +190,7 @@ __device__ __forceinline__ void attn_mma(const AttnParams& p, AttnShared& sh, ui
   const uint64_t dp0 = umma_desc(smem_u32(p0_s), 16, 1024);                 // K-major
   const uint64_t dp1 = umma_desc(smem_u32(p1_s), 16, 1024);
   const uint64_t dv0 = umma_desc(smem_u32(v_s), C::KV_HALF, 1024);          // MN-major
-  SegWalker walk(p, sh.total_tiles, sh.g_eff, blockIdx.x);
+  SegWalker walk(sh, p.kv.n_kv_heads, blockIdx.x);
   Segment sg;
   uint32_t gt = 0, n_seg = 0;
   auto issue_qk = [&](uint32_t g2) {
@@ -261,7 +264,7 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared& sh
   uint8_t* p_s = grp ? p1_s : p0_s;
   float* xch = reinterpret_cast<float*>(q_s);                  // [NO][128] group-merge buffer (Q + P1 regions)
   const int T = sh.total_tiles, G = sh.g_eff;
-  SegWalker walk(p, T, G, blockIdx.x);
+  SegWalker walk(sh, p.kv.n_kv_heads, blockIdx.x);
   Segment sg;
   uint32_t gt0 = 0;                                            // global tile counter at the start of the segment
   while (walk.next(sg)) {
@@ -382,6 +385,16 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared& sh
     }
     gt0 += sg.n_tiles;
 
+    // Shared pair: arrive NOW (one packed counter: arrived in the low half, published in the high half); the
+    // round trip overlaps the group merge below.  Arriving only decides who merges, it publishes nothing.
+    int c_first = 0, n_seg = 1;
+    unsigned int arrive_old = 0;
+    if (sg.partial && grp == 0) {
+      c_first = cta_of_tile(sg.flat0, T, G);
+      n_seg = cta_of_tile(sg.flat0 + sg.nt - 1, T, G) - c_first + 1;
+      if (stid == 0) arrive_old = atomicAdd(&p.counters[sg.b * Hkv + sg.g], 1u);
+    }
+
     // ---- group 1 hands (m, l, O) to group 0 through smem (Q and P1 are idle: every MMA has retired) ----
     if (grp == 1) {
 #pragma unroll
@@ -436,12 +449,10 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared& sh
     //      partial in fragment order (thread-major float4: coalesced for writer and reader alike).
     //      In steady state the last arriver is the CTA that holds the pair's head at the end of its range,
     //      and the others published long ago. ----
-    const int c_first = cta_of_tile(sg.flat0, T, G), c_last = cta_of_tile(sg.flat0 + sg.nt - 1, T, G);
-    const int n_seg = c_last - c_first + 1;
-    unsigned int* cnt = p.counters + 2 * (sg.b * Hkv + sg.g);  // [0] arrived, [1] published
-    if (stid == 0) sh.last = (atomicAdd(&cnt[0], 1u) == (unsigned int)n_seg - 1);
+    unsigned int* cnt = p.counters + sg.b * Hkv + sg.g;
+    if (stid == 0) sh.last = (arrive_old & 0xffffu) == (unsigned int)n_seg - 1 ? 1 + (int)(arrive_old >> 16) : 0;
     named_bar_sync(3, 128);
-    const bool last = sh.last != 0;
+    const int last = sh.last;                                  // 0: not last; else 1 + partials already published
     if (!last) {
       float4* dst = p.ws_o + (size_t)sg.slot * (NO / 4) * 128 + stid;
 #pragma unroll
@@ -449,16 +460,18 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared& sh
       p.ws_ml[(size_t)sg.slot * 128 + stid] = make_float4(m_run[0], l_run[0], m_run[1], l_run[1]);
       __threadfence();
       named_bar_sync(3, 128);                                  // also: sh.last may be rewritten
-      if (stid == 0) atomicAdd(&cnt[1], 1u);
+      if (stid == 0) atomicAdd(cnt, 0x10000u);
       continue;
     }
-    if (stid == 0) {                                           // the others have arrived, so they are running: bounded wait
-      for (uint32_t spins = 0; atomicAdd(&cnt[1], 0u) < (unsigned int)n_seg - 1; ++spins)
-        if (spins > (1u << 24)) __trap();
-      cnt[0] = 0; cnt[1] = 0;                                  // self-resetting for the next launch
-      __threadfence();
+    if (last - 1 < n_seg - 1) {                                // rare: somebody arrived but has not published yet
+      if (stid == 0) {                                         // it has arrived, so it is running: bounded wait
+        for (uint32_t spins = 0; (atomicAdd(cnt, 0u) >> 16) < (unsigned int)n_seg - 1; ++spins)
+          if (spins > (1u << 24)) __trap();
+      }
+      named_bar_sync(3, 128);
     }
-    named_bar_sync(3, 128);
+    if (stid == 0) *cnt = 0;                                   // self-resetting for the next launch
+    __threadfence();
     // the head partial of every CTA is slot 2c; only the first CTA can hold the pair as its tail (slot 2c+1)
     const int first_slot = 2 * c_first + ((int)((long long)c_first * T / G) < sg.flat0 ? 1 : 0);
     const int s_own = (int)blockIdx.x - c_first;
@@ -507,20 +520,15 @@ __global__ void __launch_bounds__(AT_THREADS, 1) wf_verify_attn_kernel(const Att
   uint8_t* k_s = p1_s + C::P_BYTES;
   uint8_t* v_s = k_s + C::STAGES_K * C::K_BYTES;
 
-  // total tiles and the longest pair, from the device-resident lengths (identical in every CTA)
-  int part = 0, longest = 0;
+  // per-sequence table (tiles per kv head, q_indptr, context) from the device-resident lengths, identical in
+  // every CTA; then total tiles and the longest pair
   for (int b = tid; b < p.B; b += AT_THREADS) {
-    const int qb = p.q_indptr[b + 1] - p.q_indptr[b];
-    const int nt = qb > 0 ? (p.kv.seq_len[b] + qb + AT_BN - 1) / AT_BN : 0;
-    part += nt;
-    longest = max(longest, nt);
+    const int r0 = p.q_indptr[b], r1 = p.q_indptr[b + 1], ctx = p.kv.seq_len[b];
+    sh.r0[b] = r0;
+    sh.ctx[b] = ctx;
+    sh.pref[b + 1] = r1 > r0 ? (ctx + (r1 - r0) + AT_BN - 1) / AT_BN : 0;
+    if (b == p.B - 1) sh.r0[p.B] = r1;
   }
-#pragma unroll
-  for (int d = 16; d > 0; d >>= 1) {
-    part += __shfl_xor_sync(0xffffffffu, part, d);
-    longest = max(longest, __shfl_xor_sync(0xffffffffu, longest, d));
-  }
-  if (lane == 0) { sh.red[0][warp] = part; sh.red[1][warp] = longest; }
   if (tid == 0) {
     for (int i = 0; i < AT_MAX_STAGES; ++i) {
       mbar_init(smem_u32(&sh.k_full[i]), 1); mbar_init(smem_u32(&sh.k_empty[i]), 1);
@@ -541,14 +549,31 @@ __global__ void __launch_bounds__(AT_THREADS, 1) wf_verify_attn_kernel(const Att
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = sh.tmem;
-  if (tid == 0) {
-    int total = 0, lg = 0;
-    for (int w = 0; w < AT_THREADS / 32; ++w) { total += sh.red[0][w]; lg = max(lg, sh.red[1][w]); }
-    total *= p.kv.n_kv_heads;
-    // ranges of at least ceil(longest / 30) tiles keep the partials of one pair <= AT_MAX_SEG
-    const int min_range = max(1, (lg + AT_MAX_SEG - 3) / (AT_MAX_SEG - 2));
-    sh.total_tiles = total;
-    sh.g_eff = max(1, min((int)gridDim.x, total / min_range));
+  if (warp == 0) {                                             // in-place scan of the tile counts, 32 sequences per step
+    int run = 0, lg = 0;
+    for (int base = 0; base < p.B; base += 32) {
+      const int n = base + lane < p.B ? sh.pref[base + lane + 1] : 0;
+      lg = max(lg, n);
+      int v = n;
+#pragma unroll
+      for (int d = 1; d < 32; d <<= 1) {
+        const int y = __shfl_up_sync(0xffffffffu, v, d);
+        if (lane >= d) v += y;
+      }
+      if (base + lane < p.B) sh.pref[base + lane + 1] = run + v;
+      run += __shfl_sync(0xffffffffu, v, 31);
+    }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) lg = max(lg, __shfl_xor_sync(0xffffffffu, lg, d));
+    if (lane == 0) {
+      sh.pref[0] = 0;
+      const int total = run * p.kv.n_kv_heads;
+      // ranges of at least ceil(longest / 30) tiles keep the partials of one pair <= AT_MAX_SEG
+      const int min_range = max(1, (lg + AT_MAX_SEG - 3) / (AT_MAX_SEG - 2));
+      sh.total_tiles = total;
+      sh.g_eff = max(1, min((int)gridDim.x, total / min_range));
+      sh.B = p.B;
+    }
   }
   __syncthreads();
 
@@ -603,7 +628,7 @@ extern "C" int wf_verify_attn(wf_ctx* ctx, const wf_paged_kv* kv, int layer, con
   if (!ctx) return WF_ERR_INVALID_ARG;
   WF_REQUIRE(ctx, kv && q && q_indptr && out && workspace, WF_ERR_INVALID_ARG, "wf_verify_attn: null argument");
   WF_REQUIRE(ctx, layer >= 0 && layer < kv->s.n_layers, WF_ERR_INVALID_ARG, "wf_verify_attn: bad layer");
-  WF_REQUIRE(ctx, B >= 0 && B <= kv->s.max_seqs && B <= AT_MAX_B && 2 * B * kv->s.n_kv_heads <= ctx->n_counters,
+  WF_REQUIRE(ctx, B >= 0 && B <= kv->s.max_seqs && B <= AT_MAX_B && B * kv->s.n_kv_heads <= ctx->n_counters,
              WF_ERR_INVALID_ARG, "wf_verify_attn: bad B (max %d)", AT_MAX_B);
   WF_REQUIRE(ctx, n_q_heads > 0 && n_q_heads % kv->s.n_kv_heads == 0, WF_ERR_INVALID_ARG,
              "wf_verify_attn: n_q_heads must be a multiple of n_kv_heads");
