@@ -13,7 +13,6 @@
 //               next tile are prefetched; a K tile is released when its QK^T retires.
 //   warp 9    : MMA issuer (one thread).  S = Q K^T (UMMA 64 x 128 x 16, both K-major) into TMEM,
 //               double buffered; O_t = P V (64 x D x 16, V MN-major) into TMEM, double buffered.
-//               QK^T of tile t+2 is issued ahead of PV of tile t.
 //   warps 0-7 : softmax, two groups of 4 warps that ping-pong over the tiles.  UMMA M = 64 puts rows
 //               16w..16w+15 on TMEM lanes 32w..32w+15, so warp w owns 16 rows; tcgen05.ld.16x256b hands
 //               them out like an mma C fragment (a quad per row).  Online softmax in the log2 domain
@@ -217,9 +216,6 @@ __device__ __forceinline__ void attn_mma(const AttnParams& p, AttnShared& sh, ui
     issue_qk(gt);
     if (sg.n_tiles > 1) issue_qk(gt + 1);
     for (int t = 0; t < sg.n_tiles; ++t, ++gt) {
-      // QK^T of tile t+2 goes ahead of PV of tile t: its S buffer was released as soon as the softmax group
-      // had S(t) in registers, so S(t+2) is ready when the group comes back and the group never idles on it.
-      if (t + 2 < sg.n_tiles) issue_qk(gt + 2);
       const int st = gt % C::STAGES_V, g = gt & 1;
       mbar_wait(smem_u32(&sh.v_full[st]), (gt / C::STAGES_V) & 1);
       mbar_wait(smem_u32(&sh.p_full[g]), (gt >> 1) & 1);
@@ -237,6 +233,8 @@ __device__ __forceinline__ void attn_mma(const AttnParams& p, AttnShared& sh, ui
         umma_commit(smem_u32(&sh.v_empty[st]));
       }
       __syncwarp();
+      // QK^T(t+2) after PV(t) (measured: issuing it ahead of PV(t) gains nothing, the loop is memory-paced)
+      if (t + 2 < sg.n_tiles) issue_qk(gt + 2);
     }
   }
 }
@@ -350,6 +348,9 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared& sh
       if (tk0 + AT_BN > sg.k1) {
         // Last tile of the sequence: keys >= k1 hold stale or never-written V bits.  Zero them so that
         // 0 * garbage cannot produce NaN in the PV product (P is exactly 0 there).
+        // The parity wait below is only unambiguous once the previous occupant of this V stage is consumed:
+        // wait for this group's previous PV first (independent of the order the MMA warp issues in).
+        if (pending) mbar_wait(smem_u32(&sh.pv_done[grp]), (g_prev >> 1) & 1);
         mbar_wait(smem_u32(&sh.v_full[g2 % C::STAGES_V]), (g2 / C::STAGES_V) & 1);
         const int key = (sg.k1 - tk0) + stid;
         if (key < AT_BN) {
