@@ -551,10 +551,11 @@ __global__ void __launch_bounds__(AT_THREADS, 1) wf_verify_attn_kernel(const Att
   tc_fence_after();
   const uint32_t tmem_base = sh.tmem;
   if (warp == 0) {                                             // in-place scan of the tile counts, 32 sequences per step
-    int run = 0, lg = 0;
+    int run = 0, lg = 0, live = 0;
     for (int base = 0; base < p.B; base += 32) {
       const int n = base + lane < p.B ? sh.pref[base + lane + 1] : 0;
       lg = max(lg, n);
+      live += n > 0;
       int v = n;
 #pragma unroll
       for (int d = 1; d < 32; d <<= 1) {
@@ -565,14 +566,28 @@ __global__ void __launch_bounds__(AT_THREADS, 1) wf_verify_attn_kernel(const Att
       run += __shfl_sync(0xffffffffu, v, 31);
     }
 #pragma unroll
-    for (int d = 16; d > 0; d >>= 1) lg = max(lg, __shfl_xor_sync(0xffffffffu, lg, d));
+    for (int d = 16; d > 0; d >>= 1) {
+      lg = max(lg, __shfl_xor_sync(0xffffffffu, lg, d));
+      live += __shfl_xor_sync(0xffffffffu, live, d);
+    }
     if (lane == 0) {
       sh.pref[0] = 0;
       const int total = run * p.kv.n_kv_heads;
       // ranges of at least ceil(longest / 30) tiles keep the partials of one pair <= AT_MAX_SEG
       const int min_range = max(1, (lg + AT_MAX_SEG - 3) / (AT_MAX_SEG - 2));
       sh.total_tiles = total;
-      sh.g_eff = max(1, min((int)gridDim.x, total / min_range));
+      // Small launches (under 24 tiles per SM) are latency-bound: every segment costs about 10k cycles of fixed
+      // latency, a pair cut into n ranges streams (tiles/n) * 1.3k cycles and its last arriver folds n partials at
+      // about 1k cycles each: least at n = sqrt(1.3 * tiles per pair).  G = n * pairs keeps the ranges aligned with
+      // the pairs (one segment per CTA) when the contexts are equal.  Large launches use one CTA per SM.
+      const int pairs = live * p.kv.n_kv_heads;
+      int G = (int)gridDim.x;
+      if (pairs > 0 && total < 24 * G) {
+        int n = (int)(sqrtf(1.3f * (float)total / (float)pairs) + 0.5f);
+        n = max(1, min(n, G / pairs));
+        G = min(G, n * pairs);
+      }
+      sh.g_eff = max(1, min(G, total / min_range));
       sh.B = p.B;
     }
   }
