@@ -27,11 +27,10 @@ namespace {
 
 constexpr int PF_BLOCK_M = 128;         // UMMA M
 constexpr int PF_BLOCK_K = 64;          // one 128-byte swizzle row of bf16
+constexpr int PF_KSUB = 2;              // 64-wide k-blocks per pipeline stage: halves the per-stage hand-offs of the one-thread loops
 constexpr int PF_MAX_MT = 2;            // m-tiles per pass (TMEM columns = PF_MAX_MT * D)
 constexpr int PF_THREADS = 192;         // warp 0: TMA, warp 1: MMA, warps 2-5: X gather + epilogue
 constexpr int PF_SMEM_BUDGET = 200 * 1024;
-constexpr int PF_GATHER_LAG = 2;        // cp.async groups kept in flight per gather thread
-
 struct RowEntry {
   const __nv_bfloat16* src;             // hidden row
   int32_t pos;                          // absolute position (RoPE)
@@ -148,8 +147,44 @@ __global__ void __launch_bounds__(1024) wf_prefill_plan_kernel(const PlanParams 
 // ---- the projection kernel ------------------------------------------------------------------
 constexpr int PF_MAX_STAGES = 12;
 
+// Per call: the rows of the plan's row table -> the shared-memory image of the A operand, k-block by k-block:
+// xpack[kb][m_pad][128 B], row m of k-block kb = X[m][64 kb .. 64 kb + 63], 16-byte chunks XOR-swizzled with (m & 7)
+// (K-major, 128-byte swizzle).  One block per row; every projection CTA then fetches a stage's A operand with
+// one bulk copy instead of gathering it with 128 threads.
+__global__ void __launch_bounds__(256) wf_pack_x_kernel(const RowEntry* __restrict__ rows, const int32_t* __restrict__ m_total,
+                                                        uint8_t* __restrict__ xpack, int hidden) {
+  const int M = *m_total;
+  const int r = blockIdx.x;                              // one row per block: every load of the block is independent
+  if (r >= M) return;
+  const int m_pad = (M + 7) & ~7;
+  const uint4* src = reinterpret_cast<const uint4*>(rows[r].src);
+  uint8_t* dst = xpack + (size_t)r * 128;
+  const size_t kb_stride = (size_t)m_pad * 128;
+  for (int q = threadIdx.x; q < hidden / 8; q += 256) {  // 16-byte chunk q of the row -> k-block q/8, chunk q%8
+    const uint4 v = __ldg(src + q);
+    *reinterpret_cast<uint4*>(dst + (size_t)(q >> 3) * kb_stride + (((q & 7) ^ (r & 7)) << 4)) = v;
+  }
+}
+
+// One-time repack of a drafter's weights (wf_drafter_create) into the exact shared-memory image of a W stage:
+// tile (layer, K|V, head) x k-block of 64 rows -> D/64 column halves x [64 k][128 B], 16-byte chunks XOR-swizzled
+// with (k & 7) (the 128-byte swizzle the MN-major UMMA descriptor expects).  A stage is then ONE contiguous
+// cp.async.bulk of 64*D*2 bytes instead of 64*D/64 strided 128-byte TMA rows out of a [hidden][Hkv*D] matrix.
+__global__ void wf_pack_w_kernel(const __nv_bfloat16* __restrict__ w, uint8_t* __restrict__ dst, int hidden, int n_cols, int D) {
+  // grid (hidden/64, n_cols/D); dst points at this (layer, K|V) block: [head][kb][D/64][64][128 B]
+  const int kb = blockIdx.x, head = blockIdx.y, n_kb = hidden / 64;
+  uint8_t* out = dst + ((size_t)head * n_kb + kb) * (64 * D * 2);
+  for (int i = threadIdx.x; i < 64 * D / 8; i += blockDim.x) {       // one 16-byte chunk per step
+    const int k = i / (D / 8), c16 = i % (D / 8);                       // row of the k-block, chunk of the D columns
+    const int j = c16 >> 3, cc = c16 & 7;                               // column half, chunk inside the 128-byte row
+    const uint4 v = *reinterpret_cast<const uint4*>(w + (size_t)(kb * 64 + k) * n_cols + head * D + c16 * 8);
+    *reinterpret_cast<uint4*>(out + j * 8192 + k * 128 + ((cc ^ (k & 7)) << 4)) = v;
+  }
+}
+
 struct GemmParams {
-  const CUtensorMap* tmaps;             // [n_layers * 2] (W_K[l], W_V[l]): dims {Hkv*D, hidden}, box {64, 64}, SW128
+  const uint8_t* wpack;                 // [n_layers][2][Hkv][hidden/64][64 * D * 2 B] pre-swizzled W stages
+  const uint8_t* xpack;                 // [hidden/64][m_pad][128 B] pre-swizzled X k-blocks of this call (wf_pack_x_kernel)
   const RowEntry* rows;
   const int32_t* m_total;
   const float2* rope;                   // [max_pos][D/2] (cos, sin)
@@ -160,7 +195,7 @@ struct GemmParams {
 
 template <int D>
 __global__ void __launch_bounds__(PF_THREADS, 1) wf_prefill_gemm_kernel(const GemmParams p) {
-  constexpr int B_BYTES = PF_BLOCK_K * D * 2;          // W stage: D/64 boxes of [64 k][128 B]
+  constexpr int B_BYTES = PF_KSUB * PF_BLOCK_K * D * 2;  // W stage: PF_KSUB k-blocks of D/64 x [64 k][128 B], contiguous in wpack
   constexpr int A_TILE = PF_BLOCK_M * PF_BLOCK_K * 2;  // 16 KB: 128 rows x 128 B
   constexpr uint32_t TMEM_COLS = PF_MAX_MT * D;        // 256 or 128: a power of two >= 32
   extern __shared__ __align__(1024) uint8_t smem[];
@@ -174,19 +209,20 @@ __global__ void __launch_bounds__(PF_THREADS, 1) wf_prefill_gemm_kernel(const Ge
   const int layer = tile / (2 * p.n_kv_heads);
   const int is_v = (tile / p.n_kv_heads) & 1;
   const int head = tile % p.n_kv_heads;
-  const int n_kb = p.hidden / PF_BLOCK_K;
+  const int n_kb = p.hidden / (PF_KSUB * PF_BLOCK_K);  // pipeline stages per pass
   const int n_pass = (M + PF_MAX_MT * PF_BLOCK_M - 1) / (PF_MAX_MT * PF_BLOCK_M);
 
   // A stage holds only the rows that exist (8-row swizzle atoms); UMMA reads 128 rows from its start,
   // the surplus lands in later stages / the W ring and feeds accumulator rows nobody reads.
   const int m_first = min(M, PF_MAX_MT * PF_BLOCK_M);
-  const int a_bytes = ((m_first + 7) / 8) * 1024;
+  const int a_sub = ((m_first + 7) / 8) * 1024;          // one 64-wide k-block of the A operand
+  const int a_bytes = PF_KSUB * a_sub;
   const int n_stages = min(PF_MAX_STAGES, PF_SMEM_BUDGET / (a_bytes + B_BYTES));
   uint8_t* a_base = smem;
   uint8_t* b_base = smem + (size_t)n_stages * a_bytes;      // 1024-aligned: a_bytes is a multiple of 1024
 
   if (tid == 0) {
-    for (int i = 0; i < n_stages; ++i) { mbar_init(smem_u32(&s_full[i]), 1 + 128); mbar_init(smem_u32(&s_empty[i]), 1); }
+    for (int i = 0; i < n_stages; ++i) { mbar_init(smem_u32(&s_full[i]), 1); mbar_init(smem_u32(&s_empty[i]), 1); }
     mbar_init(smem_u32(&s_acc_full), 1);
     mbar_init(smem_u32(&s_acc_empty), 128);
     fence_barrier_init();
@@ -198,87 +234,78 @@ __global__ void __launch_bounds__(PF_THREADS, 1) wf_prefill_gemm_kernel(const Ge
   const uint32_t tmem_base = s_tmem;
 
   if (warp == 0) {
-    // ===== TMA producer: stream this tile's W slab, one [64 k][D] block per stage =====
+    // ===== bulk-copy producer: per stage ONE contiguous copy of the pre-swizzled W k-block and ONE of the packed X
+    //       k-block (wf_pack_x_kernel): no thread touches operand bytes.  Stage index, phase and addresses advance
+    //       incrementally: a runtime division per k-block in a one-thread loop costs more than the MMAs it feeds. =====
     if (lane == 0) {
-      const CUtensorMap* tm = p.tmaps + layer * 2 + is_v;
-      int it = 0;
-      for (int pass = 0; pass < n_pass; ++pass)
-        for (int kb = 0; kb < n_kb; ++kb, ++it) {
-          const int s = it % n_stages;
-          mbar_wait(smem_u32(&s_empty[s]), ((it / n_stages) & 1) ^ 1);
-          mbar_arrive_expect_tx(smem_u32(&s_full[s]), B_BYTES);
-#pragma unroll
-          for (int j = 0; j < D / 64; ++j)
-            tma_load_2d(smem_u32(b_base + (size_t)s * B_BYTES + j * 8192), tm, head * D + j * 64, kb * PF_BLOCK_K,
-                        smem_u32(&s_full[s]));
-        }
-    }
-  } else if (warp == 1) {
-    // ===== MMA issuer: one thread drives the tensor core for the CTA =====
-    if (lane == 0) {
-      const uint32_t idesc = umma_idesc(PF_BLOCK_M, D);
-      int it = 0;
+      const uint8_t* w_src = p.wpack + (size_t)tile * n_kb * B_BYTES;    // tile = (layer, K|V, head), packed in that order
+      const size_t x_kb_stride = (size_t)((M + 7) & ~7) * 128;
+      const uint32_t full0 = smem_u32(&s_full[0]), empty0 = smem_u32(&s_empty[0]);
+      const uint32_t a0 = smem_u32(a_base), b0 = smem_u32(b_base);
+      int s = 0;
+      uint32_t ph = 1;                                   // parity to wait for on s_empty: the ring starts empty
       for (int pass = 0; pass < n_pass; ++pass) {
         const int rows_here = min(M - pass * PF_MAX_MT * PF_BLOCK_M, PF_MAX_MT * PF_BLOCK_M);
-        const int n_mt = (rows_here + PF_BLOCK_M - 1) / PF_BLOCK_M;
-        if (pass > 0) { mbar_wait(smem_u32(&s_acc_empty), (pass - 1) & 1); tc_fence_after(); }
-        for (int kb = 0; kb < n_kb; ++kb, ++it) {
-          const int s = it % n_stages;
-          mbar_wait(smem_u32(&s_full[s]), (it / n_stages) & 1);
-          tc_fence_after();
-          const uint32_t a_s = smem_u32(a_base + (size_t)s * a_bytes);
-          const uint32_t b_s = smem_u32(b_base + (size_t)s * B_BYTES);
-          for (int mt = 0; mt < n_mt; ++mt)
+        const uint32_t x_bytes = (uint32_t)((rows_here + 7) / 8) * 1024;
+        const uint8_t* x_src = p.xpack + (size_t)pass * PF_MAX_MT * PF_BLOCK_M * 128;
+        const uint8_t* w_kb = w_src;
+        for (int kb = 0; kb < n_kb; ++kb) {
+          mbar_wait(empty0 + 8 * s, ph);
+          const uint32_t bar = full0 + 8 * s;
+          mbar_arrive_expect_tx(bar, B_BYTES + PF_KSUB * x_bytes);
+          bulk_load(b0 + s * B_BYTES, w_kb, B_BYTES, bar);
 #pragma unroll
-            for (int k16 = 0; k16 < PF_BLOCK_K / 16; ++k16) {
-              const uint64_t da = umma_desc(a_s + mt * A_TILE + k16 * 32, 16, 1024);        // K-major
-              const uint64_t db = umma_desc(b_s + k16 * 2048, 8192, 1024);                 // MN-major
-              umma_bf16(tmem_base + mt * D, da, db, idesc, (kb | k16) != 0);
-            }
-          umma_commit(smem_u32(&s_empty[s]));            // frees the stage when these MMAs retire
+          for (int u = 0; u < PF_KSUB; ++u) bulk_load(a0 + s * a_bytes + u * a_sub, x_src + u * x_kb_stride, x_bytes, bar);
+          w_kb += B_BYTES;
+          x_src += PF_KSUB * x_kb_stride;
+          if (++s == n_stages) { s = 0; ph ^= 1; }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ===== MMA issuer: one thread drives the tensor core for the CTA.  Descriptors are built once and advanced by
+    //       constant offsets =====
+    if (lane == 0) {
+      const uint32_t idesc = umma_idesc(PF_BLOCK_M, D);
+      const uint64_t da0 = umma_desc(smem_u32(a_base), 16, 1024);          // K-major
+      const uint64_t db0 = umma_desc(smem_u32(b_base), 8192, 1024);        // MN-major
+      const uint32_t full0 = smem_u32(&s_full[0]), empty0 = smem_u32(&s_empty[0]);
+      const uint64_t da_step = (uint64_t)(a_bytes >> 4), db_step = (uint64_t)(B_BYTES >> 4);
+      int s = 0;
+      uint32_t ph = 0;
+      uint64_t da = da0, db = db0;
+      for (int pass = 0; pass < n_pass; ++pass) {
+        const int rows_here = min(M - pass * PF_MAX_MT * PF_BLOCK_M, PF_MAX_MT * PF_BLOCK_M);
+        const bool two = rows_here > PF_BLOCK_M;
+        if (pass > 0) { mbar_wait(smem_u32(&s_acc_empty), (pass - 1) & 1); tc_fence_after(); }
+        for (int kb = 0; kb < n_kb; ++kb) {
+          mbar_wait(full0 + 8 * s, ph);
+          tc_fence_after();
+          // k16 step j of the stage: A k-block j/4 (a_sub apart), 32 bytes per step; W k-block j/4 (64*D*2 apart), 2 KB per step
+#pragma unroll
+          for (int k16 = 0; k16 < PF_KSUB * PF_BLOCK_K / 16; ++k16)
+            umma_bf16(tmem_base, da + (uint64_t)(((k16 >> 2) * a_sub + (k16 & 3) * 32) >> 4),
+                      db + (uint64_t)(((k16 >> 2) * (PF_BLOCK_K * D * 2) + (k16 & 3) * 2048) >> 4), idesc, (kb | k16) != 0);
+          if (two) {
+#pragma unroll
+            for (int k16 = 0; k16 < PF_KSUB * PF_BLOCK_K / 16; ++k16)
+              umma_bf16(tmem_base + D, da + (uint64_t)(((k16 >> 2) * a_sub + A_TILE + (k16 & 3) * 32) >> 4),
+                        db + (uint64_t)(((k16 >> 2) * (PF_BLOCK_K * D * 2) + (k16 & 3) * 2048) >> 4), idesc, (kb | k16) != 0);
+          }
+          umma_commit(empty0 + 8 * s);                   // frees the stage when these MMAs retire
+          da += da_step; db += db_step;
+          if (++s == n_stages) { s = 0; ph ^= 1; da = da0; db = db0; }
         }
         umma_commit(smem_u32(&s_acc_full));
       }
     }
   } else {
-    // ===== warps 2-5: gather X rows into the swizzled A stages, then run the epilogue =====
-    const int gt = tid - 64;                             // 0..127: row inside an m-tile
+    // ===== warps 2-5: epilogue =====
     const int quarter = warp & 3;                        // TMEM lane quarter this warp may read
-    int it = 0;
     for (int pass = 0; pass < n_pass; ++pass) {
       const int m_base = pass * PF_MAX_MT * PF_BLOCK_M;
       const int rows_here = min(M - m_base, PF_MAX_MT * PF_BLOCK_M);
       const int n_mt = (rows_here + PF_BLOCK_M - 1) / PF_BLOCK_M;
-      const __nv_bfloat16* src[PF_MAX_MT];
-#pragma unroll
-      for (int mt = 0; mt < PF_MAX_MT; ++mt) {
-        const int m = m_base + mt * PF_BLOCK_M + gt;
-        src[mt] = m < M ? p.rows[m].src : nullptr;
-      }
-      const int it0 = it;
-      for (int kb = 0; kb < n_kb; ++kb, ++it) {
-        const int s = it % n_stages;
-        mbar_wait(smem_u32(&s_empty[s]), ((it / n_stages) & 1) ^ 1);
-        const uint32_t a_s = smem_u32(a_base + (size_t)s * a_bytes);
-#pragma unroll
-        for (int mt = 0; mt < PF_MAX_MT; ++mt)
-          if (src[mt]) {
-            const uint32_t row_s = a_s + mt * A_TILE + gt * 128;
-#pragma unroll
-            for (int c = 0; c < 8; ++c)
-              cp_async16(row_s + ((c ^ (gt & 7)) << 4), src[mt] + kb * PF_BLOCK_K + c * 8);
-          }
-        cp_async_commit();
-        if (it - it0 >= PF_GATHER_LAG) {                 // publish the stage filled LAG iterations ago
-          cp_async_wait<PF_GATHER_LAG>();
-          fence_proxy_async();                           // generic-proxy writes -> visible to the tensor core
-          mbar_arrive(smem_u32(&s_full[(it - PF_GATHER_LAG) % n_stages]));
-        }
-      }
-      cp_async_wait<0>();
-      fence_proxy_async();
-      for (int j = max(it0, it - PF_GATHER_LAG); j < it; ++j) mbar_arrive(smem_u32(&s_full[j % n_stages]));
-
       // ---- epilogue: TMEM -> registers -> (RoPE) -> bf16 -> paged pool ----
       mbar_wait(smem_u32(&s_acc_full), pass & 1);
       tc_fence_after();
@@ -356,7 +383,8 @@ struct wf_drafter {
   wf_paged_kv* kv;
   const __nv_bfloat16* backlog;
   int32_t* backlog_len;
-  CUtensorMap* d_tmaps;        // [n_layers * 2]
+  uint8_t* d_wpack;            // library-owned pre-swizzled copy of the weights (see wf_pack_w_kernel)
+  uint8_t* d_xpack;            // library-owned [hidden/64][row_cap][128 B] scratch (see wf_pack_x_kernel)
   float2* d_rope;              // [max_pos][D/2]
   RowEntry* d_rows;
   int row_cap;
@@ -375,7 +403,7 @@ int launch_gemm(wf_drafter* d, cudaStream_t st) {
     configured = true;
   }
   GemmParams g;
-  g.tmaps = d->d_tmaps; g.rows = d->d_rows; g.m_total = d->d_m_total; g.rope = d->d_rope;
+  g.wpack = d->d_wpack; g.xpack = d->d_xpack; g.rows = d->d_rows; g.m_total = d->d_m_total; g.rope = d->d_rope;
   g.k_pool = d->kv->k_pool; g.v_pool = d->kv->v_pool;
   g.hidden = d->s.hidden; g.n_kv_heads = d->s.n_kv_heads; g.num_pages = d->kv->s.num_pages;
   const int grid = d->s.n_layers * 2 * d->s.n_kv_heads;
@@ -384,7 +412,7 @@ int launch_gemm(wf_drafter* d, cudaStream_t st) {
 }
 
 // plan + projection: the one device path behind eager prefill, flush and forced flush
-int run_prefill(wf_drafter* d, PlanParams& pp, cudaStream_t st) {
+int run_prefill(wf_drafter* d, PlanParams& pp, int rows_upper, cudaStream_t st) {
   wf_ctx* ctx = d->ctx;
   pp.hidden = d->s.hidden; pp.cap = d->s.backlog_cap; pp.max_pos = d->s.max_pos; pp.row_cap = d->row_cap;
   pp.backlog = d->backlog; pp.backlog_len = d->backlog_len;
@@ -394,6 +422,10 @@ int run_prefill(wf_drafter* d, PlanParams& pp, cudaStream_t st) {
   pp.status = ctx->d_status;
   wf_prefill_plan_kernel<<<1, 1024, 0, st>>>(pp);
   int rc = wf_check_launch(ctx, "wf_prefill_plan_kernel");
+  if (rc != WF_OK) return rc;
+  rows_upper = rows_upper < d->row_cap ? rows_upper : d->row_cap;
+  wf_pack_x_kernel<<<rows_upper > 0 ? rows_upper : 1, 256, 0, st>>>(d->d_rows, d->d_m_total, d->d_xpack, d->s.hidden);
+  rc = wf_check_launch(ctx, "wf_pack_x_kernel");
   if (rc != WF_OK) return rc;
   return d->s.head_dim == 128 ? launch_gemm<128>(d, st) : launch_gemm<64>(d, st);
 }
@@ -409,18 +441,15 @@ extern "C" int wf_drafter_create(wf_ctx* ctx, const wf_drafter_shape* s, const v
   WF_REQUIRE(ctx, s->n_layers == kv->s.n_layers && s->n_kv_heads == kv->s.n_kv_heads && s->head_dim == kv->s.head_dim,
              WF_ERR_INVALID_ARG, "wf_drafter_create: drafter shape does not match its KV cache");
   WF_REQUIRE(ctx, s->head_dim == 64 || s->head_dim == 128, WF_ERR_UNSUPPORTED_SHAPE, "wf_drafter_create: head_dim must be 64 or 128");
-  WF_REQUIRE(ctx, s->hidden > 0 && s->hidden % PF_BLOCK_K == 0, WF_ERR_UNSUPPORTED_SHAPE,
-             "wf_drafter_create: hidden must be a positive multiple of %d", PF_BLOCK_K);
+  WF_REQUIRE(ctx, s->hidden > 0 && s->hidden % (PF_KSUB * PF_BLOCK_K) == 0, WF_ERR_UNSUPPORTED_SHAPE,
+             "wf_drafter_create: hidden must be a positive multiple of %d", PF_KSUB * PF_BLOCK_K);
   WF_REQUIRE(ctx, s->max_pos > 0 && s->rope_theta > 0.f && s->backlog_cap >= 0, WF_ERR_INVALID_ARG, "wf_drafter_create: bad max_pos/theta/cap");
   WF_REQUIRE(ctx, s->backlog_cap == 0 || (backlog && backlog_len), WF_ERR_INVALID_ARG, "wf_drafter_create: backlog buffers missing");
   const int L = s->n_layers, D = s->head_dim, N = s->n_kv_heads * D;
-  std::vector<CUtensorMap> maps(L * 2);
   for (int l = 0; l < L; ++l)
     for (int v = 0; v < 2; ++v) {
       const void* w = v ? w_v_host_ptrs[l] : w_k_host_ptrs[l];
       WF_REQUIRE(ctx, w && (uintptr_t)w % 16 == 0, WF_ERR_INVALID_ARG, "wf_drafter_create: weight pointer null or unaligned");
-      const int rc = wf_make_tmap_2d(ctx, &maps[l * 2 + v], w, (uint64_t)s->hidden, (uint64_t)N, 64, PF_BLOCK_K);
-      if (rc != WF_OK) return rc;
     }
   // RoPE table in fp64 on the host (C17): angle = pos * theta^(-2r/D)
   const int half = D / 2;
@@ -437,14 +466,23 @@ extern "C" int wf_drafter_create(wf_ctx* ctx, const wf_drafter_shape* s, const v
   if (!d) return wf_set_error(ctx, WF_ERR_INVALID_ARG, "wf_drafter_create: host allocation failed");
   d->ctx = ctx; d->s = *s; d->kv = kv;
   d->backlog = (const __nv_bfloat16*)backlog; d->backlog_len = backlog_len;
-  d->d_tmaps = nullptr; d->d_rope = nullptr; d->d_rows = nullptr; d->d_m_total = nullptr; d->d_plan = nullptr;
+  d->d_wpack = nullptr; d->d_xpack = nullptr; d->d_rope = nullptr; d->d_rows = nullptr; d->d_m_total = nullptr; d->d_plan = nullptr;
   d->row_cap = kv->s.max_seqs * (s->backlog_cap > 64 ? s->backlog_cap : 64);
-  cudaError_t e = cudaMalloc(&d->d_tmaps, sizeof(CUtensorMap) * maps.size());
+  const size_t w_bytes = (size_t)s->hidden * N * 2;                    // one [hidden][Hkv*D] matrix
+  cudaError_t e = cudaMalloc(&d->d_wpack, w_bytes * 2 * L);
+  if (e == cudaSuccess) e = cudaMalloc(&d->d_xpack, (size_t)s->hidden * 2 * d->row_cap);
   if (e == cudaSuccess) e = cudaMalloc(&d->d_rope, sizeof(float2) * rope.size());
   if (e == cudaSuccess) e = cudaMalloc(&d->d_rows, sizeof(RowEntry) * d->row_cap);
   if (e == cudaSuccess) e = cudaMalloc(&d->d_m_total, sizeof(int32_t));
   if (e == cudaSuccess) e = cudaMalloc(&d->d_plan, sizeof(int32_t) * 2 * kv->s.max_seqs);
-  if (e == cudaSuccess) e = cudaMemcpy(d->d_tmaps, maps.data(), sizeof(CUtensorMap) * maps.size(), cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) {
+    for (int l = 0; l < L; ++l)
+      for (int v = 0; v < 2; ++v)
+        wf_pack_w_kernel<<<dim3(s->hidden / PF_BLOCK_K, s->n_kv_heads), 256>>>(
+            (const __nv_bfloat16*)(v ? w_v_host_ptrs[l] : w_k_host_ptrs[l]), d->d_wpack + (size_t)(l * 2 + v) * w_bytes, s->hidden, N, D);
+    e = cudaGetLastError();
+    if (e == cudaSuccess) e = cudaDeviceSynchronize();   // creation is synchronous: the caller may free or rewrite W afterwards
+  }
   if (e == cudaSuccess) e = cudaMemcpy(d->d_rope, rope.data(), sizeof(float2) * rope.size(), cudaMemcpyHostToDevice);
   if (e == cudaSuccess) e = cudaMemset(d->d_m_total, 0, sizeof(int32_t));
   if (e != cudaSuccess) {
@@ -457,7 +495,7 @@ extern "C" int wf_drafter_create(wf_ctx* ctx, const wf_drafter_shape* s, const v
 
 extern "C" int wf_drafter_destroy(wf_drafter* d) {
   if (!d) return WF_ERR_INVALID_ARG;
-  cudaFree(d->d_tmaps); cudaFree(d->d_rope); cudaFree(d->d_rows); cudaFree(d->d_m_total); cudaFree(d->d_plan);
+  cudaFree(d->d_wpack); cudaFree(d->d_xpack); cudaFree(d->d_rope); cudaFree(d->d_rows); cudaFree(d->d_m_total); cudaFree(d->d_plan);
   delete d;
   return WF_OK;
 }
@@ -474,7 +512,7 @@ extern "C" int wf_kv_only_prefill(wf_ctx* ctx, wf_drafter* d, const void* hidden
   pp.mode = PLAN_EAGER; pp.B = B;
   pp.hidden_rows = (const __nv_bfloat16*)hidden; pp.q_indptr = q_indptr; pp.n_rows = n_rows; pp.seq_ids = seq_ids;
   pp.mask = nullptr;
-  return run_prefill(d, pp, (cudaStream_t)stream);
+  return run_prefill(d, pp, B * max_rows, (cudaStream_t)stream);
 }
 
 extern "C" int wf_lazy_catchup_flush(wf_ctx* ctx, wf_drafter* d, const int32_t* flush_mask, int B, void* stream) {
@@ -484,7 +522,7 @@ extern "C" int wf_lazy_catchup_flush(wf_ctx* ctx, wf_drafter* d, const int32_t* 
   if (B == 0) return WF_OK;
   PlanParams pp{};
   pp.mode = PLAN_FLUSH; pp.B = B; pp.mask = flush_mask;
-  return run_prefill(d, pp, (cudaStream_t)stream);
+  return run_prefill(d, pp, B * d->s.backlog_cap, (cudaStream_t)stream);
 }
 
 namespace {
@@ -523,7 +561,7 @@ extern "C" int wf_lazy_catchup_enqueue(wf_ctx* ctx, wf_drafter* d, const void* h
   PlanParams pp{};
   pp.mode = PLAN_FORCED; pp.B = B;
   pp.q_indptr = q_indptr; pp.n_rows = n_rows; pp.seq_ids = seq_ids; pp.mask = idle_mask;
-  int rc = run_prefill(d, pp, st);
+  int rc = run_prefill(d, pp, B * d->s.backlog_cap, st);
   if (rc != WF_OK) return rc;
   // (2) append the rows, (3) advance the lengths
   wf_enqueue_kernel<<<dim3(max_rows, B), 128, 0, st>>>((const __nv_bfloat16*)hidden, q_indptr, n_rows, seq_ids, idle_mask,
