@@ -6,14 +6,18 @@
 //   plan kernel (1 CTA)  : which rows go where.  Compacts the rows of the call into a row table
 //                          (source pointer, RoPE position, physical page*16+slot), reserves pages in
 //                          the drafter's block table (C24) and advances seq_len / backlog_len.
-//   projection kernel    : out[M, D] tile per (layer, K|V, kv head) = X[M, hidden] . W[hidden, D-slice]
-//                          on tcgen05 (UMMA 128 x D x 16, bf16 in, fp32 accumulators in TMEM).
-//                          W streams through a TMA + mbarrier ring (MN-major, 128B swizzle); the
-//                          gathered X rows are staged with 16-byte cp.async into the K-major 128B
-//                          swizzle layout.  Epilogue: tcgen05.ld, RoPE (fp32, host-built fp64 table)
-//                          on K tiles, bf16 RNE, 16-byte stores straight into the paged pool.
-// A row's bits do not depend on M, on its tile position or on the call that carries it: one code
-// path, a fixed K order, no split-K.
+//   pack kernel          : the call's rows -> the shared-memory image of the X operand, k-block by k-block
+//                          (K-major, 128-byte swizzle), so that a projection CTA fetches a stage's X with one
+//                          bulk copy instead of gathering rows with its own threads.
+//   projection kernel    : one CTA per (layer, K|V, kv head): out^T[D, tokens] = W^T[D, hidden] . X^T on tcgen05
+//                          (UMMA 128 x tokens x 16, bf16 in, fp32 accumulators in TMEM; swapped operands, so an
+//                          MMA costs tokens/2 cycles).  W was repacked once at wf_drafter_create into stage
+//                          images (MN-major, 128-byte swizzle): a stage is one cp.async.bulk for W and one per X
+//                          k-block, completing on an mbarrier ring.  Epilogue: tcgen05.ld, transpose through
+//                          shared memory, RoPE (fp32, host-built fp64 table) on K tiles, bf16 RNE, 16-byte
+//                          stores straight into the paged pool.
+// A row's bits do not depend on M, on its position in the call or on the call that carries it: one code
+// path, a fixed K order, no split-K; an accumulator column depends only on its own X row.
 #include <cuda.h>
 #include <math.h>
 
@@ -29,7 +33,7 @@ constexpr int PF_BLOCK_M = 128;         // UMMA M
 constexpr int PF_BLOCK_K = 64;          // one 128-byte swizzle row of bf16
 constexpr int PF_KSUB = 2;              // 64-wide k-blocks per pipeline stage: halves the per-stage hand-offs of the one-thread loops
 constexpr int PF_MAX_MT = 2;            // m-tiles per pass (TMEM columns = PF_MAX_MT * D)
-constexpr int PF_THREADS = 192;         // warp 0: TMA, warp 1: MMA, warps 2-5: X gather + epilogue
+constexpr int PF_THREADS = 192;         // warp 0: bulk-copy producer, warp 1: MMA, warps 2-5: epilogue
 constexpr int PF_SMEM_BUDGET = 200 * 1024;
 struct RowEntry {
   const __nv_bfloat16* src;             // hidden row
@@ -195,9 +199,15 @@ struct GemmParams {
 
 template <int D>
 __global__ void __launch_bounds__(PF_THREADS, 1) wf_prefill_gemm_kernel(const GemmParams p) {
-  constexpr int B_BYTES = PF_KSUB * PF_BLOCK_K * D * 2;  // W stage: PF_KSUB k-blocks of D/64 x [64 k][128 B], contiguous in wpack
-  constexpr int A_TILE = PF_BLOCK_M * PF_BLOCK_K * 2;  // 16 KB: 128 rows x 128 B
-  constexpr uint32_t TMEM_COLS = PF_MAX_MT * D;        // 256 or 128: a power of two >= 32
+  // Swapped operands: out^T[D x tokens] = W^T[D x hidden] . X^T[hidden x tokens].  The head's D output columns are the
+  // UMMA M dimension (always issued as M = 128; for D = 64 the upper 64 lanes compute on whatever follows in the
+  // ring and are never read), the call's tokens are the UMMA N dimension (padded to 16).  An MMA then costs
+  // max(128, M) * N / 256 = tokens / 2 cycles instead of 64: small calls stop being tensor-issue bound, and there
+  // is still ONE code path for every token count (lazy == eager bit for bit).
+  constexpr int W_SUB = PF_BLOCK_K * D * 2;               // one 64-row k-block of the W tile: D/64 x [64 k][128 B]
+  constexpr int W_BYTES = PF_KSUB * W_SUB;                // W stage, contiguous in wpack
+  constexpr int N_MAX = PF_MAX_MT * PF_BLOCK_M;           // tokens per pass (TMEM columns)
+  constexpr uint32_t TMEM_COLS = N_MAX;                   // 256: a power of two >= 32
   extern __shared__ __align__(1024) uint8_t smem[];
   __shared__ __align__(8) uint64_t s_full[PF_MAX_STAGES], s_empty[PF_MAX_STAGES], s_acc_full, s_acc_empty;
   __shared__ uint32_t s_tmem;
@@ -210,16 +220,16 @@ __global__ void __launch_bounds__(PF_THREADS, 1) wf_prefill_gemm_kernel(const Ge
   const int is_v = (tile / p.n_kv_heads) & 1;
   const int head = tile % p.n_kv_heads;
   const int n_kb = p.hidden / (PF_KSUB * PF_BLOCK_K);  // pipeline stages per pass
-  const int n_pass = (M + PF_MAX_MT * PF_BLOCK_M - 1) / (PF_MAX_MT * PF_BLOCK_M);
+  const int n_pass = (M + N_MAX - 1) / N_MAX;
 
-  // A stage holds only the rows that exist (8-row swizzle atoms); UMMA reads 128 rows from its start,
-  // the surplus lands in later stages / the W ring and feeds accumulator rows nobody reads.
-  const int m_first = min(M, PF_MAX_MT * PF_BLOCK_M);
-  const int a_sub = ((m_first + 7) / 8) * 1024;          // one 64-wide k-block of the A operand
-  const int a_bytes = PF_KSUB * a_sub;
-  const int n_stages = min(PF_MAX_STAGES, PF_SMEM_BUDGET / (a_bytes + B_BYTES));
-  uint8_t* a_base = smem;
-  uint8_t* b_base = smem + (size_t)n_stages * a_bytes;      // 1024-aligned: a_bytes is a multiple of 1024
+  // An X stage holds only the rows that exist (8-row swizzle atoms); UMMA reads n_pad (multiple of 16) rows from
+  // its start, the few surplus rows feed accumulator columns nobody reads.
+  const int m_first = min(M, N_MAX);
+  const int x_sub = ((m_first + 7) / 8) * 1024;          // one 64-wide k-block of the X operand
+  const int x_stage = PF_KSUB * x_sub;
+  const int n_stages = min(PF_MAX_STAGES, PF_SMEM_BUDGET / (x_stage + W_BYTES));
+  uint8_t* x_base = smem;
+  uint8_t* w_base = smem + (size_t)n_stages * x_stage;     // 1024-aligned: x_stage is a multiple of 1024
 
   if (tid == 0) {
     for (int i = 0; i < n_stages; ++i) { mbar_init(smem_u32(&s_full[i]), 1); mbar_init(smem_u32(&s_empty[i]), 1); }
@@ -234,29 +244,36 @@ __global__ void __launch_bounds__(PF_THREADS, 1) wf_prefill_gemm_kernel(const Ge
   const uint32_t tmem_base = s_tmem;
 
   if (warp == 0) {
-    // ===== bulk-copy producer: per stage ONE contiguous copy of the pre-swizzled W k-block and ONE of the packed X
+    // ===== bulk-copy producer: per stage ONE contiguous copy of the pre-swizzled W k-blocks and one per packed X
     //       k-block (wf_pack_x_kernel): no thread touches operand bytes.  Stage index, phase and addresses advance
-    //       incrementally: a runtime division per k-block in a one-thread loop costs more than the MMAs it feeds. =====
-    if (lane == 0) {
-      const uint8_t* w_src = p.wpack + (size_t)tile * n_kb * B_BYTES;    // tile = (layer, K|V, head), packed in that order
+    //       incrementally: a runtime division per stage in a one-thread loop costs more than the MMAs it feeds.
+    //       The whole warp runs the loop (warp-uniform control flow) and one elected lane issues: ptxas then emits
+    //       straight-line UBLKCP / UTCHMMA instead of a divergence loop around every instruction. =====
+    {
+      const uint8_t* w_src = p.wpack + (size_t)tile * n_kb * W_BYTES;    // tile = (layer, K|V, head), packed in that order
       const size_t x_kb_stride = (size_t)((M + 7) & ~7) * 128;
       const uint32_t full0 = smem_u32(&s_full[0]), empty0 = smem_u32(&s_empty[0]);
-      const uint32_t a0 = smem_u32(a_base), b0 = smem_u32(b_base);
+      const uint32_t x0 = smem_u32(x_base), w0 = smem_u32(w_base);
       int s = 0;
       uint32_t ph = 1;                                   // parity to wait for on s_empty: the ring starts empty
       for (int pass = 0; pass < n_pass; ++pass) {
-        const int rows_here = min(M - pass * PF_MAX_MT * PF_BLOCK_M, PF_MAX_MT * PF_BLOCK_M);
+        const int rows_here = min(M - pass * N_MAX, N_MAX);
         const uint32_t x_bytes = (uint32_t)((rows_here + 7) / 8) * 1024;
-        const uint8_t* x_src = p.xpack + (size_t)pass * PF_MAX_MT * PF_BLOCK_M * 128;
+        const uint8_t* x_src = p.xpack + (size_t)pass * N_MAX * 128;
         const uint8_t* w_kb = w_src;
+        // the epilogue of the previous pass transposes through the ring: do not refill it before it is done
+        if (pass > 0) mbar_wait(smem_u32(&s_acc_empty), (pass - 1) & 1);
         for (int kb = 0; kb < n_kb; ++kb) {
           mbar_wait(empty0 + 8 * s, ph);
-          const uint32_t bar = full0 + 8 * s;
-          mbar_arrive_expect_tx(bar, B_BYTES + PF_KSUB * x_bytes);
-          bulk_load(b0 + s * B_BYTES, w_kb, B_BYTES, bar);
+          if (elect_one()) {
+            const uint32_t bar = full0 + 8 * s;
+            mbar_arrive_expect_tx(bar, W_BYTES + PF_KSUB * x_bytes);
+            bulk_load(w0 + s * W_BYTES, w_kb, W_BYTES, bar);
 #pragma unroll
-          for (int u = 0; u < PF_KSUB; ++u) bulk_load(a0 + s * a_bytes + u * a_sub, x_src + u * x_kb_stride, x_bytes, bar);
-          w_kb += B_BYTES;
+            for (int u = 0; u < PF_KSUB; ++u) bulk_load(x0 + s * x_stage + u * x_sub, x_src + u * x_kb_stride, x_bytes, bar);
+          }
+          __syncwarp();
+          w_kb += W_BYTES;
           x_src += PF_KSUB * x_kb_stride;
           if (++s == n_stages) { s = 0; ph ^= 1; }
         }
@@ -264,107 +281,99 @@ __global__ void __launch_bounds__(PF_THREADS, 1) wf_prefill_gemm_kernel(const Ge
     }
   } else if (warp == 1) {
     // ===== MMA issuer: one thread drives the tensor core for the CTA.  Descriptors are built once and advanced by
-    //       constant offsets =====
-    if (lane == 0) {
-      const uint32_t idesc = umma_idesc(PF_BLOCK_M, D);
-      const uint64_t da0 = umma_desc(smem_u32(a_base), 16, 1024);          // K-major
-      const uint64_t db0 = umma_desc(smem_u32(b_base), 8192, 1024);        // MN-major
+    //       constant offsets.  A = W tile (MN-major, 128-byte swizzle), B = X rows (K-major, 128-byte swizzle). =====
+    {
+      const uint64_t dw0 = umma_desc(smem_u32(w_base), 8192, 1024);        // MN-major: 64-column halves 8 KB apart
+      const uint64_t dx0 = umma_desc(smem_u32(x_base), 16, 1024);          // K-major
       const uint32_t full0 = smem_u32(&s_full[0]), empty0 = smem_u32(&s_empty[0]);
-      const uint64_t da_step = (uint64_t)(a_bytes >> 4), db_step = (uint64_t)(B_BYTES >> 4);
+      const uint64_t dw_step = (uint64_t)(W_BYTES >> 4), dx_step = (uint64_t)(x_stage >> 4);
       int s = 0;
       uint32_t ph = 0;
-      uint64_t da = da0, db = db0;
+      uint64_t dw = dw0, dx = dx0;
       for (int pass = 0; pass < n_pass; ++pass) {
-        const int rows_here = min(M - pass * PF_MAX_MT * PF_BLOCK_M, PF_MAX_MT * PF_BLOCK_M);
-        const bool two = rows_here > PF_BLOCK_M;
+        const int rows_here = min(M - pass * N_MAX, N_MAX);
+        const uint32_t idesc = umma_idesc_mn_k(128, (rows_here + 15) & ~15);
         if (pass > 0) { mbar_wait(smem_u32(&s_acc_empty), (pass - 1) & 1); tc_fence_after(); }
         for (int kb = 0; kb < n_kb; ++kb) {
           mbar_wait(full0 + 8 * s, ph);
           tc_fence_after();
-          // k16 step j of the stage: A k-block j/4 (a_sub apart), 32 bytes per step; W k-block j/4 (64*D*2 apart), 2 KB per step
+          if (elect_one()) {
+          // k16 step j of the stage: W k-block j/4 (W_SUB apart), 16 k-rows = 2 KB per step; X k-block j/4 (x_sub apart),
+          // 32 bytes per step
 #pragma unroll
           for (int k16 = 0; k16 < PF_KSUB * PF_BLOCK_K / 16; ++k16)
-            umma_bf16(tmem_base, da + (uint64_t)(((k16 >> 2) * a_sub + (k16 & 3) * 32) >> 4),
-                      db + (uint64_t)(((k16 >> 2) * (PF_BLOCK_K * D * 2) + (k16 & 3) * 2048) >> 4), idesc, (kb | k16) != 0);
-          if (two) {
-#pragma unroll
-            for (int k16 = 0; k16 < PF_KSUB * PF_BLOCK_K / 16; ++k16)
-              umma_bf16(tmem_base + D, da + (uint64_t)(((k16 >> 2) * a_sub + A_TILE + (k16 & 3) * 32) >> 4),
-                        db + (uint64_t)(((k16 >> 2) * (PF_BLOCK_K * D * 2) + (k16 & 3) * 2048) >> 4), idesc, (kb | k16) != 0);
-          }
+            umma_bf16(tmem_base, dw + (uint64_t)(((k16 >> 2) * W_SUB + (k16 & 3) * 2048) >> 4),
+                      dx + (uint64_t)(((k16 >> 2) * x_sub + (k16 & 3) * 32) >> 4), idesc, (kb | k16) != 0);
           umma_commit(empty0 + 8 * s);                   // frees the stage when these MMAs retire
-          da += da_step; db += db_step;
-          if (++s == n_stages) { s = 0; ph ^= 1; da = da0; db = db0; }
+          }
+          __syncwarp();
+          dw += dw_step; dx += dx_step;
+          if (++s == n_stages) { s = 0; ph ^= 1; dw = dw0; dx = dx0; }
         }
-        umma_commit(smem_u32(&s_acc_full));
+        if (elect_one()) umma_commit(smem_u32(&s_acc_full));
+        __syncwarp();
       }
     }
   } else {
-    // ===== warps 2-5: epilogue =====
+    // ===== warps 2-5: epilogue.  TMEM lane = output column d of the head, TMEM column = token.  The accumulator is
+    //       transposed through shared memory (the operand ring is idle: every MMA of the pass has retired and the
+    //       producer waits for s_acc_empty), then each thread finishes 8 + 8 columns (r.., r + D/2..) of one token:
+    //       RoPE in fp32 on K tiles, bf16 RNE, two 16-byte stores straight into the paged pool. =====
     const int quarter = warp & 3;                        // TMEM lane quarter this warp may read
+    const int et = quarter * 32 + lane;                  // 0..127
+    float* tr = reinterpret_cast<float*>(smem);          // [tokens][D] fp32
+    constexpr int PC = D / 16;                           // column-pair chunks per token
     for (int pass = 0; pass < n_pass; ++pass) {
-      const int m_base = pass * PF_MAX_MT * PF_BLOCK_M;
-      const int rows_here = min(M - m_base, PF_MAX_MT * PF_BLOCK_M);
-      const int n_mt = (rows_here + PF_BLOCK_M - 1) / PF_BLOCK_M;
-      // ---- epilogue: TMEM -> registers -> (RoPE) -> bf16 -> paged pool ----
+      const int m_base = pass * N_MAX;
+      const int rows_here = min(M - m_base, N_MAX);
+      const int n_pad = (rows_here + 15) & ~15;
       mbar_wait(smem_u32(&s_acc_full), pass & 1);
       tc_fence_after();
-      for (int mt = 0; mt < n_mt; ++mt) {
-        const int m = m_base + mt * PF_BLOCK_M + quarter * 32 + lane;
-        const bool valid = m < M;
-        RowEntry e;
-        e.src = nullptr; e.pos = 0; e.page_slot = 0;
-        if (valid) e = p.rows[m];
-        __nv_bfloat16* dst = (is_v ? p.v_pool : p.k_pool) +
-            ((((size_t)layer * p.num_pages + (e.page_slot >> 4)) * p.n_kv_heads + head) * 16 + (e.page_slot & 15)) * D;
-        const uint32_t t_row = tmem_base + ((uint32_t)(quarter * 32) << 16) + mt * D;
-        if (!is_v) {
-          const float2* cs = p.rope + (size_t)e.pos * (D / 2);
+      for (int col0 = 0; col0 < n_pad; col0 += 32) {     // a load past n_pad stays inside the 256 allocated columns
+        uint32_t v[32];
+        tmem_ld32(tmem_base + ((uint32_t)(quarter * 32) << 16) + col0, v);
+        tmem_ld_wait();
+        if (et < D) {
 #pragma unroll
-          for (int j = 0; j < D / 64; ++j) {             // 32 rotation pairs (r, r + D/2) per step
-            uint32_t lo[32], hi[32];
-            tmem_ld32(t_row + j * 32, lo);
-            tmem_ld32(t_row + D / 2 + j * 32, hi);
-            tmem_ld_wait();
-            if (valid) {
-              uint32_t olo[16], ohi[16];
-#pragma unroll
-              for (int i = 0; i < 32; i += 2) {
-                const float4 c2 = *reinterpret_cast<const float4*>(cs + j * 32 + i);   // (cos,sin) x 2
-                const float a0 = __uint_as_float(lo[i]), b0 = __uint_as_float(hi[i]);
-                const float a1 = __uint_as_float(lo[i + 1]), b1 = __uint_as_float(hi[i + 1]);
-                olo[i / 2] = pack_bf16(a0 * c2.x - b0 * c2.y, a1 * c2.z - b1 * c2.w);
-                ohi[i / 2] = pack_bf16(b0 * c2.x + a0 * c2.y, b1 * c2.z + a1 * c2.w);
-              }
-#pragma unroll
-              for (int q4 = 0; q4 < 4; ++q4) {
-                *reinterpret_cast<uint4*>(dst + j * 32 + q4 * 8) = make_uint4(olo[q4 * 4], olo[q4 * 4 + 1], olo[q4 * 4 + 2], olo[q4 * 4 + 3]);
-                *reinterpret_cast<uint4*>(dst + D / 2 + j * 32 + q4 * 8) = make_uint4(ohi[q4 * 4], ohi[q4 * 4 + 1], ohi[q4 * 4 + 2], ohi[q4 * 4 + 3]);
-              }
-            }
-          }
-        } else {
-#pragma unroll
-          for (int j = 0; j < D / 32; ++j) {
-            uint32_t v[32];
-            tmem_ld32(t_row + j * 32, v);
-            tmem_ld_wait();
-            if (valid) {
-#pragma unroll
-              for (int q4 = 0; q4 < 4; ++q4) {
-                uint4 o;
-                o.x = pack_bf16(__uint_as_float(v[q4 * 8 + 0]), __uint_as_float(v[q4 * 8 + 1]));
-                o.y = pack_bf16(__uint_as_float(v[q4 * 8 + 2]), __uint_as_float(v[q4 * 8 + 3]));
-                o.z = pack_bf16(__uint_as_float(v[q4 * 8 + 4]), __uint_as_float(v[q4 * 8 + 5]));
-                o.w = pack_bf16(__uint_as_float(v[q4 * 8 + 6]), __uint_as_float(v[q4 * 8 + 7]));
-                *reinterpret_cast<uint4*>(dst + j * 32 + q4 * 8) = o;
-              }
-            }
-          }
+          for (int j = 0; j < 32; ++j)
+            if (col0 + j < rows_here) tr[(col0 + j) * D + et] = __uint_as_float(v[j]);
         }
       }
       tc_fence_before();
-      mbar_arrive(smem_u32(&s_acc_empty));               // TMEM may be overwritten by the next pass
+      named_bar_sync(1, 128);
+      for (int idx = et; idx < rows_here * PC; idx += 128) {
+        const int t = idx / PC, pc = idx % PC;
+        const RowEntry e = p.rows[m_base + t];
+        const float* lo = tr + t * D + pc * 8;
+        const float4 a0 = *reinterpret_cast<const float4*>(lo), a1 = *reinterpret_cast<const float4*>(lo + 4);
+        const float4 b0 = *reinterpret_cast<const float4*>(lo + D / 2), b1 = *reinterpret_cast<const float4*>(lo + D / 2 + 4);
+        const float a[8] = {a0.x, a0.y, a0.z, a0.w, a1.x, a1.y, a1.z, a1.w};
+        const float b[8] = {b0.x, b0.y, b0.z, b0.w, b1.x, b1.y, b1.z, b1.w};
+        float olo[8], ohi[8];
+        if (!is_v) {
+          const float4* cs = reinterpret_cast<const float4*>(p.rope + (size_t)e.pos * (D / 2) + pc * 8);   // (cos, sin) x 2
+#pragma unroll
+          for (int i = 0; i < 8; i += 2) {
+            const float4 c2 = __ldg(cs + i / 2);
+            olo[i] = a[i] * c2.x - b[i] * c2.y;
+            ohi[i] = b[i] * c2.x + a[i] * c2.y;
+            olo[i + 1] = a[i + 1] * c2.z - b[i + 1] * c2.w;
+            ohi[i + 1] = b[i + 1] * c2.z + a[i + 1] * c2.w;
+          }
+        } else {
+#pragma unroll
+          for (int i = 0; i < 8; ++i) { olo[i] = a[i]; ohi[i] = b[i]; }
+        }
+        __nv_bfloat16* dst = (is_v ? p.v_pool : p.k_pool) +
+            ((((size_t)layer * p.num_pages + (e.page_slot >> 4)) * p.n_kv_heads + head) * 16 + (e.page_slot & 15)) * D + pc * 8;
+        *reinterpret_cast<uint4*>(dst) = make_uint4(pack_bf16(olo[0], olo[1]), pack_bf16(olo[2], olo[3]),
+                                                    pack_bf16(olo[4], olo[5]), pack_bf16(olo[6], olo[7]));
+        *reinterpret_cast<uint4*>(dst + D / 2) = make_uint4(pack_bf16(ohi[0], ohi[1]), pack_bf16(ohi[2], ohi[3]),
+                                                            pack_bf16(ohi[4], ohi[5]), pack_bf16(ohi[6], ohi[7]));
+      }
+      fence_proxy_async();                               // generic reads of the ring before the next async-proxy writes
+      named_bar_sync(1, 128);                            // the transpose buffer is read: the ring may be refilled
+      mbar_arrive(smem_u32(&s_acc_empty));               // TMEM and the ring may be overwritten by the next pass
     }
   }
   tc_fence_before();

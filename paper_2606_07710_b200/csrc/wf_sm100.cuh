@@ -116,6 +116,10 @@ __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
 }
 
 
+// instruction descriptor: A MN-major, B K-major
+__device__ __forceinline__ uint32_t umma_idesc_mn_k(int M, int N) {
+  return (1u << 4) | (1u << 7) | (1u << 10) | (1u << 15) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
+}
 // instruction descriptor with both operands K-major
 __device__ __forceinline__ uint32_t umma_idesc_kk(int M, int N) {
   return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
