@@ -41,6 +41,8 @@ wf_accept_kernel(const float* __restrict__ logits, int V, int n_chunks, const in
                  int32_t* __restrict__ accept_len, int32_t* __restrict__ bonus_token, float* __restrict__ entropy,
                  int32_t* __restrict__ route, int32_t* __restrict__ n_commit, int32_t* __restrict__ kv_seq_len,
                  AccPartial* __restrict__ partials, unsigned int* __restrict__ counters) {
+  wf_pdl_trigger();
+  wf_pdl_wait();
   const int b = blockIdx.z, i = blockIdx.y, chunk = blockIdx.x;
   const int r0 = q_indptr[b];
   const int q_b = q_indptr[b + 1] - r0;
@@ -232,10 +234,10 @@ extern "C" int wf_accept_entropy_route(wf_ctx* ctx, const float* logits, int V, 
   int32_t* kv_len = target_kv ? target_kv->seq_len : nullptr;
   const bool vec = (V % 4 == 0) && ((uintptr_t)logits % 16 == 0);
   if (vec)
-    wf_accept_kernel<true><<<grid, ACC_THREADS, 0, st>>>(logits, V, n_chunks, draft_tokens, q_indptr, tau,
+    wf_launch(wf_accept_kernel<true>, grid, dim3(ACC_THREADS), 0, st, logits, V, n_chunks, draft_tokens, q_indptr, tau,
         tau_is_scalar, accept_len, bonus_token, entropy, route, n_commit, kv_len, (AccPartial*)workspace, ctx->d_counters);
   else
-    wf_accept_kernel<false><<<grid, ACC_THREADS, 0, st>>>(logits, V, n_chunks, draft_tokens, q_indptr, tau,
+    wf_launch(wf_accept_kernel<false>, grid, dim3(ACC_THREADS), 0, st, logits, V, n_chunks, draft_tokens, q_indptr, tau,
         tau_is_scalar, accept_len, bonus_token, entropy, route, n_commit, kv_len, (AccPartial*)workspace, ctx->d_counters);
   return wf_check_launch(ctx, "wf_accept_kernel");
 }

@@ -521,15 +521,9 @@ __global__ void __launch_bounds__(AT_THREADS, 1) wf_verify_attn_kernel(const Att
   uint8_t* k_s = p1_s + C::P_BYTES;
   uint8_t* v_s = k_s + C::STAGES_K * C::K_BYTES;
 
-  // per-sequence table (tiles per kv head, q_indptr, context) from the device-resident lengths, identical in
-  // every CTA; then total tiles and the longest pair
-  for (int b = tid; b < p.B; b += AT_THREADS) {
-    const int r0 = p.q_indptr[b], r1 = p.q_indptr[b + 1], ctx = p.kv.seq_len[b];
-    sh.r0[b] = r0;
-    sh.ctx[b] = ctx;
-    sh.pref[b + 1] = r1 > r0 ? (ctx + (r1 - r0) + AT_BN - 1) / AT_BN : 0;
-    if (b == p.B - 1) sh.r0[p.B] = r1;
-  }
+  // barrier init and TMEM allocation touch no global memory: they run before the dependency wait and overlap the
+  // tail of the previous kernel of the stream (programmatic dependent launch)
+  wf_pdl_trigger();
   if (tid == 0) {
     for (int i = 0; i < AT_MAX_STAGES; ++i) {
       mbar_init(smem_u32(&sh.k_full[i]), 1); mbar_init(smem_u32(&sh.k_empty[i]), 1);
@@ -546,6 +540,16 @@ __global__ void __launch_bounds__(AT_THREADS, 1) wf_verify_attn_kernel(const Att
     fence_barrier_init();
   }
   if (warp == 9) tmem_alloc(smem_u32(&sh.tmem), 512);
+  wf_pdl_wait();
+  // per-sequence table (tiles per kv head, q_indptr, context) from the device-resident lengths, identical in
+  // every CTA; then total tiles and the longest pair
+  for (int b = tid; b < p.B; b += AT_THREADS) {
+    const int r0 = p.q_indptr[b], r1 = p.q_indptr[b + 1], ctx = p.kv.seq_len[b];
+    sh.r0[b] = r0;
+    sh.ctx[b] = ctx;
+    sh.pref[b + 1] = r1 > r0 ? (ctx + (r1 - r0) + AT_BN - 1) / AT_BN : 0;
+    if (b == p.B - 1) sh.r0[p.B] = r1;
+  }
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
@@ -625,7 +629,7 @@ int launch_attn(wf_ctx* ctx, const AttnParams& p, cudaStream_t st) {
     configured = true;
   }
   const int grid = ctx->sm_count < AT_MAX_CTAS ? ctx->sm_count : AT_MAX_CTAS;   // one persistent CTA per SM
-  wf_verify_attn_kernel<D><<<grid, AT_THREADS, smem, st>>>(p);
+  wf_launch(wf_verify_attn_kernel<D>, dim3(grid), dim3(AT_THREADS), smem, st, p);
   return wf_check_launch(ctx, "wf_verify_attn_kernel");
 }
 

@@ -180,6 +180,8 @@ extern "C" const int32_t* wf_kv_pages_held(const wf_paged_kv* kv) { return kv ? 
 
 __global__ void __launch_bounds__(1024) wf_kv_reserve_kernel(KvView kv, const int32_t* __restrict__ add_tokens,
                                                              int B, int* status) {
+  wf_pdl_trigger();
+  wf_pdl_wait();
   kv_reserve_block(kv, B, [&](int b) { return add_tokens[b]; }, [](int b) { return b; }, status);
 }
 
@@ -188,12 +190,14 @@ extern "C" int wf_kv_reserve(wf_paged_kv* kv, const int32_t* add_tokens, int B, 
   wf_ctx* ctx = kv->ctx;
   WF_REQUIRE(ctx, add_tokens && B >= 0 && B <= kv->s.max_seqs, WF_ERR_INVALID_ARG, "wf_kv_reserve: bad arguments");
   if (B == 0) return WF_OK;
-  wf_kv_reserve_kernel<<<1, 1024, 0, (cudaStream_t)stream>>>(kv_view(kv), add_tokens, B, ctx->d_status);
+  wf_launch(wf_kv_reserve_kernel, dim3(1), dim3(1024), 0, (cudaStream_t)stream, kv_view(kv), add_tokens, B, ctx->d_status);
   return wf_check_launch(ctx, "wf_kv_reserve");
 }
 
 __global__ void wf_kv_release_kernel(KvView kv, int seq) {
   // pages return to the ring tail in block-table order
+  wf_pdl_trigger();
+  wf_pdl_wait();
   const int held = kv.pages_held[seq];
   const int head = kv.ring_state[0], count = kv.ring_state[1];
   int32_t* row = kv.block_table + (size_t)seq * kv.max_pages_per_seq;
@@ -213,6 +217,6 @@ extern "C" int wf_kv_release_seq(wf_paged_kv* kv, int seq, void* stream) {
   if (!kv) return WF_ERR_INVALID_ARG;
   wf_ctx* ctx = kv->ctx;
   WF_REQUIRE(ctx, seq >= 0 && seq < kv->s.max_seqs, WF_ERR_INVALID_ARG, "wf_kv_release_seq: bad sequence index");
-  wf_kv_release_kernel<<<1, 256, 0, (cudaStream_t)stream>>>(kv_view(kv), seq);
+  wf_launch(wf_kv_release_kernel, dim3(1), dim3(256), 0, (cudaStream_t)stream, kv_view(kv), seq);
   return wf_check_launch(ctx, "wf_kv_release_seq");
 }

@@ -73,6 +73,30 @@ int wf_make_tmap_2d(wf_ctx* ctx, CUtensorMap* out, const void* base, uint64_t ro
                     uint32_t box_rows);
 int wf_check_launch(wf_ctx* ctx, const char* what);   // cudaGetLastError -> WF_ERR_CUDA; counts the launch
 
+// ---------------------------------------------------------------------------------------------
+// Programmatic dependent launch.  Every kernel of the library is launched with programmatic stream
+// serialisation: it may be scheduled while the previous kernel of the stream is still running.  A
+// kernel calls wf_pdl_trigger() first (its successor may start launching) and wf_pdl_wait() before
+// its first access to global memory (blocks until the previous grid has completed and its writes
+// are visible); since every kernel waits before it finishes, completion is transitive.  What runs
+// before the wait (barrier init, TMEM allocation, launch latency) overlaps the predecessor's tail.
+// ---------------------------------------------------------------------------------------------
+#ifdef __CUDACC__
+__device__ __forceinline__ void wf_pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void wf_pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+template <typename... KArgs, typename... Args>
+inline cudaError_t wf_launch(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args&&... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr; cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+}
+#endif
+
 #define WF_REQUIRE(ctx, cond, code, ...)                         \
   do {                                                           \
     if (!(cond)) return wf_set_error((ctx), (code), __VA_ARGS__); \
@@ -93,16 +117,23 @@ int wf_check_launch(wf_ctx* ctx, const char* what);   // cudaGetLastError -> WF_
 // is allocated, *status becomes WF_ERR_OUT_OF_PAGES and false is returned (block-uniform).
 // Requires blockDim.x a multiple of 32, <= 1024.
 // ---------------------------------------------------------------------------------------------
+constexpr int KV_RESERVE_SMEM = 1024;
 template <typename AddFn, typename SeqFn>
 __device__ inline bool kv_reserve_block(const KvView& kv, int B, AddFn add, SeqFn seq, int* status) {
   __shared__ int s_warp[32];
   __shared__ int s_carry;
   __shared__ int s_bad;
+  // need / offset per sequence: shared memory for the first KV_RESERVE_SMEM sequences (the usual case: no global
+  // round trip between the scan and the ring copy), the library's global scratch beyond
+  __shared__ int s_need[KV_RESERVE_SMEM], s_off[KV_RESERVE_SMEM];
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5, nw = blockDim.x >> 5;
+  const int head = kv.ring_state[0], count = kv.ring_state[1];     // issued early: off the critical path
   if (tid == 0) { s_carry = 0; s_bad = 0; }
   __syncthreads();
-  int* need = kv.scratch;
-  int* off = kv.scratch + kv.max_seqs;
+  int* g_need = kv.scratch;
+  int* g_off = kv.scratch + kv.max_seqs;
+  auto need = [&](int b) -> int& { return b < KV_RESERVE_SMEM ? s_need[b] : g_need[b]; };
+  auto off = [&](int b) -> int& { return b < KV_RESERVE_SMEM ? s_off[b] : g_off[b]; };
   for (int base = 0; base < B; base += blockDim.x) {
     const int b = base + tid;
     int n = 0;
@@ -131,20 +162,19 @@ __device__ inline bool kv_reserve_block(const KvView& kv, int B, AddFn add, SeqF
     }
     __syncthreads();
     const int warp_excl = wid == 0 ? 0 : s_warp[wid - 1];
-    if (b < B) { need[b] = n; off[b] = s_carry + warp_excl + x - n; }
+    if (b < B) { need(b) = n; off(b) = s_carry + warp_excl + x - n; }
     __syncthreads();
     if (tid == 0) s_carry += s_warp[nw - 1];
     __syncthreads();
   }
   const int total = s_carry;
-  const int head = kv.ring_state[0], count = kv.ring_state[1];
   if (s_bad || total > count) {
     if (tid == 0) *status = WF_ERR_OUT_OF_PAGES;
     return false;
   }
   for (int b = wid; b < B; b += nw) {            // one warp per sequence copies its ring entries
     const int s = seq(b);
-    const int n = need[b], o = off[b], held = kv.pages_held[s];
+    const int n = need(b), o = off(b), held = kv.pages_held[s];
     for (int i = lane; i < n; i += 32)
       kv.block_table[(size_t)s * kv.max_pages_per_seq + held + i] = kv.free_ring[(head + o + i) % kv.num_pages];
     __syncwarp();

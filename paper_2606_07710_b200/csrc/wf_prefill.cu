@@ -64,7 +64,13 @@ struct PlanParams {
 __global__ void __launch_bounds__(1024) wf_prefill_plan_kernel(const PlanParams p) {
   __shared__ int s_warp[32];
   __shared__ int s_carry;
+  // rows / first compact row per sequence: shared memory for the first 1024 sequences, global scratch beyond
+  __shared__ int s_pn[KV_RESERVE_SMEM], s_po[KV_RESERVE_SMEM];
+  auto plan_n = [&](int b) -> int& { return b < KV_RESERVE_SMEM ? s_pn[b] : p.plan_n[b]; };
+  auto plan_off = [&](int b) -> int& { return b < KV_RESERVE_SMEM ? s_po[b] : p.plan_off[b]; };
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5, nw = blockDim.x >> 5;
+  wf_pdl_trigger();
+  wf_pdl_wait();
   auto seq_of = [&](int b) { return (p.mode != PLAN_FLUSH && p.seq_ids) ? p.seq_ids[b] : b; };
   // rows each sequence contributes to this call
   for (int b = tid; b < p.B; b += blockDim.x) {
@@ -79,12 +85,12 @@ __global__ void __launch_bounds__(1024) wf_prefill_plan_kernel(const PlanParams 
       if (p.mask[b] && add > p.cap) *p.status = WF_ERR_QUEUE_OVERFLOW;
       n = (p.mask[b] && add <= p.cap && p.backlog_len[sq] + add > p.cap) ? p.backlog_len[sq] : 0;
     }
-    p.plan_n[b] = n;
+    plan_n(b) = n;
   }
   if (tid == 0) s_carry = 0;
   __syncthreads();
   // pages first (C24: ascending b, consecutive ring entries); nothing is written if they do not fit
-  const bool ok = kv_reserve_block(p.kv, p.B, [&](int b) { return p.plan_n[b]; }, seq_of, p.status);
+  const bool ok = kv_reserve_block(p.kv, p.B, [&](int b) { return plan_n(b); }, seq_of, p.status);
   if (!ok) {
     if (tid == 0) *p.m_total = 0;
     return;
@@ -92,7 +98,7 @@ __global__ void __launch_bounds__(1024) wf_prefill_plan_kernel(const PlanParams 
   // exclusive scan of plan_n -> plan_off
   for (int base = 0; base < p.B; base += blockDim.x) {
     const int b = base + tid;
-    const int n = b < p.B ? p.plan_n[b] : 0;
+    const int n = b < p.B ? plan_n(b) : 0;
     int x = n;
 #pragma unroll
     for (int d = 1; d < 32; d <<= 1) {
@@ -111,7 +117,7 @@ __global__ void __launch_bounds__(1024) wf_prefill_plan_kernel(const PlanParams 
       s_warp[lane] = w;
     }
     __syncthreads();
-    if (b < p.B) p.plan_off[b] = s_carry + (wid ? s_warp[wid - 1] : 0) + x - n;
+    if (b < p.B) plan_off(b) = s_carry + (wid ? s_warp[wid - 1] : 0) + x - n;
     __syncthreads();
     if (tid == 0) s_carry += s_warp[nw - 1];
     __syncthreads();
@@ -124,7 +130,7 @@ __global__ void __launch_bounds__(1024) wf_prefill_plan_kernel(const PlanParams 
   // row table: one warp per sequence
   for (int b = wid; b < p.B; b += nw) {
     const int sq = seq_of(b);
-    const int n = p.plan_n[b], off = p.plan_off[b];
+    const int n = plan_n(b), off = plan_off(b);
     const int p0 = p.kv.seq_len[sq];
     const __nv_bfloat16* base = p.mode == PLAN_EAGER
         ? p.hidden_rows + (size_t)p.q_indptr[b] * p.hidden
@@ -157,6 +163,8 @@ constexpr int PF_MAX_STAGES = 12;
 // one bulk copy instead of gathering it with 128 threads.
 __global__ void __launch_bounds__(256) wf_pack_x_kernel(const RowEntry* __restrict__ rows, const int32_t* __restrict__ m_total,
                                                         uint8_t* __restrict__ xpack, int hidden) {
+  wf_pdl_trigger();
+  wf_pdl_wait();
   const int M = *m_total;
   const int r = blockIdx.x;                              // one row per block: every load of the block is independent
   if (r >= M) return;
@@ -195,6 +203,11 @@ struct GemmParams {
   __nv_bfloat16* k_pool;
   __nv_bfloat16* v_pool;
   int hidden, n_kv_heads, num_pages;
+  // split-K (fixed per drafter, so the summation order never depends on the call): CTA = (tile, split), partials
+  // [tile][split][row_cap][D] fp32, one self-resetting counter per (tile, pass)
+  int n_split, row_cap, max_pass;
+  float* ws_part;
+  unsigned int* split_cnt;
 };
 
 template <int D>
@@ -211,15 +224,21 @@ __global__ void __launch_bounds__(PF_THREADS, 1) wf_prefill_gemm_kernel(const Ge
   extern __shared__ __align__(1024) uint8_t smem[];
   __shared__ __align__(8) uint64_t s_full[PF_MAX_STAGES], s_empty[PF_MAX_STAGES], s_acc_full, s_acc_empty;
   __shared__ uint32_t s_tmem;
+  __shared__ int s_last;
 
+  wf_pdl_trigger();
+  wf_pdl_wait();
   const int M = *p.m_total;
   if (M == 0) return;                                  // nothing queued for this call
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int tile = blockIdx.x;                         // (layer, K|V, kv head)
+  const int tile = blockIdx.x / p.n_split;             // (layer, K|V, kv head)
+  const int split = blockIdx.x % p.n_split;            // this CTA's share of the k-blocks
   const int layer = tile / (2 * p.n_kv_heads);
   const int is_v = (tile / p.n_kv_heads) & 1;
   const int head = tile % p.n_kv_heads;
-  const int n_kb = p.hidden / (PF_KSUB * PF_BLOCK_K);  // pipeline stages per pass
+  const int n_kb_tile = p.hidden / (PF_KSUB * PF_BLOCK_K);   // pipeline stages of a whole tile
+  const int n_kb = n_kb_tile / p.n_split;                    // stages this CTA runs per pass (n_split divides them)
+  const int kb0 = split * n_kb;
   const int n_pass = (M + N_MAX - 1) / N_MAX;
 
   // An X stage holds only the rows that exist (8-row swizzle atoms); UMMA reads n_pad (multiple of 16) rows from
@@ -250,7 +269,7 @@ __global__ void __launch_bounds__(PF_THREADS, 1) wf_prefill_gemm_kernel(const Ge
     //       The whole warp runs the loop (warp-uniform control flow) and one elected lane issues: ptxas then emits
     //       straight-line UBLKCP / UTCHMMA instead of a divergence loop around every instruction. =====
     {
-      const uint8_t* w_src = p.wpack + (size_t)tile * n_kb * W_BYTES;    // tile = (layer, K|V, head), packed in that order
+      const uint8_t* w_src = p.wpack + ((size_t)tile * n_kb_tile + kb0) * W_BYTES;   // tile = (layer, K|V, head), packed in that order
       const size_t x_kb_stride = (size_t)((M + 7) & ~7) * 128;
       const uint32_t full0 = smem_u32(&s_full[0]), empty0 = smem_u32(&s_empty[0]);
       const uint32_t x0 = smem_u32(x_base), w0 = smem_u32(w_base);
@@ -259,7 +278,7 @@ __global__ void __launch_bounds__(PF_THREADS, 1) wf_prefill_gemm_kernel(const Ge
       for (int pass = 0; pass < n_pass; ++pass) {
         const int rows_here = min(M - pass * N_MAX, N_MAX);
         const uint32_t x_bytes = (uint32_t)((rows_here + 7) / 8) * 1024;
-        const uint8_t* x_src = p.xpack + (size_t)pass * N_MAX * 128;
+        const uint8_t* x_src = p.xpack + (size_t)pass * N_MAX * 128 + (size_t)kb0 * PF_KSUB * x_kb_stride;
         const uint8_t* w_kb = w_src;
         // the epilogue of the previous pass transposes through the ring: do not refill it before it is done
         if (pass > 0) mbar_wait(smem_u32(&s_acc_empty), (pass - 1) & 1);
@@ -329,19 +348,76 @@ __global__ void __launch_bounds__(PF_THREADS, 1) wf_prefill_gemm_kernel(const Ge
       const int n_pad = (rows_here + 15) & ~15;
       mbar_wait(smem_u32(&s_acc_full), pass & 1);
       tc_fence_after();
-      for (int col0 = 0; col0 < n_pad; col0 += 32) {     // a load past n_pad stays inside the 256 allocated columns
-        uint32_t v[32];
-        tmem_ld32(tmem_base + ((uint32_t)(quarter * 32) << 16) + col0, v);
-        tmem_ld_wait();
-        if (et < D) {
+      bool finish = true;                                // this CTA writes the pass's rows (always, without split-K)
+      if (p.n_split == 1) {
+        for (int col0 = 0; col0 < n_pad; col0 += 32) {   // a load past n_pad stays inside the 256 allocated columns
+          uint32_t v[32];
+          tmem_ld32(tmem_base + ((uint32_t)(quarter * 32) << 16) + col0, v);
+          tmem_ld_wait();
+          if (et < D) {
 #pragma unroll
-          for (int j = 0; j < 32; ++j)
-            if (col0 + j < rows_here) tr[(col0 + j) * D + et] = __uint_as_float(v[j]);
+            for (int j = 0; j < 32; ++j)
+              if (col0 + j < rows_here) tr[(col0 + j) * D + et] = __uint_as_float(v[j]);
+          }
+        }
+        tc_fence_before();
+        named_bar_sync(1, 128);
+      } else {
+        // split-K: publish this CTA's partial [token][D] (coalesced: lane = column); the last CTA of the tile to
+        // arrive sums the n_split partials in split order 0, 1, ... (its own included, re-read from L2), so the
+        // bits never depend on which CTA finishes last.
+        float* mine = p.ws_part + (((size_t)tile * p.n_split + split) * p.row_cap + m_base) * D;
+        for (int col0 = 0; col0 < n_pad; col0 += 32) {
+          uint32_t v[32];
+          tmem_ld32(tmem_base + ((uint32_t)(quarter * 32) << 16) + col0, v);
+          tmem_ld_wait();
+          if (et < D) {
+#pragma unroll
+            for (int j = 0; j < 32; ++j)
+              if (col0 + j < rows_here) mine[(size_t)(col0 + j) * D + et] = __uint_as_float(v[j]);
+          }
+        }
+        tc_fence_before();
+        __threadfence();
+        named_bar_sync(1, 128);
+        if (et == 0) {
+          unsigned int* cnt = p.split_cnt + tile * p.max_pass + pass;
+          const unsigned int old = atomicAdd(cnt, 1u);
+          s_last = (old == (unsigned int)p.n_split - 1);
+          if (s_last) *cnt = 0;                          // self-resetting for the next call
+        }
+        named_bar_sync(1, 128);
+        finish = s_last != 0;
+        if (finish) {
+          __threadfence();
+          const float* part0 = p.ws_part + ((size_t)tile * p.n_split * p.row_cap + m_base) * D;
+          const size_t split_stride = (size_t)p.row_cap * D;
+          // every load of a step is issued before the first is consumed (8 splits x 4 positions in flight per thread);
+          // the additions run in split order
+          constexpr int UI = 4, MAXS = 8;
+          const int n_pos = rows_here * (D / 4);               // float4 positions: idx = token * D/4 + chunk
+          for (int base = et; base < n_pos; base += 128 * UI) {
+            float4 x[UI][MAXS];
+#pragma unroll
+            for (int u = 0; u < UI; ++u)
+#pragma unroll
+              for (int sp = 0; sp < MAXS; ++sp)
+                if (sp < p.n_split && base + u * 128 < n_pos)
+                  x[u][sp] = __ldcg(reinterpret_cast<const float4*>(part0 + sp * split_stride) + base + u * 128);
+#pragma unroll
+            for (int u = 0; u < UI; ++u) {
+              if (base + u * 128 >= n_pos) continue;
+              float4 acc = x[u][0];
+#pragma unroll
+              for (int sp = 1; sp < MAXS; ++sp)
+                if (sp < p.n_split) { acc.x += x[u][sp].x; acc.y += x[u][sp].y; acc.z += x[u][sp].z; acc.w += x[u][sp].w; }
+              reinterpret_cast<float4*>(tr)[base + u * 128] = acc;
+            }
+          }
+          named_bar_sync(1, 128);
         }
       }
-      tc_fence_before();
-      named_bar_sync(1, 128);
-      for (int idx = et; idx < rows_here * PC; idx += 128) {
+      for (int idx = et; finish && idx < rows_here * PC; idx += 128) {
         const int t = idx / PC, pc = idx % PC;
         const RowEntry e = p.rows[m_base + t];
         const float* lo = tr + t * D + pc * 8;
@@ -394,6 +470,10 @@ struct wf_drafter {
   int32_t* backlog_len;
   uint8_t* d_wpack;            // library-owned pre-swizzled copy of the weights (see wf_pack_w_kernel)
   uint8_t* d_xpack;            // library-owned [hidden/64][row_cap][128 B] scratch (see wf_pack_x_kernel)
+  int n_split;                 // split-K factor of the projection, fixed at creation (a power of two)
+  int max_pass;
+  float* d_ws_part;            // [tiles][n_split][row_cap][D] fp32 partials (n_split > 1)
+  unsigned int* d_split_cnt;   // [tiles][max_pass]
   float2* d_rope;              // [max_pos][D/2]
   RowEntry* d_rows;
   int row_cap;
@@ -415,8 +495,9 @@ int launch_gemm(wf_drafter* d, cudaStream_t st) {
   g.wpack = d->d_wpack; g.xpack = d->d_xpack; g.rows = d->d_rows; g.m_total = d->d_m_total; g.rope = d->d_rope;
   g.k_pool = d->kv->k_pool; g.v_pool = d->kv->v_pool;
   g.hidden = d->s.hidden; g.n_kv_heads = d->s.n_kv_heads; g.num_pages = d->kv->s.num_pages;
-  const int grid = d->s.n_layers * 2 * d->s.n_kv_heads;
-  wf_prefill_gemm_kernel<D><<<grid, PF_THREADS, PF_SMEM_BUDGET, st>>>(g);
+  g.n_split = d->n_split; g.row_cap = d->row_cap; g.max_pass = d->max_pass; g.ws_part = d->d_ws_part; g.split_cnt = d->d_split_cnt;
+  const int grid = d->s.n_layers * 2 * d->s.n_kv_heads * d->n_split;
+  wf_launch(wf_prefill_gemm_kernel<D>, dim3(grid), dim3(PF_THREADS), PF_SMEM_BUDGET, st, g);
   return wf_check_launch(ctx, "wf_prefill_gemm_kernel");
 }
 
@@ -429,11 +510,11 @@ int run_prefill(wf_drafter* d, PlanParams& pp, int rows_upper, cudaStream_t st) 
   pp.rows = d->d_rows; pp.m_total = d->d_m_total;
   pp.plan_n = d->d_plan; pp.plan_off = d->d_plan + d->kv->s.max_seqs;
   pp.status = ctx->d_status;
-  wf_prefill_plan_kernel<<<1, 1024, 0, st>>>(pp);
+  wf_launch(wf_prefill_plan_kernel, dim3(1), dim3(1024), 0, st, pp);
   int rc = wf_check_launch(ctx, "wf_prefill_plan_kernel");
   if (rc != WF_OK) return rc;
   rows_upper = rows_upper < d->row_cap ? rows_upper : d->row_cap;
-  wf_pack_x_kernel<<<rows_upper > 0 ? rows_upper : 1, 256, 0, st>>>(d->d_rows, d->d_m_total, d->d_xpack, d->s.hidden);
+  wf_launch(wf_pack_x_kernel, dim3(rows_upper > 0 ? rows_upper : 1), dim3(256), 0, st, (const RowEntry*)d->d_rows, (const int32_t*)d->d_m_total, d->d_xpack, d->s.hidden);
   rc = wf_check_launch(ctx, "wf_pack_x_kernel");
   if (rc != WF_OK) return rc;
   return d->s.head_dim == 128 ? launch_gemm<128>(d, st) : launch_gemm<64>(d, st);
@@ -475,11 +556,27 @@ extern "C" int wf_drafter_create(wf_ctx* ctx, const wf_drafter_shape* s, const v
   if (!d) return wf_set_error(ctx, WF_ERR_INVALID_ARG, "wf_drafter_create: host allocation failed");
   d->ctx = ctx; d->s = *s; d->kv = kv;
   d->backlog = (const __nv_bfloat16*)backlog; d->backlog_len = backlog_len;
-  d->d_wpack = nullptr; d->d_xpack = nullptr; d->d_rope = nullptr; d->d_rows = nullptr; d->d_m_total = nullptr; d->d_plan = nullptr;
+  d->d_wpack = nullptr; d->d_xpack = nullptr; d->d_rope = nullptr; d->d_ws_part = nullptr; d->d_split_cnt = nullptr; d->d_rows = nullptr; d->d_m_total = nullptr; d->d_plan = nullptr;
   d->row_cap = kv->s.max_seqs * (s->backlog_cap > 64 ? s->backlog_cap : 64);
+  // Split-K: a call with few tiles (a 1-layer drafter has 16) cannot pull HBM bandwidth through 16 SMs; spread each
+  // tile's k-blocks over the largest power of two of CTAs that still fits one CTA per SM.  The factor depends on the
+  // drafter's shape only, never on the call, so a row's bits do not depend on M (lazy == eager).
+  {
+    const int tiles = L * 2 * s->n_kv_heads, stages = s->hidden / (PF_KSUB * PF_BLOCK_K);
+    int ns = 1;
+    while (ns * 2 <= 8 && tiles * ns * 2 <= ctx->sm_count && stages % (ns * 2) == 0) ns *= 2;
+    d->n_split = ns;
+    d->max_pass = (d->row_cap + PF_MAX_MT * PF_BLOCK_M - 1) / (PF_MAX_MT * PF_BLOCK_M);
+  }
   const size_t w_bytes = (size_t)s->hidden * N * 2;                    // one [hidden][Hkv*D] matrix
   cudaError_t e = cudaMalloc(&d->d_wpack, w_bytes * 2 * L);
   if (e == cudaSuccess) e = cudaMalloc(&d->d_xpack, (size_t)s->hidden * 2 * d->row_cap);
+  if (e == cudaSuccess && d->n_split > 1) {
+    const size_t tiles = (size_t)L * 2 * s->n_kv_heads;
+    e = cudaMalloc(&d->d_ws_part, tiles * d->n_split * d->row_cap * D * sizeof(float));
+    if (e == cudaSuccess) e = cudaMalloc(&d->d_split_cnt, tiles * d->max_pass * sizeof(unsigned int));
+    if (e == cudaSuccess) e = cudaMemset(d->d_split_cnt, 0, tiles * d->max_pass * sizeof(unsigned int));
+  }
   if (e == cudaSuccess) e = cudaMalloc(&d->d_rope, sizeof(float2) * rope.size());
   if (e == cudaSuccess) e = cudaMalloc(&d->d_rows, sizeof(RowEntry) * d->row_cap);
   if (e == cudaSuccess) e = cudaMalloc(&d->d_m_total, sizeof(int32_t));
@@ -504,7 +601,7 @@ extern "C" int wf_drafter_create(wf_ctx* ctx, const wf_drafter_shape* s, const v
 
 extern "C" int wf_drafter_destroy(wf_drafter* d) {
   if (!d) return WF_ERR_INVALID_ARG;
-  cudaFree(d->d_wpack); cudaFree(d->d_xpack); cudaFree(d->d_rope); cudaFree(d->d_rows); cudaFree(d->d_m_total); cudaFree(d->d_plan);
+  cudaFree(d->d_wpack); cudaFree(d->d_xpack); cudaFree(d->d_ws_part); cudaFree(d->d_split_cnt); cudaFree(d->d_rope); cudaFree(d->d_rows); cudaFree(d->d_m_total); cudaFree(d->d_plan);
   delete d;
   return WF_OK;
 }
@@ -540,6 +637,8 @@ __global__ void wf_enqueue_kernel(const __nv_bfloat16* __restrict__ hidden, cons
                                   const int32_t* __restrict__ n_rows, const int32_t* __restrict__ seq_ids,
                                   const int32_t* __restrict__ idle_mask, __nv_bfloat16* __restrict__ backlog,
                                   const int32_t* __restrict__ backlog_len, int hidden_dim, int cap) {
+  wf_pdl_trigger();
+  wf_pdl_wait();
   const int b = blockIdx.y, t = blockIdx.x;
   if (!idle_mask[b]) return;
   const int n = n_rows[b];
@@ -551,6 +650,8 @@ __global__ void wf_enqueue_kernel(const __nv_bfloat16* __restrict__ hidden, cons
 }
 __global__ void wf_enqueue_len_kernel(const int32_t* __restrict__ n_rows, const int32_t* __restrict__ seq_ids,
                                       const int32_t* __restrict__ idle_mask, int32_t* __restrict__ backlog_len, int B, int cap) {
+  wf_pdl_trigger();
+  wf_pdl_wait();
   const int b = blockIdx.x * blockDim.x + threadIdx.x;
   if (b < B && idle_mask[b] && n_rows[b] <= cap) backlog_len[seq_ids ? seq_ids[b] : b] += n_rows[b];
 }
@@ -573,10 +674,10 @@ extern "C" int wf_lazy_catchup_enqueue(wf_ctx* ctx, wf_drafter* d, const void* h
   int rc = run_prefill(d, pp, B * d->s.backlog_cap, st);
   if (rc != WF_OK) return rc;
   // (2) append the rows, (3) advance the lengths
-  wf_enqueue_kernel<<<dim3(max_rows, B), 128, 0, st>>>((const __nv_bfloat16*)hidden, q_indptr, n_rows, seq_ids, idle_mask,
-                                                      const_cast<__nv_bfloat16*>(d->backlog), d->backlog_len, d->s.hidden, d->s.backlog_cap);
+  wf_launch(wf_enqueue_kernel, dim3(max_rows, B), dim3(128), 0, st, (const __nv_bfloat16*)hidden, q_indptr, n_rows, seq_ids, idle_mask,
+            const_cast<__nv_bfloat16*>(d->backlog), (const int32_t*)d->backlog_len, d->s.hidden, d->s.backlog_cap);
   rc = wf_check_launch(ctx, "wf_enqueue_kernel");
   if (rc != WF_OK) return rc;
-  wf_enqueue_len_kernel<<<(B + 255) / 256, 256, 0, st>>>(n_rows, seq_ids, idle_mask, d->backlog_len, B, d->s.backlog_cap);
+  wf_launch(wf_enqueue_len_kernel, dim3((B + 255) / 256), dim3(256), 0, st, n_rows, seq_ids, idle_mask, d->backlog_len, B, d->s.backlog_cap);
   return wf_check_launch(ctx, "wf_enqueue_len_kernel");
 }
