@@ -30,6 +30,7 @@ constexpr int AT_MAX_B = 1024;
 constexpr int AT_MAX_STAGES = 4;
 constexpr int AT_MAX_CTAS = 160;       // workspace is sized for this many persistent CTAs
 constexpr int AT_MAX_SEG = 32;         // partials merged per (b, g) pair
+constexpr int AT_SEG_COST = 3;         // fixed cost of a segment (Q load, pipeline restart, merge, stores) in tiles
 constexpr float LOG2E = 1.4426950408889634f;
 
 struct AttnParams {
@@ -64,7 +65,7 @@ struct AttnShared {
   uint64_t k_full[AT_MAX_STAGES], k_empty[AT_MAX_STAGES], v_full[AT_MAX_STAGES], v_empty[AT_MAX_STAGES];
   uint64_t s_full[2], s_empty[2], o_empty[2], p_full[2], pv_done[2], q_ready;
   float xm[2][128], xl[2][128];        // group-1 running max / row-sum partials for the group merge
-  int pref[AT_MAX_B + 1];              // exclusive prefix of 128-key tiles per kv head over the sequences
+  int pref[AT_MAX_B + 1];              // exclusive prefix over the sequences of (tiles per kv head + AT_SEG_COST)
   int r0[AT_MAX_B + 1];                // q_indptr
   int ctx[AT_MAX_B];                   // seq_len
   int total_tiles, g_eff, B;
@@ -76,16 +77,20 @@ struct Segment {
   int b, g, t_lo, t_hi, nt;            // tiles [t_lo, t_hi) of the pair's nt tiles
   int r0, q_b, ctx, k0, k1, n_tiles;
   int partial, slot;                   // partial: the pair is shared with other CTAs; slot = 2c + (0 head | 1 tail)
-  int flat0;                           // flattened index of the pair's tile 0
+  int flat0;                           // weighted position of the pair (its tile t sits at flat0 + AT_SEG_COST + t)
 };
 
-// Walks the tile range of one CTA over the flattened (b, g, tile) list; every role keeps its own walker.
-// The per-sequence table lives in shared memory (built once in the prologue), so a walk costs no global
-// round trips.
+// Walks the range of one CTA over the flattened, WEIGHTED (b, g, tile) list; every role keeps its own walker.
+// A pair of nt tiles occupies AT_SEG_COST + nt positions: the first AT_SEG_COST stand for the fixed cost of a
+// segment, tile t sits at position AT_SEG_COST + t.  Equal shares of positions are then equal shares of time
+// even when some CTAs get many short pairs (cfg5: 16 five-tile pairs in one range cost twice the average
+// before).  The per-sequence table lives in shared memory (built once in the prologue), so a walk costs no
+// global round trips.
 struct SegWalker {
   const AttnShared& sh;
   int Hkv, c;
   int lo, hi, x, b;
+  bool first = true;
   __device__ SegWalker(const AttnShared& sh_, int Hkv_, int c_) : sh(sh_), Hkv(Hkv_), c(c_) {
     const int T = sh.total_tiles, G = sh.g_eff;
     lo = (int)((long long)c * T / G);
@@ -99,25 +104,30 @@ struct SegWalker {
     b = l;
   }
   __device__ bool next(Segment& s) {
-    if (x >= hi) return false;
-    while (x >= Hkv * sh.pref[b + 1]) ++b;                     // also skips empty sequences
-    const int nt = sh.pref[b + 1] - sh.pref[b];
-    const int pref = Hkv * sh.pref[b];
-    const int local = x - pref;
-    s.b = b; s.nt = nt;
-    s.g = local / nt; s.t_lo = local % nt;
-    s.t_hi = min(nt, s.t_lo + (hi - x));
-    s.flat0 = pref + s.g * nt;
-    s.r0 = sh.r0[b];
-    s.q_b = sh.r0[b + 1] - s.r0;
-    s.ctx = sh.ctx[b];
-    s.k0 = s.t_lo * AT_BN;
-    s.k1 = min(s.ctx + s.q_b, s.t_hi * AT_BN);
-    s.n_tiles = s.t_hi - s.t_lo;
-    s.partial = !(s.t_lo == 0 && s.t_hi == nt);
-    s.slot = 2 * c + (x == lo ? 0 : 1);
-    x += s.n_tiles;
-    return true;
+    while (x < hi) {
+      while (x >= Hkv * sh.pref[b + 1]) ++b;                   // also skips empty sequences
+      const int wlen = sh.pref[b + 1] - sh.pref[b], nt = wlen - AT_SEG_COST;
+      const int base = Hkv * sh.pref[b];
+      const int g = (x - base) / wlen;
+      const int wbase = base + g * wlen;
+      const int t_lo = max(0, x - wbase - AT_SEG_COST);
+      const int t_hi = min(nt, hi - wbase - AT_SEG_COST);
+      x = t_hi >= nt ? wbase + wlen : hi;                      // the pair is finished, or the range is
+      if (t_hi <= t_lo) continue;                              // the range ends inside the cost positions
+      s.b = b; s.nt = nt; s.g = g; s.t_lo = t_lo; s.t_hi = t_hi;
+      s.flat0 = wbase;
+      s.r0 = sh.r0[b];
+      s.q_b = sh.r0[b + 1] - s.r0;
+      s.ctx = sh.ctx[b];
+      s.k0 = t_lo * AT_BN;
+      s.k1 = min(s.ctx + s.q_b, t_hi * AT_BN);
+      s.n_tiles = t_hi - t_lo;
+      s.partial = !(t_lo == 0 && t_hi == nt);
+      s.slot = 2 * c + (first ? 0 : 1);
+      first = false;
+      return true;
+    }
+    return false;
   }
 };
 
@@ -267,6 +277,21 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared& sh
   uint32_t gt0 = 0;                                            // global tile counter at the start of the segment
   while (walk.next(sg)) {
     const int R = sg.q_b * p.group;
+    {
+      // The NEXT segment's Q rows go to L2 now: under a saturated HBM a cold Q load took 6k cycles at every
+      // segment start.  A token's `group` heads are contiguous: group * D * 2 bytes = D / 64 * group lines of 128 B.
+      SegWalker peek = walk;
+      Segment nx;
+      if (peek.next(nx)) {
+        const int lines_per_tok = p.group * D * 2 / 128;
+        const int idx = grp * 128 + stid;
+        if (idx < nx.q_b * lines_per_tok) {
+          const char* a = reinterpret_cast<const char*>(p.q + ((size_t)(nx.r0 + idx / lines_per_tok) * p.n_q_heads + nx.g * p.group) * D) +
+                          (idx % lines_per_tok) * 128;
+          asm volatile("prefetch.global.L2 [%0];" ::"l"(a));
+        }
+      }
+    }
     // ---- Q tile -> smem (K-major, 128-byte swizzle) by both groups; rows >= R are zero.  Every MMA of the
     //      previous segment has retired (both groups waited for their last pv_done). ----
     for (int c = grp * 128 + stid; c < AT_ROWS * (D / 8); c += 256) {
@@ -391,8 +416,8 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared& sh
     int c_first = 0, n_seg = 1;
     unsigned int arrive_old = 0;
     if (sg.partial && grp == 0) {
-      c_first = cta_of_tile(sg.flat0, T, G);
-      n_seg = cta_of_tile(sg.flat0 + sg.nt - 1, T, G) - c_first + 1;
+      c_first = cta_of_tile(sg.flat0 + AT_SEG_COST, T, G);
+      n_seg = cta_of_tile(sg.flat0 + AT_SEG_COST + sg.nt - 1, T, G) - c_first + 1;
       if (stid == 0) arrive_old = atomicAdd(&p.counters[sg.b * Hkv + sg.g], 1u);
     }
 
@@ -547,7 +572,7 @@ __global__ void __launch_bounds__(AT_THREADS, 1) wf_verify_attn_kernel(const Att
     const int r0 = p.q_indptr[b], r1 = p.q_indptr[b + 1], ctx = p.kv.seq_len[b];
     sh.r0[b] = r0;
     sh.ctx[b] = ctx;
-    sh.pref[b + 1] = r1 > r0 ? (ctx + (r1 - r0) + AT_BN - 1) / AT_BN : 0;
+    sh.pref[b + 1] = r1 > r0 ? (ctx + (r1 - r0) + AT_BN - 1) / AT_BN + AT_SEG_COST : 0;
     if (b == p.B - 1) sh.r0[p.B] = r1;
   }
   tc_fence_before();
