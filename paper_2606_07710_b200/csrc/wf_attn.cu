@@ -30,7 +30,7 @@ constexpr int AT_MAX_B = 1024;
 constexpr int AT_MAX_STAGES = 4;
 constexpr int AT_MAX_CTAS = 160;       // workspace is sized for this many persistent CTAs
 constexpr int AT_MAX_SEG = 32;         // partials merged per (b, g) pair
-constexpr int AT_SEG_COST = 3;         // fixed cost of a segment (Q load, pipeline restart, merge, stores) in tiles
+constexpr int AT_SEG_COST = 4;         // fixed cost of a segment (Q load, pipeline restart, merge, stores) in tiles
 constexpr float LOG2E = 1.4426950408889634f;
 
 struct AttnParams {
@@ -294,14 +294,26 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared& sh
     }
     // ---- Q tile -> smem (K-major, 128-byte swizzle) by both groups; rows >= R are zero.  Every MMA of the
     //      previous segment has retired (both groups waited for their last pv_done). ----
-    for (int c = grp * 128 + stid; c < AT_ROWS * (D / 8); c += 256) {
-      const int rr = c / (D / 8), chn = c % (D / 8);
-      uint4 v = make_uint4(0, 0, 0, 0);
-      if (rr < R) {
-        const int i2 = rr / p.group, h2 = rr % p.group;
-        v = __ldg(reinterpret_cast<const uint4*>(p.q + ((size_t)(sg.r0 + i2) * p.n_q_heads + sg.g * p.group + h2) * D) + chn);
+    {
+      // all loads first, then the stores: one round trip instead of one per chunk
+      constexpr int NQ = AT_ROWS * (D / 8) / 256;
+      uint4 qv[NQ];
+#pragma unroll
+      for (int u = 0; u < NQ; ++u) {
+        const int c = grp * 128 + stid + u * 256;
+        const int rr = c / (D / 8), chn = c % (D / 8);
+        qv[u] = make_uint4(0, 0, 0, 0);
+        if (rr < R) {
+          const int i2 = rr / p.group, h2 = rr % p.group;
+          qv[u] = __ldg(reinterpret_cast<const uint4*>(p.q + ((size_t)(sg.r0 + i2) * p.n_q_heads + sg.g * p.group + h2) * D) + chn);
+        }
       }
-      *reinterpret_cast<uint4*>(q_s + (chn >> 3) * C::Q_HALF + rr * 128 + (((chn & 7) ^ (rr & 7)) << 4)) = v;
+#pragma unroll
+      for (int u = 0; u < NQ; ++u) {
+        const int c = grp * 128 + stid + u * 256;
+        const int rr = c / (D / 8), chn = c % (D / 8);
+        *reinterpret_cast<uint4*>(q_s + (chn >> 3) * C::Q_HALF + rr * 128 + (((chn & 7) ^ (rr & 7)) << 4)) = qv[u];
+      }
     }
     fence_proxy_async();
     mbar_arrive(smem_u32(&sh.q_ready));
