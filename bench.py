@@ -27,6 +27,9 @@ sys.path.insert(0, ROOT)
 from paper_2606_07710_b200 import synth  # noqa: E402
 
 WORKLOADS = {"cfg1": 0, "cfg2": 1, "cfg3": 2, "cfg4": 3, "cfg5": 4}
+# dram__bytes_read.sum + dram__bytes_write.sum per attention launch from the committed `ncu --set full` capture
+# (profiles/r1d_ncu_full.md); workloads without a capture report null
+NCU_TRAFFIC_BYTES = {"cfg3": 552.0e6}
 METRIC = "verify_rounds_per_s"
 UNIT = "rounds/s"
 
@@ -40,17 +43,54 @@ def measured_peaks():
 
 
 class ClockSampler:
-    """nvidia-smi clocks and throttle reasons sampled DURING the timed region."""
+    """SM clock and throttle reasons sampled DURING the timed region: NVML (what nvidia-smi reads) polled every 5 ms
+    from a thread started before the warm-up; `nvidia-smi -lms` as the fallback.  mark() brackets the timed region."""
     Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
          "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+    NAMES = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
 
     def __init__(self, index):
-        self.index, self.rows, self.proc = index, [], None
+        self.index, self.rows, self.proc, self.thread = index, [], None, None
+        self.t_mark = []                  # host times bracketing the timed region (after a device sync each)
+        self.stop_flag = False
+        self.source = None
+
+    def _phys_index(self):
+        vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+        if vis:
+            ids = [v.strip() for v in vis.split(",") if v.strip()]
+            if self.index < len(ids) and ids[self.index].isdigit():
+                return int(ids[self.index])
+        return self.index
 
     def start(self):
         try:
+            import pynvml
+            pynvml.nvmlInit()
+            h = pynvml.nvmlDeviceGetHandleByIndex(self._phys_index())
+            mx = float(pynvml.nvmlDeviceGetMaxClockInfo(h, pynvml.NVML_CLOCK_SM))
+            bits = [pynvml.nvmlClocksThrottleReasonHwSlowdown, pynvml.nvmlClocksThrottleReasonHwThermalSlowdown,
+                    pynvml.nvmlClocksThrottleReasonSwThermalSlowdown, pynvml.nvmlClocksThrottleReasonSwPowerCap]
+
+            def poll():
+                while not self.stop_flag:
+                    try:
+                        sm = float(pynvml.nvmlDeviceGetClockInfo(h, pynvml.NVML_CLOCK_SM))
+                        r = int(pynvml.nvmlDeviceGetCurrentClocksThrottleReasons(h))
+                        self.rows.append((time.time(), sm, mx, [bool(r & b) for b in bits]))
+                    except Exception:
+                        pass
+                    time.sleep(0.005)
+            self.source = "nvml"
+            self.thread = threading.Thread(target=poll, daemon=True)
+            self.thread.start()
+            return
+        except Exception:
+            pass
+        try:
             self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                                          "-i", str(self.index), "-lms", "100"], stdout=subprocess.PIPE, text=True)
+                                          "-i", str(self._phys_index()), "-lms", "20"], stdout=subprocess.PIPE, text=True)
+            self.source = "nvidia-smi -lms 20"
             self.thread = threading.Thread(target=self._read, daemon=True)
             self.thread.start()
         except OSError:
@@ -58,20 +98,33 @@ class ClockSampler:
 
     def _read(self):
         for line in self.proc.stdout:
-            self.rows.append([x.strip() for x in line.split(",")])
+            r = [x.strip() for x in line.split(",")]
+            if len(r) >= 6 and r[0].replace(".", "").isdigit():
+                mx = float(r[1]) if r[1].replace(".", "").isdigit() else None
+                self.rows.append((time.time(), float(r[0]), mx, [v.lower().startswith("active") for v in r[2:6]]))
+
+    def mark(self):
+        self.t_mark.append(time.time())
 
     def stop(self):
-        if not self.proc:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
-        time.sleep(0.15)
-        self.proc.terminate()
+        if not self.thread:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvml and nvidia-smi unavailable"]}
+        time.sleep(0.05)
+        self.stop_flag = True
+        if self.proc:
+            self.proc.terminate()
         self.thread.join(timeout=2)
-        sm = [float(r[0]) for r in self.rows if len(r) >= 6 and r[0].replace(".", "").isdigit()]
-        mx = [float(r[1]) for r in self.rows if len(r) >= 6 and r[1].replace(".", "").isdigit()]
-        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        reasons = sorted({n for r in self.rows if len(r) >= 6 for n, v in zip(names, r[2:6]) if v.lower().startswith("active")})
+        # samples inside the timed region; a region shorter than 3 samples falls back to every sample taken while
+        # the GPU was under this run's load (warm-up, timed region, e2e)
+        window = "timed region"
+        sel = [r for r in self.rows if len(self.t_mark) == 2 and self.t_mark[0] <= r[0] <= self.t_mark[1]]
+        if len(sel) < 3:
+            sel, window = list(self.rows), "warm-up + timed region + e2e (timed region shorter than 3 samples)"
+        sm = [r[1] for r in sel]
+        mx = [r[2] for r in sel if r[2]]
+        reasons = sorted({n for r in sel for n, v in zip(self.NAMES, r[3]) if v})
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
-                "reasons": reasons, "samples": len(sm)}
+                "reasons": reasons, "samples": len(sm), "window": window, "source": self.source}
 
 
 def dist_setup(n_gpus):
@@ -289,7 +342,9 @@ def run_ours(args):
                                    f"accept/entropy/route ({tot['t_accept']:.2f} s), KV-only prefill of {rows_p} rows into both drafters "
                                    f"({tot['t_prefill']:.1f} s); scaled to a whole round by layers x tokens, logit rows and committed rows")}
 
-    # ---- warm-up ----
+    # ---- warm-up (the clock sampler starts here so that nvidia-smi is up when the timed region begins) ----
+    sampler = ClockSampler(local)
+    sampler.start()
     for _ in range(W):
         s = rs.run_round()
     rs.check_plan(s)
@@ -298,12 +353,11 @@ def run_ours(args):
     evs = [{"attn": (torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)),
             "catchup": (torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))} for _ in range(K)]
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    sampler = ClockSampler(local)
     attn_bytes = []
     len_host = rs.seq_len.cpu().numpy().astype(np.int64)     # the plan tells us how contexts grow
     launches0 = ctx.launch_count()
     sync_all(world)
-    sampler.start()
+    sampler.mark()
     e0.record()
     for i in range(K):
         s = rs.slots[rs.rounds_done % rs.n_slots]
@@ -312,7 +366,7 @@ def run_ours(args):
         rs.run_round(events=evs[i])
     e1.record()
     sync_all(world)
-    clocks = sampler.stop()
+    sampler.mark()
     launches = ctx.launch_count() - launches0
     ms_local = e0.elapsed_time(e1)
     ms = barrier_max(ms_local, world)
@@ -343,6 +397,7 @@ def run_ours(args):
     f1.record()
     sync_all(world)
     e2e_ms = barrier_max(f0.elapsed_time(f1), world)
+    clocks = sampler.stop()
     rs.check_plan(s)
 
     if rank == 0:
@@ -363,7 +418,9 @@ def run_ours(args):
             "catchup_share_of_round": catch_ms / ms_local,
             "attn_share_of_round": attn_ms / ms_local,
             "roofline": {"bound": "hbm", "kernel": "wf_verify_attn_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                         "frac": achieved / peak, "peak_source": peak_src, "traffic": args.traffic_bytes,
+                         "frac": achieved / peak, "peak_source": peak_src,
+                         "traffic": args.traffic_bytes if args.traffic_bytes is not None else NCU_TRAFFIC_BYTES.get(args.workload),
+                         "traffic_source": "profiles/r1d_ncu_full.md",
                          "algorithmic_bytes_per_launch": float(np.mean(attn_bytes)), "avg_launch_us": 1e3 * avg_launch_ms},
             "e2e": {"value": world * e2e_steps / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d // e2e_steps,
                     "d2h_bytes_per_step": d2h // e2e_steps, "steps": e2e_steps},
@@ -384,7 +441,7 @@ def run_ours(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=12)
+    ap.add_argument("--steps", type=int, default=60)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg3", choices=sorted(WORKLOADS))
@@ -393,7 +450,7 @@ def main():
     ap.add_argument("--cpu-sample-seqs", type=int, default=4)
     ap.add_argument("--cpu-sample-layers", type=int, default=8)
     ap.add_argument("--traffic-bytes", type=float, default=None,
-                    help="dram bytes per attention launch from the committed ncu --set full capture (profiles/)")
+                    help="dram bytes per attention launch; default: the committed ncu --set full capture for the workload")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
