@@ -400,6 +400,18 @@ def run_ours(args):
     clocks = sampler.stop()
     rs.check_plan(s)
 
+    # ---- WhiFlash-Neural router, timed on its own: the round above uses the entropy policy ----
+    n0, n1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    for _ in range(3):
+        rs.run_neural_route(s)
+    torch.cuda.synchronize()
+    n0.record()
+    for _ in range(20):
+        rs.run_neural_route(s)
+    n1.record()
+    torch.cuda.synchronize()
+    neural_us = 1e3 * n0.elapsed_time(n1) / 20
+
     if rank == 0:
         peak, peak_src = measured_peaks()
         avg_launch_ms = attn_ms / (K * L)
@@ -425,6 +437,8 @@ def run_ours(args):
             "e2e": {"value": world * e2e_steps / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d // e2e_steps,
                     "d2h_bytes_per_step": d2h // e2e_steps, "steps": e2e_steps},
             "gpu_launches": int(launches),
+            "neural_router": {"us_per_call": neural_us, "params": rs.nr.d * rs.nr.m + 2 * rs.nr.m + 1, "batch": B,
+                              "note": "WhiFlash-Neural policy (d -> d/8 -> GELU -> 1), back-to-back calls, not part of the round"},
             "clocks": clocks,
         }
         if cpu_baseline:

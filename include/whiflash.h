@@ -155,6 +155,24 @@ int wf_lazy_catchup_enqueue(wf_ctx* ctx, wf_drafter* d, const void* hidden, cons
                             int B, int max_rows, void* stream);
 int wf_lazy_catchup_flush(wf_ctx* ctx, wf_drafter* d, const int32_t* flush_mask, int B, void* stream);
 
+/* ---- (f1) WhiFlash-Neural routing policy --------------------------------------------------------
+ * PAPER.md:87 (§3.3.2), :103-107 (decision rule), :325 (App. A architecture); readings N1-N6.
+ * For each sequence b with a non-empty block: h = hidden_final[q_indptr[b] + accept_len[b]] (the target's
+ * final hidden row of the last accepted position), dAL = <w2, GELU(W1 h + b1)> + b2 with the exact (erf)
+ * GELU, route = WF_ROUTE_AR if dAL > tau else WF_ROUTE_DIFFUSION (ties -> diffusion).  An empty block
+ * yields (0, WF_ROUTE_DIFFUSION).
+ * hidden_final: bf16 [sum_q][d]; q_indptr int32 [B+1]; accept_len int32 [B] (device; the output of
+ * wf_accept_entropy_route; NULL = row 0 of every block); w1: bf16 [m][d] (one row per hidden unit,
+ * nn.Linear layout), b1: fp32 [m], w2: bf16 [m], b2: fp32 [1]; tau: fp32 [B] or [1]; delta_al: fp32 [B];
+ * route: int32 [B].  All device pointers, 16-byte aligned; d % 8 == 0, m <= 8192, B <= 1024.
+ * workspace: wf_neural_route_workspace_bytes(B, m) bytes.  bf16 inputs, fp32 accumulation in a fixed order
+ * (deterministic).  Asynchronous on `stream`. */
+size_t wf_neural_route_workspace_bytes(int B, int m);
+int wf_neural_route(wf_ctx* ctx, const void* hidden_final, const int32_t* q_indptr, const int32_t* accept_len,
+                    int B, int d, int m, const void* w1, const float* b1, const void* w2, const float* b2,
+                    const float* tau, int tau_is_scalar, float* delta_al, int32_t* route,
+                    void* workspace, size_t workspace_bytes, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

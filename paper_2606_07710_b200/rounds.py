@@ -92,6 +92,18 @@ class RoundState:
                                    dtype=torch.uint8, device=device)
         self.acc_ws = torch.empty(wf.wf_accept_workspace_bytes(B * self.qmax, sh.vocab), dtype=torch.uint8, device=device)
         self.sm_scale = 1.0 / math.sqrt(sh.head_dim)
+        # ---- WhiFlash-Neural router: d -> d/8 -> 1, seeded random weights ----
+        d, m = sh.hidden, sh.hidden // 8
+        self.nr = Slot()
+        self.nr.d, self.nr.m = d, m
+        self.nr.w1 = synth.device_normal_bf16((m, d), 0.02, wl.seed, 60, device)
+        self.nr.b1 = synth.device_normal_f32((m,), 0.1, wl.seed, 61, device)
+        self.nr.w2 = synth.device_normal_bf16((m,), 0.3, wl.seed, 62, device)
+        self.nr.b2 = torch.full((1,), -0.2, dtype=torch.float32, device=device)
+        self.nr.tau = torch.zeros(1, dtype=torch.float32, device=device)
+        self.nr.delta_al = torch.zeros(B, dtype=torch.float32, device=device)
+        self.nr.route = torch.zeros(B, dtype=torch.int32, device=device)
+        self.nr.ws = torch.empty(wf.wf_neural_route_workspace_bytes(B, m), dtype=torch.uint8, device=device)
         self.rounds_done = 0
         torch.cuda.synchronize()
 
@@ -189,6 +201,13 @@ class RoundState:
         wf.wf_accept_entropy_route(self.ctx, s.logits, self.sh.vocab, s.drafts, s.q_indptr, self.B, self.qmax, self.tau, True,
                                    o["accept_len"], o["bonus_token"], self.entropy, o["route"], o["n_commit"],
                                    self.target_kv, self.acc_ws, stream)
+
+    def run_neural_route(self, s, stream=None):
+        """The learned policy on the final hidden row of the last accepted position (the block's hidden rows stand in
+        for the target's final hidden states); reads accept_len left on the device by run_accept."""
+        n = self.nr
+        wf.wf_neural_route(self.ctx, s.hidden, s.q_indptr, self.out["accept_len"], self.B, n.d, n.m, n.w1, n.b1, n.w2, n.b2,
+                           n.tau, True, n.delta_al, n.route, n.ws, stream)
 
     def run_catchup(self, s, stream=None, lazy=True):
         """Drafter-cache maintenance after the accept: lazy (the paper's scheme) or eager (its baseline)."""
