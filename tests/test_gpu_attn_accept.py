@@ -232,3 +232,43 @@ def test_attn_single_query_and_zero_context(wf):
     """q = 1 (plain decode) and ctx = 0 (the block is the whole sequence)."""
     max_abs, rel = _attn_case(wf, [0, 0, 700], [16, 1, 1], 8, 2, 64, seed=12)
     assert max_abs <= ATTN_MAX_ABS and rel <= ATTN_REL_L2, (max_abs, rel)
+
+
+def test_attn_group_shapes(wf):
+    """GQA group sizes 1 (MHA: 16 rows per kv head), 8 (q = 8 -> 64 rows) and 2, with D = 64 and D = 128."""
+    for (Hq, Hkv, D, q_lens, ctx) in [(4, 4, 64, [16, 3], [300, 77]), (64, 8, 128, [8, 8], [700, 129]),
+                                      (8, 4, 128, [16, 16, 5], [1000, 15, 260])]:
+        max_abs, rel = _attn_case(wf, ctx, q_lens, Hq, Hkv, D, seed=21 + Hq)
+        assert max_abs <= ATTN_MAX_ABS and rel <= ATTN_REL_L2, (Hq, Hkv, D, max_abs, rel)
+
+
+def test_attn_many_short_sequences_with_empty_blocks(wf):
+    """200 sequences with contexts 0..40 and blocks of 0, 1, 8 or 16 rows: far more (sequence, kv head) pairs than CTAs,
+    every range holds many one-tile segments, empty blocks in between (the weighted walker must skip them)."""
+    g = synth.rng(77, 5)
+    ctx = [int(x) for x in g.integers(0, 41, size=200)]
+    q_lens = [int(x) for x in g.choice([0, 1, 8, 16], size=200)]
+    max_abs, rel = _attn_case(wf, ctx, q_lens, 32, 8, 128, seed=31)
+    assert max_abs <= ATTN_MAX_ABS and rel <= ATTN_REL_L2, (max_abs, rel)
+
+
+def test_attn_all_blocks_empty(wf):
+    """B > 0 but nothing to verify: the launch must be a no-op (outputs untouched, no fault, status clean)."""
+    import torch
+    import gpu_harness as H
+    binding, ctx = wf
+    pair = H.make_kv_pair(ctx, [50, 9], [0, 0], 1, 2, 64, seed=3)
+    q = torch.zeros((1, 4, 64), dtype=torch.bfloat16, device="cuda")
+    out = torch.full_like(q, 3.0)
+    ws = torch.empty(binding.wf_verify_attn_workspace_bytes(pair.shape, 2, 4, 1), dtype=torch.uint8, device="cuda")
+    binding.wf_verify_attn(ctx, pair.gpu, 0, q, H.i32([0, 0, 0]), 2, 4, 1, 0.125, out, ws)
+    torch.cuda.synchronize()
+    assert ctx.poll_status() == 0 and float(out.float().min()) == 3.0
+    pair.close()
+
+
+def test_attn_long_single_sequence_many_partials(wf):
+    """One sequence of 70 000 tokens, 2 kv heads: 547 tiles per pair, so a pair is cut into the maximum number of
+    ranges the merge allows (the min-range rule caps the partials per pair)."""
+    max_abs, rel = _attn_case(wf, [70000], [16], 8, 2, 128, seed=41)
+    assert max_abs <= ATTN_MAX_ABS and rel <= ATTN_REL_L2, (max_abs, rel)
