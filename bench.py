@@ -302,7 +302,8 @@ def run_ours(args):
     ctx = wf.Ctx(local)
     K, W = args.steps, max(args.warmup, 3)
     e2e_steps = max(1, min(K, args.e2e_steps))
-    rs = RoundState(ctx, wl, n_slots=4, n_rounds_max=W + K + e2e_steps + 4, host_copies=True)
+    eager_steps = 8
+    rs = RoundState(ctx, wl, n_slots=4, n_rounds_max=W + K + e2e_steps + eager_steps + 4, host_copies=True)
     B, L = rs.B, rs.L
 
     # ---- cpu_baseline + full-size sampled parity (rank 0 of a 1-GPU run only) ----
@@ -429,6 +430,23 @@ def run_ours(args):
     clocks = sampler.stop()
     rs.check_plan(s)
 
+    # ---- the eager baseline of PAPER.md Table 3 at kernel level: both drafters get a KV-only prefill every round
+    #      (no deferral, no flush); same rounds otherwise ----
+    ev_e = [{"attn": (torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)),
+             "catchup": (torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))} for _ in range(eager_steps)]
+    g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    # flush what the lazy rounds left queued, so that the eager appends continue from complete caches
+    for d in rs.drafters.values():
+        wf.wf_lazy_catchup_flush(ctx, d.handle, None, B)
+    torch.cuda.synchronize()
+    g0.record()
+    for i in range(eager_steps):
+        rs.run_round(lazy=False, events=ev_e[i])
+    g1.record()
+    torch.cuda.synchronize()
+    eager_ms = g0.elapsed_time(g1)
+    eager_catch_ms = sum(e["catchup"][0].elapsed_time(e["catchup"][1]) for e in ev_e)
+
     # ---- WhiFlash-Neural router, timed on its own: the round above uses the entropy policy ----
     n0, n1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     for _ in range(3):
@@ -457,6 +475,9 @@ def run_ours(args):
             "kv_read_gbs": achieved,
             "catchup_us_per_round": 1e3 * catch_ms / K,
             "catchup_share_of_round": catch_ms / ms_local,
+            "catchup_eager": {"us_per_round": 1e3 * eager_catch_ms / eager_steps, "share_of_round": eager_catch_ms / eager_ms,
+                              "rounds_per_s": eager_steps / (eager_ms * 1e-3), "steps": eager_steps,
+                              "note": "Lazy Catch-up off (PAPER.md Table 3 baseline): KV-only prefill into both drafters every round"},
             "attn_share_of_round": attn_ms / ms_local,
             "roofline": {"bound": "hbm", "kernel": "wf_verify_attn_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
                          "frac": achieved / peak, "peak_source": peak_src,

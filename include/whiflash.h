@@ -155,6 +155,22 @@ int wf_lazy_catchup_enqueue(wf_ctx* ctx, wf_drafter* d, const void* hidden, cons
                             int B, int max_rows, void* stream);
 int wf_lazy_catchup_flush(wf_ctx* ctx, wf_drafter* d, const int32_t* flush_mask, int B, void* stream);
 
+/* ---- (c) + (d) fused: everything one round asks of a drafter, in ONE projection ---------------------
+ * PAPER.md:117-119.  Per sequence b in [0,B), with idle = idle_mask && idle_mask[b], flush = flush_mask && flush_mask[b]:
+ *   not idle          : the drafter is active for b: its backlog (normally empty) and then rows 0..n_rows[b]-1 of the
+ *                       block are projected and appended (= wf_kv_only_prefill);
+ *   idle and flush    : b switches to this drafter: its backlog and then this round's rows are projected and appended,
+ *                       backlog_len <- 0 (= wf_lazy_catchup_enqueue followed by wf_lazy_catchup_flush, reading C21);
+ *   idle, no flush    : the rows are enqueued (a backlog that would overflow is projected first, C20)
+ *                       (= wf_lazy_catchup_enqueue).
+ * All projected rows of the call share one plan, one operand pack and one projection: a drafter's weights are streamed
+ * once per round instead of up to three times.  A row's K/V bits are those of the separate calls (same device code,
+ * per-row results do not depend on the call that carries them).  idle_mask / flush_mask may be NULL (none idle / none
+ * flushed).  B <= 1024, max_rows <= 64 (and <= backlog_cap when idle_mask is given). */
+int wf_lazy_catchup_round(wf_ctx* ctx, wf_drafter* d, const void* hidden, const int32_t* q_indptr,
+                          const int32_t* n_rows, const int32_t* seq_ids, const int32_t* idle_mask,
+                          const int32_t* flush_mask, int B, int max_rows, void* stream);
+
 /* ---- (f1) WhiFlash-Neural routing policy --------------------------------------------------------
  * PAPER.md:87 (§3.3.2), :103-107 (decision rule), :325 (App. A architecture); readings N1-N6.
  * For each sequence b with a non-empty block: h = hidden_final[q_indptr[b] + accept_len[b]] (the target's

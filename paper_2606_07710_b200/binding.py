@@ -31,7 +31,7 @@ EXPORTS = [
     "wf_accept_entropy_route", "wf_accept_workspace_bytes",
     "wf_drafter_create", "wf_drafter_destroy", "wf_kv_only_prefill",
     "wf_lazy_catchup_enqueue", "wf_lazy_catchup_flush",
-    "wf_neural_route", "wf_neural_route_workspace_bytes",
+    "wf_neural_route", "wf_neural_route_workspace_bytes", "wf_lazy_catchup_round",
 ]
 
 
@@ -66,6 +66,7 @@ _SIG = {
     "wf_kv_only_prefill": (_i, [_vp, _vp, _vp, _vp, _vp, _vp, _i, _i, _vp]),
     "wf_lazy_catchup_enqueue": (_i, [_vp, _vp, _vp, _vp, _vp, _vp, _vp, _i, _i, _vp]),
     "wf_lazy_catchup_flush": (_i, [_vp, _vp, _vp, _i, _vp]),
+    "wf_lazy_catchup_round": (_i, [_vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _i, _i, _vp]),
     "wf_neural_route_workspace_bytes": (_sz, [_i, _i]),
     "wf_neural_route": (_i, [_vp, _vp, _vp, _vp, _i, _i, _i, _vp, _vp, _vp, _vp, _vp, _i, _vp, _vp, _vp, _sz, _vp]),
 }
@@ -212,3 +213,8 @@ def wf_neural_route(ctx, hidden_final, q_indptr, accept_len, B, d, m, w1, b1, w2
     ctx.check(lib.wf_neural_route(ctx.h, _ptr(hidden_final), _ptr(q_indptr), _ptr(accept_len), B, d, m, _ptr(w1), _ptr(b1),
                                   _ptr(w2), _ptr(b2), _ptr(tau), int(tau_is_scalar), _ptr(delta_al), _ptr(route),
                                   _ptr(workspace), workspace.numel() * workspace.element_size(), _stream(stream)))
+
+
+def wf_lazy_catchup_round(ctx, drafter, hidden, q_indptr, n_rows, seq_ids, idle_mask, flush_mask, B, max_rows, stream=None):
+    ctx.check(lib.wf_lazy_catchup_round(ctx.h, drafter.h, _ptr(hidden), _ptr(q_indptr), _ptr(n_rows), _ptr(seq_ids),
+                                        _ptr(idle_mask), _ptr(flush_mask), B, max_rows, _stream(stream)))

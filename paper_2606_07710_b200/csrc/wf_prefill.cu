@@ -42,7 +42,10 @@ struct RowEntry {
 };
 
 // ---- the plan kernel -------------------------------------------------------------------------
-enum PlanMode { PLAN_EAGER = 0, PLAN_FLUSH = 1, PLAN_FORCED = 2 };
+// PLAN_ROUND fuses what one round asks of a drafter into ONE projection: block rows of the sequences it is active for,
+// backlog + block rows of the sequences that switch to it (flush), a forced flush where an enqueue would overflow;
+// the rows of idle sequences are enqueued afterwards (wf_enqueue_round_kernel) at the offsets this plan decides.
+enum PlanMode { PLAN_EAGER = 0, PLAN_FLUSH = 1, PLAN_FORCED = 2, PLAN_ROUND = 3 };
 
 struct PlanParams {
   int mode, B, hidden, cap, max_pos, row_cap;
@@ -50,7 +53,9 @@ struct PlanParams {
   const int32_t* q_indptr;              // EAGER / FORCED
   const int32_t* n_rows;                // EAGER / FORCED
   const int32_t* seq_ids;               // EAGER / FORCED (NULL = identity)
-  const int32_t* mask;                  // FLUSH: flush_mask (NULL = all); FORCED: idle_mask
+  const int32_t* mask;                  // FLUSH: flush_mask (NULL = all); FORCED / ROUND: idle_mask (ROUND: NULL = none idle)
+  const int32_t* mask2;                 // ROUND: flush_mask (NULL = none)
+  int32_t* enq_base;                    // ROUND: [B] backlog offset at which the block rows are enqueued afterwards, -1 = none
   const __nv_bfloat16* backlog;         // [max_seqs][cap][hidden]
   int32_t* backlog_len;
   KvView kv;
@@ -66,6 +71,8 @@ __global__ void __launch_bounds__(1024) wf_prefill_plan_kernel(const PlanParams 
   __shared__ int s_carry;
   // rows / first compact row per sequence: shared memory for the first 1024 sequences, global scratch beyond
   __shared__ int s_pn[KV_RESERVE_SMEM], s_po[KV_RESERVE_SMEM];
+  // ROUND (B <= 1024): backlog rows at the front of b's rows, backlog length after the call, enqueue offset (-1 = none)
+  __shared__ int s_nb[KV_RESERVE_SMEM], s_nl[KV_RESERVE_SMEM], s_eb[KV_RESERVE_SMEM];
   auto plan_n = [&](int b) -> int& { return b < KV_RESERVE_SMEM ? s_pn[b] : p.plan_n[b]; };
   auto plan_off = [&](int b) -> int& { return b < KV_RESERVE_SMEM ? s_po[b] : p.plan_off[b]; };
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5, nw = blockDim.x >> 5;
@@ -76,7 +83,19 @@ __global__ void __launch_bounds__(1024) wf_prefill_plan_kernel(const PlanParams 
   for (int b = tid; b < p.B; b += blockDim.x) {
     const int sq = seq_of(b);
     int n;
-    if (p.mode == PLAN_EAGER) {
+    if (p.mode == PLAN_ROUND) {
+      const int add = p.n_rows[b], len = p.cap > 0 ? p.backlog_len[sq] : 0;
+      const bool idle = p.mask && p.mask[b], fl = p.mask2 && p.mask2[b];
+      const bool project_block = !idle || fl;
+      int n_enq = project_block ? 0 : add;
+      if (n_enq > p.cap) { *p.status = WF_ERR_QUEUE_OVERFLOW; n_enq = 0; }     // rows skipped, as in enqueue
+      // the backlog goes first whenever anything of this sequence is projected (FIFO), or when the enqueue would overflow
+      const int n_back = (project_block || len + n_enq > p.cap) ? len : 0;
+      s_nb[b] = n_back;
+      n = n_back + (project_block ? add : 0);
+      s_eb[b] = n_enq > 0 ? (n_back > 0 ? 0 : len) : -1;
+      s_nl[b] = (n_back > 0 ? 0 : len) + n_enq;
+    } else if (p.mode == PLAN_EAGER) {
       n = p.n_rows[b];
     } else if (p.mode == PLAN_FLUSH) {
       n = (!p.mask || p.mask[b]) ? p.backlog_len[sq] : 0;
@@ -91,8 +110,10 @@ __global__ void __launch_bounds__(1024) wf_prefill_plan_kernel(const PlanParams 
   __syncthreads();
   // pages first (C24: ascending b, consecutive ring entries); nothing is written if they do not fit
   const bool ok = kv_reserve_block(p.kv, p.B, [&](int b) { return plan_n(b); }, seq_of, p.status);
-  if (!ok) {
+  if (!ok) {                                                   // nothing is projected, nothing is enqueued, no length moves
     if (tid == 0) *p.m_total = 0;
+    if (p.mode == PLAN_ROUND)
+      for (int b = tid; b < p.B; b += blockDim.x) p.enq_base[b] = -1;
     return;
   }
   // exclusive scan of plan_n -> plan_off
@@ -132,23 +153,28 @@ __global__ void __launch_bounds__(1024) wf_prefill_plan_kernel(const PlanParams 
     const int sq = seq_of(b);
     const int n = plan_n(b), off = plan_off(b);
     const int p0 = p.kv.seq_len[sq];
-    const __nv_bfloat16* base = p.mode == PLAN_EAGER
-        ? p.hidden_rows + (size_t)p.q_indptr[b] * p.hidden
-        : p.backlog + (size_t)sq * p.cap * p.hidden;
+    const bool from_block = p.mode == PLAN_EAGER || p.mode == PLAN_ROUND;
+    const int n_back = p.mode == PLAN_ROUND ? s_nb[b] : (from_block ? 0 : n);
+    const __nv_bfloat16* blk = from_block ? p.hidden_rows + (size_t)p.q_indptr[b] * p.hidden : nullptr;
+    const __nv_bfloat16* bkl = p.backlog + (size_t)sq * p.cap * p.hidden;
     for (int t = lane; t < n; t += 32) {
       const int pos = p0 + t;
       if (pos >= p.max_pos) *p.status = WF_ERR_INVALID_ARG;
       const int page = p.kv.block_table[(size_t)sq * p.kv.max_pages_per_seq + (pos >> 4)];
       RowEntry e;
-      e.src = base + (size_t)t * p.hidden;
+      e.src = t < n_back ? bkl + (size_t)t * p.hidden : blk + (size_t)(t - n_back) * p.hidden;
       e.pos = min(pos, p.max_pos - 1);
       e.page_slot = page * 16 + (pos & 15);
       p.rows[off + t] = e;
     }
     __syncwarp();
+    if (lane == 0 && p.mode == PLAN_ROUND) {
+      p.enq_base[b] = s_eb[b];
+      if (p.cap > 0) p.backlog_len[sq] = s_nl[b];
+    }
     if (lane == 0 && n > 0) {
       p.kv.seq_len[sq] = p0 + n;
-      if (p.mode != PLAN_EAGER) p.backlog_len[sq] = 0;
+      if (p.mode == PLAN_FLUSH || p.mode == PLAN_FORCED) p.backlog_len[sq] = 0;
     }
   }
   if (tid == 0) *p.m_total = total;
@@ -478,7 +504,7 @@ struct wf_drafter {
   RowEntry* d_rows;
   int row_cap;
   int32_t* d_m_total;
-  int32_t* d_plan;             // [2 * max_seqs]: plan_n, plan_off
+  int32_t* d_plan;             // [3 * max_seqs]: plan_n, plan_off, enq_base
 };
 
 namespace {
@@ -508,7 +534,7 @@ int run_prefill(wf_drafter* d, PlanParams& pp, int rows_upper, cudaStream_t st) 
   pp.backlog = d->backlog; pp.backlog_len = d->backlog_len;
   pp.kv = kv_view(d->kv);
   pp.rows = d->d_rows; pp.m_total = d->d_m_total;
-  pp.plan_n = d->d_plan; pp.plan_off = d->d_plan + d->kv->s.max_seqs;
+  pp.plan_n = d->d_plan; pp.plan_off = d->d_plan + d->kv->s.max_seqs; pp.enq_base = d->d_plan + 2 * d->kv->s.max_seqs;
   pp.status = ctx->d_status;
   wf_launch(wf_prefill_plan_kernel, dim3(1), dim3(1024), 0, st, pp);
   int rc = wf_check_launch(ctx, "wf_prefill_plan_kernel");
@@ -557,7 +583,8 @@ extern "C" int wf_drafter_create(wf_ctx* ctx, const wf_drafter_shape* s, const v
   d->ctx = ctx; d->s = *s; d->kv = kv;
   d->backlog = (const __nv_bfloat16*)backlog; d->backlog_len = backlog_len;
   d->d_wpack = nullptr; d->d_xpack = nullptr; d->d_rope = nullptr; d->d_ws_part = nullptr; d->d_split_cnt = nullptr; d->d_rows = nullptr; d->d_m_total = nullptr; d->d_plan = nullptr;
-  d->row_cap = kv->s.max_seqs * (s->backlog_cap > 64 ? s->backlog_cap : 64);
+  // rows one call can carry: a whole backlog plus a block (64 rows at most) per sequence (wf_lazy_catchup_round)
+  d->row_cap = kv->s.max_seqs * ((s->backlog_cap > 64 ? s->backlog_cap : 64) + 64);
   // Split-K: a call with few tiles (a 1-layer drafter has 16) cannot pull HBM bandwidth through 16 SMs; spread each
   // tile's k-blocks over the largest power of two of CTAs that still fits one CTA per SM.  The factor depends on the
   // drafter's shape only, never on the call, so a row's bits do not depend on M (lazy == eager).
@@ -580,7 +607,7 @@ extern "C" int wf_drafter_create(wf_ctx* ctx, const wf_drafter_shape* s, const v
   if (e == cudaSuccess) e = cudaMalloc(&d->d_rope, sizeof(float2) * rope.size());
   if (e == cudaSuccess) e = cudaMalloc(&d->d_rows, sizeof(RowEntry) * d->row_cap);
   if (e == cudaSuccess) e = cudaMalloc(&d->d_m_total, sizeof(int32_t));
-  if (e == cudaSuccess) e = cudaMalloc(&d->d_plan, sizeof(int32_t) * 2 * kv->s.max_seqs);
+  if (e == cudaSuccess) e = cudaMalloc(&d->d_plan, sizeof(int32_t) * 3 * kv->s.max_seqs);
   if (e == cudaSuccess) {
     for (int l = 0; l < L; ++l)
       for (int v = 0; v < 2; ++v)
@@ -648,6 +675,22 @@ __global__ void wf_enqueue_kernel(const __nv_bfloat16* __restrict__ hidden, cons
   uint4* dst = reinterpret_cast<uint4*>(backlog + ((size_t)sq * cap + backlog_len[sq] + t) * hidden_dim);
   for (int i = threadIdx.x; i < hidden_dim / 8; i += blockDim.x) dst[i] = src[i];
 }
+// ROUND: rows 0..n_rows[b]-1 of each block go to backlog[seq][enq_base[b] + t] (enq_base < 0: nothing to enqueue);
+// the lengths were already advanced by the plan
+__global__ void wf_enqueue_round_kernel(const __nv_bfloat16* __restrict__ hidden, const int32_t* __restrict__ q_indptr,
+                                        const int32_t* __restrict__ n_rows, const int32_t* __restrict__ seq_ids,
+                                        const int32_t* __restrict__ enq_base, __nv_bfloat16* __restrict__ backlog,
+                                        int hidden_dim, int cap) {
+  wf_pdl_trigger();
+  wf_pdl_wait();
+  const int b = blockIdx.y, t = blockIdx.x;
+  const int base = enq_base[b];
+  if (base < 0 || t >= n_rows[b]) return;
+  const int sq = seq_ids ? seq_ids[b] : b;
+  const uint4* src = reinterpret_cast<const uint4*>(hidden + (size_t)(q_indptr[b] + t) * hidden_dim);
+  uint4* dst = reinterpret_cast<uint4*>(backlog + ((size_t)sq * cap + base + t) * hidden_dim);
+  for (int i = threadIdx.x; i < hidden_dim / 8; i += blockDim.x) dst[i] = src[i];
+}
 __global__ void wf_enqueue_len_kernel(const int32_t* __restrict__ n_rows, const int32_t* __restrict__ seq_ids,
                                       const int32_t* __restrict__ idle_mask, int32_t* __restrict__ backlog_len, int B, int cap) {
   wf_pdl_trigger();
@@ -680,4 +723,30 @@ extern "C" int wf_lazy_catchup_enqueue(wf_ctx* ctx, wf_drafter* d, const void* h
   if (rc != WF_OK) return rc;
   wf_launch(wf_enqueue_len_kernel, dim3((B + 255) / 256), dim3(256), 0, st, n_rows, seq_ids, idle_mask, d->backlog_len, B, d->s.backlog_cap);
   return wf_check_launch(ctx, "wf_enqueue_len_kernel");
+}
+
+extern "C" int wf_lazy_catchup_round(wf_ctx* ctx, wf_drafter* d, const void* hidden, const int32_t* q_indptr,
+                                     const int32_t* n_rows, const int32_t* seq_ids, const int32_t* idle_mask,
+                                     const int32_t* flush_mask, int B, int max_rows, void* stream) {
+  if (!ctx || !d) return WF_ERR_INVALID_ARG;
+  WF_REQUIRE(ctx, hidden && q_indptr && n_rows, WF_ERR_INVALID_ARG, "wf_lazy_catchup_round: null argument");
+  WF_REQUIRE(ctx, B >= 0 && B <= d->kv->s.max_seqs && B <= KV_RESERVE_SMEM && max_rows >= 0 && max_rows <= 64, WF_ERR_INVALID_ARG,
+             "wf_lazy_catchup_round: need B <= min(max_seqs, %d) and max_rows <= 64", KV_RESERVE_SMEM);
+  WF_REQUIRE(ctx, !idle_mask || (d->s.backlog_cap > 0 && max_rows <= d->s.backlog_cap), WF_ERR_INVALID_ARG,
+             "wf_lazy_catchup_round: idle sequences need a backlog with max_rows <= backlog_cap");
+  WF_REQUIRE(ctx, (long long)B * (d->s.backlog_cap + max_rows) <= d->row_cap, WF_ERR_INVALID_ARG,
+             "wf_lazy_catchup_round: B * (backlog_cap + max_rows) exceeds the row table (%d)", d->row_cap);
+  WF_REQUIRE(ctx, (uintptr_t)hidden % 16 == 0, WF_ERR_INVALID_ARG, "wf_lazy_catchup_round: hidden must be 16-byte aligned");
+  if (B == 0 || max_rows == 0) return WF_OK;
+  cudaStream_t st = (cudaStream_t)stream;
+  PlanParams pp{};
+  pp.mode = PLAN_ROUND; pp.B = B;
+  pp.hidden_rows = (const __nv_bfloat16*)hidden; pp.q_indptr = q_indptr; pp.n_rows = n_rows; pp.seq_ids = seq_ids;
+  pp.mask = idle_mask; pp.mask2 = flush_mask;
+  int rc = run_prefill(d, pp, B * (d->s.backlog_cap + max_rows), st);
+  if (rc != WF_OK || !idle_mask) return rc;
+  // the projection's operand was packed from the backlog by wf_pack_x_kernel (stream order): the backlog may be overwritten
+  wf_launch(wf_enqueue_round_kernel, dim3(max_rows, B), dim3(128), 0, st, (const __nv_bfloat16*)hidden, q_indptr, n_rows, seq_ids,
+            (const int32_t*)(d->d_plan + 2 * d->kv->s.max_seqs), const_cast<__nv_bfloat16*>(d->backlog), d->s.hidden, d->s.backlog_cap);
+  return wf_check_launch(ctx, "wf_enqueue_round_kernel");
 }

@@ -201,3 +201,66 @@ def test_enqueue_overflow_status(wf):
         binding.wf_lazy_catchup_enqueue(ctx, dp.gpu, H.bits_to_bf16_tensor(X), H.i32([0, 16, 32]), H.i32([9, 1]), None,
                                         H.i32([1, 1]), 2, 16)
     dp.close()
+
+
+@pytest.mark.parametrize("shape", ["tiny", "8b"])
+def test_fused_round_bit_identical_to_eager(wf, shape):
+    """wf_lazy_catchup_round (one projection per drafter per round: active rows, switching sequences' backlog + rows,
+    forced flushes; idle rows enqueued afterwards) over random rounds: backlog lengths follow the enqueue/flush rules
+    (C20, C21) and, after a final flush, the logical cache equals an eager drafter's bit for bit."""
+    import torch
+    import gpu_harness as H
+    binding, ctx = wf
+    L, hidden, Hkv, D = (1, 256, 2, 64) if shape == "tiny" else (5, 4096, 8, 128)
+    S, cap, rounds = 5, 32, 24
+    eager = _mk(ctx, L, hidden, Hkv, D, S, 44, seed=66, cap=cap, shuffled=False)
+    fused = _mk(ctx, L, hidden, Hkv, D, S, 44, seed=66, cap=cap, shuffled=True, weights=eager.weights)
+    start = [70, 0, 15, 33, 128]
+    _start_ctx(eager, start)
+    _start_ctx(fused, start)
+    g = synth.rng(66, 808)
+    q_lens = [16, 8, 16, 8, 16]
+    q_indptr = np.concatenate([[0], np.cumsum(q_lens)]).astype(np.int32)
+    total = np.array(start)
+    blen = np.zeros(S, dtype=np.int64)                       # model of the backlog lengths
+    cached = np.array(start)                                 # model of the fused drafter's cache lengths
+    forced = 0
+    for rnd in range(rounds):
+        X = synth.normal_bf16(g, (int(q_indptr[-1]), hidden), 1.0)
+        n = [int(g.integers(0, q + 1)) for q in q_lens]
+        idle = [int(g.random() < 0.9) for _ in range(S)]
+        flush = [int(i and g.random() < 0.15) for i in idle]
+        if rnd == 5:
+            idle, flush = [0] * S, [0] * S                   # a round with nobody idle: the masks may also be NULL
+        Xg = H.bits_to_bf16_tensor(X)
+        binding.wf_kv_only_prefill(ctx, eager.gpu, Xg, H.i32(q_indptr), H.i32(n), None, S, 16)
+        binding.wf_lazy_catchup_round(ctx, fused.gpu, Xg, H.i32(q_indptr), H.i32(n), None,
+                                      None if rnd == 5 else H.i32(idle), None if rnd == 5 else H.i32(flush), S, 16)
+        for b in range(S):
+            if not idle[b] or flush[b]:
+                cached[b] += blen[b] + n[b]; blen[b] = 0
+            elif blen[b] + n[b] > cap:
+                cached[b] += blen[b]; blen[b] = n[b]; forced += 1
+            else:
+                blen[b] += n[b]
+        total += np.array(n)
+        torch.cuda.synchronize()
+        assert ctx.poll_status() == 0
+        np.testing.assert_array_equal(fused.backlog_len.cpu().numpy(), blen)
+        np.testing.assert_array_equal(fused.kvp.seq_len.cpu().numpy(), cached)
+    assert forced >= 1 and blen.sum() > 0                    # the run exercised a forced flush and ends with rows queued
+    binding.wf_lazy_catchup_flush(ctx, fused.gpu, None, S)
+    torch.cuda.synchronize()
+    assert ctx.poll_status() == 0
+    np.testing.assert_array_equal(fused.kvp.seq_len.cpu().numpy(), total)
+    np.testing.assert_array_equal(eager.kvp.seq_len.cpu().numpy(), total)
+    assert int(fused.backlog_len.sum()) == 0
+    for l in range(L):
+        for b in range(S):
+            n0, n1 = start[b], int(total[b])
+            Ke, Ve = eager.gather_gpu(l, b, n1)
+            Kf, Vf = fused.gather_gpu(l, b, n1)
+            np.testing.assert_array_equal(Ke[n0:], Kf[n0:])
+            np.testing.assert_array_equal(Ve[n0:], Vf[n0:])
+    eager.close()
+    fused.close()
