@@ -470,7 +470,7 @@ def run_ours(args):
             "config": {"workload": wl.name, "batch": B, "ctx": str(wl.ctx), "gammas": list(wl.gammas), "layers": L,
                        "vocab": sh.vocab, "backlog_cap": wl.backlog_cap, "parallelism": "replicas only" if world > 1 else "1 gpu",
                        "l2": f"inputs larger than L2: {np.mean(attn_bytes) / 1e6:.0f} MB of KV per attention launch, distinct per layer",
-                       "catchup": "lazy"},
+                       "catchup": "lazy, one wf_lazy_catchup_round per drafter per round"},
             "committed_tokens_per_s": world * commits * K / (ms * 1e-3),
             "kv_read_gbs": achieved,
             "catchup_us_per_round": 1e3 * catch_ms / K,

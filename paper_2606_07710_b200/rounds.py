@@ -1,9 +1,9 @@
 """Round driver: one verify-and-switch round of the hot path on synthetic, device-resident inputs.
 
     reserve target pages -> 36 x wf_verify_attn -> wf_accept_entropy_route
-      -> active drafter: wf_kv_only_prefill (stands in for its own forward, reading C22)
-      -> idle drafter:   wf_lazy_catchup_enqueue
-      -> switching sequences: wf_lazy_catchup_flush of the incoming drafter (C21)
+      -> per drafter ONE wf_lazy_catchup_round: the sequences it is active for get a KV-only prefill (stands in for
+         its own forward, reading C22), idle sequences are enqueued, sequences that switch to it are flushed
+         together with this round's rows (C21)
 
 Everything is launched on one stream with no host synchronisation inside the round.
 The route trace is seeded and planted in the logits (spike on the row of the last accepted token),
@@ -209,13 +209,19 @@ class RoundState:
         wf.wf_neural_route(self.ctx, s.hidden, s.q_indptr, self.out["accept_len"], self.B, n.d, n.m, n.w1, n.b1, n.w2, n.b2,
                            n.tau, True, n.delta_al, n.route, n.ws, stream)
 
-    def run_catchup(self, s, stream=None, lazy=True):
-        """Drafter-cache maintenance after the accept: lazy (the paper's scheme) or eager (its baseline)."""
+    def run_catchup(self, s, stream=None, lazy=True, fused=True):
+        """Drafter-cache maintenance after the accept: lazy (the paper's scheme) or eager (its baseline).
+        lazy + fused: one wf_lazy_catchup_round per drafter (one projection: active rows, switching sequences' backlog
+        and rows; idle rows are enqueued); lazy + not fused: the three separate calls it is equivalent to."""
         torch, B = self.torch, self.B
         n_commit = self.out["n_commit"]
         for name, d in self.drafters.items():
             m = s.masks[name]
-            if lazy:
+            if lazy and fused:
+                wf.wf_lazy_catchup_round(self.ctx, d.handle, s.hidden, s.q_indptr, n_commit, None,
+                                         m.idle if m.idle_host.any() else None, m.flush if m.flush_host.any() else None,
+                                         B, self.qmax, stream)
+            elif lazy:
                 if m.active_host.any():
                     torch.mul(n_commit, m.active, out=m.n_rows)            # argument marshalling, not the path
                     wf.wf_kv_only_prefill(self.ctx, d.handle, s.hidden, s.q_indptr, m.n_rows, None, B, self.qmax, stream)
@@ -226,7 +232,7 @@ class RoundState:
             else:
                 wf.wf_kv_only_prefill(self.ctx, d.handle, s.hidden, s.q_indptr, n_commit, None, B, self.qmax, stream)
 
-    def run_round(self, stream=None, lazy=True, events=None):
+    def run_round(self, stream=None, lazy=True, events=None, fused=True):
         """One whole round.  events: optional dict of (start, end) CUDA event pairs to record around parts."""
         s = self.slots[self.rounds_done % self.n_slots]
         self.target_kv.reserve(s.add_tokens, self.B, stream)
@@ -238,7 +244,7 @@ class RoundState:
         self.run_accept(s, stream)
         if events:
             events["catchup"][0].record()
-        self.run_catchup(s, stream, lazy)
+        self.run_catchup(s, stream, lazy, fused)
         if events:
             events["catchup"][1].record()
         self.rounds_done += 1
