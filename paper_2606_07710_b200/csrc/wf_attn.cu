@@ -277,12 +277,14 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared& sh
   uint32_t gt0 = 0;                                            // global tile counter at the start of the segment
   while (walk.next(sg)) {
     const int R = sg.q_b * p.group;
+    bool has_next;                                             // this CTA has another segment after this one
     {
       // The NEXT segment's Q rows go to L2 now: under a saturated HBM a cold Q load took 6k cycles at every
       // segment start.  A token's `group` heads are contiguous: group * D * 2 bytes = D / 64 * group lines of 128 B.
       SegWalker peek = walk;
       Segment nx;
-      if (peek.next(nx)) {
+      has_next = peek.next(nx);
+      if (has_next) {
         const int lines_per_tok = p.group * D * 2 / 128;
         const int idx = grp * 128 + stid;
         if (idx < nx.q_b * lines_per_tok) {
@@ -513,14 +515,7 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared& sh
     // the head partial of every CTA is slot 2c; only the first CTA can hold the pair as its tail (slot 2c+1)
     const int first_slot = 2 * c_first + ((int)((long long)c_first * T / G) < sg.flat0 ? 1 : 0);
     const int s_own = (int)blockIdx.x - c_first;
-    for (int s2 = 0; s2 < n_seg; ++s2) {
-      if (s2 == s_own) continue;
-      const int slot = s2 == 0 ? first_slot : 2 * (c_first + s2);
-      const float4* src = p.ws_o + (size_t)slot * (NO / 4) * 128 + stid;
-      float4 x[NO / 4];
-#pragma unroll
-      for (int k = 0; k < NO / 4; ++k) x[k] = __ldcg(src + k * 128);
-      const float4 ml = __ldcg(&p.ws_ml[(size_t)slot * 128 + stid]);
+    auto fold = [&](const float4 (&x)[NO / 4], const float4 ml) {    // (m, l, O) <- (m, l, O) (+) one published partial
       float e0[2], e1[2];
 #pragma unroll
       for (int h = 0; h < 2; ++h) {
@@ -540,6 +535,48 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared& sh
           const int c = 4 * k + u;
           o[c] = o[c] * e0[(c >> 1) & 1] + xv[u] * e1[(c >> 1) & 1];
         }
+      }
+    };
+    auto slot_of = [&](int s2) { return s2 == 0 ? first_slot : 2 * (c_first + s2); };
+    if (!has_next && n_seg > 2) {
+      // Many partials (small launches cut a pair into up to 32 ranges): folding them one load round trip at a time
+      // cost 2.2k cycles each.  This is the CTA's last segment, so its whole shared memory is idle: every thread
+      // copies ITS OWN fragments of up to `cap` partials with cp.async (all in flight together), waits for its
+      // own copies only, and folds them out of shared memory in slot order.
+      constexpr int PART_BYTES = NO * 512 + 2048;              // O fragments + (m, l) of one partial
+      constexpr int cap = C::SMEM / PART_BYTES;
+      const uint32_t base_s = smem_u32(p0_s);
+      for (int s0 = 0; s0 < n_seg; s0 += cap) {
+        const int s1 = min(n_seg, s0 + cap);
+        for (int s2 = s0; s2 < s1; ++s2) {
+          if (s2 == s_own) continue;
+          const int slot = slot_of(s2);
+          const uint32_t dst = base_s + (uint32_t)(s2 - s0) * PART_BYTES + stid * 16;
+          const float4* src = p.ws_o + (size_t)slot * (NO / 4) * 128 + stid;
+#pragma unroll
+          for (int k = 0; k < NO / 4; ++k) cp_async16(dst + k * 2048, src + k * 128);
+          cp_async16(dst + NO * 512, p.ws_ml + (size_t)slot * 128 + stid);
+        }
+        cp_async_commit();
+        cp_async_wait<0>();
+        for (int s2 = s0; s2 < s1; ++s2) {
+          if (s2 == s_own) continue;
+          const float4* lp = reinterpret_cast<const float4*>(p0_s + (size_t)(s2 - s0) * PART_BYTES) + stid;
+          float4 x[NO / 4];
+#pragma unroll
+          for (int k = 0; k < NO / 4; ++k) x[k] = lp[k * 128];
+          fold(x, lp[(NO / 4) * 128]);
+        }
+      }
+    } else {
+      for (int s2 = 0; s2 < n_seg; ++s2) {
+        if (s2 == s_own) continue;
+        const int slot = slot_of(s2);
+        const float4* src = p.ws_o + (size_t)slot * (NO / 4) * 128 + stid;
+        float4 x[NO / 4];
+#pragma unroll
+        for (int k = 0; k < NO / 4; ++k) x[k] = __ldcg(src + k * 128);
+        fold(x, __ldcg(&p.ws_ml[(size_t)slot * 128 + stid]));
       }
     }
     write_rows();
