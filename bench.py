@@ -28,8 +28,8 @@ from paper_2606_07710_b200 import synth  # noqa: E402
 
 WORKLOADS = {"cfg1": 0, "cfg2": 1, "cfg3": 2, "cfg4": 3, "cfg5": 4}
 # dram__bytes_read.sum + dram__bytes_write.sum per attention launch from the committed `ncu --set full` capture
-# (profiles/r1d_ncu_full.md); workloads without a capture report null
-NCU_TRAFFIC_BYTES = {"cfg3": 552.0e6}
+# (profiles/r1e_final_cfg3.md); workloads without a capture report null
+NCU_TRAFFIC_BYTES = {"cfg3": 553.0e6}
 METRIC = "verify_rounds_per_s"
 UNIT = "rounds/s"
 
@@ -482,7 +482,7 @@ def run_ours(args):
             "roofline": {"bound": "hbm", "kernel": "wf_verify_attn_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
                          "frac": achieved / peak, "peak_source": peak_src,
                          "traffic": args.traffic_bytes if args.traffic_bytes is not None else NCU_TRAFFIC_BYTES.get(args.workload),
-                         "traffic_source": "profiles/r1d_ncu_full.md",
+                         "traffic_source": "profiles/r1e_final_cfg3.md",
                          "algorithmic_bytes_per_launch": float(np.mean(attn_bytes)), "avg_launch_us": 1e3 * avg_launch_ms},
             "e2e": {"value": world * e2e_steps / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d // e2e_steps,
                     "d2h_bytes_per_step": d2h // e2e_steps, "steps": e2e_steps,
