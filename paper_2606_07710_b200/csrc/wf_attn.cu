@@ -3,11 +3,15 @@
 //
 // Split-KV, decode-style, tcgen05.  The query tile of a (sequence b, kv head g) pair is all q_b rows of
 // the `group` query heads that share kv head g (<= 64 rows), so K and V are read from HBM once per kv
-// head.  Work is the flattened list of 128-key tiles over all (b, g) pairs; persistent CTA c (one per
-// SM) owns the contiguous tile range [c*T/G, (c+1)*T/G) (stream-K), which every CTA derives from the
-// device-resident lengths (no host sync).  A range cuts at most two (b, g) pairs.  The last CTA to
-// arrive at a shared pair keeps its partial in registers and folds in the partials the others
-// published (fragment-order float4, coalesced); nobody re-reads its own partial.  Warp roles:
+// head.  Work is the flattened list of 128-key tiles over all (b, g) pairs, each pair preceded by
+// AT_SEG_COST positions that stand for the fixed cost of a segment; persistent CTA c (one per SM) owns the
+// contiguous position range [c*T/G, (c+1)*T/G) (cost-weighted stream-K), which every CTA derives from the
+// device-resident lengths through a per-sequence table in shared memory (no host sync, no global round
+// trips in the walkers).  A range cuts at most two (b, g) pairs.  The last CTA to arrive at a shared pair
+// keeps its partial in registers and folds in the partials the others published (fragment-order float4,
+// coalesced; more than two are staged through the idle shared memory with cp.async); nobody re-reads
+// its own partial.  Launched with programmatic dependent launch: barrier init and TMEM allocation run
+// before griddepcontrol.wait.  Warp roles:
 //   warps 8,10: TMA producers (K ring, V ring).  One elected lane issues the 16 page boxes of a tile
 //               (cp.async.bulk.tensor.2d, 128-byte swizzle) in straight-line code; the page ids of the
 //               next tile are prefetched; a K tile is released when its QK^T retires.
@@ -17,7 +21,8 @@
 //               16w..16w+15 on TMEM lanes 32w..32w+15, so warp w owns 16 rows; tcgen05.ld.16x256b hands
 //               them out like an mma C fragment (a quad per row).  Online softmax in the log2 domain
 //               with quad shuffles, P goes to smem as the bf16 A operand of the PV MMA, the per-tile
-//               O_t is folded into fp32 registers with the running rescale.
+//               O_t is folded into fp32 registers with the running rescale.  The next segment's Q rows
+//               are prefetched into L2; the Q tile is loaded with all loads ahead of the stores.
 #include "wf_internal.cuh"
 #include "wf_sm100.cuh"
 

@@ -264,3 +264,29 @@ def test_fused_round_bit_identical_to_eager(wf, shape):
             np.testing.assert_array_equal(Ve[n0:], Vf[n0:])
     eager.close()
     fused.close()
+
+
+def test_fused_round_argument_and_overflow_errors(wf):
+    """wf_lazy_catchup_round: idle sequences on a drafter without a backlog are refused on the host; a block larger than
+    the backlog is refused up front (max_rows <= backlog_cap); a backlog that would overflow is projected first (C20)."""
+    import torch
+    import gpu_harness as H
+    binding, ctx = wf
+    dp = _mk(ctx, 1, 256, 2, 64, 2, 8, seed=9, cap=8)
+    _start_ctx(dp, [3, 5])
+    g = synth.rng(9, 1)
+    X = H.bits_to_bf16_tensor(synth.normal_bf16(g, (32, 256), 1.0))
+    q_indptr = H.i32([0, 16, 32])
+    with pytest.raises(binding.WhiFlashError):                     # max_rows (16) > backlog_cap (8) with idle sequences
+        binding.wf_lazy_catchup_round(ctx, dp.gpu, X, q_indptr, H.i32([1, 1]), None, H.i32([1, 0]), None, 2, 16)
+    # sequence 0 idle: 8 rows fill its backlog exactly; sequence 1 active: 4 rows appended
+    binding.wf_lazy_catchup_round(ctx, dp.gpu, X, q_indptr, H.i32([8, 4]), None, H.i32([1, 0]), None, 2, 8)
+    torch.cuda.synchronize()
+    assert ctx.poll_status() == 0
+    np.testing.assert_array_equal(dp.backlog_len.cpu().numpy(), [8, 0])
+    np.testing.assert_array_equal(dp.kvp.seq_len.cpu().numpy(), [3, 9])
+    binding.wf_lazy_catchup_round(ctx, dp.gpu, X, q_indptr, H.i32([3, 0]), None, H.i32([1, 0]), None, 2, 8)   # 8 + 3 > 8: forced flush
+    torch.cuda.synchronize()
+    np.testing.assert_array_equal(dp.backlog_len.cpu().numpy(), [3, 0])
+    np.testing.assert_array_equal(dp.kvp.seq_len.cpu().numpy(), [11, 9])
+    dp.close()
