@@ -178,6 +178,77 @@ def make_logits_block(g, q_lens, vocab, sigma, accept_prefix, spike):
     return logits, drafts, q_indptr, winners
 
 
+def draw_tree(g, n_nodes, max_depth=8, top_k=10):
+    """Draft-tree shape like the AR drafter's (depth 8, top-k 10, 60 draft tokens): parent int32
+    [n_nodes], parent[0] = -1 (the root = last committed token), nodes in topological order.  Node i >= 1 hangs
+    under a uniformly drawn earlier node that is above the depth limit and has fewer than top_k children."""
+    parent = np.full(n_nodes, -1, dtype=np.int32)
+    depth = np.zeros(n_nodes, dtype=np.int32)
+    kids = np.zeros(n_nodes, dtype=np.int32)
+    for i in range(1, n_nodes):
+        ok = [j for j in range(i) if depth[j] < max_depth and kids[j] < top_k]
+        j = int(ok[g.integers(0, len(ok))])
+        parent[i] = j
+        depth[i] = depth[j] + 1
+        kids[j] += 1
+    return parent
+
+
+def chain_parent(n_nodes):
+    """The chain block as a tree: parent[i] = i - 1."""
+    return np.arange(-1, n_nodes - 1, dtype=np.int32)
+
+
+def make_tree_logits_block(g, parents, vocab, sigma, accept_depth, spike):
+    """Target logits + node tokens for one tree round with a planted outcome.
+
+    parents: list of per-sequence parent arrays.  Rows get planted unique winners as in make_logits_block.
+    For sequence b a downward walk of at most accept_depth[b] steps is drawn from the root; each node on it
+    carries its parent's winner, every other child of a walked node carries a different token (siblings get
+    distinct tokens), and `spike[b]` is added to the winner of the walk's last node.
+
+    Returns logits, tokens (int32 [sum_q]), parent (int32 [sum_q], concatenated), q_indptr, planned paths.
+    """
+    B = len(parents)
+    q_lens = np.array([len(p) for p in parents], dtype=np.int64)
+    q_indptr = np.zeros(B + 1, dtype=np.int32)
+    q_indptr[1:] = np.cumsum(q_lens)
+    n = int(q_indptr[-1])
+    logits = normal_f32(g, (n, vocab), sigma)
+    winners = g.integers(0, vocab, size=n).astype(np.int32)
+    gaps = g.uniform(0.05, 1.0, size=n).astype(np.float32)
+    rows = np.arange(n)
+    logits[rows, winners] = -np.inf
+    logits[rows, winners] = logits.max(axis=1) + gaps
+    tokens = g.integers(0, vocab, size=n).astype(np.int32)
+    paths = []
+    for b in range(B):
+        r0, par = int(q_indptr[b]), parents[b]
+        m = len(par)
+        if m == 0:
+            paths.append([])
+            continue
+        children = [[c for c in range(m) if par[c] == j] for j in range(m)]
+        for j in range(m):                                   # siblings: distinct tokens, none equal to the winner
+            used = {int(winners[r0 + j])}
+            for c in children[j]:
+                t = int(tokens[r0 + c])
+                while t in used:
+                    t = (t + 1) % vocab
+                tokens[r0 + c] = t
+                used.add(t)
+        cur, path = 0, [0]
+        while len(path) - 1 < int(accept_depth[b]) and children[cur]:
+            c = int(children[cur][g.integers(0, len(children[cur]))])
+            tokens[r0 + c] = winners[r0 + cur]
+            cur = c
+            path.append(cur)
+        logits[r0 + cur, winners[r0 + cur]] += np.float32(spike[b])
+        paths.append(path)
+    parent = np.concatenate([np.asarray(p, dtype=np.int32) for p in parents]) if n else np.zeros(0, np.int32)
+    return logits, tokens, parent, q_indptr, paths
+
+
 # ---------------------------------------------------------------------------
 # device-side generators (torch; benchmark-scale tensors)
 # ---------------------------------------------------------------------------
