@@ -189,6 +189,48 @@ int wf_neural_route(wf_ctx* ctx, const void* hidden_final, const int32_t* q_indp
                     const float* tau, int tau_is_scalar, float* delta_al, int32_t* route,
                     void* workspace, size_t workspace_bytes, void* stream);
 
+/* ---- (f2) tree verification: ancestor masks, tree attention, acceptance walk, path compaction -------
+ * PAPER.md:65 ("an autoregressive drafter which produces a tree of candidate tokens ... returned to the
+ * target model for parallel verification"), :39, :317/:327 (depth 8, top-k 10, 60 draft tokens);
+ * DESIGN.md readings T1-T5; SURVEY.md §8(f) f2.
+ * Block layout (T1): row 0 of sequence b's block is the committed root, rows 1..n_b-1 are tree nodes in
+ * topological order: parent[r0_b + i] in [0, i) (an index INSIDE the block), parent[r0_b] = -1, n_b <= 64.
+ * Node i's K/V sit at cache position seq_len[b] + i.  A chain block is parent[i] = i - 1, so one call
+ * serves batches that mix trees and chains.  All pointers are device pointers; every call is asynchronous
+ * on `stream`.
+ *
+ * wf_tree_masks: parent int32 [sum_q] -> tree_mask uint64 [sum_q], bit j of row i set iff node j is i or
+ * an ancestor of i (T2).  Once per round: every layer uses the same masks.  A pointer that breaks T1
+ * raises WF_ERR_INVALID_ARG in the sticky device status (wf_poll_status) and leaves that row its own bit.
+ *
+ * wf_verify_attn_tree: as wf_verify_attn, but row i of sequence b sees keys 0..seq_len[b]-1 and
+ * seq_len[b] + j for the set bits j of tree_mask[r0_b + i].  max_nodes <= 64;
+ * B * ceil(max_nodes * group / 64) <= 1024.  workspace: wf_verify_attn_workspace_bytes(.., max_nodes).
+ *
+ * wf_accept_tree_entropy_route: as wf_accept_entropy_route with the greedy tree walk (T3): from the root,
+ * step to the lowest-index child whose token equals the argmax of the current node's logits, until none
+ * does.  accept_len = steps, bonus_token = argmax at the last node, entropy / route from that node's
+ * logits (T4), n_commit = accept_len + 1, path[b][0..accept_len] = the nodes visited, -1 beyond
+ * (path: int32 [B][path_stride], path_stride >= max_nodes).  The target cache length is NOT advanced:
+ *
+ * wf_kv_compact_path: for every layer of `kv` move the K/V rows of path[b][k] from position
+ * seq_len[b] + path[b][k] to seq_len[b] + k (k = 1..n_commit[b]-1), then seq_len[b] += n_commit[b] (T5).
+ * Rows are moved as if every source were read before any destination is written.  A path entry outside
+ * [k, 64) raises WF_ERR_INVALID_ARG in the sticky device status and moves nothing for that step. */
+int wf_tree_masks(wf_ctx* ctx, const int32_t* parent, const int32_t* q_indptr, int B, int max_nodes,
+                  uint64_t* tree_mask, void* stream);
+int wf_verify_attn_tree(wf_ctx* ctx, const wf_paged_kv* kv, int layer, const void* q, const int32_t* q_indptr,
+                        const uint64_t* tree_mask, int B, int n_q_heads, int max_nodes, float sm_scale,
+                        void* out, void* workspace, size_t workspace_bytes, void* stream);
+int wf_accept_tree_entropy_route(wf_ctx* ctx, const float* logits, int V, const int32_t* node_tokens,
+                                 const int32_t* parent, const int32_t* q_indptr, int B, int max_nodes,
+                                 const float* tau, int tau_is_scalar, int32_t* accept_len,
+                                 int32_t* bonus_token, float* entropy, int32_t* route, int32_t* n_commit,
+                                 int32_t* path, int path_stride, void* workspace, size_t workspace_bytes,
+                                 void* stream);
+int wf_kv_compact_path(wf_paged_kv* kv, const int32_t* path, int path_stride, const int32_t* n_commit, int B,
+                       void* stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -32,6 +32,7 @@ EXPORTS = [
     "wf_drafter_create", "wf_drafter_destroy", "wf_kv_only_prefill",
     "wf_lazy_catchup_enqueue", "wf_lazy_catchup_flush",
     "wf_neural_route", "wf_neural_route_workspace_bytes", "wf_lazy_catchup_round",
+    "wf_tree_masks", "wf_verify_attn_tree", "wf_accept_tree_entropy_route", "wf_kv_compact_path",
 ]
 
 
@@ -69,6 +70,11 @@ _SIG = {
     "wf_lazy_catchup_round": (_i, [_vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _i, _i, _vp]),
     "wf_neural_route_workspace_bytes": (_sz, [_i, _i]),
     "wf_neural_route": (_i, [_vp, _vp, _vp, _vp, _i, _i, _i, _vp, _vp, _vp, _vp, _vp, _i, _vp, _vp, _vp, _sz, _vp]),
+    "wf_tree_masks": (_i, [_vp, _vp, _vp, _i, _i, _vp, _vp]),
+    "wf_verify_attn_tree": (_i, [_vp, _vp, _i, _vp, _vp, _vp, _i, _i, _i, C.c_float, _vp, _vp, _sz, _vp]),
+    "wf_accept_tree_entropy_route": (_i, [_vp, _vp, _i, _vp, _vp, _vp, _i, _i, _vp, _i, _vp, _vp, _vp, _vp, _vp, _vp, _i,
+                                          _vp, _sz, _vp]),
+    "wf_kv_compact_path": (_i, [_vp, _vp, _i, _vp, _i, _vp]),
 }
 for _name, (_res, _args) in _SIG.items():
     _f = getattr(lib, _name)
@@ -218,3 +224,27 @@ def wf_neural_route(ctx, hidden_final, q_indptr, accept_len, B, d, m, w1, b1, w2
 def wf_lazy_catchup_round(ctx, drafter, hidden, q_indptr, n_rows, seq_ids, idle_mask, flush_mask, B, max_rows, stream=None):
     ctx.check(lib.wf_lazy_catchup_round(ctx.h, drafter.h, _ptr(hidden), _ptr(q_indptr), _ptr(n_rows), _ptr(seq_ids),
                                         _ptr(idle_mask), _ptr(flush_mask), B, max_rows, _stream(stream)))
+
+
+def wf_tree_masks(ctx, parent, q_indptr, B, max_nodes, tree_mask, stream=None):
+    ctx.check(lib.wf_tree_masks(ctx.h, _ptr(parent), _ptr(q_indptr), B, max_nodes, _ptr(tree_mask), _stream(stream)))
+
+
+def wf_verify_attn_tree(ctx, kv, layer, q, q_indptr, tree_mask, B, n_q_heads, max_nodes, sm_scale, out, workspace,
+                        stream=None):
+    ctx.check(lib.wf_verify_attn_tree(ctx.h, kv.h, layer, _ptr(q), _ptr(q_indptr), _ptr(tree_mask), B, n_q_heads, max_nodes,
+                                      C.c_float(sm_scale), _ptr(out), _ptr(workspace),
+                                      workspace.numel() * workspace.element_size(), _stream(stream)))
+
+
+def wf_accept_tree_entropy_route(ctx, logits, V, node_tokens, parent, q_indptr, B, max_nodes, tau, tau_is_scalar,
+                                 accept_len, bonus_token, entropy, route, n_commit, path, path_stride, workspace,
+                                 stream=None):
+    ctx.check(lib.wf_accept_tree_entropy_route(
+        ctx.h, _ptr(logits), V, _ptr(node_tokens), _ptr(parent), _ptr(q_indptr), B, max_nodes, _ptr(tau),
+        int(tau_is_scalar), _ptr(accept_len), _ptr(bonus_token), _ptr(entropy), _ptr(route), _ptr(n_commit), _ptr(path),
+        path_stride, _ptr(workspace), workspace.numel() * workspace.element_size(), _stream(stream)))
+
+
+def wf_kv_compact_path(ctx, kv, path, path_stride, n_commit, B, stream=None):
+    ctx.check(lib.wf_kv_compact_path(kv.h, _ptr(path), path_stride, _ptr(n_commit), B, _stream(stream)))

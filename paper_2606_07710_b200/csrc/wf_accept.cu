@@ -40,7 +40,10 @@ wf_accept_kernel(const float* __restrict__ logits, int V, int n_chunks, const in
                  const int32_t* __restrict__ q_indptr, const float* __restrict__ tau, int tau_is_scalar,
                  int32_t* __restrict__ accept_len, int32_t* __restrict__ bonus_token, float* __restrict__ entropy,
                  int32_t* __restrict__ route, int32_t* __restrict__ n_commit, int32_t* __restrict__ kv_seq_len,
-                 AccPartial* __restrict__ partials, unsigned int* __restrict__ counters) {
+                 AccPartial* __restrict__ partials, unsigned int* __restrict__ counters,
+                 const int32_t* __restrict__ parent, int32_t* __restrict__ path, int path_stride) {
+  // parent == nullptr: chain block (C6).  Else tree block (T1-T4): greedy walk over parent pointers, the accepted
+  // node indices go to path[b][0..a] (-1 beyond), and the cache length is left to wf_kv_compact_path.
   wf_pdl_trigger();
   wf_pdl_wait();
   const int b = blockIdx.z, i = blockIdx.y, chunk = blockIdx.x;
@@ -49,6 +52,7 @@ wf_accept_kernel(const float* __restrict__ logits, int V, int n_chunks, const in
   if (q_b == 0 && i == 0 && blockIdx.x == 0 && threadIdx.x == 0) {
     // empty block: nothing verified, nothing committed
     accept_len[b] = 0; bonus_token[b] = 0; entropy[b] = 0.f; route[b] = 0; n_commit[b] = 0;
+    if (path) for (int k = 0; k < path_stride; ++k) path[(size_t)b * path_stride + k] = -1;
   }
   if (i >= q_b) return;                                   // whole CTA exits together
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
@@ -164,17 +168,43 @@ wf_accept_kernel(const float* __restrict__ logits, int V, int n_chunks, const in
     }
     if (lane == 0) s_g[r] = ri;
   }
+  __shared__ int s_row;                                    // the row whose logits give the bonus token and the entropy
+  __shared__ int s_par[ACC_MAX_Q], s_tok[ACC_MAX_Q];
+  if (parent && tid < q_b) { s_par[tid] = parent[r0 + tid]; s_tok[tid] = draft_tokens[r0 + tid]; }
   __syncthreads();
-  if (tid == 0) {                                          // longest accepted prefix (C6)
-    const int gamma = q_b - 1;
-    int a = 0;
-    while (a < gamma && draft_tokens[r0 + a + 1] == s_g[a]) ++a;
-    s_a = a;
+  if (!parent) {
+    if (tid == 0) {                                        // longest accepted prefix (C6)
+      const int gamma = q_b - 1;
+      int a = 0;
+      while (a < gamma && draft_tokens[r0 + a + 1] == s_g[a]) ++a;
+      s_a = a;
+      s_row = a;
+    }
+  } else if (wid == 0) {                                   // greedy walk from the root (T3), one warp
+    int cur = 0, a = 0;
+    int32_t* pb = path ? path + (size_t)b * path_stride : nullptr;
+    if (pb) for (int k = lane; k < path_stride; k += 32) pb[k] = k == 0 ? 0 : -1;
+    __syncwarp();
+    for (;;) {
+      const int g = s_g[cur];
+      int nxt = -1;
+      for (int base = cur + 1; base < q_b && nxt < 0; base += 32) {   // children sit above their parent (T1)
+        const int c = base + lane;
+        const bool hit = c < q_b && s_par[c] == cur && s_tok[c] == g;
+        const unsigned int bal = __ballot_sync(0xffffffffu, hit);
+        if (bal) nxt = base + __ffs(bal) - 1;              // the lowest-index matching child
+      }
+      if (nxt < 0) break;
+      cur = nxt;
+      ++a;
+      if (pb && lane == 0 && a < path_stride) pb[a] = cur;
+    }
+    if (lane == 0) { s_a = a; s_row = cur; }
   }
   __syncthreads();
-  if (wid == 0) {                                          // entropy of row a, fp64 combine (C3, C4)
-    const int a = s_a;
-    const AccPartial* pr = &partials[(size_t)(r0 + a) * n_chunks];
+  if (wid == 0) {                                          // entropy of the last accepted row, fp64 combine (C3, C4, T4)
+    const int a = s_a, row_a = s_row;
+    const AccPartial* pr = &partials[(size_t)(r0 + row_a) * n_chunks];
     float gm = -INFINITY;
     for (int c = lane; c < n_chunks; c += 32) gm = fmaxf(gm, __ldcg(&pr[c].m));
 #pragma unroll
@@ -199,7 +229,7 @@ wf_accept_kernel(const float* __restrict__ logits, int V, int n_chunks, const in
       const float H = (float)(log(Zd) - Sd / Zd);
       const float t = tau_is_scalar ? tau[0] : tau[b];
       accept_len[b] = a;
-      bonus_token[b] = s_g[a];
+      bonus_token[b] = s_g[row_a];
       n_commit[b] = a + 1;
       entropy[b] = H;
       route[b] = (H > t) ? WF_ROUTE_AR : WF_ROUTE_DIFFUSION;     // C1, C2
@@ -216,12 +246,43 @@ extern "C" size_t wf_accept_workspace_bytes(int sum_q, int V) {
   return (size_t)sum_q * n_chunks * sizeof(AccPartial);
 }
 
+namespace {
+int accept_launch(wf_ctx* ctx, const float* logits, int V, const int32_t* draft_tokens, const int32_t* q_indptr, int B,
+                  int max_q_len, const float* tau, int tau_is_scalar, int32_t* accept_len, int32_t* bonus_token,
+                  float* entropy, int32_t* route, int32_t* n_commit, wf_paged_kv* target_kv, void* workspace,
+                  size_t workspace_bytes, void* stream, const int32_t* parent, int32_t* path, int path_stride);
+}
+
 extern "C" int wf_accept_entropy_route(wf_ctx* ctx, const float* logits, int V, const int32_t* draft_tokens,
                                        const int32_t* q_indptr, int B, int max_q_len, const float* tau,
                                        int tau_is_scalar, int32_t* accept_len, int32_t* bonus_token,
                                        float* entropy, int32_t* route, int32_t* n_commit,
                                        wf_paged_kv* target_kv, void* workspace, size_t workspace_bytes,
                                        void* stream) {
+  return accept_launch(ctx, logits, V, draft_tokens, q_indptr, B, max_q_len, tau, tau_is_scalar, accept_len,
+                       bonus_token, entropy, route, n_commit, target_kv, workspace, workspace_bytes, stream, nullptr,
+                       nullptr, 0);
+}
+
+extern "C" int wf_accept_tree_entropy_route(wf_ctx* ctx, const float* logits, int V, const int32_t* node_tokens,
+                                            const int32_t* parent, const int32_t* q_indptr, int B, int max_nodes,
+                                            const float* tau, int tau_is_scalar, int32_t* accept_len,
+                                            int32_t* bonus_token, float* entropy, int32_t* route, int32_t* n_commit,
+                                            int32_t* path, int path_stride, void* workspace, size_t workspace_bytes,
+                                            void* stream) {
+  if (!ctx) return WF_ERR_INVALID_ARG;
+  WF_REQUIRE(ctx, parent && path && path_stride >= 1 && path_stride >= max_nodes, WF_ERR_INVALID_ARG,
+             "wf_accept_tree_entropy_route: parent / path missing or path_stride < max_nodes");
+  return accept_launch(ctx, logits, V, node_tokens, q_indptr, B, max_nodes, tau, tau_is_scalar, accept_len,
+                       bonus_token, entropy, route, n_commit, nullptr, workspace, workspace_bytes, stream, parent, path,
+                       path_stride);
+}
+
+namespace {
+int accept_launch(wf_ctx* ctx, const float* logits, int V, const int32_t* draft_tokens, const int32_t* q_indptr, int B,
+                  int max_q_len, const float* tau, int tau_is_scalar, int32_t* accept_len, int32_t* bonus_token,
+                  float* entropy, int32_t* route, int32_t* n_commit, wf_paged_kv* target_kv, void* workspace,
+                  size_t workspace_bytes, void* stream, const int32_t* parent, int32_t* path, int path_stride) {
   if (!ctx) return WF_ERR_INVALID_ARG;
   WF_REQUIRE(ctx, logits && draft_tokens && q_indptr && tau && accept_len && bonus_token && entropy && route &&
                  n_commit && workspace, WF_ERR_INVALID_ARG, "wf_accept_entropy_route: null argument");
@@ -241,9 +302,12 @@ extern "C" int wf_accept_entropy_route(wf_ctx* ctx, const float* logits, int V, 
   const bool vec = (V % 4 == 0) && ((uintptr_t)logits % 16 == 0);
   if (vec)
     wf_launch(wf_accept_kernel<true>, grid, dim3(ACC_THREADS), 0, st, logits, V, n_chunks, draft_tokens, q_indptr, tau,
-        tau_is_scalar, accept_len, bonus_token, entropy, route, n_commit, kv_len, (AccPartial*)workspace, ctx->d_counters);
+        tau_is_scalar, accept_len, bonus_token, entropy, route, n_commit, kv_len, (AccPartial*)workspace, ctx->d_counters,
+        parent, path, path_stride);
   else
     wf_launch(wf_accept_kernel<false>, grid, dim3(ACC_THREADS), 0, st, logits, V, n_chunks, draft_tokens, q_indptr, tau,
-        tau_is_scalar, accept_len, bonus_token, entropy, route, n_commit, kv_len, (AccPartial*)workspace, ctx->d_counters);
+        tau_is_scalar, accept_len, bonus_token, entropy, route, n_commit, kv_len, (AccPartial*)workspace, ctx->d_counters,
+        parent, path, path_stride);
   return wf_check_launch(ctx, "wf_accept_kernel");
 }
+}  // namespace

@@ -42,6 +42,7 @@ struct AttnParams {
   const __nv_bfloat16* q;
   __nv_bfloat16* out;
   const int32_t* q_indptr;
+  const unsigned long long* tree_mask; // TREE only: [sum_q] ancestor mask of each row (bit j = node j of its sequence)
   KvView kv;
   int layer, B, n_q_heads, group;
   float scale_log2;                    // sm_scale * log2(e)
@@ -65,7 +66,9 @@ struct AttnCfg {
   static constexpr uint32_t TM_S = 0, TM_O = 2 * AT_BN;     // TMEM columns: S0, S1, then O0, O1
 };
 
-// shared state of one CTA (static smem)
+// shared state of one CTA (static smem).  TREE: the table is indexed by SUB-BLOCK (a sequence's tree of up to 64
+// nodes is cut into sub-blocks of 64 / group nodes = one 64-row query tile each), see the kernel prologue.
+template <bool TREE>
 struct AttnShared {
   uint64_t k_full[AT_MAX_STAGES], k_empty[AT_MAX_STAGES], v_full[AT_MAX_STAGES], v_empty[AT_MAX_STAGES];
   uint64_t s_full[2], s_empty[2], o_empty[2], p_full[2], pv_done[2], q_ready;
@@ -73,14 +76,16 @@ struct AttnShared {
   int pref[AT_MAX_B + 1];              // exclusive prefix over the sequences of (tiles per kv head + AT_SEG_COST)
   int r0[AT_MAX_B + 1];                // q_indptr
   int ctx[AT_MAX_B];                   // seq_len
+  int meta[TREE ? AT_MAX_B : 1];       // TREE: nodes in the sub-block | nodes of the tree << 7 | first node << 14 | sequence << 21
   int total_tiles, g_eff, B;
   uint32_t tmem;
   int last;
 };
 
 struct Segment {
-  int b, g, t_lo, t_hi, nt;            // tiles [t_lo, t_hi) of the pair's nt tiles
-  int r0, q_b, ctx, k0, k1, n_tiles;
+  int b, g, t_lo, t_hi, nt;            // tiles [t_lo, t_hi) of the pair's nt tiles; b = sequence (block table row)
+  int pb;                              // table index of the pair (TREE: the sub-block; else b): merge counter
+  int r0, q_b, ctx, k0, k1, n_tiles;   // r0 / q_b: first query row and rows/group of this tile (TREE: of the sub-block)
   int partial, slot;                   // partial: the pair is shared with other CTAs; slot = 2c + (0 head | 1 tail)
   int flat0;                           // weighted position of the pair (its tile t sits at flat0 + AT_SEG_COST + t)
 };
@@ -91,12 +96,13 @@ struct Segment {
 // even when some CTAs get many short pairs (cfg5: 16 five-tile pairs in one range cost twice the average
 // before).  The per-sequence table lives in shared memory (built once in the prologue), so a walk costs no
 // global round trips.
+template <bool TREE>
 struct SegWalker {
-  const AttnShared& sh;
+  const AttnShared<TREE>& sh;
   int Hkv, c;
   int lo, hi, x, b;
   bool first = true;
-  __device__ SegWalker(const AttnShared& sh_, int Hkv_, int c_) : sh(sh_), Hkv(Hkv_), c(c_) {
+  __device__ SegWalker(const AttnShared<TREE>& sh_, int Hkv_, int c_) : sh(sh_), Hkv(Hkv_), c(c_) {
     const int T = sh.total_tiles, G = sh.g_eff;
     lo = (int)((long long)c * T / G);
     hi = (int)((long long)(c + 1) * T / G);
@@ -119,13 +125,22 @@ struct SegWalker {
       const int t_hi = min(nt, hi - wbase - AT_SEG_COST);
       x = t_hi >= nt ? wbase + wlen : hi;                      // the pair is finished, or the range is
       if (t_hi <= t_lo) continue;                              // the range ends inside the cost positions
-      s.b = b; s.nt = nt; s.g = g; s.t_lo = t_lo; s.t_hi = t_hi;
+      s.b = b; s.pb = b; s.nt = nt; s.g = g; s.t_lo = t_lo; s.t_hi = t_hi;
       s.flat0 = wbase;
       s.r0 = sh.r0[b];
-      s.q_b = sh.r0[b + 1] - s.r0;
       s.ctx = sh.ctx[b];
+      int q_tot;
+      if constexpr (TREE) {
+        const int meta = sh.meta[b];
+        s.q_b = meta & 127;
+        q_tot = (meta >> 7) & 127;
+        s.b = meta >> 21;
+      } else {
+        s.q_b = sh.r0[b + 1] - s.r0;
+        q_tot = s.q_b;
+      }
       s.k0 = t_lo * AT_BN;
-      s.k1 = min(s.ctx + s.q_b, t_hi * AT_BN);
+      s.k1 = min(s.ctx + q_tot, t_hi * AT_BN);
       s.n_tiles = t_hi - t_lo;
       s.partial = !(t_lo == 0 && t_hi == nt);
       s.slot = 2 * c + (first ? 0 : 1);
@@ -145,13 +160,13 @@ __device__ __forceinline__ int cta_of_tile(int x, int T, int G) {      // larges
 
 // ================= warps 8 (K) and 10 (V): TMA producers =================
 // K and V have separate rings so that a K tile is released as soon as its QK^T retires: more bytes in flight.
-template <int D>
-__device__ __forceinline__ void attn_loader(const AttnParams& p, AttnShared& sh, uint8_t* ring, int which, int lane) {
+template <int D, bool TREE>
+__device__ __forceinline__ void attn_loader(const AttnParams& p, AttnShared<TREE>& sh, uint8_t* ring, int which, int lane) {
   using C = AttnCfg<D>;
   const KvView& kv = p.kv;
   uint64_t* full = which ? sh.v_full : sh.k_full;
   uint64_t* empty = which ? sh.v_empty : sh.k_empty;
-  SegWalker walk(sh, p.kv.n_kv_heads, blockIdx.x);
+  SegWalker<TREE> walk(sh, p.kv.n_kv_heads, blockIdx.x);
   Segment sg;
   uint32_t gt = 0;
   constexpr int PP = AT_BN / 16;                              // pages per tile
@@ -193,8 +208,8 @@ __device__ __forceinline__ void attn_loader(const AttnParams& p, AttnShared& sh,
 // Tile g2 (global tile counter) belongs to softmax group g2 & 1, which owns S[g2&1], P[g2&1], O[g2&1].
 // The whole warp runs the loop so that addresses and descriptors stay warp-uniform; one elected lane
 // issues the tcgen05 instructions.  Descriptors are built once and advanced by constant offsets.
-template <int D>
-__device__ __forceinline__ void attn_mma(const AttnParams& p, AttnShared& sh, uint8_t* q_s, uint8_t* p0_s, uint8_t* p1_s,
+template <int D, bool TREE>
+__device__ __forceinline__ void attn_mma(const AttnParams& p, AttnShared<TREE>& sh, uint8_t* q_s, uint8_t* p0_s, uint8_t* p1_s,
                                          uint8_t* k_s, uint8_t* v_s, uint32_t tmem_base) {
   using C = AttnCfg<D>;
   const uint32_t idesc_qk = umma_idesc_kk(AT_ROWS, AT_BN);
@@ -204,7 +219,7 @@ __device__ __forceinline__ void attn_mma(const AttnParams& p, AttnShared& sh, ui
   const uint64_t dp0 = umma_desc(smem_u32(p0_s), 16, 1024);                 // K-major
   const uint64_t dp1 = umma_desc(smem_u32(p1_s), 16, 1024);
   const uint64_t dv0 = umma_desc(smem_u32(v_s), C::KV_HALF, 1024);          // MN-major
-  SegWalker walk(sh, p.kv.n_kv_heads, blockIdx.x);
+  SegWalker<TREE> walk(sh, p.kv.n_kv_heads, blockIdx.x);
   Segment sg;
   uint32_t gt = 0, n_seg = 0;
   auto issue_qk = [&](uint32_t g2) {
@@ -263,8 +278,8 @@ __device__ __forceinline__ void tmem_ld_frag(uint32_t taddr, uint32_t (&v)[N]) {
 // ================= warps 0-3 (group 0) and 4-7 (group 1): softmax, O accumulation, output, merges =================
 // The two groups ping-pong over the tiles: group g takes the tiles whose global counter has parity g and
 // keeps its own running (m, l, O); at the end of a segment group 1 hands its state to group 0 through smem.
-template <int D>
-__device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared& sh, uint8_t* q_s, uint8_t* p0_s, uint8_t* p1_s,
+template <int D, bool TREE>
+__device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared<TREE>& sh, uint8_t* q_s, uint8_t* p0_s, uint8_t* p1_s,
                                              uint8_t* v_s, uint32_t tmem_base, int warp, int lane) {
   using C = AttnCfg<D>;
   constexpr int NO = D / 2;                                    // O registers per thread (2 rows x D/4 columns)
@@ -277,7 +292,7 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared& sh
   uint8_t* p_s = grp ? p1_s : p0_s;
   float* xch = reinterpret_cast<float*>(q_s);                  // [NO][128] group-merge buffer (Q + P1 regions)
   const int T = sh.total_tiles, G = sh.g_eff;
-  SegWalker walk(sh, p.kv.n_kv_heads, blockIdx.x);
+  SegWalker<TREE> walk(sh, p.kv.n_kv_heads, blockIdx.x);
   Segment sg;
   uint32_t gt0 = 0;                                            // global tile counter at the start of the segment
   while (walk.next(sg)) {
@@ -286,7 +301,7 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared& sh
     {
       // The NEXT segment's Q rows go to L2 now: under a saturated HBM a cold Q load took 6k cycles at every
       // segment start.  A token's `group` heads are contiguous: group * D * 2 bytes = D / 64 * group lines of 128 B.
-      SegWalker peek = walk;
+      SegWalker<TREE> peek = walk;
       Segment nx;
       has_next = peek.next(nx);
       if (has_next) {
@@ -332,6 +347,16 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared& sh
     int lim[2];                                                // keys j < lim[h] are visible to row (row_lo + 8h)
     lim[0] = min(sg.k1, sg.ctx + row_lo / p.group + 1);
     lim[1] = min(sg.k1, sg.ctx + (row_lo + 8) / p.group + 1);
+    // TREE: keys below ctx are visible to every row; key ctx + j only if bit j of the row's ancestor mask is set
+    // (the row's own bit is always set, so a live row sees at least one key).  Padding rows see the context only.
+    unsigned long long anc[2] = {0ull, 0ull};
+    if constexpr (TREE) {
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        const int node = (row_lo + 8 * h) / p.group;
+        if (node < sg.q_b) anc[h] = __ldg(p.tree_mask + sg.r0 + node);
+      }
+    }
 
     auto fold_o = [&]() {                                      // o = o * alpha_prev + O_tile (this group's buffer)
       uint32_t v[NO];
@@ -357,7 +382,17 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared& sh
       tc_fence_before();
       mbar_arrive(smem_u32(&sh.s_empty[grp]));                 // S buffer may be overwritten by QK(g2 + 2)
 
-      if (tk0 + AT_BN > min(sg.ctx + 1, sg.k1)) {              // causal / tail mask
+      if constexpr (TREE) {
+        if (tk0 + AT_BN > sg.ctx) {                            // the tile holds tree keys (or the tail beyond them)
+          const int rel0 = tk0 + cq - sg.ctx;                  // key of element c, relative to the first tree key
+#pragma unroll
+          for (int c = 0; c < 64; ++c) {
+            const int rel = rel0 + (c >> 2) * 8 + (c & 1);
+            const bool vis = rel < 0 || (rel < 64 && ((anc[(c >> 1) & 1] >> (rel & 63)) & 1ull));
+            if (!vis) sv[c] = 0xff800000u;                     // -inf
+          }
+        }
+      } else if (tk0 + AT_BN > min(sg.ctx + 1, sg.k1)) {       // causal / tail mask
 #pragma unroll
         for (int c = 0; c < 64; ++c) {
           const int j = tk0 + (c >> 2) * 8 + cq + (c & 1);
@@ -437,7 +472,7 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared& sh
     if (sg.partial && grp == 0) {
       c_first = cta_of_tile(sg.flat0 + AT_SEG_COST, T, G);
       n_seg = cta_of_tile(sg.flat0 + AT_SEG_COST + sg.nt - 1, T, G) - c_first + 1;
-      if (stid == 0) arrive_old = atomicAdd(&p.counters[sg.b * Hkv + sg.g], 1u);
+      if (stid == 0) arrive_old = atomicAdd(&p.counters[sg.pb * Hkv + sg.g], 1u);
     }
 
     // ---- group 1 hands (m, l, O) to group 0 through smem (Q and P1 are idle: every MMA has retired) ----
@@ -494,7 +529,7 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared& sh
     //      partial in fragment order (thread-major float4: coalesced for writer and reader alike).
     //      In steady state the last arriver is the CTA that holds the pair's head at the end of its range,
     //      and the others published long ago. ----
-    unsigned int* cnt = p.counters + sg.b * Hkv + sg.g;
+    unsigned int* cnt = p.counters + sg.pb * Hkv + sg.g;
     if (stid == 0) sh.last = (arrive_old & 0xffffu) == (unsigned int)n_seg - 1 ? 1 + (int)(arrive_old >> 16) : 0;
     named_bar_sync(3, 128);
     const int last = sh.last;                                  // 0: not last; else 1 + partials already published
@@ -588,11 +623,11 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared& sh
   }
 }
 
-template <int D>
+template <int D, bool TREE>
 __global__ void __launch_bounds__(AT_THREADS, 1) wf_verify_attn_kernel(const AttnParams p) {
   using C = AttnCfg<D>;
   extern __shared__ __align__(1024) uint8_t smem[];
-  __shared__ __align__(8) AttnShared sh;
+  __shared__ __align__(8) AttnShared<TREE> sh;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   uint8_t* p0_s = smem;                                        // smem map: P0 | Q | P1 | K ring | V ring
   uint8_t* q_s = p0_s + C::P_BYTES;
@@ -622,21 +657,63 @@ __global__ void __launch_bounds__(AT_THREADS, 1) wf_verify_attn_kernel(const Att
   wf_pdl_wait();
   // per-sequence table (tiles per kv head, q_indptr, context) from the device-resident lengths, identical in
   // every CTA; then total tiles and the longest pair
+  // TREE: the per-sequence values go to the (still idle) dynamic shared memory first; warp 0 then expands them
+  // into the sub-block table below.
+  int* t_r0 = reinterpret_cast<int*>(smem);
+  int* t_ctx = t_r0 + AT_MAX_B;
+  int* t_q = t_ctx + AT_MAX_B;
   for (int b = tid; b < p.B; b += AT_THREADS) {
     const int r0 = p.q_indptr[b], r1 = p.q_indptr[b + 1], ctx = p.kv.seq_len[b];
-    sh.r0[b] = r0;
-    sh.ctx[b] = ctx;
-    sh.pref[b + 1] = r1 > r0 ? (ctx + (r1 - r0) + AT_BN - 1) / AT_BN + AT_SEG_COST : 0;
-    if (b == p.B - 1) sh.r0[p.B] = r1;
+    if constexpr (TREE) {
+      t_r0[b] = r0;
+      t_ctx[b] = ctx;
+      t_q[b] = min(r1 - r0, 64);
+    } else {
+      sh.r0[b] = r0;
+      sh.ctx[b] = ctx;
+      sh.pref[b + 1] = r1 > r0 ? (ctx + (r1 - r0) + AT_BN - 1) / AT_BN + AT_SEG_COST : 0;
+      if (b == p.B - 1) sh.r0[p.B] = r1;
+    }
   }
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = sh.tmem;
   if (warp == 0) {                                             // in-place scan of the tile counts, 32 sequences per step
+    int n_tab = p.B;                                           // table entries
+    if constexpr (TREE) {
+      // Sub-block s of sequence b = nodes [s * npt, (s+1) * npt), npt = 64 / group nodes = one query tile.  Each
+      // sub-block is a pair of its own that streams the sequence's whole KV; the table lists them LEVEL-MAJOR
+      // (all first sub-blocks, then all second ones, ...): with equal trees the level copies of a (b, g) pair
+      // sit T / levels positions apart, i.e. in CTAs c, c + G / levels, ... at the same offset of their ranges,
+      // which stream the same K/V tiles at the same time: HBM serves one of them, L2 the rest.
+      const int npt = AT_ROWS / p.group;
+      int cursor = 0;
+      for (int s0 = 0; s0 < 64; s0 += npt) {
+        const int before = cursor;
+        for (int base = 0; base < p.B; base += 32) {
+          const int b = base + lane;
+          const int q = b < p.B ? t_q[b] : 0;
+          const bool on = q > s0;
+          const unsigned int bal = __ballot_sync(0xffffffffu, on);
+          const int idx = cursor + __popc(bal & ((1u << lane) - 1u));
+          if (on && idx < AT_MAX_B) {
+            const int ctx = t_ctx[b];
+            sh.r0[idx] = t_r0[b] + s0;
+            sh.ctx[idx] = ctx;
+            sh.meta[idx] = min(npt, q - s0) | (q << 7) | (s0 << 14) | (b << 21);
+            sh.pref[idx + 1] = (ctx + q + AT_BN - 1) / AT_BN + AT_SEG_COST;
+          }
+          cursor += __popc(bal);
+        }
+        if (cursor == before) break;                           // no tree is this large
+      }
+      n_tab = min(cursor, AT_MAX_B);
+      __syncwarp();
+    }
     int run = 0, lg = 0, live = 0;
-    for (int base = 0; base < p.B; base += 32) {
-      const int n = base + lane < p.B ? sh.pref[base + lane + 1] : 0;
+    for (int base = 0; base < n_tab; base += 32) {
+      const int n = base + lane < n_tab ? sh.pref[base + lane + 1] : 0;
       lg = max(lg, n);
       live += n > 0;
       int v = n;
@@ -645,7 +722,7 @@ __global__ void __launch_bounds__(AT_THREADS, 1) wf_verify_attn_kernel(const Att
         const int y = __shfl_up_sync(0xffffffffu, v, d);
         if (lane >= d) v += y;
       }
-      if (base + lane < p.B) sh.pref[base + lane + 1] = run + v;
+      if (base + lane < n_tab) sh.pref[base + lane + 1] = run + v;
       run += __shfl_sync(0xffffffffu, v, 31);
     }
 #pragma unroll
@@ -671,7 +748,7 @@ __global__ void __launch_bounds__(AT_THREADS, 1) wf_verify_attn_kernel(const Att
         G = min(G, n * pairs);
       }
       sh.g_eff = max(1, min(G, total / min_range));
-      sh.B = p.B;
+      sh.B = n_tab;
     }
   }
   __syncthreads();
@@ -679,12 +756,12 @@ __global__ void __launch_bounds__(AT_THREADS, 1) wf_verify_attn_kernel(const Att
   if (sh.total_tiles > 0 && (int)blockIdx.x < sh.g_eff) {
     if (warp < 8) {
       asm volatile("setmaxnreg.inc.sync.aligned.u32 216;");
-      attn_softmax<D>(p, sh, q_s, p0_s, p1_s, v_s, tmem_base, warp, lane);
+      attn_softmax<D, TREE>(p, sh, q_s, p0_s, p1_s, v_s, tmem_base, warp, lane);
     } else {
       asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
-      if (warp == 8) attn_loader<D>(p, sh, k_s, 0, lane);
-      else if (warp == 10) attn_loader<D>(p, sh, v_s, 1, lane);
-      else if (warp == 9) attn_mma<D>(p, sh, q_s, p0_s, p1_s, k_s, v_s, tmem_base);
+      if (warp == 8) attn_loader<D, TREE>(p, sh, k_s, 0, lane);
+      else if (warp == 10) attn_loader<D, TREE>(p, sh, v_s, 1, lane);
+      else if (warp == 9) attn_mma<D, TREE>(p, sh, q_s, p0_s, p1_s, k_s, v_s, tmem_base);
     }
   }
   tc_fence_before();
@@ -699,17 +776,42 @@ __global__ void __launch_bounds__(AT_THREADS, 1) wf_verify_attn_kernel(const Att
 // ------------------------------------------------------------------------------------------------
 namespace {
 
-template <int D>
+template <int D, bool TREE>
 int launch_attn(wf_ctx* ctx, const AttnParams& p, cudaStream_t st) {
   static bool configured = false;
   const size_t smem = AttnCfg<D>::SMEM;
   if (!configured) {
-    WF_CUDA(ctx, cudaFuncSetAttribute(wf_verify_attn_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    WF_CUDA(ctx, cudaFuncSetAttribute(wf_verify_attn_kernel<D, TREE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     configured = true;
   }
   const int grid = ctx->sm_count < AT_MAX_CTAS ? ctx->sm_count : AT_MAX_CTAS;   // one persistent CTA per SM
-  wf_launch(wf_verify_attn_kernel<D>, dim3(grid), dim3(AT_THREADS), smem, st, p);
-  return wf_check_launch(ctx, "wf_verify_attn_kernel");
+  wf_launch(wf_verify_attn_kernel<D, TREE>, dim3(grid), dim3(AT_THREADS), smem, st, p);
+  return wf_check_launch(ctx, TREE ? "wf_verify_attn_kernel<tree>" : "wf_verify_attn_kernel");
+}
+
+// One thread per tree node walks its parent pointers (staged in shared memory) up to the root and ORs the bits.
+// A node whose pointers do not lead to the root through strictly decreasing indices (reading T1) raises
+// WF_ERR_INVALID_ARG in the sticky status word and keeps only its own bit.
+__global__ void __launch_bounds__(64) wf_tree_masks_kernel(const int32_t* parent, const int32_t* q_indptr,
+                                                           unsigned long long* mask, int* status) {
+  __shared__ int par[64];
+  wf_pdl_trigger();
+  wf_pdl_wait();
+  const int b = blockIdx.x, i = threadIdx.x;
+  const int r0 = q_indptr[b], n = min(q_indptr[b + 1] - r0, 64);
+  if (i < n) par[i] = parent[r0 + i];
+  __syncthreads();
+  if (i >= n) return;
+  unsigned long long m = 1ull << i;
+  bool bad = i == 0 && par[0] != -1;
+  for (int j = i; j > 0;) {
+    const int pj = par[j];
+    if (pj < 0 || pj >= j) { bad = true; m = 1ull << i; break; }
+    j = pj;
+    m |= 1ull << j;
+  }
+  if (bad) atomicCAS(status, 0, (int)WF_ERR_INVALID_ARG);
+  mask[r0 + i] = m;
 }
 
 }  // namespace
@@ -753,7 +855,60 @@ extern "C" int wf_verify_attn(wf_ctx* ctx, const wf_paged_kv* kv, int layer, con
   p.counters = ctx->d_counters_attn;
   cudaStream_t st = (cudaStream_t)stream;
   const int D = kv->s.head_dim;
-  if (D == 128) return launch_attn<128>(ctx, p, st);
-  if (D == 64) return launch_attn<64>(ctx, p, st);
+  p.tree_mask = nullptr;
+  if (D == 128) return launch_attn<128, false>(ctx, p, st);
+  if (D == 64) return launch_attn<64, false>(ctx, p, st);
   return wf_set_error(ctx, WF_ERR_UNSUPPORTED_SHAPE, "wf_verify_attn: head_dim %d unsupported", D);
+}
+
+extern "C" int wf_tree_masks(wf_ctx* ctx, const int32_t* parent, const int32_t* q_indptr, int B, int max_nodes,
+                             uint64_t* tree_mask, void* stream) {
+  if (!ctx) return WF_ERR_INVALID_ARG;
+  WF_REQUIRE(ctx, parent && q_indptr && tree_mask && B >= 0, WF_ERR_INVALID_ARG, "wf_tree_masks: bad argument");
+  WF_REQUIRE(ctx, max_nodes >= 1 && max_nodes <= 64, WF_ERR_UNSUPPORTED_SHAPE, "wf_tree_masks: max_nodes must be in [1, 64]");
+  if (B == 0) return WF_OK;
+  wf_launch(wf_tree_masks_kernel, dim3(B), dim3(64), 0, (cudaStream_t)stream, parent, q_indptr,
+            (unsigned long long*)tree_mask, ctx->d_status);
+  return wf_check_launch(ctx, "wf_tree_masks_kernel");
+}
+
+extern "C" int wf_verify_attn_tree(wf_ctx* ctx, const wf_paged_kv* kv, int layer, const void* q, const int32_t* q_indptr,
+                                   const uint64_t* tree_mask, int B, int n_q_heads, int max_nodes, float sm_scale,
+                                   void* out, void* workspace, size_t workspace_bytes, void* stream) {
+  if (!ctx) return WF_ERR_INVALID_ARG;
+  WF_REQUIRE(ctx, kv && q && q_indptr && tree_mask && out && workspace, WF_ERR_INVALID_ARG, "wf_verify_attn_tree: null argument");
+  WF_REQUIRE(ctx, layer >= 0 && layer < kv->s.n_layers, WF_ERR_INVALID_ARG, "wf_verify_attn_tree: bad layer");
+  WF_REQUIRE(ctx, n_q_heads > 0 && n_q_heads % kv->s.n_kv_heads == 0, WF_ERR_INVALID_ARG,
+             "wf_verify_attn_tree: n_q_heads must be a multiple of n_kv_heads");
+  const int group = n_q_heads / kv->s.n_kv_heads;
+  WF_REQUIRE(ctx, group <= 64 && max_nodes >= 1 && max_nodes <= 64, WF_ERR_UNSUPPORTED_SHAPE,
+             "wf_verify_attn_tree: max_nodes must be in [1, 64] and the GQA group <= 64");
+  const int npt = AT_ROWS / group;                           // nodes per 64-row query tile
+  const int levels = (max_nodes + npt - 1) / npt;            // sub-blocks per tree
+  WF_REQUIRE(ctx, B >= 0 && B <= kv->s.max_seqs && (long long)B * levels <= AT_MAX_B &&
+                      (long long)B * levels * kv->s.n_kv_heads <= ctx->n_counters,
+             WF_ERR_INVALID_ARG, "wf_verify_attn_tree: B * ceil(max_nodes * group / 64) must be <= %d", AT_MAX_B);
+  WF_REQUIRE(ctx, workspace_bytes >= wf_verify_attn_workspace_bytes(&kv->s, B, n_q_heads, max_nodes),
+             WF_ERR_INVALID_ARG, "wf_verify_attn_tree: workspace too small");
+  WF_REQUIRE(ctx, ((uintptr_t)q % 16 == 0) && ((uintptr_t)out % 16 == 0) && ((uintptr_t)workspace % 16 == 0) &&
+                      ((uintptr_t)tree_mask % 8 == 0),
+             WF_ERR_INVALID_ARG, "wf_verify_attn_tree: q/out/workspace must be 16-byte aligned");
+  if (B == 0) return WF_OK;
+  const size_t items = 2 * (size_t)AT_MAX_CTAS;
+  AttnParams p;
+  p.q = (const __nv_bfloat16*)q;
+  p.out = (__nv_bfloat16*)out;
+  p.q_indptr = q_indptr;
+  p.tree_mask = (const unsigned long long*)tree_mask;
+  p.kv = kv_view(kv);
+  p.layer = layer; p.B = B; p.n_q_heads = n_q_heads; p.group = group;
+  p.scale_log2 = sm_scale * LOG2E;
+  p.ws_o = (float4*)workspace;
+  p.ws_ml = (float4*)((char*)workspace + items * AT_ROWS * kv->s.head_dim * sizeof(float));
+  p.counters = ctx->d_counters_attn;
+  cudaStream_t st = (cudaStream_t)stream;
+  const int D = kv->s.head_dim;
+  if (D == 128) return launch_attn<128, true>(ctx, p, st);
+  if (D == 64) return launch_attn<64, true>(ctx, p, st);
+  return wf_set_error(ctx, WF_ERR_UNSUPPORTED_SHAPE, "wf_verify_attn_tree: head_dim %d unsupported", D);
 }

@@ -220,3 +220,75 @@ extern "C" int wf_kv_release_seq(wf_paged_kv* kv, int seq, void* stream) {
   wf_launch(wf_kv_release_kernel, dim3(1), dim3(256), 0, (cudaStream_t)stream, kv_view(kv), seq);
   return wf_check_launch(ctx, "wf_kv_release_seq");
 }
+
+// ---------------------------------------------------------------------------------------------
+// Tree verification, step 3: path compaction (reading T5).  One CTA per (sequence, layer).
+// A thread owns one 16-byte column (K or V, kv head, 8 elements) of the rows and moves it for every
+// step k of the path: position ctx + path[k] -> ctx + k.  The only overlap between the moves is a
+// destination that is another step's source, always in the same column, i.e. in the same thread:
+// it reads a batch of 8 sources before it writes the batch, and batches ascend (path[j] > j, so a
+// later source is never an earlier destination).  No barrier, no second buffer.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) wf_kv_compact_path_kernel(KvView kv, const int32_t* __restrict__ path,
+                                                                 int path_stride, const int32_t* __restrict__ n_commit,
+                                                                 int* status) {
+  __shared__ int s_src[64], s_dst[64];                      // row index in the pool's [page][head][slot] order, head 0
+  wf_pdl_trigger();
+  wf_pdl_wait();
+  const int b = blockIdx.x, layer = blockIdx.y;
+  const int nc = min(n_commit[b], 64);
+  if (nc <= 1) return;                                      // the root is in place
+  const int ctx = kv.seq_len[b];
+  const int32_t* bt = kv.block_table + (size_t)b * kv.max_pages_per_seq;
+  if (threadIdx.x < nc) {
+    const int k = threadIdx.x;
+    const int node = path[(size_t)b * path_stride + k];
+    const bool ok = node >= k && node < 64 && (ctx + node) / 16 < kv.max_pages_per_seq;
+    if (!ok && layer == 0) atomicCAS(status, 0, (int)WF_ERR_INVALID_ARG);
+    const int ps = ok ? ctx + node : ctx + k, pd = ctx + k;
+    s_src[k] = (bt[ps >> 4] * kv.n_kv_heads) * 16 + (ps & 15);
+    s_dst[k] = (bt[pd >> 4] * kv.n_kv_heads) * 16 + (pd & 15);
+  }
+  __syncthreads();
+  const int cpr = kv.head_dim / 8;                          // 16-byte chunks per row
+  const int cols = 2 * kv.n_kv_heads * cpr;
+  const size_t layer_rows = (size_t)layer * kv.num_pages * kv.n_kv_heads * 16;
+  for (int col = threadIdx.x; col < cols; col += blockDim.x) {
+    const int which = col / (kv.n_kv_heads * cpr), rem = col % (kv.n_kv_heads * cpr);
+    const int head = rem / cpr, chunk = rem % cpr;
+    uint4* pool = reinterpret_cast<uint4*>(which ? kv.v_pool : kv.k_pool);
+    auto at = [&](int row0) { return pool + (layer_rows + (size_t)row0 + (size_t)head * 16) * cpr + chunk; };
+    for (int k0 = 1; k0 < nc; k0 += 8) {
+      uint4 x[8];
+#pragma unroll
+      for (int u = 0; u < 8; ++u)
+        if (k0 + u < nc) x[u] = *at(s_src[k0 + u]);
+#pragma unroll
+      for (int u = 0; u < 8; ++u)
+        if (k0 + u < nc && s_src[k0 + u] != s_dst[k0 + u]) *at(s_dst[k0 + u]) = x[u];
+    }
+  }
+}
+
+__global__ void wf_kv_advance_kernel(int32_t* __restrict__ seq_len, const int32_t* __restrict__ n_commit, int B) {
+  wf_pdl_trigger();
+  wf_pdl_wait();
+  const int b = blockIdx.x * blockDim.x + threadIdx.x;
+  if (b < B) seq_len[b] += n_commit[b];
+}
+
+extern "C" int wf_kv_compact_path(wf_paged_kv* kv, const int32_t* path, int path_stride, const int32_t* n_commit, int B,
+                                  void* stream) {
+  if (!kv) return WF_ERR_INVALID_ARG;
+  wf_ctx* ctx = kv->ctx;
+  WF_REQUIRE(ctx, path && n_commit && path_stride >= 1 && B >= 0 && B <= kv->s.max_seqs, WF_ERR_INVALID_ARG,
+             "wf_kv_compact_path: bad arguments");
+  if (B == 0) return WF_OK;
+  cudaStream_t st = (cudaStream_t)stream;
+  wf_launch(wf_kv_compact_path_kernel, dim3(B, kv->s.n_layers), dim3(256), 0, st, kv_view(kv), path, path_stride,
+            n_commit, ctx->d_status);
+  int rc = wf_check_launch(ctx, "wf_kv_compact_path_kernel");
+  if (rc != WF_OK) return rc;
+  wf_launch(wf_kv_advance_kernel, dim3((B + 255) / 256), dim3(256), 0, st, kv->seq_len, n_commit, B);
+  return wf_check_launch(ctx, "wf_kv_advance_kernel");
+}
