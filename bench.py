@@ -303,7 +303,7 @@ def run_ours(args):
     K, W = args.steps, max(args.warmup, 3)
     e2e_steps = max(1, min(K, args.e2e_steps))
     eager_steps = 8
-    rs = RoundState(ctx, wl, n_slots=4, n_rounds_max=W + K + e2e_steps + eager_steps + 4, host_copies=True)
+    rs = RoundState(ctx, wl, n_slots=4, n_rounds_max=W + K + e2e_steps + eager_steps + 4 + 10, host_copies=True)   # + 10: pages for the tree leg
     B, L = rs.B, rs.L
 
     # ---- cpu_baseline + full-size sampled parity (rank 0 of a 1-GPU run only) ----
@@ -459,8 +459,40 @@ def run_ours(args):
     torch.cuda.synchronize()
     neural_us = 1e3 * n0.elapsed_time(n1) / 20
 
+    # ---- tree verification round, timed on its own: every sequence brings a 60-node draft tree
+    #      (PAPER.md:317); masks + L x tree attention + acceptance walk + path compaction ----
+    tree = None
+    if not args.no_tree:
+        tsl = rs.make_tree_slot(60)
+        tree_steps = 6
+        ev_t = [{"attn": (torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))} for _ in range(tree_steps)]
+        for _ in range(2):
+            rs.run_tree_round(tsl)
+        rs.check_tree_plan(tsl)
+        t_len = rs.seq_len.cpu().numpy().astype(np.int64)
+        t_commit = np.array([len(p) for p in tsl.paths], dtype=np.int64)
+        t_bytes = []
+        t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        t0.record()
+        for i in range(tree_steps):
+            t_bytes.append(int((t_len + 60).sum()) * sh.n_kv_heads * sh.head_dim * 2 * 2)
+            t_len = t_len + t_commit
+            rs.run_tree_round(tsl, events=ev_t[i])
+        t1.record()
+        rs.check_tree_plan(tsl)
+        tree_ms = t0.elapsed_time(t1)
+        tree_attn_ms = sum(e["attn"][0].elapsed_time(e["attn"][1]) for e in ev_t)
+        tree = {"rounds_per_s": tree_steps / (tree_ms * 1e-3), "ms_per_round": tree_ms / tree_steps, "steps": tree_steps,
+                "nodes": 60, "attn_us_per_launch": 1e3 * tree_attn_ms / (tree_steps * L),
+                "kv_read_gbs": float(np.mean(t_bytes)) / (tree_attn_ms / (tree_steps * L) * 1e-3) / 1e9,
+                "committed_tokens_per_round": float(t_commit.sum()),
+                "note": "all sequences AR-routed with depth-8 / top-k-10 / 60-node trees (PAPER.md:317); 240 query rows per "
+                        "kv head = 4 sub-blocks that stream the same K/V (HBM once, L2 for the rest)"}
+
     if rank == 0:
         peak, peak_src = measured_peaks()
+        if tree:
+            tree["frac_of_hbm_peak"] = tree["kv_read_gbs"] / peak
         avg_launch_ms = attn_ms / (K * L)
         achieved = float(np.mean(attn_bytes)) / (avg_launch_ms * 1e-3) / 1e9
         line = {
@@ -492,6 +524,8 @@ def run_ours(args):
                               "note": "WhiFlash-Neural policy (d -> d/8 -> GELU -> 1), back-to-back calls, not part of the round"},
             "clocks": clocks,
         }
+        if tree:
+            line["tree_verify"] = tree
         if cpu_baseline:
             line["cpu_baseline"] = cpu_baseline
             line["parity_sample"] = parity
@@ -512,6 +546,7 @@ def main():
     ap.add_argument("--workload", default="cfg3", choices=sorted(WORKLOADS))
     ap.add_argument("--e2e-steps", type=int, default=30)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-tree", action="store_true", help="skip the tree-verification leg (SURVEY.md §8(f) f2)")
     ap.add_argument("--cpu-sample-seqs", type=int, default=4)
     ap.add_argument("--cpu-sample-layers", type=int, default=8)
     ap.add_argument("--traffic-bytes", type=float, default=None,

@@ -250,6 +250,84 @@ class RoundState:
         self.rounds_done += 1
         return s
 
+    # ------------------------------------------------------------------------------------------
+    # Tree verification round: every sequence is AR-routed and brings a draft tree of
+    # `n_nodes` rows (depth 8, top-k 10, 60 draft tokens).  Inputs and calls only.
+    def make_tree_slot(self, n_nodes=60, depth=8, top_k=10):
+        torch, sh, wl, dev, B = self.torch, self.sh, self.wl, self.device, self.B
+        g = synth.rng(wl.seed, 3000)
+        t = Slot()
+        t.n_nodes = n_nodes
+        parents = [synth.draw_tree(g, n_nodes, depth, top_k) for _ in range(B)]
+        n = B * n_nodes
+        t.q_indptr_host = np.arange(0, n + 1, n_nodes, dtype=np.int32)
+        t.q = synth.device_normal_bf16((n, sh.n_q_heads, sh.head_dim), 1.0, wl.seed, 3001, dev)
+        t.attn_out = torch.zeros_like(t.q)
+        t.logits = synth.device_normal_f32((n, sh.vocab), sh.logit_sigma, wl.seed, 3002, dev)
+        winners = g.integers(0, sh.vocab, size=n).astype(np.int64)
+        gaps = g.uniform(0.05, 1.0, size=n).astype(np.float32)
+        tokens = g.integers(0, sh.vocab, size=n).astype(np.int32)
+        want = synth.draw_accept_prefix(g, np.full(B, depth), wl.mean_accept)
+        t.paths = []
+        for b in range(B):
+            r0, par = b * n_nodes, parents[b]
+            kids = [[c for c in range(n_nodes) if par[c] == j] for j in range(n_nodes)]
+            for j in range(n_nodes):                         # siblings carry distinct tokens, none the winner
+                used = {int(winners[r0 + j])}
+                for c in kids[j]:
+                    while int(tokens[r0 + c]) in used:
+                        tokens[r0 + c] = (tokens[r0 + c] + 1) % sh.vocab
+                    used.add(int(tokens[r0 + c]))
+            cur, path = 0, [0]
+            while len(path) - 1 < int(want[b]) and kids[cur]:
+                c = int(kids[cur][g.integers(0, len(kids[cur]))])
+                tokens[r0 + c] = winners[r0 + cur]
+                cur = c
+                path.append(cur)
+            t.paths.append(path)
+        rows = torch.arange(n, device=dev)
+        w_t = torch.from_numpy(winners).to(dev)
+        t.logits[rows, w_t] = -float("inf")
+        t.logits[rows, w_t] = t.logits.amax(dim=1) + torch.from_numpy(gaps).to(dev)
+        t.tokens = _i32(tokens, dev)
+        t.parent = _i32(np.concatenate(parents), dev)
+        t.q_indptr = _i32(t.q_indptr_host, dev)
+        t.add_tokens = _i32(np.full(B, n_nodes), dev)
+        t.masks = torch.zeros(n, dtype=torch.int64, device=dev)
+        t.path = torch.full((B, n_nodes), -1, dtype=torch.int32, device=dev)
+        t.attn_ws = torch.empty(wf.wf_verify_attn_workspace_bytes(self.kv_shape, B, sh.n_q_heads, n_nodes),
+                                dtype=torch.uint8, device=dev)
+        t.acc_ws = torch.empty(wf.wf_accept_workspace_bytes(n, sh.vocab), dtype=torch.uint8, device=dev)
+        return t
+
+    def run_tree_round(self, t, stream=None, events=None):
+        """reserve -> ancestor masks (once) -> L x tree attention -> acceptance walk -> path compaction."""
+        sh, B, o = self.sh, self.B, self.out
+        self.target_kv.reserve(t.add_tokens, B, stream)
+        wf.wf_tree_masks(self.ctx, t.parent, t.q_indptr, B, t.n_nodes, t.masks, stream)
+        if events:
+            events["attn"][0].record()
+        for l in range(self.L):
+            wf.wf_verify_attn_tree(self.ctx, self.target_kv, l, t.q, t.q_indptr, t.masks, B, sh.n_q_heads, t.n_nodes,
+                                   self.sm_scale, t.attn_out, t.attn_ws, stream)
+        if events:
+            events["attn"][1].record()
+        wf.wf_accept_tree_entropy_route(self.ctx, t.logits, sh.vocab, t.tokens, t.parent, t.q_indptr, B, t.n_nodes, self.tau,
+                                        True, o["accept_len"], o["bonus_token"], self.entropy, o["route"], o["n_commit"],
+                                        t.path, t.n_nodes, t.acc_ws, stream)
+        wf.wf_kv_compact_path(self.ctx, self.target_kv, t.path, t.n_nodes, o["n_commit"], B, stream)
+
+    def check_tree_plan(self, t):
+        self.torch.cuda.synchronize()
+        st = self.ctx.poll_status()
+        if st != 0:
+            raise RuntimeError(f"device status {st}")
+        a = self.out["accept_len"].cpu().numpy()
+        path = t.path.cpu().numpy()
+        for b, want in enumerate(t.paths):
+            if int(a[b]) != len(want) - 1 or list(path[b][:len(want)]) != want:
+                raise RuntimeError(f"tree round: sequence {b} accepted {list(path[b][:int(a[b]) + 1])}, planted {want}")
+
     def check_plan(self, s):
         """After a sync: the device's outputs of the last round must equal the planted plan."""
         self.torch.cuda.synchronize()
