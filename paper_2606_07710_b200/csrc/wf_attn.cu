@@ -15,8 +15,8 @@
 //   warps 8,10: TMA producers (K ring, V ring).  One elected lane issues the 16 page boxes of a tile
 //               (cp.async.bulk.tensor.2d, 128-byte swizzle) in straight-line code; the page ids of the
 //               next tile are prefetched; a K tile is released when its QK^T retires.
-//   warp 9    : MMA issuer (one thread).  S = Q K^T (UMMA 64 x 128 x 16, both K-major) into TMEM,
-//               double buffered; O_t = P V (64 x D x 16, V MN-major) into TMEM, double buffered.
+//   warps 9,11: MMA issuers (one elected thread each).  Warp 9: S = Q K^T (UMMA 64 x 128 x 16, both K-major) into
+//               TMEM, double buffered; warp 11: O_t = P V (64 x D x 16, V MN-major) into TMEM, double buffered.
 //   warps 0-7 : softmax, two groups of 4 warps that ping-pong over the tiles.  UMMA M = 64 puts rows
 //               16w..16w+15 on TMEM lanes 32w..32w+15, so warp w owns 16 rows; tcgen05.ld.16x256b hands
 //               them out like an mma C fragment (a quad per row).  Online softmax in the log2 domain
@@ -28,7 +28,7 @@
 
 namespace {
 
-constexpr int AT_THREADS = 384;           // 12 warps: 0-3 / 4-7 softmax groups, 8 K loader, 9 MMA, 10 V loader
+constexpr int AT_THREADS = 384;           // 12 warps: 0-3 / 4-7 softmax groups, 8 K loader, 9 QK^T issuer, 10 V loader, 11 PV issuer
 constexpr int AT_BN = 128;             // keys per tile
 constexpr int AT_ROWS = 64;            // query rows = UMMA M
 constexpr int AT_MAX_B = 1024;
@@ -204,47 +204,61 @@ __device__ __forceinline__ void attn_loader(const AttnParams& p, AttnShared<TREE
   }
 }
 
-// ================= warp 9: MMA issuer =================
+// ================= warps 9 (S = Q K^T) and 11 (O_t = P V): MMA issuers =================
 // Tile g2 (global tile counter) belongs to softmax group g2 & 1, which owns S[g2&1], P[g2&1], O[g2&1].
-// The whole warp runs the loop so that addresses and descriptors stay warp-uniform; one elected lane
-// issues the tcgen05 instructions.  Descriptors are built once and advanced by constant offsets.
+// The two products have their own issuing warp: a tcgen05.mma is accepted at the pace of the tensor pipe and every
+// mbarrier poll costs the issuing thread about a hundred cycles, so ONE warp that polls five barriers per tile
+// between its two batches left the pipe idle half of the time whenever the loop was compute-paced (L2-resident
+// K/V: tree sub-blocks, small launches).  With two issuers one polls while the other's batch executes.  The whole
+// warp runs the loop so that addresses and descriptors stay warp-uniform; one elected lane issues.  Descriptors
+// are built once and advanced by constant offsets.  Hazards are carried by the barriers alone: QK^T(g2) needs
+// K(g2) and S[g2&1] read out by the softmax of tile g2 - 2 (s_empty); PV(g2) needs V(g2), P(g2) (p_full) and
+// O[g2&1] folded (o_empty).  tcgen05.commit covers the MMAs of the committing thread, i.e. exactly its batch.
 template <int D, bool TREE>
-__device__ __forceinline__ void attn_mma(const AttnParams& p, AttnShared<TREE>& sh, uint8_t* q_s, uint8_t* p0_s, uint8_t* p1_s,
-                                         uint8_t* k_s, uint8_t* v_s, uint32_t tmem_base) {
+__device__ __forceinline__ void attn_mma_qk(const AttnParams& p, AttnShared<TREE>& sh, uint8_t* q_s, uint8_t* k_s,
+                                            uint32_t tmem_base) {
   using C = AttnCfg<D>;
   const uint32_t idesc_qk = umma_idesc_kk(AT_ROWS, AT_BN);
-  const uint32_t idesc_pv = umma_idesc(AT_ROWS, D);
   const uint64_t dq0 = umma_desc(smem_u32(q_s), 16, 1024);                  // K-major
   const uint64_t dk0 = umma_desc(smem_u32(k_s), 16, 1024);                  // K-major
+  SegWalker<TREE> walk(sh, p.kv.n_kv_heads, blockIdx.x);
+  Segment sg;
+  uint32_t gt = 0, n_seg = 0;
+  while (walk.next(sg)) {
+    mbar_wait(smem_u32(&sh.q_ready), n_seg & 1);
+    ++n_seg;
+    for (int t = 0; t < sg.n_tiles; ++t, ++gt) {
+      const int st = gt % C::STAGES_K;
+      mbar_wait(smem_u32(&sh.k_full[st]), (gt / C::STAGES_K) & 1);
+      mbar_wait(smem_u32(&sh.s_empty[gt & 1]), ((gt >> 1) & 1) ^ 1);
+      tc_fence_after();
+      if (elect_one()) {
+        const uint64_t dk = dk0 + (uint64_t)((st * C::K_BYTES) >> 4);
+        const uint32_t td = tmem_base + C::TM_S + (gt & 1) * AT_BN;
+#pragma unroll
+        for (int k16 = 0; k16 < D / 16; ++k16)
+          umma_bf16(td, dq0 + (uint64_t)(((k16 >> 2) * C::Q_HALF + (k16 & 3) * 32) >> 4),
+                    dk + (uint64_t)(((k16 >> 2) * C::KV_HALF + (k16 & 3) * 32) >> 4), idesc_qk, k16 != 0);
+        umma_commit(smem_u32(&sh.s_full[gt & 1]));
+        umma_commit(smem_u32(&sh.k_empty[st]));                // the K tile is free once QK^T has retired
+      }
+      __syncwarp();
+    }
+  }
+}
+
+template <int D, bool TREE>
+__device__ __forceinline__ void attn_mma_pv(const AttnParams& p, AttnShared<TREE>& sh, uint8_t* p0_s, uint8_t* p1_s,
+                                            uint8_t* v_s, uint32_t tmem_base) {
+  using C = AttnCfg<D>;
+  const uint32_t idesc_pv = umma_idesc(AT_ROWS, D);
   const uint64_t dp0 = umma_desc(smem_u32(p0_s), 16, 1024);                 // K-major
   const uint64_t dp1 = umma_desc(smem_u32(p1_s), 16, 1024);
   const uint64_t dv0 = umma_desc(smem_u32(v_s), C::KV_HALF, 1024);          // MN-major
   SegWalker<TREE> walk(sh, p.kv.n_kv_heads, blockIdx.x);
   Segment sg;
-  uint32_t gt = 0, n_seg = 0;
-  auto issue_qk = [&](uint32_t g2) {
-    const int st = g2 % C::STAGES_K;
-    mbar_wait(smem_u32(&sh.k_full[st]), (g2 / C::STAGES_K) & 1);
-    mbar_wait(smem_u32(&sh.s_empty[g2 & 1]), ((g2 >> 1) & 1) ^ 1);
-    tc_fence_after();
-    if (elect_one()) {
-      const uint64_t dk = dk0 + (uint64_t)((st * C::K_BYTES) >> 4);
-      const uint32_t td = tmem_base + C::TM_S + (g2 & 1) * AT_BN;
-#pragma unroll
-      for (int k16 = 0; k16 < D / 16; ++k16)
-        umma_bf16(td, dq0 + (uint64_t)(((k16 >> 2) * C::Q_HALF + (k16 & 3) * 32) >> 4),
-                  dk + (uint64_t)(((k16 >> 2) * C::KV_HALF + (k16 & 3) * 32) >> 4), idesc_qk, k16 != 0);
-      umma_commit(smem_u32(&sh.s_full[g2 & 1]));
-      umma_commit(smem_u32(&sh.k_empty[st]));                  // the K tile is free once QK^T has retired
-    }
-    __syncwarp();
-  };
+  uint32_t gt = 0;
   while (walk.next(sg)) {
-    mbar_wait(smem_u32(&sh.q_ready), n_seg & 1);
-    ++n_seg;
-    tc_fence_after();
-    issue_qk(gt);
-    if (sg.n_tiles > 1) issue_qk(gt + 1);
     for (int t = 0; t < sg.n_tiles; ++t, ++gt) {
       const int st = gt % C::STAGES_V, g = gt & 1;
       mbar_wait(smem_u32(&sh.v_full[st]), (gt / C::STAGES_V) & 1);
@@ -263,8 +277,6 @@ __device__ __forceinline__ void attn_mma(const AttnParams& p, AttnShared<TREE>& 
         umma_commit(smem_u32(&sh.v_empty[st]));
       }
       __syncwarp();
-      // QK^T(t+2) after PV(t) (measured: issuing it ahead of PV(t) gains nothing, the loop is memory-paced)
-      if (t + 2 < sg.n_tiles) issue_qk(gt + 2);
     }
   }
 }
@@ -761,7 +773,8 @@ __global__ void __launch_bounds__(AT_THREADS, 1) wf_verify_attn_kernel(const Att
       asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
       if (warp == 8) attn_loader<D, TREE>(p, sh, k_s, 0, lane);
       else if (warp == 10) attn_loader<D, TREE>(p, sh, v_s, 1, lane);
-      else if (warp == 9) attn_mma<D, TREE>(p, sh, q_s, p0_s, p1_s, k_s, v_s, tmem_base);
+      else if (warp == 9) attn_mma_qk<D, TREE>(p, sh, q_s, k_s, tmem_base);
+      else if (warp == 11) attn_mma_pv<D, TREE>(p, sh, p0_s, p1_s, v_s, tmem_base);
     }
   }
   tc_fence_before();
