@@ -459,6 +459,36 @@ def run_ours(args):
     torch.cuda.synchronize()
     neural_us = 1e3 * n0.elapsed_time(n1) / 20
 
+    # ---- stochastic acceptance next to the greedy sweep, both on the last slot's logits, cache
+    #      length untouched (target_kv = NULL): one sweep over the logits + the per-sequence inverse-CDF draw ----
+    gsmp = torch.Generator(device="cuda")
+    gsmp.manual_seed(wl.seed)
+    u_acc = torch.rand(s.sum_q, dtype=torch.float32, device="cuda", generator=gsmp)
+    u_smp = torch.rand(B, dtype=torch.float32, device="cuda", generator=gsmp)
+    tok_out = torch.zeros(B, dtype=torch.int32, device="cuda")
+    acc_us = {}
+    for mode in ("greedy", "sample"):
+        def call():
+            o = rs.out
+            if mode == "greedy":
+                wf.wf_accept_entropy_route(ctx, s.logits, sh.vocab, s.drafts, s.q_indptr, B, rs.qmax, rs.tau, True, o["accept_len"],
+                                           tok_out, rs.entropy, o["route"], o["n_commit"], None, rs.acc_ws)
+            else:
+                wf.wf_accept_sample_entropy_route(ctx, s.logits, sh.vocab, s.drafts, s.q_indptr, B, rs.qmax, 0.8, None, u_acc, u_smp,
+                                                  rs.tau, True, o["accept_len"], tok_out, rs.entropy, o["route"], o["n_commit"],
+                                                  None, rs.acc_ws)
+        for _ in range(3):
+            call()
+        torch.cuda.synchronize()
+        a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a0.record()
+        for _ in range(20):
+            call()
+        a1.record()
+        torch.cuda.synchronize()
+        acc_us[mode] = 1e3 * a0.elapsed_time(a1) / 20
+    logit_bytes = float(s.sum_q) * sh.vocab * 4
+
     # ---- tree verification round, timed on its own: every sequence brings a 60-node draft tree
     #      (PAPER.md:317); masks + L x tree attention + acceptance walk + path compaction ----
     tree = None
@@ -524,6 +554,12 @@ def run_ours(args):
                               "note": "WhiFlash-Neural policy (d -> d/8 -> GELU -> 1), back-to-back calls, not part of the round"},
             "clocks": clocks,
         }
+        line["stochastic_accept"] = {"us_per_call": acc_us["sample"], "greedy_us_per_call": acc_us["greedy"], "temperature": 0.8,
+                                     "logits_gbs": logit_bytes / (acc_us["sample"] * 1e-6) / 1e9,
+                                     "greedy_logits_gbs": logit_bytes / (acc_us["greedy"] * 1e-6) / 1e9,
+                                     "note": "speculative sampling (one-hot drafter, uniforms as inputs): same sweep over the "
+                                             "logits plus one inverse-CDF draw per sequence; back-to-back calls on L2-cold-ish "
+                                             "logits of the last slot, not part of the round"}
         if tree:
             line["tree_verify"] = tree
         if cpu_baseline:

@@ -231,6 +231,27 @@ int wf_accept_tree_entropy_route(wf_ctx* ctx, const float* logits, int V, const 
 int wf_kv_compact_path(wf_paged_kv* kv, const int32_t* path, int path_stride, const int32_t* n_commit, int B,
                        void* stream);
 
+/* ---- (f4) stochastic acceptance: speculative sampling with temperature ----------------------------
+ * PAPER.md:19 (the speculative-decoding rule of the papers cited there), :79-81 (under sampling the
+ * softmax already exists and the router reads its entropy); readings S1-S5; SURVEY.md §8(f) f4.
+ * Chain block layout as wf_accept_entropy_route.  p_i = softmax(logits[r0+i] / temperature).
+ * draft_q: fp32 [sum_q][V], row r0+i = the drafter's distribution for the token after row i, or NULL for a
+ * deterministic drafter (one-hot at the proposed token).  u_accept: fp32 [sum_q], u_sample: fp32 [B],
+ * uniforms in [0, 1) drawn by the caller (row r0 of u_accept is unused).
+ *     draft j (j = 1..gamma) is accepted iff u_accept[r0+j] < min(1, p_{j-1}(x_j) / q_{j-1}(x_j)) (q = 0: ratio 1);
+ *     accept_len = a = drafts accepted before the first rejection; n_commit = a + 1;
+ *     token = inverse CDF at u_sample[b], in vocabulary order, of max(0, p_a - q_a) if a < gamma (of p_a if
+ *     that is empty), of p_a if a = gamma: the smallest v whose cumulative mass exceeds u * total;
+ *     entropy = H(p_a) in nats, route = AR iff entropy > tau.
+ * If target_kv != NULL, target_kv.seq_len[b] += n_commit[b].  Probabilities are evaluated in fp32 and accumulated
+ * in fp64; workspace as wf_accept_workspace_bytes(B * max_q_len, V).  Asynchronous on `stream`. */
+int wf_accept_sample_entropy_route(wf_ctx* ctx, const float* logits, int V, const int32_t* draft_tokens,
+                                   const int32_t* q_indptr, int B, int max_q_len, float temperature,
+                                   const float* draft_q, const float* u_accept, const float* u_sample,
+                                   const float* tau, int tau_is_scalar, int32_t* accept_len, int32_t* token,
+                                   float* entropy, int32_t* route, int32_t* n_commit, wf_paged_kv* target_kv,
+                                   void* workspace, size_t workspace_bytes, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

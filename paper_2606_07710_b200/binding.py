@@ -33,6 +33,7 @@ EXPORTS = [
     "wf_lazy_catchup_enqueue", "wf_lazy_catchup_flush",
     "wf_neural_route", "wf_neural_route_workspace_bytes", "wf_lazy_catchup_round",
     "wf_tree_masks", "wf_verify_attn_tree", "wf_accept_tree_entropy_route", "wf_kv_compact_path",
+    "wf_accept_sample_entropy_route",
 ]
 
 
@@ -75,6 +76,8 @@ _SIG = {
     "wf_accept_tree_entropy_route": (_i, [_vp, _vp, _i, _vp, _vp, _vp, _i, _i, _vp, _i, _vp, _vp, _vp, _vp, _vp, _vp, _i,
                                           _vp, _sz, _vp]),
     "wf_kv_compact_path": (_i, [_vp, _vp, _i, _vp, _i, _vp]),
+    "wf_accept_sample_entropy_route": (_i, [_vp, _vp, _i, _vp, _vp, _i, _i, C.c_float, _vp, _vp, _vp, _vp, _i, _vp, _vp, _vp,
+                                            _vp, _vp, _vp, _vp, _sz, _vp]),
 }
 for _name, (_res, _args) in _SIG.items():
     _f = getattr(lib, _name)
@@ -248,3 +251,13 @@ def wf_accept_tree_entropy_route(ctx, logits, V, node_tokens, parent, q_indptr, 
 
 def wf_kv_compact_path(ctx, kv, path, path_stride, n_commit, B, stream=None):
     ctx.check(lib.wf_kv_compact_path(kv.h, _ptr(path), path_stride, _ptr(n_commit), B, _stream(stream)))
+
+
+def wf_accept_sample_entropy_route(ctx, logits, V, draft_tokens, q_indptr, B, max_q_len, temperature, draft_q, u_accept,
+                                   u_sample, tau, tau_is_scalar, accept_len, token, entropy, route, n_commit, target_kv,
+                                   workspace, stream=None):
+    ctx.check(lib.wf_accept_sample_entropy_route(
+        ctx.h, _ptr(logits), V, _ptr(draft_tokens), _ptr(q_indptr), B, max_q_len, C.c_float(temperature), _ptr(draft_q),
+        _ptr(u_accept), _ptr(u_sample), _ptr(tau), int(tau_is_scalar), _ptr(accept_len), _ptr(token), _ptr(entropy),
+        _ptr(route), _ptr(n_commit), target_kv.h if target_kv is not None else None, _ptr(workspace),
+        workspace.numel() * workspace.element_size(), _stream(stream)))

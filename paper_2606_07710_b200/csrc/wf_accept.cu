@@ -34,6 +34,15 @@ __device__ __forceinline__ void argmax_merge(float& m, int& i, float om, int oi)
   if (om > m || (om == m && oi < i)) { m = om; i = oi; }
 }
 
+// Stochastic acceptance (readings S1-S5): u_accept != nullptr switches the finalise step from the greedy prefix to
+// speculative sampling at temperature 1 / inv_t.
+struct AccSample {
+  const float* u_accept;     // [sum_q] uniforms, one per draft row (row 0 of a block unused)
+  const float* u_sample;     // [B] uniform of the residual / bonus draw
+  const float* draft_q;      // nullptr (deterministic drafter: one-hot at the proposed token) or [sum_q][V]
+  float inv_t;               // 1 / temperature; 1.0f in the greedy modes (z * 1.0f is exact)
+};
+
 template <bool VEC>
 __global__ void __launch_bounds__(ACC_THREADS)
 wf_accept_kernel(const float* __restrict__ logits, int V, int n_chunks, const int32_t* __restrict__ draft_tokens,
@@ -41,7 +50,7 @@ wf_accept_kernel(const float* __restrict__ logits, int V, int n_chunks, const in
                  int32_t* __restrict__ accept_len, int32_t* __restrict__ bonus_token, float* __restrict__ entropy,
                  int32_t* __restrict__ route, int32_t* __restrict__ n_commit, int32_t* __restrict__ kv_seq_len,
                  AccPartial* __restrict__ partials, unsigned int* __restrict__ counters,
-                 const int32_t* __restrict__ parent, int32_t* __restrict__ path, int path_stride) {
+                 const int32_t* __restrict__ parent, int32_t* __restrict__ path, int path_stride, const AccSample smp) {
   // parent == nullptr: chain block (C6).  Else tree block (T1-T4): greedy walk over parent pointers, the accepted
   // node indices go to path[b][0..a] (-1 beyond), and the cache length is left to wf_kv_compact_path.
   wf_pdl_trigger();
@@ -68,7 +77,7 @@ wf_accept_kernel(const float* __restrict__ logits, int V, int n_chunks, const in
       const int e = (k * ACC_THREADS + tid) * 4;
       float4 x = make_float4(-INFINITY, -INFINITY, -INFINITY, -INFINITY);
       if (e < n_here) x = ld_stream(p + k * ACC_THREADS + tid);     // V % 4 == 0: all or nothing
-      v[4 * k + 0] = x.x; v[4 * k + 1] = x.y; v[4 * k + 2] = x.z; v[4 * k + 3] = x.w;
+      v[4 * k + 0] = x.x * smp.inv_t; v[4 * k + 1] = x.y * smp.inv_t; v[4 * k + 2] = x.z * smp.inv_t; v[4 * k + 3] = x.w * smp.inv_t;
     }
   } else {
 #pragma unroll
@@ -76,7 +85,7 @@ wf_accept_kernel(const float* __restrict__ logits, int V, int n_chunks, const in
 #pragma unroll
       for (int j = 0; j < 4; ++j) {
         const int e = (k * ACC_THREADS + tid) * 4 + j;
-        v[4 * k + j] = e < n_here ? __ldg(row + c0 + e) : -INFINITY;
+        v[4 * k + j] = e < n_here ? __ldg(row + c0 + e) * smp.inv_t : -INFINITY;
       }
   }
 
@@ -172,7 +181,43 @@ wf_accept_kernel(const float* __restrict__ logits, int V, int n_chunks, const in
   __shared__ int s_par[ACC_MAX_Q], s_tok[ACC_MAX_Q];
   if (parent && tid < q_b) { s_par[tid] = parent[r0 + tid]; s_tok[tid] = draft_tokens[r0 + tid]; }
   __syncthreads();
-  if (!parent) {
+  __shared__ float s_M[ACC_MAX_Q];
+  __shared__ double s_Z[ACC_MAX_Q];
+  __shared__ int s_ok[ACC_MAX_Q];
+  if (smp.u_accept) {
+    // ---- speculative sampling (S3): p_{j-1}(x_j) from row j-1's slice partials and one gathered logit ----
+    for (int r = wid; r < q_b; r += ACC_THREADS / 32) {   // one warp per row: (max, Z) over the slices
+      const AccPartial* pr = &partials[(size_t)(r0 + r) * n_chunks];
+      float gm = -INFINITY;
+      for (int c = lane; c < n_chunks; c += 32) gm = fmaxf(gm, __ldcg(&pr[c].m));
+#pragma unroll
+      for (int d = 16; d > 0; d >>= 1) gm = fmaxf(gm, __shfl_xor_sync(0xffffffffu, gm, d));
+      double Zd = 0.0;
+      for (int c = lane; c < n_chunks; c += 32) {
+        const float pm = __ldcg(&pr[c].m);
+        if (pm > -INFINITY) Zd += (double)__ldcg(&pr[c].Z) * exp((double)pm - (double)gm);
+      }
+#pragma unroll
+      for (int d = 16; d > 0; d >>= 1) Zd += __shfl_xor_sync(0xffffffffu, Zd, d);
+      if (lane == 0) { s_M[r] = gm; s_Z[r] = Zd; }
+    }
+    __syncthreads();
+    if (tid >= 1 && tid < q_b) {                           // draft j = tid against row j - 1
+      const int x = draft_tokens[r0 + tid];
+      const size_t at = (size_t)(r0 + tid - 1) * V + x;
+      const double px = exp((double)(logits[at] * smp.inv_t) - (double)s_M[tid - 1]) / s_Z[tid - 1];
+      const double qx = smp.draft_q ? (double)smp.draft_q[at] : 1.0;
+      const double ratio = qx <= 0.0 ? 1.0 : fmin(1.0, px / qx);
+      s_ok[tid] = (double)smp.u_accept[r0 + tid] < ratio;
+    }
+    __syncthreads();
+    if (tid == 0) {
+      int a = 0;
+      while (a < q_b - 1 && s_ok[a + 1]) ++a;
+      s_a = a;
+      s_row = a;
+    }
+  } else if (!parent) {
     if (tid == 0) {                                        // longest accepted prefix (C6)
       const int gamma = q_b - 1;
       int a = 0;
@@ -229,12 +274,81 @@ wf_accept_kernel(const float* __restrict__ logits, int V, int n_chunks, const in
       const float H = (float)(log(Zd) - Sd / Zd);
       const float t = tau_is_scalar ? tau[0] : tau[b];
       accept_len[b] = a;
-      bonus_token[b] = s_g[row_a];
+      if (!smp.u_accept) bonus_token[b] = s_g[row_a];
       n_commit[b] = a + 1;
       entropy[b] = H;
       route[b] = (H > t) ? WF_ROUTE_AR : WF_ROUTE_DIFFUSION;     // C1, C2
       if (kv_seq_len) kv_seq_len[b] += a + 1;
     }
+  }
+  if (!smp.u_accept) return;
+
+  // ---- the token after the accepted prefix (S4): inverse CDF, in vocabulary order, of the residual max(0, p - q)
+  //      of row a (of p itself for the bonus token, or if the residual is empty).  Thread t owns the contiguous
+  //      vocabulary segment t; masses are evaluated in fp32, accumulated in fp64. ----
+  __shared__ double s_seg[ACC_THREADS];
+  __shared__ double s_target;
+  __shared__ int s_pick, s_resid, s_tok_out;
+  const int a = s_a, gamma = q_b - 1;
+  const float* zr = logits + (size_t)(r0 + a) * V;
+  const float* qr = smp.draft_q ? smp.draft_q + (size_t)(r0 + a) * V : nullptr;
+  const int xrej = a < gamma ? draft_tokens[r0 + a + 1] : -1;
+  const float Mr = s_M[a];
+  const double Zinv = 1.0 / s_Z[a];
+  const int seg = (V + ACC_THREADS - 1) / ACC_THREADS;
+  const int lo = min(V, tid * seg), hi = min(V, lo + seg);
+  auto mass = [&](int v, bool resid) -> double {
+    const float z = zr[v] * smp.inv_t;
+    const double pv = z == -INFINITY ? 0.0 : (double)expf(z - Mr) * Zinv;
+    if (!resid) return pv;
+    const double qv = qr ? (double)qr[v] : (v == xrej ? 1.0 : 0.0);
+    return fmax(0.0, pv - qv);
+  };
+  if (tid == 0) { s_resid = a < gamma; s_tok_out = -1; }
+  __syncthreads();
+  for (int attempt = 0; attempt < 2; ++attempt) {
+    const bool resid = s_resid != 0;
+    double acc = 0.0;
+    for (int v = lo; v < hi; ++v) acc += mass(v, resid);
+    s_seg[tid] = acc;
+    __syncthreads();
+    if (tid == 0) {
+      double run = 0.0;
+      for (int t = 0; t < ACC_THREADS; ++t) { const double x = s_seg[t]; s_seg[t] = run; run += x; }   // exclusive prefix
+      s_target = (double)smp.u_sample[b] * run;
+      int pick = -1;
+      if (run > 0.0) {
+        pick = 0;
+        for (int t = 1; t < ACC_THREADS; ++t)
+          if (s_seg[t] <= s_target) pick = t;              // the last segment that starts at or below the target
+      }
+      s_pick = pick;
+      if (pick < 0) s_resid = 0;                           // empty residual (p <= q everywhere): draw from p itself
+    }
+    __syncthreads();
+    if (s_pick >= 0) break;
+  }
+  if (tid == s_pick) {
+    const bool resid = s_resid != 0;
+    double run = s_seg[tid];
+    int tok = -1, last = -1;
+    for (int v = lo; v < hi; ++v) {
+      const double mv = mass(v, resid);
+      if (mv > 0.0) last = v;
+      run += mv;
+      if (run > s_target && mv > 0.0) { tok = v; break; }
+    }
+    s_tok_out = tok >= 0 ? tok : last;                     // rounding at the segment's end: its last token with mass
+  }
+  __syncthreads();
+  if (tid == 0) {
+    int tok = s_tok_out;
+    if (tok < 0) {                                         // the picked segment held no mass at all (rounding): next one that does
+      tok = 0;
+      for (int v = min(V, (s_pick + 1) * seg); v < V; ++v)
+        if (mass(v, s_resid != 0) > 0.0) { tok = v; break; }
+    }
+    bonus_token[b] = tok;
   }
 }
 
@@ -250,7 +364,9 @@ namespace {
 int accept_launch(wf_ctx* ctx, const float* logits, int V, const int32_t* draft_tokens, const int32_t* q_indptr, int B,
                   int max_q_len, const float* tau, int tau_is_scalar, int32_t* accept_len, int32_t* bonus_token,
                   float* entropy, int32_t* route, int32_t* n_commit, wf_paged_kv* target_kv, void* workspace,
-                  size_t workspace_bytes, void* stream, const int32_t* parent, int32_t* path, int path_stride);
+                  size_t workspace_bytes, void* stream, const int32_t* parent, int32_t* path, int path_stride,
+                  const AccSample& smp);
+const AccSample kGreedy = {nullptr, nullptr, nullptr, 1.0f};
 }
 
 extern "C" int wf_accept_entropy_route(wf_ctx* ctx, const float* logits, int V, const int32_t* draft_tokens,
@@ -261,7 +377,22 @@ extern "C" int wf_accept_entropy_route(wf_ctx* ctx, const float* logits, int V, 
                                        void* stream) {
   return accept_launch(ctx, logits, V, draft_tokens, q_indptr, B, max_q_len, tau, tau_is_scalar, accept_len,
                        bonus_token, entropy, route, n_commit, target_kv, workspace, workspace_bytes, stream, nullptr,
-                       nullptr, 0);
+                       nullptr, 0, kGreedy);
+}
+
+extern "C" int wf_accept_sample_entropy_route(wf_ctx* ctx, const float* logits, int V, const int32_t* draft_tokens,
+                                              const int32_t* q_indptr, int B, int max_q_len, float temperature,
+                                              const float* draft_q, const float* u_accept, const float* u_sample,
+                                              const float* tau, int tau_is_scalar, int32_t* accept_len, int32_t* token,
+                                              float* entropy, int32_t* route, int32_t* n_commit, wf_paged_kv* target_kv,
+                                              void* workspace, size_t workspace_bytes, void* stream) {
+  if (!ctx) return WF_ERR_INVALID_ARG;
+  WF_REQUIRE(ctx, u_accept && u_sample, WF_ERR_INVALID_ARG, "wf_accept_sample_entropy_route: the uniforms are inputs");
+  WF_REQUIRE(ctx, temperature > 0.f && temperature < INFINITY, WF_ERR_INVALID_ARG,
+             "wf_accept_sample_entropy_route: temperature must be positive and finite");
+  const AccSample smp = {u_accept, u_sample, draft_q, 1.0f / temperature};
+  return accept_launch(ctx, logits, V, draft_tokens, q_indptr, B, max_q_len, tau, tau_is_scalar, accept_len, token,
+                       entropy, route, n_commit, target_kv, workspace, workspace_bytes, stream, nullptr, nullptr, 0, smp);
 }
 
 extern "C" int wf_accept_tree_entropy_route(wf_ctx* ctx, const float* logits, int V, const int32_t* node_tokens,
@@ -275,14 +406,15 @@ extern "C" int wf_accept_tree_entropy_route(wf_ctx* ctx, const float* logits, in
              "wf_accept_tree_entropy_route: parent / path missing or path_stride < max_nodes");
   return accept_launch(ctx, logits, V, node_tokens, q_indptr, B, max_nodes, tau, tau_is_scalar, accept_len,
                        bonus_token, entropy, route, n_commit, nullptr, workspace, workspace_bytes, stream, parent, path,
-                       path_stride);
+                       path_stride, kGreedy);
 }
 
 namespace {
 int accept_launch(wf_ctx* ctx, const float* logits, int V, const int32_t* draft_tokens, const int32_t* q_indptr, int B,
                   int max_q_len, const float* tau, int tau_is_scalar, int32_t* accept_len, int32_t* bonus_token,
                   float* entropy, int32_t* route, int32_t* n_commit, wf_paged_kv* target_kv, void* workspace,
-                  size_t workspace_bytes, void* stream, const int32_t* parent, int32_t* path, int path_stride) {
+                  size_t workspace_bytes, void* stream, const int32_t* parent, int32_t* path, int path_stride,
+                  const AccSample& smp) {
   if (!ctx) return WF_ERR_INVALID_ARG;
   WF_REQUIRE(ctx, logits && draft_tokens && q_indptr && tau && accept_len && bonus_token && entropy && route &&
                  n_commit && workspace, WF_ERR_INVALID_ARG, "wf_accept_entropy_route: null argument");
@@ -303,11 +435,11 @@ int accept_launch(wf_ctx* ctx, const float* logits, int V, const int32_t* draft_
   if (vec)
     wf_launch(wf_accept_kernel<true>, grid, dim3(ACC_THREADS), 0, st, logits, V, n_chunks, draft_tokens, q_indptr, tau,
         tau_is_scalar, accept_len, bonus_token, entropy, route, n_commit, kv_len, (AccPartial*)workspace, ctx->d_counters,
-        parent, path, path_stride);
+        parent, path, path_stride, smp);
   else
     wf_launch(wf_accept_kernel<false>, grid, dim3(ACC_THREADS), 0, st, logits, V, n_chunks, draft_tokens, q_indptr, tau,
         tau_is_scalar, accept_len, bonus_token, entropy, route, n_commit, kv_len, (AccPartial*)workspace, ctx->d_counters,
-        parent, path, path_stride);
+        parent, path, path_stride, smp);
   return wf_check_launch(ctx, "wf_accept_kernel");
 }
 }  // namespace
