@@ -34,6 +34,8 @@ __device__ __forceinline__ void argmax_merge(float& m, int& i, float om, int oi)
   if (om > m || (om == m && oi < i)) { m = om; i = oi; }
 }
 
+__device__ __forceinline__ int thi_of(int t, int lo, int hi, int piece) { return min(hi, min(hi, lo + t * piece) + piece); }
+
 // Stochastic acceptance (readings S1-S5): u_accept != nullptr switches the finalise step from the greedy prefix to
 // speculative sampling at temperature 1 / inv_t.
 struct AccSample {
@@ -284,8 +286,8 @@ wf_accept_kernel(const float* __restrict__ logits, int V, int n_chunks, const in
   if (!smp.u_accept) return;
 
   // ---- the token after the accepted prefix (S4): inverse CDF, in vocabulary order, of the residual max(0, p - q)
-  //      of row a (of p itself for the bonus token, or if the residual is empty).  Thread t owns the contiguous
-  //      vocabulary segment t; masses are evaluated in fp32, accumulated in fp64. ----
+  //      of row a (of p itself for the bonus token, or if the residual is empty).  Masses are evaluated in fp32 and
+  //      accumulated in fp64. ----
   __shared__ double s_seg[ACC_THREADS];
   __shared__ double s_target;
   __shared__ int s_pick, s_resid, s_tok_out;
@@ -295,58 +297,151 @@ wf_accept_kernel(const float* __restrict__ logits, int V, int n_chunks, const in
   const int xrej = a < gamma ? draft_tokens[r0 + a + 1] : -1;
   const float Mr = s_M[a];
   const double Zinv = 1.0 / s_Z[a];
-  const int seg = (V + ACC_THREADS - 1) / ACC_THREADS;
-  const int lo = min(V, tid * seg), hi = min(V, lo + seg);
-  auto mass = [&](int v, bool resid) -> double {
-    const float z = zr[v] * smp.inv_t;
-    const double pv = z == -INFINITY ? 0.0 : (double)expf(z - Mr) * Zinv;
-    if (!resid) return pv;
-    const double qv = qr ? (double)qr[v] : (v == xrej ? 1.0 : 0.0);
-    return fmax(0.0, pv - qv);
+  const float Zinv_f = (float)Zinv;
+  auto mass = [&](int v, bool resid) -> double {           // fp32 per token (MUFU exp: a -inf logit gives exactly 0)
+    float e;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"((zr[v] * smp.inv_t - Mr) * 1.4426950408889634f));
+    float pv = e * Zinv_f;
+    if (resid) pv = fmaxf(0.f, pv - (qr ? qr[v] : (v == xrej ? 1.f : 0.f)));
+    return (double)pv;
   };
+  // Search from coarse to fine, every level parallel over the CTA.  Level 0 costs no memory pass when the drafter is
+  // deterministic (or for the bonus token): the sweep's slice partials already hold each 8192-token slice's share of
+  // the mass (minus the rejected token's in its slice).  Then the range is cut into 8 contiguous parts, warp w sums
+  // part w with its lanes striding through it, and thread 0 picks the part that holds the target (twice when level 0
+  // had to be skipped because the residual needs the drafter's full row); the last ~1k tokens are cut into one short
+  // piece per thread and the owner of the piece that holds the target walks it.
+  constexpr int NW = ACC_THREADS / 32;
   if (tid == 0) { s_resid = a < gamma; s_tok_out = -1; }
   __syncthreads();
-  for (int attempt = 0; attempt < 2; ++attempt) {
+  int lo = 0, hi = V;
+  double base = 0.0;                                       // mass below lo
+  int levels = 2;
+  if (!qr && n_chunks <= ACC_THREADS) {
+    const AccPartial* pr = &partials[(size_t)(r0 + a) * n_chunks];
+    for (int attempt = 0; attempt < 2; ++attempt) {
+      double mc = 0.0;
+      if (tid < n_chunks) {
+        const float pm = __ldcg(&pr[tid].m);
+        if (pm > -INFINITY) mc = (double)__ldcg(&pr[tid].Z) * exp((double)pm - (double)Mr) * Zinv;
+        if (s_resid && xrej / ACC_CHUNK == tid)
+          mc = fmax(0.0, mc - exp((double)(zr[xrej] * smp.inv_t) - (double)Mr) * Zinv);
+      }
+      s_seg[tid] = mc;
+      __syncthreads();
+      if (tid == 0) {
+        double run = 0.0;
+        for (int t = 0; t < n_chunks; ++t) { const double x = s_seg[t]; s_seg[t] = run; run += x; }
+        if (!(run > 0.0) && s_resid) { s_resid = 0; s_pick = -1; }      // the rejected token held all the mass: draw from p
+        else {
+          s_target = (double)smp.u_sample[b] * run;
+          int pick = 0;
+          for (int t = 1; t < n_chunks; ++t)
+            if (s_seg[t] <= s_target) pick = t;
+          s_pick = pick;
+        }
+      }
+      __syncthreads();
+      if (s_pick >= 0) break;
+      __syncthreads();
+    }
+    base = s_seg[s_pick];
+    lo = s_pick * ACC_CHUNK;
+    hi = min(V, lo + ACC_CHUNK);
+    levels = 1;
+    __syncthreads();
+  }
+  for (int level = 0; level < levels; ++level) {
+    const bool first = levels == 2 && level == 0;          // this level also fixes the total and the target
+    const int part = (hi - lo + NW - 1) / NW;
     const bool resid = s_resid != 0;
+    const int plo = min(hi, lo + wid * part), phi = min(hi, plo + part);
     double acc = 0.0;
-    for (int v = lo; v < hi; ++v) acc += mass(v, resid);
-    s_seg[tid] = acc;
+    for (int v0 = plo + lane; v0 < phi; v0 += 32 * 8) {    // 8 loads in flight per lane
+      float zz[8], qq[8];
+#pragma unroll
+      for (int k = 0; k < 8; ++k) {
+        const int v = v0 + 32 * k;
+        zz[k] = v < phi ? zr[v] : -INFINITY;
+        qq[k] = (resid && qr && v < phi) ? qr[v] : 0.f;
+      }
+#pragma unroll
+      for (int k = 0; k < 8; ++k) {
+        const int v = v0 + 32 * k;
+        float e;
+        asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"((zz[k] * smp.inv_t - Mr) * 1.4426950408889634f));
+        float pv = e * Zinv_f;
+        if (resid) pv = fmaxf(0.f, pv - (qr ? qq[k] : (v == xrej ? 1.f : 0.f)));
+        acc += (double)pv;
+      }
+    }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, d);
+    if (lane == 0) s_seg[wid] = acc;
     __syncthreads();
     if (tid == 0) {
-      double run = 0.0;
-      for (int t = 0; t < ACC_THREADS; ++t) { const double x = s_seg[t]; s_seg[t] = run; run += x; }   // exclusive prefix
-      s_target = (double)smp.u_sample[b] * run;
-      int pick = -1;
-      if (run > 0.0) {
-        pick = 0;
-        for (int t = 1; t < ACC_THREADS; ++t)
-          if (s_seg[t] <= s_target) pick = t;              // the last segment that starts at or below the target
+      double run = base;
+      for (int t = 0; t < NW; ++t) { const double x = s_seg[t]; s_seg[t] = run; run += x; }     // mass below part t
+      s_pick = 0;
+      if (first) {
+        if (!(run > 0.0) && s_resid) { s_resid = 0; s_pick = -1; }    // empty residual (p <= q everywhere): draw from p
+        else s_target = (double)smp.u_sample[b] * run;
       }
-      s_pick = pick;
-      if (pick < 0) s_resid = 0;                           // empty residual (p <= q everywhere): draw from p itself
+      if (s_pick >= 0) {
+        int pick = 0;
+        for (int t = 1; t < NW; ++t)
+          if (s_seg[t] <= s_target) pick = t;              // the last part that starts at or below the target
+        s_pick = pick;
+      }
     }
     __syncthreads();
-    if (s_pick >= 0) break;
+    if (s_pick < 0) { level = -1; __syncthreads(); continue; }        // block-uniform: start over without the residual
+    base = s_seg[s_pick];
+    lo = min(hi, lo + s_pick * part);
+    hi = min(hi, lo + part);
+    __syncthreads();
   }
+  const bool resid = s_resid != 0;
+  const int piece = (hi - lo + ACC_THREADS - 1) / ACC_THREADS;
+  const int tlo = min(hi, lo + tid * piece), thi = min(hi, tlo + piece);
+  {
+    double acc = 0.0;
+    for (int v = tlo; v < thi; ++v) acc += mass(v, resid);
+    s_seg[tid] = acc;
+  }
+  __syncthreads();
+  if (tid == 0) {
+    double run = base;
+    int pick = 0;
+    for (int t = 0; t < ACC_THREADS; ++t) {
+      const double x = s_seg[t];
+      s_seg[t] = run;
+      if (run <= s_target) pick = t;
+      run += x;
+    }
+    s_pick = pick;
+  }
+  __syncthreads();
   if (tid == s_pick) {
-    const bool resid = s_resid != 0;
     double run = s_seg[tid];
-    int tok = -1, last = -1;
-    for (int v = lo; v < hi; ++v) {
+    int tok = -1;
+    for (int v = tlo; v < thi; ++v) {
       const double mv = mass(v, resid);
-      if (mv > 0.0) last = v;
       run += mv;
       if (run > s_target && mv > 0.0) { tok = v; break; }
     }
-    s_tok_out = tok >= 0 ? tok : last;                     // rounding at the segment's end: its last token with mass
+    s_tok_out = tok;
   }
   __syncthreads();
   if (tid == 0) {
     int tok = s_tok_out;
-    if (tok < 0) {                                         // the picked segment held no mass at all (rounding): next one that does
-      tok = 0;
-      for (int v = min(V, (s_pick + 1) * seg); v < V; ++v)
-        if (mass(v, s_resid != 0) > 0.0) { tok = v; break; }
+    if (tok < 0) {
+      // rounding put the target at or past the end of the picked piece: the next token with mass, else the last one
+      for (int v = min(V, thi_of(s_pick, lo, hi, piece)); v < V && tok < 0; ++v)
+        if (mass(v, resid) > 0.0) tok = v;
+      for (int v = V - 1; v >= 0 && tok < 0; --v)
+        if (mass(v, resid) > 0.0) tok = v;
+      if (tok < 0) tok = 0;
     }
     bonus_token[b] = tok;
   }
