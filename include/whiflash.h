@@ -205,7 +205,7 @@ int wf_neural_route(wf_ctx* ctx, const void* hidden_final, const int32_t* q_indp
  *
  * wf_verify_attn_tree: as wf_verify_attn, but row i of sequence b sees keys 0..seq_len[b]-1 and
  * seq_len[b] + j for the set bits j of tree_mask[r0_b + i].  max_nodes <= 64;
- * B * ceil(max_nodes * group / 64) <= 1024.  workspace: wf_verify_attn_workspace_bytes(.., max_nodes).
+ * B * ceil(max_nodes * group / 128) <= 1024.  workspace: wf_verify_attn_workspace_bytes(.., max_nodes).
  *
  * wf_accept_tree_entropy_route: as wf_accept_entropy_route with the greedy tree walk (T3): from the root,
  * step to the lowest-index child whose token equals the argmax of the current node's logits, until none

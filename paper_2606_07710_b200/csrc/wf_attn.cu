@@ -51,18 +51,23 @@ struct AttnParams {
   unsigned int* counters;              // [B * Hkv] arrived | published << 16, self-resetting
 };
 
-template <int D>
+// TREE: the query tile has 128 rows (UMMA M = 128): two 64-row sub-blocks of a draft tree stacked on the TMEM lanes, rows
+// of sub-block A on lanes 32w..32w+15 and of sub-block B on lanes 32w+16..32w+31 of every warp quadrant w, so that softmax
+// group 0 works on A and group 1 on B of the SAME K/V tile with the chain kernel's fragment code (M = 64 puts its rows on
+// lanes 32w..32w+15 as well).  One P buffer of 128 rows, S and O double buffered over the tiles.
+template <int D, bool TREE>
 struct AttnCfg {
   static constexpr int NH = D / 64;                         // 64-element (128-byte) column halves of a K/V row
-  static constexpr int Q_HALF = AT_ROWS * 128;              // 64 rows x 128 B
+  static constexpr int Q_ROWS = TREE ? 128 : AT_ROWS;
+  static constexpr int Q_HALF = Q_ROWS * 128;               // rows x 128 B: one 64-column half of the Q (or P) tile
   static constexpr int Q_BYTES = NH * Q_HALF;
-  static constexpr int P_BYTES = 2 * Q_HALF;                // 2 key halves x 64 rows x 128 B
+  static constexpr int P_BYTES = 2 * Q_HALF;                // 2 key halves x rows x 128 B
   static constexpr int KV_HALF = AT_BN * 128;               // one column half of a K (or V) tile: 16 KB
   static constexpr int K_BYTES = NH * KV_HALF;               // one K (or V) tile
-  static constexpr int STAGES_K = D == 128 ? 3 : 4;          // K ring
-  static constexpr int STAGES_V = D == 128 ? 2 : 4;          // V ring
-  // smem map: P0 | Q | P1 | K ring | V ring   (Q + P1 double as the group-merge buffer)
-  static constexpr int SMEM = Q_BYTES + 2 * P_BYTES + (STAGES_K + STAGES_V) * K_BYTES;
+  static constexpr int STAGES_K = D == 128 ? (TREE ? 2 : 3) : 4;          // K ring
+  static constexpr int STAGES_V = D == 128 ? 2 : 4;                       // V ring
+  // smem map, chain: P0 | Q | P1 | K ring | V ring (Q + P1 double as the group-merge buffer); tree: P | Q | K | V
+  static constexpr int SMEM = Q_BYTES + (TREE ? 1 : 2) * P_BYTES + (STAGES_K + STAGES_V) * K_BYTES;
   static constexpr uint32_t TM_S = 0, TM_O = 2 * AT_BN;     // TMEM columns: S0, S1, then O0, O1
 };
 
@@ -162,7 +167,7 @@ __device__ __forceinline__ int cta_of_tile(int x, int T, int G) {      // larges
 // K and V have separate rings so that a K tile is released as soon as its QK^T retires: more bytes in flight.
 template <int D, bool TREE>
 __device__ __forceinline__ void attn_loader(const AttnParams& p, AttnShared<TREE>& sh, uint8_t* ring, int which, int lane) {
-  using C = AttnCfg<D>;
+  using C = AttnCfg<D, TREE>;
   const KvView& kv = p.kv;
   uint64_t* full = which ? sh.v_full : sh.k_full;
   uint64_t* empty = which ? sh.v_empty : sh.k_empty;
@@ -217,8 +222,8 @@ __device__ __forceinline__ void attn_loader(const AttnParams& p, AttnShared<TREE
 template <int D, bool TREE>
 __device__ __forceinline__ void attn_mma_qk(const AttnParams& p, AttnShared<TREE>& sh, uint8_t* q_s, uint8_t* k_s,
                                             uint32_t tmem_base) {
-  using C = AttnCfg<D>;
-  const uint32_t idesc_qk = umma_idesc_kk(AT_ROWS, AT_BN);
+  using C = AttnCfg<D, TREE>;
+  const uint32_t idesc_qk = umma_idesc_kk(C::Q_ROWS, AT_BN);
   const uint64_t dq0 = umma_desc(smem_u32(q_s), 16, 1024);                  // K-major
   const uint64_t dk0 = umma_desc(smem_u32(k_s), 16, 1024);                  // K-major
   SegWalker<TREE> walk(sh, p.kv.n_kv_heads, blockIdx.x);
@@ -250,8 +255,8 @@ __device__ __forceinline__ void attn_mma_qk(const AttnParams& p, AttnShared<TREE
 template <int D, bool TREE>
 __device__ __forceinline__ void attn_mma_pv(const AttnParams& p, AttnShared<TREE>& sh, uint8_t* p0_s, uint8_t* p1_s,
                                             uint8_t* v_s, uint32_t tmem_base) {
-  using C = AttnCfg<D>;
-  const uint32_t idesc_pv = umma_idesc(AT_ROWS, D);
+  using C = AttnCfg<D, TREE>;
+  const uint32_t idesc_pv = umma_idesc(C::Q_ROWS, D);
   const uint64_t dp0 = umma_desc(smem_u32(p0_s), 16, 1024);                 // K-major
   const uint64_t dp1 = umma_desc(smem_u32(p1_s), 16, 1024);
   const uint64_t dv0 = umma_desc(smem_u32(v_s), C::KV_HALF, 1024);          // MN-major
@@ -262,12 +267,13 @@ __device__ __forceinline__ void attn_mma_pv(const AttnParams& p, AttnShared<TREE
     for (int t = 0; t < sg.n_tiles; ++t, ++gt) {
       const int st = gt % C::STAGES_V, g = gt & 1;
       mbar_wait(smem_u32(&sh.v_full[st]), (gt / C::STAGES_V) & 1);
-      mbar_wait(smem_u32(&sh.p_full[g]), (gt >> 1) & 1);
+      if constexpr (TREE) mbar_wait(smem_u32(&sh.p_full[0]), gt & 1);       // one P buffer, one phase per tile
+      else mbar_wait(smem_u32(&sh.p_full[g]), (gt >> 1) & 1);
       mbar_wait(smem_u32(&sh.o_empty[g]), ((gt >> 1) & 1) ^ 1);
       tc_fence_after();
       if (elect_one()) {
         const uint64_t dv = dv0 + (uint64_t)((st * C::K_BYTES) >> 4);
-        const uint64_t dp = g ? dp1 : dp0;
+        const uint64_t dp = (!TREE && g) ? dp1 : dp0;
         const uint32_t td = tmem_base + C::TM_O + g * D;
 #pragma unroll
         for (int k16 = 0; k16 < AT_BN / 16; ++k16)
@@ -293,7 +299,7 @@ __device__ __forceinline__ void tmem_ld_frag(uint32_t taddr, uint32_t (&v)[N]) {
 template <int D, bool TREE>
 __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared<TREE>& sh, uint8_t* q_s, uint8_t* p0_s, uint8_t* p1_s,
                                              uint8_t* v_s, uint32_t tmem_base, int warp, int lane) {
-  using C = AttnCfg<D>;
+  using C = AttnCfg<D, TREE>;
   constexpr int NO = D / 2;                                    // O registers per thread (2 rows x D/4 columns)
   const int Hkv = p.kv.n_kv_heads;
   const int grp = warp >> 2, qw = warp & 3;                    // group, TMEM lane quarter
@@ -635,16 +641,268 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared<TRE
   }
 }
 
+// ================= TREE: warps 0-3 (sub-block A) and 4-7 (sub-block B) on the same K/V tile =================
+// Group g owns the 64 rows of sub-block g of the 128-row tile (TMEM lanes 32w + 16g .. +15 of quadrant w) for EVERY tile
+// of the segment: running (m, l, O) per group, no hand-over between the groups; S and O alternate between two TMEM
+// buffers from tile to tile, P has one 128-row buffer (the store of P(t) waits for PV(t-1)).  Fragment code, mask,
+// partial publishing and the last-arriver fold are those of the chain kernel; a partial slot is (CTA slot, group).
+template <int D>
+__device__ __forceinline__ void attn_softmax_tree(const AttnParams& p, AttnShared<true>& sh, uint8_t* q_s, uint8_t* p_s,
+                                                  uint8_t* v_s, uint32_t tmem_base, int warp, int lane) {
+  using C = AttnCfg<D, true>;
+  constexpr int NO = D / 2;                                    // O registers per thread (2 rows x D/4 columns)
+  const int Hkv = p.kv.n_kv_heads;
+  const int grp = warp >> 2, qw = warp & 3;                    // sub-block, TMEM lane quarter
+  const int stid = qw * 32 + lane;                             // 0..127 inside the group
+  const int rw = lane >> 2, cq = (lane & 3) * 2;               // row within the 8-row group, first column of the pair
+  const int row_lo = qw * 16 + rw;                             // this thread's rows of the sub-block: row_lo and row_lo + 8
+  const int trow = qw * 32 + grp * 16 + rw;                    // the same row in the 128-row tile (and + 8)
+  const uint32_t t_lane = tmem_base + ((uint32_t)(qw * 32 + grp * 16) << 16);
+  const int npt = AT_ROWS / p.group;                           // nodes per sub-block
+  const int T = sh.total_tiles, G = sh.g_eff;
+  SegWalker<true> walk(sh, p.kv.n_kv_heads, blockIdx.x);
+  Segment sg;
+  uint32_t gt0 = 0;                                            // global tile counter at the start of the segment
+  while (walk.next(sg)) {
+    const int n_mine = max(0, min(sg.q_b - grp * npt, npt));   // nodes of this group's sub-block
+    const int R = n_mine * p.group;                            // its live rows
+    const int node0 = sg.r0 + grp * npt;                       // its first node's row in q / out / tree_mask
+    {
+      SegWalker<true> peek = walk;                             // next segment's Q rows -> L2 (see the chain kernel)
+      Segment nx;
+      if (peek.next(nx)) {
+        const int lines_per_tok = p.group * D * 2 / 128;
+        const int idx = grp * 128 + stid;
+        if (idx < nx.q_b * lines_per_tok) {
+          const char* a = reinterpret_cast<const char*>(p.q + ((size_t)(nx.r0 + idx / lines_per_tok) * p.n_q_heads + nx.g * p.group) * D) +
+                          (idx % lines_per_tok) * 128;
+          asm volatile("prefetch.global.L2 [%0];" ::"l"(a));
+        }
+      }
+    }
+    // ---- Q tile -> smem: 128 rows (K-major, 128-byte swizzle) by both groups; padding rows are zero.  Every MMA of the
+    //      previous segment has retired (both groups waited for the last pv_done). ----
+    {
+      constexpr int NQ = 128 * (D / 8) / 256;
+      uint4 qv[NQ];
+#pragma unroll
+      for (int u = 0; u < NQ; ++u) {
+        const int c = grp * 128 + stid + u * 256;
+        const int tr = c / (D / 8), chn = c % (D / 8);         // tile row -> (quadrant, sub-block, row in the 16)
+        const int rr = (tr >> 5) * 16 + (tr & 15), sb = (tr >> 4) & 1;
+        const int node = sb * npt + rr / p.group, h2 = rr % p.group;
+        qv[u] = make_uint4(0, 0, 0, 0);
+        if (node < sg.q_b)
+          qv[u] = __ldg(reinterpret_cast<const uint4*>(p.q + ((size_t)(sg.r0 + node) * p.n_q_heads + sg.g * p.group + h2) * D) + chn);
+      }
+#pragma unroll
+      for (int u = 0; u < NQ; ++u) {
+        const int c = grp * 128 + stid + u * 256;
+        const int tr = c / (D / 8), chn = c % (D / 8);
+        *reinterpret_cast<uint4*>(q_s + (chn >> 3) * C::Q_HALF + tr * 128 + (((chn & 7) ^ (tr & 7)) << 4)) = qv[u];
+      }
+    }
+    fence_proxy_async();
+    mbar_arrive(smem_u32(&sh.q_ready));
+
+    float m_run[2] = {-INFINITY, -INFINITY}, l_run[2] = {0.f, 0.f}, alpha_prev[2] = {0.f, 0.f};
+    float o[NO];
+#pragma unroll
+    for (int c = 0; c < NO; ++c) o[c] = 0.f;
+    unsigned long long anc[2] = {0ull, 0ull};                  // ancestor masks of this thread's two rows (0: padding row)
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+      const int node = (row_lo + 8 * h) / p.group;
+      if (node < n_mine) anc[h] = __ldg(p.tree_mask + node0 + node);
+    }
+
+    auto fold_o = [&](uint32_t gprev) {                        // o = o * alpha_prev + O_tile of tile gprev
+      uint32_t v[NO];
+      tmem_ld_frag<NO>(t_lane + C::TM_O + (gprev & 1) * D, v);
+      tmem_ld_wait();
+      tc_fence_before();
+      mbar_arrive(smem_u32(&sh.o_empty[gprev & 1]));
+#pragma unroll
+      for (int c = 0; c < NO; ++c) o[c] = fmaf(o[c], alpha_prev[(c >> 1) & 1], __uint_as_float(v[c]));
+    };
+
+    for (int t = 0; t < sg.n_tiles; ++t) {
+      const uint32_t g2 = gt0 + t;
+      const int sb = g2 & 1;
+      const int tk0 = sg.k0 + t * AT_BN;
+      mbar_wait(smem_u32(&sh.s_full[sb]), (g2 >> 1) & 1);
+      tc_fence_after();
+      uint32_t sv[64];
+      tmem_ld_16x256b_x16(t_lane + C::TM_S + sb * AT_BN, sv);
+      tmem_ld_wait();
+      tc_fence_before();
+      mbar_arrive(smem_u32(&sh.s_empty[sb]));                  // S buffer may be overwritten by QK(g2 + 2)
+
+      if (tk0 + AT_BN > sg.ctx) {                              // the tile holds tree keys (or the tail beyond them)
+        const int rel0 = tk0 + cq - sg.ctx;
+#pragma unroll
+        for (int c = 0; c < 64; ++c) {
+          const int rel = rel0 + (c >> 2) * 8 + (c & 1);
+          const bool vis = rel < 0 || (rel < 64 && ((anc[(c >> 1) & 1] >> (rel & 63)) & 1ull));
+          if (!vis) sv[c] = 0xff800000u;                       // -inf
+        }
+      }
+      float mx[2] = {-INFINITY, -INFINITY};
+#pragma unroll
+      for (int c = 0; c < 64; ++c) mx[(c >> 1) & 1] = fmaxf(mx[(c >> 1) & 1], __uint_as_float(sv[c]));
+      float alpha[2], m_use[2], rs[2] = {0.f, 0.f};
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        mx[h] = fmaxf(mx[h], __shfl_xor_sync(0xffffffffu, mx[h], 1));
+        mx[h] = fmaxf(mx[h], __shfl_xor_sync(0xffffffffu, mx[h], 2));
+        const float m_new = fmaxf(m_run[h], mx[h] * p.scale_log2);
+        m_use[h] = m_new == -INFINITY ? 0.f : m_new;
+        alpha[h] = fast_exp2(m_run[h] - m_use[h]);
+        m_run[h] = m_new;
+      }
+      uint32_t pk[32];
+#pragma unroll
+      for (int c = 0; c < 64; c += 2) {
+        const int h = (c >> 1) & 1;
+        const float p0 = fast_exp2(fmaf(__uint_as_float(sv[c]), p.scale_log2, -m_use[h]));
+        const float p1 = fast_exp2(fmaf(__uint_as_float(sv[c + 1]), p.scale_log2, -m_use[h]));
+        rs[h] += p0 + p1;
+        pk[c >> 1] = pack_bf16(p0, p1);
+      }
+      l_run[0] = l_run[0] * alpha[0] + rs[0];
+      l_run[1] = l_run[1] * alpha[1] + rs[1];
+
+      // P(t) overwrites P(t-1): wait for PV(t-1) (it also makes O(t-1) ready and, the pipe being in order, every
+      // earlier PV retired: the V stage of this tile holds no older tile any more)
+      if (t > 0) mbar_wait(smem_u32(&sh.pv_done[(g2 - 1) & 1]), ((g2 - 1) >> 1) & 1);
+      if (tk0 + AT_BN > sg.k1 && grp == 0) {
+        // Last tile of the sequence: keys >= k1 hold stale or never-written V bits; zero them so that 0 * garbage cannot
+        // produce NaN in the PV product (P is exactly 0 there).  Group 0 does it; PV waits for all 256 P arrivals.
+        mbar_wait(smem_u32(&sh.v_full[g2 % C::STAGES_V]), (g2 / C::STAGES_V) & 1);
+        const int key = (sg.k1 - tk0) + stid;
+        if (key < AT_BN) {
+          uint8_t* vrow = v_s + (size_t)(g2 % C::STAGES_V) * C::K_BYTES + key * 128;
+#pragma unroll
+          for (int h = 0; h < C::NH; ++h)
+#pragma unroll
+            for (int c = 0; c < 8; ++c) *reinterpret_cast<uint4*>(vrow + h * C::KV_HALF + c * 16) = make_uint4(0, 0, 0, 0);
+        }
+      }
+#pragma unroll
+      for (int j = 0; j < 16; ++j) {                           // P -> smem, K-major 128-byte swizzle, rows trow and trow + 8
+        const uint32_t off = (j >> 3) * C::Q_HALF + (((j & 7) ^ (rw & 7)) << 4) + cq * 2;
+        *reinterpret_cast<uint32_t*>(p_s + off + trow * 128) = pk[2 * j];
+        *reinterpret_cast<uint32_t*>(p_s + off + (trow + 8) * 128) = pk[2 * j + 1];
+      }
+      fence_proxy_async();
+      mbar_arrive(smem_u32(&sh.p_full[0]));
+      if (t > 0) { tc_fence_after(); fold_o(g2 - 1); }
+      alpha_prev[0] = alpha[0];
+      alpha_prev[1] = alpha[1];
+    }
+    {
+      const uint32_t gl = gt0 + sg.n_tiles - 1;
+      mbar_wait(smem_u32(&sh.pv_done[gl & 1]), (gl >> 1) & 1);
+      tc_fence_after();
+      fold_o(gl);
+    }
+    gt0 += sg.n_tiles;
+
+    // ---- finish the rows: quad-reduce the row sums, write final rows or the partial ----
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+      l_run[h] += __shfl_xor_sync(0xffffffffu, l_run[h], 1);
+      l_run[h] += __shfl_xor_sync(0xffffffffu, l_run[h], 2);
+    }
+    auto write_rows = [&]() {                                  // normalise and store this thread's two rows
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        const int r = row_lo + 8 * h;
+        if (r >= R) continue;
+        const float inv = 1.f / l_run[h];                      // every live row sees itself: l > 0
+        const int qi = r / p.group, hg = r % p.group;
+        __nv_bfloat16* dst = p.out + ((size_t)(node0 + qi) * p.n_q_heads + sg.g * p.group + hg) * D + cq;
+#pragma unroll
+        for (int j = 0; j < D / 8; ++j)
+          *reinterpret_cast<uint32_t*>(dst + 8 * j) = pack_bf16(o[4 * j + 2 * h] * inv, o[4 * j + 2 * h + 1] * inv);
+      }
+    };
+    if (!sg.partial) { write_rows(); continue; }
+
+    // ---- the pair is shared with other CTAs: last-arriver fold as in the chain kernel, both groups in step ----
+    unsigned int* cnt = p.counters + sg.pb * Hkv + sg.g;
+    const int c_first = cta_of_tile(sg.flat0 + AT_SEG_COST, T, G);
+    const int n_seg = cta_of_tile(sg.flat0 + AT_SEG_COST + sg.nt - 1, T, G) - c_first + 1;
+    if (grp == 0 && stid == 0) {
+      const unsigned int arrive_old = atomicAdd(cnt, 1u);
+      sh.last = (arrive_old & 0xffffu) == (unsigned int)n_seg - 1 ? 1 + (int)(arrive_old >> 16) : 0;
+    }
+    named_bar_sync(3, 256);
+    const int last = sh.last;                                  // 0: not last; else 1 + partials already published
+    if (!last) {
+      float4* dst = p.ws_o + (size_t)(sg.slot * 2 + grp) * (NO / 4) * 128 + stid;
+#pragma unroll
+      for (int k = 0; k < NO / 4; ++k) dst[k * 128] = make_float4(o[4 * k], o[4 * k + 1], o[4 * k + 2], o[4 * k + 3]);
+      p.ws_ml[(size_t)(sg.slot * 2 + grp) * 128 + stid] = make_float4(m_run[0], l_run[0], m_run[1], l_run[1]);
+      __threadfence();
+      named_bar_sync(3, 256);                                  // also: sh.last may be rewritten
+      if (grp == 0 && stid == 0) atomicAdd(cnt, 0x10000u);
+      continue;
+    }
+    if (last - 1 < n_seg - 1) {                                // rare: somebody arrived but has not published yet
+      if (grp == 0 && stid == 0) {
+        for (uint32_t spins = 0; (atomicAdd(cnt, 0u) >> 16) < (unsigned int)n_seg - 1; ++spins)
+          if (spins > (1u << 24)) __trap();
+      }
+    }
+    named_bar_sync(3, 256);                                    // also: sh.last may be rewritten
+    if (grp == 0 && stid == 0) *cnt = 0;                       // self-resetting for the next launch
+    __threadfence();
+    const int first_slot = 2 * c_first + ((int)((long long)c_first * T / G) < sg.flat0 ? 1 : 0);
+    const int s_own = (int)blockIdx.x - c_first;
+    for (int s2 = 0; s2 < n_seg; ++s2) {
+      if (s2 == s_own) continue;
+      const int slot = (s2 == 0 ? first_slot : 2 * (c_first + s2)) * 2 + grp;
+      const float4* src = p.ws_o + (size_t)slot * (NO / 4) * 128 + stid;
+      float4 x[NO / 4];
+#pragma unroll
+      for (int k = 0; k < NO / 4; ++k) x[k] = __ldcg(src + k * 128);
+      const float4 ml = __ldcg(&p.ws_ml[(size_t)slot * 128 + stid]);
+      float e0[2], e1[2];
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        const float m1 = h ? ml.z : ml.x, l1 = h ? ml.w : ml.y;
+        const float m = fmaxf(m_run[h], m1);
+        const float mu = m == -INFINITY ? 0.f : m;
+        e0[h] = fast_exp2(m_run[h] - mu);
+        e1[h] = fast_exp2(m1 - mu);
+        l_run[h] = l_run[h] * e0[h] + l1 * e1[h];
+        m_run[h] = m;
+      }
+#pragma unroll
+      for (int k = 0; k < NO / 4; ++k) {
+        const float xv[4] = {x[k].x, x[k].y, x[k].z, x[k].w};
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          const int c = 4 * k + u;
+          o[c] = o[c] * e0[(c >> 1) & 1] + xv[u] * e1[(c >> 1) & 1];
+        }
+      }
+    }
+    write_rows();
+  }
+}
+
 template <int D, bool TREE>
 __global__ void __launch_bounds__(AT_THREADS, 1) wf_verify_attn_kernel(const AttnParams p) {
-  using C = AttnCfg<D>;
+  using C = AttnCfg<D, TREE>;
   extern __shared__ __align__(1024) uint8_t smem[];
   __shared__ __align__(8) AttnShared<TREE> sh;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   uint8_t* p0_s = smem;                                        // smem map: P0 | Q | P1 | K ring | V ring
   uint8_t* q_s = p0_s + C::P_BYTES;
   uint8_t* p1_s = q_s + C::Q_BYTES;
-  uint8_t* k_s = p1_s + C::P_BYTES;
+  uint8_t* k_s = p1_s + (TREE ? 0 : C::P_BYTES);             // TREE: one P buffer (p0_s), no p1_s
   uint8_t* v_s = k_s + C::STAGES_K * C::K_BYTES;
 
   // barrier init and TMEM allocation touch no global memory: they run before the dependency wait and overlap the
@@ -657,9 +915,9 @@ __global__ void __launch_bounds__(AT_THREADS, 1) wf_verify_attn_kernel(const Att
     }
     for (int i = 0; i < 2; ++i) {
       mbar_init(smem_u32(&sh.s_full[i]), 1);
-      mbar_init(smem_u32(&sh.s_empty[i]), 128);
-      mbar_init(smem_u32(&sh.o_empty[i]), 128);
-      mbar_init(smem_u32(&sh.p_full[i]), 128);
+      mbar_init(smem_u32(&sh.s_empty[i]), TREE ? 256 : 128);   // TREE: both groups read every S, O and write every P
+      mbar_init(smem_u32(&sh.o_empty[i]), TREE ? 256 : 128);
+      mbar_init(smem_u32(&sh.p_full[i]), TREE ? 256 : 128);
       mbar_init(smem_u32(&sh.pv_done[i]), 1);
     }
     mbar_init(smem_u32(&sh.q_ready), 256);
@@ -694,12 +952,12 @@ __global__ void __launch_bounds__(AT_THREADS, 1) wf_verify_attn_kernel(const Att
   if (warp == 0) {                                             // in-place scan of the tile counts, 32 sequences per step
     int n_tab = p.B;                                           // table entries
     if constexpr (TREE) {
-      // Sub-block s of sequence b = nodes [s * npt, (s+1) * npt), npt = 64 / group nodes = one query tile.  Each
-      // sub-block is a pair of its own that streams the sequence's whole KV; the table lists them LEVEL-MAJOR
-      // (all first sub-blocks, then all second ones, ...): with equal trees the level copies of a (b, g) pair
+      // Block s of sequence b = nodes [s * npt, (s+1) * npt), npt = 2 * 64 / group nodes = one 128-row query tile
+      // (two sub-blocks).  Each block is a pair of its own that streams the sequence's whole KV; the table lists them
+      // LEVEL-MAJOR (all first blocks, then all second ones, ...): with equal trees the level copies of a (b, g) pair
       // sit T / levels positions apart, i.e. in CTAs c, c + G / levels, ... at the same offset of their ranges,
       // which stream the same K/V tiles at the same time: HBM serves one of them, L2 the rest.
-      const int npt = AT_ROWS / p.group;
+      const int npt = 2 * (AT_ROWS / p.group);                // nodes per 128-row tile (two sub-blocks)
       int cursor = 0;
       for (int s0 = 0; s0 < 64; s0 += npt) {
         const int before = cursor;
@@ -768,7 +1026,8 @@ __global__ void __launch_bounds__(AT_THREADS, 1) wf_verify_attn_kernel(const Att
   if (sh.total_tiles > 0 && (int)blockIdx.x < sh.g_eff) {
     if (warp < 8) {
       asm volatile("setmaxnreg.inc.sync.aligned.u32 216;");
-      attn_softmax<D, TREE>(p, sh, q_s, p0_s, p1_s, v_s, tmem_base, warp, lane);
+      if constexpr (TREE) attn_softmax_tree<D>(p, sh, q_s, p0_s, v_s, tmem_base, warp, lane);
+      else attn_softmax<D, TREE>(p, sh, q_s, p0_s, p1_s, v_s, tmem_base, warp, lane);
     } else {
       asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
       if (warp == 8) attn_loader<D, TREE>(p, sh, k_s, 0, lane);
@@ -792,7 +1051,7 @@ namespace {
 template <int D, bool TREE>
 int launch_attn(wf_ctx* ctx, const AttnParams& p, cudaStream_t st) {
   static bool configured = false;
-  const size_t smem = AttnCfg<D>::SMEM;
+  const size_t smem = AttnCfg<D, TREE>::SMEM;
   if (!configured) {
     WF_CUDA(ctx, cudaFuncSetAttribute(wf_verify_attn_kernel<D, TREE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     configured = true;
@@ -831,7 +1090,7 @@ __global__ void __launch_bounds__(64) wf_tree_masks_kernel(const int32_t* parent
 
 extern "C" size_t wf_verify_attn_workspace_bytes(const wf_kv_shape* s, int B, int n_q_heads, int max_q_len) {
   if (!s || B <= 0 || n_q_heads <= 0 || s->n_kv_heads <= 0) return 16;
-  const size_t items = 2 * (size_t)AT_MAX_CTAS;            // a CTA writes at most a head and a tail partial
+  const size_t items = 4 * (size_t)AT_MAX_CTAS;            // a CTA writes at most a head and a tail partial (tree: per group)
   const size_t r_pad = AT_ROWS;
   return items * (r_pad * (size_t)s->head_dim * sizeof(float) + 128 * sizeof(float4));
 }
@@ -855,7 +1114,7 @@ extern "C" int wf_verify_attn(wf_ctx* ctx, const wf_paged_kv* kv, int layer, con
              WF_ERR_INVALID_ARG, "wf_verify_attn: q/out/workspace must be 16-byte aligned");
   if (B == 0) return WF_OK;
   const int r_pad = AT_ROWS;
-  const size_t items = 2 * (size_t)AT_MAX_CTAS;
+  const size_t items = 4 * (size_t)AT_MAX_CTAS;
   AttnParams p;
   p.q = (const __nv_bfloat16*)q;
   p.out = (__nv_bfloat16*)out;
@@ -896,18 +1155,18 @@ extern "C" int wf_verify_attn_tree(wf_ctx* ctx, const wf_paged_kv* kv, int layer
   const int group = n_q_heads / kv->s.n_kv_heads;
   WF_REQUIRE(ctx, group <= 64 && max_nodes >= 1 && max_nodes <= 64, WF_ERR_UNSUPPORTED_SHAPE,
              "wf_verify_attn_tree: max_nodes must be in [1, 64] and the GQA group <= 64");
-  const int npt = AT_ROWS / group;                           // nodes per 64-row query tile
-  const int levels = (max_nodes + npt - 1) / npt;            // sub-blocks per tree
+  const int npt = 2 * (AT_ROWS / group);                     // nodes per 128-row query tile (two 64-row sub-blocks)
+  const int levels = (max_nodes + npt - 1) / npt;            // tiles per tree
   WF_REQUIRE(ctx, B >= 0 && B <= kv->s.max_seqs && (long long)B * levels <= AT_MAX_B &&
                       (long long)B * levels * kv->s.n_kv_heads <= ctx->n_counters,
-             WF_ERR_INVALID_ARG, "wf_verify_attn_tree: B * ceil(max_nodes * group / 64) must be <= %d", AT_MAX_B);
+             WF_ERR_INVALID_ARG, "wf_verify_attn_tree: B * ceil(max_nodes * group / 128) must be <= %d", AT_MAX_B);
   WF_REQUIRE(ctx, workspace_bytes >= wf_verify_attn_workspace_bytes(&kv->s, B, n_q_heads, max_nodes),
              WF_ERR_INVALID_ARG, "wf_verify_attn_tree: workspace too small");
   WF_REQUIRE(ctx, ((uintptr_t)q % 16 == 0) && ((uintptr_t)out % 16 == 0) && ((uintptr_t)workspace % 16 == 0) &&
                       ((uintptr_t)tree_mask % 8 == 0),
              WF_ERR_INVALID_ARG, "wf_verify_attn_tree: q/out/workspace must be 16-byte aligned");
   if (B == 0) return WF_OK;
-  const size_t items = 2 * (size_t)AT_MAX_CTAS;
+  const size_t items = 4 * (size_t)AT_MAX_CTAS;
   AttnParams p;
   p.q = (const __nv_bfloat16*)q;
   p.out = (__nv_bfloat16*)out;
