@@ -459,11 +459,15 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared<TRE
         }
       }
       if (pending) mbar_wait(smem_u32(&sh.pv_done[grp]), (g_prev >> 1) & 1);   // own PV retired: P is free, O is ready
+      {
+        // P -> smem, K-major 128-byte swizzle.  The fragment is four 8x8 matrices per pair of 16-byte chunks (rows 0-7 /
+        // 8-15 of the warp's 16, chunks j / j+1): one stmatrix.x4 each instead of four 4-byte stores per thread.
+        const int mi = lane >> 3, r8 = lane & 7;
+        const uint32_t prow = smem_u32(p_s) + (uint32_t)(qw * 16 + (mi & 1) * 8 + r8) * 128;
 #pragma unroll
-      for (int j = 0; j < 16; ++j) {                           // P -> smem, K-major 128-byte swizzle
-        const uint32_t off = (j >> 3) * C::Q_HALF + (((j & 7) ^ (rw & 7)) << 4) + cq * 2;
-        *reinterpret_cast<uint32_t*>(p_s + off + row_lo * 128) = pk[2 * j];
-        *reinterpret_cast<uint32_t*>(p_s + off + (row_lo + 8) * 128) = pk[2 * j + 1];
+        for (int j = 0; j < 16; j += 2)
+          stmatrix_x4(prow + (j >> 3) * C::Q_HALF + ((((j & 7) + (mi >> 1)) ^ r8) << 4), pk[2 * j], pk[2 * j + 1], pk[2 * j + 2],
+                      pk[2 * j + 3]);
       }
       fence_proxy_async();
       mbar_arrive(smem_u32(&sh.p_full[grp]));
@@ -656,7 +660,6 @@ __device__ __forceinline__ void attn_softmax_tree(const AttnParams& p, AttnShare
   const int stid = qw * 32 + lane;                             // 0..127 inside the group
   const int rw = lane >> 2, cq = (lane & 3) * 2;               // row within the 8-row group, first column of the pair
   const int row_lo = qw * 16 + rw;                             // this thread's rows of the sub-block: row_lo and row_lo + 8
-  const int trow = qw * 32 + grp * 16 + rw;                    // the same row in the 128-row tile (and + 8)
   const uint32_t t_lane = tmem_base + ((uint32_t)(qw * 32 + grp * 16) << 16);
   const int npt = AT_ROWS / p.group;                           // nodes per sub-block
   const int T = sh.total_tiles, G = sh.g_eff;
@@ -788,11 +791,14 @@ __device__ __forceinline__ void attn_softmax_tree(const AttnParams& p, AttnShare
             for (int c = 0; c < 8; ++c) *reinterpret_cast<uint4*>(vrow + h * C::KV_HALF + c * 16) = make_uint4(0, 0, 0, 0);
         }
       }
+      {
+        // P -> smem, K-major 128-byte swizzle, this warp's 16 rows of the 128-row tile: stmatrix.x4 per chunk pair
+        const int mi = lane >> 3, r8 = lane & 7;
+        const uint32_t prow = smem_u32(p_s) + (uint32_t)(qw * 32 + grp * 16 + (mi & 1) * 8 + r8) * 128;
 #pragma unroll
-      for (int j = 0; j < 16; ++j) {                           // P -> smem, K-major 128-byte swizzle, rows trow and trow + 8
-        const uint32_t off = (j >> 3) * C::Q_HALF + (((j & 7) ^ (rw & 7)) << 4) + cq * 2;
-        *reinterpret_cast<uint32_t*>(p_s + off + trow * 128) = pk[2 * j];
-        *reinterpret_cast<uint32_t*>(p_s + off + (trow + 8) * 128) = pk[2 * j + 1];
+        for (int j = 0; j < 16; j += 2)
+          stmatrix_x4(prow + (j >> 3) * C::Q_HALF + ((((j & 7) + (mi >> 1)) ^ r8) << 4), pk[2 * j], pk[2 * j + 1], pk[2 * j + 2],
+                      pk[2 * j + 3]);
       }
       fence_proxy_async();
       mbar_arrive(smem_u32(&sh.p_full[0]));

@@ -128,6 +128,11 @@ __device__ __forceinline__ void cp_async16_zfill(uint32_t dst, const void* src, 
   const int n = valid ? 16 : 0;
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(n) : "memory");
 }
+// four 8x8 b16 matrices from mma-C-fragment registers to shared memory: lane L supplies the address of row L & 7 of
+// matrix L >> 3 (16 bytes each); thread L holds row L / 4, columns 2 (L % 4) and + 1 of every matrix
+__device__ __forceinline__ void stmatrix_x4(uint32_t addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
+  asm volatile("stmatrix.sync.aligned.m8n8.x4.shared.b16 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
+}
 // 2^x on the SFU: one MUFU.EX2, flush-to-zero, ex2(-inf) = +0 (exp2f() adds range-scaling code around it)
 __device__ __forceinline__ float fast_exp2(float x) {
   float y;
