@@ -766,9 +766,13 @@ __device__ __forceinline__ void attn_softmax_tree(const AttnParams& p, AttnShare
       uint32_t pk[32];
 #pragma unroll
       for (int c = 0; c < 64; c += 2) {
+        // Both groups run this phase at the same time and the four MUFUs of a sub-partition are its bottleneck (64 ex2
+        // per thread and tile): every fourth pair is evaluated on the FMA pipe instead, which balances the two pipes.
         const int h = (c >> 1) & 1;
-        const float p0 = fast_exp2(fmaf(__uint_as_float(sv[c]), p.scale_log2, -m_use[h]));
-        const float p1 = fast_exp2(fmaf(__uint_as_float(sv[c + 1]), p.scale_log2, -m_use[h]));
+        const float x0 = fmaf(__uint_as_float(sv[c]), p.scale_log2, -m_use[h]);
+        const float x1 = fmaf(__uint_as_float(sv[c + 1]), p.scale_log2, -m_use[h]);
+        const float p0 = (c & 6) == 0 ? poly_exp2(x0) : fast_exp2(x0);
+        const float p1 = (c & 6) == 0 ? poly_exp2(x1) : fast_exp2(x1);
         rs[h] += p0 + p1;
         pk[c >> 1] = pack_bf16(p0, p1);
       }

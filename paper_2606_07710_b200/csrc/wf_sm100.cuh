@@ -128,6 +128,19 @@ __device__ __forceinline__ void cp_async16_zfill(uint32_t dst, const void* src, 
   const int n = valid ? 16 : 0;
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(n) : "memory");
 }
+// 2^x on the FMA pipe (no MUFU): round-to-nearest split x = n + f, |f| <= 0.5, degree-4 Taylor polynomial of 2^f
+// (relative error < 5e-5, far below the bf16 rounding of P), exponent added as an integer.  x <= 0 expected; anything
+// below -126 (including -inf) returns a denormal-scale value that flushes to 0 in the bf16 pack and the row sum.
+__device__ __forceinline__ float poly_exp2(float x) {
+  x = fmaxf(x, -126.f);
+  const float t = x + 12582912.f;                            // 1.5 * 2^23: n sits in the low mantissa bits
+  const float f = x - (t - 12582912.f);
+  float p = fmaf(f, 0.0096181291f, 0.0555041087f);
+  p = fmaf(p, f, 0.2402265070f);
+  p = fmaf(p, f, 0.6931471806f);
+  p = fmaf(p, f, 1.0f);
+  return __int_as_float(__float_as_int(p) + (__float_as_int(t) << 23));
+}
 // four 8x8 b16 matrices from mma-C-fragment registers to shared memory: lane L supplies the address of row L & 7 of
 // matrix L >> 3 (16 bytes each); thread L holds row L / 4, columns 2 (L % 4) and + 1 of every matrix
 __device__ __forceinline__ void stmatrix_x4(uint32_t addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
