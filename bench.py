@@ -29,7 +29,7 @@ from paper_2606_07710_b200 import synth  # noqa: E402
 WORKLOADS = {"cfg1": 0, "cfg2": 1, "cfg3": 2, "cfg4": 3, "cfg5": 4}
 # dram__bytes_read.sum + dram__bytes_write.sum per attention launch from the committed `ncu --set full` capture
 # (profiles/r1e_final_cfg3.md); workloads without a capture report null
-NCU_TRAFFIC_BYTES = {"cfg3": 553.0e6}
+NCU_TRAFFIC_BYTES = {"cfg3": 552.5e6}
 METRIC = "verify_rounds_per_s"
 UNIT = "rounds/s"
 
@@ -517,7 +517,7 @@ def run_ours(args):
                 "kv_read_gbs": float(np.mean(t_bytes)) / (tree_attn_ms / (tree_steps * L) * 1e-3) / 1e9,
                 "committed_tokens_per_round": float(t_commit.sum()),
                 "note": "all sequences AR-routed with depth-8 / top-k-10 / 60-node trees (PAPER.md:317); 240 query rows per "
-                        "kv head = 4 sub-blocks that stream the same K/V (HBM once, L2 for the rest)"}
+                        "kv head = two 128-row query tiles (UMMA M = 128) that stream the same K/V (HBM once, L2 for the second)"}
 
     if rank == 0:
         peak, peak_src = measured_peaks()
@@ -544,7 +544,7 @@ def run_ours(args):
             "roofline": {"bound": "hbm", "kernel": "wf_verify_attn_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
                          "frac": achieved / peak, "peak_source": peak_src,
                          "traffic": args.traffic_bytes if args.traffic_bytes is not None else NCU_TRAFFIC_BYTES.get(args.workload),
-                         "traffic_source": "profiles/r1e_final_cfg3.md",
+                         "traffic_source": "profiles/r1g_final.md",
                          "algorithmic_bytes_per_launch": float(np.mean(attn_bytes)), "avg_launch_us": 1e3 * avg_launch_ms},
             "e2e": {"value": world * e2e_steps / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d // e2e_steps,
                     "d2h_bytes_per_step": d2h // e2e_steps, "steps": e2e_steps,
