@@ -63,3 +63,54 @@ def test_attention_full_size_sampled(workload, sample):
     finally:
         rs.close()
         ctx.close()
+
+
+@pytest.mark.parametrize("workload,sample", [(2, (0, 6, 15)), (4, (3, 40, 63))])
+def test_tree_attention_full_size_sampled(workload, sample):
+    """The tree launch bench.py times (60-node trees for every sequence at configs[2] / configs[4] shapes, one layer):
+    every SM busy, the two 128-row tiles of a tree in different CTAs, pairs cut by stream-K ranges, repeated launches.
+    Checked per (sequence, kv head) pair against oracle O7 on sampled sequences (all 60 rows)."""
+    import torch
+    from oracle import tree_verify
+    from oracle.paged_kv import PagedKV
+    from paper_2606_07710_b200 import binding as wf
+    from paper_2606_07710_b200.rounds import RoundState
+    wl = synth.WORKLOADS[workload]
+    sh = wl.shapes
+    ctx = wf.Ctx(0)
+    rs = RoundState(ctx, wl, n_slots=1, n_rounds_max=6, layers=1)
+    try:
+        t = rs.make_tree_slot(60)
+        rs.target_kv.reserve(t.add_tokens, rs.B)
+        wf.wf_tree_masks(ctx, t.parent, t.q_indptr, rs.B, 60, t.masks)
+        torch.cuda.synchronize()
+        bits = lambda x: x.contiguous().view(torch.int16).cpu().numpy().view(np.uint16)
+        parent = t.parent.cpu().numpy()
+        want = {}
+        for b in sample:
+            ctx_b = int(rs.seq_len[b].item())
+            n_tok = ctx_b + 60
+            n_pg = -(-n_tok // sh.page_size)
+            pages = rs.block_table[b, :n_pg].long()
+            kv = PagedKV(1, sh.n_kv_heads, sh.head_dim, sh.page_size, n_pg, 1, n_pg)
+            kv.reserve([n_tok])
+            kv.k_pool[0, kv.block_table[0, :n_pg]] = bits(rs.k_pool[0][pages])
+            kv.v_pool[0, kv.block_table[0, :n_pg]] = bits(rs.v_pool[0][pages])
+            kv.seq_len[0] = ctx_b
+            r0 = int(t.q_indptr_host[b])
+            want[b] = tree_verify.tree_attn(kv, 0, bits(t.q[r0:r0 + 60]), np.array([0, 60], np.int32), parent[r0:r0 + 60],
+                                            sh.n_q_heads, rs.sm_scale)
+        for rep in range(3):
+            t.attn_out.zero_()
+            wf.wf_verify_attn_tree(ctx, rs.target_kv, 0, t.q, t.q_indptr, t.masks, rs.B, sh.n_q_heads, 60, rs.sm_scale,
+                                   t.attn_out, t.attn_ws)
+            torch.cuda.synchronize()
+            assert ctx.poll_status() == 0
+            for b in sample:
+                r0 = int(t.q_indptr_host[b])
+                got = t.attn_out[r0:r0 + 60].float().cpu().numpy().astype(np.float64)
+                for h, (max_abs, rel) in enumerate(_pair_errors(got, want[b], sh.n_kv_heads)):
+                    assert max_abs <= ATTN_MAX_ABS and rel <= ATTN_REL_L2, (rep, b, h, max_abs, rel)
+    finally:
+        rs.close()
+        ctx.close()
