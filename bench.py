@@ -303,7 +303,7 @@ def run_ours(args):
     K, W = args.steps, max(args.warmup, 3)
     e2e_steps = max(1, min(K, args.e2e_steps))
     eager_steps = 8
-    rs = RoundState(ctx, wl, n_slots=4, n_rounds_max=W + K + e2e_steps + eager_steps + 4 + 10, host_copies=True)   # + 10: pages for the tree leg
+    rs = RoundState(ctx, wl, n_slots=4, n_rounds_max=W + K + e2e_steps + eager_steps + 4 + 10 + 24, host_copies=True)   # + 10: tree leg, + 24: graph leg
     B, L = rs.B, rs.L
 
     # ---- cpu_baseline + full-size sampled parity (rank 0 of a 1-GPU run only) ----
@@ -379,6 +379,8 @@ def run_ours(args):
     ms = barrier_max(ms_local, world)
     rs.check_plan(s)
     attn_ms = sum(e["attn"][0].elapsed_time(e["attn"][1]) for e in evs)
+    # per-round spans from the per-part events (attention start of round i to attention start of round i+1)
+    spans = [evs[i]["attn"][0].elapsed_time(evs[i + 1]["attn"][0]) for i in range(K - 1)]
     catch_ms = sum(e["catchup"][0].elapsed_time(e["catchup"][1]) for e in evs)
     commits = float(np.mean([np.sum(sl.u + 1) for sl in rs.slots]))
 
@@ -446,6 +448,36 @@ def run_ours(args):
     torch.cuda.synchronize()
     eager_ms = g0.elapsed_time(g1)
     eager_catch_ms = sum(e["catchup"][0].elapsed_time(e["catchup"][1]) for e in ev_e)
+
+    # ---- the same round replayed from CUDA graphs (SURVEY.md §8(d) timing protocol): one graph per round slot, captured
+    #      from the very calls above (every argument is a device pointer or a constant; lengths live on the device) ----
+    graph_leg = None
+    try:
+        side = torch.cuda.Stream()
+        side.wait_stream(torch.cuda.current_stream())
+        graphs = []
+        for _ in range(rs.n_slots):
+            gph = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(gph, stream=side):
+                rs.run_round()
+            graphs.append(gph)
+        torch.cuda.synchronize()
+        g_steps = 20
+        for i in range(rs.n_slots):
+            graphs[i].replay()
+        torch.cuda.synchronize()
+        h0, h1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        h0.record()
+        for i in range(g_steps):
+            graphs[i % rs.n_slots].replay()
+        h1.record()
+        torch.cuda.synchronize()
+        rs.check_plan(rs.slots[(rs.rounds_done - 1) % rs.n_slots])
+        graph_leg = {"rounds_per_s": g_steps / (h0.elapsed_time(h1) * 1e-3), "steps": g_steps,
+                     "note": "whole round replayed from one CUDA graph per round slot, captured from the same C-ABI calls"}
+    except Exception as e:                                   # capture is optional evidence, never the headline
+        graph_leg = {"error": f"{type(e).__name__}: {e}"[:200]}
+        torch.cuda.synchronize()
 
     # ---- WhiFlash-Neural router, timed on its own: the round above uses the entropy policy ----
     n0, n1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -527,7 +559,7 @@ def run_ours(args):
         achieved = float(np.mean(attn_bytes)) / (avg_launch_ms * 1e-3) / 1e9
         line = {
             "metric": METRIC, "value": whole_job_value(K, world, ms), "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
-            "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
+            "ms_per_step": ms / K, "ms_per_step_median": float(np.median(spans)) if spans else ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
             "data": "synthetic",
             "config": {"workload": wl.name, "batch": B, "ctx": str(wl.ctx), "gammas": list(wl.gammas), "layers": L,
                        "vocab": sh.vocab, "backlog_cap": wl.backlog_cap, "parallelism": "replicas only" if world > 1 else "1 gpu",
@@ -560,6 +592,7 @@ def run_ours(args):
                                      "note": "speculative sampling (one-hot drafter, uniforms as inputs): same sweep over the "
                                              "logits plus one inverse-CDF draw per sequence; back-to-back calls on L2-cold-ish "
                                              "logits of the last slot, not part of the round"}
+        line["graph_replay"] = graph_leg
         if tree:
             line["tree_verify"] = tree
         if cpu_baseline:
