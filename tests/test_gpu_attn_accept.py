@@ -96,7 +96,7 @@ def _check_accept(res, want, tau):
     return int(near.sum())
 
 
-@pytest.mark.parametrize("seed", range(16))
+@pytest.mark.parametrize("seed", range(64))
 def test_accept_cfg1_tiny(wf, seed):
     """configs[0]: vocab 4096, gamma 7, planted prefix uniform 0..7, spike puts H on both sides of tau."""
     binding, ctx = wf
@@ -208,8 +208,8 @@ def _attn_case(wf, ctx_lens, q_lens, Hq, Hkv, D, seed, n_layers=1, layer=0, q_st
 
 
 def test_attn_cfg1_tiny(wf):
-    """configs[0]: 4 q / 2 kv heads, D 64, ctx 512, gamma 7."""
-    for seed in range(4):
+    """configs[0]: 4 q / 2 kv heads, D 64, ctx 512, gamma 7; 64 seeds."""
+    for seed in range(64):
         max_abs, rel = _attn_case(wf, [512], [8], 4, 2, 64, seed=synth.SEED_BASE + seed)
         assert max_abs <= ATTN_MAX_ABS and rel <= ATTN_REL_L2, (max_abs, rel)
 
