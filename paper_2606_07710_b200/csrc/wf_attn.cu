@@ -23,6 +23,12 @@
 //               with quad shuffles, P goes to smem as the bf16 A operand of the PV MMA, the per-tile
 //               O_t is folded into fp32 registers with the running rescale.  The next segment's Q rows
 //               are prefetched into L2; the Q tile is loaded with all loads ahead of the stores.
+//
+// Tree mode (wf_verify_attn_tree; template flag TREE, readings T1-T2): the draft tree of a
+// sequence (<= 64 nodes, one 64-bit ancestor mask per row) is cut into blocks of 128 query rows = UMMA M = 128: two 64-row
+// sub-blocks stacked on the TMEM lanes (A on lanes 32w..32w+15, B on 32w+16..32w+31 of quadrant w).  Softmax group g
+// works on sub-block g of the same K/V tile (attn_softmax_tree); the blocks of a tree are listed level-major so that
+// they stream the same K/V tiles from different CTAs at the same time: HBM is read once, the second reader hits L2.
 #include "wf_internal.cuh"
 #include "wf_sm100.cuh"
 
@@ -296,10 +302,10 @@ __device__ __forceinline__ void tmem_ld_frag(uint32_t taddr, uint32_t (&v)[N]) {
 // ================= warps 0-3 (group 0) and 4-7 (group 1): softmax, O accumulation, output, merges =================
 // The two groups ping-pong over the tiles: group g takes the tiles whose global counter has parity g and
 // keeps its own running (m, l, O); at the end of a segment group 1 hands its state to group 0 through smem.
-template <int D, bool TREE>
-__device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared<TREE>& sh, uint8_t* q_s, uint8_t* p0_s, uint8_t* p1_s,
+template <int D>
+__device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared<false>& sh, uint8_t* q_s, uint8_t* p0_s, uint8_t* p1_s,
                                              uint8_t* v_s, uint32_t tmem_base, int warp, int lane) {
-  using C = AttnCfg<D, TREE>;
+  using C = AttnCfg<D, false>;
   constexpr int NO = D / 2;                                    // O registers per thread (2 rows x D/4 columns)
   const int Hkv = p.kv.n_kv_heads;
   const int grp = warp >> 2, qw = warp & 3;                    // group, TMEM lane quarter
@@ -310,7 +316,7 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared<TRE
   uint8_t* p_s = grp ? p1_s : p0_s;
   float* xch = reinterpret_cast<float*>(q_s);                  // [NO][128] group-merge buffer (Q + P1 regions)
   const int T = sh.total_tiles, G = sh.g_eff;
-  SegWalker<TREE> walk(sh, p.kv.n_kv_heads, blockIdx.x);
+  SegWalker<false> walk(sh, p.kv.n_kv_heads, blockIdx.x);
   Segment sg;
   uint32_t gt0 = 0;                                            // global tile counter at the start of the segment
   while (walk.next(sg)) {
@@ -319,7 +325,7 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared<TRE
     {
       // The NEXT segment's Q rows go to L2 now: under a saturated HBM a cold Q load took 6k cycles at every
       // segment start.  A token's `group` heads are contiguous: group * D * 2 bytes = D / 64 * group lines of 128 B.
-      SegWalker<TREE> peek = walk;
+      SegWalker<false> peek = walk;
       Segment nx;
       has_next = peek.next(nx);
       if (has_next) {
@@ -365,16 +371,6 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared<TRE
     int lim[2];                                                // keys j < lim[h] are visible to row (row_lo + 8h)
     lim[0] = min(sg.k1, sg.ctx + row_lo / p.group + 1);
     lim[1] = min(sg.k1, sg.ctx + (row_lo + 8) / p.group + 1);
-    // TREE: keys below ctx are visible to every row; key ctx + j only if bit j of the row's ancestor mask is set
-    // (the row's own bit is always set, so a live row sees at least one key).  Padding rows see the context only.
-    unsigned long long anc[2] = {0ull, 0ull};
-    if constexpr (TREE) {
-#pragma unroll
-      for (int h = 0; h < 2; ++h) {
-        const int node = (row_lo + 8 * h) / p.group;
-        if (node < sg.q_b) anc[h] = __ldg(p.tree_mask + sg.r0 + node);
-      }
-    }
 
     auto fold_o = [&]() {                                      // o = o * alpha_prev + O_tile (this group's buffer)
       uint32_t v[NO];
@@ -400,17 +396,7 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared<TRE
       tc_fence_before();
       mbar_arrive(smem_u32(&sh.s_empty[grp]));                 // S buffer may be overwritten by QK(g2 + 2)
 
-      if constexpr (TREE) {
-        if (tk0 + AT_BN > sg.ctx) {                            // the tile holds tree keys (or the tail beyond them)
-          const int rel0 = tk0 + cq - sg.ctx;                  // key of element c, relative to the first tree key
-#pragma unroll
-          for (int c = 0; c < 64; ++c) {
-            const int rel = rel0 + (c >> 2) * 8 + (c & 1);
-            const bool vis = rel < 0 || (rel < 64 && ((anc[(c >> 1) & 1] >> (rel & 63)) & 1ull));
-            if (!vis) sv[c] = 0xff800000u;                     // -inf
-          }
-        }
-      } else if (tk0 + AT_BN > min(sg.ctx + 1, sg.k1)) {       // causal / tail mask
+      if (tk0 + AT_BN > min(sg.ctx + 1, sg.k1)) {              // causal / tail mask
 #pragma unroll
         for (int c = 0; c < 64; ++c) {
           const int j = tk0 + (c >> 2) * 8 + cq + (c & 1);
@@ -1037,7 +1023,7 @@ __global__ void __launch_bounds__(AT_THREADS, 1) wf_verify_attn_kernel(const Att
     if (warp < 8) {
       asm volatile("setmaxnreg.inc.sync.aligned.u32 216;");
       if constexpr (TREE) attn_softmax_tree<D>(p, sh, q_s, p0_s, v_s, tmem_base, warp, lane);
-      else attn_softmax<D, TREE>(p, sh, q_s, p0_s, p1_s, v_s, tmem_base, warp, lane);
+      else attn_softmax<D>(p, sh, q_s, p0_s, p1_s, v_s, tmem_base, warp, lane);
     } else {
       asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
       if (warp == 8) attn_loader<D, TREE>(p, sh, k_s, 0, lane);
