@@ -129,10 +129,10 @@ __device__ __forceinline__ void cp_async16_zfill(uint32_t dst, const void* src, 
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(n) : "memory");
 }
 // 2^x on the FMA pipe (no MUFU): round-to-nearest split x = n + f, |f| <= 0.5, degree-4 Taylor polynomial of 2^f
-// (relative error < 5e-5, far below the bf16 rounding of P), exponent added as an integer.  x <= 0 expected; anything
-// below -126 (including -inf) returns a denormal-scale value that flushes to 0 in the bf16 pack and the row sum.
+// (relative error < 5e-5, far below the bf16 rounding of P), exponent added as an integer.  x <= 0 expected.  The clamp
+// makes a masked key (x = -inf) exactly +0: n = -127, f = 0, p = 1.0f, and 0x3F800000 - (127 << 23) = 0.
 __device__ __forceinline__ float poly_exp2(float x) {
-  x = fmaxf(x, -126.f);
+  x = fmaxf(x, -127.f);
   const float t = x + 12582912.f;                            // 1.5 * 2^23: n sits in the low mantissa bits
   const float f = x - (t - 12582912.f);
   float p = fmaf(f, 0.0096181291f, 0.0555041087f);

@@ -337,3 +337,36 @@ def test_compact_bad_path_flagged(wf):
     assert ctx.poll_status() == binding.WF_ERR_INVALID_ARG
     assert int(pair.seq_len[0]) == 23
     pair.close()
+
+
+def test_tree_attn_ignores_everything_outside_the_visible_keys(wf):
+    """Every K/V slot that no row may read (beyond ctx + n in the last page, and all unused pages) holds NaN bits: the
+    outputs stay finite and equal to the oracle's.  Non-ancestor tree nodes keep finite K/V (they are masked, and a
+    masked key must contribute exactly 0, also on the polynomial exp2 path)."""
+    import gpu_harness as H
+    binding, ctx = wf
+    Hq, Hkv, D = 32, 8, 128
+    g = synth.rng(71, 1)
+    ctx_lens, sizes = [300, 1027, 60], [60, 45, 33]          # ragged tails inside the last tile and the last page
+    parents, parent, ip = _trees(g, sizes)
+    pair = H.make_kv_pair(ctx, ctx_lens, sizes, 1, Hkv, D, seed=71)
+    live_k, live_v = pair.oracle.k_pool.copy(), pair.oracle.v_pool.copy()
+    pair.oracle.k_pool[:] = 0x7FC0                           # bf16 NaN everywhere ...
+    pair.oracle.v_pool[:] = 0x7FC0
+    for b in range(3):                                       # ... except the positions a row may see
+        for j in range(ctx_lens[b] + sizes[b]):
+            pg, slot = pair.oracle.locate(b, j)
+            pair.oracle.k_pool[0, pg, :, slot, :] = live_k[0, pg, :, slot, :]
+            pair.oracle.v_pool[0, pg, :, slot, :] = live_v[0, pg, :, slot, :]
+    pair.upload_pools()
+    Q = synth.normal_bf16(g, (int(ip[-1]), Hq, D), 1.0)
+    scale = 1.0 / math.sqrt(D)
+    got = _tree_attn(binding, ctx, pair, 0, Q, ip, parent, Hq, scale, 60)
+    want = tree_verify.tree_attn(pair.oracle, 0, Q, ip, parent, Hq, scale)
+    gf = (got.astype(np.uint32) << 16).view(np.float32)
+    assert np.isfinite(gf).all() and np.isfinite(want).all()
+    for b in range(3):
+        r0, r1 = int(ip[b]), int(ip[b + 1])
+        ma, rl = H.attn_errors(got[r0:r1], want[r0:r1])
+        assert ma <= ATTN_MAX_ABS and rl <= ATTN_REL_L2, (b, ma, rl)
+    pair.close()
