@@ -370,3 +370,31 @@ def test_tree_attn_ignores_everything_outside_the_visible_keys(wf):
         ma, rl = H.attn_errors(got[r0:r1], want[r0:r1])
         assert ma <= ATTN_MAX_ABS and rl <= ATTN_REL_L2, (b, ma, rl)
     pair.close()
+
+
+def test_compact_long_overlapping_path(wf):
+    """A 21-step path [0, 2, 4, .., 40] (a comb tree: every accepted node has a rejected sibling before it): three
+    batches of eight moves per column, and every even destination is an earlier step's source.  Two layers, two
+    sequences (the second keeps its rows: path[k] = k), bit-exact against the oracle, rows below ctx untouched."""
+    import torch
+    import gpu_harness as H
+    binding, ctx = wf
+    ctx_lens, sizes = [37, 100], [41, 12]
+    pair = H.make_kv_pair(ctx, ctx_lens, sizes, 2, 8, 128, seed=73)
+    path = np.full((2, 64), -1, np.int32)
+    path[0, :21] = np.arange(0, 42, 2)
+    path[1, :12] = np.arange(12)
+    n_commit = np.array([21, 12], np.int32)
+    binding.wf_kv_compact_path(ctx, pair.gpu, H.i32(path), 64, H.i32(n_commit), 2)
+    torch.cuda.synchronize()
+    assert ctx.poll_status() == 0
+    tree_verify.compact_path(pair.oracle, path, n_commit)
+    np.testing.assert_array_equal(pair.seq_len.cpu().numpy()[:2], pair.oracle.seq_len[:2])
+    k_bits, v_bits = H.bf16_tensor_to_bits(pair.k_pool), H.bf16_tensor_to_bits(pair.v_pool)
+    for b in range(2):
+        n = int(pair.oracle.seq_len[b])
+        for j0 in range(0, n, 16):
+            pg, cnt = int(pair.oracle.block_table[b, j0 // 16]), min(16, n - j0)
+            np.testing.assert_array_equal(k_bits[:, pg, :, :cnt, :], pair.oracle.k_pool[:, pg, :, :cnt, :])
+            np.testing.assert_array_equal(v_bits[:, pg, :, :cnt, :], pair.oracle.v_pool[:, pg, :, :cnt, :])
+    pair.close()
