@@ -499,10 +499,16 @@ def run_ours(args):
     u_smp = torch.rand(B, dtype=torch.float32, device="cuda", generator=gsmp)
     tok_out = torch.zeros(B, dtype=torch.int32, device="cuda")
     acc_us = {}
-    for mode in ("greedy", "sample"):
+    # a drafter distribution per row for the full-q variant: softmax of a perturbed copy of the logits (input construction)
+    q_full = torch.softmax(s.logits / 0.8 * 0.9 + torch.randn(s.logits.shape, device="cuda", generator=gsmp), dim=1)
+    for mode in ("greedy", "sample", "sample_full_q"):
         def call():
             o = rs.out
-            if mode == "greedy":
+            if mode == "sample_full_q":
+                wf.wf_accept_sample_entropy_route(ctx, s.logits, sh.vocab, s.drafts, s.q_indptr, B, rs.qmax, 0.8, q_full, u_acc, u_smp,
+                                                  rs.tau, True, o["accept_len"], tok_out, rs.entropy, o["route"], o["n_commit"],
+                                                  None, rs.acc_ws)
+            elif mode == "greedy":
                 wf.wf_accept_entropy_route(ctx, s.logits, sh.vocab, s.drafts, s.q_indptr, B, rs.qmax, rs.tau, True, o["accept_len"],
                                            tok_out, rs.entropy, o["route"], o["n_commit"], None, rs.acc_ws)
             else:
@@ -520,6 +526,7 @@ def run_ours(args):
         torch.cuda.synchronize()
         acc_us[mode] = 1e3 * a0.elapsed_time(a1) / 20
     logit_bytes = float(s.sum_q) * sh.vocab * 4
+    del q_full
 
     # ---- tree verification round, timed on its own: every sequence brings a 60-node draft tree
     #      (PAPER.md:317); masks + L x tree attention + acceptance walk + path compaction ----
@@ -586,7 +593,8 @@ def run_ours(args):
                               "note": "WhiFlash-Neural policy (d -> d/8 -> GELU -> 1), back-to-back calls, not part of the round"},
             "clocks": clocks,
         }
-        line["stochastic_accept"] = {"us_per_call": acc_us["sample"], "greedy_us_per_call": acc_us["greedy"], "temperature": 0.8,
+        line["stochastic_accept"] = {"us_per_call": acc_us["sample"], "greedy_us_per_call": acc_us["greedy"],
+                                     "full_q_us_per_call": acc_us["sample_full_q"], "temperature": 0.8,
                                      "logits_gbs": logit_bytes / (acc_us["sample"] * 1e-6) / 1e9,
                                      "greedy_logits_gbs": logit_bytes / (acc_us["greedy"] * 1e-6) / 1e9,
                                      "note": "speculative sampling (one-hot drafter, uniforms as inputs): same sweep over the "

@@ -353,10 +353,36 @@ wf_accept_kernel(const float* __restrict__ logits, int V, int n_chunks, const in
   }
   for (int level = 0; level < levels; ++level) {
     const bool first = levels == 2 && level == 0;          // this level also fixes the total and the target
-    const int part = (hi - lo + NW - 1) / NW;
+    const int part = (((hi - lo + NW - 1) / NW) + 127) & ~127;             // whole 128-token strips: 16-byte loads stay aligned
     const bool resid = s_resid != 0;
     const int plo = min(hi, lo + wid * part), phi = min(hi, plo + part);
     double acc = 0.0;
+    if (VEC) {
+      // V % 4 == 0 and 16-byte aligned rows: 8 x 16-byte loads of z (and of q) in flight per lane; the pass is one CTA
+      // streaming up to 2 x 600 KB, i.e. bound by the bytes it keeps in flight
+      for (int v0 = plo + 4 * lane; v0 < phi; v0 += 128 * 8) {
+        float4 zz[8], qq[8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+          const int v = v0 + 128 * k;
+          zz[k] = v < phi ? *reinterpret_cast<const float4*>(zr + v) : make_float4(-INFINITY, -INFINITY, -INFINITY, -INFINITY);
+          qq[k] = (resid && qr && v < phi) ? *reinterpret_cast<const float4*>(qr + v) : make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+          const float z4[4] = {zz[k].x, zz[k].y, zz[k].z, zz[k].w}, q4[4] = {qq[k].x, qq[k].y, qq[k].z, qq[k].w};
+#pragma unroll
+          for (int j = 0; j < 4; ++j) {
+            const int v = v0 + 128 * k + j;
+            float e;
+            asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"((z4[j] * smp.inv_t - Mr) * 1.4426950408889634f));
+            float pv = e * Zinv_f;
+            if (resid) pv = fmaxf(0.f, pv - (qr ? q4[j] : (v == xrej ? 1.f : 0.f)));
+            acc += (double)pv;
+          }
+        }
+      }
+    } else
     for (int v0 = plo + lane; v0 < phi; v0 += 32 * 8) {    // 8 loads in flight per lane
       float zz[8], qq[8];
 #pragma unroll
