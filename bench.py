@@ -1,12 +1,14 @@
 #!/usr/bin/env python
 """bench.py -- whole verify-and-switch rounds of the WhiFlash hot path on synthetic data (B200).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg3] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg5] [--sub-workloads cfg2,cfg3,cfg4] [--impl reference]
 
 A step is one round of the whole path over one batch: target-page
-reserve, 36 layers of verify attention, accept/entropy/route, then drafter catch-up (eager append for
-the active drafter, lazy enqueue for the idle one, flush for sequences that switch).  One JSON line is
-printed by rank 0.  Multi-GPU: the path does not shard (BASELINE.json north_star: one GPU, no
+reserve, 36 layers of verify attention, accept/entropy/route, then the switch (wf_switch_round: eager
+append for the active drafter, lazy enqueue for the idle one, flush for sequences the router switches,
+all derived on the device from the route).  The headline workload is cfg5 (BASELINE.json configs[4],
+the largest single-GPU config); cfg2-cfg4 ride on the same line as compact `per_config` sub-records.
+One JSON line is printed by rank 0.  Multi-GPU: the path does not shard (BASELINE.json north_star: one GPU, no
 collectives) -> "replicas only": every rank runs the same workload independently, timed as the max
 over ranks.  `--impl reference` times the CPU oracle (oracle/) on a bounded sample instead.
 """
@@ -27,9 +29,9 @@ sys.path.insert(0, ROOT)
 from paper_2606_07710_b200 import synth  # noqa: E402
 
 WORKLOADS = {"cfg1": 0, "cfg2": 1, "cfg3": 2, "cfg4": 3, "cfg5": 4}
-# dram__bytes_read.sum + dram__bytes_write.sum per attention launch from the committed `ncu --set full` capture
-# (profiles/r1e_final_cfg3.md); workloads without a capture report null
-NCU_TRAFFIC_BYTES = {"cfg3": 552.5e6}
+# dram__bytes_read.sum + dram__bytes_write.sum per attention launch, from the committed `ncu --set full` capture named
+# beside each figure (a profiler cannot run inside the timed region); workloads without a capture report null
+NCU_TRAFFIC = {"cfg3": (552.5e6, "profiles/r1g_final.md (ncu --set full, chain kernel, round 1 commit abe3062)")}
 METRIC = "verify_rounds_per_s"
 UNIT = "rounds/s"
 
@@ -272,84 +274,122 @@ def run_reference(args):
             times.append((time.perf_counter() - t0, t))
     per_round = float(np.mean([scale_sample_to_round(t, lens, q_lens, sh.n_layers, b0, wl.mean_accept + 1, n_rows) for _, t in times]))
     ms_step = 1e3 * float(np.mean([w for w, _ in times]))
-    cores = os.cpu_count()
-    try:
-        from threadpoolctl import threadpool_info
-        cores = max([p.get("num_threads", 1) for p in threadpool_info()] + [1])
-    except Exception:
-        pass
+    cores = oracle_cores()
     sample = (f"per step: 1 of {wl.batch} sequences (ctx {seq_ctx}, {q_len} query rows): 1 of {sh.n_layers} attention layers, "
               f"its accept/entropy/route, KV-only prefill of {n_rows} rows into both drafters; scaled to a whole round "
               f"by layers x tokens, rows and sequences")
     value = 1.0 / per_round
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f64", "data": "synthetic", "config": {"workload": wl.name, "batch": wl.batch, "ctx": str(wl.ctx)},
+            "dtype": "f64", "data": "synthetic", "config": config_dict(wl),
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
 
 
-def run_ours(args):
-    import torch
-    rank, world, local = dist_setup(args.gpus)
-    torch.cuda.set_device(local)
-    from paper_2606_07710_b200 import binding as wf          # raises if libwhiflash.so is missing: no fallback
-    from paper_2606_07710_b200.rounds import RoundState
-    wl = synth.WORKLOADS[WORKLOADS[args.workload]]
+def config_dict(wl, world=1):
+    """The workload as both arms print it (ours and --impl reference): only what defines the work."""
     sh = wl.shapes
-    ctx = wf.Ctx(local)
-    K, W = args.steps, max(args.warmup, 3)
-    e2e_steps = max(1, min(K, args.e2e_steps))
-    eager_steps = 8
-    rs = RoundState(ctx, wl, n_slots=4, n_rounds_max=W + K + e2e_steps + eager_steps + 4 + 10 + 24, host_copies=True)   # + 10: tree leg, + 24: graph leg
+    return {"workload": wl.name, "batch": wl.batch, "ctx": str(wl.ctx), "gammas": list(wl.gammas), "layers": sh.n_layers,
+            "vocab": sh.vocab, "backlog_cap": wl.backlog_cap, "switch_prob": wl.switch_prob, "mean_accept": wl.mean_accept,
+            "parallelism": "replicas only" if world > 1 else "1 gpu"}
+
+
+def oracle_cores():
+    cores = os.cpu_count()
+    try:
+        from threadpoolctl import threadpool_info
+        cores = max([p.get("num_threads", 1) for p in threadpool_info()] + [1])
+    except Exception:
+        pass
+    return cores
+
+
+def cpu_baseline_and_parity(rs, wl, ctx, wf, n_seq, n_lay):
+    """The oracle timed on a bounded sample of slot 0's round (sequences 0..n_seq-1, n_lay attention layers, their
+    accept and prefill), which is also the full-size sampled parity check of attention layer 0.  n_seq = B and
+    n_lay = L is one WHOLE round, unscaled."""
+    import torch
+    sh, B, L = rs.sh, rs.B, rs.L
+    s0 = rs.slots[0]
+    rs.target_kv.reserve(s0.add_tokens, B)                    # pages for the block's own tokens (idempotent)
+    wf.wf_verify_attn(ctx, rs.target_kv, 0, s0.q, s0.q_indptr, B, sh.n_q_heads, rs.qmax, rs.sm_scale, s0.attn_out, rs.attn_ws)
+    torch.cuda.synchronize()
+    lens = round_units(rs, s0)
+    tot = {"t_attn": 0.0, "t_accept": 0.0, "t_prefill": 0.0}
+    tok = rows_q = rows_p = 0
+    worst_rel = worst_abs = 0.0
+    for b0 in range(n_seq):
+        smp = gather_sample(rs, b0, s0, n_lay)
+        n_rows = int(s0.u[b0]) + 1
+        t = oracle_sample(wl, smp["seq_ctx"], smp["q_len"], n_rows, smp["kv_bits"], smp["q_bits"], smp["logits"],
+                          smp["drafts"], smp["weights"], smp["x_bits"], attn_layers=n_lay)
+        for k2 in tot:
+            tot[k2] += t[k2]
+        tok += int(lens[b0]); rows_q += smp["q_len"]; rows_p += n_rows
+        r0, r1 = int(s0.q_indptr_host[b0]), int(s0.q_indptr_host[b0 + 1])
+        got = s0.attn_out[r0:r1].float().cpu().numpy().astype(np.float64)     # layer 0 of the launch above
+        want = t["attn_out"][0]
+        worst_rel = max(worst_rel, float(np.sqrt(((got - want) ** 2).sum() / (want ** 2).sum())))
+        worst_abs = max(worst_abs, float(np.abs(got - want).max()))
+        if int(t["accept"]["accept_len"][0]) != int(s0.u[b0]):
+            raise SystemExit("full-size sampled parity failed: oracle accept_len differs from the planted plan")
+    parity = {"attn_rel_l2_layer0_worst": worst_rel, "attn_max_abs_worst": worst_abs, "sequences": n_seq}
+    if worst_rel > 5e-3 or worst_abs > 2e-2:
+        raise SystemExit(f"full-size sampled parity failed: {parity}")
+    whole = n_seq == B and n_lay == L
+    if whole:
+        per_round = tot["t_attn"] + tot["t_accept"] + tot["t_prefill"]
+        sample = (f"ONE WHOLE round, unscaled: all {B} sequence(s) x all {L} attention layers ({tot['t_attn']:.1f} s), accept/entropy/route "
+                  f"({tot['t_accept']:.2f} s), KV-only prefill of {rows_p} rows into both drafters ({tot['t_prefill']:.1f} s)")
+    else:
+        per_round = (tot["t_attn"] * (L / n_lay) * float(lens.sum()) / tok + tot["t_accept"] * float(s0.q_lens.sum()) / rows_q
+                     + tot["t_prefill"] * float(np.sum(s0.u + 1)) / rows_p)
+        sample = (f"SCALED sample: sequences 0..{n_seq - 1} of {B}: {n_lay} of {L} attention layers ({tot['t_attn']:.1f} s), their "
+                  f"accept/entropy/route ({tot['t_accept']:.2f} s), KV-only prefill of {rows_p} rows into both drafters "
+                  f"({tot['t_prefill']:.1f} s); scaled to a whole round by layers x tokens, logit rows and committed rows")
+    return {"value": 1.0 / per_round, "unit": UNIT, "cores": oracle_cores(), "kind": "oracle", "sample": sample}, parity
+
+
+def timed_rounds(rs, n, mode, torch):
+    """n whole rounds with the given catch-up mode; returns (total ms, catch-up ms)."""
+    ev = [{"attn": (torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)),
+           "catchup": (torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))} for _ in range(n)]
+    g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    g0.record()
+    for i in range(n):
+        rs.run_round(events=ev[i], mode=mode)
+    g1.record()
+    torch.cuda.synchronize()
+    return g0.elapsed_time(g1), sum(e["catchup"][0].elapsed_time(e["catchup"][1]) for e in ev)
+
+
+def measure(ctx, wf, key, args, rank, world, local, main):
+    """One workload: K timed rounds (device-resident inputs), the e2e leg (host inputs), the catch-up legs, and for the
+    main workload the side legs (graph replay, neural router, stochastic acceptance, tree verification)."""
+    import torch
+    from paper_2606_07710_b200.rounds import RoundState
+    wl = synth.WORKLOADS[WORKLOADS[key]]
+    sh = wl.shapes
+    K, W = (args.steps, max(args.warmup, 3)) if main else (min(args.steps, args.sub_steps), 3)
+    e2e_steps = max(1, min(K, args.e2e_steps if main else args.sub_e2e_steps))
+    leg_steps = 8
+    n_slots = args.slots
+    extra = (10 + n_slots + 20) if main else 0                # tree leg, graph leg
+    rs = RoundState(ctx, wl, n_slots=n_slots, n_rounds_max=W + K + e2e_steps + 2 * leg_steps + 4 + extra, host_copies=True)
     B, L = rs.B, rs.L
 
     # ---- cpu_baseline + full-size sampled parity (rank 0 of a 1-GPU run only) ----
     cpu_baseline, parity = None, None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        s0 = rs.slots[0]
-        rs.target_kv.reserve(s0.add_tokens, B)                # pages for the block's own tokens (idempotent)
-        wf.wf_verify_attn(ctx, rs.target_kv, 0, s0.q, s0.q_indptr, B, sh.n_q_heads, rs.qmax, rs.sm_scale, s0.attn_out, rs.attn_ws)
-        torch.cuda.synchronize()
-        lens = round_units(rs, s0)
-        n_seq, n_lay = min(B, args.cpu_sample_seqs), min(L, args.cpu_sample_layers)
-        tot = {"t_attn": 0.0, "t_accept": 0.0, "t_prefill": 0.0}
-        tok = rows_q = rows_p = 0
-        worst_rel = worst_abs = 0.0
-        for b0 in range(n_seq):
-            smp = gather_sample(rs, b0, s0, n_lay)
-            n_rows = int(s0.u[b0]) + 1
-            t = oracle_sample(wl, smp["seq_ctx"], smp["q_len"], n_rows, smp["kv_bits"], smp["q_bits"], smp["logits"],
-                              smp["drafts"], smp["weights"], smp["x_bits"], attn_layers=n_lay)
-            for k2 in tot:
-                tot[k2] += t[k2]
-            tok += int(lens[b0]); rows_q += smp["q_len"]; rows_p += n_rows
-            r0, r1 = int(s0.q_indptr_host[b0]), int(s0.q_indptr_host[b0 + 1])
-            got = s0.attn_out[r0:r1].float().cpu().numpy().astype(np.float64)     # layer 0 of the launch above
-            want = t["attn_out"][0]
-            worst_rel = max(worst_rel, float(np.sqrt(((got - want) ** 2).sum() / (want ** 2).sum())))
-            worst_abs = max(worst_abs, float(np.abs(got - want).max()))
-            if int(t["accept"]["accept_len"][0]) != int(s0.u[b0]):
-                raise SystemExit("full-size sampled parity failed: oracle accept_len differs from the planted plan")
-        parity = {"attn_rel_l2_layer0_worst": worst_rel, "attn_max_abs_worst": worst_abs, "sequences": n_seq}
-        if worst_rel > 5e-3 or worst_abs > 2e-2:
-            raise SystemExit(f"full-size sampled parity failed: {parity}")
-        per_round = (tot["t_attn"] * (L / n_lay) * float(lens.sum()) / tok + tot["t_accept"] * float(s0.q_lens.sum()) / rows_q
-                     + tot["t_prefill"] * float(np.sum(s0.u + 1)) / rows_p)
-        cores = os.cpu_count()
-        try:
-            from threadpoolctl import threadpool_info
-            cores = max([p.get("num_threads", 1) for p in threadpool_info()] + [1])
-        except Exception:
-            pass
-        cpu_baseline = {"value": 1.0 / per_round, "unit": UNIT, "cores": cores, "kind": "oracle",
-                        "sample": (f"sequences 0..{n_seq - 1} of {B}: {n_lay} of {L} attention layers ({tot['t_attn']:.1f} s), their "
-                                   f"accept/entropy/route ({tot['t_accept']:.2f} s), KV-only prefill of {rows_p} rows into both drafters "
-                                   f"({tot['t_prefill']:.1f} s); scaled to a whole round by layers x tokens, logit rows and committed rows")}
+        if main:
+            cpu_baseline, parity = cpu_baseline_and_parity(rs, wl, ctx, wf, min(B, args.cpu_sample_seqs), min(L, args.cpu_sample_layers))
+        elif key == "cfg2":
+            cpu_baseline, parity = cpu_baseline_and_parity(rs, wl, ctx, wf, B, L)      # a whole round, no scaling
 
-    # ---- warm-up (the clock sampler starts here so that nvidia-smi is up when the timed region begins) ----
+    # ---- warm-up (the clock sampler starts here so that it is up when the timed region begins) ----
     sampler = ClockSampler(local)
     sampler.start()
     for _ in range(W):
@@ -383,6 +423,7 @@ def run_ours(args):
     spans = [evs[i]["attn"][0].elapsed_time(evs[i + 1]["attn"][0]) for i in range(K - 1)]
     catch_ms = sum(e["catchup"][0].elapsed_time(e["catchup"][1]) for e in evs)
     commits = float(np.mean([np.sum(sl.u + 1) for sl in rs.slots]))
+    flips = float(np.mean([np.mean(sl.cur != sl.next) for sl in rs.slots]))
 
     # ---- e2e: the same rounds through the C-ABI with HOST inputs: H2D of the round's inputs and D2H of
     #      its results inside the timed region (the KV cache is state and stays resident) ----
@@ -432,26 +473,68 @@ def run_ours(args):
     clocks = sampler.stop()
     rs.check_plan(s)
 
-    # ---- the eager baseline of PAPER.md Table 3 at kernel level: both drafters get a KV-only prefill every round
-    #      (no deferral, no flush); same rounds otherwise ----
-    ev_e = [{"attn": (torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)),
-             "catchup": (torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))} for _ in range(eager_steps)]
-    g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    # flush what the lazy rounds left queued, so that the eager appends continue from complete caches
-    for d in rs.drafters.values():
+    # ---- catch-up legs, same rounds otherwise (Table 3 at kernel level):
+    #      eager  = Lazy Catch-up off: a KV-only prefill into BOTH drafters every round;
+    #      active = only the active drafter's own append (reading C22: it stands in for that drafter's forward, which is
+    #               drafting cost, not switching cost): lazy - active = what the switch machinery costs per round ----
+    for d in rs.drafters.values():                           # flush what the lazy rounds left queued: complete caches
         wf.wf_lazy_catchup_flush(ctx, d.handle, None, B)
-    torch.cuda.synchronize()
-    g0.record()
-    for i in range(eager_steps):
-        rs.run_round(lazy=False, events=ev_e[i])
-    g1.record()
-    torch.cuda.synchronize()
-    eager_ms = g0.elapsed_time(g1)
-    eager_catch_ms = sum(e["catchup"][0].elapsed_time(e["catchup"][1]) for e in ev_e)
+    eager_ms, eager_catch_ms = timed_rounds(rs, leg_steps, "eager", torch)
+    active_ms, active_catch_ms = timed_rounds(rs, leg_steps, "active", torch)
+    rs.check_plan(rs.slots[(rs.rounds_done - 1) % rs.n_slots], switched=False)
+    rs.sync_cur()
+    lazy_us, eager_us, active_us = 1e3 * catch_ms / K, 1e3 * eager_catch_ms / leg_steps, 1e3 * active_catch_ms / leg_steps
+    round_us = 1e3 * ms_local / K
 
+    peak, peak_src = measured_peaks()
+    avg_launch_ms = attn_ms / (K * L)
+    achieved = float(np.mean(attn_bytes)) / (avg_launch_ms * 1e-3) / 1e9
+    traffic, traffic_src = NCU_TRAFFIC.get(key, (None, None))
+    if main and args.traffic_bytes is not None:
+        traffic, traffic_src = args.traffic_bytes, "--traffic-bytes"
+    rec = {
+        "value": whole_job_value(K, world, ms), "unit": UNIT, "steps": K, "warmup": W,
+        "ms_per_step": ms / K, "ms_per_step_median": float(np.median(spans)) if spans else ms / K,
+        "config": config_dict(wl, world),
+        "run_notes": {"slots": rs.n_slots, "realised_switch_rate": flips,
+                      "l2": f"inputs larger than L2: {np.mean(attn_bytes) / 1e6:.0f} MB of KV per attention launch, distinct per layer",
+                      "catchup": "lazy: one wf_switch_round per round (both drafters, masks derived on the device from route)"},
+        "committed_tokens_per_s": world * commits * K / (ms * 1e-3),
+        "kv_read_gbs": achieved,
+        "attn_share_of_round": attn_ms / ms_local,
+        "catchup_us_per_round": lazy_us,
+        "catchup_share_of_round": catch_ms / ms_local,
+        "catchup": {"lazy_us_per_round": lazy_us, "eager_us_per_round": eager_us, "active_append_us_per_round": active_us,
+                    "switch_us_per_round": lazy_us - active_us, "share_of_round": lazy_us / round_us,
+                    "switch_share_of_round": (lazy_us - active_us) / round_us, "eager_share_of_round": eager_catch_ms / eager_ms,
+                    "eager_rounds_per_s": leg_steps / (eager_ms * 1e-3), "leg_steps": leg_steps,
+                    "note": "lazy = wf_switch_round inside the timed rounds; eager = KV-only prefill into both drafters every round "
+                            "(Lazy Catch-up off, PAPER.md Table 3 baseline); active_append = only the active drafter's own append "
+                            "(reading C22: drafting cost, not switching cost); switch = lazy - active_append (derived)"},
+        "roofline": {"bound": "hbm", "kernel": "wf_verify_attn_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                     "frac": achieved / peak, "peak_source": peak_src, "traffic": traffic, "traffic_source": traffic_src,
+                     "algorithmic_bytes_per_launch": float(np.mean(attn_bytes)), "avg_launch_us": 1e3 * avg_launch_ms},
+        "e2e": {"value": world * e2e_steps / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d // e2e_steps,
+                "d2h_bytes_per_step": d2h // e2e_steps, "steps": e2e_steps,
+                "overlap": "H2D of step i+1 on a copy stream while step i computes; every copy is inside the timed region"},
+        "gpu_launches": int(launches),
+        "clocks": clocks,
+    }
+    if cpu_baseline:
+        rec["cpu_baseline"] = cpu_baseline
+        rec["parity_sample"] = parity
+    if main:
+        rec.update(side_legs(rs, ctx, wf, wl, args, s, peak, torch))
+    rs.close()
+    return rec
+
+
+def side_legs(rs, ctx, wf, wl, args, s, peak, torch):
+    """Legs timed on their own after the headline region: graph replay, neural router, stochastic acceptance, tree verify."""
+    sh, B, L = rs.sh, rs.B, rs.L
+    out = {}
     # ---- the same round replayed from CUDA graphs (SURVEY.md §8(d) timing protocol): one graph per round slot, captured
     #      from the very calls above (every argument is a device pointer or a constant; lengths live on the device) ----
-    graph_leg = None
     try:
         side = torch.cuda.Stream()
         side.wait_stream(torch.cuda.current_stream())
@@ -472,11 +555,13 @@ def run_ours(args):
             graphs[i % rs.n_slots].replay()
         h1.record()
         torch.cuda.synchronize()
-        rs.check_plan(rs.slots[(rs.rounds_done - 1) % rs.n_slots])
-        graph_leg = {"rounds_per_s": g_steps / (h0.elapsed_time(h1) * 1e-3), "steps": g_steps,
-                     "note": "whole round replayed from one CUDA graph per round slot, captured from the same C-ABI calls"}
+        rs.check_plan(rs.slots[(rs.rounds_done + g_steps - 1) % rs.n_slots])
+        rs.rounds_done += g_steps                            # the replays advanced the device state by g_steps rounds
+        out["graph_replay"] = {"rounds_per_s": g_steps / (h0.elapsed_time(h1) * 1e-3), "steps": g_steps,
+                               "note": "whole round replayed from one CUDA graph per round slot, captured from the same C-ABI calls"}
+        del graphs
     except Exception as e:                                   # capture is optional evidence, never the headline
-        graph_leg = {"error": f"{type(e).__name__}: {e}"[:200]}
+        out["graph_replay"] = {"error": f"{type(e).__name__}: {e}"[:200]}
         torch.cuda.synchronize()
 
     # ---- WhiFlash-Neural router, timed on its own: the round above uses the entropy policy ----
@@ -489,7 +574,8 @@ def run_ours(args):
         rs.run_neural_route(s)
     n1.record()
     torch.cuda.synchronize()
-    neural_us = 1e3 * n0.elapsed_time(n1) / 20
+    out["neural_router"] = {"us_per_call": 1e3 * n0.elapsed_time(n1) / 20, "params": rs.nr.d * rs.nr.m + 2 * rs.nr.m + 1, "batch": B,
+                            "note": "WhiFlash-Neural policy (d -> d/8 -> GELU -> 1), back-to-back calls, not part of the round"}
 
     # ---- stochastic acceptance next to the greedy sweep, both on the last slot's logits, cache
     #      length untouched (target_kv = NULL): one sweep over the logits + the per-sequence inverse-CDF draw ----
@@ -501,19 +587,21 @@ def run_ours(args):
     acc_us = {}
     # a drafter distribution per row for the full-q variant: softmax of a perturbed copy of the logits (input construction)
     q_full = torch.softmax(s.logits / 0.8 * 0.9 + torch.randn(s.logits.shape, device="cuda", generator=gsmp), dim=1)
+    scratch = {k: torch.zeros_like(v) for k, v in rs.out.items()}          # the round's own outputs stay untouched
+    ent = torch.zeros_like(rs.entropy)
     for mode in ("greedy", "sample", "sample_full_q"):
         def call():
-            o = rs.out
+            o = scratch
             if mode == "sample_full_q":
                 wf.wf_accept_sample_entropy_route(ctx, s.logits, sh.vocab, s.drafts, s.q_indptr, B, rs.qmax, 0.8, q_full, u_acc, u_smp,
-                                                  rs.tau, True, o["accept_len"], tok_out, rs.entropy, o["route"], o["n_commit"],
+                                                  rs.tau, True, o["accept_len"], tok_out, ent, o["route"], o["n_commit"],
                                                   None, rs.acc_ws)
             elif mode == "greedy":
                 wf.wf_accept_entropy_route(ctx, s.logits, sh.vocab, s.drafts, s.q_indptr, B, rs.qmax, rs.tau, True, o["accept_len"],
-                                           tok_out, rs.entropy, o["route"], o["n_commit"], None, rs.acc_ws)
+                                           tok_out, ent, o["route"], o["n_commit"], None, rs.acc_ws)
             else:
                 wf.wf_accept_sample_entropy_route(ctx, s.logits, sh.vocab, s.drafts, s.q_indptr, B, rs.qmax, 0.8, None, u_acc, u_smp,
-                                                  rs.tau, True, o["accept_len"], tok_out, rs.entropy, o["route"], o["n_commit"],
+                                                  rs.tau, True, o["accept_len"], tok_out, ent, o["route"], o["n_commit"],
                                                   None, rs.acc_ws)
         for _ in range(3):
             call()
@@ -527,10 +615,17 @@ def run_ours(args):
         acc_us[mode] = 1e3 * a0.elapsed_time(a1) / 20
     logit_bytes = float(s.sum_q) * sh.vocab * 4
     del q_full
+    out["stochastic_accept"] = {"us_per_call": acc_us["sample"], "greedy_us_per_call": acc_us["greedy"],
+                                "full_q_us_per_call": acc_us["sample_full_q"], "temperature": 0.8,
+                                "logits_gbs": logit_bytes / (acc_us["sample"] * 1e-6) / 1e9,
+                                "greedy_logits_gbs": logit_bytes / (acc_us["greedy"] * 1e-6) / 1e9,
+                                "greedy_frac_of_hbm_peak": logit_bytes / (acc_us["greedy"] * 1e-6) / 1e9 / peak,
+                                "note": "speculative sampling (one-hot drafter, uniforms as inputs): same sweep over the "
+                                        "logits plus one inverse-CDF draw per sequence; back-to-back calls on the "
+                                        "logits of the last slot, not part of the round"}
 
     # ---- tree verification round, timed on its own: every sequence brings a 60-node draft tree
     #      (PAPER.md:317); masks + L x tree attention + acceptance walk + path compaction ----
-    tree = None
     if not args.no_tree:
         tsl = rs.make_tree_slot(60)
         tree_steps = 6
@@ -551,63 +646,39 @@ def run_ours(args):
         rs.check_tree_plan(tsl)
         tree_ms = t0.elapsed_time(t1)
         tree_attn_ms = sum(e["attn"][0].elapsed_time(e["attn"][1]) for e in ev_t)
-        tree = {"rounds_per_s": tree_steps / (tree_ms * 1e-3), "ms_per_round": tree_ms / tree_steps, "steps": tree_steps,
-                "nodes": 60, "attn_us_per_launch": 1e3 * tree_attn_ms / (tree_steps * L),
-                "kv_read_gbs": float(np.mean(t_bytes)) / (tree_attn_ms / (tree_steps * L) * 1e-3) / 1e9,
-                "committed_tokens_per_round": float(t_commit.sum()),
-                "note": "all sequences AR-routed with depth-8 / top-k-10 / 60-node trees (PAPER.md:317); 240 query rows per "
-                        "kv head = two 128-row query tiles (UMMA M = 128) that stream the same K/V (HBM once, L2 for the second)"}
+        gbs = float(np.mean(t_bytes)) / (tree_attn_ms / (tree_steps * L) * 1e-3) / 1e9
+        out["tree_verify"] = {"rounds_per_s": tree_steps / (tree_ms * 1e-3), "ms_per_round": tree_ms / tree_steps, "steps": tree_steps,
+                              "nodes": 60, "attn_us_per_launch": 1e3 * tree_attn_ms / (tree_steps * L), "kv_read_gbs": gbs,
+                              "frac_of_hbm_peak": gbs / peak, "committed_tokens_per_round": float(t_commit.sum()),
+                              "note": "all sequences AR-routed with depth-8 / top-k-10 / 60-node trees (PAPER.md:317); 240 query rows per "
+                                      "kv head = two 128-row query tiles (UMMA M = 128) that stream the same K/V (HBM once, L2 for the second)"}
+    return out
 
+
+def run_ours(args):
+    import torch
+    rank, world, local = dist_setup(args.gpus)
+    torch.cuda.set_device(local)
+    from paper_2606_07710_b200 import binding as wf          # raises if libwhiflash.so is missing: no fallback
+    ctx = wf.Ctx(local)
+    rec = measure(ctx, wf, args.workload, args, rank, world, local, main=True)
+    per_config = {}
+    for key in [k for k in args.sub_workloads.split(",") if k and k != args.workload]:
+        torch.cuda.empty_cache()
+        sub = measure(ctx, wf, key, args, rank, world, local, main=False)
+        keep = ("value", "unit", "steps", "ms_per_step", "kv_read_gbs", "attn_share_of_round", "catchup", "roofline", "e2e",
+                "clocks", "cpu_baseline", "parity_sample", "committed_tokens_per_s", "gpu_launches")
+        per_config[key] = {k: sub[k] for k in keep if k in sub}
+        per_config[key]["workload"] = sub["config"]["workload"]
+        per_config[key]["realised_switch_rate"] = sub["run_notes"]["realised_switch_rate"]
     if rank == 0:
-        peak, peak_src = measured_peaks()
-        if tree:
-            tree["frac_of_hbm_peak"] = tree["kv_read_gbs"] / peak
-        avg_launch_ms = attn_ms / (K * L)
-        achieved = float(np.mean(attn_bytes)) / (avg_launch_ms * 1e-3) / 1e9
-        line = {
-            "metric": METRIC, "value": whole_job_value(K, world, ms), "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
-            "ms_per_step": ms / K, "ms_per_step_median": float(np.median(spans)) if spans else ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
-            "data": "synthetic",
-            "config": {"workload": wl.name, "batch": B, "ctx": str(wl.ctx), "gammas": list(wl.gammas), "layers": L,
-                       "vocab": sh.vocab, "backlog_cap": wl.backlog_cap, "parallelism": "replicas only" if world > 1 else "1 gpu",
-                       "l2": f"inputs larger than L2: {np.mean(attn_bytes) / 1e6:.0f} MB of KV per attention launch, distinct per layer",
-                       "catchup": "lazy, one wf_lazy_catchup_round per drafter per round"},
-            "committed_tokens_per_s": world * commits * K / (ms * 1e-3),
-            "kv_read_gbs": achieved,
-            "catchup_us_per_round": 1e3 * catch_ms / K,
-            "catchup_share_of_round": catch_ms / ms_local,
-            "catchup_eager": {"us_per_round": 1e3 * eager_catch_ms / eager_steps, "share_of_round": eager_catch_ms / eager_ms,
-                              "rounds_per_s": eager_steps / (eager_ms * 1e-3), "steps": eager_steps,
-                              "note": "Lazy Catch-up off (PAPER.md Table 3 baseline): KV-only prefill into both drafters every round"},
-            "attn_share_of_round": attn_ms / ms_local,
-            "roofline": {"bound": "hbm", "kernel": "wf_verify_attn_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                         "frac": achieved / peak, "peak_source": peak_src,
-                         "traffic": args.traffic_bytes if args.traffic_bytes is not None else NCU_TRAFFIC_BYTES.get(args.workload),
-                         "traffic_source": "profiles/r1g_final.md",
-                         "algorithmic_bytes_per_launch": float(np.mean(attn_bytes)), "avg_launch_us": 1e3 * avg_launch_ms},
-            "e2e": {"value": world * e2e_steps / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d // e2e_steps,
-                    "d2h_bytes_per_step": d2h // e2e_steps, "steps": e2e_steps,
-                    "overlap": "H2D of step i+1 on a copy stream while step i computes; every copy is inside the timed region"},
-            "gpu_launches": int(launches),
-            "neural_router": {"us_per_call": neural_us, "params": rs.nr.d * rs.nr.m + 2 * rs.nr.m + 1, "batch": B,
-                              "note": "WhiFlash-Neural policy (d -> d/8 -> GELU -> 1), back-to-back calls, not part of the round"},
-            "clocks": clocks,
-        }
-        line["stochastic_accept"] = {"us_per_call": acc_us["sample"], "greedy_us_per_call": acc_us["greedy"],
-                                     "full_q_us_per_call": acc_us["sample_full_q"], "temperature": 0.8,
-                                     "logits_gbs": logit_bytes / (acc_us["sample"] * 1e-6) / 1e9,
-                                     "greedy_logits_gbs": logit_bytes / (acc_us["greedy"] * 1e-6) / 1e9,
-                                     "note": "speculative sampling (one-hot drafter, uniforms as inputs): same sweep over the "
-                                             "logits plus one inverse-CDF draw per sequence; back-to-back calls on L2-cold-ish "
-                                             "logits of the last slot, not part of the round"}
-        line["graph_replay"] = graph_leg
-        if tree:
-            line["tree_verify"] = tree
-        if cpu_baseline:
-            line["cpu_baseline"] = cpu_baseline
-            line["parity_sample"] = parity
+        line = {"metric": METRIC, "value": rec.pop("value"), "unit": rec.pop("unit"), "n_gpus": world, "steps": rec.pop("steps"),
+                "warmup": rec.pop("warmup"), "ms_per_step": rec.pop("ms_per_step"), "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "bf16", "data": "synthetic"}
+        line.update(rec)
+        if per_config:
+            line["per_config"] = per_config
         print(json.dumps(line), flush=True)
-    rs.close()
     ctx.close()
     if world > 1:
         import torch.distributed as dist
@@ -620,7 +691,13 @@ def main():
     ap.add_argument("--steps", type=int, default=60)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="cfg3", choices=sorted(WORKLOADS))
+    ap.add_argument("--workload", default="cfg5", choices=sorted(WORKLOADS),
+                    help="the headline workload: cfg5 = BASELINE.json configs[4], the largest single-GPU config")
+    ap.add_argument("--sub-workloads", default="cfg2,cfg3,cfg4",
+                    help="comma-separated workloads reported as compact per_config sub-records of the same line ('' = none)")
+    ap.add_argument("--sub-steps", type=int, default=30)
+    ap.add_argument("--sub-e2e-steps", type=int, default=10)
+    ap.add_argument("--slots", type=int, default=16, help="round slots of the cyclic schedule (distinct inputs and plans)")
     ap.add_argument("--e2e-steps", type=int, default=30)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-tree", action="store_true", help="skip the tree-verification leg (SURVEY.md §8(f) f2)")

@@ -9,8 +9,12 @@
  *    16-byte aligned.  bf16 tensors are passed as void* (raw bf16 bits, little endian).
  *  - Hot calls are asynchronous on the caller's CUDA stream (a cudaStream_t passed as void*; NULL =
  *    the legacy default stream) and never synchronise the host.  Conditions only the device can
- *    see (page exhaustion, backlog overflow) set a sticky device status word read by
- *    wf_poll_status.
+ *    see (page exhaustion, backlog overflow, a length beyond the host bound that sized a launch)
+ *    set a sticky device status word read by wf_poll_status; the first error of a poll interval
+ *    wins.
+ *  - Calls that share a wf_ctx, a wf_paged_kv or a wf_drafter must be stream-ordered with respect to
+ *    one another (one stream, or events between streams): the handles own per-call scratch
+ *    (completion counters, row plans, operand packs).  Distinct contexts may run concurrently.
  *  - Ownership: the caller allocates and owns every tensor (pools, block tables, lengths, weights,
  *    backlog, workspaces).  Handles (wf_ctx, wf_paged_kv, wf_drafter) are opaque, created and
  *    destroyed here; they borrow the caller's pointers and own only small bookkeeping buffers
@@ -87,7 +91,8 @@ const int32_t* wf_kv_pages_held(const wf_paged_kv* kv);
  *     O[i,h,:] = sum_j softmax(s)_j V[b,j,g,:]                          (fp32 accumulate, C13)
  * The block's own K/V must already be in the cache at positions ctx_b .. ctx_b+q_b-1 (C10).
  * q, out: bf16 [sum_q][n_q_heads][head_dim].  workspace: >= wf_verify_attn_workspace_bytes.
- * Supported: head_dim 64 or 128; page_size 16; q_b * group <= 64 (group = n_q_heads/n_kv_heads). */
+ * Supported: head_dim 64 or 128; page_size 16; q_b * group <= 64 (group = n_q_heads/n_kv_heads; rows beyond that
+ * are not computed and the sticky status becomes WF_ERR_INVALID_ARG). */
 int wf_verify_attn(wf_ctx* ctx, const wf_paged_kv* target_kv, int layer,
                    const void* q, const int32_t* q_indptr, int B, int n_q_heads, int max_q_len,
                    float sm_scale, void* out, void* workspace, size_t workspace_bytes, void* stream);
@@ -100,7 +105,8 @@ size_t wf_verify_attn_workspace_bytes(const wf_kv_shape* shape, int B, int n_q_h
  *     H = Shannon entropy (nats) of softmax(logits[r0+a]);  route = AR(1) if H > tau else 0.
  * If target_kv != NULL, target_kv.seq_len[b] += n_commit[b].
  * tau: device fp32 [B], or [1] if tau_is_scalar.  logits rows must be finite or -inf (C23).
- * max_q_len: host upper bound on q_b (<= 64) that sizes the grid.
+ * max_q_len: host upper bound on q_b (<= 64) that sizes the grid; a longer block is verified up to the bound and
+ * raises WF_ERR_INVALID_ARG in the sticky status.
  * workspace: >= wf_accept_workspace_bytes(B * max_q_len, V); contents need no initialisation. */
 int wf_accept_entropy_route(wf_ctx* ctx, const float* logits, int V, const int32_t* draft_tokens,
                             const int32_t* q_indptr, int B, int max_q_len, const float* tau,
@@ -136,7 +142,10 @@ int wf_drafter_destroy(wf_drafter* d);
  * p0+t, p0 = drafter_kv.seq_len[seq_ids[b]]) and W_V, rounded to bf16 (RNE) and written at logical
  * positions p0+t through the drafter's block table (pages reserved first, C24);
  * drafter_kv.seq_len[seq] += n_rows[b].  No attention, MLP or LM head runs.
- * seq_ids may be NULL (= identity).  n_rows[b] <= max_rows (host upper bound that sizes grids). */
+ * seq_ids may be NULL (= identity).  n_rows[b] <= max_rows (host upper bound that sizes grids; a larger
+ * n_rows[b] is clamped and raises WF_ERR_INVALID_ARG in the sticky status).  B <= 1024.
+ * Every call of sections (c)/(d) is two launches: plan + operand pack, then the projection (which also
+ * carries the enqueue copies and commits the backlog lengths). */
 int wf_kv_only_prefill(wf_ctx* ctx, wf_drafter* d, const void* hidden, const int32_t* q_indptr,
                        const int32_t* n_rows, const int32_t* seq_ids, int B, int max_rows,
                        void* stream);
@@ -147,6 +156,8 @@ int wf_kv_only_prefill(wf_ctx* ctx, wf_drafter* d, const void* hidden, const int
  * done.  If the rows would not fit (len + n > backlog_cap) that sequence's backlog is flushed first
  * (one batched prefill for all such sequences of the call), then the rows are enqueued: rows are
  * never dropped or reordered (C20).  n > backlog_cap sets WF_ERR_QUEUE_OVERFLOW and skips the rows.
+ * If the forced flush cannot get its pages the sticky status becomes WF_ERR_OUT_OF_PAGES and the call
+ * changes nothing (no row is written, no length moves).
  * flush: one batched KV-only prefill (same device code as (c)) over the whole backlog of every
  * sequence b in [0,B) with flush_mask[b] != 0 (NULL = all); backlog_len <- 0 for those.
  * Postcondition: the drafter cache is bit-identical to eager per-round appends. */
@@ -164,12 +175,29 @@ int wf_lazy_catchup_flush(wf_ctx* ctx, wf_drafter* d, const int32_t* flush_mask,
  *   idle, no flush    : the rows are enqueued (a backlog that would overflow is projected first, C20)
  *                       (= wf_lazy_catchup_enqueue).
  * All projected rows of the call share one plan, one operand pack and one projection: a drafter's weights are streamed
- * once per round instead of up to three times.  A row's K/V bits are those of the separate calls (same device code,
+ * once per round instead of up to three times.  If the pages do not fit (WF_ERR_OUT_OF_PAGES) the call changes nothing.  A row's K/V bits are those of the separate calls (same device code,
  * per-row results do not depend on the call that carries them).  idle_mask / flush_mask may be NULL (none idle / none
  * flushed).  B <= 1024, max_rows <= 64 (and <= backlog_cap when idle_mask is given). */
 int wf_lazy_catchup_round(wf_ctx* ctx, wf_drafter* d, const void* hidden, const int32_t* q_indptr,
                           const int32_t* n_rows, const int32_t* seq_ids, const int32_t* idle_mask,
                           const int32_t* flush_mask, int B, int max_rows, void* stream);
+
+/* ---- the switch, driven on the device by the router's output --------------------------------------------
+ * PAPER.md:117 ("Upon preparing for a switch, the incoming drafter prefills its KV cache over all tokens accepted during
+ * its inactivity as a single batched operation"), :65 (the chosen drafter drafts the next round); reading C21.
+ * cur_drafter: device int32 [B], in/out: the drafter that drafted THIS round's block (WF_ROUTE_AR / WF_ROUTE_DIFFUSION).
+ * route: device int32 [B]: this round's output of wf_accept_entropy_route (or wf_neural_route).  For drafter X with
+ * route code c_X (drafter_ar: WF_ROUTE_AR, drafter_diffusion: WF_ROUTE_DIFFUSION) the call derives
+ *     idle_X[b] = cur_drafter[b] != c_X,      flush_X[b] = idle_X[b] && route[b] == c_X
+ * and does for BOTH drafters what wf_lazy_catchup_round(idle_X, flush_X) does for one, in the same two launches (the
+ * tiles of both projections share one grid).  Afterwards cur_drafter[b] <- route[b] and, if next_q_len != NULL,
+ * next_q_len[b] <- (route[b] == WF_ROUTE_AR ? q_len_ar : q_len_diffusion): the block length the chosen drafter will
+ * bring next round.  No mask and no length crosses the host.  Both drafters need the same hidden size and head_dim and
+ * distinct caches; other limits as wf_lazy_catchup_round. */
+int wf_switch_round(wf_ctx* ctx, wf_drafter* drafter_ar, wf_drafter* drafter_diffusion, const void* hidden,
+                    const int32_t* q_indptr, const int32_t* n_rows, const int32_t* seq_ids, const int32_t* route,
+                    int32_t* cur_drafter, int32_t* next_q_len, int q_len_ar, int q_len_diffusion, int B, int max_rows,
+                    void* stream);
 
 /* ---- (f1) WhiFlash-Neural routing policy --------------------------------------------------------
  * PAPER.md:87 (§3.3.2), :103-107 (decision rule), :325 (App. A architecture); readings N1-N6.

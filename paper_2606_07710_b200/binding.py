@@ -33,7 +33,7 @@ EXPORTS = [
     "wf_lazy_catchup_enqueue", "wf_lazy_catchup_flush",
     "wf_neural_route", "wf_neural_route_workspace_bytes", "wf_lazy_catchup_round",
     "wf_tree_masks", "wf_verify_attn_tree", "wf_accept_tree_entropy_route", "wf_kv_compact_path",
-    "wf_accept_sample_entropy_route",
+    "wf_accept_sample_entropy_route", "wf_switch_round",
 ]
 
 
@@ -69,6 +69,7 @@ _SIG = {
     "wf_lazy_catchup_enqueue": (_i, [_vp, _vp, _vp, _vp, _vp, _vp, _vp, _i, _i, _vp]),
     "wf_lazy_catchup_flush": (_i, [_vp, _vp, _vp, _i, _vp]),
     "wf_lazy_catchup_round": (_i, [_vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _i, _i, _vp]),
+    "wf_switch_round": (_i, [_vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _i, _i, _i, _i, _vp]),
     "wf_neural_route_workspace_bytes": (_sz, [_i, _i]),
     "wf_neural_route": (_i, [_vp, _vp, _vp, _vp, _i, _i, _i, _vp, _vp, _vp, _vp, _vp, _i, _vp, _vp, _vp, _sz, _vp]),
     "wf_tree_masks": (_i, [_vp, _vp, _vp, _i, _i, _vp, _vp]),
@@ -227,6 +228,13 @@ def wf_neural_route(ctx, hidden_final, q_indptr, accept_len, B, d, m, w1, b1, w2
 def wf_lazy_catchup_round(ctx, drafter, hidden, q_indptr, n_rows, seq_ids, idle_mask, flush_mask, B, max_rows, stream=None):
     ctx.check(lib.wf_lazy_catchup_round(ctx.h, drafter.h, _ptr(hidden), _ptr(q_indptr), _ptr(n_rows), _ptr(seq_ids),
                                         _ptr(idle_mask), _ptr(flush_mask), B, max_rows, _stream(stream)))
+
+
+def wf_switch_round(ctx, drafter_ar, drafter_diffusion, hidden, q_indptr, n_rows, seq_ids, route, cur_drafter, next_q_len,
+                    q_len_ar, q_len_diffusion, B, max_rows, stream=None):
+    ctx.check(lib.wf_switch_round(ctx.h, drafter_ar.h, drafter_diffusion.h, _ptr(hidden), _ptr(q_indptr), _ptr(n_rows),
+                                  _ptr(seq_ids), _ptr(route), _ptr(cur_drafter), _ptr(next_q_len), q_len_ar, q_len_diffusion,
+                                  B, max_rows, _stream(stream)))
 
 
 def wf_tree_masks(ctx, parent, q_indptr, B, max_nodes, tree_mask, stream=None):

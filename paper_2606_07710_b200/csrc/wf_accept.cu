@@ -52,14 +52,22 @@ wf_accept_kernel(const float* __restrict__ logits, int V, int n_chunks, const in
                  int32_t* __restrict__ accept_len, int32_t* __restrict__ bonus_token, float* __restrict__ entropy,
                  int32_t* __restrict__ route, int32_t* __restrict__ n_commit, int32_t* __restrict__ kv_seq_len,
                  AccPartial* __restrict__ partials, unsigned int* __restrict__ counters,
-                 const int32_t* __restrict__ parent, int32_t* __restrict__ path, int path_stride, const AccSample smp) {
+                 const int32_t* __restrict__ parent, int32_t* __restrict__ path, int path_stride, const AccSample smp,
+                 int* __restrict__ status) {
   // parent == nullptr: chain block (C6).  Else tree block (T1-T4): greedy walk over parent pointers, the accepted
   // node indices go to path[b][0..a] (-1 beyond), and the cache length is left to wf_kv_compact_path.
   wf_pdl_trigger();
   wf_pdl_wait();
   const int b = blockIdx.z, i = blockIdx.y, chunk = blockIdx.x;
   const int r0 = q_indptr[b];
-  const int q_b = q_indptr[b + 1] - r0;
+  const size_t prow0 = (size_t)b * gridDim.y;             // partials are indexed by (sequence, row): in bounds whatever q_indptr says
+  int q_b = q_indptr[b + 1] - r0;
+  if (q_b > (int)gridDim.y) {
+    // the host bound max_q_len sizes the grid: a longer block is verified up to the bound (its counter still reaches
+    // its total and resets) and the sticky status says so
+    if (i == 0 && blockIdx.x == 0 && threadIdx.x == 0) wf_raise(status, (int)WF_ERR_INVALID_ARG);
+    q_b = (int)gridDim.y;
+  }
   if (q_b == 0 && i == 0 && blockIdx.x == 0 && threadIdx.x == 0) {
     // empty block: nothing verified, nothing committed
     accept_len[b] = 0; bonus_token[b] = 0; entropy[b] = 0.f; route[b] = 0; n_commit[b] = 0;
@@ -148,7 +156,7 @@ wf_accept_kernel(const float* __restrict__ logits, int V, int n_chunks, const in
 #pragma unroll
     for (int w = 0; w < ACC_THREADS / 32; ++w) { Zt += s_z[w]; St += s_s[w]; }
     AccPartial p; p.m = m; p.idx = mi; p.Z = Zt; p.S = St;
-    partials[(size_t)(r0 + i) * n_chunks + chunk] = p;
+    partials[(prow0 + i) * n_chunks + chunk] = p;
     __threadfence();
     const unsigned int total = (unsigned int)(q_b * n_chunks);
     const unsigned int old = atomicAdd(&counters[b], 1u);
@@ -166,7 +174,7 @@ wf_accept_kernel(const float* __restrict__ logits, int V, int n_chunks, const in
     float rm = -INFINITY;
     int ri = 0x7fffffff;
     for (int c = lane; c < n_chunks; c += 32) {
-      const AccPartial* pp = &partials[(size_t)(r0 + r) * n_chunks + c];
+      const AccPartial* pp = &partials[(prow0 + r) * n_chunks + c];
       const float pm = __ldcg(&pp->m);
       const int pi = __ldcg(&pp->idx);
       argmax_merge(rm, ri, pm, pi);
@@ -189,7 +197,7 @@ wf_accept_kernel(const float* __restrict__ logits, int V, int n_chunks, const in
   if (smp.u_accept) {
     // ---- speculative sampling (S3): p_{j-1}(x_j) from row j-1's slice partials and one gathered logit ----
     for (int r = wid; r < q_b; r += ACC_THREADS / 32) {   // one warp per row: (max, Z) over the slices
-      const AccPartial* pr = &partials[(size_t)(r0 + r) * n_chunks];
+      const AccPartial* pr = &partials[(prow0 + r) * n_chunks];
       float gm = -INFINITY;
       for (int c = lane; c < n_chunks; c += 32) gm = fmaxf(gm, __ldcg(&pr[c].m));
 #pragma unroll
@@ -206,11 +214,16 @@ wf_accept_kernel(const float* __restrict__ logits, int V, int n_chunks, const in
     __syncthreads();
     if (tid >= 1 && tid < q_b) {                           // draft j = tid against row j - 1
       const int x = draft_tokens[r0 + tid];
-      const size_t at = (size_t)(r0 + tid - 1) * V + x;
-      const double px = exp((double)(logits[at] * smp.inv_t) - (double)s_M[tid - 1]) / s_Z[tid - 1];
-      const double qx = smp.draft_q ? (double)smp.draft_q[at] : 1.0;
-      const double ratio = qx <= 0.0 ? 1.0 : fmin(1.0, px / qx);
-      s_ok[tid] = (double)smp.u_accept[r0 + tid] < ratio;
+      if (x < 0 || x >= V) {                               // not a token: rejected, never gathered
+        wf_raise(status, (int)WF_ERR_INVALID_ARG);
+        s_ok[tid] = 0;
+      } else {
+        const size_t at = (size_t)(r0 + tid - 1) * V + x;
+        const double px = exp((double)(logits[at] * smp.inv_t) - (double)s_M[tid - 1]) / s_Z[tid - 1];
+        const double qx = smp.draft_q ? (double)smp.draft_q[at] : 1.0;
+        const double ratio = qx <= 0.0 ? 1.0 : fmin(1.0, px / qx);
+        s_ok[tid] = (double)smp.u_accept[r0 + tid] < ratio;
+      }
     }
     __syncthreads();
     if (tid == 0) {
@@ -251,7 +264,7 @@ wf_accept_kernel(const float* __restrict__ logits, int V, int n_chunks, const in
   __syncthreads();
   if (wid == 0) {                                          // entropy of the last accepted row, fp64 combine (C3, C4, T4)
     const int a = s_a, row_a = s_row;
-    const AccPartial* pr = &partials[(size_t)(r0 + row_a) * n_chunks];
+    const AccPartial* pr = &partials[(prow0 + row_a) * n_chunks];
     float gm = -INFINITY;
     for (int c = lane; c < n_chunks; c += 32) gm = fmaxf(gm, __ldcg(&pr[c].m));
 #pragma unroll
@@ -294,7 +307,8 @@ wf_accept_kernel(const float* __restrict__ logits, int V, int n_chunks, const in
   const int a = s_a, gamma = q_b - 1;
   const float* zr = logits + (size_t)(r0 + a) * V;
   const float* qr = smp.draft_q ? smp.draft_q + (size_t)(r0 + a) * V : nullptr;
-  const int xrej = a < gamma ? draft_tokens[r0 + a + 1] : -1;
+  int xrej = a < gamma ? draft_tokens[r0 + a + 1] : -1;
+  if (xrej >= V || xrej < 0) xrej = -1;                                 // an out-of-range draft (flagged above) removes no mass
   const float Mr = s_M[a];
   const double Zinv = 1.0 / s_Z[a];
   const float Zinv_f = (float)Zinv;
@@ -318,13 +332,13 @@ wf_accept_kernel(const float* __restrict__ logits, int V, int n_chunks, const in
   double base = 0.0;                                       // mass below lo
   int levels = 2;
   if (!qr && n_chunks <= ACC_THREADS) {
-    const AccPartial* pr = &partials[(size_t)(r0 + a) * n_chunks];
+    const AccPartial* pr = &partials[(prow0 + a) * n_chunks];
     for (int attempt = 0; attempt < 2; ++attempt) {
       double mc = 0.0;
       if (tid < n_chunks) {
         const float pm = __ldcg(&pr[tid].m);
         if (pm > -INFINITY) mc = (double)__ldcg(&pr[tid].Z) * exp((double)pm - (double)Mr) * Zinv;
-        if (s_resid && xrej / ACC_CHUNK == tid)
+        if (s_resid && xrej >= 0 && xrej / ACC_CHUNK == tid)
           mc = fmax(0.0, mc - exp((double)(zr[xrej] * smp.inv_t) - (double)Mr) * Zinv);
       }
       s_seg[tid] = mc;
@@ -552,15 +566,15 @@ int accept_launch(wf_ctx* ctx, const float* logits, int V, const int32_t* draft_
   WF_REQUIRE(ctx, workspace_bytes >= wf_accept_workspace_bytes(B * max_q_len, V), WF_ERR_INVALID_ARG, "wf_accept_entropy_route: workspace too small");
   dim3 grid(n_chunks, max_q_len, B);
   int32_t* kv_len = target_kv ? target_kv->seq_len : nullptr;
-  const bool vec = (V % 4 == 0) && ((uintptr_t)logits % 16 == 0);
+  const bool vec = (V % 4 == 0) && ((uintptr_t)logits % 16 == 0) && (!smp.draft_q || (uintptr_t)smp.draft_q % 16 == 0);
   if (vec)
     wf_launch(wf_accept_kernel<true>, grid, dim3(ACC_THREADS), 0, st, logits, V, n_chunks, draft_tokens, q_indptr, tau,
         tau_is_scalar, accept_len, bonus_token, entropy, route, n_commit, kv_len, (AccPartial*)workspace, ctx->d_counters,
-        parent, path, path_stride, smp);
+        parent, path, path_stride, smp, ctx->d_status);
   else
     wf_launch(wf_accept_kernel<false>, grid, dim3(ACC_THREADS), 0, st, logits, V, n_chunks, draft_tokens, q_indptr, tau,
         tau_is_scalar, accept_len, bonus_token, entropy, route, n_commit, kv_len, (AccPartial*)workspace, ctx->d_counters,
-        parent, path, path_stride, smp);
+        parent, path, path_stride, smp, ctx->d_status);
   return wf_check_launch(ctx, "wf_accept_kernel");
 }
 }  // namespace

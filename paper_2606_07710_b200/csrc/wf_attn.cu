@@ -55,6 +55,7 @@ struct AttnParams {
   float4* ws_o;                        // [2 * CTAs][D/8][128 threads] float4: unnormalised O in fragment order
   float4* ws_ml;                       // [2 * CTAs][128 threads] (m, l) of the thread's two rows (m in log2 units)
   unsigned int* counters;              // [B * Hkv] arrived | published << 16, self-resetting
+  int* status;                         // sticky device status word
 };
 
 // TREE: the query tile has 128 rows (UMMA M = 128): two 64-row sub-blocks of a draft tree stacked on the TMEM lanes, rows
@@ -930,6 +931,8 @@ __global__ void __launch_bounds__(AT_THREADS, 1) wf_verify_attn_kernel(const Att
   int* t_q = t_ctx + AT_MAX_B;
   for (int b = tid; b < p.B; b += AT_THREADS) {
     const int r0 = p.q_indptr[b], r1 = p.q_indptr[b + 1], ctx = p.kv.seq_len[b];
+    // the host bound max_q_len / max_nodes is a promise: a longer block has its rows beyond the query tile dropped
+    if (blockIdx.x == 0 && (TREE ? r1 - r0 > 64 : (r1 - r0) * p.group > AT_ROWS)) wf_raise(p.status, (int)WF_ERR_INVALID_ARG);
     if constexpr (TREE) {
       t_r0[b] = r0;
       t_ctx[b] = ctx;
@@ -1046,12 +1049,8 @@ namespace {
 
 template <int D, bool TREE>
 int launch_attn(wf_ctx* ctx, const AttnParams& p, cudaStream_t st) {
-  static bool configured = false;
   const size_t smem = AttnCfg<D, TREE>::SMEM;
-  if (!configured) {
-    WF_CUDA(ctx, cudaFuncSetAttribute(wf_verify_attn_kernel<D, TREE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    configured = true;
-  }
+  WF_CONFIGURE_ONCE(ctx, (TREE ? WF_FUNC_ATTN_TREE_128 : WF_FUNC_ATTN_128) + (D == 64 ? 1 : 0), (wf_verify_attn_kernel<D, TREE>), smem);
   const int grid = ctx->sm_count < AT_MAX_CTAS ? ctx->sm_count : AT_MAX_CTAS;   // one persistent CTA per SM
   wf_launch(wf_verify_attn_kernel<D, TREE>, dim3(grid), dim3(AT_THREADS), smem, st, p);
   return wf_check_launch(ctx, TREE ? "wf_verify_attn_kernel<tree>" : "wf_verify_attn_kernel");
@@ -1121,6 +1120,7 @@ extern "C" int wf_verify_attn(wf_ctx* ctx, const wf_paged_kv* kv, int layer, con
   p.ws_o = (float4*)workspace;
   p.ws_ml = (float4*)((char*)workspace + items * r_pad * kv->s.head_dim * sizeof(float));
   p.counters = ctx->d_counters_attn;
+  p.status = ctx->d_status;
   cudaStream_t st = (cudaStream_t)stream;
   const int D = kv->s.head_dim;
   p.tree_mask = nullptr;
@@ -1174,6 +1174,7 @@ extern "C" int wf_verify_attn_tree(wf_ctx* ctx, const wf_paged_kv* kv, int layer
   p.ws_o = (float4*)workspace;
   p.ws_ml = (float4*)((char*)workspace + items * AT_ROWS * kv->s.head_dim * sizeof(float));
   p.counters = ctx->d_counters_attn;
+  p.status = ctx->d_status;
   cudaStream_t st = (cudaStream_t)stream;
   const int D = kv->s.head_dim;
   if (D == 128) return launch_attn<128, true>(ctx, p, st);

@@ -65,6 +65,8 @@ extern "C" int wf_ctx_create(wf_ctx** out, int device_ordinal) {
   c->device = device_ordinal;
   c->sm_count = prop.multiProcessorCount;
   c->launches = 0;
+  c->func_configured = 0;
+  c->deterministic = 0;
   c->err[0] = 0;
   c->n_counters = 1 << 16;
   if (cudaMalloc(&c->d_status, sizeof(int)) != cudaSuccess ||

@@ -18,8 +18,24 @@ struct wf_ctx {
   unsigned int* d_counters_attn; // same, per (sequence, kv head), for the split-KV combine
   int n_counters;
   int64_t launches;            // kernels launched through this ctx (host counter)
+  unsigned int func_configured; // bit k: kernel k's dynamic-smem opt-in was made on THIS ctx's device (WF_FUNC_*)
+  int deterministic;           // wf_ctx_set_deterministic: fixed-order split merges
   char err[256];
 };
+
+// kernels that need cudaFuncSetAttribute(MaxDynamicSharedMemorySize): the attribute is per device, so the
+// bookkeeping is per ctx (a ctx is bound to one device), never per process
+enum {
+  WF_FUNC_ATTN_128 = 0, WF_FUNC_ATTN_64, WF_FUNC_ATTN_TREE_128, WF_FUNC_ATTN_TREE_64, WF_FUNC_GEMM_128, WF_FUNC_GEMM_64,
+  WF_FUNC_NEURAL, WF_FUNC_ACCEPT, WF_FUNC_FINAL_TOKEN, WF_FUNC_GEMV
+};
+#define WF_CONFIGURE_ONCE(ctx, bit, kernel, bytes)                                                          \
+  do {                                                                                                      \
+    if (!((ctx)->func_configured & (1u << (bit)))) {                                                        \
+      WF_CUDA((ctx), cudaFuncSetAttribute((kernel), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(bytes))); \
+      (ctx)->func_configured |= 1u << (bit);                                                                \
+    }                                                                                                       \
+  } while (0)
 
 struct wf_paged_kv {
   wf_ctx* ctx;
@@ -84,6 +100,8 @@ int wf_check_launch(wf_ctx* ctx, const char* what);   // cudaGetLastError -> WF_
 #ifdef __CUDACC__
 __device__ __forceinline__ void wf_pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 __device__ __forceinline__ void wf_pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+// sticky device status: the FIRST error of a poll interval wins (a later one never overwrites it)
+__device__ __forceinline__ void wf_raise(int* status, int code) { atomicCAS(status, 0, code); }
 
 template <typename... KArgs, typename... Args>
 inline cudaError_t wf_launch(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args&&... args) {
@@ -169,7 +187,7 @@ __device__ inline bool kv_reserve_block(const KvView& kv, int B, AddFn add, SeqF
   }
   const int total = s_carry;
   if (s_bad || total > count) {
-    if (tid == 0) *status = WF_ERR_OUT_OF_PAGES;
+    if (tid == 0) wf_raise(status, (int)WF_ERR_OUT_OF_PAGES);
     return false;
   }
   for (int b = wid; b < B; b += nw) {            // one warp per sequence copies its ring entries

@@ -163,11 +163,7 @@ extern "C" int wf_neural_route(wf_ctx* ctx, const void* hidden_final, const int3
   WF_REQUIRE(ctx, workspace_bytes >= wf_neural_route_workspace_bytes(B, m), WF_ERR_INVALID_ARG, "wf_neural_route: workspace too small");
   if (B == 0) return WF_OK;
   const size_t smem = (size_t)NR_TILE_B * d * 2;
-  static bool configured = false;
-  if (!configured) {
-    WF_CUDA(ctx, cudaFuncSetAttribute(wf_neural_route_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
-    configured = true;
-  }
+  WF_CONFIGURE_ONCE(ctx, WF_FUNC_NEURAL, wf_neural_route_kernel, 200 * 1024);
   NeuralParams p;
   p.hidden = (const __nv_bfloat16*)hidden_final; p.q_indptr = q_indptr; p.accept_len = accept_len;
   p.w1 = (const __nv_bfloat16*)w1; p.b1 = b1; p.w2 = (const __nv_bfloat16*)w2; p.b2 = b2; p.tau = tau;

@@ -33,93 +33,125 @@ constexpr int PF_BLOCK_M = 128;         // UMMA M
 constexpr int PF_BLOCK_K = 64;          // one 128-byte swizzle row of bf16
 constexpr int PF_KSUB = 2;              // 64-wide k-blocks per pipeline stage: halves the per-stage hand-offs of the one-thread loops
 constexpr int PF_MAX_MT = 2;            // m-tiles per pass (TMEM columns = PF_MAX_MT * D)
-constexpr int PF_THREADS = 192;         // warp 0: bulk-copy producer, warp 1: MMA, warps 2-5: epilogue
+constexpr int PF_THREADS = 192;         // warp 0: bulk-copy producer, warp 1: MMA, warps 2-5: epilogue (+ enqueue, commit)
 constexpr int PF_SMEM_BUDGET = 200 * 1024;
+constexpr int PP_THREADS = 256;         // plan + pack kernel
+constexpr int PP_MAX_B = KV_RESERVE_SMEM;   // sequences per call (the per-sequence plan lives in shared memory)
+constexpr int PP_MAX_PACK_CTAS = 296;   // pack CTAs per drafter: two per SM
 struct RowEntry {
-  const __nv_bfloat16* src;             // hidden row
   int32_t pos;                          // absolute position (RoPE)
   int32_t page_slot;                    // physical page * 16 + slot in the drafter cache
 };
 
-// ---- the plan kernel -------------------------------------------------------------------------
-// PLAN_ROUND fuses what one round asks of a drafter into ONE projection: block rows of the sequences it is active for,
-// backlog + block rows of the sequences that switch to it (flush), a forced flush where an enqueue would overflow;
-// the rows of idle sequences are enqueued afterwards (wf_enqueue_round_kernel) at the offsets this plan decides.
-enum PlanMode { PLAN_EAGER = 0, PLAN_FLUSH = 1, PLAN_FORCED = 2, PLAN_ROUND = 3 };
+// ---- kernel 1 of 2: plan + pack ------------------------------------------------------------------
+// What one call asks of a drafter, per sequence b (seq = seq_ids ? seq_ids[b] : b, len = its backlog length, add = n_rows[b]):
+//   EAGER   : the block rows are projected (wf_kv_only_prefill).
+//   FLUSH   : the backlog of every flagged sequence is projected (wf_lazy_catchup_flush).
+//   ENQUEUE : the block rows of idle sequences are enqueued; a backlog they would overflow is projected first (C20).
+//   ROUND   : everything a round asks of the drafter in ONE projection: active sequences (not idle) and sequences that
+//             switch to it (idle and flush) get backlog + block rows projected; the others are enqueued as in ENQUEUE.
+//             idle / flush come from host-planned masks (wf_lazy_catchup_round) or, device-driven, from the router's
+//             output: idle = cur[b] != code, flush = idle && route[b] == code (wf_switch_round, reading C21).
+// Every CTA of the launch derives the same per-sequence plan in shared memory from the device-resident inputs (they are
+// read-only in this kernel: lengths that the call changes are committed by kernel 2).  CTA 0 of a drafter is its PLANNER:
+// reserves pages (C24), writes the row table (RoPE position, physical page*16+slot), the enqueue offsets and the new
+// backlog lengths, and advances the cache length.  The other CTAs PACK: row r of the call -> the shared-memory image
+// of the X operand, k-block by k-block (xpack[hidden/64][m_pad][128 B], K-major, 16-byte chunks XOR-swizzled with r & 7),
+// so that a projection CTA fetches a stage's X with one bulk copy.  Two drafters share one launch (blockIdx picks).
+enum PlanMode { PLAN_EAGER = 0, PLAN_FLUSH = 1, PLAN_ENQUEUE = 2, PLAN_ROUND = 3 };
 
-struct PlanParams {
-  int mode, B, hidden, cap, max_pos, row_cap;
-  const __nv_bfloat16* hidden_rows;     // EAGER: block hidden states [sum_q][hidden]
-  const int32_t* q_indptr;              // EAGER / FORCED
-  const int32_t* n_rows;                // EAGER / FORCED
-  const int32_t* seq_ids;               // EAGER / FORCED (NULL = identity)
-  const int32_t* mask;                  // FLUSH: flush_mask (NULL = all); FORCED / ROUND: idle_mask (ROUND: NULL = none idle)
-  const int32_t* mask2;                 // ROUND: flush_mask (NULL = none)
-  int32_t* enq_base;                    // ROUND: [B] backlog offset at which the block rows are enqueued afterwards, -1 = none
+struct PlanJob {
+  int mode, B, hidden, cap, max_pos, row_cap, max_rows;
+  int code;                             // ROUND, device-driven: this drafter's route code (WF_ROUTE_AR / WF_ROUTE_DIFFUSION)
+  const __nv_bfloat16* hidden_rows;     // block hidden states [sum_q][hidden]
+  const int32_t* q_indptr;
+  const int32_t* n_rows;
+  const int32_t* seq_ids;               // NULL = identity
+  const int32_t* idle_mask;             // ENQUEUE / ROUND (host masks; NULL = none idle)
+  const int32_t* flush_mask;            // FLUSH (NULL = all) / ROUND (host masks; NULL = none)
+  const int32_t* route;                 // ROUND, device-driven (route != NULL): the router's output this round
+  const int32_t* cur;                   //                       the drafter that drafted this round's block
   const __nv_bfloat16* backlog;         // [max_seqs][cap][hidden]
-  int32_t* backlog_len;
+  const int32_t* backlog_len;
   KvView kv;
   RowEntry* rows;
   int32_t* m_total;
-  int32_t* plan_n;                      // [max_seqs] rows of sequence b in this call
-  int32_t* plan_off;                    // [max_seqs] first compact row of sequence b
+  int32_t* enq_base;                    // [B] backlog offset at which kernel 2 enqueues the block rows, -1 = none
+  int32_t* new_blen;                    // [B] backlog length kernel 2 commits, -1 = unchanged
+  uint8_t* xpack;
   int* status;
 };
 
-__global__ void __launch_bounds__(1024) wf_prefill_plan_kernel(const PlanParams p) {
+struct PlanPackParams {
+  PlanJob job[2];
+  int n_jobs, ctas_job0;                // CTAs [0, ctas_job0) serve job 0, the rest job 1
+};
+
+__global__ void __launch_bounds__(PP_THREADS) wf_plan_pack_kernel(const __grid_constant__ PlanPackParams pp) {
   __shared__ int s_warp[32];
   __shared__ int s_carry;
-  // rows / first compact row per sequence: shared memory for the first 1024 sequences, global scratch beyond
-  __shared__ int s_pn[KV_RESERVE_SMEM], s_po[KV_RESERVE_SMEM];
-  // ROUND (B <= 1024): backlog rows at the front of b's rows, backlog length after the call, enqueue offset (-1 = none)
-  __shared__ int s_nb[KV_RESERVE_SMEM], s_nl[KV_RESERVE_SMEM], s_eb[KV_RESERVE_SMEM];
-  auto plan_n = [&](int b) -> int& { return b < KV_RESERVE_SMEM ? s_pn[b] : p.plan_n[b]; };
-  auto plan_off = [&](int b) -> int& { return b < KV_RESERVE_SMEM ? s_po[b] : p.plan_off[b]; };
-  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5, nw = blockDim.x >> 5;
+  __shared__ int s_n[PP_MAX_B], s_nb[PP_MAX_B], s_off[PP_MAX_B + 1], s_eb[PP_MAX_B], s_nl[PP_MAX_B];
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5, nw = PP_THREADS >> 5;
   wf_pdl_trigger();
   wf_pdl_wait();
-  auto seq_of = [&](int b) { return (p.mode != PLAN_FLUSH && p.seq_ids) ? p.seq_ids[b] : b; };
-  // rows each sequence contributes to this call
-  for (int b = tid; b < p.B; b += blockDim.x) {
+  const int jb = (int)blockIdx.x >= pp.ctas_job0 ? 1 : 0;
+  const PlanJob& p = pp.job[jb];
+  const int c = (int)blockIdx.x - (jb ? pp.ctas_job0 : 0);
+  const int n_pack = (jb ? (int)gridDim.x - pp.ctas_job0 : pp.ctas_job0) - 1;
+  const bool planner = c == 0;
+  auto seq_of = [&](int b) { return p.seq_ids ? p.seq_ids[b] : b; };
+  // ---- the per-sequence plan (every CTA, identical) ----
+  for (int b = tid; b < p.B; b += PP_THREADS) {
     const int sq = seq_of(b);
-    int n;
-    if (p.mode == PLAN_ROUND) {
-      const int add = p.n_rows[b], len = p.cap > 0 ? p.backlog_len[sq] : 0;
-      const bool idle = p.mask && p.mask[b], fl = p.mask2 && p.mask2[b];
-      const bool project_block = !idle || fl;
-      int n_enq = project_block ? 0 : add;
-      if (n_enq > p.cap) { *p.status = WF_ERR_QUEUE_OVERFLOW; n_enq = 0; }     // rows skipped, as in enqueue
-      // the backlog goes first whenever anything of this sequence is projected (FIFO), or when the enqueue would overflow
-      const int n_back = (project_block || len + n_enq > p.cap) ? len : 0;
-      s_nb[b] = n_back;
-      n = n_back + (project_block ? add : 0);
-      s_eb[b] = n_enq > 0 ? (n_back > 0 ? 0 : len) : -1;
-      s_nl[b] = (n_back > 0 ? 0 : len) + n_enq;
-    } else if (p.mode == PLAN_EAGER) {
-      n = p.n_rows[b];
-    } else if (p.mode == PLAN_FLUSH) {
-      n = (!p.mask || p.mask[b]) ? p.backlog_len[sq] : 0;
-    } else {                                                   // forced flush before an enqueue (C20)
-      const int add = p.n_rows[b];
-      if (p.mask[b] && add > p.cap) *p.status = WF_ERR_QUEUE_OVERFLOW;
-      n = (p.mask[b] && add <= p.cap && p.backlog_len[sq] + add > p.cap) ? p.backlog_len[sq] : 0;
+    const int len = p.cap > 0 ? p.backlog_len[sq] : 0;
+    int add = p.mode == PLAN_FLUSH ? 0 : p.n_rows[b];
+    if (add > p.max_rows || add < 0) {                         // the host bound sizes the launch: clamp, never overrun
+      if (planner) wf_raise(p.status, (int)WF_ERR_INVALID_ARG);
+      add = min(max(add, 0), p.max_rows);
     }
-    plan_n(b) = n;
+    bool idle = false, fl = false;
+    if (p.mode == PLAN_ROUND) {
+      if (p.route) { idle = p.cur[b] != p.code; fl = idle && p.route[b] == p.code; }
+      else { idle = p.idle_mask && p.idle_mask[b]; fl = p.flush_mask && p.flush_mask[b]; }
+    } else if (p.mode == PLAN_ENQUEUE) {
+      idle = p.idle_mask[b] != 0;
+    } else if (p.mode == PLAN_FLUSH) {
+      fl = !p.flush_mask || p.flush_mask[b];
+    }
+    int n_back = 0, n_blk = 0, n_enq = 0;
+    if (p.mode == PLAN_EAGER) n_blk = add;
+    else if (p.mode == PLAN_FLUSH) n_back = fl ? len : 0;
+    else {
+      const bool project_block = p.mode == PLAN_ROUND && (!idle || fl);
+      n_enq = (idle && !project_block) ? add : 0;
+      if (n_enq > p.cap) {                                     // one round's rows alone exceed the cap: skipped (R1)
+        if (planner) wf_raise(p.status, (int)WF_ERR_QUEUE_OVERFLOW);
+        n_enq = 0;
+      }
+      // the backlog goes first whenever anything of this sequence is projected (FIFO), or when the enqueue would overflow
+      n_back = (project_block || (n_enq > 0 && len + n_enq > p.cap)) ? len : 0;
+      n_blk = project_block ? add : 0;
+    }
+    s_nb[b] = n_back;
+    s_n[b] = n_back + n_blk;
+    s_eb[b] = n_enq > 0 ? (n_back > 0 ? 0 : len) : -1;
+    s_nl[b] = (p.mode == PLAN_EAGER || p.cap == 0) ? -1 : (n_back > 0 ? 0 : len) + n_enq;
   }
   if (tid == 0) s_carry = 0;
   __syncthreads();
-  // pages first (C24: ascending b, consecutive ring entries); nothing is written if they do not fit
-  const bool ok = kv_reserve_block(p.kv, p.B, [&](int b) { return plan_n(b); }, seq_of, p.status);
-  if (!ok) {                                                   // nothing is projected, nothing is enqueued, no length moves
+  auto nothing = [&]() {                                       // planner: the call projects and enqueues nothing
     if (tid == 0) *p.m_total = 0;
-    if (p.mode == PLAN_ROUND)
-      for (int b = tid; b < p.B; b += blockDim.x) p.enq_base[b] = -1;
-    return;
+    for (int b = tid; b < p.B; b += PP_THREADS) { p.enq_base[b] = -1; p.new_blen[b] = -1; }
+  };
+  // pages first (C24: ascending b, consecutive ring entries); nothing is written if they do not fit
+  if (planner) {
+    const bool ok = kv_reserve_block(p.kv, p.B, [&](int b) { return s_n[b]; }, seq_of, p.status);
+    if (!ok) { nothing(); return; }
   }
-  // exclusive scan of plan_n -> plan_off
-  for (int base = 0; base < p.B; base += blockDim.x) {
+  // exclusive scan of the row counts -> first compact row of each sequence
+  for (int base = 0; base < p.B; base += PP_THREADS) {
     const int b = base + tid;
-    const int n = b < p.B ? plan_n(b) : 0;
+    const int n = b < p.B ? s_n[b] : 0;
     int x = n;
 #pragma unroll
     for (int d = 1; d < 32; d <<= 1) {
@@ -138,71 +170,65 @@ __global__ void __launch_bounds__(1024) wf_prefill_plan_kernel(const PlanParams 
       s_warp[lane] = w;
     }
     __syncthreads();
-    if (b < p.B) plan_off(b) = s_carry + (wid ? s_warp[wid - 1] : 0) + x - n;
+    if (b < p.B) s_off[b] = s_carry + (wid ? s_warp[wid - 1] : 0) + x - n;
     __syncthreads();
     if (tid == 0) s_carry += s_warp[nw - 1];
     __syncthreads();
   }
   const int total = s_carry;
   if (total > p.row_cap) {                                     // host bounds make this unreachable
-    if (tid == 0) { *p.status = WF_ERR_INVALID_ARG; *p.m_total = 0; }
+    if (planner) { if (tid == 0) wf_raise(p.status, (int)WF_ERR_INVALID_ARG); nothing(); }
     return;
   }
-  // row table: one warp per sequence
-  for (int b = wid; b < p.B; b += nw) {
+  if (planner) {
+    // row table: one warp per sequence
+    for (int b = wid; b < p.B; b += nw) {
+      const int sq = seq_of(b);
+      const int n = s_n[b], off = s_off[b];
+      const int p0 = p.kv.seq_len[sq];
+      for (int t = lane; t < n; t += 32) {
+        const int pos = p0 + t;
+        if (pos >= p.max_pos) wf_raise(p.status, (int)WF_ERR_INVALID_ARG);
+        const int page = p.kv.block_table[(size_t)sq * p.kv.max_pages_per_seq + (pos >> 4)];
+        RowEntry e;
+        e.pos = min(pos, p.max_pos - 1);
+        e.page_slot = page * 16 + (pos & 15);
+        p.rows[off + t] = e;
+      }
+      __syncwarp();
+      if (lane == 0) {
+        p.enq_base[b] = s_eb[b];
+        p.new_blen[b] = s_nl[b];
+        if (n > 0) p.kv.seq_len[sq] = p0 + n;
+      }
+    }
+    if (tid == 0) *p.m_total = total;
+    return;
+  }
+  // ---- pack: rows c-1, c-1+n_pack, ... of the call ----
+  const int m_pad = (total + 7) & ~7;
+  const size_t kb_stride = (size_t)m_pad * 128;
+  for (int r = c - 1; r < total; r += n_pack) {
+    int lo = 0, hi = p.B;                                      // the sequence whose rows hold r: largest b with off[b] <= r
+    while (hi - lo > 1) {                                      // and n[b] > 0 (empty sequences share their successor's offset)
+      const int mid = (lo + hi) >> 1;
+      if (s_off[mid] <= r) lo = mid; else hi = mid;
+    }
+    const int b = lo, t = r - s_off[b];
     const int sq = seq_of(b);
-    const int n = plan_n(b), off = plan_off(b);
-    const int p0 = p.kv.seq_len[sq];
-    const bool from_block = p.mode == PLAN_EAGER || p.mode == PLAN_ROUND;
-    const int n_back = p.mode == PLAN_ROUND ? s_nb[b] : (from_block ? 0 : n);
-    const __nv_bfloat16* blk = from_block ? p.hidden_rows + (size_t)p.q_indptr[b] * p.hidden : nullptr;
-    const __nv_bfloat16* bkl = p.backlog + (size_t)sq * p.cap * p.hidden;
-    for (int t = lane; t < n; t += 32) {
-      const int pos = p0 + t;
-      if (pos >= p.max_pos) *p.status = WF_ERR_INVALID_ARG;
-      const int page = p.kv.block_table[(size_t)sq * p.kv.max_pages_per_seq + (pos >> 4)];
-      RowEntry e;
-      e.src = t < n_back ? bkl + (size_t)t * p.hidden : blk + (size_t)(t - n_back) * p.hidden;
-      e.pos = min(pos, p.max_pos - 1);
-      e.page_slot = page * 16 + (pos & 15);
-      p.rows[off + t] = e;
-    }
-    __syncwarp();
-    if (lane == 0 && p.mode == PLAN_ROUND) {
-      p.enq_base[b] = s_eb[b];
-      if (p.cap > 0) p.backlog_len[sq] = s_nl[b];
-    }
-    if (lane == 0 && n > 0) {
-      p.kv.seq_len[sq] = p0 + n;
-      if (p.mode == PLAN_FLUSH || p.mode == PLAN_FORCED) p.backlog_len[sq] = 0;
+    const __nv_bfloat16* srow = t < s_nb[b] ? p.backlog + ((size_t)sq * p.cap + t) * p.hidden
+                                            : p.hidden_rows + (size_t)(p.q_indptr[b] + t - s_nb[b]) * p.hidden;
+    const uint4* src = reinterpret_cast<const uint4*>(srow);
+    uint8_t* dst = p.xpack + (size_t)r * 128;
+    for (int q = tid; q < p.hidden / 8; q += PP_THREADS) {   // 16-byte chunk q of the row -> k-block q/8, chunk q%8
+      const uint4 v = __ldg(src + q);
+      *reinterpret_cast<uint4*>(dst + (size_t)(q >> 3) * kb_stride + (((q & 7) ^ (r & 7)) << 4)) = v;
     }
   }
-  if (tid == 0) *p.m_total = total;
 }
 
 // ---- the projection kernel ------------------------------------------------------------------
 constexpr int PF_MAX_STAGES = 12;
-
-// Per call: the rows of the plan's row table -> the shared-memory image of the A operand, k-block by k-block:
-// xpack[kb][m_pad][128 B], row m of k-block kb = X[m][64 kb .. 64 kb + 63], 16-byte chunks XOR-swizzled with (m & 7)
-// (K-major, 128-byte swizzle).  One block per row; every projection CTA then fetches a stage's A operand with
-// one bulk copy instead of gathering it with 128 threads.
-__global__ void __launch_bounds__(256) wf_pack_x_kernel(const RowEntry* __restrict__ rows, const int32_t* __restrict__ m_total,
-                                                        uint8_t* __restrict__ xpack, int hidden) {
-  wf_pdl_trigger();
-  wf_pdl_wait();
-  const int M = *m_total;
-  const int r = blockIdx.x;                              // one row per block: every load of the block is independent
-  if (r >= M) return;
-  const int m_pad = (M + 7) & ~7;
-  const uint4* src = reinterpret_cast<const uint4*>(rows[r].src);
-  uint8_t* dst = xpack + (size_t)r * 128;
-  const size_t kb_stride = (size_t)m_pad * 128;
-  for (int q = threadIdx.x; q < hidden / 8; q += 256) {  // 16-byte chunk q of the row -> k-block q/8, chunk q%8
-    const uint4 v = __ldg(src + q);
-    *reinterpret_cast<uint4*>(dst + (size_t)(q >> 3) * kb_stride + (((q & 7) ^ (r & 7)) << 4)) = v;
-  }
-}
 
 // One-time repack of a drafter's weights (wf_drafter_create) into the exact shared-memory image of a W stage:
 // tile (layer, K|V, head) x k-block of 64 rows -> D/64 column halves x [64 k][128 B], 16-byte chunks XOR-swizzled
@@ -220,9 +246,10 @@ __global__ void wf_pack_w_kernel(const __nv_bfloat16* __restrict__ w, uint8_t* _
   }
 }
 
-struct GemmParams {
+// ---- kernel 2 of 2: projection + enqueue + commit ----------------------------------------------------
+struct GemmJob {
   const uint8_t* wpack;                 // [n_layers][2][Hkv][hidden/64][64 * D * 2 B] pre-swizzled W stages
-  const uint8_t* xpack;                 // [hidden/64][m_pad][128 B] pre-swizzled X k-blocks of this call (wf_pack_x_kernel)
+  const uint8_t* xpack;                 // [hidden/64][m_pad][128 B] pre-swizzled X k-blocks of this call (kernel 1)
   const RowEntry* rows;
   const int32_t* m_total;
   const float2* rope;                   // [max_pos][D/2] (cos, sin)
@@ -234,10 +261,30 @@ struct GemmParams {
   int n_split, row_cap, max_pass;
   float* ws_part;
   unsigned int* split_cnt;
+  // enqueue (ENQUEUE / ROUND): block row t of sequence b -> backlog[seq][enq_base[b] + t]; commit: backlog lengths
+  const __nv_bfloat16* hidden_rows;
+  const int32_t* q_indptr;
+  const int32_t* n_rows;
+  const int32_t* seq_ids;
+  const int32_t* enq_base;              // NULL: the call enqueues nothing
+  const int32_t* new_blen;              // NULL: the call changes no backlog length
+  __nv_bfloat16* backlog;
+  int32_t* backlog_len;
+  int B, cap, max_rows;
+  // device-driven switch (wf_switch_round; job 0 commits): cur <- route, next block length per sequence
+  const int32_t* route;
+  int32_t* cur;
+  int32_t* next_q_len;                  // nullable
+  int q_len_ar, q_len_diffusion;
+};
+
+struct GemmParams {
+  GemmJob job[2];
+  int n_jobs, ctas_job0;
 };
 
 template <int D>
-__global__ void __launch_bounds__(PF_THREADS, 1) wf_prefill_gemm_kernel(const GemmParams p) {
+__global__ void __launch_bounds__(PF_THREADS, 1) wf_prefill_gemm_kernel(const __grid_constant__ GemmParams gp) {
   // Swapped operands: out^T[D x tokens] = W^T[D x hidden] . X^T[hidden x tokens].  The head's D output columns are the
   // UMMA M dimension (always issued as M = 128; for D = 64 the upper 64 lanes compute on whatever follows in the
   // ring and are never read), the call's tokens are the UMMA N dimension (padded to 16).  An MMA then costs
@@ -254,11 +301,49 @@ __global__ void __launch_bounds__(PF_THREADS, 1) wf_prefill_gemm_kernel(const Ge
 
   wf_pdl_trigger();
   wf_pdl_wait();
-  const int M = *p.m_total;
-  if (M == 0) return;                                  // nothing queued for this call
+  const int jb = (int)blockIdx.x >= gp.ctas_job0 ? 1 : 0;
+  const GemmJob& p = gp.job[jb];
+  const int cta = (int)blockIdx.x - (jb ? gp.ctas_job0 : 0);
+  const int n_ctas = jb ? (int)gridDim.x - gp.ctas_job0 : gp.ctas_job0;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int tile = blockIdx.x / p.n_split;             // (layer, K|V, kv head)
-  const int split = blockIdx.x % p.n_split;            // this CTA's share of the k-blocks
+  const int M = *p.m_total;
+
+  // Enqueue and commit ride on this kernel (kernel 1 has packed the projection's operand, backlog rows included, so
+  // the backlog may be overwritten; nobody in this kernel reads a length).  The (sequence, row) pairs are dealt
+  // round-robin to the drafter's CTAs; its CTA 0 commits the backlog lengths the planner decided, and job 0's CTA 0
+  // the switch itself (cur <- route, the next block's length).  The epilogue warps do it while the operands stream.
+  auto enqueue_commit = [&](int t0, int nt) {
+    if (p.enq_base) {
+      for (int pair = cta; pair < p.B * p.max_rows; pair += n_ctas) {
+        const int b = pair / p.max_rows, t = pair % p.max_rows;
+        const int base = p.enq_base[b];
+        if (base < 0 || t >= p.n_rows[b]) continue;
+        const int sq = p.seq_ids ? p.seq_ids[b] : b;
+        const uint4* src = reinterpret_cast<const uint4*>(p.hidden_rows + (size_t)(p.q_indptr[b] + t) * p.hidden);
+        uint4* dst = reinterpret_cast<uint4*>(p.backlog + ((size_t)sq * p.cap + base + t) * p.hidden);
+        for (int i = t0; i < p.hidden / 8; i += nt) dst[i] = __ldg(src + i);
+      }
+    }
+    if (cta == 0) {
+      if (p.new_blen)
+        for (int b = t0; b < p.B; b += nt) {
+          const int nl = p.new_blen[b];
+          if (nl >= 0) p.backlog_len[p.seq_ids ? p.seq_ids[b] : b] = nl;
+        }
+      if (p.route && jb == 0)
+        for (int b = t0; b < p.B; b += nt) {
+          const int r = p.route[b];
+          p.cur[b] = r;
+          if (p.next_q_len) p.next_q_len[b] = r == WF_ROUTE_AR ? p.q_len_ar : p.q_len_diffusion;
+        }
+    }
+  };
+  if (M == 0) {                                        // nothing to project for this drafter: no barriers, no TMEM
+    enqueue_commit(tid, PF_THREADS);
+    return;
+  }
+  const int tile = cta / p.n_split;                    // (layer, K|V, kv head)
+  const int split = cta % p.n_split;                   // this CTA's share of the k-blocks
   const int layer = tile / (2 * p.n_kv_heads);
   const int is_v = (tile / p.n_kv_heads) & 1;
   const int head = tile % p.n_kv_heads;
@@ -367,6 +452,7 @@ __global__ void __launch_bounds__(PF_THREADS, 1) wf_prefill_gemm_kernel(const Ge
     const int quarter = warp & 3;                        // TMEM lane quarter this warp may read
     const int et = quarter * 32 + lane;                  // 0..127
     float* tr = reinterpret_cast<float*>(smem);          // [tokens][D] fp32
+    enqueue_commit(et, 128);                             // while the first stages stream
     constexpr int PC = D / 16;                           // column-pair chunks per token
     for (int pass = 0; pass < n_pass; ++pass) {
       const int m_base = pass * N_MAX;
@@ -504,46 +590,75 @@ struct wf_drafter {
   RowEntry* d_rows;
   int row_cap;
   int32_t* d_m_total;
-  int32_t* d_plan;             // [3 * max_seqs]: plan_n, plan_off, enq_base
+  int32_t* d_plan;             // [2 * max_seqs]: enq_base, new_blen (planner -> kernel 2)
 };
 
 namespace {
 
-template <int D>
-int launch_gemm(wf_drafter* d, cudaStream_t st) {
-  wf_ctx* ctx = d->ctx;
-  static bool configured = false;
-  if (!configured) {
-    WF_CUDA(ctx, cudaFuncSetAttribute(wf_prefill_gemm_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, PF_SMEM_BUDGET));
-    configured = true;
+// One call = ONE launch of each of the two kernels, for one drafter or for both drafters of a round.  This is the only
+// device path behind eager prefill, flush, enqueue (with its forced flush) and the fused round calls.
+struct CallJob {
+  wf_drafter* d;
+  PlanJob plan;                         // mode, B, inputs and masks filled by the caller
+  int rows_upper;                       // host upper bound of the rows the call projects (sizes the pack grid)
+  bool enqueues;                        // ENQUEUE / ROUND with idle sequences
+};
+
+int run_jobs(wf_ctx* ctx, CallJob* jobs, int n_jobs, const int32_t* route, int32_t* cur, int32_t* next_q_len, int q_len_ar,
+             int q_len_diffusion, cudaStream_t st) {
+  PlanPackParams pp{};
+  GemmParams gp{};
+  pp.n_jobs = gp.n_jobs = n_jobs;
+  int pack_grid = 0, gemm_grid = 0;
+  const int D = jobs[0].d->s.head_dim;
+  for (int j = 0; j < n_jobs; ++j) {
+    wf_drafter* d = jobs[j].d;
+    PlanJob& pj = jobs[j].plan;
+    const int S = d->kv->s.max_seqs;
+    pj.hidden = d->s.hidden; pj.cap = d->s.backlog_cap; pj.max_pos = d->s.max_pos; pj.row_cap = d->row_cap;
+    pj.backlog = d->backlog; pj.backlog_len = d->backlog_len;
+    pj.kv = kv_view(d->kv);
+    pj.rows = d->d_rows; pj.m_total = d->d_m_total;
+    pj.enq_base = d->d_plan; pj.new_blen = d->d_plan + S;
+    pj.xpack = d->d_xpack;
+    pj.status = ctx->d_status;
+    pp.job[j] = pj;
+    int rows_upper = jobs[j].rows_upper < d->row_cap ? jobs[j].rows_upper : d->row_cap;
+    const int n_pack = rows_upper < 1 ? 1 : (rows_upper > PP_MAX_PACK_CTAS ? PP_MAX_PACK_CTAS : rows_upper);
+    pack_grid += 1 + n_pack;
+    if (j == 0) pp.ctas_job0 = 1 + n_pack;
+    GemmJob& g = gp.job[j];
+    g.wpack = d->d_wpack; g.xpack = d->d_xpack; g.rows = d->d_rows; g.m_total = d->d_m_total; g.rope = d->d_rope;
+    g.k_pool = d->kv->k_pool; g.v_pool = d->kv->v_pool;
+    g.hidden = d->s.hidden; g.n_kv_heads = d->s.n_kv_heads; g.num_pages = d->kv->s.num_pages;
+    g.n_split = d->n_split; g.row_cap = d->row_cap; g.max_pass = d->max_pass; g.ws_part = d->d_ws_part; g.split_cnt = d->d_split_cnt;
+    g.hidden_rows = pj.hidden_rows; g.q_indptr = pj.q_indptr; g.n_rows = pj.n_rows; g.seq_ids = pj.seq_ids;
+    g.enq_base = jobs[j].enqueues ? pj.enq_base : nullptr;
+    g.new_blen = (pj.mode == PLAN_EAGER || pj.cap == 0) ? nullptr : pj.new_blen;
+    g.backlog = const_cast<__nv_bfloat16*>(d->backlog); g.backlog_len = d->backlog_len;
+    g.B = pj.B; g.cap = pj.cap; g.max_rows = pj.max_rows;
+    g.route = route; g.cur = cur; g.next_q_len = next_q_len; g.q_len_ar = q_len_ar; g.q_len_diffusion = q_len_diffusion;
+    const int ctas = d->s.n_layers * 2 * d->s.n_kv_heads * d->n_split;
+    gemm_grid += ctas;
+    if (j == 0) gp.ctas_job0 = ctas;
   }
-  GemmParams g;
-  g.wpack = d->d_wpack; g.xpack = d->d_xpack; g.rows = d->d_rows; g.m_total = d->d_m_total; g.rope = d->d_rope;
-  g.k_pool = d->kv->k_pool; g.v_pool = d->kv->v_pool;
-  g.hidden = d->s.hidden; g.n_kv_heads = d->s.n_kv_heads; g.num_pages = d->kv->s.num_pages;
-  g.n_split = d->n_split; g.row_cap = d->row_cap; g.max_pass = d->max_pass; g.ws_part = d->d_ws_part; g.split_cnt = d->d_split_cnt;
-  const int grid = d->s.n_layers * 2 * d->s.n_kv_heads * d->n_split;
-  wf_launch(wf_prefill_gemm_kernel<D>, dim3(grid), dim3(PF_THREADS), PF_SMEM_BUDGET, st, g);
+  if (n_jobs == 1) { pp.ctas_job0 = pack_grid; gp.ctas_job0 = gemm_grid; }
+  wf_launch(wf_plan_pack_kernel, dim3(pack_grid), dim3(PP_THREADS), 0, st, pp);
+  int rc = wf_check_launch(ctx, "wf_plan_pack_kernel");
+  if (rc != WF_OK) return rc;
+  if (D == 128) {
+    WF_CONFIGURE_ONCE(ctx, WF_FUNC_GEMM_128, wf_prefill_gemm_kernel<128>, PF_SMEM_BUDGET);
+    wf_launch(wf_prefill_gemm_kernel<128>, dim3(gemm_grid), dim3(PF_THREADS), PF_SMEM_BUDGET, st, gp);
+  } else {
+    WF_CONFIGURE_ONCE(ctx, WF_FUNC_GEMM_64, wf_prefill_gemm_kernel<64>, PF_SMEM_BUDGET);
+    wf_launch(wf_prefill_gemm_kernel<64>, dim3(gemm_grid), dim3(PF_THREADS), PF_SMEM_BUDGET, st, gp);
+  }
   return wf_check_launch(ctx, "wf_prefill_gemm_kernel");
 }
 
-// plan + projection: the one device path behind eager prefill, flush and forced flush
-int run_prefill(wf_drafter* d, PlanParams& pp, int rows_upper, cudaStream_t st) {
-  wf_ctx* ctx = d->ctx;
-  pp.hidden = d->s.hidden; pp.cap = d->s.backlog_cap; pp.max_pos = d->s.max_pos; pp.row_cap = d->row_cap;
-  pp.backlog = d->backlog; pp.backlog_len = d->backlog_len;
-  pp.kv = kv_view(d->kv);
-  pp.rows = d->d_rows; pp.m_total = d->d_m_total;
-  pp.plan_n = d->d_plan; pp.plan_off = d->d_plan + d->kv->s.max_seqs; pp.enq_base = d->d_plan + 2 * d->kv->s.max_seqs;
-  pp.status = ctx->d_status;
-  wf_launch(wf_prefill_plan_kernel, dim3(1), dim3(1024), 0, st, pp);
-  int rc = wf_check_launch(ctx, "wf_prefill_plan_kernel");
-  if (rc != WF_OK) return rc;
-  rows_upper = rows_upper < d->row_cap ? rows_upper : d->row_cap;
-  wf_launch(wf_pack_x_kernel, dim3(rows_upper > 0 ? rows_upper : 1), dim3(256), 0, st, (const RowEntry*)d->d_rows, (const int32_t*)d->d_m_total, d->d_xpack, d->s.hidden);
-  rc = wf_check_launch(ctx, "wf_pack_x_kernel");
-  if (rc != WF_OK) return rc;
-  return d->s.head_dim == 128 ? launch_gemm<128>(d, st) : launch_gemm<64>(d, st);
+int run_one(wf_ctx* ctx, wf_drafter* d, const PlanJob& pj, int rows_upper, bool enqueues, cudaStream_t st) {
+  CallJob job{d, pj, rows_upper, enqueues};
+  return run_jobs(ctx, &job, 1, nullptr, nullptr, nullptr, 0, 0, st);
 }
 
 }  // namespace
@@ -637,116 +752,97 @@ extern "C" int wf_kv_only_prefill(wf_ctx* ctx, wf_drafter* d, const void* hidden
                                   const int32_t* n_rows, const int32_t* seq_ids, int B, int max_rows, void* stream) {
   if (!ctx || !d) return WF_ERR_INVALID_ARG;
   WF_REQUIRE(ctx, hidden && q_indptr && n_rows, WF_ERR_INVALID_ARG, "wf_kv_only_prefill: null argument");
-  WF_REQUIRE(ctx, B >= 0 && B <= d->kv->s.max_seqs && max_rows >= 0 && (long long)B * max_rows <= d->row_cap,
-             WF_ERR_INVALID_ARG, "wf_kv_only_prefill: B * max_rows exceeds the row table (%d)", d->row_cap);
+  WF_REQUIRE(ctx, B >= 0 && B <= d->kv->s.max_seqs && B <= PP_MAX_B && max_rows >= 0 && (long long)B * max_rows <= d->row_cap,
+             WF_ERR_INVALID_ARG, "wf_kv_only_prefill: need B <= %d and B * max_rows <= the row table (%d)", PP_MAX_B, d->row_cap);
   WF_REQUIRE(ctx, (uintptr_t)hidden % 16 == 0, WF_ERR_INVALID_ARG, "wf_kv_only_prefill: hidden must be 16-byte aligned");
   if (B == 0 || max_rows == 0) return WF_OK;
-  PlanParams pp{};
-  pp.mode = PLAN_EAGER; pp.B = B;
-  pp.hidden_rows = (const __nv_bfloat16*)hidden; pp.q_indptr = q_indptr; pp.n_rows = n_rows; pp.seq_ids = seq_ids;
-  pp.mask = nullptr;
-  return run_prefill(d, pp, B * max_rows, (cudaStream_t)stream);
+  PlanJob pj{};
+  pj.mode = PLAN_EAGER; pj.B = B; pj.max_rows = max_rows;
+  pj.hidden_rows = (const __nv_bfloat16*)hidden; pj.q_indptr = q_indptr; pj.n_rows = n_rows; pj.seq_ids = seq_ids;
+  return run_one(ctx, d, pj, B * max_rows, false, (cudaStream_t)stream);
 }
 
 extern "C" int wf_lazy_catchup_flush(wf_ctx* ctx, wf_drafter* d, const int32_t* flush_mask, int B, void* stream) {
   if (!ctx || !d) return WF_ERR_INVALID_ARG;
-  WF_REQUIRE(ctx, B >= 0 && B <= d->kv->s.max_seqs, WF_ERR_INVALID_ARG, "wf_lazy_catchup_flush: bad B");
+  WF_REQUIRE(ctx, B >= 0 && B <= d->kv->s.max_seqs && B <= PP_MAX_B, WF_ERR_INVALID_ARG, "wf_lazy_catchup_flush: bad B (max %d)", PP_MAX_B);
   WF_REQUIRE(ctx, d->s.backlog_cap > 0, WF_ERR_INVALID_ARG, "wf_lazy_catchup_flush: drafter has no backlog");
   if (B == 0) return WF_OK;
-  PlanParams pp{};
-  pp.mode = PLAN_FLUSH; pp.B = B; pp.mask = flush_mask;
-  return run_prefill(d, pp, B * d->s.backlog_cap, (cudaStream_t)stream);
+  PlanJob pj{};
+  pj.mode = PLAN_FLUSH; pj.B = B; pj.flush_mask = flush_mask; pj.max_rows = 0;
+  return run_one(ctx, d, pj, B * d->s.backlog_cap, false, (cudaStream_t)stream);
 }
-
-namespace {
-// copy rows 0..n_rows[b]-1 of each idle sequence's block to the tail of its backlog (FIFO)
-__global__ void wf_enqueue_kernel(const __nv_bfloat16* __restrict__ hidden, const int32_t* __restrict__ q_indptr,
-                                  const int32_t* __restrict__ n_rows, const int32_t* __restrict__ seq_ids,
-                                  const int32_t* __restrict__ idle_mask, __nv_bfloat16* __restrict__ backlog,
-                                  const int32_t* __restrict__ backlog_len, int hidden_dim, int cap) {
-  wf_pdl_trigger();
-  wf_pdl_wait();
-  const int b = blockIdx.y, t = blockIdx.x;
-  if (!idle_mask[b]) return;
-  const int n = n_rows[b];
-  if (t >= n || n > cap) return;
-  const int sq = seq_ids ? seq_ids[b] : b;
-  const uint4* src = reinterpret_cast<const uint4*>(hidden + (size_t)(q_indptr[b] + t) * hidden_dim);
-  uint4* dst = reinterpret_cast<uint4*>(backlog + ((size_t)sq * cap + backlog_len[sq] + t) * hidden_dim);
-  for (int i = threadIdx.x; i < hidden_dim / 8; i += blockDim.x) dst[i] = src[i];
-}
-// ROUND: rows 0..n_rows[b]-1 of each block go to backlog[seq][enq_base[b] + t] (enq_base < 0: nothing to enqueue);
-// the lengths were already advanced by the plan
-__global__ void wf_enqueue_round_kernel(const __nv_bfloat16* __restrict__ hidden, const int32_t* __restrict__ q_indptr,
-                                        const int32_t* __restrict__ n_rows, const int32_t* __restrict__ seq_ids,
-                                        const int32_t* __restrict__ enq_base, __nv_bfloat16* __restrict__ backlog,
-                                        int hidden_dim, int cap) {
-  wf_pdl_trigger();
-  wf_pdl_wait();
-  const int b = blockIdx.y, t = blockIdx.x;
-  const int base = enq_base[b];
-  if (base < 0 || t >= n_rows[b]) return;
-  const int sq = seq_ids ? seq_ids[b] : b;
-  const uint4* src = reinterpret_cast<const uint4*>(hidden + (size_t)(q_indptr[b] + t) * hidden_dim);
-  uint4* dst = reinterpret_cast<uint4*>(backlog + ((size_t)sq * cap + base + t) * hidden_dim);
-  for (int i = threadIdx.x; i < hidden_dim / 8; i += blockDim.x) dst[i] = src[i];
-}
-__global__ void wf_enqueue_len_kernel(const int32_t* __restrict__ n_rows, const int32_t* __restrict__ seq_ids,
-                                      const int32_t* __restrict__ idle_mask, int32_t* __restrict__ backlog_len, int B, int cap) {
-  wf_pdl_trigger();
-  wf_pdl_wait();
-  const int b = blockIdx.x * blockDim.x + threadIdx.x;
-  if (b < B && idle_mask[b] && n_rows[b] <= cap) backlog_len[seq_ids ? seq_ids[b] : b] += n_rows[b];
-}
-}  // namespace
 
 extern "C" int wf_lazy_catchup_enqueue(wf_ctx* ctx, wf_drafter* d, const void* hidden, const int32_t* q_indptr,
                                        const int32_t* n_rows, const int32_t* seq_ids, const int32_t* idle_mask,
                                        int B, int max_rows, void* stream) {
   if (!ctx || !d) return WF_ERR_INVALID_ARG;
   WF_REQUIRE(ctx, hidden && q_indptr && n_rows && idle_mask, WF_ERR_INVALID_ARG, "wf_lazy_catchup_enqueue: null argument");
-  WF_REQUIRE(ctx, B >= 0 && B <= d->kv->s.max_seqs && max_rows >= 0, WF_ERR_INVALID_ARG, "wf_lazy_catchup_enqueue: bad B");
+  WF_REQUIRE(ctx, B >= 0 && B <= d->kv->s.max_seqs && B <= PP_MAX_B && max_rows >= 0, WF_ERR_INVALID_ARG,
+             "wf_lazy_catchup_enqueue: bad B (max %d)", PP_MAX_B);
   WF_REQUIRE(ctx, d->s.backlog_cap > 0 && max_rows <= d->s.backlog_cap, WF_ERR_INVALID_ARG,
              "wf_lazy_catchup_enqueue: max_rows exceeds backlog_cap");
+  WF_REQUIRE(ctx, (uintptr_t)hidden % 16 == 0, WF_ERR_INVALID_ARG, "wf_lazy_catchup_enqueue: hidden must be 16-byte aligned");
   if (B == 0 || max_rows == 0) return WF_OK;
-  cudaStream_t st = (cudaStream_t)stream;
-  // (1) forced flush of the sequences whose backlog would overflow (C20): same device path as flush
-  PlanParams pp{};
-  pp.mode = PLAN_FORCED; pp.B = B;
-  pp.q_indptr = q_indptr; pp.n_rows = n_rows; pp.seq_ids = seq_ids; pp.mask = idle_mask;
-  int rc = run_prefill(d, pp, B * d->s.backlog_cap, st);
-  if (rc != WF_OK) return rc;
-  // (2) append the rows, (3) advance the lengths
-  wf_launch(wf_enqueue_kernel, dim3(max_rows, B), dim3(128), 0, st, (const __nv_bfloat16*)hidden, q_indptr, n_rows, seq_ids, idle_mask,
-            const_cast<__nv_bfloat16*>(d->backlog), (const int32_t*)d->backlog_len, d->s.hidden, d->s.backlog_cap);
-  rc = wf_check_launch(ctx, "wf_enqueue_kernel");
-  if (rc != WF_OK) return rc;
-  wf_launch(wf_enqueue_len_kernel, dim3((B + 255) / 256), dim3(256), 0, st, n_rows, seq_ids, idle_mask, d->backlog_len, B, d->s.backlog_cap);
-  return wf_check_launch(ctx, "wf_enqueue_len_kernel");
+  // the forced flush of the sequences whose backlog would overflow (C20) and the append are one call: the planner
+  // decides the offsets (-1 where nothing may be written, e.g. when the forced flush found no pages)
+  PlanJob pj{};
+  pj.mode = PLAN_ENQUEUE; pj.B = B; pj.max_rows = max_rows;
+  pj.hidden_rows = (const __nv_bfloat16*)hidden; pj.q_indptr = q_indptr; pj.n_rows = n_rows; pj.seq_ids = seq_ids;
+  pj.idle_mask = idle_mask;
+  return run_one(ctx, d, pj, B * d->s.backlog_cap, true, (cudaStream_t)stream);
 }
+
+namespace {
+int check_round_args(wf_ctx* ctx, wf_drafter* d, const char* who, const void* hidden, const int32_t* q_indptr,
+                     const int32_t* n_rows, int B, int max_rows, bool may_idle) {
+  WF_REQUIRE(ctx, hidden && q_indptr && n_rows, WF_ERR_INVALID_ARG, "%s: null argument", who);
+  WF_REQUIRE(ctx, B >= 0 && B <= d->kv->s.max_seqs && B <= PP_MAX_B && max_rows >= 0 && max_rows <= 64, WF_ERR_INVALID_ARG,
+             "%s: need B <= min(max_seqs, %d) and max_rows <= 64", who, PP_MAX_B);
+  WF_REQUIRE(ctx, !may_idle || (d->s.backlog_cap > 0 && max_rows <= d->s.backlog_cap), WF_ERR_INVALID_ARG,
+             "%s: idle sequences need a backlog with max_rows <= backlog_cap", who);
+  WF_REQUIRE(ctx, (long long)B * (d->s.backlog_cap + max_rows) <= d->row_cap, WF_ERR_INVALID_ARG,
+             "%s: B * (backlog_cap + max_rows) exceeds the row table (%d)", who, d->row_cap);
+  WF_REQUIRE(ctx, (uintptr_t)hidden % 16 == 0, WF_ERR_INVALID_ARG, "%s: hidden must be 16-byte aligned", who);
+  return WF_OK;
+}
+}  // namespace
 
 extern "C" int wf_lazy_catchup_round(wf_ctx* ctx, wf_drafter* d, const void* hidden, const int32_t* q_indptr,
                                      const int32_t* n_rows, const int32_t* seq_ids, const int32_t* idle_mask,
                                      const int32_t* flush_mask, int B, int max_rows, void* stream) {
   if (!ctx || !d) return WF_ERR_INVALID_ARG;
-  WF_REQUIRE(ctx, hidden && q_indptr && n_rows, WF_ERR_INVALID_ARG, "wf_lazy_catchup_round: null argument");
-  WF_REQUIRE(ctx, B >= 0 && B <= d->kv->s.max_seqs && B <= KV_RESERVE_SMEM && max_rows >= 0 && max_rows <= 64, WF_ERR_INVALID_ARG,
-             "wf_lazy_catchup_round: need B <= min(max_seqs, %d) and max_rows <= 64", KV_RESERVE_SMEM);
-  WF_REQUIRE(ctx, !idle_mask || (d->s.backlog_cap > 0 && max_rows <= d->s.backlog_cap), WF_ERR_INVALID_ARG,
-             "wf_lazy_catchup_round: idle sequences need a backlog with max_rows <= backlog_cap");
-  WF_REQUIRE(ctx, (long long)B * (d->s.backlog_cap + max_rows) <= d->row_cap, WF_ERR_INVALID_ARG,
-             "wf_lazy_catchup_round: B * (backlog_cap + max_rows) exceeds the row table (%d)", d->row_cap);
-  WF_REQUIRE(ctx, (uintptr_t)hidden % 16 == 0, WF_ERR_INVALID_ARG, "wf_lazy_catchup_round: hidden must be 16-byte aligned");
+  int rc = check_round_args(ctx, d, "wf_lazy_catchup_round", hidden, q_indptr, n_rows, B, max_rows, idle_mask != nullptr);
+  if (rc != WF_OK) return rc;
   if (B == 0 || max_rows == 0) return WF_OK;
-  cudaStream_t st = (cudaStream_t)stream;
-  PlanParams pp{};
-  pp.mode = PLAN_ROUND; pp.B = B;
-  pp.hidden_rows = (const __nv_bfloat16*)hidden; pp.q_indptr = q_indptr; pp.n_rows = n_rows; pp.seq_ids = seq_ids;
-  pp.mask = idle_mask; pp.mask2 = flush_mask;
-  int rc = run_prefill(d, pp, B * (d->s.backlog_cap + max_rows), st);
-  if (rc != WF_OK || !idle_mask) return rc;
-  // the projection's operand was packed from the backlog by wf_pack_x_kernel (stream order): the backlog may be overwritten
-  wf_launch(wf_enqueue_round_kernel, dim3(max_rows, B), dim3(128), 0, st, (const __nv_bfloat16*)hidden, q_indptr, n_rows, seq_ids,
-            (const int32_t*)(d->d_plan + 2 * d->kv->s.max_seqs), const_cast<__nv_bfloat16*>(d->backlog), d->s.hidden, d->s.backlog_cap);
-  return wf_check_launch(ctx, "wf_enqueue_round_kernel");
+  PlanJob pj{};
+  pj.mode = PLAN_ROUND; pj.B = B; pj.max_rows = max_rows;
+  pj.hidden_rows = (const __nv_bfloat16*)hidden; pj.q_indptr = q_indptr; pj.n_rows = n_rows; pj.seq_ids = seq_ids;
+  pj.idle_mask = idle_mask; pj.flush_mask = flush_mask;
+  return run_one(ctx, d, pj, B * (d->s.backlog_cap + max_rows), idle_mask != nullptr, (cudaStream_t)stream);
+}
+
+extern "C" int wf_switch_round(wf_ctx* ctx, wf_drafter* drafter_ar, wf_drafter* drafter_diffusion, const void* hidden,
+                               const int32_t* q_indptr, const int32_t* n_rows, const int32_t* seq_ids,
+                               const int32_t* route, int32_t* cur_drafter, int32_t* next_q_len, int q_len_ar,
+                               int q_len_diffusion, int B, int max_rows, void* stream) {
+  if (!ctx || !drafter_ar || !drafter_diffusion) return WF_ERR_INVALID_ARG;
+  WF_REQUIRE(ctx, route && cur_drafter, WF_ERR_INVALID_ARG, "wf_switch_round: null route / cur_drafter");
+  WF_REQUIRE(ctx, drafter_ar != drafter_diffusion && drafter_ar->kv != drafter_diffusion->kv, WF_ERR_INVALID_ARG,
+             "wf_switch_round: the two drafters must be distinct and own distinct caches");
+  WF_REQUIRE(ctx, drafter_ar->s.head_dim == drafter_diffusion->s.head_dim && drafter_ar->s.hidden == drafter_diffusion->s.hidden,
+             WF_ERR_UNSUPPORTED_SHAPE, "wf_switch_round: the drafters must share hidden size and head_dim");
+  wf_drafter* ds[2] = {drafter_diffusion, drafter_ar};     // the 5-layer stream first: its CTAs are the long ones
+  const int codes[2] = {WF_ROUTE_DIFFUSION, WF_ROUTE_AR};
+  CallJob jobs[2];
+  for (int j = 0; j < 2; ++j) {
+    int rc = check_round_args(ctx, ds[j], "wf_switch_round", hidden, q_indptr, n_rows, B, max_rows, true);
+    if (rc != WF_OK) return rc;
+    PlanJob pj{};
+    pj.mode = PLAN_ROUND; pj.B = B; pj.max_rows = max_rows; pj.code = codes[j];
+    pj.hidden_rows = (const __nv_bfloat16*)hidden; pj.q_indptr = q_indptr; pj.n_rows = n_rows; pj.seq_ids = seq_ids;
+    pj.route = route; pj.cur = cur_drafter;
+    jobs[j] = CallJob{ds[j], pj, B * (ds[j]->s.backlog_cap + max_rows), true};
+  }
+  if (B == 0 || max_rows == 0) return WF_OK;
+  return run_jobs(ctx, jobs, 2, route, cur_drafter, next_q_len, q_len_ar, q_len_diffusion, (cudaStream_t)stream);
 }

@@ -1,14 +1,17 @@
 """Round driver: one verify-and-switch round of the hot path on synthetic, device-resident inputs.
 
     reserve target pages -> 36 x wf_verify_attn -> wf_accept_entropy_route
-      -> per drafter ONE wf_lazy_catchup_round: the sequences it is active for get a KV-only prefill (stands in for
-         its own forward, reading C22), idle sequences are enqueued, sequences that switch to it are flushed
-         together with this round's rows (C21)
+      -> ONE wf_switch_round for both drafters, driven on the device by this round's `route` and the `cur_drafter`
+         array: the drafter that is active for a sequence gets a KV-only prefill of its rows (stands in for its own
+         forward, reading C22), the idle one has them enqueued, a sequence that the router switches is flushed
+         together with this round's rows (C21); cur_drafter <- route.  No mask crosses the host.
 
 Everything is launched on one stream with no host synchronisation inside the round.
-The route trace is seeded and planted in the logits (spike on the row of the last accepted token),
-so the host knows every round's block lengths in advance; the device still computes every output and
-`check_plan` compares them with the plan afterwards.  This module holds no method arithmetic: it
+The route trace is a seeded per-sequence Markov chain (flip with probability Workload.switch_prob per
+round, BASELINE.json configs[4]) planted in the logits (spike on the row of the last accepted token), so
+the host knows every round's block lengths in advance and can lay out the ragged inputs; the device still
+computes every output, derives every mask from its own route, and `check_plan` compares outputs and
+cur_drafter with the plan afterwards.  This module holds no method arithmetic: it
 only builds inputs (synth) and calls the C-ABI binding.  It never imports oracle/.
 """
 
@@ -34,7 +37,7 @@ class Slot:
 
 
 class RoundState:
-    def __init__(self, ctx, wl: synth.Workload, n_slots=4, n_rounds_max=64, device="cuda", layers=None,
+    def __init__(self, ctx, wl: synth.Workload, n_slots=16, n_rounds_max=64, device="cuda", layers=None,
                  host_copies=False):
         import torch
         self.torch, self.ctx, self.wl, self.device = torch, ctx, wl, device
@@ -51,6 +54,7 @@ class RoundState:
         self.max_pages_per_seq = int(-(-(int(self.ctx0.max()) + grow) // sh.page_size)) + 1
         num_pages = int(sum(-(-(int(c) + grow) // sh.page_size) for c in self.ctx0)) + 8
         free = synth.draw_free_list(num_pages, g, wl.shuffled_pages)
+        self.free = free
         self.kv_shape = wf.KvShape(self.L, sh.n_kv_heads, sh.head_dim, sh.page_size, num_pages, B, self.max_pages_per_seq)
         pool = (self.L, num_pages, sh.n_kv_heads, sh.page_size, sh.head_dim)
         kv_std = 1.0 / math.sqrt(sh.head_dim)
@@ -68,9 +72,9 @@ class RoundState:
         self.drafters = {}
         for name, n_layers in zip(("A", "D"), sh.drafter_layers if len(sh.drafter_layers) == 2 else (sh.drafter_layers[0],) * 2):
             self.drafters[name] = self._make_drafter(name, n_layers, grow, g)
-        # ---- cyclic schedule of n_slots rounds ----
+        # ---- cyclic schedule of n_slots rounds: route OUTPUT of slot k (1 = AR) ----
         self.n_slots = n_slots
-        route = (g.random((n_slots, B)) < 0.5).astype(np.int32)            # planned route OUTPUT of slot k (1 = AR)
+        route = synth.draw_route_trace(g, n_slots, B, wl.switch_prob)
         if len(wl.gammas) == 1:
             gam_of = lambda r: wl.gammas[0]
         else:
@@ -85,6 +89,10 @@ class RoundState:
             s.spike = np.where(s.next == wf.ROUTE_AR, SPIKE_HIGH_ENTROPY, SPIKE_LOW_ENTROPY)
             self._make_slot_inputs(s, k, host_copies)
             self.slots.append(s)
+        # the drafter that drafted the block of the next round to run (device state, advanced by wf_switch_round)
+        self.cur_drafter = _i32(self.slots[0].cur, device)
+        self.next_q_len = torch.zeros(B, dtype=torch.int32, device=device)
+        self.q_len_of = {wf.ROUTE_AR: gam_of(wf.ROUTE_AR) + 1, wf.ROUTE_DIFFUSION: gam_of(wf.ROUTE_DIFFUSION) + 1}
         self.tau = torch.full((1,), sh.tau, dtype=torch.float32, device=device)
         self.out = {n: torch.zeros(B, dtype=torch.int32, device=device) for n in ("accept_len", "bonus_token", "route", "n_commit")}
         self.entropy = torch.zeros(B, dtype=torch.float32, device=device)
@@ -118,6 +126,7 @@ class RoundState:
         shape = wf.KvShape(n_layers, sh.n_kv_heads, sh.head_dim, sh.page_size, num_pages, B, per_seq)
         pool = (n_layers, num_pages, sh.n_kv_heads, sh.page_size, sh.head_dim)
         d = Slot()
+        d.free, d.n_layers = free, n_layers
         d.k_pool = torch.zeros(pool, dtype=torch.bfloat16, device=self.device)
         d.v_pool = torch.zeros(pool, dtype=torch.bfloat16, device=self.device)
         d.block_table = torch.full((B, per_seq), -1, dtype=torch.int32, device=self.device)
@@ -209,19 +218,38 @@ class RoundState:
         wf.wf_neural_route(self.ctx, s.hidden, s.q_indptr, self.out["accept_len"], self.B, n.d, n.m, n.w1, n.b1, n.w2, n.b2,
                            n.tau, True, n.delta_al, n.route, n.ws, stream)
 
-    def run_catchup(self, s, stream=None, lazy=True, fused=True):
-        """Drafter-cache maintenance after the accept: lazy (the paper's scheme) or eager (its baseline).
-        lazy + fused: one wf_lazy_catchup_round per drafter (one projection: active rows, switching sequences' backlog
-        and rows; idle rows are enqueued); lazy + not fused: the three separate calls it is equivalent to."""
+    def sync_cur(self):
+        """cur_drafter <- the plan's value for the next round to run (after legs that do not drive the switch)."""
+        self.cur_drafter.copy_(_i32(self.slots[self.rounds_done % self.n_slots].cur, self.device))
+
+    def run_catchup(self, s, stream=None, lazy=True, fused=True, mode=None):
+        """Drafter-cache maintenance after the accept.
+        mode "switch" (default): ONE wf_switch_round for both drafters, masks derived on the device from route and
+             cur_drafter (the paper's scheme: Lazy Catch-up + KV-only prefill at the switch);
+        mode "round": one wf_lazy_catchup_round per drafter with host-planned masks;
+        mode "separate": the three separate calls a round is equivalent to;
+        mode "eager": the paper's baseline, a KV-only prefill into both drafters every round;
+        mode "active": only the active drafter's own append (reading C22), nothing for the idle one."""
         torch, B = self.torch, self.B
         n_commit = self.out["n_commit"]
+        if mode is None:
+            mode = "eager" if not lazy else ("switch" if fused else "separate")
+        if mode == "switch":
+            wf.wf_switch_round(self.ctx, self.drafters["A"].handle, self.drafters["D"].handle, s.hidden, s.q_indptr, n_commit,
+                               None, self.out["route"], self.cur_drafter, self.next_q_len, self.q_len_of[wf.ROUTE_AR],
+                               self.q_len_of[wf.ROUTE_DIFFUSION], B, self.qmax, stream)
+            return
         for name, d in self.drafters.items():
             m = s.masks[name]
-            if lazy and fused:
+            if mode == "round":
                 wf.wf_lazy_catchup_round(self.ctx, d.handle, s.hidden, s.q_indptr, n_commit, None,
                                          m.idle if m.idle_host.any() else None, m.flush if m.flush_host.any() else None,
                                          B, self.qmax, stream)
-            elif lazy:
+            elif mode == "active":
+                if m.active_host.any():
+                    torch.mul(n_commit, m.active, out=m.n_rows)            # argument marshalling, not the path
+                    wf.wf_kv_only_prefill(self.ctx, d.handle, s.hidden, s.q_indptr, m.n_rows, None, B, self.qmax, stream)
+            elif mode == "separate":
                 if m.active_host.any():
                     torch.mul(n_commit, m.active, out=m.n_rows)            # argument marshalling, not the path
                     wf.wf_kv_only_prefill(self.ctx, d.handle, s.hidden, s.q_indptr, m.n_rows, None, B, self.qmax, stream)
@@ -232,7 +260,7 @@ class RoundState:
             else:
                 wf.wf_kv_only_prefill(self.ctx, d.handle, s.hidden, s.q_indptr, n_commit, None, B, self.qmax, stream)
 
-    def run_round(self, stream=None, lazy=True, events=None, fused=True):
+    def run_round(self, stream=None, lazy=True, events=None, fused=True, mode=None):
         """One whole round.  events: optional dict of (start, end) CUDA event pairs to record around parts."""
         s = self.slots[self.rounds_done % self.n_slots]
         self.target_kv.reserve(s.add_tokens, self.B, stream)
@@ -244,7 +272,7 @@ class RoundState:
         self.run_accept(s, stream)
         if events:
             events["catchup"][0].record()
-        self.run_catchup(s, stream, lazy, fused)
+        self.run_catchup(s, stream, lazy, fused, mode)
         if events:
             events["catchup"][1].record()
         self.rounds_done += 1
@@ -328,8 +356,9 @@ class RoundState:
             if int(a[b]) != len(want) - 1 or list(path[b][:len(want)]) != want:
                 raise RuntimeError(f"tree round: sequence {b} accepted {list(path[b][:int(a[b]) + 1])}, planted {want}")
 
-    def check_plan(self, s):
-        """After a sync: the device's outputs of the last round must equal the planted plan."""
+    def check_plan(self, s, switched=True):
+        """After a sync: the device's outputs of the last round must equal the planted plan (and, when the round went
+        through wf_switch_round, so must the device-side drafter state and the next block lengths)."""
         self.torch.cuda.synchronize()
         st = self.ctx.poll_status()
         if st != 0:
@@ -338,6 +367,12 @@ class RoundState:
         r = self.out["route"].cpu().numpy()
         if not (np.array_equal(a, s.u) and np.array_equal(r, s.next)):
             raise RuntimeError(f"device outputs differ from the planted plan: accept {a} vs {s.u}; route {r} vs {s.next}")
+        if switched:
+            c = self.cur_drafter.cpu().numpy()
+            nq = self.next_q_len.cpu().numpy()
+            want_q = np.array([self.q_len_of[int(x)] for x in s.next])
+            if not (np.array_equal(c, s.next) and np.array_equal(nq, want_q)):
+                raise RuntimeError(f"device-driven switch: cur_drafter {c} vs {s.next}; next block lengths {nq} vs {want_q}")
 
     def close(self):
         for d in self.drafters.values():

@@ -123,6 +123,25 @@ def draw_free_list(num_pages, g, shuffled):
     return np.arange(num_pages, dtype=np.int32)
 
 
+def draw_route_trace(g, n_slots, batch, switch_prob):
+    """Planned router output per (round slot, sequence): a per-sequence Markov chain that flips with probability
+    switch_prob per round (BASELINE.json configs[4]: "switch probability 0.3 per round"; PAPER.md:59 the preferable
+    drafter swings within a sequence).  The schedule is replayed cyclically, so the last slot's flip is the one that
+    closes the cycle (an even number of flips per sequence); with 16 slots the realised flip rate is about
+    (15 * p + 0.5) / 16.  route[k][b] in {0 = diffusion, 1 = AR}."""
+    route = np.zeros((n_slots, batch), dtype=np.int32)
+    state = (g.random(batch) < 0.5).astype(np.int32)                 # output of the slot before slot 0 = of slot n-1
+    first = state.copy()
+    for k in range(n_slots):
+        if k < n_slots - 1:
+            flip = (g.random(batch) < switch_prob).astype(np.int32)
+            state = state ^ flip
+        else:
+            state = first                                            # closes the cycle
+        route[k] = state
+    return route
+
+
 def draw_accept_prefix(g, gammas, mean_accept=None):
     """Planned accepted-prefix length u_b per sequence.
 

@@ -127,6 +127,21 @@ def test_accept_8b_vocab_mixed_gamma(wf):
     assert res["n_commit"][2] == 0 and res["accept_len"][2] == 0
 
 
+def test_accept_block_longer_than_the_host_bound_is_flagged(wf):
+    """q_b > max_q_len (the host bound that sizes the grid): the sticky status says so, the block is verified up to the
+    bound, and the context's completion counter still resets: the next, valid call is correct."""
+    binding, ctx = wf
+    g = synth.rng(5, 5)
+    logits, drafts, q_indptr, _ = synth.make_logits_block(g, [16, 8], 4096, 2.0, [15, 2], [0.0, 9.0])
+    res = _run_accept(binding, ctx, logits, drafts, q_indptr, 2.0, 8)          # sequence 0 has 16 rows, the bound says 8
+    assert ctx.poll_status() == binding.WF_ERR_INVALID_ARG
+    assert res["accept_len"][0] == 7 and res["accept_len"][1] == 2              # verified up to the bound
+    want = accept_route.accept_entropy_route(logits, drafts, q_indptr, 2.0)
+    res = _run_accept(binding, ctx, logits, drafts, q_indptr, 2.0, 16)
+    assert ctx.poll_status() == 0
+    _check_accept(res, want, 2.0)
+
+
 def test_accept_edge_rows(wf):
     """-inf (masked vocabulary), exact ties (lowest id wins), V % 4 != 0 (scalar path), closed forms."""
     binding, ctx = wf
@@ -223,9 +238,13 @@ def test_attn_8b_shapes_ragged_split(wf):
 
 
 def test_attn_peaked_scores(wf):
-    """Stress the online-softmax rescaling: Q scaled so that the score std is about 4."""
+    """Stress the online-softmax rescaling: Q and K scaled so that the score std is about 4 (SURVEY.md §8(c) tolerance
+    note asks for this case to be reported separately).  Here the attention weights concentrate on a few keys, P has
+    entries near 1 whose bf16 rounding (2^-9 relative) is no longer averaged over thousands of keys: the measured rel-L2
+    is printed, and the assertion is north_star's 5e-3 like everywhere else."""
     max_abs, rel = _attn_case(wf, [2100, 300], [16, 8], 32, 8, 128, seed=10, q_std=4.0, kv_std=1.0)
-    assert max_abs <= ATTN_MAX_ABS and rel <= 2 * ATTN_REL_L2, (max_abs, rel)
+    print(f"peaked scores: max-abs {max_abs:.3e}, rel-L2 {rel:.3e}")
+    assert max_abs <= ATTN_MAX_ABS and rel <= ATTN_REL_L2, (max_abs, rel)
 
 
 def test_attn_single_query_and_zero_context(wf):

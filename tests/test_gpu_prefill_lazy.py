@@ -290,3 +290,137 @@ def test_fused_round_argument_and_overflow_errors(wf):
     np.testing.assert_array_equal(dp.backlog_len.cpu().numpy(), [3, 0])
     np.testing.assert_array_equal(dp.kvp.seq_len.cpu().numpy(), [11, 9])
     dp.close()
+
+
+def test_enqueue_forced_flush_out_of_pages_changes_nothing(wf):
+    """A forced flush (C20) that finds no pages: the sticky status becomes WF_ERR_OUT_OF_PAGES and the call changes
+    nothing: no backlog row is written (not this sequence's, not its neighbours'), no length moves, backlog_len <= cap."""
+    import torch
+    import gpu_harness as H
+    binding, ctx = wf
+    S, cap, hidden = 3, 8, 256
+    dp = _mk(ctx, 1, hidden, 2, 64, S, 4, seed=12, cap=cap, num_pages=2)       # a ring of 2 pages = 32 tokens in all
+    g = synth.rng(12, 1)
+    q_indptr = H.i32([0, 8, 16, 24])
+    X1 = synth.normal_bf16(g, (24, hidden), 1.0)
+    binding.wf_lazy_catchup_enqueue(ctx, dp.gpu, H.bits_to_bf16_tensor(X1), q_indptr, H.i32([8, 6, 8]), None, H.i32([1, 1, 1]), S, 8)
+    torch.cuda.synchronize()
+    assert ctx.poll_status() == 0
+    np.testing.assert_array_equal(dp.backlog_len.cpu().numpy(), [8, 6, 8])
+    # use up the ring: sequence 1 (idle elsewhere) takes both pages through an eager twin call on the same cache
+    dp.kvp.gpu.reserve(H.i32([0, 32, 0]), S)
+    torch.cuda.synchronize()
+    before = H.bf16_tensor_to_bits(dp.backlog).copy()
+    X2 = synth.normal_bf16(g, (24, hidden), 1.0)
+    # sequences 0 and 2 are full: the enqueue needs a forced flush of 16 rows = pages the ring no longer has
+    binding.wf_lazy_catchup_enqueue(ctx, dp.gpu, H.bits_to_bf16_tensor(X2), q_indptr, H.i32([3, 1, 5]), None, H.i32([1, 1, 1]), S, 8)
+    torch.cuda.synchronize()
+    assert ctx.poll_status() == binding.WF_ERR_OUT_OF_PAGES
+    np.testing.assert_array_equal(dp.backlog_len.cpu().numpy(), [8, 6, 8])
+    assert int(dp.backlog_len.max()) <= cap
+    np.testing.assert_array_equal(H.bf16_tensor_to_bits(dp.backlog), before)
+    np.testing.assert_array_equal(dp.kvp.seq_len.cpu().numpy(), [0, 0, 0])
+    # the same through the fused round call
+    binding.wf_lazy_catchup_round(ctx, dp.gpu, H.bits_to_bf16_tensor(X2), q_indptr, H.i32([3, 1, 5]), None, H.i32([1, 1, 1]), None, S, 8)
+    torch.cuda.synchronize()
+    assert ctx.poll_status() == binding.WF_ERR_OUT_OF_PAGES
+    np.testing.assert_array_equal(dp.backlog_len.cpu().numpy(), [8, 6, 8])
+    np.testing.assert_array_equal(H.bf16_tensor_to_bits(dp.backlog), before)
+    dp.close()
+
+
+def test_rows_beyond_the_host_bound_are_clamped_and_flagged(wf):
+    """n_rows[b] > max_rows (the host bound that sizes the launch): rows up to the bound are projected, the sticky status
+    is WF_ERR_INVALID_ARG, nothing stale is consumed (the projected rows still match the oracle)."""
+    import torch
+    import gpu_harness as H
+    binding, ctx = wf
+    dp = _mk(ctx, 1, 256, 2, 64, 2, 8, seed=13, cap=0)
+    g = synth.rng(13, 1)
+    X = synth.normal_bf16(g, (32, 256), 1.0)
+    q_indptr = np.array([0, 16, 32], np.int32)
+    binding.wf_kv_only_prefill(ctx, dp.gpu, H.bits_to_bf16_tensor(X), H.i32(q_indptr), H.i32([9, 2]), None, 2, 4)   # 9 > 4
+    torch.cuda.synchronize()
+    assert ctx.poll_status() == binding.WF_ERR_INVALID_ARG
+    un = kv_prefill.kv_only_prefill(dp.oracle, X, q_indptr, [4, 2])
+    assert _check_new_rows(dp, un, [0, 0]) <= KV_REL_L2
+    dp.close()
+
+
+def test_switch_round_device_driven_routes_not_planted(wf):
+    """wf_switch_round over 30 rounds in which nothing is planned per round slot: every round's route comes from the
+    accept/entropy/route kernel itself on logits whose spike magnitude is random (the entropy lands on either side of
+    tau, the test learns the route only from the device), masks and cur_drafter never leave the device.  After every
+    round both drafters' cache lengths, backlog lengths, block tables and cur_drafter equal the oracle's (driven by the
+    oracle's own route); at the end the rows written are within tolerance and, after a final flush, the lazily
+    maintained caches equal eager twins bit for bit."""
+    import torch
+    import gpu_harness as H
+    from oracle import accept_route, lazy_catchup
+    binding, ctx = wf
+    S, cap, hidden, Hkv, D, V, tau = 6, 24, 256, 2, 64, 4096, 2.0
+    mk = lambda L, seed, shuffled, weights=None: _mk(ctx, L, hidden, Hkv, D, S, 60, seed=seed, cap=cap, shuffled=shuffled, weights=weights)
+    dr = {1: mk(1, 71, True), 0: mk(3, 72, True)}                   # route code -> drafter (AR: 1 layer, diffusion: 3)
+    tw = {c: mk(d.shape.n_layers, 80 + c, False, d.weights) for c, d in dr.items()}     # eager twins
+    start = [40, 0, 7, 16, 99, 3]
+    for d in list(dr.values()) + list(tw.values()):
+        _start_ctx(d, start)
+    lz = {c: d.oracle_lazy for c, d in dr.items()}
+    g = synth.rng(71, 9)
+    cur_o = g.integers(0, 2, size=S).astype(np.int32)
+    cur = H.i32(cur_o)
+    nq = torch.zeros(S, dtype=torch.int32, device="cuda")
+    q_len_of = {1: 8, 0: 16}
+    q_lens = np.array([q_len_of[int(c)] for c in cur_o])
+    outs = {k: torch.zeros(S, dtype=torch.int32, device="cuda") for k in ("accept_len", "bonus", "route", "n_commit")}
+    ent = torch.zeros(S, dtype=torch.float32, device="cuda")
+    ws = torch.empty(binding.wf_accept_workspace_bytes(S * 16, V), dtype=torch.uint8, device="cuda")
+    seen, flushes, near = set(), 0, 0
+    for rnd in range(30):
+        u = synth.draw_accept_prefix(g, q_lens - 1, 3.5)
+        spike = g.uniform(0.0, 10.0, size=S)                       # H lands on either side of tau: not a planned route
+        logits, drafts, q_indptr, _ = synth.make_logits_block(g, q_lens, V, 2.0, u, spike)
+        X = synth.normal_bf16(g, (int(q_indptr[-1]), hidden), 1.0)
+        Xg, qi = H.bits_to_bf16_tensor(X), H.i32(q_indptr)
+        binding.wf_accept_entropy_route(ctx, H.f32(logits), V, H.i32(drafts), qi, S, 16, H.f32([tau]), True, outs["accept_len"],
+                                        outs["bonus"], ent, outs["route"], outs["n_commit"], None, ws)
+        binding.wf_switch_round(ctx, dr[1].gpu, dr[0].gpu, Xg, qi, outs["n_commit"], None, outs["route"], cur, nq, 8, 16, S, 16)
+        for c in dr:
+            binding.wf_kv_only_prefill(ctx, tw[c].gpu, Xg, qi, outs["n_commit"], None, S, 16)
+        want = accept_route.accept_entropy_route(logits, drafts, q_indptr, tau)
+        torch.cuda.synchronize()
+        assert ctx.poll_status() == 0
+        band = np.abs(want["entropy"] - tau) < 1e-4
+        near += int(band.sum())
+        route_o = np.where(band, outs["route"].cpu().numpy(), want["route"]).astype(np.int32)
+        np.testing.assert_array_equal(outs["route"].cpu().numpy(), route_o)
+        np.testing.assert_array_equal(outs["n_commit"].cpu().numpy(), want["n_commit"])
+        flushes += int((route_o != cur_o).sum())
+        seen |= set(route_o.tolist())
+        cur_o, nq_o, _ = lazy_catchup.switch_round(lz, X, q_indptr, want["n_commit"], route_o, cur_o, q_len_of)
+        np.testing.assert_array_equal(cur.cpu().numpy(), cur_o)
+        np.testing.assert_array_equal(nq.cpu().numpy(), nq_o)
+        for c, d in dr.items():
+            d.kvp.assert_tables_equal()
+            np.testing.assert_array_equal(d.backlog_len.cpu().numpy(), lz[c].backlog_len)
+        q_lens = nq_o.astype(np.int64)                              # the chosen drafter's block length next round
+    assert seen == {0, 1} and flushes >= 10, (seen, flushes)
+    total = dr[0].kvp.oracle.seq_len + lz[0].backlog_len
+    for c, d in dr.items():
+        binding.wf_lazy_catchup_flush(ctx, d.gpu, None, S)
+        lz[c].flush(None, S)
+    torch.cuda.synchronize()
+    assert ctx.poll_status() == 0
+    for c, d in dr.items():
+        d.kvp.assert_tables_equal()
+        np.testing.assert_array_equal(d.kvp.seq_len.cpu().numpy(), total)
+        for l in range(d.shape.n_layers):
+            for b in range(S):
+                Kl, Vl = d.gather_gpu(l, b, int(total[b]))
+                Ke, Ve = tw[c].gather_gpu(l, b, int(total[b]))
+                np.testing.assert_array_equal(Kl[start[b]:], Ke[start[b]:])
+                np.testing.assert_array_equal(Vl[start[b]:], Ve[start[b]:])
+                Ko, Vo = d.kvp.oracle.gather(l, b, int(total[b]))
+                assert H.rel_l2(Kl[start[b]:], H.bf16_f64(Ko[start[b]:])) <= KV_REL_L2
+    for d in list(dr.values()) + list(tw.values()):
+        d.close()

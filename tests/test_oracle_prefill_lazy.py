@@ -245,3 +245,80 @@ def test_paged_kv_allocation_order_and_release():
     kv.reserve([12, 0, 0])
     assert list(kv.block_table[0, :3]) == [4, 5, 2]
     assert kv.locate(0, 9) == (2, 1)
+
+
+# ------------------------------------------------------------------ the switch (reading C21)
+def test_switch_masks_truth_table():
+    """the inactive drafter gets no work until the router switches to it.  All four (cur, route) cases,
+    for both route codes; exactly one drafter is active per sequence and at most one is flushed."""
+    cur = np.array([0, 0, 1, 1])
+    route = np.array([0, 1, 0, 1])
+    idle_d, fl_d = lazy_catchup.switch_masks(route, cur, 0)        # the diffusion drafter (code 0)
+    idle_a, fl_a = lazy_catchup.switch_masks(route, cur, 1)        # the autoregressive drafter (code 1)
+    assert idle_d.tolist() == [0, 0, 1, 1] and fl_d.tolist() == [0, 0, 1, 0]
+    assert idle_a.tolist() == [1, 1, 0, 0] and fl_a.tolist() == [0, 1, 0, 0]
+    assert ((1 - idle_d) + (1 - idle_a)).tolist() == [1, 1, 1, 1]
+    assert (fl_d + fl_a).tolist() == [0, 1, 1, 0]                  # a flush exactly where route != cur
+
+
+def test_o4_round_equals_separate_calls_and_eager():
+    """LazyCatchup.round (one batched prefill per round) leaves the logical cache, the cache length and the backlog
+    identical to the three separate calls it stands for (kv_only_prefill for the active sequences, enqueue, flush), and
+    after a final flush identical to eager appends: 300 random rounds with a route that follows a random walk, cap 8
+    (forced flushes happen), rows 0..5 per round."""
+    g = synth.rng(21, 3)
+    S, cap, hidden = 3, 8, 32
+    fused = lazy_catchup.LazyCatchup(_drafter(seed=5, max_seqs=S, num_pages=1200), cap)
+    sep = lazy_catchup.LazyCatchup(_drafter(seed=5, max_seqs=S, num_pages=1200), cap)
+    eager = _drafter(seed=5, max_seqs=S, num_pages=1200)
+    code = 1
+    cur = g.integers(0, 2, size=S)
+    q_indptr = (np.arange(S + 1) * 6).astype(np.int32)
+    forced = 0
+    for rnd in range(300):
+        X = synth.normal_bf16(g, (S * 6, hidden), 1.0)
+        n = g.integers(0, 6, size=S)
+        route = np.where(g.random(S) < 0.3, 1 - cur, cur)
+        idle, fl = lazy_catchup.switch_masks(route, cur, code)
+        forced += int(((sep.backlog_len[:S] + n > cap) & (idle == 1) & (fl == 0)).sum())
+        fused.round(X, q_indptr, n, idle, fl)
+        kv_prefill.kv_only_prefill(sep.drafter, X, q_indptr, n * (1 - idle))
+        sep.enqueue(X, q_indptr, n, idle)
+        sep.flush(fl, S)
+        kv_prefill.kv_only_prefill(eager, X, q_indptr, n)
+        _same_cache(fused.drafter.kv, sep.drafter.kv)
+        assert np.array_equal(fused.backlog_len, sep.backlog_len)
+        for b in range(S):
+            assert np.array_equal(fused.backlog[b, :fused.backlog_len[b]], sep.backlog[b, :sep.backlog_len[b]])
+        cur = route
+    assert forced > 5, "the run must exercise forced flushes"
+    fused.flush(None, S)
+    _same_cache(fused.drafter.kv, eager.kv)
+
+
+def test_switch_round_drives_both_drafters():
+    """switch_round: per round exactly the active drafter's cache grows by n_rows, the other one's backlog does (or it
+    is flushed on a switch); cur' = route; the next block length follows the route."""
+    g = synth.rng(22, 3)
+    S, cap = 3, 16
+    lz = {0: lazy_catchup.LazyCatchup(_drafter(seed=6, L=2, max_seqs=S, num_pages=600), cap),
+          1: lazy_catchup.LazyCatchup(_drafter(seed=7, L=1, max_seqs=S, num_pages=600), cap)}
+    cur = np.array([0, 1, 0])
+    q_indptr = (np.arange(S + 1) * 4).astype(np.int32)
+    total = np.zeros(S, dtype=np.int64)
+    for rnd in range(40):
+        X = synth.normal_bf16(g, (S * 4, 32), 1.0)
+        n = g.integers(1, 5, size=S)
+        route = g.integers(0, 2, size=S)
+        before = {c: (l.drafter.kv.seq_len.copy(), l.backlog_len.copy()) for c, l in lz.items()}
+        cur2, nq, _ = lazy_catchup.switch_round(lz, X, q_indptr, n, route, cur, {0: 16, 1: 8})
+        total += n
+        for b in range(S):
+            act, oth = int(cur[b]), 1 - int(cur[b])
+            assert lz[act].drafter.kv.seq_len[b] == before[act][0][b] + n[b] and lz[act].backlog_len[b] == 0
+            if route[b] != cur[b]:                                  # the other drafter catches up completely
+                assert lz[oth].backlog_len[b] == 0 and lz[oth].drafter.kv.seq_len[b] == total[b]
+            else:
+                assert lz[oth].drafter.kv.seq_len[b] + lz[oth].backlog_len[b] == total[b]
+        assert np.array_equal(cur2, route) and nq.tolist() == [16 if r == 0 else 8 for r in route]
+        cur = cur2
