@@ -20,6 +20,8 @@ written in the paper's order and notation so it can be checked against
   O7  tree_verify.tree_attn / tree_accept_entropy_route / compact_path
                                          PAPER.md:65, :39, :317, :327 (tree verification)
   O8  spec_sample.spec_sample_entropy_route  PAPER.md:19, :79-81 (stochastic acceptance with temperature)
+  O9  final_token.final_tokens_full      PAPER.md:119, :206 (the final backlog token through the drafter layer in full;
+                                         SURVEY.md §8(f) f3)
 
 Pins (tests/test_oracle_*.py, `-m "not gpu"`): closed forms, invariants,
 textbook special cases and pure-Python brute force; see DESIGN.md §"Oracle pins".
@@ -28,4 +30,4 @@ which the paper prints no worked numeric example ("parity unpinned" for the
 end-to-end round values only; each part is pinned separately).
 """
 
-from . import bf16, paged_kv, verify_attn, accept_route, kv_prefill, lazy_catchup, neural_route, tree_verify, spec_sample  # noqa: F401
+from . import bf16, paged_kv, verify_attn, accept_route, kv_prefill, lazy_catchup, neural_route, tree_verify, spec_sample, final_token  # noqa: F401
