@@ -192,12 +192,45 @@ int wf_lazy_catchup_round(wf_ctx* ctx, wf_drafter* d, const void* hidden, const 
  * and does for BOTH drafters what wf_lazy_catchup_round(idle_X, flush_X) does for one, in the same two launches (the
  * tiles of both projections share one grid).  Afterwards cur_drafter[b] <- route[b] and, if next_q_len != NULL,
  * next_q_len[b] <- (route[b] == WF_ROUTE_AR ? q_len_ar : q_len_diffusion): the block length the chosen drafter will
- * bring next round.  No mask and no length crosses the host.  Both drafters need the same hidden size and head_dim and
- * distinct caches; other limits as wf_lazy_catchup_round. */
+ * bring next round; if switched != NULL, switched[b] <- route[b] where the sequence switched drafters this round
+ * (route[b] != the old cur_drafter[b]), else -1: the selection wf_final_token_full takes.  No mask and no length crosses
+ * the host.  Both drafters need the same hidden size and head_dim and distinct caches; other limits as
+ * wf_lazy_catchup_round. */
 int wf_switch_round(wf_ctx* ctx, wf_drafter* drafter_ar, wf_drafter* drafter_diffusion, const void* hidden,
                     const int32_t* q_indptr, const int32_t* n_rows, const int32_t* seq_ids, const int32_t* route,
-                    int32_t* cur_drafter, int32_t* next_q_len, int q_len_ar, int q_len_diffusion, int B, int max_rows,
-                    void* stream);
+                    int32_t* cur_drafter, int32_t* next_q_len, int32_t* switched, int q_len_ar, int q_len_diffusion,
+                    int B, int max_rows, void* stream);
+
+/* ---- (f3) the final backlog token in full -----------------------------------------------------------
+ * PAPER.md:119 (§3.4: "we compute only the attention layer on tokens accepted by another drafter, processing only the
+ * final token in full, so that its post-MLP hidden state can feed the next draft round"), :206; SURVEY.md §8(f) f3;
+ * DESIGN.md readings F1-F6.
+ *
+ * wf_drafter_set_full_layer: gives the drafter the weights KV-only prefill skips, per layer l (HOST arrays of
+ * n_layers DEVICE pointers, bf16, row vector times matrix as C18): W_Q [hidden][n_q_heads*head_dim],
+ * W_O [n_q_heads*head_dim][hidden], W_up [hidden][ffn], W_down [ffn][hidden].  The library keeps its own repacked
+ * copy (the caller's matrices are not read again) and activation scratch for max_tokens (<= 256) tokens per call.
+ * hidden, n_q_heads*head_dim and ffn must be multiples of 128.  Synchronous; once per drafter.
+ *
+ * wf_final_token_full: for every b in [0,B) with (select == NULL || select[b] == select_code), n_rows[b] > 0 and a
+ * non-empty cache: x = hidden[q_indptr[b] + n_rows[b] - 1] (the last row this round's catch-up prefill appended),
+ * p = drafter_kv.seq_len[b] - 1 (its position; its K/V are in the cache already: call this AFTER the switch / flush
+ * of the round), and for every drafter layer l (independent branches over the same x, reading C14 / F3)
+ *     q = RoPE(x W_Q[l], p);  att = softmax(q K_l^T / sqrt(head_dim)) V_l over cache positions 0..p (GQA map C11);
+ *     y = x + att W_O[l];     h_out[b][l] = y + GELU(y W_up[l]) W_down[l]     (tanh-form GELU, no norms, no biases).
+ * h_out: bf16 [B][n_layers][hidden]; rows of unselected sequences are not written.  bf16 operands, fp32 accumulation,
+ * bf16 RNE at q, att, the operand copies of y and GELU(.), and h_out; split-K sums in a fixed order (deterministic).
+ * More selected sequences than max_tokens: the surplus (highest b) is skipped and the sticky status becomes
+ * WF_ERR_INVALID_ARG.  Sequence b uses block-table row b (no seq_ids).  select is typically the `switched` output of
+ * wf_switch_round with select_code = this drafter's route code, or a 0/1 mask with select_code = 1.
+ * workspace: >= wf_final_token_workspace_bytes(d, B).  5 + n_layers launches, asynchronous on `stream`. */
+int wf_drafter_set_full_layer(wf_ctx* ctx, wf_drafter* d, int n_q_heads, int ffn, int max_tokens,
+                              const void* const* w_q_host_ptrs, const void* const* w_o_host_ptrs,
+                              const void* const* w_up_host_ptrs, const void* const* w_down_host_ptrs);
+size_t wf_final_token_workspace_bytes(const wf_drafter* d, int B);
+int wf_final_token_full(wf_ctx* ctx, wf_drafter* d, const void* hidden, const int32_t* q_indptr, const int32_t* n_rows,
+                        const int32_t* select, int select_code, int B, void* h_out, void* workspace,
+                        size_t workspace_bytes, void* stream);
 
 /* ---- (f1) WhiFlash-Neural routing policy --------------------------------------------------------
  * PAPER.md:87 (§3.3.2), :103-107 (decision rule), :325 (App. A architecture); readings N1-N6.

@@ -34,6 +34,7 @@ EXPORTS = [
     "wf_neural_route", "wf_neural_route_workspace_bytes", "wf_lazy_catchup_round",
     "wf_tree_masks", "wf_verify_attn_tree", "wf_accept_tree_entropy_route", "wf_kv_compact_path",
     "wf_accept_sample_entropy_route", "wf_switch_round",
+    "wf_drafter_set_full_layer", "wf_final_token_workspace_bytes", "wf_final_token_full",
 ]
 
 
@@ -69,7 +70,10 @@ _SIG = {
     "wf_lazy_catchup_enqueue": (_i, [_vp, _vp, _vp, _vp, _vp, _vp, _vp, _i, _i, _vp]),
     "wf_lazy_catchup_flush": (_i, [_vp, _vp, _vp, _i, _vp]),
     "wf_lazy_catchup_round": (_i, [_vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _i, _i, _vp]),
-    "wf_switch_round": (_i, [_vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _i, _i, _i, _i, _vp]),
+    "wf_switch_round": (_i, [_vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _i, _i, _i, _i, _vp]),
+    "wf_drafter_set_full_layer": (_i, [_vp, _vp, _i, _i, _i, C.POINTER(_vp), C.POINTER(_vp), C.POINTER(_vp), C.POINTER(_vp)]),
+    "wf_final_token_workspace_bytes": (_sz, [_vp, _i]),
+    "wf_final_token_full": (_i, [_vp, _vp, _vp, _vp, _vp, _vp, _i, _i, _vp, _vp, _sz, _vp]),
     "wf_neural_route_workspace_bytes": (_sz, [_i, _i]),
     "wf_neural_route": (_i, [_vp, _vp, _vp, _vp, _i, _i, _i, _vp, _vp, _vp, _vp, _vp, _i, _vp, _vp, _vp, _sz, _vp]),
     "wf_tree_masks": (_i, [_vp, _vp, _vp, _i, _i, _vp, _vp]),
@@ -194,6 +198,12 @@ class Drafter:
         ctx.check(lib.wf_drafter_create(ctx.h, C.byref(shape), wk, wv, kv.h, _ptr(backlog), _ptr(backlog_len), C.byref(h)))
         self.h = h
 
+    def set_full_layer(self, n_q_heads, ffn, max_tokens, w_q, w_o, w_up, w_down):
+        """(f3) the weights of the drafter layer that KV-only prefill skips; the library repacks its own copy."""
+        L = self.shape.n_layers
+        arrs = [(_vp * L)(*[_ptr(w) for w in ws]) for ws in (w_q, w_o, w_up, w_down)]
+        self.ctx.check(lib.wf_drafter_set_full_layer(self.ctx.h, self.h, n_q_heads, ffn, max_tokens, *arrs))
+
     def close(self):
         if self.h:
             lib.wf_drafter_destroy(self.h)
@@ -231,10 +241,20 @@ def wf_lazy_catchup_round(ctx, drafter, hidden, q_indptr, n_rows, seq_ids, idle_
 
 
 def wf_switch_round(ctx, drafter_ar, drafter_diffusion, hidden, q_indptr, n_rows, seq_ids, route, cur_drafter, next_q_len,
-                    q_len_ar, q_len_diffusion, B, max_rows, stream=None):
+                    q_len_ar, q_len_diffusion, B, max_rows, stream=None, switched=None):
     ctx.check(lib.wf_switch_round(ctx.h, drafter_ar.h, drafter_diffusion.h, _ptr(hidden), _ptr(q_indptr), _ptr(n_rows),
-                                  _ptr(seq_ids), _ptr(route), _ptr(cur_drafter), _ptr(next_q_len), q_len_ar, q_len_diffusion,
-                                  B, max_rows, _stream(stream)))
+                                  _ptr(seq_ids), _ptr(route), _ptr(cur_drafter), _ptr(next_q_len), _ptr(switched),
+                                  q_len_ar, q_len_diffusion, B, max_rows, _stream(stream)))
+
+
+def wf_final_token_workspace_bytes(drafter, B):
+    return int(lib.wf_final_token_workspace_bytes(drafter.h, B))
+
+
+def wf_final_token_full(ctx, drafter, hidden, q_indptr, n_rows, select, select_code, B, h_out, workspace, stream=None):
+    ctx.check(lib.wf_final_token_full(ctx.h, drafter.h, _ptr(hidden), _ptr(q_indptr), _ptr(n_rows), _ptr(select),
+                                      select_code, B, _ptr(h_out), _ptr(workspace),
+                                      workspace.numel() * workspace.element_size(), _stream(stream)))
 
 
 def wf_tree_masks(ctx, parent, q_indptr, B, max_nodes, tree_mask, stream=None):

@@ -51,6 +51,8 @@ struct AttnParams {
   const unsigned long long* tree_mask; // TREE only: [sum_q] ancestor mask of each row (bit j = node j of its sequence)
   KvView kv;
   int layer, B, n_q_heads, group;
+  int ctx_adj;                         // added to seq_len: 0 for verification (the block sits behind the cache length, C10);
+                                       // -1 for the final-token path (wf_final.cu: the token is the last cached one, F1)
   float scale_log2;                    // sm_scale * log2(e)
   float4* ws_o;                        // [2 * CTAs][D/8][128 threads] float4: unnormalised O in fragment order
   float4* ws_ml;                       // [2 * CTAs][128 threads] (m, l) of the thread's two rows (m in log2 units)
@@ -930,7 +932,7 @@ __global__ void __launch_bounds__(AT_THREADS, 1) wf_verify_attn_kernel(const Att
   int* t_ctx = t_r0 + AT_MAX_B;
   int* t_q = t_ctx + AT_MAX_B;
   for (int b = tid; b < p.B; b += AT_THREADS) {
-    const int r0 = p.q_indptr[b], r1 = p.q_indptr[b + 1], ctx = p.kv.seq_len[b];
+    const int r0 = p.q_indptr[b], r1 = p.q_indptr[b + 1], ctx = p.kv.seq_len[b] + p.ctx_adj;
     // the host bound max_q_len / max_nodes is a promise: a longer block has its rows beyond the query tile dropped
     if (blockIdx.x == 0 && (TREE ? r1 - r0 > 64 : (r1 - r0) * p.group > AT_ROWS)) wf_raise(p.status, (int)WF_ERR_INVALID_ARG);
     if constexpr (TREE) {
@@ -1090,23 +1092,24 @@ extern "C" size_t wf_verify_attn_workspace_bytes(const wf_kv_shape* s, int B, in
   return items * (r_pad * (size_t)s->head_dim * sizeof(float) + 128 * sizeof(float4));
 }
 
-extern "C" int wf_verify_attn(wf_ctx* ctx, const wf_paged_kv* kv, int layer, const void* q,
-                              const int32_t* q_indptr, int B, int n_q_heads, int max_q_len, float sm_scale,
-                              void* out, void* workspace, size_t workspace_bytes, void* stream) {
-  if (!ctx) return WF_ERR_INVALID_ARG;
-  WF_REQUIRE(ctx, kv && q && q_indptr && out && workspace, WF_ERR_INVALID_ARG, "wf_verify_attn: null argument");
-  WF_REQUIRE(ctx, layer >= 0 && layer < kv->s.n_layers, WF_ERR_INVALID_ARG, "wf_verify_attn: bad layer");
+// shared by wf_verify_attn (ctx_adj = 0) and the final-token path of wf_final.cu (ctx_adj = -1, one query row per
+// selected sequence over a drafter's cache)
+int wf_attn_launch_chain(wf_ctx* ctx, const wf_paged_kv* kv, int layer, const void* q, const int32_t* q_indptr, int B,
+                         int n_q_heads, int max_q_len, float sm_scale, int ctx_adj, void* out, void* workspace,
+                         size_t workspace_bytes, void* stream, const char* who) {
+  WF_REQUIRE(ctx, kv && q && q_indptr && out && workspace, WF_ERR_INVALID_ARG, "%s: null argument", who);
+  WF_REQUIRE(ctx, layer >= 0 && layer < kv->s.n_layers, WF_ERR_INVALID_ARG, "%s: bad layer", who);
   WF_REQUIRE(ctx, B >= 0 && B <= kv->s.max_seqs && B <= AT_MAX_B && B * kv->s.n_kv_heads <= ctx->n_counters,
-             WF_ERR_INVALID_ARG, "wf_verify_attn: bad B (max %d)", AT_MAX_B);
+             WF_ERR_INVALID_ARG, "%s: bad B (max %d)", who, AT_MAX_B);
   WF_REQUIRE(ctx, n_q_heads > 0 && n_q_heads % kv->s.n_kv_heads == 0, WF_ERR_INVALID_ARG,
-             "wf_verify_attn: n_q_heads must be a multiple of n_kv_heads");
+             "%s: n_q_heads must be a multiple of n_kv_heads", who);
   const int group = n_q_heads / kv->s.n_kv_heads;
   WF_REQUIRE(ctx, max_q_len >= 1 && max_q_len * group <= 64, WF_ERR_UNSUPPORTED_SHAPE,
-             "wf_verify_attn: max_q_len * group must be in [1, 64]");
+             "%s: max_q_len * group must be in [1, 64]", who);
   WF_REQUIRE(ctx, workspace_bytes >= wf_verify_attn_workspace_bytes(&kv->s, B, n_q_heads, max_q_len),
-             WF_ERR_INVALID_ARG, "wf_verify_attn: workspace too small");
+             WF_ERR_INVALID_ARG, "%s: workspace too small", who);
   WF_REQUIRE(ctx, ((uintptr_t)q % 16 == 0) && ((uintptr_t)out % 16 == 0) && ((uintptr_t)workspace % 16 == 0),
-             WF_ERR_INVALID_ARG, "wf_verify_attn: q/out/workspace must be 16-byte aligned");
+             WF_ERR_INVALID_ARG, "%s: q/out/workspace must be 16-byte aligned", who);
   if (B == 0) return WF_OK;
   const int r_pad = AT_ROWS;
   const size_t items = 4 * (size_t)AT_MAX_CTAS;
@@ -1116,6 +1119,7 @@ extern "C" int wf_verify_attn(wf_ctx* ctx, const wf_paged_kv* kv, int layer, con
   p.q_indptr = q_indptr;
   p.kv = kv_view(kv);
   p.layer = layer; p.B = B; p.n_q_heads = n_q_heads; p.group = group;
+  p.ctx_adj = ctx_adj;
   p.scale_log2 = sm_scale * LOG2E;
   p.ws_o = (float4*)workspace;
   p.ws_ml = (float4*)((char*)workspace + items * r_pad * kv->s.head_dim * sizeof(float));
@@ -1126,7 +1130,15 @@ extern "C" int wf_verify_attn(wf_ctx* ctx, const wf_paged_kv* kv, int layer, con
   p.tree_mask = nullptr;
   if (D == 128) return launch_attn<128, false>(ctx, p, st);
   if (D == 64) return launch_attn<64, false>(ctx, p, st);
-  return wf_set_error(ctx, WF_ERR_UNSUPPORTED_SHAPE, "wf_verify_attn: head_dim %d unsupported", D);
+  return wf_set_error(ctx, WF_ERR_UNSUPPORTED_SHAPE, "%s: head_dim %d unsupported", who, D);
+}
+
+extern "C" int wf_verify_attn(wf_ctx* ctx, const wf_paged_kv* kv, int layer, const void* q,
+                              const int32_t* q_indptr, int B, int n_q_heads, int max_q_len, float sm_scale,
+                              void* out, void* workspace, size_t workspace_bytes, void* stream) {
+  if (!ctx) return WF_ERR_INVALID_ARG;
+  return wf_attn_launch_chain(ctx, kv, layer, q, q_indptr, B, n_q_heads, max_q_len, sm_scale, 0, out, workspace,
+                              workspace_bytes, stream, "wf_verify_attn");
 }
 
 extern "C" int wf_tree_masks(wf_ctx* ctx, const int32_t* parent, const int32_t* q_indptr, int B, int max_nodes,
@@ -1170,6 +1182,7 @@ extern "C" int wf_verify_attn_tree(wf_ctx* ctx, const wf_paged_kv* kv, int layer
   p.tree_mask = (const unsigned long long*)tree_mask;
   p.kv = kv_view(kv);
   p.layer = layer; p.B = B; p.n_q_heads = n_q_heads; p.group = group;
+  p.ctx_adj = 0;
   p.scale_log2 = sm_scale * LOG2E;
   p.ws_o = (float4*)workspace;
   p.ws_ml = (float4*)((char*)workspace + items * AT_ROWS * kv->s.head_dim * sizeof(float));

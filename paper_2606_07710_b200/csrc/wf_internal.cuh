@@ -27,7 +27,7 @@ struct wf_ctx {
 // bookkeeping is per ctx (a ctx is bound to one device), never per process
 enum {
   WF_FUNC_ATTN_128 = 0, WF_FUNC_ATTN_64, WF_FUNC_ATTN_TREE_128, WF_FUNC_ATTN_TREE_64, WF_FUNC_GEMM_128, WF_FUNC_GEMM_64,
-  WF_FUNC_NEURAL, WF_FUNC_ACCEPT, WF_FUNC_FINAL_TOKEN, WF_FUNC_GEMV
+  WF_FUNC_NEURAL, WF_FUNC_ACCEPT, WF_FUNC_FINAL_TOKEN /* + EPI 0..3 */, WF_FUNC_FINAL_TOKEN_LAST = WF_FUNC_FINAL_TOKEN + 3
 };
 #define WF_CONFIGURE_ONCE(ctx, bit, kernel, bytes)                                                          \
   do {                                                                                                      \
@@ -77,6 +77,37 @@ static inline KvView kv_view(const wf_paged_kv* kv) {
   v.max_pages_per_seq = kv->s.max_pages_per_seq;
   return v;
 }
+
+struct wf_row_entry {
+  int32_t pos;                 // absolute position (RoPE)
+  int32_t page_slot;           // physical page * 16 + slot in the drafter cache
+};
+struct wf_full_layer;          // wf_final.cu: the weights and scratch of the final-token path (f3)
+
+struct wf_drafter {
+  wf_ctx* ctx;
+  wf_drafter_shape s;
+  wf_paged_kv* kv;
+  const __nv_bfloat16* backlog;
+  int32_t* backlog_len;
+  uint8_t* d_wpack;            // library-owned pre-swizzled copy of the weights (see wf_pack_w_kernel)
+  uint8_t* d_xpack;            // library-owned [hidden/64][row_cap][128 B] scratch (see wf_plan_pack_kernel)
+  int n_split;                 // split-K factor of the projection, fixed at creation (a power of two)
+  int max_pass;
+  float* d_ws_part;            // [tiles][n_split][row_cap][D] fp32 partials (n_split > 1)
+  unsigned int* d_split_cnt;   // [tiles][max_pass]
+  float2* d_rope;              // [max_pos][D/2]
+  wf_row_entry* d_rows;
+  int row_cap;
+  int32_t* d_m_total;
+  int32_t* d_plan;             // [2 * max_seqs]: enq_base, new_blen (planner -> kernel 2)
+  wf_full_layer* full;         // NULL until wf_drafter_set_full_layer
+};
+void wf_full_layer_destroy(wf_full_layer* f);
+// wf_attn.cu: the chain attention kernel with seq_len + ctx_adj as the context (see AttnParams::ctx_adj)
+int wf_attn_launch_chain(wf_ctx* ctx, const wf_paged_kv* kv, int layer, const void* q, const int32_t* q_indptr, int B,
+                         int n_q_heads, int max_q_len, float sm_scale, int ctx_adj, void* out, void* workspace,
+                         size_t workspace_bytes, void* stream, const char* who);
 
 int wf_set_error(wf_ctx* ctx, int code, const char* fmt, ...);
 // cuTensorMapEncodeTiled through the runtime's driver entry point (no link-time libcuda dependency)

@@ -38,10 +38,7 @@ constexpr int PF_SMEM_BUDGET = 200 * 1024;
 constexpr int PP_THREADS = 256;         // plan + pack kernel
 constexpr int PP_MAX_B = KV_RESERVE_SMEM;   // sequences per call (the per-sequence plan lives in shared memory)
 constexpr int PP_MAX_PACK_CTAS = 296;   // pack CTAs per drafter: two per SM
-struct RowEntry {
-  int32_t pos;                          // absolute position (RoPE)
-  int32_t page_slot;                    // physical page * 16 + slot in the drafter cache
-};
+using RowEntry = wf_row_entry;
 
 // ---- kernel 1 of 2: plan + pack ------------------------------------------------------------------
 // What one call asks of a drafter, per sequence b (seq = seq_ids ? seq_ids[b] : b, len = its backlog length, add = n_rows[b]):
@@ -275,6 +272,7 @@ struct GemmJob {
   const int32_t* route;
   int32_t* cur;
   int32_t* next_q_len;                  // nullable
+  int32_t* switched;                    // nullable: route[b] where it differs from cur[b] (a switch), else -1
   int q_len_ar, q_len_diffusion;
 };
 
@@ -333,6 +331,7 @@ __global__ void __launch_bounds__(PF_THREADS, 1) wf_prefill_gemm_kernel(const __
       if (p.route && jb == 0)
         for (int b = t0; b < p.B; b += nt) {
           const int r = p.route[b];
+          if (p.switched) p.switched[b] = r != p.cur[b] ? r : -1;
           p.cur[b] = r;
           if (p.next_q_len) p.next_q_len[b] = r == WF_ROUTE_AR ? p.q_len_ar : p.q_len_diffusion;
         }
@@ -574,24 +573,6 @@ __global__ void __launch_bounds__(PF_THREADS, 1) wf_prefill_gemm_kernel(const __
 // ------------------------------------------------------------------------------------------------
 // host side
 // ------------------------------------------------------------------------------------------------
-struct wf_drafter {
-  wf_ctx* ctx;
-  wf_drafter_shape s;
-  wf_paged_kv* kv;
-  const __nv_bfloat16* backlog;
-  int32_t* backlog_len;
-  uint8_t* d_wpack;            // library-owned pre-swizzled copy of the weights (see wf_pack_w_kernel)
-  uint8_t* d_xpack;            // library-owned [hidden/64][row_cap][128 B] scratch (see wf_pack_x_kernel)
-  int n_split;                 // split-K factor of the projection, fixed at creation (a power of two)
-  int max_pass;
-  float* d_ws_part;            // [tiles][n_split][row_cap][D] fp32 partials (n_split > 1)
-  unsigned int* d_split_cnt;   // [tiles][max_pass]
-  float2* d_rope;              // [max_pos][D/2]
-  RowEntry* d_rows;
-  int row_cap;
-  int32_t* d_m_total;
-  int32_t* d_plan;             // [2 * max_seqs]: enq_base, new_blen (planner -> kernel 2)
-};
 
 namespace {
 
@@ -604,8 +585,8 @@ struct CallJob {
   bool enqueues;                        // ENQUEUE / ROUND with idle sequences
 };
 
-int run_jobs(wf_ctx* ctx, CallJob* jobs, int n_jobs, const int32_t* route, int32_t* cur, int32_t* next_q_len, int q_len_ar,
-             int q_len_diffusion, cudaStream_t st) {
+int run_jobs(wf_ctx* ctx, CallJob* jobs, int n_jobs, const int32_t* route, int32_t* cur, int32_t* next_q_len,
+             int32_t* switched, int q_len_ar, int q_len_diffusion, cudaStream_t st) {
   PlanPackParams pp{};
   GemmParams gp{};
   pp.n_jobs = gp.n_jobs = n_jobs;
@@ -637,7 +618,7 @@ int run_jobs(wf_ctx* ctx, CallJob* jobs, int n_jobs, const int32_t* route, int32
     g.new_blen = (pj.mode == PLAN_EAGER || pj.cap == 0) ? nullptr : pj.new_blen;
     g.backlog = const_cast<__nv_bfloat16*>(d->backlog); g.backlog_len = d->backlog_len;
     g.B = pj.B; g.cap = pj.cap; g.max_rows = pj.max_rows;
-    g.route = route; g.cur = cur; g.next_q_len = next_q_len; g.q_len_ar = q_len_ar; g.q_len_diffusion = q_len_diffusion;
+    g.route = route; g.cur = cur; g.next_q_len = next_q_len; g.switched = switched; g.q_len_ar = q_len_ar; g.q_len_diffusion = q_len_diffusion;
     const int ctas = d->s.n_layers * 2 * d->s.n_kv_heads * d->n_split;
     gemm_grid += ctas;
     if (j == 0) gp.ctas_job0 = ctas;
@@ -658,7 +639,7 @@ int run_jobs(wf_ctx* ctx, CallJob* jobs, int n_jobs, const int32_t* route, int32
 
 int run_one(wf_ctx* ctx, wf_drafter* d, const PlanJob& pj, int rows_upper, bool enqueues, cudaStream_t st) {
   CallJob job{d, pj, rows_upper, enqueues};
-  return run_jobs(ctx, &job, 1, nullptr, nullptr, nullptr, 0, 0, st);
+  return run_jobs(ctx, &job, 1, nullptr, nullptr, nullptr, nullptr, 0, 0, st);
 }
 
 }  // namespace
@@ -697,7 +678,7 @@ extern "C" int wf_drafter_create(wf_ctx* ctx, const wf_drafter_shape* s, const v
   if (!d) return wf_set_error(ctx, WF_ERR_INVALID_ARG, "wf_drafter_create: host allocation failed");
   d->ctx = ctx; d->s = *s; d->kv = kv;
   d->backlog = (const __nv_bfloat16*)backlog; d->backlog_len = backlog_len;
-  d->d_wpack = nullptr; d->d_xpack = nullptr; d->d_rope = nullptr; d->d_ws_part = nullptr; d->d_split_cnt = nullptr; d->d_rows = nullptr; d->d_m_total = nullptr; d->d_plan = nullptr;
+  d->d_wpack = nullptr; d->d_xpack = nullptr; d->d_rope = nullptr; d->d_ws_part = nullptr; d->d_split_cnt = nullptr; d->d_rows = nullptr; d->d_m_total = nullptr; d->d_plan = nullptr; d->full = nullptr;
   // rows one call can carry: a whole backlog plus a block (64 rows at most) per sequence (wf_lazy_catchup_round)
   d->row_cap = kv->s.max_seqs * ((s->backlog_cap > 64 ? s->backlog_cap : 64) + 64);
   // Split-K: a call with few tiles (a 1-layer drafter has 16) cannot pull HBM bandwidth through 16 SMs; spread each
@@ -744,6 +725,7 @@ extern "C" int wf_drafter_create(wf_ctx* ctx, const wf_drafter_shape* s, const v
 extern "C" int wf_drafter_destroy(wf_drafter* d) {
   if (!d) return WF_ERR_INVALID_ARG;
   cudaFree(d->d_wpack); cudaFree(d->d_xpack); cudaFree(d->d_ws_part); cudaFree(d->d_split_cnt); cudaFree(d->d_rope); cudaFree(d->d_rows); cudaFree(d->d_m_total); cudaFree(d->d_plan);
+  if (d->full) wf_full_layer_destroy(d->full);
   delete d;
   return WF_OK;
 }
@@ -823,8 +805,8 @@ extern "C" int wf_lazy_catchup_round(wf_ctx* ctx, wf_drafter* d, const void* hid
 
 extern "C" int wf_switch_round(wf_ctx* ctx, wf_drafter* drafter_ar, wf_drafter* drafter_diffusion, const void* hidden,
                                const int32_t* q_indptr, const int32_t* n_rows, const int32_t* seq_ids,
-                               const int32_t* route, int32_t* cur_drafter, int32_t* next_q_len, int q_len_ar,
-                               int q_len_diffusion, int B, int max_rows, void* stream) {
+                               const int32_t* route, int32_t* cur_drafter, int32_t* next_q_len, int32_t* switched,
+                               int q_len_ar, int q_len_diffusion, int B, int max_rows, void* stream) {
   if (!ctx || !drafter_ar || !drafter_diffusion) return WF_ERR_INVALID_ARG;
   WF_REQUIRE(ctx, route && cur_drafter, WF_ERR_INVALID_ARG, "wf_switch_round: null route / cur_drafter");
   WF_REQUIRE(ctx, drafter_ar != drafter_diffusion && drafter_ar->kv != drafter_diffusion->kv, WF_ERR_INVALID_ARG,
@@ -844,5 +826,5 @@ extern "C" int wf_switch_round(wf_ctx* ctx, wf_drafter* drafter_ar, wf_drafter* 
     jobs[j] = CallJob{ds[j], pj, B * (ds[j]->s.backlog_cap + max_rows), true};
   }
   if (B == 0 || max_rows == 0) return WF_OK;
-  return run_jobs(ctx, jobs, 2, route, cur_drafter, next_q_len, q_len_ar, q_len_diffusion, (cudaStream_t)stream);
+  return run_jobs(ctx, jobs, 2, route, cur_drafter, next_q_len, switched, q_len_ar, q_len_diffusion, (cudaStream_t)stream);
 }

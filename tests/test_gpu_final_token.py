@@ -1,0 +1,212 @@
+"""GPU parity (through the C-ABI) for (f3) the final backlog token run in full, against oracle O9.
+
+PAPER.md:119, :206; readings F1-F6.  Tolerance (F6): the post-MLP state within relative L2
+5e-3 and max-abs 2e-2 x its RMS of the oracle's unrounded fp64 value, per (sequence, layer); which sequences are computed
+(and which rows of h_out stay untouched) is exact.
+"""
+
+import numpy as np
+import pytest
+
+from oracle import final_token, kv_prefill, lazy_catchup
+from paper_2606_07710_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+H_REL_L2 = 5e-3
+
+
+@pytest.fixture(scope="module")
+def wf():
+    import torch
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device"
+    from paper_2606_07710_b200 import binding
+    ctx = binding.Ctx(0)
+    yield binding, ctx
+    ctx.close()
+
+
+def _mk(ctx, L, hidden, Hq, Hkv, D, F, S, pages_per_seq, seed, max_tokens, cap=32, w_std=0.02):
+    import gpu_harness as H
+    g = synth.rng(seed, 505)
+    P = S * pages_per_seq + 7
+    free = synth.draw_free_list(P, g, True)
+    dp = H.DrafterPair(ctx, L, hidden, Hkv, D, P, S, pages_per_seq, free, seed, backlog_cap=cap, w_std=w_std)
+    shapes = [(hidden, Hq * D), (Hq * D, hidden), (hidden, F), (F, hidden)]
+    bits = [[synth.normal_bf16(g, sh, w_std) for _ in range(L)] for sh in shapes]
+    dp.full = final_token.FullLayer(bits[0], bits[1], bits[2], bits[3], Hq)
+    dp.full_gpu = [[H.bits_to_bf16_tensor(w) for w in ws] for ws in bits]
+    dp.gpu.set_full_layer(Hq, F, max_tokens, *dp.full_gpu)
+    return dp, g
+
+
+def _run(binding, ctx, dp, X, q_indptr, n_rows, select, code, sentinel=True):
+    """Calls wf_final_token_full and returns h_out as fp64 [B][L][hidden] plus the raw bits."""
+    import torch
+    import gpu_harness as H
+    B = len(n_rows)
+    L, hid = dp.shape.n_layers, dp.shape.hidden
+    h_out = torch.full((B, L, hid), 7.0, dtype=torch.bfloat16, device="cuda")
+    ws = torch.empty(binding.wf_final_token_workspace_bytes(dp.gpu, B), dtype=torch.uint8, device="cuda")
+    sel = None if select is None else H.i32(select)
+    binding.wf_final_token_full(ctx, dp.gpu, H.bits_to_bf16_tensor(X), H.i32(q_indptr), H.i32(n_rows), sel, code, B, h_out, ws)
+    torch.cuda.synchronize()
+    return H.bf16_f64(H.bf16_tensor_to_bits(h_out))
+
+
+def _compare(got, want_by_b, B, tag=""):
+    worst = 0.0
+    for b in range(B):
+        if b not in want_by_b:
+            assert np.all(got[b] == 7.0), f"{tag}: h_out of unselected sequence {b} was written"
+            continue
+        for l in range(got.shape[1]):
+            w = want_by_b[b][l]
+            rel = float(np.sqrt(((got[b, l] - w) ** 2).sum() / (w ** 2).sum()))
+            rms = float(np.sqrt((w ** 2).mean()))
+            assert rel <= H_REL_L2, f"{tag}: seq {b} layer {l}: rel-L2 {rel:.3e}"
+            assert np.abs(got[b, l] - w).max() <= 2e-2 * max(rms, 1.0), f"{tag}: seq {b} layer {l}: max-abs"
+            worst = max(worst, rel)
+    return worst
+
+
+def _prefill_both(binding, ctx, dp, X, q_indptr, n_rows):
+    import gpu_harness as H
+    kv_prefill.kv_only_prefill(dp.oracle, X, q_indptr, n_rows)
+    binding.wf_kv_only_prefill(ctx, dp.gpu, H.bits_to_bf16_tensor(X), H.i32(q_indptr), H.i32(n_rows), None, len(n_rows),
+                               int(max(max(n_rows), 1)))
+
+
+def test_final_token_cfg1_tiny(wf):
+    """configs[0] shapes: hidden 256, 4 q / 2 kv heads, head_dim 64, 1-layer drafter, FFN 768; 16 seeds."""
+    binding, ctx = wf
+    for seed in range(16):
+        dp, g = _mk(ctx, 1, 256, 4, 2, 64, 768, 3, 40, 900 + seed, max_tokens=8)
+        lens = [int(v) for v in g.integers(0, 500, 3)]
+        dp.kvp.reserve(lens)
+        dp.kvp.fill_random(g, 0.3)
+        dp.kvp.set_seq_len(lens)
+        n_rows = [int(v) for v in g.integers(1, 9, 3)]
+        q_indptr = np.concatenate([[0], np.cumsum([8, 8, 8])]).astype(np.int32)
+        X = synth.normal_bf16(g, (24, 256), 1.0)
+        _prefill_both(binding, ctx, dp, X, q_indptr, n_rows)
+        select = [int(v) for v in g.integers(0, 2, 3)]
+        want = final_token.final_tokens_full(dp.oracle, dp.full, X, q_indptr, n_rows, select)
+        got = _run(binding, ctx, dp, X, q_indptr, n_rows, select, 1)
+        _compare(got, want, 3, f"seed {seed}")
+        assert ctx.poll_status() == 0
+        dp.close()
+
+
+def test_final_token_8b_shapes_one_layer_drafter(wf):
+    """The paper's AR drafter (a single transformer layer) at 8B-class shapes: hidden 4096, 32 q / 8 kv heads,
+    head_dim 128, FFN 12288; ragged caches (a sequence whose whole cache is this round's rows; one across many tiles),
+    selection through switch codes."""
+    binding, ctx = wf
+    dp, g = _mk(ctx, 1, 4096, 32, 8, 128, 12288, 4, 80, 77, max_tokens=32)
+    lens = [300, 0, 1000, 17]
+    dp.kvp.reserve(lens)
+    dp.kvp.fill_random(g, 0.5)
+    dp.kvp.set_seq_len(lens)
+    n_rows = [5, 3, 1, 2]
+    q_indptr = np.array([0, 8, 24, 32, 40], dtype=np.int32)
+    X = synth.normal_bf16(g, (40, 4096), 1.0)
+    _prefill_both(binding, ctx, dp, X, q_indptr, n_rows)
+    switched = [1, 1, 0, 1]                                     # sequence 2 switched to the OTHER drafter
+    want = final_token.final_tokens_full(dp.oracle, dp.full, X, q_indptr, n_rows, [s == 1 for s in switched])
+    got = _run(binding, ctx, dp, X, q_indptr, n_rows, switched, 1)
+    worst = _compare(got, want, 4, "8b")
+    print(f"final token 8B shapes: worst rel-L2 {worst:.2e}")
+    assert ctx.poll_status() == 0
+    # select == NULL takes every sequence with committed rows
+    want = final_token.final_tokens_full(dp.oracle, dp.full, X, q_indptr, n_rows, [1, 1, 1, 1])
+    _compare(_run(binding, ctx, dp, X, q_indptr, n_rows, None, 0), want, 4, "8b all")
+    dp.close()
+
+
+def test_final_token_multi_layer_many_tokens(wf):
+    """A 3-layer drafter (reading F3: one state per layer), 45 selected tokens (two TMA boxes of the X operand), empty
+    blocks and unselected sequences in between; repeated calls give identical bits (fixed-order split-K)."""
+    binding, ctx = wf
+    S = 50
+    dp, g = _mk(ctx, 3, 512, 8, 2, 128, 1024, S, 12, 5, max_tokens=64, w_std=0.05)
+    lens = [int(v) for v in g.integers(0, 150, S)]
+    dp.kvp.reserve(lens)
+    dp.kvp.fill_random(g, 0.4)
+    dp.kvp.set_seq_len(lens)
+    n_rows = [int(v) for v in g.integers(0, 5, S)]
+    n_rows[3] = 0
+    q_indptr = (np.arange(S + 1) * 4).astype(np.int32)
+    X = synth.normal_bf16(g, (4 * S, 512), 1.0)
+    _prefill_both(binding, ctx, dp, X, q_indptr, n_rows)
+    select = [1] * S
+    select[7] = select[20] = 0
+    want = final_token.final_tokens_full(dp.oracle, dp.full, X, q_indptr, n_rows, select)
+    assert len(want) > 32
+    got = _run(binding, ctx, dp, X, q_indptr, n_rows, select, 1)
+    _compare(got, want, S, "multi")
+    for _ in range(3):
+        assert np.array_equal(got, _run(binding, ctx, dp, X, q_indptr, n_rows, select, 1))
+    assert ctx.poll_status() == 0
+    dp.close()
+
+
+def test_final_token_more_switches_than_slots(wf):
+    """max_tokens = 32 slots, 40 selected sequences: the first 32 (ascending b) are computed, the rest skipped and the
+    sticky status reports it."""
+    binding, ctx = wf
+    S = 40
+    dp, g = _mk(ctx, 1, 256, 4, 2, 64, 256, S, 6, 11, max_tokens=32, w_std=0.05)
+    n_rows = [2] * S
+    q_indptr = (np.arange(S + 1) * 2).astype(np.int32)
+    X = synth.normal_bf16(g, (2 * S, 256), 1.0)
+    _prefill_both(binding, ctx, dp, X, q_indptr, n_rows)
+    want = final_token.final_tokens_full(dp.oracle, dp.full, X, q_indptr, n_rows, [1] * 32 + [0] * 8)
+    got = _run(binding, ctx, dp, X, q_indptr, n_rows, [1] * S, 1)
+    _compare(got, want, S, "overflow")
+    assert ctx.poll_status() == binding.WF_ERR_INVALID_ARG
+    dp.close()
+
+
+def test_switch_then_final_token_device_driven(wf):
+    """The whole switch as the paper defines it: wf_switch_round (catch-up prefill of the backlog, driven
+    by route and cur on the device, `switched` out) followed by wf_final_token_full for the AR drafter on the sequences
+    that switched to it -- against the oracle's switch_round + final_tokens_full driven by the same route."""
+    import torch
+    import gpu_harness as H
+    binding, ctx = wf
+    S, hid = 6, 512
+    dA, g = _mk(ctx, 1, hid, 8, 2, 128, 1024, S, 20, 21, max_tokens=32, cap=32, w_std=0.05)
+    gd = synth.rng(22, 404)
+    PD = S * 20 + 7
+    dD = H.DrafterPair(ctx, 2, hid, 2, 128, PD, S, 20, synth.draw_free_list(PD, gd, True), 23, backlog_cap=32, w_std=0.05)
+    lz = {binding.ROUTE_AR: dA.oracle_lazy, binding.ROUTE_DIFFUSION: dD.oracle_lazy}
+    cur_o = np.array([0, 0, 1, 0, 1, 0], dtype=np.int32)       # who drafted the first block
+    cur = H.i32(cur_o)
+    nq = torch.zeros(S, dtype=torch.int32, device="cuda")
+    switched = torch.zeros(S, dtype=torch.int32, device="cuda")
+    ws = torch.empty(binding.wf_final_token_workspace_bytes(dA.gpu, S), dtype=torch.uint8, device="cuda")
+    n_final = 0
+    for rnd in range(8):
+        q_len = np.where(cur_o == 1, 8, 16)
+        q_indptr = np.concatenate([[0], np.cumsum(q_len)]).astype(np.int32)
+        n_rows = np.array([int(g.integers(1, q + 1)) for q in q_len], dtype=np.int32)
+        route = g.integers(0, 2, S).astype(np.int32)
+        X = synth.normal_bf16(g, (int(q_indptr[-1]), hid), 1.0)
+        Xg = H.bits_to_bf16_tensor(X)
+        binding.wf_switch_round(ctx, dA.gpu, dD.gpu, Xg, H.i32(q_indptr), H.i32(n_rows), None, H.i32(route), cur, nq, 8, 16, S, 16,
+                                switched=switched)
+        h_out = torch.full((S, 1, hid), 7.0, dtype=torch.bfloat16, device="cuda")
+        binding.wf_final_token_full(ctx, dA.gpu, Xg, H.i32(q_indptr), H.i32(n_rows), switched, binding.ROUTE_AR, S, h_out, ws)
+        torch.cuda.synchronize()
+        sel = (cur_o != binding.ROUTE_AR) & (route == binding.ROUTE_AR)
+        np.testing.assert_array_equal(switched.cpu().numpy(), np.where(route != cur_o, route, -1))
+        cur_o, _, _ = lazy_catchup.switch_round(lz, X, q_indptr, n_rows, route, cur_o, {0: 16, 1: 8})
+        want = final_token.final_tokens_full(dA.oracle, dA.full, X, q_indptr, n_rows, sel)
+        n_final += len(want)
+        _compare(H.bf16_f64(H.bf16_tensor_to_bits(h_out)), want, S, f"round {rnd}")
+        dA.kvp.assert_tables_equal()
+    assert n_final >= 4
+    assert ctx.poll_status() == 0
+    dA.close()
+    dD.close()
