@@ -398,7 +398,8 @@ def measure(ctx, wf, key, args, rank, world, local, main):
 
     # ---- timed region: K whole rounds, device-resident inputs, CUDA events on the launching stream ----
     evs = [{"attn": (torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)),
-            "catchup": (torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))} for _ in range(K)]
+            "catchup": (torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)),
+            "final": (torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))} for _ in range(K)]
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     attn_bytes = []
     len_host = rs.seq_len.cpu().numpy().astype(np.int64)     # the plan tells us how contexts grow
@@ -422,6 +423,7 @@ def measure(ctx, wf, key, args, rank, world, local, main):
     # per-round spans from the per-part events (attention start of round i to attention start of round i+1)
     spans = [evs[i]["attn"][0].elapsed_time(evs[i + 1]["attn"][0]) for i in range(K - 1)]
     catch_ms = sum(e["catchup"][0].elapsed_time(e["catchup"][1]) for e in evs)
+    final_ms = sum(e["final"][0].elapsed_time(e["final"][1]) for e in evs)
     commits = float(np.mean([np.sum(sl.u + 1) for sl in rs.slots]))
     flips = float(np.mean([np.mean(sl.cur != sl.next) for sl in rs.slots]))
 
@@ -484,9 +486,36 @@ def measure(ctx, wf, key, args, rank, world, local, main):
     rs.check_plan(rs.slots[(rs.rounds_done - 1) % rs.n_slots], switched=False)
     rs.sync_cur()
     lazy_us, eager_us, active_us = 1e3 * catch_ms / K, 1e3 * eager_catch_ms / leg_steps, 1e3 * active_catch_ms / leg_steps
+    final_us = 1e3 * final_ms / K
     round_us = 1e3 * ms_local / K
 
+    # ---- (f3) the final backlog token in full, on its own: back-to-back calls for the sequences slot `s` switches to the
+    #      AR drafter, and for the whole batch (the weights of the layer are streamed once per call either way) ----
+    ft_rec = None
+    if rs.ft is not None:
+        ft_rec = {"weight_bytes": rs.ft.weight_bytes, "ffn": rs.ft.ffn, "layers": rs.drafters["A"].n_layers}
+        sel_sw = s.masks["A"].flush
+        for tag, sel, n_tok in (("switching", sel_sw, int(s.masks["A"].flush_host.sum())), ("whole_batch", None, B)):
+            for _ in range(3):
+                rs.run_final_token(s, sel, 1)
+            t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            t0.record()
+            for _ in range(20):
+                rs.run_final_token(s, sel, 1)
+            t1.record()
+            torch.cuda.synchronize()
+            us = 1e3 * t0.elapsed_time(t1) / 20
+            ft_rec[tag] = {"tokens": n_tok, "us_per_call": us, "weight_gbs": rs.ft.weight_bytes / (us * 1e-6) / 1e9 if n_tok else None}
+
     peak, peak_src = measured_peaks()
+    if ft_rec:
+        for tag in ("switching", "whole_batch"):
+            g_ = ft_rec[tag]["weight_gbs"]
+            ft_rec[tag]["frac_of_hbm_peak"] = g_ / peak if g_ else None
+        ft_rec["note"] = ("wf_final_token_full for the AR drafter (one transformer layer, PAPER.md:231): Q/O/up/down weight streams "
+                          "(bytes = weight_bytes) + one-row attention over the drafter cache; 'switching' = the sequences the "
+                          "last timed slot switches to the AR drafter, 'whole_batch' = every sequence; back-to-back calls")
     avg_launch_ms = attn_ms / (K * L)
     achieved = float(np.mean(attn_bytes)) / (avg_launch_ms * 1e-3) / 1e9
     traffic, traffic_src = NCU_TRAFFIC.get(key, (None, None))
@@ -498,19 +527,23 @@ def measure(ctx, wf, key, args, rank, world, local, main):
         "config": config_dict(wl, world),
         "run_notes": {"slots": rs.n_slots, "realised_switch_rate": flips,
                       "l2": f"inputs larger than L2: {np.mean(attn_bytes) / 1e6:.0f} MB of KV per attention launch, distinct per layer",
-                      "catchup": "lazy: one wf_switch_round per round (both drafters, masks derived on the device from route)"},
+                      "catchup": "lazy: one wf_switch_round per round (both drafters, masks derived on the device from route), then "
+                                 "wf_final_token_full for the sequences that switched to the AR drafter"},
         "committed_tokens_per_s": world * commits * K / (ms * 1e-3),
         "kv_read_gbs": achieved,
         "attn_share_of_round": attn_ms / ms_local,
         "catchup_us_per_round": lazy_us,
         "catchup_share_of_round": catch_ms / ms_local,
         "catchup": {"lazy_us_per_round": lazy_us, "eager_us_per_round": eager_us, "active_append_us_per_round": active_us,
+                    "final_token_us_per_round": final_us, "flush_us_per_round": lazy_us - final_us,
                     "switch_us_per_round": lazy_us - active_us, "share_of_round": lazy_us / round_us,
                     "switch_share_of_round": (lazy_us - active_us) / round_us, "eager_share_of_round": eager_catch_ms / eager_ms,
                     "eager_rounds_per_s": leg_steps / (eager_ms * 1e-3), "leg_steps": leg_steps,
                     "note": "lazy = wf_switch_round inside the timed rounds; eager = KV-only prefill into both drafters every round "
                             "(Lazy Catch-up off, PAPER.md Table 3 baseline); active_append = only the active drafter's own append "
-                            "(reading C22: drafting cost, not switching cost); switch = lazy - active_append (derived)"},
+                            "(reading C22: drafting cost, not switching cost); switch = lazy - active_append (derived); "
+                            "final_token = wf_final_token_full for the sequences that switched to the AR drafter (PAPER.md:119), "
+                            "inside lazy and eager alike; flush = lazy - final_token"},
         "roofline": {"bound": "hbm", "kernel": "wf_verify_attn_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
                      "frac": achieved / peak, "peak_source": peak_src, "traffic": traffic, "traffic_source": traffic_src,
                      "algorithmic_bytes_per_launch": float(np.mean(attn_bytes)), "avg_launch_us": 1e3 * avg_launch_ms},
@@ -520,6 +553,8 @@ def measure(ctx, wf, key, args, rank, world, local, main):
         "gpu_launches": int(launches),
         "clocks": clocks,
     }
+    if ft_rec:
+        rec["final_token"] = ft_rec
     if cpu_baseline:
         rec["cpu_baseline"] = cpu_baseline
         rec["parity_sample"] = parity
@@ -666,7 +701,7 @@ def run_ours(args):
     for key in [k for k in args.sub_workloads.split(",") if k and k != args.workload]:
         torch.cuda.empty_cache()
         sub = measure(ctx, wf, key, args, rank, world, local, main=False)
-        keep = ("value", "unit", "steps", "ms_per_step", "kv_read_gbs", "attn_share_of_round", "catchup", "roofline", "e2e",
+        keep = ("value", "unit", "steps", "ms_per_step", "kv_read_gbs", "attn_share_of_round", "catchup", "final_token", "roofline", "e2e",
                 "clocks", "cpu_baseline", "parity_sample", "committed_tokens_per_s", "gpu_launches")
         per_config[key] = {k: sub[k] for k in keep if k in sub}
         per_config[key]["workload"] = sub["config"]["workload"]

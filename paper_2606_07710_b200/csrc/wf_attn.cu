@@ -51,11 +51,13 @@ struct AttnParams {
   const unsigned long long* tree_mask; // TREE only: [sum_q] ancestor mask of each row (bit j = node j of its sequence)
   KvView kv;
   int layer, B, n_q_heads, group;
+  int cl;                              // > 0: cluster mode (launched with clusters of `cl` CTAs, one cluster per (b, g) pair)
   int ctx_adj;                         // added to seq_len: 0 for verification (the block sits behind the cache length, C10);
                                        // -1 for the final-token path (wf_final.cu: the token is the last cached one, F1)
   float scale_log2;                    // sm_scale * log2(e)
   float4* ws_o;                        // [2 * CTAs][D/8][128 threads] float4: unnormalised O in fragment order
   float4* ws_ml;                       // [2 * CTAs][128 threads] (m, l) of the thread's two rows (m in log2 units)
+  int* tiles_hint;                     // mapped host memory: total tiles of this launch (read by the host before a later launch)
   unsigned int* counters;              // [B * Hkv] arrived | published << 16, self-resetting
   int* status;                         // sticky device status word
 };
@@ -92,6 +94,7 @@ struct AttnShared {
   int ctx[AT_MAX_B];                   // seq_len
   int meta[TREE ? AT_MAX_B : 1];       // TREE: nodes in the sub-block | nodes of the tree << 7 | first node << 14 | sequence << 21
   int total_tiles, g_eff, B;
+  int cl;                              // cluster mode: CTAs per (b, g) pair (0 = stream-K ranges)
   uint32_t tmem;
   int last;
 };
@@ -117,6 +120,7 @@ struct SegWalker {
   int lo, hi, x, b;
   bool first = true;
   __device__ SegWalker(const AttnShared<TREE>& sh_, int Hkv_, int c_) : sh(sh_), Hkv(Hkv_), c(c_) {
+    if (sh.cl > 0) { lo = hi = x = b = 0; return; }          // cluster mode: next() derives the one segment of this CTA
     const int T = sh.total_tiles, G = sh.g_eff;
     lo = (int)((long long)c * T / G);
     hi = (int)((long long)(c + 1) * T / G);
@@ -129,6 +133,30 @@ struct SegWalker {
     b = l;
   }
   __device__ bool next(Segment& s) {
+    if (sh.cl > 0) {
+      // Cluster mode: cluster `pair` = (b, g) over ALL sequences of the call (an empty one idles its cluster); CTA rank r of
+      // the cluster owns tiles [r * nt / cl, (r + 1) * nt / cl) of the pair: pair-aligned, equal shares, one segment.
+      if (!first) return false;
+      first = false;
+      const int pair = c / sh.cl, rank = c % sh.cl;
+      const int bb = pair / Hkv;
+      if (bb >= sh.B) return false;
+      const int nt = sh.pref[bb + 1] - sh.pref[bb] - AT_SEG_COST;
+      if (nt <= 0) return false;
+      const int t_lo = (int)((long long)rank * nt / sh.cl), t_hi = (int)((long long)(rank + 1) * nt / sh.cl);
+      if (t_hi <= t_lo) return false;
+      s.b = bb; s.pb = bb; s.nt = nt; s.g = pair % Hkv; s.t_lo = t_lo; s.t_hi = t_hi;
+      s.flat0 = 0;
+      s.r0 = sh.r0[bb];
+      s.ctx = sh.ctx[bb];
+      s.q_b = sh.r0[bb + 1] - s.r0;
+      s.k0 = t_lo * AT_BN;
+      s.k1 = min(s.ctx + s.q_b, t_hi * AT_BN);
+      s.n_tiles = t_hi - t_lo;
+      s.partial = 1;
+      s.slot = 0;
+      return true;
+    }
     while (x < hi) {
       while (x >= Hkv * sh.pref[b + 1]) ++b;                   // also skips empty sequences
       const int wlen = sh.pref[b + 1] - sh.pref[b], nt = wlen - AT_SEG_COST;
@@ -302,12 +330,79 @@ __device__ __forceinline__ void tmem_ld_frag(uint32_t taddr, uint32_t (&v)[N]) {
   if constexpr (N == 64) tmem_ld_16x256b_x16(taddr, v); else tmem_ld_16x256b_x8(taddr, v);
 }
 
+// ---- thread-block cluster helpers (cluster mode) ----
+__device__ __forceinline__ void cluster_sync_all() {           // every thread of every CTA of the cluster
+  asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
+  asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+__device__ __forceinline__ uint32_t mapa_u32(uint32_t addr, uint32_t rank) {   // my shared address -> the same offset in CTA `rank`
+  uint32_t r;
+  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(addr), "r"(rank));
+  return r;
+}
+__device__ __forceinline__ float4 ld_dsmem_f4(uint32_t addr) {
+  float4 v;
+  asm volatile("ld.shared::cluster.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr) : "memory");
+  return v;
+}
+__device__ __forceinline__ float2 ld_dsmem_f2(uint32_t addr) {
+  float2 v;
+  asm volatile("ld.shared::cluster.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(addr) : "memory");
+  return v;
+}
+
+// Cluster mode, after the first cluster barrier: the CTA of rank r folds rows [r * 64 / cl, (r + 1) * 64 / cl) of the pair out
+// of the partials in the shared memory of all cl CTAs, in rank order (the bits do not depend on timing), normalises and
+// stores them.  All loads of a position are issued before the first is consumed (one DSMEM round trip).
+template <int D>
+__device__ __forceinline__ void attn_cluster_merge(const AttnParams& p, const AttnShared<false>& sh, uint8_t* part_s, int tid256) {
+  constexpr int MAXCL = 16;
+  const int cl = sh.cl, pair = (int)blockIdx.x / cl, rank = (int)blockIdx.x % cl;
+  const int Hkv = p.kv.n_kv_heads, b = pair / Hkv, g = pair % Hkv;
+  if (b >= sh.B) return;
+  const int r0 = sh.r0[b], R = (sh.r0[b + 1] - r0) * p.group;
+  const int rpr = AT_ROWS / cl;                               // rows per rank
+  const uint32_t base = smem_u32(part_s);
+  constexpr uint32_t ML_OFF = AT_ROWS * (D + 8) * 4;
+  for (int idx = tid256; idx < rpr * (D / 4); idx += 256) {
+    const int row = rank * rpr + idx / (D / 4), c4 = idx % (D / 4);
+    if (row >= R) continue;
+    float2 ml[MAXCL];
+    float4 ov[MAXCL];
+#pragma unroll
+    for (int s2 = 0; s2 < MAXCL; ++s2)
+      if (s2 < cl) {
+        const uint32_t rb = mapa_u32(base, (uint32_t)s2);
+        ml[s2] = ld_dsmem_f2(rb + ML_OFF + row * 8);
+        ov[s2] = ld_dsmem_f4(rb + (uint32_t)(row * (D + 8) + c4 * 4) * 4);
+      }
+    float m = -INFINITY;
+#pragma unroll
+    for (int s2 = 0; s2 < MAXCL; ++s2)
+      if (s2 < cl) m = fmaxf(m, ml[s2].x);
+    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+    float l = 0.f;
+#pragma unroll
+    for (int s2 = 0; s2 < MAXCL; ++s2)
+      if (s2 < cl && ml[s2].y > 0.f) {                         // a CTA without tiles (or without a visible key) holds l = 0
+        const float w = fast_exp2(ml[s2].x - m);
+        l = fmaf(w, ml[s2].y, l);
+        acc.x = fmaf(w, ov[s2].x, acc.x); acc.y = fmaf(w, ov[s2].y, acc.y);
+        acc.z = fmaf(w, ov[s2].z, acc.z); acc.w = fmaf(w, ov[s2].w, acc.w);
+      }
+    const float inv = 1.f / l;                                 // every row sees key 0: l > 0
+    const int qi = row / p.group, hg = row % p.group;
+    __nv_bfloat16* dst = p.out + ((size_t)(r0 + qi) * p.n_q_heads + g * p.group + hg) * D + c4 * 4;
+    *reinterpret_cast<uint2*>(dst) = make_uint2(pack_bf16(acc.x * inv, acc.y * inv), pack_bf16(acc.z * inv, acc.w * inv));
+  }
+}
+
 // ================= warps 0-3 (group 0) and 4-7 (group 1): softmax, O accumulation, output, merges =================
 // The two groups ping-pong over the tiles: group g takes the tiles whose global counter has parity g and
 // keeps its own running (m, l, O); at the end of a segment group 1 hands its state to group 0 through smem.
 template <int D>
 __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared<false>& sh, uint8_t* q_s, uint8_t* p0_s, uint8_t* p1_s,
-                                             uint8_t* v_s, uint32_t tmem_base, int warp, int lane) {
+                                             uint8_t* v_s, uint8_t* part_s, uint32_t tmem_base, int warp, int lane) {
   using C = AttnCfg<D, false>;
   constexpr int NO = D / 2;                                    // O registers per thread (2 rows x D/4 columns)
   const int Hkv = p.kv.n_kv_heads;
@@ -480,7 +575,7 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared<fal
     // round trip overlaps the group merge below.  Arriving only decides who merges, it publishes nothing.
     int c_first = 0, n_seg = 1;
     unsigned int arrive_old = 0;
-    if (sg.partial && grp == 0) {
+    if (sg.partial && grp == 0 && sh.cl == 0) {
       c_first = cta_of_tile(sg.flat0 + AT_SEG_COST, T, G);
       n_seg = cta_of_tile(sg.flat0 + AT_SEG_COST + sg.nt - 1, T, G) - c_first + 1;
       if (stid == 0) arrive_old = atomicAdd(&p.counters[sg.pb * Hkv + sg.g], 1u);
@@ -519,6 +614,21 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared<fal
     for (int h = 0; h < 2; ++h) {
       l_run[h] += __shfl_xor_sync(0xffffffffu, l_run[h], 1);
       l_run[h] += __shfl_xor_sync(0xffffffffu, l_run[h], 2);
+    }
+    if (sh.cl > 0) {
+      // Cluster mode: the partial (m, l, unnormalised O) of this CTA goes to its OWN shared memory (the K ring is idle: every
+      // MMA has retired); after the cluster barrier every CTA of the pair folds one slice of the rows out of all the
+      // CTAs' partials through distributed shared memory (attn_cluster_merge).  Nothing touches global memory.
+      float* po = reinterpret_cast<float*>(part_s);
+      float2* pml = reinterpret_cast<float2*>(part_s + AT_ROWS * (D + 8) * 4);
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        float* prow = po + (row_lo + 8 * h) * (D + 8) + cq;
+#pragma unroll
+        for (int j = 0; j < D / 8; ++j) *reinterpret_cast<float2*>(prow + 8 * j) = make_float2(o[4 * j + 2 * h], o[4 * j + 2 * h + 1]);
+        if ((lane & 3) == 0) pml[row_lo + 8 * h] = make_float2(m_run[h], l_run[h]);
+      }
+      continue;
     }
     auto write_rows = [&]() {                                  // normalise and store this thread's two rows
 #pragma unroll
@@ -631,6 +741,15 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared<fal
       }
     }
     write_rows();
+  }
+  if (sh.cl > 0) {
+    // cluster mode: a CTA without tiles publishes an empty partial (l = 0), then barrier, fold of this CTA's rows, barrier
+    // (nobody leaves while a peer may still read its shared memory)
+    if (gt0 == 0 && grp == 0 && stid < AT_ROWS)
+      reinterpret_cast<float2*>(part_s + AT_ROWS * (D + 8) * 4)[stid] = make_float2(-INFINITY, 0.f);
+    cluster_sync_all();
+    attn_cluster_merge<D>(p, sh, part_s, grp * 128 + stid);
+    cluster_sync_all();
   }
 }
 
@@ -1018,17 +1137,20 @@ __global__ void __launch_bounds__(AT_THREADS, 1) wf_verify_attn_kernel(const Att
         n = max(1, min(n, G / pairs));
         G = min(G, n * pairs);
       }
-      sh.g_eff = max(1, min(G, total / min_range));
+      sh.g_eff = p.cl > 0 ? (int)gridDim.x : max(1, min(G, total / min_range));
       sh.B = n_tab;
+      sh.cl = TREE ? 0 : p.cl;
+      if (blockIdx.x == 0 && p.tiles_hint) *p.tiles_hint = total;      // feedback for the host's next choice of launch shape
     }
   }
   __syncthreads();
 
-  if (sh.total_tiles > 0 && (int)blockIdx.x < sh.g_eff) {
+  const bool run = sh.total_tiles > 0 && (int)blockIdx.x < sh.g_eff;
+  if (run) {
     if (warp < 8) {
       asm volatile("setmaxnreg.inc.sync.aligned.u32 216;");
       if constexpr (TREE) attn_softmax_tree<D>(p, sh, q_s, p0_s, v_s, tmem_base, warp, lane);
-      else attn_softmax<D>(p, sh, q_s, p0_s, p1_s, v_s, tmem_base, warp, lane);
+      else attn_softmax<D>(p, sh, q_s, p0_s, p1_s, v_s, k_s, tmem_base, warp, lane);
     } else {
       asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
       if (warp == 8) attn_loader<D, TREE>(p, sh, k_s, 0, lane);
@@ -1036,6 +1158,10 @@ __global__ void __launch_bounds__(AT_THREADS, 1) wf_verify_attn_kernel(const Att
       else if (warp == 9) attn_mma_qk<D, TREE>(p, sh, q_s, k_s, tmem_base);
       else if (warp == 11) attn_mma_pv<D, TREE>(p, sh, p0_s, p1_s, v_s, tmem_base);
     }
+  }
+  if constexpr (!TREE) {
+    // cluster mode: the softmax warps of a running CTA take the two cluster barriers inside attn_softmax; everybody else here
+    if (sh.cl > 0 && !(run && warp < 8)) { cluster_sync_all(); cluster_sync_all(); }
   }
   tc_fence_before();
   __syncthreads();

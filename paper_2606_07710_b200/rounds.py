@@ -38,7 +38,7 @@ class Slot:
 
 class RoundState:
     def __init__(self, ctx, wl: synth.Workload, n_slots=16, n_rounds_max=64, device="cuda", layers=None,
-                 host_copies=False):
+                 host_copies=False, final_token=True):
         import torch
         self.torch, self.ctx, self.wl, self.device = torch, ctx, wl, device
         sh = wl.shapes
@@ -112,8 +112,30 @@ class RoundState:
         self.nr.delta_al = torch.zeros(B, dtype=torch.float32, device=device)
         self.nr.route = torch.zeros(B, dtype=torch.int32, device=device)
         self.nr.ws = torch.empty(wf.wf_neural_route_workspace_bytes(B, m), dtype=torch.uint8, device=device)
+        # ---- (f3) the final backlog token in full, for the AR drafter (the drafter whose catch-up the paper profiles,
+        #      PAPER.md:206; a single transformer layer): W_Q, W_O and a two-matrix MLP of width `ffn` ----
+        self.switched = torch.full((B,), -1, dtype=torch.int32, device=device)
+        self.ft = None
+        if final_token:
+            ft = Slot()
+            dA = self.drafters["A"]
+            qd, ffn = sh.n_q_heads * sh.head_dim, sh.ffn
+            ft.ffn = ffn
+            mk = lambda shape, stream: [synth.device_normal_bf16(shape, 0.02, wl.seed, stream + l, device) for l in range(dA.n_layers)]
+            ws_ = (mk((sh.hidden, qd), 70), mk((qd, sh.hidden), 75), mk((sh.hidden, ffn), 80), mk((ffn, sh.hidden), 85))
+            dA.handle.set_full_layer(sh.n_q_heads, ffn, min(B, 256), *ws_)       # the library keeps its own repacked copy
+            del ws_
+            ft.weight_bytes = dA.n_layers * 2 * (2 * sh.hidden * qd + 2 * sh.hidden * ffn)
+            ft.h_out = torch.zeros((B, dA.n_layers, sh.hidden), dtype=torch.bfloat16, device=device)
+            ft.ws = torch.empty(wf.wf_final_token_workspace_bytes(dA.handle, B), dtype=torch.uint8, device=device)
+            self.ft = ft
         self.rounds_done = 0
         torch.cuda.synchronize()
+
+    def run_final_token(self, s, select, code, stream=None):
+        """(f3) the last committed row of every selected sequence through the AR drafter's layer in full."""
+        wf.wf_final_token_full(self.ctx, self.drafters["A"].handle, s.hidden, s.q_indptr, self.out["n_commit"], select, code,
+                               self.B, self.ft.h_out, self.ft.ws, stream)
 
     # ------------------------------------------------------------------------------------------
     def _make_drafter(self, name, n_layers, grow, g):
@@ -222,7 +244,7 @@ class RoundState:
         """cur_drafter <- the plan's value for the next round to run (after legs that do not drive the switch)."""
         self.cur_drafter.copy_(_i32(self.slots[self.rounds_done % self.n_slots].cur, self.device))
 
-    def run_catchup(self, s, stream=None, lazy=True, fused=True, mode=None):
+    def run_catchup(self, s, stream=None, lazy=True, fused=True, mode=None, events=None):
         """Drafter-cache maintenance after the accept.
         mode "switch" (default): ONE wf_switch_round for both drafters, masks derived on the device from route and
              cur_drafter (the paper's scheme: Lazy Catch-up + KV-only prefill at the switch);
@@ -237,7 +259,13 @@ class RoundState:
         if mode == "switch":
             wf.wf_switch_round(self.ctx, self.drafters["A"].handle, self.drafters["D"].handle, s.hidden, s.q_indptr, n_commit,
                                None, self.out["route"], self.cur_drafter, self.next_q_len, self.q_len_of[wf.ROUTE_AR],
-                               self.q_len_of[wf.ROUTE_DIFFUSION], B, self.qmax, stream)
+                               self.q_len_of[wf.ROUTE_DIFFUSION], B, self.qmax, stream, switched=self.switched)
+            if self.ft is not None:                            # the switch as the paper defines it ends with the final token
+                if events:
+                    events["final"][0].record()
+                self.run_final_token(s, self.switched, wf.ROUTE_AR, stream)
+                if events:
+                    events["final"][1].record()
             return
         for name, d in self.drafters.items():
             m = s.masks[name]
@@ -259,6 +287,8 @@ class RoundState:
                     wf.wf_lazy_catchup_flush(self.ctx, d.handle, m.flush, B, stream)
             else:
                 wf.wf_kv_only_prefill(self.ctx, d.handle, s.hidden, s.q_indptr, n_commit, None, B, self.qmax, stream)
+        if self.ft is not None and mode != "active" and s.masks["A"].flush_host.any():
+            self.run_final_token(s, s.masks["A"].flush, 1, stream)
 
     def run_round(self, stream=None, lazy=True, events=None, fused=True, mode=None):
         """One whole round.  events: optional dict of (start, end) CUDA event pairs to record around parts."""
@@ -272,7 +302,7 @@ class RoundState:
         self.run_accept(s, stream)
         if events:
             events["catchup"][0].record()
-        self.run_catchup(s, stream, lazy, fused, mode)
+        self.run_catchup(s, stream, lazy, fused, mode, events if events and "final" in events else None)
         if events:
             events["catchup"][1].record()
         self.rounds_done += 1

@@ -42,6 +42,11 @@ class Shapes:
     def group(self):
         return self.n_q_heads // self.n_kv_heads
 
+    @property
+    def ffn(self):
+        """MLP width of the drafter layer of the final-token path (reading F5): 3 x hidden (12288 at 8B-class shapes)."""
+        return 3 * self.hidden
+
 
 TINY = Shapes("tiny", hidden=256, n_q_heads=4, n_kv_heads=2, head_dim=64, n_layers=1,
               vocab=4096, logit_sigma=2.0, drafter_layers=(1,))
