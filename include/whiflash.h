@@ -97,6 +97,12 @@ int wf_verify_attn(wf_ctx* ctx, const wf_paged_kv* target_kv, int layer,
                    const void* q, const int32_t* q_indptr, int B, int n_q_heads, int max_q_len,
                    float sm_scale, void* out, void* workspace, size_t workspace_bytes, void* stream);
 size_t wf_verify_attn_workspace_bytes(const wf_kv_shape* shape, int B, int n_q_heads, int max_q_len);
+/* Launch shape of wf_verify_attn (a tuning / test hook; results are within tolerance of one another, not bit-equal).
+ * -1 (default): automatic: with few (sequence, kv head) pairs (batch 1-2 at 8 kv heads) one thread-block cluster per pair,
+ * partials folded through distributed shared memory in a fixed order (bit-reproducible); otherwise, and whenever the
+ * last launch over the same cache was long enough to be HBM-paced, persistent stream-K ranges over all SMs.
+ * 0: never use clusters.  2..16: force that cluster size whenever the pairs fit (else stream-K). */
+int wf_ctx_set_attn_cluster(wf_ctx* ctx, int cluster_size);
 
 /* ---- (b) accept + bonus + entropy + route -------------------------------------------------------
  * PAPER.md:65, 75-81 (§3.3.1), 135; readings C1-C9.  Per sequence b (block rows r0..r0+gamma):

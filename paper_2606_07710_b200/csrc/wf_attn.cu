@@ -32,13 +32,22 @@
 #include "wf_internal.cuh"
 #include "wf_sm100.cuh"
 
+// Timeline probes (clock64 per CTA; compiled in only with -DWF_PROBE): slot k of CTA c.
+#ifdef WF_PROBE
+__device__ long long* wf_probe_buf = nullptr;
+#define WF_PROBE_AT(k, cond) do { if (wf_probe_buf && (cond)) wf_probe_buf[blockIdx.x * 32 + (k)] = clock64(); } while (0)
+extern "C" int wf_debug_set_attn_probe(long long* buf) { return (int)cudaMemcpyToSymbol(wf_probe_buf, &buf, sizeof(buf)); }
+#else
+#define WF_PROBE_AT(k, cond) do { } while (0)
+#endif
+
 namespace {
 
 constexpr int AT_THREADS = 384;           // 12 warps: 0-3 / 4-7 softmax groups, 8 K loader, 9 QK^T issuer, 10 V loader, 11 PV issuer
 constexpr int AT_BN = 128;             // keys per tile
 constexpr int AT_ROWS = 64;            // query rows = UMMA M
 constexpr int AT_MAX_B = 1024;
-constexpr int AT_MAX_STAGES = 4;
+constexpr int AT_MAX_STAGES = 5;
 constexpr int AT_MAX_CTAS = 160;       // workspace is sized for this many persistent CTAs
 constexpr int AT_MAX_SEG = 32;         // partials merged per (b, g) pair
 constexpr int AT_SEG_COST = 4;         // fixed cost of a segment (Q load, pipeline restart, merge, stores) in tiles
@@ -82,6 +91,14 @@ struct AttnCfg {
   static constexpr uint32_t TM_S = 0, TM_O = 2 * AT_BN;     // TMEM columns: S0, S1, then O0, O1
 };
 
+struct Segment {
+  int b, g, t_lo, t_hi, nt;            // tiles [t_lo, t_hi) of the pair's nt tiles; b = sequence (block table row)
+  int pb;                              // table index of the pair (TREE: the sub-block; else b): merge counter
+  int r0, q_b, ctx, k0, k1, n_tiles;   // r0 / q_b: first query row and rows/group of this tile (TREE: of the sub-block)
+  int partial, slot;                   // partial: the pair is shared with other CTAs; slot = 2c + (0 head | 1 tail)
+  int flat0;                           // weighted position of the pair (its tile t sits at flat0 + AT_SEG_COST + t)
+};
+
 // shared state of one CTA (static smem).  TREE: the table is indexed by SUB-BLOCK (a sequence's tree of up to 64
 // nodes is cut into sub-blocks of 64 / group nodes = one 64-row query tile each), see the kernel prologue.
 template <bool TREE>
@@ -95,17 +112,19 @@ struct AttnShared {
   int meta[TREE ? AT_MAX_B : 1];       // TREE: nodes in the sub-block | nodes of the tree << 7 | first node << 14 | sequence << 21
   int total_tiles, g_eff, B;
   int cl;                              // cluster mode: CTAs per (b, g) pair (0 = stream-K ranges)
+  int cl_b;                            // cluster mode: the sequence of this CTA's pair (its table entry is index 0)
+  Segment seg;                         // cluster mode: this CTA's one segment (n_tiles = 0: none), derived once in the prologue
+  int n_stk, n_stv;                    // K / V ring depths
+  uint64_t k_done;                     // cluster mode: this CTA's last QK^T has retired: its K ring is free to receive
+  uint64_t cl_ready;                   // cluster mode: every CTA of the cluster can receive (cl arrivals)
+  uint64_t cl_bar;                     // cluster mode: completes when every CTA of the pair has pushed its slice for this CTA's rows
+  float2 cl_ml[AT_ROWS + 16];          // cluster mode: received (m, l), [sender][row of this CTA's slice]
+  int cl_rb[17];                       // cluster mode: rank o owns rows [cl_rb[o], cl_rb[o + 1]) of the pair's live rows
+  int cl_dst[AT_ROWS];                 // cluster mode: row -> owner rank | element offset of the row in `out` << 5
   uint32_t tmem;
   int last;
 };
 
-struct Segment {
-  int b, g, t_lo, t_hi, nt;            // tiles [t_lo, t_hi) of the pair's nt tiles; b = sequence (block table row)
-  int pb;                              // table index of the pair (TREE: the sub-block; else b): merge counter
-  int r0, q_b, ctx, k0, k1, n_tiles;   // r0 / q_b: first query row and rows/group of this tile (TREE: of the sub-block)
-  int partial, slot;                   // partial: the pair is shared with other CTAs; slot = 2c + (0 head | 1 tail)
-  int flat0;                           // weighted position of the pair (its tile t sits at flat0 + AT_SEG_COST + t)
-};
 
 // Walks the range of one CTA over the flattened, WEIGHTED (b, g, tile) list; every role keeps its own walker.
 // A pair of nt tiles occupies AT_SEG_COST + nt positions: the first AT_SEG_COST stand for the fixed cost of a
@@ -134,27 +153,11 @@ struct SegWalker {
   }
   __device__ bool next(Segment& s) {
     if (sh.cl > 0) {
-      // Cluster mode: cluster `pair` = (b, g) over ALL sequences of the call (an empty one idles its cluster); CTA rank r of
-      // the cluster owns tiles [r * nt / cl, (r + 1) * nt / cl) of the pair: pair-aligned, equal shares, one segment.
-      if (!first) return false;
+      // Cluster mode: the one segment of this CTA was derived in the prologue (thread 0: a walk costs 1.2k cycles of
+      // integer divisions, measured, and every role would repeat it on the critical path of a batch-1 launch)
+      if (!first || sh.seg.n_tiles <= 0) return false;
       first = false;
-      const int pair = c / sh.cl, rank = c % sh.cl;
-      const int bb = pair / Hkv;
-      if (bb >= sh.B) return false;
-      const int nt = sh.pref[bb + 1] - sh.pref[bb] - AT_SEG_COST;
-      if (nt <= 0) return false;
-      const int t_lo = (int)((long long)rank * nt / sh.cl), t_hi = (int)((long long)(rank + 1) * nt / sh.cl);
-      if (t_hi <= t_lo) return false;
-      s.b = bb; s.pb = bb; s.nt = nt; s.g = pair % Hkv; s.t_lo = t_lo; s.t_hi = t_hi;
-      s.flat0 = 0;
-      s.r0 = sh.r0[bb];
-      s.ctx = sh.ctx[bb];
-      s.q_b = sh.r0[bb + 1] - s.r0;
-      s.k0 = t_lo * AT_BN;
-      s.k1 = min(s.ctx + s.q_b, t_hi * AT_BN);
-      s.n_tiles = t_hi - t_lo;
-      s.partial = 1;
-      s.slot = 0;
+      s = sh.seg;
       return true;
     }
     while (x < hi) {
@@ -221,7 +224,7 @@ __device__ __forceinline__ void attn_loader(const AttnParams& p, AttnShared<TREE
     // critical path.  Lane q holds page q of the tile.
     int page_next = lane < min(PP, pages_seg) ? __ldg(bt + lane) : 0;
     for (int t = 0; t < sg.n_tiles; ++t, ++gt) {
-      const int n_st = which ? C::STAGES_V : C::STAGES_K;
+      const int n_st = which ? sh.n_stv : sh.n_stk;
       const int st = gt % n_st;
       const int npages = min(PP, pages_seg - t * PP);
       const int row = (((p.layer * kv.num_pages + page_next) * kv.n_kv_heads) + sg.g) * 16;
@@ -256,6 +259,8 @@ __device__ __forceinline__ void attn_loader(const AttnParams& p, AttnShared<TREE
 // are built once and advanced by constant offsets.  Hazards are carried by the barriers alone: QK^T(g2) needs
 // K(g2) and S[g2&1] read out by the softmax of tile g2 - 2 (s_empty); PV(g2) needs V(g2), P(g2) (p_full) and
 // O[g2&1] folded (o_empty).  tcgen05.commit covers the MMAs of the committing thread, i.e. exactly its batch.
+__device__ __forceinline__ uint32_t mapa_u32(uint32_t addr, uint32_t rank);
+
 template <int D, bool TREE>
 __device__ __forceinline__ void attn_mma_qk(const AttnParams& p, AttnShared<TREE>& sh, uint8_t* q_s, uint8_t* k_s,
                                             uint32_t tmem_base) {
@@ -270,8 +275,10 @@ __device__ __forceinline__ void attn_mma_qk(const AttnParams& p, AttnShared<TREE
     mbar_wait(smem_u32(&sh.q_ready), n_seg & 1);
     ++n_seg;
     for (int t = 0; t < sg.n_tiles; ++t, ++gt) {
-      const int st = gt % C::STAGES_K;
-      mbar_wait(smem_u32(&sh.k_full[st]), (gt / C::STAGES_K) & 1);
+      const int n_stk = sh.n_stk;
+      const int st = gt % n_stk;
+      mbar_wait(smem_u32(&sh.k_full[st]), (gt / n_stk) & 1);
+      WF_PROBE_AT(12 + (gt < 3 ? (int)gt : 3), (threadIdx.x & 31) == 0 && gt < 3);
       mbar_wait(smem_u32(&sh.s_empty[gt & 1]), ((gt >> 1) & 1) ^ 1);
       tc_fence_after();
       if (elect_one()) {
@@ -285,6 +292,20 @@ __device__ __forceinline__ void attn_mma_qk(const AttnParams& p, AttnShared<TREE
         umma_commit(smem_u32(&sh.k_empty[st]));                // the K tile is free once QK^T has retired
       }
       __syncwarp();
+    }
+  }
+  if constexpr (!TREE) {
+    if (sh.cl > 0) {
+      // Cluster mode: once the last QK^T has retired this CTA's K ring is idle and becomes its receive buffer: tell every
+      // CTA of the cluster (they push their slices only when all are ready; in practice long before anybody is done)
+      if (gt > 0) {
+        if (elect_one()) umma_commit(smem_u32(&sh.k_done));
+        __syncwarp();
+        mbar_wait(smem_u32(&sh.k_done), 0);
+      }
+      const int lane = threadIdx.x & 31;
+      if (lane < sh.cl)
+        asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(mapa_u32(smem_u32(&sh.cl_ready), (uint32_t)lane)) : "memory");
     }
   }
 }
@@ -302,8 +323,8 @@ __device__ __forceinline__ void attn_mma_pv(const AttnParams& p, AttnShared<TREE
   uint32_t gt = 0;
   while (walk.next(sg)) {
     for (int t = 0; t < sg.n_tiles; ++t, ++gt) {
-      const int st = gt % C::STAGES_V, g = gt & 1;
-      mbar_wait(smem_u32(&sh.v_full[st]), (gt / C::STAGES_V) & 1);
+      const int st = gt % sh.n_stv, g = gt & 1;
+      mbar_wait(smem_u32(&sh.v_full[st]), (gt / sh.n_stv) & 1);
       if constexpr (TREE) mbar_wait(smem_u32(&sh.p_full[0]), gt & 1);       // one P buffer, one phase per tile
       else mbar_wait(smem_u32(&sh.p_full[g]), (gt >> 1) & 1);
       mbar_wait(smem_u32(&sh.o_empty[g]), ((gt >> 1) & 1) ^ 1);
@@ -331,50 +352,68 @@ __device__ __forceinline__ void tmem_ld_frag(uint32_t taddr, uint32_t (&v)[N]) {
 }
 
 // ---- thread-block cluster helpers (cluster mode) ----
-__device__ __forceinline__ void cluster_sync_all() {           // every thread of every CTA of the cluster
-  asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
-  asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
-}
 __device__ __forceinline__ uint32_t mapa_u32(uint32_t addr, uint32_t rank) {   // my shared address -> the same offset in CTA `rank`
   uint32_t r;
   asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(addr), "r"(rank));
   return r;
 }
-__device__ __forceinline__ float4 ld_dsmem_f4(uint32_t addr) {
-  float4 v;
-  asm volatile("ld.shared::cluster.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr) : "memory");
-  return v;
+__device__ __forceinline__ void cluster_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
+__device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
+// bulk copy own shared memory -> a peer CTA's shared memory, completing (bytes) on the PEER's mbarrier
+__device__ __forceinline__ void bulk_push_dsmem(uint32_t dst_cluster, uint32_t src_cta, uint32_t bytes, uint32_t bar_cluster) {
+  asm volatile("cp.async.bulk.shared::cluster.shared::cta.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(dst_cluster), "r"(src_cta), "r"(bytes), "r"(bar_cluster) : "memory");
 }
-__device__ __forceinline__ float2 ld_dsmem_f2(uint32_t addr) {
-  float2 v;
-  asm volatile("ld.shared::cluster.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(addr) : "memory");
-  return v;
+// 8-byte store into a peer CTA's shared memory, completing (8 bytes) on the PEER's mbarrier
+__device__ __forceinline__ void st_async_f2(uint32_t dst_cluster, float a, float b, uint32_t bar_cluster) {
+  asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v2.f32 [%0], {%1, %2}, [%3];"
+               ::"r"(dst_cluster), "f"(a), "f"(b), "r"(bar_cluster) : "memory");
 }
 
-// Cluster mode, after the first cluster barrier: the CTA of rank r folds rows [r * 64 / cl, (r + 1) * 64 / cl) of the pair out
-// of the partials in the shared memory of all cl CTAs, in rank order (the bits do not depend on timing), normalises and
-// stores them.  All loads of a position are issued before the first is consumed (one DSMEM round trip).
+// Cluster mode: how the R live rows of a pair are dealt to the cl CTAs of its cluster (rank o owns rows [a_o, b_o)).
+__device__ __forceinline__ int cl_row_begin(int o, int R, int cl) { return o * R / cl; }
+__device__ __forceinline__ int cl_row_owner(int r, int R, int cl) { return ((r + 1) * cl - 1) / R; }   // largest o with a_o <= r
+
+// Cluster mode, sender side (lane o of one warp serves owner o): the partial lies in this CTA's shared memory as
+// [64 rows][D fp32], 16-byte chunks XOR-swizzled with (row & 7); every owner gets its rows with ONE bulk copy through
+// distributed shared memory, into slot `rank` of its receive buffer, completing on ITS mbarrier.  Nothing crosses global
+// memory and nobody waits for anybody here.  (Measured alternatives: one thread walking the owners, 240 cycles per owner;
+// every thread storing its fragment straight into the owners' buffers with st.async, 4.0k cycles against 2.5k for this.)
 template <int D>
-__device__ __forceinline__ void attn_cluster_merge(const AttnParams& p, const AttnShared<false>& sh, uint8_t* part_s, int tid256) {
+__device__ __forceinline__ void attn_cluster_push(const AttnShared<false>& sh, uint8_t* part_s, uint8_t* recv_s, int lane) {
+  const int cl = sh.cl, rank = (int)blockIdx.x % cl;
+  if (lane < cl) {
+    const int a = sh.cl_rb[lane], n = sh.cl_rb[lane + 1] - a;
+    if (n > 0)
+      bulk_push_dsmem(mapa_u32(smem_u32(recv_s) + (uint32_t)(rank * n) * (D * 4), (uint32_t)lane), smem_u32(part_s) + (uint32_t)a * (D * 4),
+                      (uint32_t)n * (D * 4), mapa_u32(smem_u32(&sh.cl_bar), (uint32_t)lane));
+  }
+}
+// (m, l) of row r (thread-held) to the owner of the row
+__device__ __forceinline__ void attn_cluster_push_ml(const AttnShared<false>& sh, int r, float m, float l) {
+  const int rank = (int)blockIdx.x % sh.cl;
+  const int o = sh.cl_dst[r] & 31;
+  const int a = sh.cl_rb[o], n = sh.cl_rb[o + 1] - a;
+  st_async_f2(mapa_u32(smem_u32(&sh.cl_ml[rank * n + (r - a)]), (uint32_t)o), m, l, mapa_u32(smem_u32(&sh.cl_bar), (uint32_t)o));
+}
+
+// Cluster mode, receiver side (all 256 softmax threads, after cl_bar completed): fold this CTA's rows out of the cl received
+// slices in sender order (the bits do not depend on timing), normalise, store.  Local shared memory only.
+template <int D>
+__device__ __forceinline__ void attn_cluster_reduce(const AttnParams& p, const AttnShared<false>& sh, const uint8_t* recv_s, int tid256) {
   constexpr int MAXCL = 16;
-  const int cl = sh.cl, pair = (int)blockIdx.x / cl, rank = (int)blockIdx.x % cl;
-  const int Hkv = p.kv.n_kv_heads, b = pair / Hkv, g = pair % Hkv;
-  if (b >= sh.B) return;
-  const int r0 = sh.r0[b], R = (sh.r0[b + 1] - r0) * p.group;
-  const int rpr = AT_ROWS / cl;                               // rows per rank
-  const uint32_t base = smem_u32(part_s);
-  constexpr uint32_t ML_OFF = AT_ROWS * (D + 8) * 4;
-  for (int idx = tid256; idx < rpr * (D / 4); idx += 256) {
-    const int row = rank * rpr + idx / (D / 4), c4 = idx % (D / 4);
-    if (row >= R) continue;
+  const int cl = sh.cl, rank = (int)blockIdx.x % cl;
+  const int row_a = sh.cl_rb[rank], n = sh.cl_rb[rank + 1] - row_a;
+  for (int idx = tid256; idx < n * (D / 4); idx += 256) {
+    const int i = idx / (D / 4), c4 = idx % (D / 4), row = row_a + i;
+    const uint8_t* base = recv_s + (size_t)i * (D * 4) + ((c4 ^ (row & 7)) << 4);
     float2 ml[MAXCL];
     float4 ov[MAXCL];
 #pragma unroll
     for (int s2 = 0; s2 < MAXCL; ++s2)
       if (s2 < cl) {
-        const uint32_t rb = mapa_u32(base, (uint32_t)s2);
-        ml[s2] = ld_dsmem_f2(rb + ML_OFF + row * 8);
-        ov[s2] = ld_dsmem_f4(rb + (uint32_t)(row * (D + 8) + c4 * 4) * 4);
+        ml[s2] = sh.cl_ml[s2 * n + i];
+        ov[s2] = *reinterpret_cast<const float4*>(base + (size_t)s2 * n * (D * 4));
       }
     float m = -INFINITY;
 #pragma unroll
@@ -384,15 +423,14 @@ __device__ __forceinline__ void attn_cluster_merge(const AttnParams& p, const At
     float l = 0.f;
 #pragma unroll
     for (int s2 = 0; s2 < MAXCL; ++s2)
-      if (s2 < cl && ml[s2].y > 0.f) {                         // a CTA without tiles (or without a visible key) holds l = 0
+      if (s2 < cl && ml[s2].y > 0.f) {                         // a CTA without tiles (or without a visible key) sends l = 0
         const float w = fast_exp2(ml[s2].x - m);
         l = fmaf(w, ml[s2].y, l);
         acc.x = fmaf(w, ov[s2].x, acc.x); acc.y = fmaf(w, ov[s2].y, acc.y);
         acc.z = fmaf(w, ov[s2].z, acc.z); acc.w = fmaf(w, ov[s2].w, acc.w);
       }
     const float inv = 1.f / l;                                 // every row sees key 0: l > 0
-    const int qi = row / p.group, hg = row % p.group;
-    __nv_bfloat16* dst = p.out + ((size_t)(r0 + qi) * p.n_q_heads + g * p.group + hg) * D + c4 * 4;
+    __nv_bfloat16* dst = p.out + ((size_t)(unsigned int)sh.cl_dst[row] >> 5) + c4 * 4;
     *reinterpret_cast<uint2*>(dst) = make_uint2(pack_bf16(acc.x * inv, acc.y * inv), pack_bf16(acc.z * inv, acc.w * inv));
   }
 }
@@ -402,7 +440,7 @@ __device__ __forceinline__ void attn_cluster_merge(const AttnParams& p, const At
 // keeps its own running (m, l, O); at the end of a segment group 1 hands its state to group 0 through smem.
 template <int D>
 __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared<false>& sh, uint8_t* q_s, uint8_t* p0_s, uint8_t* p1_s,
-                                             uint8_t* v_s, uint8_t* part_s, uint32_t tmem_base, int warp, int lane) {
+                                             uint8_t* v_s, uint8_t* part_s, uint8_t* recv_s, uint32_t tmem_base, int warp, int lane) {
   using C = AttnCfg<D, false>;
   constexpr int NO = D / 2;                                    // O registers per thread (2 rows x D/4 columns)
   const int Hkv = p.kv.n_kv_heads;
@@ -417,7 +455,20 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared<fal
   SegWalker<false> walk(sh, p.kv.n_kv_heads, blockIdx.x);
   Segment sg;
   uint32_t gt0 = 0;                                            // global tile counter at the start of the segment
+  if (sh.cl > 0) {
+    // cluster mode: the row-dealing tables of the merge, by threads that would otherwise idle through the Q load's
+    // integer work: group 1 builds them, everybody reads them behind the named barriers of the group merge
+    const int Rt = min((sh.r0[1] - sh.r0[0]) * p.group, AT_ROWS);
+    if (grp == 1 && stid <= sh.cl) sh.cl_rb[stid] = cl_row_begin(stid, Rt, sh.cl);
+    if (grp == 1 && stid >= 64 && stid - 64 < Rt) {
+      const int r = stid - 64, qi = r / p.group, hg = r % p.group;
+      const unsigned int off = (unsigned int)(((sh.r0[0] + qi) * p.n_q_heads + sh.seg.g * p.group + hg) * D);
+      sh.cl_dst[r] = (int)((off << 5) | (unsigned int)cl_row_owner(r, Rt, sh.cl));
+    }
+  }
+  WF_PROBE_AT(16, warp == 0 && lane == 0);
   while (walk.next(sg)) {
+    WF_PROBE_AT(17, warp == 0 && lane == 0);
     const int R = sg.q_b * p.group;
     bool has_next;                                             // this CTA has another segment after this one
     {
@@ -452,15 +503,18 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared<fal
           qv[u] = __ldg(reinterpret_cast<const uint4*>(p.q + ((size_t)(sg.r0 + i2) * p.n_q_heads + sg.g * p.group + h2) * D) + chn);
         }
       }
+      WF_PROBE_AT(18, warp == 0 && lane == 0);
 #pragma unroll
       for (int u = 0; u < NQ; ++u) {
         const int c = grp * 128 + stid + u * 256;
         const int rr = c / (D / 8), chn = c % (D / 8);
         *reinterpret_cast<uint4*>(q_s + (chn >> 3) * C::Q_HALF + rr * 128 + (((chn & 7) ^ (rr & 7)) << 4)) = qv[u];
       }
+      WF_PROBE_AT(19, warp == 0 && lane == 0 && qv[0].x != 0x12345678u);
     }
     fence_proxy_async();
     mbar_arrive(smem_u32(&sh.q_ready));
+    WF_PROBE_AT(3, warp == 0 && lane == 0);
 
     float m_run[2] = {-INFINITY, -INFINITY}, l_run[2] = {0.f, 0.f}, alpha_prev[2] = {0.f, 0.f};
     float o[NO];
@@ -487,6 +541,9 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared<fal
       const uint32_t g2 = gt0 + t;
       const int tk0 = sg.k0 + t * AT_BN;
       mbar_wait(smem_u32(&sh.s_full[grp]), (g2 >> 1) & 1);
+      const int pti = (t - t_first) >> 1;
+      WF_PROBE_AT(20 + 6 * pti, warp == 4 && lane == 0 && pti < 2);
+      WF_PROBE_AT(4, warp == 0 && lane == 0 && t == t_first);
       tc_fence_after();
       uint32_t sv[64];
       tmem_ld_16x256b_x16(t_lane + C::TM_S + grp * AT_BN, sv);
@@ -525,6 +582,7 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared<fal
       }
       l_run[0] = l_run[0] * alpha[0] + rs[0];
       l_run[1] = l_run[1] * alpha[1] + rs[1];
+      WF_PROBE_AT(21 + 6 * pti, warp == 4 && lane == 0 && pti < 2);
 
       if (tk0 + AT_BN > sg.k1) {
         // Last tile of the sequence: keys >= k1 hold stale or never-written V bits.  Zero them so that
@@ -532,10 +590,10 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared<fal
         // The parity wait below is only unambiguous once the previous occupant of this V stage is consumed:
         // wait for this group's previous PV first (independent of the order the MMA warp issues in).
         if (pending) mbar_wait(smem_u32(&sh.pv_done[grp]), (g_prev >> 1) & 1);
-        mbar_wait(smem_u32(&sh.v_full[g2 % C::STAGES_V]), (g2 / C::STAGES_V) & 1);
+        mbar_wait(smem_u32(&sh.v_full[g2 % sh.n_stv]), (g2 / sh.n_stv) & 1);
         const int key = (sg.k1 - tk0) + stid;
         if (key < AT_BN) {
-          uint8_t* vrow = v_s + (size_t)(g2 % C::STAGES_V) * C::K_BYTES + key * 128;
+          uint8_t* vrow = v_s + (size_t)(g2 % sh.n_stv) * C::K_BYTES + key * 128;
 #pragma unroll
           for (int h = 0; h < C::NH; ++h)
 #pragma unroll
@@ -555,7 +613,9 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared<fal
       }
       fence_proxy_async();
       mbar_arrive(smem_u32(&sh.p_full[grp]));
+      WF_PROBE_AT(22 + 6 * pti, warp == 4 && lane == 0 && pti < 2);
       if (pending) { tc_fence_after(); fold_o(); }
+      WF_PROBE_AT(23 + 6 * pti, warp == 4 && lane == 0 && pti < 2);
       alpha_prev[0] = alpha[0];
       alpha_prev[1] = alpha[1];
       pending = true;
@@ -563,13 +623,16 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared<fal
     }
     if (pending) {
       mbar_wait(smem_u32(&sh.pv_done[grp]), (g_prev >> 1) & 1);
+      WF_PROBE_AT(24, warp == 4 && lane == 0);
       tc_fence_after();
       fold_o();
+      WF_PROBE_AT(25, warp == 4 && lane == 0);
     } else {
       // one-tile segment owned by the other group: wait for its PV so that every MMA reading Q / P has retired
       mbar_wait(smem_u32(&sh.pv_done[grp ^ 1]), (gt0 >> 1) & 1);
     }
     gt0 += sg.n_tiles;
+    WF_PROBE_AT(5, warp == 0 && lane == 0);
 
     // Shared pair: arrive NOW (one packed counter: arrived in the low half, published in the high half); the
     // round trip overlaps the group merge below.  Arriving only decides who merges, it publishes nothing.
@@ -608,6 +671,7 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared<fal
       for (int c = 0; c < NO; ++c) o[c] = o[c] * e0[(c >> 1) & 1] + xch[c * 128 + stid] * e1[(c >> 1) & 1];
     }
     named_bar_sync(5, 256);
+    WF_PROBE_AT(6, warp == 0 && lane == 0);
 
     // ---- finish the rows: quad-reduce the row sums, write final rows or the partial ----
 #pragma unroll
@@ -616,17 +680,26 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared<fal
       l_run[h] += __shfl_xor_sync(0xffffffffu, l_run[h], 2);
     }
     if (sh.cl > 0) {
-      // Cluster mode: the partial (m, l, unnormalised O) of this CTA goes to its OWN shared memory (the K ring is idle: every
-      // MMA has retired); after the cluster barrier every CTA of the pair folds one slice of the rows out of all the
-      // CTAs' partials through distributed shared memory (attn_cluster_merge).  Nothing touches global memory.
-      float* po = reinterpret_cast<float*>(part_s);
-      float2* pml = reinterpret_cast<float2*>(part_s + AT_ROWS * (D + 8) * 4);
+      // Cluster mode: the partial (m, l, unnormalised O) of this CTA goes to its OWN shared memory (K stage 1 is idle: every
+      // MMA has retired), then warp 0 pushes every owner its rows (attn_cluster_push).  Group 0 only.
+      const int Rc = min(R, AT_ROWS);
 #pragma unroll
       for (int h = 0; h < 2; ++h) {
-        float* prow = po + (row_lo + 8 * h) * (D + 8) + cq;
+        const int r = row_lo + 8 * h;
+        uint8_t* prow = part_s + (size_t)r * (D * 4) + (cq & 3) * 4;
 #pragma unroll
-        for (int j = 0; j < D / 8; ++j) *reinterpret_cast<float2*>(prow + 8 * j) = make_float2(o[4 * j + 2 * h], o[4 * j + 2 * h + 1]);
-        if ((lane & 3) == 0) pml[row_lo + 8 * h] = make_float2(m_run[h], l_run[h]);
+        for (int j = 0; j < D / 8; ++j)
+          *reinterpret_cast<float2*>(prow + (((2 * j + (cq >> 2)) ^ (r & 7)) << 4)) = make_float2(o[4 * j + 2 * h], o[4 * j + 2 * h + 1]);
+      }
+      fence_proxy_async();
+      named_bar_sync(3, 128);
+      // (m, l) go to cl_ml of the owner, which is static shared memory nobody else uses: no readiness needed
+#pragma unroll
+      for (int h = 0; h < 2; ++h)
+        if ((lane & 3) == 0 && row_lo + 8 * h < Rc) attn_cluster_push_ml(sh, row_lo + 8 * h, m_run[h], l_run[h]);
+      if (warp == 0) {
+        mbar_wait(smem_u32(&sh.cl_ready), 0);                  // every CTA of the cluster can receive (its K ring is idle)
+        attn_cluster_push<D>(sh, part_s, recv_s, lane);
       }
       continue;
     }
@@ -743,13 +816,24 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared<fal
     write_rows();
   }
   if (sh.cl > 0) {
-    // cluster mode: a CTA without tiles publishes an empty partial (l = 0), then barrier, fold of this CTA's rows, barrier
-    // (nobody leaves while a peer may still read its shared memory)
-    if (gt0 == 0 && grp == 0 && stid < AT_ROWS)
-      reinterpret_cast<float2*>(part_s + AT_ROWS * (D + 8) * 4)[stid] = make_float2(-INFINITY, 0.f);
-    cluster_sync_all();
-    attn_cluster_merge<D>(p, sh, part_s, grp * 128 + stid);
-    cluster_sync_all();
+    const int R = min((sh.r0[1] - sh.r0[0]) * p.group, AT_ROWS);
+    if (gt0 == 0) {
+      // a CTA without tiles still owes every owner a slice: l = 0 marks it empty (its O bits are never read)
+      named_bar_sync(4, 256);                                  // the tables above
+      if (grp == 0 && stid < R) attn_cluster_push_ml(sh, stid, -INFINITY, 0.f);
+      if (warp == 0) {
+        mbar_wait(smem_u32(&sh.cl_ready), 0);
+        attn_cluster_push<D>(sh, part_s, recv_s, lane);
+      }
+    }
+    WF_PROBE_AT(7, warp == 0 && lane == 0);
+    mbar_wait(smem_u32(&sh.cl_bar), 0);                        // every slice of this CTA's rows has landed
+    WF_PROBE_AT(8, warp == 0 && lane == 0);
+    cluster_arrive();                                          // "what was pushed to me has landed": see the kernel's epilogue
+    attn_cluster_reduce<D>(p, sh, recv_s, grp * 128 + stid);
+    WF_PROBE_AT(9, warp == 0 && lane == 0);
+    cluster_wait();
+    WF_PROBE_AT(10, warp == 0 && lane == 0);
   }
 }
 
@@ -893,10 +977,10 @@ __device__ __forceinline__ void attn_softmax_tree(const AttnParams& p, AttnShare
       if (tk0 + AT_BN > sg.k1 && grp == 0) {
         // Last tile of the sequence: keys >= k1 hold stale or never-written V bits; zero them so that 0 * garbage cannot
         // produce NaN in the PV product (P is exactly 0 there).  Group 0 does it; PV waits for all 256 P arrivals.
-        mbar_wait(smem_u32(&sh.v_full[g2 % C::STAGES_V]), (g2 / C::STAGES_V) & 1);
+        mbar_wait(smem_u32(&sh.v_full[g2 % sh.n_stv]), (g2 / sh.n_stv) & 1);
         const int key = (sg.k1 - tk0) + stid;
         if (key < AT_BN) {
-          uint8_t* vrow = v_s + (size_t)(g2 % C::STAGES_V) * C::K_BYTES + key * 128;
+          uint8_t* vrow = v_s + (size_t)(g2 % sh.n_stv) * C::K_BYTES + key * 128;
 #pragma unroll
           for (int h = 0; h < C::NH; ++h)
 #pragma unroll
@@ -1025,6 +1109,7 @@ __global__ void __launch_bounds__(AT_THREADS, 1) wf_verify_attn_kernel(const Att
 
   // barrier init and TMEM allocation touch no global memory: they run before the dependency wait and overlap the
   // tail of the previous kernel of the stream (programmatic dependent launch)
+  WF_PROBE_AT(0, tid == 0);
   wf_pdl_trigger();
   if (tid == 0) {
     for (int i = 0; i < AT_MAX_STAGES; ++i) {
@@ -1039,118 +1124,168 @@ __global__ void __launch_bounds__(AT_THREADS, 1) wf_verify_attn_kernel(const Att
       mbar_init(smem_u32(&sh.pv_done[i]), 1);
     }
     mbar_init(smem_u32(&sh.q_ready), 256);
+    if constexpr (!TREE) {
+      mbar_init(smem_u32(&sh.cl_bar), 1);
+      mbar_init(smem_u32(&sh.k_done), 1);
+      mbar_init(smem_u32(&sh.cl_ready), p.cl > 0 ? p.cl : 1);
+    }
+    sh.n_stk = C::STAGES_K;
+    sh.n_stv = C::STAGES_V;
     fence_barrier_init();
   }
   if (warp == 9) tmem_alloc(smem_u32(&sh.tmem), 512);
+  if constexpr (!TREE) {
+    // cluster mode: peers push into this CTA's shared memory and arrive on its mbarrier: nobody may do so before the
+    // barrier exists.  This cluster barrier sits ahead of the dependency wait: it overlaps the previous kernel's tail.
+    if (p.cl > 0) { cluster_arrive(); cluster_wait(); }
+  }
+  if (tid == 32 * 8 || tid == 32 * 10)                         // the K / V tensor maps are constants: fetch them ahead of the wait
+    asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(p.kv.tmaps + (tid == 32 * 10 ? 1 : 0))) : "memory");
   wf_pdl_wait();
-  // per-sequence table (tiles per kv head, q_indptr, context) from the device-resident lengths, identical in
-  // every CTA; then total tiles and the longest pair
-  // TREE: the per-sequence values go to the (still idle) dynamic shared memory first; warp 0 then expands them
-  // into the sub-block table below.
-  int* t_r0 = reinterpret_cast<int*>(smem);
-  int* t_ctx = t_r0 + AT_MAX_B;
-  int* t_q = t_ctx + AT_MAX_B;
-  for (int b = tid; b < p.B; b += AT_THREADS) {
-    const int r0 = p.q_indptr[b], r1 = p.q_indptr[b + 1], ctx = p.kv.seq_len[b] + p.ctx_adj;
-    // the host bound max_q_len / max_nodes is a promise: a longer block has its rows beyond the query tile dropped
-    if (blockIdx.x == 0 && (TREE ? r1 - r0 > 64 : (r1 - r0) * p.group > AT_ROWS)) wf_raise(p.status, (int)WF_ERR_INVALID_ARG);
-    if constexpr (TREE) {
-      t_r0[b] = r0;
-      t_ctx[b] = ctx;
-      t_q[b] = min(r1 - r0, 64);
-    } else {
-      sh.r0[b] = r0;
-      sh.ctx[b] = ctx;
-      sh.pref[b + 1] = r1 > r0 ? (ctx + (r1 - r0) + AT_BN - 1) / AT_BN + AT_SEG_COST : 0;
-      if (b == p.B - 1) sh.r0[p.B] = r1;
-    }
-  }
-  tc_fence_before();
-  __syncthreads();
-  tc_fence_after();
-  const uint32_t tmem_base = sh.tmem;
-  if (warp == 0) {                                             // in-place scan of the tile counts, 32 sequences per step
-    int n_tab = p.B;                                           // table entries
-    if constexpr (TREE) {
-      // Block s of sequence b = nodes [s * npt, (s+1) * npt), npt = 2 * 64 / group nodes = one 128-row query tile
-      // (two sub-blocks).  Each block is a pair of its own that streams the sequence's whole KV; the table lists them
-      // LEVEL-MAJOR (all first blocks, then all second ones, ...): with equal trees the level copies of a (b, g) pair
-      // sit T / levels positions apart, i.e. in CTAs c, c + G / levels, ... at the same offset of their ranges,
-      // which stream the same K/V tiles at the same time: HBM serves one of them, L2 the rest.
-      const int npt = 2 * (AT_ROWS / p.group);                // nodes per 128-row tile (two sub-blocks)
-      int cursor = 0;
-      for (int s0 = 0; s0 < 64; s0 += npt) {
-        const int before = cursor;
-        for (int base = 0; base < p.B; base += 32) {
-          const int b = base + lane;
-          const int q = b < p.B ? t_q[b] : 0;
-          const bool on = q > s0;
-          const unsigned int bal = __ballot_sync(0xffffffffu, on);
-          const int idx = cursor + __popc(bal & ((1u << lane) - 1u));
-          if (on && idx < AT_MAX_B) {
-            const int ctx = t_ctx[b];
-            sh.r0[idx] = t_r0[b] + s0;
-            sh.ctx[idx] = ctx;
-            sh.meta[idx] = min(npt, q - s0) | (q << 7) | (s0 << 14) | (b << 21);
-            sh.pref[idx + 1] = (ctx + q + AT_BN - 1) / AT_BN + AT_SEG_COST;
-          }
-          cursor += __popc(bal);
-        }
-        if (cursor == before) break;                           // no tree is this large
-      }
-      n_tab = min(cursor, AT_MAX_B);
-      __syncwarp();
-    }
-    int run = 0, lg = 0, live = 0;
-    for (int base = 0; base < n_tab; base += 32) {
-      const int n = base + lane < n_tab ? sh.pref[base + lane + 1] : 0;
-      lg = max(lg, n);
-      live += n > 0;
-      int v = n;
-#pragma unroll
-      for (int d = 1; d < 32; d <<= 1) {
-        const int y = __shfl_up_sync(0xffffffffu, v, d);
-        if (lane >= d) v += y;
-      }
-      if (base + lane < n_tab) sh.pref[base + lane + 1] = run + v;
-      run += __shfl_sync(0xffffffffu, v, 31);
-    }
-#pragma unroll
-    for (int d = 16; d > 0; d >>= 1) {
-      lg = max(lg, __shfl_xor_sync(0xffffffffu, lg, d));
-      live += __shfl_xor_sync(0xffffffffu, live, d);
-    }
-    if (lane == 0) {
+  WF_PROBE_AT(1, tid == 0);
+  // Cluster mode: a CTA serves ONE (b, g) pair, so it tabulates only that sequence: one global round trip, one barrier
+  // (the full table costs two barriers and a scan: 2.4k cycles, measured, on the critical path of a batch-1 launch).
+  const bool lean = !TREE && p.cl > 0;
+  if (lean) {
+    if (tid == 0) {
+      const int pair = (int)blockIdx.x / p.cl, b = pair / p.kv.n_kv_heads;
+      const int r0 = p.q_indptr[b], r1 = p.q_indptr[b + 1], ctx = p.kv.seq_len[b] + p.ctx_adj;
+      if ((int)blockIdx.x % p.cl == 0 && pair % p.kv.n_kv_heads == 0 && (r1 - r0) * p.group > AT_ROWS) wf_raise(p.status, (int)WF_ERR_INVALID_ARG);
+      sh.r0[0] = r0; sh.r0[1] = r1; sh.ctx[0] = ctx;
       sh.pref[0] = 0;
-      const int total = run * p.kv.n_kv_heads;
-      // ranges of at least ceil(longest / 30) tiles keep the partials of one pair <= AT_MAX_SEG
-      const int min_range = max(1, (lg + AT_MAX_SEG - 3) / (AT_MAX_SEG - 2));
-      sh.total_tiles = total;
-      // Small launches (under 24 tiles per SM) are latency-bound: every segment costs about 10k cycles of fixed
-      // latency, a pair cut into n ranges streams (tiles/n) * 1.3k cycles and its last arriver folds n partials at
-      // about 1k cycles each: least at n = sqrt(1.3 * tiles per pair).  G = n * pairs keeps the ranges aligned with
-      // the pairs (one segment per CTA) when the contexts are equal.  Large launches use one CTA per SM.
-      const int pairs = live * p.kv.n_kv_heads;
-      int G = (int)gridDim.x;
-      if (pairs > 0 && total < 24 * G) {
-        int n = (int)(sqrtf(1.3f * (float)total / (float)pairs) + 0.5f);
-        n = max(1, min(n, G / pairs));
-        G = min(G, n * pairs);
-      }
-      sh.g_eff = p.cl > 0 ? (int)gridDim.x : max(1, min(G, total / min_range));
-      sh.B = n_tab;
-      sh.cl = TREE ? 0 : p.cl;
-      if (blockIdx.x == 0 && p.tiles_hint) *p.tiles_hint = total;      // feedback for the host's next choice of launch shape
+      sh.pref[1] = r1 > r0 ? (ctx + (r1 - r0) + AT_BN - 1) / AT_BN + AT_SEG_COST : 0;
+      const int nt = max(0, sh.pref[1] - AT_SEG_COST);
+      sh.total_tiles = nt;
+      sh.g_eff = (int)gridDim.x; sh.B = 1; sh.cl = p.cl; sh.cl_b = b;
+      // cluster `pair` = (b, g) over ALL sequences of the call (an empty one idles its cluster); CTA rank r of the cluster owns
+      // tiles [r * nt / cl, (r + 1) * nt / cl) of the pair: pair-aligned, equal shares, one segment
+      const int rank = (int)blockIdx.x % p.cl;
+      Segment sg;
+      sg.b = b; sg.pb = 0; sg.nt = nt; sg.g = pair % p.kv.n_kv_heads;
+      sg.t_lo = rank * nt / p.cl; sg.t_hi = (rank + 1) * nt / p.cl;
+      sg.flat0 = 0; sg.r0 = r0; sg.ctx = ctx; sg.q_b = r1 - r0;
+      sg.k0 = sg.t_lo * AT_BN; sg.k1 = min(ctx + sg.q_b, sg.t_hi * AT_BN);
+      sg.n_tiles = sg.t_hi - sg.t_lo; sg.partial = 1; sg.slot = 0;
+      sh.seg = sg;
+      // what this CTA will receive: from each of the cl CTAs, its rows [row_a, row_b) of (m, l) and of O
+      const int R = min((r1 - r0) * p.group, AT_ROWS);
+      const int n_mine = cl_row_begin(rank + 1, R, p.cl) - cl_row_begin(rank, R, p.cl);
+      if (nt > 0) mbar_arrive_expect_tx(smem_u32(&sh.cl_bar), (uint32_t)(p.cl * n_mine * (D * 4 + 8)));
     }
-  }
-  __syncthreads();
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+  } else {
+    // per-sequence table (tiles per kv head, q_indptr, context) from the device-resident lengths, identical in
+    // every CTA; then total tiles and the longest pair
+    // TREE: the per-sequence values go to the (still idle) dynamic shared memory first; warp 0 then expands them
+    // into the sub-block table below.
+    int* t_r0 = reinterpret_cast<int*>(smem);
+    int* t_ctx = t_r0 + AT_MAX_B;
+    int* t_q = t_ctx + AT_MAX_B;
+    for (int b = tid; b < p.B; b += AT_THREADS) {
+      const int r0 = p.q_indptr[b], r1 = p.q_indptr[b + 1], ctx = p.kv.seq_len[b] + p.ctx_adj;
+      // the host bound max_q_len / max_nodes is a promise: a longer block has its rows beyond the query tile dropped
+      if (blockIdx.x == 0 && (TREE ? r1 - r0 > 64 : (r1 - r0) * p.group > AT_ROWS)) wf_raise(p.status, (int)WF_ERR_INVALID_ARG);
+      if constexpr (TREE) {
+        t_r0[b] = r0;
+        t_ctx[b] = ctx;
+        t_q[b] = min(r1 - r0, 64);
+      } else {
+        sh.r0[b] = r0;
+        sh.ctx[b] = ctx;
+        sh.pref[b + 1] = r1 > r0 ? (ctx + (r1 - r0) + AT_BN - 1) / AT_BN + AT_SEG_COST : 0;
+        if (b == p.B - 1) sh.r0[p.B] = r1;
+      }
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    if (warp == 0) {                                             // in-place scan of the tile counts, 32 sequences per step
+      int n_tab = p.B;                                           // table entries
+      if constexpr (TREE) {
+        // Block s of sequence b = nodes [s * npt, (s+1) * npt), npt = 2 * 64 / group nodes = one 128-row query tile
+        // (two sub-blocks).  Each block is a pair of its own that streams the sequence's whole KV; the table lists them
+        // LEVEL-MAJOR (all first blocks, then all second ones, ...): with equal trees the level copies of a (b, g) pair
+        // sit T / levels positions apart, i.e. in CTAs c, c + G / levels, ... at the same offset of their ranges,
+        // which stream the same K/V tiles at the same time: HBM serves one of them, L2 the rest.
+        const int npt = 2 * (AT_ROWS / p.group);                // nodes per 128-row tile (two sub-blocks)
+        int cursor = 0;
+        for (int s0 = 0; s0 < 64; s0 += npt) {
+          const int before = cursor;
+          for (int base = 0; base < p.B; base += 32) {
+            const int b = base + lane;
+            const int q = b < p.B ? t_q[b] : 0;
+            const bool on = q > s0;
+            const unsigned int bal = __ballot_sync(0xffffffffu, on);
+            const int idx = cursor + __popc(bal & ((1u << lane) - 1u));
+            if (on && idx < AT_MAX_B) {
+              const int ctx = t_ctx[b];
+              sh.r0[idx] = t_r0[b] + s0;
+              sh.ctx[idx] = ctx;
+              sh.meta[idx] = min(npt, q - s0) | (q << 7) | (s0 << 14) | (b << 21);
+              sh.pref[idx + 1] = (ctx + q + AT_BN - 1) / AT_BN + AT_SEG_COST;
+            }
+            cursor += __popc(bal);
+          }
+          if (cursor == before) break;                           // no tree is this large
+        }
+        n_tab = min(cursor, AT_MAX_B);
+        __syncwarp();
+      }
+      int run = 0, lg = 0, live = 0;
+      for (int base = 0; base < n_tab; base += 32) {
+        const int n = base + lane < n_tab ? sh.pref[base + lane + 1] : 0;
+        lg = max(lg, n);
+        live += n > 0;
+        int v = n;
+  #pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+          const int y = __shfl_up_sync(0xffffffffu, v, d);
+          if (lane >= d) v += y;
+        }
+        if (base + lane < n_tab) sh.pref[base + lane + 1] = run + v;
+        run += __shfl_sync(0xffffffffu, v, 31);
+      }
+  #pragma unroll
+      for (int d = 16; d > 0; d >>= 1) {
+        lg = max(lg, __shfl_xor_sync(0xffffffffu, lg, d));
+        live += __shfl_xor_sync(0xffffffffu, live, d);
+      }
+      if (lane == 0) {
+        sh.pref[0] = 0;
+        const int total = run * p.kv.n_kv_heads;
+        // ranges of at least ceil(longest / 30) tiles keep the partials of one pair <= AT_MAX_SEG
+        const int min_range = max(1, (lg + AT_MAX_SEG - 3) / (AT_MAX_SEG - 2));
+        sh.total_tiles = total;
+        // Small launches (under 24 tiles per SM) are latency-bound: every segment costs about 10k cycles of fixed
+        // latency, a pair cut into n ranges streams (tiles/n) * 1.3k cycles and its last arriver folds n partials at
+        // about 1k cycles each: least at n = sqrt(1.3 * tiles per pair).  G = n * pairs keeps the ranges aligned with
+        // the pairs (one segment per CTA) when the contexts are equal.  Large launches use one CTA per SM.
+        const int pairs = live * p.kv.n_kv_heads;
+        int G = (int)gridDim.x;
+        if (pairs > 0 && total < 24 * G) {
+          int n = (int)(sqrtf(1.3f * (float)total / (float)pairs) + 0.5f);
+          n = max(1, min(n, G / pairs));
+          G = min(G, n * pairs);
+        }
+        sh.g_eff = p.cl > 0 ? (int)gridDim.x : max(1, min(G, total / min_range));
+        sh.B = n_tab;
+        sh.cl = TREE ? 0 : p.cl;
+        if (blockIdx.x == 0 && p.tiles_hint) *p.tiles_hint = total;      // feedback for the host's next choice of launch shape
+      }
+    }
+    __syncthreads();
 
+  }
+  const uint32_t tmem_base = sh.tmem;
   const bool run = sh.total_tiles > 0 && (int)blockIdx.x < sh.g_eff;
+  WF_PROBE_AT(2, tid == 0);
   if (run) {
     if (warp < 8) {
       asm volatile("setmaxnreg.inc.sync.aligned.u32 216;");
       if constexpr (TREE) attn_softmax_tree<D>(p, sh, q_s, p0_s, v_s, tmem_base, warp, lane);
-      else attn_softmax<D>(p, sh, q_s, p0_s, p1_s, v_s, k_s, tmem_base, warp, lane);
+      else attn_softmax<D>(p, sh, q_s, p0_s, p1_s, v_s, k_s + C::K_BYTES, k_s, tmem_base, warp, lane);
     } else {
       asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
       if (warp == 8) attn_loader<D, TREE>(p, sh, k_s, 0, lane);
@@ -1160,11 +1295,21 @@ __global__ void __launch_bounds__(AT_THREADS, 1) wf_verify_attn_kernel(const Att
     }
   }
   if constexpr (!TREE) {
-    // cluster mode: the softmax warps of a running CTA take the two cluster barriers inside attn_softmax; everybody else here
-    if (sh.cl > 0 && !(run && warp < 8)) { cluster_sync_all(); cluster_sync_all(); }
+    if (lean && blockIdx.x == 0 && tid == 32 * 8 && p.tiles_hint) {   // off the critical path: the loader warp is done
+      int total = 0;
+      for (int b = 0; b < p.B; ++b) {
+        const int q = p.q_indptr[b + 1] - p.q_indptr[b];
+        if (q > 0) total += (p.kv.seq_len[b] + p.ctx_adj + q + AT_BN - 1) / AT_BN;
+      }
+      *p.tiles_hint = total * p.kv.n_kv_heads;
+    }
+    // cluster mode: nobody leaves while a copy it pushed may still be reading its shared memory: a CTA arrives once
+    // everything pushed TO it has landed (the softmax warps of a running CTA do so inside attn_softmax), and all wait
+    if (sh.cl > 0 && !(run && warp < 8)) { cluster_arrive(); cluster_wait(); }
   }
   tc_fence_before();
   __syncthreads();
+  WF_PROBE_AT(11, tid == 0);
   if (warp == 9) tmem_dealloc(tmem_base, 512);
 }
 
@@ -1176,10 +1321,56 @@ __global__ void __launch_bounds__(AT_THREADS, 1) wf_verify_attn_kernel(const Att
 namespace {
 
 template <int D, bool TREE>
-int launch_attn(wf_ctx* ctx, const AttnParams& p, cudaStream_t st) {
+int launch_attn(wf_ctx* ctx, AttnParams& p, int* h_hint, cudaStream_t st) {
   const size_t smem = AttnCfg<D, TREE>::SMEM;
   WF_CONFIGURE_ONCE(ctx, (TREE ? WF_FUNC_ATTN_TREE_128 : WF_FUNC_ATTN_128) + (D == 64 ? 1 : 0), (wf_verify_attn_kernel<D, TREE>), smem);
   const int grid = ctx->sm_count < AT_MAX_CTAS ? ctx->sm_count : AT_MAX_CTAS;   // one persistent CTA per SM
+  p.cl = 0;
+  p.tiles_hint = nullptr;
+  if (h_hint) WF_CUDA(ctx, cudaHostGetDevicePointer((void**)&p.tiles_hint, h_hint, 0));
+  if constexpr (!TREE) {
+    // Launch shape.  Few (b, g) pairs (batch 1-2): one thread-block CLUSTER per pair, the pair's tiles split evenly over
+    // its CTAs, partials folded through distributed shared memory (no global round trip, fixed order).  The cluster size is
+    // the largest that lets every pair's cluster be resident at once (GPC sizes allow 7 clusters of 12-16 CTAs, 11 of 10,
+    // 15 of 8-9, 22 of 6, 33 of 4 with one CTA per SM).  Whether a launch is long enough for stream-K over all SMs to win
+    // (HBM-paced: >= 24 tiles per SM) depends on the device-resident lengths: the kernel leaves the tile count of each
+    // launch in mapped host memory, and the host reads the last value it can see (no synchronisation; either shape
+    // is correct for any lengths, the hint only picks the faster one).
+    const int pairs = p.B * p.kv.n_kv_heads;
+    int* tab = ctx->attn_max_clusters[D == 64 ? 1 : 0];
+    if (!tab[0]) {
+      tab[0] = 1;
+      cudaFuncSetAttribute(wf_verify_attn_kernel<D, TREE>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+      for (int cl = 2; cl <= 16; ++cl) {
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(cl); cfg.blockDim = dim3(AT_THREADS); cfg.dynamicSmemBytes = smem;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeClusterDimension;
+        at[0].val.clusterDim.x = cl; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+        cfg.attrs = at; cfg.numAttrs = 1;
+        int n = 0;
+        if (cudaOccupancyMaxActiveClusters(&n, wf_verify_attn_kernel<D, TREE>, &cfg) != cudaSuccess) n = 0;
+        tab[cl] = n;
+      }
+      cudaGetLastError();
+    }
+    int cl = 0;
+    const int hint = h_hint ? *(volatile int*)h_hint : -1;
+    const bool hbm_paced = hint >= 24 * grid;
+    if (ctx->attn_cluster_override > 0) cl = ctx->attn_cluster_override;
+    else if (ctx->attn_cluster_override < 0 && pairs > 0) {
+      for (int c2 = 16; c2 >= 4; --c2)
+        if (tab[c2] >= pairs) { cl = c2; break; }
+      // an HBM-paced launch wants every SM: clusters only if they cover most of the machine (measured at batch 4, context
+      // 32768: 32 clusters of 4 = 128 CTAs stream 5.88 TB/s against 5.68 for stream-K ranges on 148: no global merge)
+      if (hbm_paced && pairs * cl * 5 < grid * 4) cl = 0;
+    }
+    if (cl > 1 && cl <= 16 && tab[cl] >= pairs) {
+      p.cl = cl;
+      wf_launch_cluster(wf_verify_attn_kernel<D, TREE>, dim3(pairs * cl), dim3(AT_THREADS), smem, cl, st, p);
+      return wf_check_launch(ctx, "wf_verify_attn_kernel<cluster>");
+    }
+  }
   wf_launch(wf_verify_attn_kernel<D, TREE>, dim3(grid), dim3(AT_THREADS), smem, st, p);
   return wf_check_launch(ctx, TREE ? "wf_verify_attn_kernel<tree>" : "wf_verify_attn_kernel");
 }
@@ -1254,8 +1445,8 @@ int wf_attn_launch_chain(wf_ctx* ctx, const wf_paged_kv* kv, int layer, const vo
   cudaStream_t st = (cudaStream_t)stream;
   const int D = kv->s.head_dim;
   p.tree_mask = nullptr;
-  if (D == 128) return launch_attn<128, false>(ctx, p, st);
-  if (D == 64) return launch_attn<64, false>(ctx, p, st);
+  if (D == 128) return launch_attn<128, false>(ctx, p, kv->h_tiles_hint, st);
+  if (D == 64) return launch_attn<64, false>(ctx, p, kv->h_tiles_hint, st);
   return wf_set_error(ctx, WF_ERR_UNSUPPORTED_SHAPE, "%s: head_dim %d unsupported", who, D);
 }
 
@@ -1316,7 +1507,15 @@ extern "C" int wf_verify_attn_tree(wf_ctx* ctx, const wf_paged_kv* kv, int layer
   p.status = ctx->d_status;
   cudaStream_t st = (cudaStream_t)stream;
   const int D = kv->s.head_dim;
-  if (D == 128) return launch_attn<128, true>(ctx, p, st);
-  if (D == 64) return launch_attn<64, true>(ctx, p, st);
+  if (D == 128) return launch_attn<128, true>(ctx, p, nullptr, st);
+  if (D == 64) return launch_attn<64, true>(ctx, p, nullptr, st);
   return wf_set_error(ctx, WF_ERR_UNSUPPORTED_SHAPE, "wf_verify_attn_tree: head_dim %d unsupported", D);
+}
+
+extern "C" int wf_ctx_set_attn_cluster(wf_ctx* ctx, int cluster_size) {
+  if (!ctx) return WF_ERR_INVALID_ARG;
+  WF_REQUIRE(ctx, cluster_size >= -1 && cluster_size <= 16 && cluster_size != 1, WF_ERR_INVALID_ARG,
+             "wf_ctx_set_attn_cluster: cluster_size must be -1 (automatic), 0 (never) or 2..16");
+  ctx->attn_cluster_override = cluster_size;
+  return WF_OK;
 }

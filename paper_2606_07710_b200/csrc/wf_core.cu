@@ -67,6 +67,8 @@ extern "C" int wf_ctx_create(wf_ctx** out, int device_ordinal) {
   c->launches = 0;
   c->func_configured = 0;
   c->deterministic = 0;
+  memset(c->attn_max_clusters, 0, sizeof(c->attn_max_clusters));
+  c->attn_cluster_override = -1;
   c->err[0] = 0;
   c->n_counters = 1 << 16;
   if (cudaMalloc(&c->d_status, sizeof(int)) != cudaSuccess ||
@@ -140,6 +142,7 @@ extern "C" int wf_kv_create(wf_ctx* ctx, const wf_kv_shape* s, void* k_pool, voi
   kv->seq_len = seq_len;
   kv->pages_held = kv->free_ring = kv->ring_state = kv->scratch = nullptr;
   kv->d_tmaps = nullptr;
+  kv->h_tiles_hint = nullptr;
   CUtensorMap maps[2];
   {
     const uint64_t rows = (uint64_t)s->n_layers * s->num_pages * s->n_kv_heads * s->page_size;
@@ -152,6 +155,8 @@ extern "C" int wf_kv_create(wf_ctx* ctx, const wf_kv_shape* s, void* k_pool, voi
   if (e == cudaSuccess) e = cudaMalloc(&kv->ring_state, sizeof(int32_t) * 2);
   if (e == cudaSuccess) e = cudaMalloc(&kv->scratch, sizeof(int32_t) * 2 * s->max_seqs);
   if (e == cudaSuccess) e = cudaMalloc(&kv->d_tmaps, sizeof(maps));
+  if (e == cudaSuccess) e = cudaHostAlloc(&kv->h_tiles_hint, sizeof(int), cudaHostAllocMapped);
+  if (e == cudaSuccess) *kv->h_tiles_hint = -1;
   if (e == cudaSuccess) e = cudaMemcpy(kv->d_tmaps, maps, sizeof(maps), cudaMemcpyHostToDevice);
   if (e == cudaSuccess) e = cudaMemset(kv->pages_held, 0, sizeof(int32_t) * s->max_seqs);
   if (e == cudaSuccess) e = cudaMemset(kv->free_ring, 0xff, sizeof(int32_t) * s->num_pages);
@@ -174,6 +179,7 @@ extern "C" int wf_kv_destroy(wf_paged_kv* kv) {
   cudaFree(kv->ring_state);
   cudaFree(kv->scratch);
   cudaFree(kv->d_tmaps);
+  if (kv->h_tiles_hint) cudaFreeHost(kv->h_tiles_hint);
   delete kv;
   return WF_OK;
 }

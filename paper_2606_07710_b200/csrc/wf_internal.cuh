@@ -20,6 +20,8 @@ struct wf_ctx {
   int64_t launches;            // kernels launched through this ctx (host counter)
   unsigned int func_configured; // bit k: kernel k's dynamic-smem opt-in was made on THIS ctx's device (WF_FUNC_*)
   int deterministic;           // wf_ctx_set_deterministic: fixed-order split merges
+  int attn_max_clusters[2][17]; // [D == 64][cluster size]: co-resident clusters of the chain attention kernel (0 = not queried)
+  int attn_cluster_override;   // test / tuning hook: -1 = automatic, 0 = never, n > 0 = force cluster size n
   char err[256];
 };
 
@@ -49,6 +51,8 @@ struct wf_paged_kv {
   int32_t* ring_state;         // library-owned [2]: head, count
   int32_t* scratch;            // library-owned [2*max_seqs]: need, offset
   CUtensorMap* d_tmaps;        // library-owned [2]: K pool, V pool as [rows][D], box {64, 16}, 128B swizzle
+  int* h_tiles_hint;           // library-owned, pinned + mapped: total 128-key tiles of the last attention launch over this
+                               // cache (written by the kernel, read without a sync by the host to pick the next launch shape)
 };
 
 // Device-side view of a paged KV cache passed by value to kernels.
@@ -133,6 +137,21 @@ __device__ __forceinline__ void wf_pdl_wait() { asm volatile("griddepcontrol.wai
 __device__ __forceinline__ void wf_pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 // sticky device status: the FIRST error of a poll interval wins (a later one never overwrites it)
 __device__ __forceinline__ void wf_raise(int* status, int code) { atomicCAS(status, 0, code); }
+
+// the same, as thread-block clusters of `cluster` CTAs (grid must be a multiple of it)
+template <typename... KArgs, typename... Args>
+inline cudaError_t wf_launch_cluster(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, int cluster, cudaStream_t st,
+                                     Args&&... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+  cudaLaunchAttribute attr[2];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  attr[1].id = cudaLaunchAttributeClusterDimension;
+  attr[1].val.clusterDim.x = (unsigned)cluster; attr[1].val.clusterDim.y = 1; attr[1].val.clusterDim.z = 1;
+  cfg.attrs = attr; cfg.numAttrs = 2;
+  return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+}
 
 template <typename... KArgs, typename... Args>
 inline cudaError_t wf_launch(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args&&... args) {

@@ -291,3 +291,35 @@ def test_attn_long_single_sequence_many_partials(wf):
     ranges the merge allows (the min-range rule caps the partials per pair)."""
     max_abs, rel = _attn_case(wf, [70000], [16], 8, 2, 128, seed=41)
     assert max_abs <= ATTN_MAX_ABS and rel <= ATTN_REL_L2, (max_abs, rel)
+
+
+def test_attn_cluster_mode_sizes_and_reproducibility(wf):
+    """The cluster launch shape (one thread-block cluster per (sequence, kv head) pair, partials folded through distributed
+    shared memory in rank order): forced cluster sizes 2..16 incl. ones that do not divide the 64 rows, pairs with fewer
+    tiles than CTAs (CTAs without tiles), gamma 7 (32 live rows), an empty block, D = 64; every size within tolerance of the
+    oracle, and five repeated launches of the same size give IDENTICAL bits (the fold order is fixed).  Size 0 = stream-K."""
+    import gpu_harness as H
+    binding, ctx = wf
+    cases = [([4096], [16], 32, 8, 128), ([700, 130], [8, 16], 8, 2, 128), ([300, 0, 40], [16, 0, 8], 4, 2, 64),
+             ([5, 2000], [16, 1], 32, 8, 128)]
+    try:
+        for ci, (ctx_lens, q_lens, Hq, Hkv, D) in enumerate(cases):
+            pair = H.make_kv_pair(ctx, ctx_lens, q_lens, 1, Hkv, D, 500 + ci)
+            g = synth.rng(500 + ci, 202)
+            q_indptr = np.zeros(len(q_lens) + 1, dtype=np.int32)
+            q_indptr[1:] = np.cumsum(q_lens)
+            Q = synth.normal_bf16(g, (int(q_indptr[-1]), Hq, D), 1.0)
+            scale = 1.0 / math.sqrt(D)
+            want = verify_attn.verify_attn(pair.oracle, 0, Q, q_indptr, Hq, scale)
+            for size in (0, 2, 3, 5, 7, 10, 16, -1):
+                ctx.set_attn_cluster(size)
+                first = _run_attn(binding, ctx, pair, 0, Q, q_indptr, Hq, max(q_lens), scale)
+                max_abs, rel = H.attn_errors(first, want)
+                assert max_abs <= ATTN_MAX_ABS and rel <= ATTN_REL_L2, (ci, size, max_abs, rel)
+                if size > 0 and len(ctx_lens) * Hkv <= 7:            # the cluster shape is what ran: bits must repeat
+                    for _ in range(4):
+                        assert np.array_equal(first, _run_attn(binding, ctx, pair, 0, Q, q_indptr, Hq, max(q_lens), scale)), (ci, size)
+            assert ctx.poll_status() == 0
+            pair.close()
+    finally:
+        ctx.set_attn_cluster(-1)
