@@ -103,6 +103,13 @@ size_t wf_verify_attn_workspace_bytes(const wf_kv_shape* shape, int B, int n_q_h
  * last launch over the same cache was long enough to be HBM-paced, persistent stream-K ranges over all SMs.
  * 0: never use clusters.  2..16: force that cluster size whenever the pairs fit (else stream-K). */
 int wf_ctx_set_attn_cluster(wf_ctx* ctx, int cluster_size);
+/* Reproducible attention bits.  A (sequence, kv head) pair whose keys are split over several CTAs is merged from partial
+ * (max, sum, O) triples.  on = 0 (default): in the stream-K shape the CTA that arrives last folds the others' partials into
+ * its own, so the order of the floating-point merges (not the tolerance) depends on timing.  on = 1: every merge folds
+ * the partials of a pair in key-range order, whoever arrives last: repeated calls on the same inputs give identical
+ * bits (costs one extra round trip of the last arriver's partial through L2).  The cluster shape and every other call of
+ * this library are order-fixed regardless.  Applies to wf_verify_attn and wf_verify_attn_tree. */
+int wf_ctx_set_deterministic(wf_ctx* ctx, int on);
 
 /* ---- (b) accept + bonus + entropy + route -------------------------------------------------------
  * PAPER.md:65, 75-81 (§3.3.1), 135; readings C1-C9.  Per sequence b (block rows r0..r0+gamma):

@@ -46,7 +46,10 @@ struct AccSample {
 };
 
 template <bool VEC>
-__global__ void __launch_bounds__(ACC_THREADS)
+// 5 CTAs per SM: the sweep keeps a CTA's 32 KB slice in registers, so the bytes in flight per SM are what the register file
+// holds: at the compiler's own 80 registers 3 CTAs fit and the sweep ran at 4.46 TB/s (cfg5), capped at 48 registers 5 CTAs
+// fit: 6.10 TB/s; the rarely executed finalise spills 80 bytes.  (4 CTAs: 5.54 TB/s; 6 CTAs spill inside the sweep: 5.44.)
+__global__ void __launch_bounds__(ACC_THREADS, 5)
 wf_accept_kernel(const float* __restrict__ logits, int V, int n_chunks, const int32_t* __restrict__ draft_tokens,
                  const int32_t* __restrict__ q_indptr, const float* __restrict__ tau, int tau_is_scalar,
                  int32_t* __restrict__ accept_len, int32_t* __restrict__ bonus_token, float* __restrict__ entropy,
@@ -189,7 +192,7 @@ wf_accept_kernel(const float* __restrict__ logits, int V, int n_chunks, const in
   }
   __shared__ int s_row;                                    // the row whose logits give the bonus token and the entropy
   __shared__ int s_par[ACC_MAX_Q], s_tok[ACC_MAX_Q];
-  if (parent && tid < q_b) { s_par[tid] = parent[r0 + tid]; s_tok[tid] = draft_tokens[r0 + tid]; }
+  if (tid < q_b) { s_par[tid] = parent ? parent[r0 + tid] : tid - 1; s_tok[tid] = draft_tokens[r0 + tid]; }   // one round trip for all
   __syncthreads();
   __shared__ float s_M[ACC_MAX_Q];
   __shared__ double s_Z[ACC_MAX_Q];
@@ -236,7 +239,7 @@ wf_accept_kernel(const float* __restrict__ logits, int V, int n_chunks, const in
     if (tid == 0) {                                        // longest accepted prefix (C6)
       const int gamma = q_b - 1;
       int a = 0;
-      while (a < gamma && draft_tokens[r0 + a + 1] == s_g[a]) ++a;
+      while (a < gamma && s_tok[a + 1] == s_g[a]) ++a;
       s_a = a;
       s_row = a;
     }

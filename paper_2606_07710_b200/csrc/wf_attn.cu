@@ -61,6 +61,7 @@ struct AttnParams {
   KvView kv;
   int layer, B, n_q_heads, group;
   int cl;                              // > 0: cluster mode (launched with clusters of `cl` CTAs, one cluster per (b, g) pair)
+  int deterministic;                   // stream-K merges fold the partials of a pair in range order, whoever arrives last
   int ctx_adj;                         // added to seq_len: 0 for verification (the block sits behind the cache length, C10);
                                        // -1 for the final-token path (wf_final.cu: the token is the last cached one, F1)
   float scale_log2;                    // sm_scale * log2(e)
@@ -772,7 +773,26 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared<fal
       }
     };
     auto slot_of = [&](int s2) { return s2 == 0 ? first_slot : 2 * (c_first + s2); };
-    if (!has_next && n_seg > 2) {
+    if (p.deterministic) {
+      // Reproducible bits: the last arriver stores its own partial like everybody else (each thread reads back exactly
+      // what it wrote), starts from the identity and folds ALL partials of the pair in range order 0, 1, ...: the chain of
+      // merges no longer depends on which CTA happened to arrive last.  One more 34 KB round trip through L2.
+      float4* own = p.ws_o + (size_t)sg.slot * (NO / 4) * 128 + stid;
+#pragma unroll
+      for (int k = 0; k < NO / 4; ++k) own[k * 128] = make_float4(o[4 * k], o[4 * k + 1], o[4 * k + 2], o[4 * k + 3]);
+      p.ws_ml[(size_t)sg.slot * 128 + stid] = make_float4(m_run[0], l_run[0], m_run[1], l_run[1]);
+      m_run[0] = m_run[1] = -INFINITY; l_run[0] = l_run[1] = 0.f;
+#pragma unroll
+      for (int c = 0; c < NO; ++c) o[c] = 0.f;
+      for (int s2 = 0; s2 < n_seg; ++s2) {
+        const int slot = slot_of(s2);
+        const float4* src = p.ws_o + (size_t)slot * (NO / 4) * 128 + stid;
+        float4 x[NO / 4];
+#pragma unroll
+        for (int k = 0; k < NO / 4; ++k) x[k] = __ldcg(src + k * 128);
+        fold(x, __ldcg(&p.ws_ml[(size_t)slot * 128 + stid]));
+      }
+    } else if (!has_next && n_seg > 2) {
       // Many partials (small launches cut a pair into up to 32 ranges): folding them one load round trip at a time
       // cost 2.2k cycles each.  This is the CTA's last segment, so its whole shared memory is idle: every thread
       // copies ITS OWN fragments of up to `cap` partials with cp.async (all in flight together), waits for its
@@ -1061,7 +1081,17 @@ __device__ __forceinline__ void attn_softmax_tree(const AttnParams& p, AttnShare
     if (grp == 0 && stid == 0) *cnt = 0;                       // self-resetting for the next launch
     __threadfence();
     const int first_slot = 2 * c_first + ((int)((long long)c_first * T / G) < sg.flat0 ? 1 : 0);
-    const int s_own = (int)blockIdx.x - c_first;
+    int s_own = (int)blockIdx.x - c_first;
+    if (p.deterministic) {                                     // as in the chain kernel: identity, then every partial in range order
+      float4* own = p.ws_o + (size_t)(sg.slot * 2 + grp) * (NO / 4) * 128 + stid;
+#pragma unroll
+      for (int k = 0; k < NO / 4; ++k) own[k * 128] = make_float4(o[4 * k], o[4 * k + 1], o[4 * k + 2], o[4 * k + 3]);
+      p.ws_ml[(size_t)(sg.slot * 2 + grp) * 128 + stid] = make_float4(m_run[0], l_run[0], m_run[1], l_run[1]);
+      m_run[0] = m_run[1] = -INFINITY; l_run[0] = l_run[1] = 0.f;
+#pragma unroll
+      for (int c = 0; c < NO; ++c) o[c] = 0.f;
+      s_own = -1;
+    }
     for (int s2 = 0; s2 < n_seg; ++s2) {
       if (s2 == s_own) continue;
       const int slot = (s2 == 0 ? first_slot : 2 * (c_first + s2)) * 2 + grp;
@@ -1437,6 +1467,7 @@ int wf_attn_launch_chain(wf_ctx* ctx, const wf_paged_kv* kv, int layer, const vo
   p.kv = kv_view(kv);
   p.layer = layer; p.B = B; p.n_q_heads = n_q_heads; p.group = group;
   p.ctx_adj = ctx_adj;
+  p.deterministic = ctx->deterministic;
   p.scale_log2 = sm_scale * LOG2E;
   p.ws_o = (float4*)workspace;
   p.ws_ml = (float4*)((char*)workspace + items * r_pad * kv->s.head_dim * sizeof(float));
@@ -1500,6 +1531,7 @@ extern "C" int wf_verify_attn_tree(wf_ctx* ctx, const wf_paged_kv* kv, int layer
   p.kv = kv_view(kv);
   p.layer = layer; p.B = B; p.n_q_heads = n_q_heads; p.group = group;
   p.ctx_adj = 0;
+  p.deterministic = ctx->deterministic;
   p.scale_log2 = sm_scale * LOG2E;
   p.ws_o = (float4*)workspace;
   p.ws_ml = (float4*)((char*)workspace + items * AT_ROWS * kv->s.head_dim * sizeof(float));
@@ -1517,5 +1549,11 @@ extern "C" int wf_ctx_set_attn_cluster(wf_ctx* ctx, int cluster_size) {
   WF_REQUIRE(ctx, cluster_size >= -1 && cluster_size <= 16 && cluster_size != 1, WF_ERR_INVALID_ARG,
              "wf_ctx_set_attn_cluster: cluster_size must be -1 (automatic), 0 (never) or 2..16");
   ctx->attn_cluster_override = cluster_size;
+  return WF_OK;
+}
+
+extern "C" int wf_ctx_set_deterministic(wf_ctx* ctx, int on) {
+  if (!ctx) return WF_ERR_INVALID_ARG;
+  ctx->deterministic = on ? 1 : 0;
   return WF_OK;
 }

@@ -287,7 +287,7 @@ class RoundState:
                     wf.wf_lazy_catchup_flush(self.ctx, d.handle, m.flush, B, stream)
             else:
                 wf.wf_kv_only_prefill(self.ctx, d.handle, s.hidden, s.q_indptr, n_commit, None, B, self.qmax, stream)
-        if self.ft is not None and mode != "active" and s.masks["A"].flush_host.any():
+        if self.ft is not None and mode != "active":             # every round, as in the device-driven mode (empty calls included)
             self.run_final_token(s, s.masks["A"].flush, 1, stream)
 
     def run_round(self, stream=None, lazy=True, events=None, fused=True, mode=None):

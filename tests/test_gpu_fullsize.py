@@ -114,3 +114,51 @@ def test_tree_attention_full_size_sampled(workload, sample):
     finally:
         rs.close()
         ctx.close()
+
+
+@pytest.mark.parametrize("workload", [2, 4])
+def test_attention_deterministic_mode_repeats_bits(workload):
+    """wf_ctx_set_deterministic(1): the stream-K merges fold a pair's partials in key-range order, whoever arrives last, so
+    five launches at the bench's full-size launch shape (every SM busy, ranges cutting pairs) give IDENTICAL bits, for the
+    chain kernel and for 60-node trees; the result stays within tolerance of the default mode's."""
+    import torch
+    from paper_2606_07710_b200 import binding as wf
+    from paper_2606_07710_b200.rounds import RoundState
+    wl = synth.WORKLOADS[workload]
+    sh = wl.shapes
+    ctx = wf.Ctx(0)
+    rs = RoundState(ctx, wl, n_slots=1, n_rounds_max=8, layers=1, final_token=False)
+    try:
+        s = rs.slots[0]
+        rs.target_kv.reserve(s.add_tokens, rs.B)
+        run = lambda: wf.wf_verify_attn(ctx, rs.target_kv, 0, s.q, s.q_indptr, rs.B, sh.n_q_heads, rs.qmax, rs.sm_scale,
+                                        s.attn_out, rs.attn_ws)
+        run()
+        torch.cuda.synchronize()
+        default = s.attn_out.float().clone()
+        ctx.set_deterministic(True)
+        outs = []
+        for _ in range(5):
+            s.attn_out.zero_()
+            run()
+            torch.cuda.synchronize()
+            outs.append(s.attn_out.view(torch.int16).clone())
+        assert all(torch.equal(outs[0], o) for o in outs[1:])
+        d = s.attn_out.float() - default
+        assert float(d.abs().max()) <= 2e-3 and float((d ** 2).sum().sqrt() / (default ** 2).sum().sqrt()) <= 3e-3
+        # trees
+        t = rs.make_tree_slot(60)
+        rs.target_kv.reserve(t.add_tokens, rs.B)
+        wf.wf_tree_masks(ctx, t.parent, t.q_indptr, rs.B, t.n_nodes, t.masks)
+        outs = []
+        for _ in range(5):
+            t.attn_out.zero_()
+            wf.wf_verify_attn_tree(ctx, rs.target_kv, 0, t.q, t.q_indptr, t.masks, rs.B, sh.n_q_heads, t.n_nodes, rs.sm_scale,
+                                   t.attn_out, t.attn_ws)
+            torch.cuda.synchronize()
+            outs.append(t.attn_out.view(torch.int16).clone())
+        assert all(torch.equal(outs[0], o) for o in outs[1:])
+        assert ctx.poll_status() == 0
+    finally:
+        rs.close()
+        ctx.close()

@@ -150,6 +150,36 @@ def test_sample_8b_vocab_and_cache_length(wf):
     pair.close()
 
 
+def test_sample_full_q_at_8b_vocab(wf):
+    """Full drafter rows at the real vocabulary (V = 151936: 19 slices, ragged last one, two warp levels over 2 x 600 KB per
+    sequence): drafts drawn from q, ratios p/q on both sides of 1, residual draws max(0, p - q), a masked range in both p
+    and q, mixed gamma and an empty block."""
+    binding, ctx = wf
+    g = synth.rng(69, 1)
+    V, T = 151936, 0.8
+    q_lens = [16, 8, 0, 16, 4]
+    ip = np.zeros(len(q_lens) + 1, np.int32)
+    ip[1:] = np.cumsum(q_lens)
+    n = int(ip[-1])
+    logits = synth.normal_f32(g, (n, V), 3.0)
+    rows = np.arange(n)
+    logits[rows, logits.argmax(axis=1)] += np.float32(7.0)      # a winner with a real share of the mass: some drafts pass
+    logits[:, 5000:9000] = -np.inf
+    q = _soft_q(g, np.where(np.isfinite(logits), logits, -1e9), T, 0.9)
+    drafts = np.zeros(n, np.int32)
+    for b in range(len(q_lens)):
+        for j in range(1, q_lens[b]):
+            r = int(ip[b]) + j
+            drafts[r] = spec_sample.inverse_cdf(q[r - 1], g.random())
+    u_acc, u_s = _uniforms(g, n, len(q_lens))
+    want = spec_sample.spec_sample_entropy_route(logits, drafts, ip, T, u_acc, u_s, 2.0, draft_q=q)
+    res = _run(binding, ctx, logits, drafts, ip, T, u_acc, u_s, 2.0, draft_q=q, max_q=16)
+    assert _check(res, want, 2.0) <= 1
+    assert not ((res["token"] >= 5000) & (res["token"] < 9000)).any()
+    assert want["accept_len"].max() >= 1 and (want["accept_len"] < np.maximum(np.array(q_lens) - 1, 0)).any()
+    assert res["n_commit"][2] == 0
+
+
 def test_sample_distribution_of_draws(wf):
     """1024 sequences share one logits row pattern (gamma = 0: pure bonus draws) with stratified uniforms: the
     histogram of emitted tokens must follow p (a wrong CDF order or a dropped segment shows up at once)."""
