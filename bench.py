@@ -353,9 +353,9 @@ def cpu_baseline_and_parity(rs, wl, ctx, wf, n_seq, n_lay):
 
 
 def timed_rounds(rs, n, mode, torch):
-    """n whole rounds with the given catch-up mode; returns (total ms, catch-up ms)."""
-    ev = [{"attn": (torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)),
-           "catchup": (torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))} for _ in range(n)]
+    """n whole rounds with the given catch-up mode; returns (total ms, catch-up ms, final-token ms inside the catch-up)."""
+    mk = lambda: (torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+    ev = [{"attn": mk(), "catchup": mk(), "final": mk()} for _ in range(n)]
     g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     torch.cuda.synchronize()
     g0.record()
@@ -363,7 +363,8 @@ def timed_rounds(rs, n, mode, torch):
         rs.run_round(events=ev[i], mode=mode)
     g1.record()
     torch.cuda.synchronize()
-    return g0.elapsed_time(g1), sum(e["catchup"][0].elapsed_time(e["catchup"][1]) for e in ev)
+    fin = sum(e["final"][0].elapsed_time(e["final"][1]) for e in ev) if (mode == "switch" and rs.ft is not None) else 0.0
+    return g0.elapsed_time(g1), sum(e["catchup"][0].elapsed_time(e["catchup"][1]) for e in ev), fin
 
 
 def measure(ctx, wf, key, args, rank, world, local, main):
@@ -375,10 +376,10 @@ def measure(ctx, wf, key, args, rank, world, local, main):
     sh = wl.shapes
     K, W = (args.steps, max(args.warmup, 3)) if main else (min(args.steps, args.sub_steps), 3)
     e2e_steps = max(1, min(K, args.e2e_steps if main else args.sub_e2e_steps))
-    leg_steps = 8
+    leg_steps = args.slots                                    # one full cycle of the round slots for every catch-up leg
     n_slots = args.slots
-    extra = (10 + n_slots + 20) if main else 0                # tree leg, graph leg
-    rs = RoundState(ctx, wl, n_slots=n_slots, n_rounds_max=W + K + e2e_steps + 2 * leg_steps + 4 + extra, host_copies=True)
+    extra = (10 + n_slots + 20) if (main or key == "cfg2") else 0      # tree leg, graph leg
+    rs = RoundState(ctx, wl, n_slots=n_slots, n_rounds_max=W + K + e2e_steps + 3 * leg_steps + 4 + extra, host_copies=True)
     B, L = rs.B, rs.L
 
     # ---- cpu_baseline + full-size sampled parity (rank 0 of a 1-GPU run only) ----
@@ -481,12 +482,18 @@ def measure(ctx, wf, key, args, rank, world, local, main):
     #               drafting cost, not switching cost): lazy - active = what the switch machinery costs per round ----
     for d in rs.drafters.values():                           # flush what the lazy rounds left queued: complete caches
         wf.wf_lazy_catchup_flush(ctx, d.handle, None, B)
-    eager_ms, eager_catch_ms = timed_rounds(rs, leg_steps, "eager", torch)
-    active_ms, active_catch_ms = timed_rounds(rs, leg_steps, "active", torch)
+    rs.sync_cur()
+    lazy_leg_ms, lazy_leg_catch_ms, lazy_leg_final_ms = timed_rounds(rs, leg_steps, "switch", torch)      # the same slots for all three legs
+    for d in rs.drafters.values():
+        wf.wf_lazy_catchup_flush(ctx, d.handle, None, B)
+    rs.rounds_done -= leg_steps
+    eager_ms, eager_catch_ms, _ = timed_rounds(rs, leg_steps, "eager", torch)
+    rs.rounds_done -= leg_steps
+    active_ms, active_catch_ms, _ = timed_rounds(rs, leg_steps, "active", torch)
     rs.check_plan(rs.slots[(rs.rounds_done - 1) % rs.n_slots], switched=False)
     rs.sync_cur()
-    lazy_us, eager_us, active_us = 1e3 * catch_ms / K, 1e3 * eager_catch_ms / leg_steps, 1e3 * active_catch_ms / leg_steps
-    final_us = 1e3 * final_ms / K
+    lazy_us, eager_us, active_us = 1e3 * lazy_leg_catch_ms / leg_steps, 1e3 * eager_catch_ms / leg_steps, 1e3 * active_catch_ms / leg_steps
+    final_us = 1e3 * lazy_leg_final_ms / leg_steps
     round_us = 1e3 * ms_local / K
 
     # ---- (f3) the final backlog token in full, on its own: back-to-back calls for the sequences slot `s` switches to the
@@ -538,8 +545,9 @@ def measure(ctx, wf, key, args, rank, world, local, main):
                     "final_token_us_per_round": final_us, "flush_us_per_round": lazy_us - final_us,
                     "switch_us_per_round": lazy_us - active_us, "share_of_round": lazy_us / round_us,
                     "switch_share_of_round": (lazy_us - active_us) / round_us, "eager_share_of_round": eager_catch_ms / eager_ms,
-                    "eager_rounds_per_s": leg_steps / (eager_ms * 1e-3), "leg_steps": leg_steps,
-                    "note": "lazy = wf_switch_round inside the timed rounds; eager = KV-only prefill into both drafters every round "
+                    "eager_rounds_per_s": leg_steps / (eager_ms * 1e-3), "lazy_rounds_per_s": leg_steps / (lazy_leg_ms * 1e-3),
+                    "leg_steps": leg_steps,
+                    "note": "three legs over the same full cycle of round slots; lazy = wf_switch_round (+ final token); eager = KV-only prefill into both drafters every round "
                             "(Lazy Catch-up off, PAPER.md Table 3 baseline); active_append = only the active drafter's own append "
                             "(reading C22: drafting cost, not switching cost); switch = lazy - active_append (derived); "
                             "final_token = wf_final_token_full for the sequences that switched to the AR drafter (PAPER.md:119), "
@@ -560,11 +568,13 @@ def measure(ctx, wf, key, args, rank, world, local, main):
         rec["parity_sample"] = parity
     if main:
         rec.update(side_legs(rs, ctx, wf, wl, args, s, peak, torch))
+    elif key == "cfg2":                                      # batch 1 is launch-paced: the graph replay is its B200-native form
+        rec.update(side_legs(rs, ctx, wf, wl, args, s, peak, torch, only_graph=True))
     rs.close()
     return rec
 
 
-def side_legs(rs, ctx, wf, wl, args, s, peak, torch):
+def side_legs(rs, ctx, wf, wl, args, s, peak, torch, only_graph=False):
     """Legs timed on their own after the headline region: graph replay, neural router, stochastic acceptance, tree verify."""
     sh, B, L = rs.sh, rs.B, rs.L
     out = {}
@@ -599,6 +609,8 @@ def side_legs(rs, ctx, wf, wl, args, s, peak, torch):
         out["graph_replay"] = {"error": f"{type(e).__name__}: {e}"[:200]}
         torch.cuda.synchronize()
 
+    if only_graph:
+        return out
     # ---- WhiFlash-Neural router, timed on its own: the round above uses the entropy policy ----
     n0, n1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     for _ in range(3):
@@ -702,7 +714,7 @@ def run_ours(args):
         torch.cuda.empty_cache()
         sub = measure(ctx, wf, key, args, rank, world, local, main=False)
         keep = ("value", "unit", "steps", "ms_per_step", "kv_read_gbs", "attn_share_of_round", "catchup", "final_token", "roofline", "e2e",
-                "clocks", "cpu_baseline", "parity_sample", "committed_tokens_per_s", "gpu_launches")
+                "clocks", "cpu_baseline", "parity_sample", "committed_tokens_per_s", "gpu_launches", "graph_replay")
         per_config[key] = {k: sub[k] for k in keep if k in sub}
         per_config[key]["workload"] = sub["config"]["workload"]
         per_config[key]["realised_switch_rate"] = sub["run_notes"]["realised_switch_rate"]

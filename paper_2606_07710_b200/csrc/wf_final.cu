@@ -35,6 +35,7 @@ constexpr int FT_MAX_TOK = 256;          // tokens per call = UMMA N (one pass)
 constexpr int FT_BOX = 32;               // token rows per TMA box of the X operand
 constexpr int FT_SMEM = 200 * 1024;
 constexpr int FT_MAX_STAGES = 12;
+constexpr int FT_W_PRE = 4;               // weight stages prefetched ahead of the dependency wait (128 KB)
 constexpr int FT_W_SUB = FT_BK * FT_TILE * 2;        // one k-block of a W tile: 2 column halves x [64 k][128 B] = 16 KB
 constexpr int FT_W_BYTES = FT_KSUB * FT_W_SUB;       // one W stage, contiguous in the packed image
 constexpr int FT_PLAN_THREADS = 256;
@@ -154,84 +155,115 @@ __device__ __forceinline__ float gelu_tanh(float u) {
 template <int EPI>
 __global__ void __launch_bounds__(FT_THREADS, 1) wf_final_gemm_kernel(const __grid_constant__ FtGemmParams p) {
   extern __shared__ __align__(1024) uint8_t smem[];
-  __shared__ __align__(8) uint64_t s_full[FT_MAX_STAGES], s_empty[FT_MAX_STAGES], s_acc_full;
+  // Two rings, as in the KV-only projection (wf_prefill.cu): W stages at offset 0, the first FT_W_PRE of them filled BEFORE
+  // the dependency wait (the weights are constants; under programmatic dependent launch the head of this kernel's weight
+  // stream overlaps the tail of the kernel that produces its activations), then the X ring, sized by the call's tokens.
+  __shared__ __align__(8) uint64_t w_full[FT_MAX_STAGES], w_empty[FT_MAX_STAGES], x_full[FT_MAX_STAGES], x_empty[FT_MAX_STAGES], s_acc_full;
   __shared__ uint32_t s_tmem;
   __shared__ int s_last;
 
   wf_pdl_trigger();
-  wf_pdl_wait();
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int M = min(*p.m_total, p.m_cap);
-  if (M == 0) return;                                         // nobody switched: no barriers, no TMEM
   const int tile = (int)blockIdx.x / p.n_split, split = (int)blockIdx.x % p.n_split;
   const int tiles_n = p.N / FT_TILE;
   const int layer = tile / tiles_n, nt = tile % tiles_n;
   const int n_kb_tile = p.K / (FT_KSUB * FT_BK);
   const int n_kb = n_kb_tile / p.n_split, kb0 = split * n_kb;
-  const int n_box = (M + FT_BOX - 1) / FT_BOX;
-  const int x_sub = n_box * FT_BOX * 128;                     // one 64-wide k-block of the X operand (whole boxes)
-  const int x_stage = FT_KSUB * x_sub;
-  const int n_stages = min(FT_MAX_STAGES, FT_SMEM / (x_stage + FT_W_BYTES));
-  uint8_t* x_base = smem;
-  uint8_t* w_base = smem + (size_t)n_stages * x_stage;        // 1024-aligned: x_stage is a multiple of 4096
-
+  const int n_pre = min(n_kb, FT_W_PRE);
   if (tid == 0) {
-    for (int i = 0; i < n_stages; ++i) { mbar_init(smem_u32(&s_full[i]), 1); mbar_init(smem_u32(&s_empty[i]), 1); }
+    for (int i = 0; i < FT_MAX_STAGES; ++i) {
+      mbar_init(smem_u32(&w_full[i]), 1); mbar_init(smem_u32(&w_empty[i]), 1);
+      mbar_init(smem_u32(&x_full[i]), 1); mbar_init(smem_u32(&x_empty[i]), 1);
+    }
     mbar_init(smem_u32(&s_acc_full), 1);
     fence_barrier_init();
   }
   if (warp == 1) tmem_alloc(smem_u32(&s_tmem), FT_MAX_TOK);
+  if (warp == 0 && lane == 0) asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(p.xmap)) : "memory");
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = s_tmem;
+  const uint8_t* w_tile = p.wpack + ((size_t)tile * n_kb_tile + kb0) * FT_W_BYTES;
+  if (warp == 0 && elect_one()) {
+    for (int s2 = 0; s2 < n_pre; ++s2) {
+      mbar_arrive_expect_tx(smem_u32(&w_full[s2]), FT_W_BYTES);
+      bulk_load(smem_u32(smem) + s2 * FT_W_BYTES, w_tile + (size_t)s2 * FT_W_BYTES, FT_W_BYTES, smem_u32(&w_full[s2]));
+    }
+  }
+  __syncwarp();
+  wf_pdl_wait();
+  const int M = min(*p.m_total, p.m_cap);
+  if (M == 0) {
+    // nobody switched: let the prefetched stages land (shared memory must outlive the copies), return the TMEM columns
+    if (warp == 0) for (int s2 = 0; s2 < n_pre; ++s2) mbar_wait(smem_u32(&w_full[s2]), 0);
+    if (warp == 1) tmem_dealloc(tmem_base, FT_MAX_TOK);
+    return;
+  }
+  const int n_box = (M + FT_BOX - 1) / FT_BOX;
+  const int x_sub = n_box * FT_BOX * 128;                     // one 64-wide k-block of the X operand (whole boxes)
+  const int x_stage = FT_KSUB * x_sub;
+  const int n_sw = (FT_SMEM - (FT_W_PRE + 1) * FT_W_BYTES) >= 2 * x_stage ? FT_W_PRE + 1 : FT_W_PRE;
+  const int n_sx = max(1, min(FT_MAX_STAGES, (FT_SMEM - n_sw * FT_W_BYTES) / x_stage));
+  uint8_t* w_base = smem;
+  uint8_t* x_base = smem + (size_t)n_sw * FT_W_BYTES;
 
   if (warp == 0) {
     // ===== producer: per stage one bulk copy of the W image and n_box TMA boxes per X k-block =====
-    const uint8_t* w_kb = p.wpack + ((size_t)tile * n_kb_tile + kb0) * FT_W_BYTES;
-    const uint32_t full0 = smem_u32(&s_full[0]), empty0 = smem_u32(&s_empty[0]);
+    const uint8_t* w_kb = w_tile;
+    const uint32_t wf0 = smem_u32(&w_full[0]), we0 = smem_u32(&w_empty[0]), xf0 = smem_u32(&x_full[0]), xe0 = smem_u32(&x_empty[0]);
     const uint32_t x0 = smem_u32(x_base), w0 = smem_u32(w_base);
     const int row0 = p.x_per_layer ? layer * p.m_cap : 0;
-    int s = 0;
-    uint32_t ph = 1;
+    int sw = 0, sx = 0;
+    uint32_t phw = 1, phx = 1;
     for (int kb = 0; kb < n_kb; ++kb) {
-      mbar_wait(empty0 + 8 * s, ph);
+      if (kb >= n_pre) {
+        mbar_wait(we0 + 8 * sw, phw);
+        if (elect_one()) {
+          mbar_arrive_expect_tx(wf0 + 8 * sw, FT_W_BYTES);
+          bulk_load(w0 + sw * FT_W_BYTES, w_kb, FT_W_BYTES, wf0 + 8 * sw);
+        }
+      }
+      mbar_wait(xe0 + 8 * sx, phx);
       if (elect_one()) {
-        const uint32_t bar = full0 + 8 * s;
-        mbar_arrive_expect_tx(bar, FT_W_BYTES + FT_KSUB * x_sub);
-        bulk_load(w0 + s * FT_W_BYTES, w_kb, FT_W_BYTES, bar);
+        const uint32_t bar = xf0 + 8 * sx;
+        mbar_arrive_expect_tx(bar, FT_KSUB * x_sub);
         for (int u = 0; u < FT_KSUB; ++u)
           for (int bx = 0; bx < n_box; ++bx)
-            tma_load_2d(x0 + s * x_stage + u * x_sub + bx * (FT_BOX * 128), p.xmap, ((kb0 + kb) * FT_KSUB + u) * FT_BK,
+            tma_load_2d(x0 + sx * x_stage + u * x_sub + bx * (FT_BOX * 128), p.xmap, ((kb0 + kb) * FT_KSUB + u) * FT_BK,
                         row0 + bx * FT_BOX, bar);
       }
       __syncwarp();
       w_kb += FT_W_BYTES;
-      if (++s == n_stages) { s = 0; ph ^= 1; }
+      if (++sw == n_sw) { sw = 0; phw ^= 1; }
+      if (++sx == n_sx) { sx = 0; phx ^= 1; }
     }
   } else if (warp == 1) {
     // ===== MMA issuer: A = W tile (MN-major), B = X rows (K-major), D[128 columns x tokens] in TMEM =====
     const uint64_t dw0 = umma_desc(smem_u32(w_base), 8192, 1024);
     const uint64_t dx0 = umma_desc(smem_u32(x_base), 16, 1024);
-    const uint32_t full0 = smem_u32(&s_full[0]), empty0 = smem_u32(&s_empty[0]);
+    const uint32_t wf0 = smem_u32(&w_full[0]), we0 = smem_u32(&w_empty[0]), xf0 = smem_u32(&x_full[0]), xe0 = smem_u32(&x_empty[0]);
     const uint64_t dw_step = (uint64_t)(FT_W_BYTES >> 4), dx_step = (uint64_t)(x_stage >> 4);
     const uint32_t idesc = umma_idesc_mn_k(128, (M + 15) & ~15);
-    int s = 0;
-    uint32_t ph = 0;
+    int sw = 0, sx = 0;
+    uint32_t phw = 0, phx = 0;
     uint64_t dw = dw0, dx = dx0;
     for (int kb = 0; kb < n_kb; ++kb) {
-      mbar_wait(full0 + 8 * s, ph);
+      mbar_wait(wf0 + 8 * sw, phw);
+      mbar_wait(xf0 + 8 * sx, phx);
       tc_fence_after();
       if (elect_one()) {
 #pragma unroll
         for (int k16 = 0; k16 < FT_KSUB * FT_BK / 16; ++k16)
           umma_bf16(tmem_base, dw + (uint64_t)(((k16 >> 2) * FT_W_SUB + (k16 & 3) * 2048) >> 4),
                     dx + (uint64_t)(((k16 >> 2) * x_sub + (k16 & 3) * 32) >> 4), idesc, (kb | k16) != 0);
-        umma_commit(empty0 + 8 * s);
+        umma_commit(we0 + 8 * sw);
+        umma_commit(xe0 + 8 * sx);
       }
       __syncwarp();
       dw += dw_step; dx += dx_step;
-      if (++s == n_stages) { s = 0; ph ^= 1; dw = dw0; dx = dx0; }
+      if (++sw == n_sw) { sw = 0; phw ^= 1; dw = dw0; }
+      if (++sx == n_sx) { sx = 0; phx ^= 1; dx = dx0; }
     }
     if (elect_one()) umma_commit(smem_u32(&s_acc_full));
     __syncwarp();

@@ -35,6 +35,9 @@ constexpr int PF_KSUB = 2;              // 64-wide k-blocks per pipeline stage: 
 constexpr int PF_MAX_MT = 2;            // m-tiles per pass (TMEM columns = PF_MAX_MT * D)
 constexpr int PF_THREADS = 192;         // warp 0: bulk-copy producer, warp 1: MMA, warps 2-5: epilogue (+ enqueue, commit)
 constexpr int PF_SMEM_BUDGET = 200 * 1024;
+constexpr int PF_SMEM_LAUNCH = PF_SMEM_BUDGET + 1024;   // UMMA reads n_pad (multiple of 16) rows of an X stage that holds a
+                                                        // multiple of 8: the last stage's surplus rows lie behind the ring
+constexpr int PF_W_PRE_BYTES = 128 * 1024;   // weight stages that are prefetched ahead of the dependency wait
 constexpr int PP_THREADS = 256;         // plan + pack kernel
 constexpr int PP_MAX_B = KV_RESERVE_SMEM;   // sequences per call (the per-sequence plan lives in shared memory)
 constexpr int PP_MAX_PACK_CTAS = 296;   // pack CTAs per drafter: two per SM
@@ -293,17 +296,55 @@ __global__ void __launch_bounds__(PF_THREADS, 1) wf_prefill_gemm_kernel(const __
   constexpr int N_MAX = PF_MAX_MT * PF_BLOCK_M;           // tokens per pass (TMEM columns)
   constexpr uint32_t TMEM_COLS = N_MAX;                   // 256: a power of two >= 32
   extern __shared__ __align__(1024) uint8_t smem[];
-  __shared__ __align__(8) uint64_t s_full[PF_MAX_STAGES], s_empty[PF_MAX_STAGES], s_acc_full, s_acc_empty;
+  // Two rings: W stages (32 KB at D = 128, contiguous in the packed image) and X stages (the call's rows, size known only
+  // after the dependency wait).  The W ring sits at offset 0 with a depth that is fixed for its first PF_W_PRE slots
+  // whatever the call's row count turns out to be, so those slots are filled BEFORE griddepcontrol.wait: the weights are
+  // constants, and under programmatic dependent launch this kernel's CTAs are resident while the plan + pack kernel (a few
+  // small CTAs) still runs: the head of the weight stream (all of it for a 1-layer drafter) overlaps the predecessor.
+  __shared__ __align__(8) uint64_t w_full[PF_MAX_STAGES], w_empty[PF_MAX_STAGES], x_full[PF_MAX_STAGES], x_empty[PF_MAX_STAGES],
+      s_acc_full, s_acc_empty;
   __shared__ uint32_t s_tmem;
   __shared__ int s_last;
+  constexpr int W_PRE = PF_W_PRE_BYTES / W_BYTES;          // W slots valid under every layout
 
   wf_pdl_trigger();
-  wf_pdl_wait();
   const int jb = (int)blockIdx.x >= gp.ctas_job0 ? 1 : 0;
   const GemmJob& p = gp.job[jb];
   const int cta = (int)blockIdx.x - (jb ? gp.ctas_job0 : 0);
   const int n_ctas = jb ? (int)gridDim.x - gp.ctas_job0 : gp.ctas_job0;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int tile = cta / p.n_split;                    // (layer, K|V, kv head)
+  const int split = cta % p.n_split;                   // this CTA's share of the k-blocks
+  const int layer = tile / (2 * p.n_kv_heads);
+  const int is_v = (tile / p.n_kv_heads) & 1;
+  const int head = tile % p.n_kv_heads;
+  const int n_kb_tile = p.hidden / (PF_KSUB * PF_BLOCK_K);   // pipeline stages of a whole tile
+  const int n_kb = n_kb_tile / p.n_split;                    // stages this CTA runs per pass (n_split divides them)
+  const int kb0 = split * n_kb;
+  const int n_pre = min(n_kb, W_PRE);
+  if (tid == 0) {
+    for (int i = 0; i < PF_MAX_STAGES; ++i) {
+      mbar_init(smem_u32(&w_full[i]), 1); mbar_init(smem_u32(&w_empty[i]), 1);
+      mbar_init(smem_u32(&x_full[i]), 1); mbar_init(smem_u32(&x_empty[i]), 1);
+    }
+    mbar_init(smem_u32(&s_acc_full), 1);
+    mbar_init(smem_u32(&s_acc_empty), 128);
+    fence_barrier_init();
+  }
+  if (warp == 1) tmem_alloc(smem_u32(&s_tmem), TMEM_COLS);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = s_tmem;
+  const uint8_t* w_tile = p.wpack + ((size_t)tile * n_kb_tile + kb0) * W_BYTES;   // tile = (layer, K|V, head), packed in that order
+  if (warp == 0 && elect_one()) {
+    for (int s2 = 0; s2 < n_pre; ++s2) {
+      mbar_arrive_expect_tx(smem_u32(&w_full[s2]), W_BYTES);
+      bulk_load(smem_u32(smem) + s2 * W_BYTES, w_tile + (size_t)s2 * W_BYTES, W_BYTES, smem_u32(&w_full[s2]));
+    }
+  }
+  __syncwarp();
+  wf_pdl_wait();
   const int M = *p.m_total;
 
   // Enqueue and commit ride on this kernel (kernel 1 has packed the projection's operand, backlog rows included, so
@@ -337,74 +378,64 @@ __global__ void __launch_bounds__(PF_THREADS, 1) wf_prefill_gemm_kernel(const __
         }
     }
   };
-  if (M == 0) {                                        // nothing to project for this drafter: no barriers, no TMEM
+  const int n_pass = (M + N_MAX - 1) / N_MAX;
+  if (M == 0) {
+    // nothing to project for this drafter: let the prefetched weight stages land (the CTA's shared memory must outlive the
+    // copies), give the TMEM columns back, do the enqueue / commit work and leave
+    if (warp == 0) for (int s2 = 0; s2 < n_pre; ++s2) mbar_wait(smem_u32(&w_full[s2]), 0);
+    if (warp == 1) tmem_dealloc(tmem_base, TMEM_COLS);
     enqueue_commit(tid, PF_THREADS);
     return;
   }
-  const int tile = cta / p.n_split;                    // (layer, K|V, kv head)
-  const int split = cta % p.n_split;                   // this CTA's share of the k-blocks
-  const int layer = tile / (2 * p.n_kv_heads);
-  const int is_v = (tile / p.n_kv_heads) & 1;
-  const int head = tile % p.n_kv_heads;
-  const int n_kb_tile = p.hidden / (PF_KSUB * PF_BLOCK_K);   // pipeline stages of a whole tile
-  const int n_kb = n_kb_tile / p.n_split;                    // stages this CTA runs per pass (n_split divides them)
-  const int kb0 = split * n_kb;
-  const int n_pass = (M + N_MAX - 1) / N_MAX;
 
   // An X stage holds only the rows that exist (8-row swizzle atoms); UMMA reads n_pad (multiple of 16) rows from
-  // its start, the few surplus rows feed accumulator columns nobody reads.
+  // its start, the few surplus rows feed accumulator columns nobody reads.  Layout: W ring (n_sw stages) | X ring (n_sx).
   const int m_first = min(M, N_MAX);
   const int x_sub = ((m_first + 7) / 8) * 1024;          // one 64-wide k-block of the X operand
   const int x_stage = PF_KSUB * x_sub;
-  const int n_stages = min(PF_MAX_STAGES, PF_SMEM_BUDGET / (x_stage + W_BYTES));
-  uint8_t* x_base = smem;
-  uint8_t* w_base = smem + (size_t)n_stages * x_stage;     // 1024-aligned: x_stage is a multiple of 1024
-
-  if (tid == 0) {
-    for (int i = 0; i < n_stages; ++i) { mbar_init(smem_u32(&s_full[i]), 1); mbar_init(smem_u32(&s_empty[i]), 1); }
-    mbar_init(smem_u32(&s_acc_full), 1);
-    mbar_init(smem_u32(&s_acc_empty), 128);
-    fence_barrier_init();
-  }
-  if (warp == 1) tmem_alloc(smem_u32(&s_tmem), TMEM_COLS);
-  tc_fence_before();
-  __syncthreads();
-  tc_fence_after();
-  const uint32_t tmem_base = s_tmem;
+  const int n_sw = (PF_SMEM_BUDGET - PF_W_PRE_BYTES - W_BYTES) >= 2 * x_stage ? W_PRE + 1 : W_PRE;
+  const int n_sx = max(1, min(PF_MAX_STAGES, (PF_SMEM_BUDGET - n_sw * W_BYTES) / x_stage));
+  uint8_t* w_base = smem;
+  uint8_t* x_base = smem + (size_t)n_sw * W_BYTES;         // 1024-aligned: W_BYTES is a multiple of 1024
 
   if (warp == 0) {
     // ===== bulk-copy producer: per stage ONE contiguous copy of the pre-swizzled W k-blocks and one per packed X
-    //       k-block (wf_pack_x_kernel): no thread touches operand bytes.  Stage index, phase and addresses advance
+    //       k-block (wf_plan_pack_kernel): no thread touches operand bytes.  Stage indices, phases and addresses advance
     //       incrementally: a runtime division per stage in a one-thread loop costs more than the MMAs it feeds.
     //       The whole warp runs the loop (warp-uniform control flow) and one elected lane issues: ptxas then emits
     //       straight-line UBLKCP / UTCHMMA instead of a divergence loop around every instruction. =====
     {
-      const uint8_t* w_src = p.wpack + ((size_t)tile * n_kb_tile + kb0) * W_BYTES;   // tile = (layer, K|V, head), packed in that order
       const size_t x_kb_stride = (size_t)((M + 7) & ~7) * 128;
-      const uint32_t full0 = smem_u32(&s_full[0]), empty0 = smem_u32(&s_empty[0]);
+      const uint32_t wf0 = smem_u32(&w_full[0]), we0 = smem_u32(&w_empty[0]), xf0 = smem_u32(&x_full[0]), xe0 = smem_u32(&x_empty[0]);
       const uint32_t x0 = smem_u32(x_base), w0 = smem_u32(w_base);
-      int s = 0;
-      uint32_t ph = 1;                                   // parity to wait for on s_empty: the ring starts empty
+      int sw = 0, sx = 0, kw = 0;                        // W slot, X slot, W stages issued so far (the first n_pre are in flight)
+      uint32_t phw = 1, phx = 1;                         // parities to wait for on the empty barriers: the rings start empty
       for (int pass = 0; pass < n_pass; ++pass) {
         const int rows_here = min(M - pass * N_MAX, N_MAX);
         const uint32_t x_bytes = (uint32_t)((rows_here + 7) / 8) * 1024;
         const uint8_t* x_src = p.xpack + (size_t)pass * N_MAX * 128 + (size_t)kb0 * PF_KSUB * x_kb_stride;
-        const uint8_t* w_kb = w_src;
-        // the epilogue of the previous pass transposes through the ring: do not refill it before it is done
+        const uint8_t* w_kb = w_tile;
+        // the epilogue of the previous pass transposes through the rings: do not refill them before it is done
         if (pass > 0) mbar_wait(smem_u32(&s_acc_empty), (pass - 1) & 1);
-        for (int kb = 0; kb < n_kb; ++kb) {
-          mbar_wait(empty0 + 8 * s, ph);
+        for (int kb = 0; kb < n_kb; ++kb, ++kw) {
+          if (kw >= n_pre) {
+            mbar_wait(we0 + 8 * sw, phw);
+            if (elect_one()) {
+              mbar_arrive_expect_tx(wf0 + 8 * sw, W_BYTES);
+              bulk_load(w0 + sw * W_BYTES, w_kb, W_BYTES, wf0 + 8 * sw);
+            }
+          }
+          mbar_wait(xe0 + 8 * sx, phx);
           if (elect_one()) {
-            const uint32_t bar = full0 + 8 * s;
-            mbar_arrive_expect_tx(bar, W_BYTES + PF_KSUB * x_bytes);
-            bulk_load(w0 + s * W_BYTES, w_kb, W_BYTES, bar);
+            mbar_arrive_expect_tx(xf0 + 8 * sx, PF_KSUB * x_bytes);
 #pragma unroll
-            for (int u = 0; u < PF_KSUB; ++u) bulk_load(x0 + s * x_stage + u * x_sub, x_src + u * x_kb_stride, x_bytes, bar);
+            for (int u = 0; u < PF_KSUB; ++u) bulk_load(x0 + sx * x_stage + u * x_sub, x_src + u * x_kb_stride, x_bytes, xf0 + 8 * sx);
           }
           __syncwarp();
           w_kb += W_BYTES;
           x_src += PF_KSUB * x_kb_stride;
-          if (++s == n_stages) { s = 0; ph ^= 1; }
+          if (++sw == n_sw) { sw = 0; phw ^= 1; }
+          if (++sx == n_sx) { sx = 0; phx ^= 1; }
         }
       }
     }
@@ -414,17 +445,18 @@ __global__ void __launch_bounds__(PF_THREADS, 1) wf_prefill_gemm_kernel(const __
     {
       const uint64_t dw0 = umma_desc(smem_u32(w_base), 8192, 1024);        // MN-major: 64-column halves 8 KB apart
       const uint64_t dx0 = umma_desc(smem_u32(x_base), 16, 1024);          // K-major
-      const uint32_t full0 = smem_u32(&s_full[0]), empty0 = smem_u32(&s_empty[0]);
+      const uint32_t wf0 = smem_u32(&w_full[0]), we0 = smem_u32(&w_empty[0]), xf0 = smem_u32(&x_full[0]), xe0 = smem_u32(&x_empty[0]);
       const uint64_t dw_step = (uint64_t)(W_BYTES >> 4), dx_step = (uint64_t)(x_stage >> 4);
-      int s = 0;
-      uint32_t ph = 0;
+      int sw = 0, sx = 0;
+      uint32_t phw = 0, phx = 0;
       uint64_t dw = dw0, dx = dx0;
       for (int pass = 0; pass < n_pass; ++pass) {
         const int rows_here = min(M - pass * N_MAX, N_MAX);
         const uint32_t idesc = umma_idesc_mn_k(128, (rows_here + 15) & ~15);
         if (pass > 0) { mbar_wait(smem_u32(&s_acc_empty), (pass - 1) & 1); tc_fence_after(); }
         for (int kb = 0; kb < n_kb; ++kb) {
-          mbar_wait(full0 + 8 * s, ph);
+          mbar_wait(wf0 + 8 * sw, phw);
+          mbar_wait(xf0 + 8 * sx, phx);
           tc_fence_after();
           if (elect_one()) {
           // k16 step j of the stage: W k-block j/4 (W_SUB apart), 16 k-rows = 2 KB per step; X k-block j/4 (x_sub apart),
@@ -433,11 +465,13 @@ __global__ void __launch_bounds__(PF_THREADS, 1) wf_prefill_gemm_kernel(const __
           for (int k16 = 0; k16 < PF_KSUB * PF_BLOCK_K / 16; ++k16)
             umma_bf16(tmem_base, dw + (uint64_t)(((k16 >> 2) * W_SUB + (k16 & 3) * 2048) >> 4),
                       dx + (uint64_t)(((k16 >> 2) * x_sub + (k16 & 3) * 32) >> 4), idesc, (kb | k16) != 0);
-          umma_commit(empty0 + 8 * s);                   // frees the stage when these MMAs retire
+          umma_commit(we0 + 8 * sw);                     // frees the stages when these MMAs retire
+          umma_commit(xe0 + 8 * sx);
           }
           __syncwarp();
           dw += dw_step; dx += dx_step;
-          if (++s == n_stages) { s = 0; ph ^= 1; dw = dw0; dx = dx0; }
+          if (++sw == n_sw) { sw = 0; phw ^= 1; dw = dw0; }
+          if (++sx == n_sx) { sx = 0; phx ^= 1; dx = dx0; }
         }
         if (elect_one()) umma_commit(smem_u32(&s_acc_full));
         __syncwarp();
@@ -628,11 +662,11 @@ int run_jobs(wf_ctx* ctx, CallJob* jobs, int n_jobs, const int32_t* route, int32
   int rc = wf_check_launch(ctx, "wf_plan_pack_kernel");
   if (rc != WF_OK) return rc;
   if (D == 128) {
-    WF_CONFIGURE_ONCE(ctx, WF_FUNC_GEMM_128, wf_prefill_gemm_kernel<128>, PF_SMEM_BUDGET);
-    wf_launch(wf_prefill_gemm_kernel<128>, dim3(gemm_grid), dim3(PF_THREADS), PF_SMEM_BUDGET, st, gp);
+    WF_CONFIGURE_ONCE(ctx, WF_FUNC_GEMM_128, wf_prefill_gemm_kernel<128>, PF_SMEM_LAUNCH);
+    wf_launch(wf_prefill_gemm_kernel<128>, dim3(gemm_grid), dim3(PF_THREADS), PF_SMEM_LAUNCH, st, gp);
   } else {
-    WF_CONFIGURE_ONCE(ctx, WF_FUNC_GEMM_64, wf_prefill_gemm_kernel<64>, PF_SMEM_BUDGET);
-    wf_launch(wf_prefill_gemm_kernel<64>, dim3(gemm_grid), dim3(PF_THREADS), PF_SMEM_BUDGET, st, gp);
+    WF_CONFIGURE_ONCE(ctx, WF_FUNC_GEMM_64, wf_prefill_gemm_kernel<64>, PF_SMEM_LAUNCH);
+    wf_launch(wf_prefill_gemm_kernel<64>, dim3(gemm_grid), dim3(PF_THREADS), PF_SMEM_LAUNCH, st, gp);
   }
   return wf_check_launch(ctx, "wf_prefill_gemm_kernel");
 }
