@@ -363,7 +363,7 @@ def timed_rounds(rs, n, mode, torch):
         rs.run_round(events=ev[i], mode=mode)
     g1.record()
     torch.cuda.synchronize()
-    fin = sum(e["final"][0].elapsed_time(e["final"][1]) for e in ev) if (mode == "switch" and rs.ft is not None) else 0.0
+    fin = sum(e["final"][0].elapsed_time(e["final"][1]) for e in ev) if (mode != "active" and rs.ft is not None) else 0.0
     return g0.elapsed_time(g1), sum(e["catchup"][0].elapsed_time(e["catchup"][1]) for e in ev), fin
 
 
@@ -487,7 +487,7 @@ def measure(ctx, wf, key, args, rank, world, local, main):
     for d in rs.drafters.values():
         wf.wf_lazy_catchup_flush(ctx, d.handle, None, B)
     rs.rounds_done -= leg_steps
-    eager_ms, eager_catch_ms, _ = timed_rounds(rs, leg_steps, "eager", torch)
+    eager_ms, eager_catch_ms, eager_final_ms = timed_rounds(rs, leg_steps, "eager", torch)
     rs.rounds_done -= leg_steps
     active_ms, active_catch_ms, _ = timed_rounds(rs, leg_steps, "active", torch)
     rs.check_plan(rs.slots[(rs.rounds_done - 1) % rs.n_slots], switched=False)
@@ -543,6 +543,7 @@ def measure(ctx, wf, key, args, rank, world, local, main):
         "catchup_share_of_round": catch_ms / ms_local,
         "catchup": {"lazy_us_per_round": lazy_us, "eager_us_per_round": eager_us, "active_append_us_per_round": active_us,
                     "final_token_us_per_round": final_us, "flush_us_per_round": lazy_us - final_us,
+                    "eager_kv_us_per_round": eager_us - 1e3 * eager_final_ms / leg_steps,
                     "switch_us_per_round": lazy_us - active_us, "share_of_round": lazy_us / round_us,
                     "switch_share_of_round": (lazy_us - active_us) / round_us, "eager_share_of_round": eager_catch_ms / eager_ms,
                     "eager_rounds_per_s": leg_steps / (eager_ms * 1e-3), "lazy_rounds_per_s": leg_steps / (lazy_leg_ms * 1e-3),
@@ -551,7 +552,8 @@ def measure(ctx, wf, key, args, rank, world, local, main):
                             "(Lazy Catch-up off, PAPER.md Table 3 baseline); active_append = only the active drafter's own append "
                             "(reading C22: drafting cost, not switching cost); switch = lazy - active_append (derived); "
                             "final_token = wf_final_token_full for the sequences that switched to the AR drafter (PAPER.md:119), "
-                            "inside lazy and eager alike; flush = lazy - final_token"},
+                            "inside lazy and eager alike; flush = lazy - final_token is what Lazy Catch-up costs per round and "
+                            "eager_kv = eager - its final token what the naive scheme costs (PAPER.md Table 3)"},
         "roofline": {"bound": "hbm", "kernel": "wf_verify_attn_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
                      "frac": achieved / peak, "peak_source": peak_src, "traffic": traffic, "traffic_source": traffic_src,
                      "algorithmic_bytes_per_launch": float(np.mean(attn_bytes)), "avg_launch_us": 1e3 * avg_launch_ms},

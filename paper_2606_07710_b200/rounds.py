@@ -288,7 +288,11 @@ class RoundState:
             else:
                 wf.wf_kv_only_prefill(self.ctx, d.handle, s.hidden, s.q_indptr, n_commit, None, B, self.qmax, stream)
         if self.ft is not None and mode != "active":             # every round, as in the device-driven mode (empty calls included)
+            if events:
+                events["final"][0].record()
             self.run_final_token(s, s.masks["A"].flush, 1, stream)
+            if events:
+                events["final"][1].record()
 
     def run_round(self, stream=None, lazy=True, events=None, fused=True, mode=None):
         """One whole round.  events: optional dict of (start, end) CUDA event pairs to record around parts."""
