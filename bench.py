@@ -31,7 +31,11 @@ from paper_2606_07710_b200 import synth  # noqa: E402
 WORKLOADS = {"cfg1": 0, "cfg2": 1, "cfg3": 2, "cfg4": 3, "cfg5": 4}
 # dram__bytes_read.sum + dram__bytes_write.sum per attention launch, from the committed `ncu --set full` capture named
 # beside each figure (a profiler cannot run inside the timed region); workloads without a capture report null
-NCU_TRAFFIC = {"cfg3": (552.5e6, "profiles/r1g_final.md (ncu --set full, chain kernel, round 1 commit abe3062)")}
+NCU_TRAFFIC = {   # dram__bytes_read.sum + dram__bytes_write.sum per attention launch, from the committed ncu --set full captures
+    "cfg5": (1059.1e6, "profiles/r2_ncu_kernels.md (ncu --set full of this workload, round 2)"),
+    "cfg2": (17.15e6, "profiles/r2_ncu_kernels.md (ncu --set full of this workload, cluster launch shape, round 2)"),
+    "cfg3": (552.5e6, "profiles/r1g_final.md (ncu --set full, chain kernel in the stream-K shape, round 1 commit abe3062)"),
+}
 METRIC = "verify_rounds_per_s"
 UNIT = "rounds/s"
 
