@@ -323,3 +323,20 @@ def test_attn_cluster_mode_sizes_and_reproducibility(wf):
             pair.close()
     finally:
         ctx.set_attn_cluster(-1)
+
+
+def test_two_contexts_in_one_process(wf):
+    """Per-context bookkeeping (dynamic shared-memory opt-in, merge counters, cluster tables): a second wf_ctx created in the
+    same process runs every large-shared-memory kernel on its own (a process-global `configured` flag broke this)."""
+    import gpu_harness as H
+    binding, ctx = wf
+    ctx2 = binding.Ctx(0)
+    try:
+        for c in (ctx2, ctx, ctx2):
+            max_abs, rel = _attn_case((binding, c), [900, 40], [16, 8], 32, 8, 128, seed=77)
+            assert max_abs <= ATTN_MAX_ABS and rel <= ATTN_REL_L2
+            max_abs, rel = _attn_case((binding, c), [2500] * 18, [16] * 18, 32, 8, 128, seed=78)     # stream-K shape
+            assert max_abs <= ATTN_MAX_ABS and rel <= ATTN_REL_L2
+            assert c.poll_status() == 0
+    finally:
+        ctx2.close()
