@@ -381,15 +381,13 @@ __device__ __forceinline__ int cl_row_owner(int r, int R, int cl) { return ((r +
 // memory and nobody waits for anybody here.  (Measured alternatives: one thread walking the owners, 240 cycles per owner;
 // every thread storing its fragment straight into the owners' buffers with st.async, 4.0k cycles against 2.5k for this.)
 template <int D>
-__device__ __forceinline__ void attn_cluster_push(const AttnShared<false>& sh, uint8_t* part_s, uint8_t* recv_s, int qw, int lane) {
-  // owner o is served by lane o / 4 of warp o % 4 of the group: a bulk copy is a warp-uniform instruction, so the lanes of one
-  // warp issue theirs one after the other (about 130 cycles each, measured): four warps issue four at a time
-  const int cl = sh.cl, rank = (int)blockIdx.x % cl, o = lane * 4 + qw;
-  if (lane < 4 && o < cl) {
-    const int a = sh.cl_rb[o], n = sh.cl_rb[o + 1] - a;
+__device__ __forceinline__ void attn_cluster_push(const AttnShared<false>& sh, uint8_t* part_s, uint8_t* recv_s, int lane) {
+  const int cl = sh.cl, rank = (int)blockIdx.x % cl;
+  if (lane < cl) {
+    const int a = sh.cl_rb[lane], n = sh.cl_rb[lane + 1] - a;
     if (n > 0)
-      bulk_push_dsmem(mapa_u32(smem_u32(recv_s) + (uint32_t)(rank * n) * (D * 4), (uint32_t)o), smem_u32(part_s) + (uint32_t)a * (D * 4),
-                      (uint32_t)n * (D * 4), mapa_u32(smem_u32(&sh.cl_bar), (uint32_t)o));
+      bulk_push_dsmem(mapa_u32(smem_u32(recv_s) + (uint32_t)(rank * n) * (D * 4), (uint32_t)lane), smem_u32(part_s) + (uint32_t)a * (D * 4),
+                      (uint32_t)n * (D * 4), mapa_u32(smem_u32(&sh.cl_bar), (uint32_t)lane));
   }
 }
 // (m, l) of row r (thread-held) to the owner of the row
@@ -407,48 +405,34 @@ __device__ __forceinline__ void attn_cluster_reduce(const AttnParams& p, const A
   constexpr int MAXCL = 16;
   const int cl = sh.cl, rank = (int)blockIdx.x % cl;
   const int row_a = sh.cl_rb[rank], n = sh.cl_rb[rank + 1] - row_a;
-  // Two adjacent lanes share one output position (row, 4 columns): lane parity h folds senders h, h + 2, ... relative to the row's
-  // global maximum (so the two halves add without rescaling), the pair is summed by one shuffle in a fixed order.
-  constexpr int HALF = MAXCL / 2;
-  const int h = tid256 & 1;
-  for (int idx0 = 0; idx0 < n * (D / 4); idx0 += 128) {
-    const int idx = idx0 + (tid256 >> 1);
-    const bool live = idx < n * (D / 4);
-    const int i = live ? idx / (D / 4) : 0, c4 = idx % (D / 4), row = row_a + i;
+  for (int idx = tid256; idx < n * (D / 4); idx += 256) {
+    const int i = idx / (D / 4), c4 = idx % (D / 4), row = row_a + i;
     const uint8_t* base = recv_s + (size_t)i * (D * 4) + ((c4 ^ (row & 7)) << 4);
-    float2 ml[HALF];
-    float4 ov[HALF];
+    float2 ml[MAXCL];
+    float4 ov[MAXCL];
+#pragma unroll
+    for (int s2 = 0; s2 < MAXCL; ++s2)
+      if (s2 < cl) {
+        ml[s2] = sh.cl_ml[s2 * n + i];
+        ov[s2] = *reinterpret_cast<const float4*>(base + (size_t)s2 * n * (D * 4));
+      }
     float m = -INFINITY;
 #pragma unroll
-    for (int u = 0; u < HALF; ++u) {
-      const int s2 = 2 * u + h;
-      if (s2 < cl) {
-        ml[u] = sh.cl_ml[s2 * n + i];
-        ov[u] = *reinterpret_cast<const float4*>(base + (size_t)s2 * n * (D * 4));
-        m = fmaxf(m, ml[u].x);
-      }
-    }
-    m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 1));
+    for (int s2 = 0; s2 < MAXCL; ++s2)
+      if (s2 < cl) m = fmaxf(m, ml[s2].x);
     float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
     float l = 0.f;
 #pragma unroll
-    for (int u = 0; u < HALF; ++u)
-      if (2 * u + h < cl && ml[u].y > 0.f) {                   // a CTA without tiles (or without a visible key) sends l = 0
-        const float w = fast_exp2(ml[u].x - m);
-        l = fmaf(w, ml[u].y, l);
-        acc.x = fmaf(w, ov[u].x, acc.x); acc.y = fmaf(w, ov[u].y, acc.y);
-        acc.z = fmaf(w, ov[u].z, acc.z); acc.w = fmaf(w, ov[u].w, acc.w);
+    for (int s2 = 0; s2 < MAXCL; ++s2)
+      if (s2 < cl && ml[s2].y > 0.f) {                         // a CTA without tiles (or without a visible key) sends l = 0
+        const float w = fast_exp2(ml[s2].x - m);
+        l = fmaf(w, ml[s2].y, l);
+        acc.x = fmaf(w, ov[s2].x, acc.x); acc.y = fmaf(w, ov[s2].y, acc.y);
+        acc.z = fmaf(w, ov[s2].z, acc.z); acc.w = fmaf(w, ov[s2].w, acc.w);
       }
-    // even half + odd half, the same order on both lanes: bit-reproducible
-    const float lo = __shfl_xor_sync(0xffffffffu, l, 1);
-    const float4 ao = make_float4(__shfl_xor_sync(0xffffffffu, acc.x, 1), __shfl_xor_sync(0xffffffffu, acc.y, 1),
-                                  __shfl_xor_sync(0xffffffffu, acc.z, 1), __shfl_xor_sync(0xffffffffu, acc.w, 1));
-    if (live && h == 0) {
-      const float inv = 1.f / (l + lo);                        // every row sees key 0: l > 0
-      __nv_bfloat16* dst = p.out + ((size_t)(unsigned int)sh.cl_dst[row] >> 5) + c4 * 4;
-      *reinterpret_cast<uint2*>(dst) = make_uint2(pack_bf16((acc.x + ao.x) * inv, (acc.y + ao.y) * inv),
-                                                  pack_bf16((acc.z + ao.z) * inv, (acc.w + ao.w) * inv));
-    }
+    const float inv = 1.f / l;                                 // every row sees key 0: l > 0
+    __nv_bfloat16* dst = p.out + ((size_t)(unsigned int)sh.cl_dst[row] >> 5) + c4 * 4;
+    *reinterpret_cast<uint2*>(dst) = make_uint2(pack_bf16(acc.x * inv, acc.y * inv), pack_bf16(acc.z * inv, acc.w * inv));
   }
 }
 
@@ -720,8 +704,10 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared<fal
 #pragma unroll
       for (int h = 0; h < 2; ++h)
         if ((lane & 3) == 0 && row_lo + 8 * h < Rc) attn_cluster_push_ml(sh, row_lo + 8 * h, m_run[h], l_run[h]);
-      mbar_wait(smem_u32(&sh.cl_ready), 0);                    // every CTA of the cluster can receive (its K ring is idle)
-      attn_cluster_push<D>(sh, part_s, recv_s, qw, lane);
+      if (warp == 0) {
+        mbar_wait(smem_u32(&sh.cl_ready), 0);                  // every CTA of the cluster can receive (its K ring is idle)
+        attn_cluster_push<D>(sh, part_s, recv_s, lane);
+      }
       continue;
     }
     auto write_rows = [&]() {                                  // normalise and store this thread's two rows
@@ -861,9 +847,9 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared<fal
       // a CTA without tiles still owes every owner a slice: l = 0 marks it empty (its O bits are never read)
       named_bar_sync(4, 256);                                  // the tables above
       if (grp == 0 && stid < R) attn_cluster_push_ml(sh, stid, -INFINITY, 0.f);
-      if (grp == 0) {
+      if (warp == 0) {
         mbar_wait(smem_u32(&sh.cl_ready), 0);
-        attn_cluster_push<D>(sh, part_s, recv_s, qw, lane);
+        attn_cluster_push<D>(sh, part_s, recv_s, lane);
       }
     }
     WF_PROBE_AT(7, warp == 0 && lane == 0);
