@@ -754,8 +754,8 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=30)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-tree", action="store_true", help="skip the tree-verification leg (SURVEY.md §8(f) f2)")
-    ap.add_argument("--cpu-sample-seqs", type=int, default=4)
-    ap.add_argument("--cpu-sample-layers", type=int, default=8)
+    ap.add_argument("--cpu-sample-seqs", type=int, default=8)
+    ap.add_argument("--cpu-sample-layers", type=int, default=16)
     ap.add_argument("--traffic-bytes", type=float, default=None,
                     help="dram bytes per attention launch; default: the committed ncu --set full capture for the workload")
     args = ap.parse_args()
