@@ -94,8 +94,10 @@ class RoundState:
         self.next_q_len = torch.zeros(B, dtype=torch.int32, device=device)
         self.q_len_of = {wf.ROUTE_AR: gam_of(wf.ROUTE_AR) + 1, wf.ROUTE_DIFFUSION: gam_of(wf.ROUTE_DIFFUSION) + 1}
         self.tau = torch.full((1,), sh.tau, dtype=torch.float32, device=device)
-        self.out = {n: torch.zeros(B, dtype=torch.int32, device=device) for n in ("accept_len", "bonus_token", "route", "n_commit")}
-        self.entropy = torch.zeros(B, dtype=torch.float32, device=device)
+        # the round's five result vectors are rows of ONE buffer: a caller reads them back with a single copy
+        self.out_all = torch.zeros((5, B), dtype=torch.int32, device=device)
+        self.out = {n: self.out_all[i] for i, n in enumerate(("accept_len", "bonus_token", "route", "n_commit"))}
+        self.entropy = self.out_all[4].view(torch.float32)
         self.attn_ws = torch.empty(wf.wf_verify_attn_workspace_bytes(self.kv_shape, B, sh.n_q_heads, self.qmax),
                                    dtype=torch.uint8, device=device)
         self.acc_ws = torch.empty(wf.wf_accept_workspace_bytes(B * self.qmax, sh.vocab), dtype=torch.uint8, device=device)
