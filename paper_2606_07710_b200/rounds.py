@@ -126,7 +126,7 @@ class RoundState:
             mk = lambda shape, stream: [synth.device_normal_bf16(shape, 0.02, wl.seed, stream + l, device) for l in range(dA.n_layers)]
             ws_ = (mk((sh.hidden, qd), 70), mk((qd, sh.hidden), 75), mk((sh.hidden, ffn), 80), mk((ffn, sh.hidden), 85))
             dA.handle.set_full_layer(sh.n_q_heads, ffn, min(B, 256), *ws_)       # the library keeps its own repacked copy
-            del ws_
+            ft.weights = ws_                                   # (W_Q, W_O, W_up, W_down) per layer: the tests hand them to the oracle
             ft.weight_bytes = dA.n_layers * 2 * (2 * sh.hidden * qd + 2 * sh.hidden * ffn)
             ft.h_out = torch.zeros((B, dA.n_layers, sh.hidden), dtype=torch.bfloat16, device=device)
             ft.ws = torch.empty(wf.wf_final_token_workspace_bytes(dA.handle, B), dtype=torch.uint8, device=device)

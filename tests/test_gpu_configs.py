@@ -1,5 +1,6 @@
 """Whole rounds at each BASELINE.json config's OWN parameters, through paper_2606_07710_b200.rounds (reserve ->
-verify attention -> accept/entropy/route -> wf_switch_round), against the oracle driven by the ORACLE's own route.
+verify attention -> accept/entropy/route -> wf_switch_round -> wf_final_token_full), against the oracle driven by the ORACLE's
+own route.
 
 north_star: "all five configs match the CPU oracle within the stated tolerances".  configs[0] (tiny) is covered by
 test_gpu_attn_accept.py / test_gpu_prefill_lazy.py (64 seeds) and smoke(); here are configs[1..4]:
@@ -14,7 +15,9 @@ every-SM-busy launch shape is test_gpu_fullsize.py's); every drafter layer is ch
 Compared per round: attention rows of sampled (sequence, query head) pairs (max-abs 2e-2, rel-L2 5e-3 per pair);
 accept_len / bonus / n_commit bit-exact, entropy 1e-3, route bit-exact outside |H - tau| < 1e-4; target and drafter
 block tables, cache lengths and backlog lengths bit-exact; the K/V rows each drafter wrote this round within rel-L2
-5e-3 of the oracle's unrounded fp64; backlog rows bit-exact; cur_drafter and the next block lengths bit-exact.
+5e-3 of the oracle's unrounded fp64; backlog rows bit-exact; cur_drafter, who switched and the next block lengths bit-exact;
+the post-MLP state of the final backlog token (f3, oracle O9) of up to two sequences per round that switched to the AR drafter
+within rel-L2 5e-3.
 """
 
 import math
@@ -22,13 +25,13 @@ import math
 import numpy as np
 import pytest
 
-from oracle import accept_route, kv_prefill, lazy_catchup, verify_attn
+from oracle import accept_route, final_token, kv_prefill, lazy_catchup, verify_attn
 from oracle.paged_kv import PagedKV as OraclePagedKV
 from paper_2606_07710_b200 import synth
 
 pytestmark = pytest.mark.gpu
 
-ATTN_MAX_ABS, ATTN_REL_L2, ENTROPY_ABS, ROUTE_BAND, KV_REL_L2 = 2e-2, 5e-3, 1e-3, 1e-4, 5e-3
+ATTN_MAX_ABS, ATTN_REL_L2, ENTROPY_ABS, ROUTE_BAND, KV_REL_L2, H_REL_L2 = 2e-2, 5e-3, 1e-3, 1e-4, 5e-3, 5e-3
 ROUTE_AR, ROUTE_DIFFUSION = 1, 0
 
 
@@ -89,6 +92,8 @@ def _round_parity(wf, index, n_rounds, sample_seqs, sample_heads, sample_rows=No
     lz = {ROUTE_DIFFUSION: _mirror_drafter(rs, rs.drafters["D"]), ROUTE_AR: _mirror_drafter(rs, rs.drafters["A"])}
     gd = {ROUTE_DIFFUSION: rs.drafters["D"], ROUTE_AR: rs.drafters["A"]}
     cur = rs.slots[0].cur.copy()
+    full = final_token.FullLayer(*[[_bits(w) for w in ws] for ws in rs.ft.weights], sh.n_q_heads)     # (f3) the AR drafter's layer
+    worst_h, n_final = 0.0, 0
     near_tau = worst_attn = worst_kv = 0
     routes_seen, flushes = set(), 0
     for rnd in range(n_rounds):
@@ -142,7 +147,19 @@ def _round_parity(wf, index, n_rounds, sample_seqs, sample_heads, sample_rows=No
         # ---- (c) + (d) the switch, driven by the oracle's route ----
         hid = _bits(s.hidden)
         flushes += int((route != cur).sum())
+        switched_to_ar = (cur != ROUTE_AR) & (route == ROUTE_AR) & (want["n_commit"] > 0)
+        np.testing.assert_array_equal(rs.switched.cpu().numpy(), np.where(route != cur, route, -1))
         cur, nq, outs = lazy_catchup.switch_round(lz, hid, s.q_indptr_host, want["n_commit"], route, cur, rs.q_len_of)
+        # ---- (f3) the final backlog token in full, for (at most two of) the sequences that switched to the AR drafter ----
+        h_gpu = rs.ft.h_out.float().cpu().numpy().astype(np.float64)
+        for b in np.nonzero(switched_to_ar)[0][:2]:
+            x_last = hid[int(s.q_indptr_host[b]) + int(want["n_commit"][b]) - 1]
+            h_want = final_token.final_token_full(lz[ROUTE_AR].drafter, full, x_last, int(b))
+            for layer in range(h_want.shape[0]):
+                rel = float(np.sqrt(((h_gpu[b, layer] - h_want[layer]) ** 2).sum() / (h_want[layer] ** 2).sum()))
+                assert rel <= H_REL_L2, (wl.name, rnd, int(b), layer, rel)
+                worst_h = max(worst_h, rel)
+            n_final += 1
         np.testing.assert_array_equal(rs.cur_drafter.cpu().numpy(), cur)
         np.testing.assert_array_equal(rs.next_q_len.cpu().numpy(), nq)
         for code, l in lz.items():
@@ -162,7 +179,8 @@ def _round_parity(wf, index, n_rounds, sample_seqs, sample_heads, sample_rows=No
                 nb = int(l.backlog_len[b])
                 assert np.array_equal(bl[b, :nb], l.backlog[b, :nb]), (wl.name, rnd, code, b, "backlog rows")
     rs.close()
-    return dict(near_tau=near_tau, worst_attn=worst_attn, worst_kv=worst_kv, routes=routes_seen, flushes=flushes)
+    return dict(near_tau=near_tau, worst_attn=worst_attn, worst_kv=worst_kv, routes=routes_seen, flushes=flushes, worst_h=worst_h,
+                n_final=n_final)
 
 
 def test_cfg2_whole_rounds(wf):
@@ -175,7 +193,7 @@ def test_cfg2_whole_rounds(wf):
 def test_cfg3_whole_rounds(wf):
     """configs[2]: batch 16, context 8192, gamma 7 / 15 by route, cap 32."""
     r = _round_parity(wf, 2, 4, lambda B: [0, 7, 15], [0, 9, 18, 31])
-    assert r["routes"] == {0, 1} and r["flushes"] > 0, r
+    assert r["routes"] == {0, 1} and r["flushes"] > 0 and r["n_final"] > 0, r
     print("cfg3", r)
 
 
@@ -188,7 +206,7 @@ def test_cfg4_whole_rounds(wf):
 def test_cfg5_whole_rounds(wf):
     """configs[4]: batch 64, log-uniform contexts, shuffled pages, mixed gamma, geometric accepts, switch prob 0.3."""
     r = _round_parity(wf, 4, 3, lambda B: [0, 21, 42, 63], [2, 13, 27], sample_rows=[0, 3, 7, 15])
-    assert r["routes"] == {0, 1} and r["flushes"] > 0, r
+    assert r["routes"] == {0, 1} and r["flushes"] > 0 and r["n_final"] > 0, r
     print("cfg5", r)
 
 
