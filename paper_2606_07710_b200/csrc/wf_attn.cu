@@ -114,7 +114,6 @@ struct AttnShared {
   int total_tiles, g_eff, B;
   int cl;                              // cluster mode: CTAs per (b, g) pair (0 = stream-K ranges)
   int cl_b;                            // cluster mode: the sequence of this CTA's pair (its table entry is index 0)
-  Segment seg;                         // cluster mode: this CTA's one segment (n_tiles = 0: none), derived once in the prologue
   int n_stk, n_stv;                    // K / V ring depths
   uint64_t k_done;                     // cluster mode: this CTA's last QK^T has retired: its K ring is free to receive
   uint64_t cl_ready;                   // cluster mode: every CTA of the cluster can receive (cl arrivals)
@@ -139,7 +138,8 @@ struct SegWalker {
   int Hkv, c;
   int lo, hi, x, b;
   bool first = true;
-  __device__ SegWalker(const AttnShared<TREE>& sh_, int Hkv_, int c_) : sh(sh_), Hkv(Hkv_), c(c_) {
+  const Segment* lean = nullptr;                               // cluster mode: this CTA's one segment, held by every thread
+  __device__ SegWalker(const AttnShared<TREE>& sh_, int Hkv_, int c_, const Segment* lean_) : sh(sh_), Hkv(Hkv_), c(c_), lean(lean_) {
     if (sh.cl > 0) { lo = hi = x = b = 0; return; }          // cluster mode: next() derives the one segment of this CTA
     const int T = sh.total_tiles, G = sh.g_eff;
     lo = (int)((long long)c * T / G);
@@ -154,11 +154,11 @@ struct SegWalker {
   }
   __device__ bool next(Segment& s) {
     if (sh.cl > 0) {
-      // Cluster mode: the one segment of this CTA was derived in the prologue (thread 0: a walk costs 1.2k cycles of
-      // integer divisions, measured, and every role would repeat it on the critical path of a batch-1 launch)
-      if (!first || sh.seg.n_tiles <= 0) return false;
+      // Cluster mode: the one segment of this CTA was derived in the prologue, by every thread for itself from one
+      // global round trip (a walk costs 1.2k cycles of integer divisions, measured, on the critical path of a batch-1 launch)
+      if (!first || lean->n_tiles <= 0) return false;
       first = false;
-      s = sh.seg;
+      s = *lean;
       return true;
     }
     while (x < hi) {
@@ -207,12 +207,13 @@ __device__ __forceinline__ int cta_of_tile(int x, int T, int G) {      // larges
 // ================= warps 8 (K) and 10 (V): TMA producers =================
 // K and V have separate rings so that a K tile is released as soon as its QK^T retires: more bytes in flight.
 template <int D, bool TREE>
-__device__ __forceinline__ void attn_loader(const AttnParams& p, AttnShared<TREE>& sh, uint8_t* ring, int which, int lane) {
+__device__ __forceinline__ void attn_loader(const AttnParams& p, AttnShared<TREE>& sh, uint8_t* ring, uint8_t* k_ring, int which, int lane,
+                                            const Segment* lean) {
   using C = AttnCfg<D, TREE>;
   const KvView& kv = p.kv;
   uint64_t* full = which ? sh.v_full : sh.k_full;
   uint64_t* empty = which ? sh.v_empty : sh.k_empty;
-  SegWalker<TREE> walk(sh, p.kv.n_kv_heads, blockIdx.x);
+  SegWalker<TREE> walk(sh, p.kv.n_kv_heads, blockIdx.x, lean);
   Segment sg;
   uint32_t gt = 0;
   constexpr int PP = AT_BN / 16;                              // pages per tile
@@ -234,13 +235,27 @@ __device__ __forceinline__ void attn_loader(const AttnParams& p, AttnShared<TREE
 #pragma unroll
       for (int q = 0; q < PP; ++q) rows[q] = __shfl_sync(0xffffffffu, row, q);
       mbar_wait(smem_u32(&empty[st]), ((gt / n_st) & 1) ^ 1);
+      // Cluster mode (latency-bound): the very first K tile of the CTA is what the first QK^T waits for, and one thread issues
+      // a box about every 70 cycles: the V loader issues the second half of that K tile (same page ids) before its own V tile.
+      const bool split_first = !TREE && sh.cl > 0 && gt == 0;
+      if (split_first && which == 1 && elect_one()) {
+        const uint32_t kbar = smem_u32(&sh.k_full[0]);
+        const uint32_t kdst = smem_u32(k_ring);
+#pragma unroll
+        for (int q = PP / 2; q < PP; ++q)
+          if (q < npages) {
+#pragma unroll
+            for (int h = 0; h < C::NH; ++h) tma_load_2d(kdst + q * 2048 + h * C::KV_HALF, kv.tmaps, h * 64, rows[q], kbar);
+          }
+      }
       if (elect_one()) {                                       // one lane issues the whole tile: straight-line TMA issue
         const uint32_t bar = smem_u32(&full[st]);
         const uint32_t dst = ring_s + (uint32_t)st * C::K_BYTES;
         mbar_arrive_expect_tx(bar, (uint32_t)npages * 16 * D * 2);
+        const int q_end = (split_first && which == 0) ? PP / 2 : PP;
 #pragma unroll
         for (int q = 0; q < PP; ++q)
-          if (q < npages) {
+          if (q < npages && q < q_end) {
 #pragma unroll
             for (int h = 0; h < C::NH; ++h) tma_load_2d(dst + q * 2048 + h * C::KV_HALF, tmap, h * 64, rows[q], bar);
           }
@@ -264,12 +279,12 @@ __device__ __forceinline__ uint32_t mapa_u32(uint32_t addr, uint32_t rank);
 
 template <int D, bool TREE>
 __device__ __forceinline__ void attn_mma_qk(const AttnParams& p, AttnShared<TREE>& sh, uint8_t* q_s, uint8_t* k_s,
-                                            uint32_t tmem_base) {
+                                            uint32_t tmem_base, const Segment* lean) {
   using C = AttnCfg<D, TREE>;
   const uint32_t idesc_qk = umma_idesc_kk(C::Q_ROWS, AT_BN);
   const uint64_t dq0 = umma_desc(smem_u32(q_s), 16, 1024);                  // K-major
   const uint64_t dk0 = umma_desc(smem_u32(k_s), 16, 1024);                  // K-major
-  SegWalker<TREE> walk(sh, p.kv.n_kv_heads, blockIdx.x);
+  SegWalker<TREE> walk(sh, p.kv.n_kv_heads, blockIdx.x, lean);
   Segment sg;
   uint32_t gt = 0, n_seg = 0;
   while (walk.next(sg)) {
@@ -313,13 +328,13 @@ __device__ __forceinline__ void attn_mma_qk(const AttnParams& p, AttnShared<TREE
 
 template <int D, bool TREE>
 __device__ __forceinline__ void attn_mma_pv(const AttnParams& p, AttnShared<TREE>& sh, uint8_t* p0_s, uint8_t* p1_s,
-                                            uint8_t* v_s, uint32_t tmem_base) {
+                                            uint8_t* v_s, uint32_t tmem_base, const Segment* lean) {
   using C = AttnCfg<D, TREE>;
   const uint32_t idesc_pv = umma_idesc(C::Q_ROWS, D);
   const uint64_t dp0 = umma_desc(smem_u32(p0_s), 16, 1024);                 // K-major
   const uint64_t dp1 = umma_desc(smem_u32(p1_s), 16, 1024);
   const uint64_t dv0 = umma_desc(smem_u32(v_s), C::KV_HALF, 1024);          // MN-major
-  SegWalker<TREE> walk(sh, p.kv.n_kv_heads, blockIdx.x);
+  SegWalker<TREE> walk(sh, p.kv.n_kv_heads, blockIdx.x, lean);
   Segment sg;
   uint32_t gt = 0;
   while (walk.next(sg)) {
@@ -441,7 +456,8 @@ __device__ __forceinline__ void attn_cluster_reduce(const AttnParams& p, const A
 // keeps its own running (m, l, O); at the end of a segment group 1 hands its state to group 0 through smem.
 template <int D>
 __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared<false>& sh, uint8_t* q_s, uint8_t* p0_s, uint8_t* p1_s,
-                                             uint8_t* v_s, uint8_t* part_s, uint8_t* recv_s, uint32_t tmem_base, int warp, int lane) {
+                                             uint8_t* v_s, uint8_t* part_s, uint8_t* recv_s, uint32_t tmem_base, int warp, int lane,
+                                             const Segment* lean) {
   using C = AttnCfg<D, false>;
   constexpr int NO = D / 2;                                    // O registers per thread (2 rows x D/4 columns)
   const int Hkv = p.kv.n_kv_heads;
@@ -453,17 +469,17 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared<fal
   uint8_t* p_s = grp ? p1_s : p0_s;
   float* xch = reinterpret_cast<float*>(q_s);                  // [NO][128] group-merge buffer (Q + P1 regions)
   const int T = sh.total_tiles, G = sh.g_eff;
-  SegWalker<false> walk(sh, p.kv.n_kv_heads, blockIdx.x);
+  SegWalker<false> walk(sh, p.kv.n_kv_heads, blockIdx.x, lean);
   Segment sg;
   uint32_t gt0 = 0;                                            // global tile counter at the start of the segment
   if (sh.cl > 0) {
     // cluster mode: the row-dealing tables of the merge, by threads that would otherwise idle through the Q load's
     // integer work: group 1 builds them, everybody reads them behind the named barriers of the group merge
-    const int Rt = min((sh.r0[1] - sh.r0[0]) * p.group, AT_ROWS);
+    const int Rt = min(lean->q_b * p.group, AT_ROWS);
     if (grp == 1 && stid <= sh.cl) sh.cl_rb[stid] = cl_row_begin(stid, Rt, sh.cl);
     if (grp == 1 && stid >= 64 && stid - 64 < Rt) {
       const int r = stid - 64, qi = r / p.group, hg = r % p.group;
-      const unsigned int off = (unsigned int)(((sh.r0[0] + qi) * p.n_q_heads + sh.seg.g * p.group + hg) * D);
+      const unsigned int off = (unsigned int)(((lean->r0 + qi) * p.n_q_heads + lean->g * p.group + hg) * D);
       sh.cl_dst[r] = (int)((off << 5) | (unsigned int)cl_row_owner(r, Rt, sh.cl));
     }
   }
@@ -842,7 +858,7 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared<fal
     write_rows();
   }
   if (sh.cl > 0) {
-    const int R = min((sh.r0[1] - sh.r0[0]) * p.group, AT_ROWS);
+    const int R = min(lean->q_b * p.group, AT_ROWS);
     if (gt0 == 0) {
       // a CTA without tiles still owes every owner a slice: l = 0 marks it empty (its O bits are never read)
       named_bar_sync(4, 256);                                  // the tables above
@@ -881,7 +897,7 @@ __device__ __forceinline__ void attn_softmax_tree(const AttnParams& p, AttnShare
   const uint32_t t_lane = tmem_base + ((uint32_t)(qw * 32 + grp * 16) << 16);
   const int npt = AT_ROWS / p.group;                           // nodes per sub-block
   const int T = sh.total_tiles, G = sh.g_eff;
-  SegWalker<true> walk(sh, p.kv.n_kv_heads, blockIdx.x);
+  SegWalker<true> walk(sh, p.kv.n_kv_heads, blockIdx.x, nullptr);
   Segment sg;
   uint32_t gt0 = 0;                                            // global tile counter at the start of the segment
   while (walk.next(sg)) {
@@ -1167,6 +1183,10 @@ __global__ void __launch_bounds__(AT_THREADS, 1) wf_verify_attn_kernel(const Att
     }
     sh.n_stk = C::STAGES_K;
     sh.n_stv = C::STAGES_V;
+    if (!TREE && p.cl > 0) {                                   // cluster mode: what does not depend on device memory
+      sh.cl = p.cl; sh.B = 1; sh.g_eff = (int)gridDim.x;
+      sh.cl_b = ((int)blockIdx.x / p.cl) / p.kv.n_kv_heads;
+    }
     fence_barrier_init();
   }
   if (warp == 9) tmem_alloc(smem_u32(&sh.tmem), 512);
@@ -1179,38 +1199,34 @@ __global__ void __launch_bounds__(AT_THREADS, 1) wf_verify_attn_kernel(const Att
     asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(p.kv.tmaps + (tid == 32 * 10 ? 1 : 0))) : "memory");
   wf_pdl_wait();
   WF_PROBE_AT(1, tid == 0);
-  // Cluster mode: a CTA serves ONE (b, g) pair, so it tabulates only that sequence: one global round trip, one barrier
-  // (the full table costs two barriers and a scan: 2.4k cycles, measured, on the critical path of a batch-1 launch).
+  // Cluster mode: a CTA serves ONE (b, g) pair.  Every thread loads that sequence's three lengths itself (one global round
+  // trip, the same for all) and derives the CTA's one segment in registers: no table, no barrier behind the dependency wait
+  // (the full table costs two barriers and a scan, 2.4k cycles; thread 0 + one barrier + a copy of the segment still cost
+  // 1.1k + 0.6k before a loader could fetch its first page id: measured, on the critical path of a batch-1 launch).  The
+  // cluster barrier ahead of the wait has already made the barriers, the TMEM address and the mode visible to everybody.
   const bool lean = !TREE && p.cl > 0;
+  Segment lean_sg;
+  lean_sg.n_tiles = 0;
+  int lean_nt = 0;
   if (lean) {
+    const int pair = (int)blockIdx.x / p.cl, rank = (int)blockIdx.x % p.cl, b = pair / p.kv.n_kv_heads;
+    const int r0 = p.q_indptr[b], r1 = p.q_indptr[b + 1], ctx = p.kv.seq_len[b] + p.ctx_adj;
+    const int nt = r1 > r0 ? (ctx + (r1 - r0) + AT_BN - 1) / AT_BN : 0;
+    lean_nt = nt;
+    // cluster `pair` = (b, g) over ALL sequences of the call (an empty one idles its cluster); CTA rank r of the cluster owns
+    // tiles [r * nt / cl, (r + 1) * nt / cl) of the pair: pair-aligned, equal shares, one segment
+    lean_sg.b = b; lean_sg.pb = 0; lean_sg.nt = nt; lean_sg.g = pair % p.kv.n_kv_heads;
+    lean_sg.t_lo = rank * nt / p.cl; lean_sg.t_hi = (rank + 1) * nt / p.cl;
+    lean_sg.flat0 = 0; lean_sg.r0 = r0; lean_sg.ctx = ctx; lean_sg.q_b = r1 - r0;
+    lean_sg.k0 = lean_sg.t_lo * AT_BN; lean_sg.k1 = min(ctx + lean_sg.q_b, lean_sg.t_hi * AT_BN);
+    lean_sg.n_tiles = lean_sg.t_hi - lean_sg.t_lo; lean_sg.partial = 1; lean_sg.slot = 0;
     if (tid == 0) {
-      const int pair = (int)blockIdx.x / p.cl, b = pair / p.kv.n_kv_heads;
-      const int r0 = p.q_indptr[b], r1 = p.q_indptr[b + 1], ctx = p.kv.seq_len[b] + p.ctx_adj;
-      if ((int)blockIdx.x % p.cl == 0 && pair % p.kv.n_kv_heads == 0 && (r1 - r0) * p.group > AT_ROWS) wf_raise(p.status, (int)WF_ERR_INVALID_ARG);
-      sh.r0[0] = r0; sh.r0[1] = r1; sh.ctx[0] = ctx;
-      sh.pref[0] = 0;
-      sh.pref[1] = r1 > r0 ? (ctx + (r1 - r0) + AT_BN - 1) / AT_BN + AT_SEG_COST : 0;
-      const int nt = max(0, sh.pref[1] - AT_SEG_COST);
-      sh.total_tiles = nt;
-      sh.g_eff = (int)gridDim.x; sh.B = 1; sh.cl = p.cl; sh.cl_b = b;
-      // cluster `pair` = (b, g) over ALL sequences of the call (an empty one idles its cluster); CTA rank r of the cluster owns
-      // tiles [r * nt / cl, (r + 1) * nt / cl) of the pair: pair-aligned, equal shares, one segment
-      const int rank = (int)blockIdx.x % p.cl;
-      Segment sg;
-      sg.b = b; sg.pb = 0; sg.nt = nt; sg.g = pair % p.kv.n_kv_heads;
-      sg.t_lo = rank * nt / p.cl; sg.t_hi = (rank + 1) * nt / p.cl;
-      sg.flat0 = 0; sg.r0 = r0; sg.ctx = ctx; sg.q_b = r1 - r0;
-      sg.k0 = sg.t_lo * AT_BN; sg.k1 = min(ctx + sg.q_b, sg.t_hi * AT_BN);
-      sg.n_tiles = sg.t_hi - sg.t_lo; sg.partial = 1; sg.slot = 0;
-      sh.seg = sg;
+      if (rank == 0 && lean_sg.g == 0 && (r1 - r0) * p.group > AT_ROWS) wf_raise(p.status, (int)WF_ERR_INVALID_ARG);
       // what this CTA will receive: from each of the cl CTAs, its rows [row_a, row_b) of (m, l) and of O
       const int R = min((r1 - r0) * p.group, AT_ROWS);
       const int n_mine = cl_row_begin(rank + 1, R, p.cl) - cl_row_begin(rank, R, p.cl);
       if (nt > 0) mbar_arrive_expect_tx(smem_u32(&sh.cl_bar), (uint32_t)(p.cl * n_mine * (D * 4 + 8)));
     }
-    tc_fence_before();
-    __syncthreads();
-    tc_fence_after();
   } else {
     // per-sequence table (tiles per kv head, q_indptr, context) from the device-resident lengths, identical in
     // every CTA; then total tiles and the longest pair
@@ -1315,19 +1331,20 @@ __global__ void __launch_bounds__(AT_THREADS, 1) wf_verify_attn_kernel(const Att
 
   }
   const uint32_t tmem_base = sh.tmem;
-  const bool run = sh.total_tiles > 0 && (int)blockIdx.x < sh.g_eff;
+  const bool run = lean ? lean_nt > 0 : (sh.total_tiles > 0 && (int)blockIdx.x < sh.g_eff);
+  const Segment* lp = lean ? &lean_sg : nullptr;
   WF_PROBE_AT(2, tid == 0);
   if (run) {
     if (warp < 8) {
       asm volatile("setmaxnreg.inc.sync.aligned.u32 216;");
       if constexpr (TREE) attn_softmax_tree<D>(p, sh, q_s, p0_s, v_s, tmem_base, warp, lane);
-      else attn_softmax<D>(p, sh, q_s, p0_s, p1_s, v_s, k_s + C::K_BYTES, k_s, tmem_base, warp, lane);
+      else attn_softmax<D>(p, sh, q_s, p0_s, p1_s, v_s, k_s + C::K_BYTES, k_s, tmem_base, warp, lane, lp);
     } else {
       asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
-      if (warp == 8) attn_loader<D, TREE>(p, sh, k_s, 0, lane);
-      else if (warp == 10) attn_loader<D, TREE>(p, sh, v_s, 1, lane);
-      else if (warp == 9) attn_mma_qk<D, TREE>(p, sh, q_s, k_s, tmem_base);
-      else if (warp == 11) attn_mma_pv<D, TREE>(p, sh, p0_s, p1_s, v_s, tmem_base);
+      if (warp == 8) attn_loader<D, TREE>(p, sh, k_s, k_s, 0, lane, lp);
+      else if (warp == 10) attn_loader<D, TREE>(p, sh, v_s, k_s, 1, lane, lp);
+      else if (warp == 9) attn_mma_qk<D, TREE>(p, sh, q_s, k_s, tmem_base, lp);
+      else if (warp == 11) attn_mma_pv<D, TREE>(p, sh, p0_s, p1_s, v_s, tmem_base, lp);
     }
   }
   if constexpr (!TREE) {
