@@ -340,3 +340,47 @@ def test_two_contexts_in_one_process(wf):
             assert c.poll_status() == 0
     finally:
         ctx2.close()
+
+
+def test_attn_maximum_batch(wf):
+    """B = 1024 sequences (the kernel's table limit), contexts 0..70, blocks of 0..16 rows, 8 kv heads: 8192 (sequence, kv head)
+    pairs, ranges of many one-tile segments; B = 1025 is refused on the host."""
+    import torch
+    import gpu_harness as H
+    binding, ctx = wf
+    g = synth.rng(91, 5)
+    ctx_lens = [int(x) for x in g.integers(0, 71, size=1024)]
+    q_lens = [int(x) for x in g.choice([0, 1, 4, 8, 16], size=1024)]
+    max_abs, rel = _attn_case(wf, ctx_lens, q_lens, 32, 8, 128, seed=92)
+    assert max_abs <= ATTN_MAX_ABS and rel <= ATTN_REL_L2, (max_abs, rel)
+    pair = H.make_kv_pair(ctx, [4] * 1025, [1] * 1025, 1, 2, 64, seed=93, fill=False)
+    q = torch.zeros((1025, 4, 64), dtype=torch.bfloat16, device="cuda")
+    ws = torch.empty(binding.wf_verify_attn_workspace_bytes(pair.shape, 1025, 4, 1), dtype=torch.uint8, device="cuda")
+    with pytest.raises(binding.WhiFlashError):
+        binding.wf_verify_attn(ctx, pair.gpu, 0, q, H.i32(np.arange(1026)), 1025, 4, 1, 0.125, torch.zeros_like(q), ws)
+    pair.close()
+
+
+def test_accept_large_batch_small_vocab(wf):
+    """B = 3000 sequences x up to 8 rows, V = 1000 (one ragged slice per row, V % 4 == 0): every output against the oracle."""
+    import torch
+    import gpu_harness as H
+    binding, ctx = wf
+    g = synth.rng(94, 1)
+    B, V = 3000, 1000
+    q_lens = [int(x) for x in g.integers(0, 9, size=B)]
+    prefix = [int(g.integers(0, max(q, 1))) for q in q_lens]
+    logits, drafts, ip, _ = synth.make_logits_block(g, q_lens, V, 2.0, prefix, g.uniform(0.0, 8.0, size=B))
+    want = accept_route.accept_entropy_route(logits, drafts, ip, 2.0)
+    o = [torch.zeros(B, dtype=torch.int32, device="cuda") for _ in range(4)]
+    ent = torch.zeros(B, dtype=torch.float32, device="cuda")
+    ws = torch.empty(binding.wf_accept_workspace_bytes(B * 8, V), dtype=torch.uint8, device="cuda")
+    binding.wf_accept_entropy_route(ctx, H.f32(logits), V, H.i32(drafts), H.i32(ip), B, 8, H.f32([2.0]), True, o[0], o[1], ent, o[2], o[3], None, ws)
+    torch.cuda.synchronize()
+    assert ctx.poll_status() == 0
+    np.testing.assert_array_equal(o[0].cpu().numpy(), want["accept_len"])
+    np.testing.assert_array_equal(o[1].cpu().numpy(), want["bonus_token"])
+    np.testing.assert_array_equal(o[3].cpu().numpy(), want["n_commit"])
+    assert np.abs(ent.cpu().numpy().astype(np.float64) - want["entropy"]).max() <= 1e-3
+    far = np.abs(want["entropy"] - 2.0) >= 1e-4
+    np.testing.assert_array_equal(o[2].cpu().numpy()[far], want["route"][far])
