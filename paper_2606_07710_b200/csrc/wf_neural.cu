@@ -4,7 +4,7 @@
 //
 // The policy is a batched GEMV against 2.1 M weights (4.2 MB of bf16 at d = 4096): HBM/latency-bound, no
 // tensor cores.  One warp owns one hidden unit j: it streams row j of W1 exactly once per tile of 16
-// sequences (16-byte coalesced loads) against the 16 hidden rows staged in shared memory, reduces with a
+// sequences (16-byte coalesced loads; the tiles are spread over blockIdx.y) against the 16 hidden rows staged in shared memory, reduces with a
 // fixed shuffle tree, applies bias and the exact (erf) GELU and scales by w2[j].  A CTA (8 warps = 8 units)
 // adds its 8 terms in unit order and publishes one partial per sequence; the last CTA to finish (self-
 // resetting counter) adds the partials in CTA order, adds b2 and thresholds.  Every sum has a fixed order:
@@ -13,7 +13,7 @@
 
 namespace {
 
-constexpr int NR_WARPS = 8;            // hidden units per CTA
+constexpr int NR_WARPS = 8;            // hidden units per CTA (4 per CTA doubles the CTAs that each stage the 16 rows: 34 us against 24 at B = 16)
 constexpr int NR_TILE_B = 16;          // sequences staged per pass
 constexpr int NR_THREADS = NR_WARPS * 32;
 
@@ -56,7 +56,9 @@ __global__ void __launch_bounds__(NR_THREADS) wf_neural_route_kernel(const Neura
   const uint4* wrow = reinterpret_cast<const uint4*>(p.w1 + (size_t)min(j, p.m - 1) * p.d);
   uint4* hs = reinterpret_cast<uint4*>(smem);
 
-  for (int b0 = 0; b0 < p.B; b0 += NR_TILE_B) {
+  // blockIdx.y = tile of 16 sequences (the tiles run side by side: at B = 64 one CTA per unit group walking four tiles in turn
+  // took 108 us on 64 SMs)
+  for (int b0 = blockIdx.y * NR_TILE_B; b0 < p.B; b0 += gridDim.y * NR_TILE_B) {
     const int nb = min(NR_TILE_B, p.B - b0);
     // stage row a_b of each block (reading N4); an empty block stages zeros
     for (int i = tid; i < nb * chunks; i += NR_THREADS) {
@@ -122,7 +124,7 @@ __global__ void __launch_bounds__(NR_THREADS) wf_neural_route_kernel(const Neura
   __syncthreads();
   if (tid == 0) {
     const unsigned int old = atomicAdd(p.counter, 1u);
-    s_last = (old == gridDim.x - 1);
+    s_last = (old == gridDim.x * gridDim.y - 1);
     if (s_last) *p.counter = 0;                                                 // self-resetting
   }
   __syncthreads();
@@ -171,6 +173,7 @@ extern "C" int wf_neural_route(wf_ctx* ctx, const void* hidden_final, const int3
   p.counter = ctx->d_counters + (ctx->n_counters - 1);     // the accept sweep uses [0, B) with B <= 65535
   p.B = B; p.d = d; p.m = m; p.tau_is_scalar = tau_is_scalar;
   const int grid = (m + NR_WARPS - 1) / NR_WARPS;
-  wf_launch(wf_neural_route_kernel, dim3(grid), dim3(NR_THREADS), smem, (cudaStream_t)stream, p);
+  const int tiles = (B + NR_TILE_B - 1) / NR_TILE_B;
+  wf_launch(wf_neural_route_kernel, dim3(grid, tiles < 8 ? tiles : 8), dim3(NR_THREADS), smem, (cudaStream_t)stream, p);
   return wf_check_launch(ctx, "wf_neural_route_kernel");
 }
