@@ -101,7 +101,8 @@ size_t wf_verify_attn_workspace_bytes(const wf_kv_shape* shape, int B, int n_q_h
  * -1 (default): automatic: with few (sequence, kv head) pairs (batch 1-2 at 8 kv heads) one thread-block cluster per pair,
  * partials folded through distributed shared memory in a fixed order (bit-reproducible); otherwise, and whenever the
  * last launch over the same cache was long enough to be HBM-paced, persistent stream-K ranges over all SMs.
- * 0: never use clusters.  2..16: force that cluster size whenever the pairs fit (else stream-K). */
+ * 0: never use clusters.  1..16: force that many CTAs per pair whenever the pairs fit (else stream-K); 1 = one CTA per pair,
+ * no merge at all (what the automatic mode picks for an HBM-paced launch whose pairs cover at least 80 % of the SMs). */
 int wf_ctx_set_attn_cluster(wf_ctx* ctx, int cluster_size);
 /* Reproducible attention bits.  A (sequence, kv head) pair whose keys are split over several CTAs is merged from partial
  * (max, sum, O) triples.  on = 0 (default): in the stream-K shape the CTA that arrives last folds the others' partials into

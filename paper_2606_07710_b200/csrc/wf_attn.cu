@@ -311,7 +311,7 @@ __device__ __forceinline__ void attn_mma_qk(const AttnParams& p, AttnShared<TREE
     }
   }
   if constexpr (!TREE) {
-    if (sh.cl > 0) {
+    if (sh.cl > 1) {
       // Cluster mode: once the last QK^T has retired this CTA's K ring is idle and becomes its receive buffer: tell every
       // CTA of the cluster (they push their slices only when all are ready; in practice long before anybody is done)
       if (gt > 0) {
@@ -472,7 +472,7 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared<fal
   SegWalker<false> walk(sh, p.kv.n_kv_heads, blockIdx.x, lean);
   Segment sg;
   uint32_t gt0 = 0;                                            // global tile counter at the start of the segment
-  if (sh.cl > 0) {
+  if (sh.cl > 1) {
     // cluster mode: the row-dealing tables of the merge, by threads that would otherwise idle through the Q load's
     // integer work: group 1 builds them, everybody reads them behind the named barriers of the group merge
     const int Rt = min(lean->q_b * p.group, AT_ROWS);
@@ -702,7 +702,7 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared<fal
       l_run[h] += __shfl_xor_sync(0xffffffffu, l_run[h], 1);
       l_run[h] += __shfl_xor_sync(0xffffffffu, l_run[h], 2);
     }
-    if (sh.cl > 0) {
+    if (sh.cl > 1) {
       // Cluster mode: the partial (m, l, unnormalised O) of this CTA goes to its OWN shared memory (K stage 1 is idle: every
       // MMA has retired), then warp 0 pushes every owner its rows (attn_cluster_push).  Group 0 only.
       const int Rc = min(R, AT_ROWS);
@@ -857,7 +857,7 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared<fal
     }
     write_rows();
   }
-  if (sh.cl > 0) {
+  if (sh.cl > 1) {
     const int R = min(lean->q_b * p.group, AT_ROWS);
     if (gt0 == 0) {
       // a CTA without tiles still owes every owner a slice: l = 0 marks it empty (its O bits are never read)
@@ -1219,13 +1219,13 @@ __global__ void __launch_bounds__(AT_THREADS, 1) wf_verify_attn_kernel(const Att
     lean_sg.t_lo = rank * nt / p.cl; lean_sg.t_hi = (rank + 1) * nt / p.cl;
     lean_sg.flat0 = 0; lean_sg.r0 = r0; lean_sg.ctx = ctx; lean_sg.q_b = r1 - r0;
     lean_sg.k0 = lean_sg.t_lo * AT_BN; lean_sg.k1 = min(ctx + lean_sg.q_b, lean_sg.t_hi * AT_BN);
-    lean_sg.n_tiles = lean_sg.t_hi - lean_sg.t_lo; lean_sg.partial = 1; lean_sg.slot = 0;
+    lean_sg.n_tiles = lean_sg.t_hi - lean_sg.t_lo; lean_sg.partial = p.cl > 1; lean_sg.slot = 0;   // one CTA per pair: no merge at all
     if (tid == 0) {
       if (rank == 0 && lean_sg.g == 0 && (r1 - r0) * p.group > AT_ROWS) wf_raise(p.status, (int)WF_ERR_INVALID_ARG);
       // what this CTA will receive: from each of the cl CTAs, its rows [row_a, row_b) of (m, l) and of O
       const int R = min((r1 - r0) * p.group, AT_ROWS);
       const int n_mine = cl_row_begin(rank + 1, R, p.cl) - cl_row_begin(rank, R, p.cl);
-      if (nt > 0) mbar_arrive_expect_tx(smem_u32(&sh.cl_bar), (uint32_t)(p.cl * n_mine * (D * 4 + 8)));
+      if (nt > 0 && p.cl > 1) mbar_arrive_expect_tx(smem_u32(&sh.cl_bar), (uint32_t)(p.cl * n_mine * (D * 4 + 8)));
     }
   } else {
     // per-sequence table (tiles per kv head, q_indptr, context) from the device-resident lengths, identical in
@@ -1358,7 +1358,7 @@ __global__ void __launch_bounds__(AT_THREADS, 1) wf_verify_attn_kernel(const Att
     }
     // cluster mode: nobody leaves while a copy it pushed may still be reading its shared memory: a CTA arrives once
     // everything pushed TO it has landed (the softmax warps of a running CTA do so inside attn_softmax), and all wait
-    if (sh.cl > 0 && !(run && warp < 8)) { cluster_arrive(); cluster_wait(); }
+    if (sh.cl > 1 && !(run && warp < 8)) { cluster_arrive(); cluster_wait(); }
   }
   tc_fence_before();
   __syncthreads();
@@ -1408,20 +1408,27 @@ int launch_attn(wf_ctx* ctx, AttnParams& p, int* h_hint, cudaStream_t st) {
       cudaGetLastError();
     }
     int cl = 0;
-    const int hint = h_hint ? *(volatile int*)h_hint : -1;
+    // (deterministic mode: the shape may not depend on when the host happens to see the feedback value, or repeated calls
+    // would differ in their bits: the hint is ignored)
+    const int hint = (h_hint && !ctx->deterministic) ? *(volatile int*)h_hint : -1;
     const bool hbm_paced = hint >= 24 * grid;
+    tab[1] = grid;                                             // one CTA per pair needs no cluster
     if (ctx->attn_cluster_override > 0) cl = ctx->attn_cluster_override;
     else if (ctx->attn_cluster_override < 0 && pairs > 0) {
-      for (int c2 = 16; c2 >= 4; --c2)
+      for (int c2 = 16; c2 >= 1; --c2)
         if (tab[c2] >= pairs) { cl = c2; break; }
-      // an HBM-paced launch wants every SM: clusters only if they cover most of the machine (measured at batch 4, context
-      // 32768: 32 clusters of 4 = 128 CTAs stream 5.88 TB/s against 5.68 for stream-K ranges on 148: no global merge)
+      // An HBM-paced launch wants (nearly) every SM streaming: pair-aligned CTAs only if they cover most of the machine.
+      // Measured: batch 4, context 32768: 32 clusters of 4 = 128 CTAs stream 5.9-6.2 TB/s against 5.7 for stream-K ranges on
+      // 148 (no global merge, no partial traffic); batch 16, context 8192: 128 CTAs, one whole pair each, no merge at all.
       if (hbm_paced && pairs * cl * 5 < grid * 4) cl = 0;
+      // a latency-bound launch with one short pair per CTA gains nothing from this shape over stream-K's own small-launch path
+      if (!hbm_paced && cl == 1) cl = 0;
     }
-    if (cl > 1 && cl <= 16 && tab[cl] >= pairs) {
+    if (cl >= 1 && cl <= 16 && tab[cl] >= pairs) {
       p.cl = cl;
-      wf_launch_cluster(wf_verify_attn_kernel<D, TREE>, dim3(pairs * cl), dim3(AT_THREADS), smem, cl, st, p);
-      return wf_check_launch(ctx, "wf_verify_attn_kernel<cluster>");
+      if (cl == 1) wf_launch(wf_verify_attn_kernel<D, TREE>, dim3(pairs), dim3(AT_THREADS), smem, st, p);
+      else wf_launch_cluster(wf_verify_attn_kernel<D, TREE>, dim3(pairs * cl), dim3(AT_THREADS), smem, cl, st, p);
+      return wf_check_launch(ctx, cl == 1 ? "wf_verify_attn_kernel<pair per CTA>" : "wf_verify_attn_kernel<cluster>");
     }
   }
   wf_launch(wf_verify_attn_kernel<D, TREE>, dim3(grid), dim3(AT_THREADS), smem, st, p);
@@ -1569,8 +1576,8 @@ extern "C" int wf_verify_attn_tree(wf_ctx* ctx, const wf_paged_kv* kv, int layer
 
 extern "C" int wf_ctx_set_attn_cluster(wf_ctx* ctx, int cluster_size) {
   if (!ctx) return WF_ERR_INVALID_ARG;
-  WF_REQUIRE(ctx, cluster_size >= -1 && cluster_size <= 16 && cluster_size != 1, WF_ERR_INVALID_ARG,
-             "wf_ctx_set_attn_cluster: cluster_size must be -1 (automatic), 0 (never) or 2..16");
+  WF_REQUIRE(ctx, cluster_size >= -1 && cluster_size <= 16, WF_ERR_INVALID_ARG,
+             "wf_ctx_set_attn_cluster: cluster_size must be -1 (automatic), 0 (never) or 1..16");
   ctx->attn_cluster_override = cluster_size;
   return WF_OK;
 }
