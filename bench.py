@@ -547,7 +547,7 @@ def measure(ctx, wf, key, args, rank, world, local, main):
         "value": whole_job_value(K, world, ms), "unit": UNIT, "steps": K, "warmup": W,
         "ms_per_step": ms / K, "ms_per_step_median": float(np.median(spans)) if spans else ms / K,
         "config": config_dict(wl, world),
-        "run_notes": {"slots": rs.n_slots, "realised_switch_rate": flips,
+        "run_notes": {"slots": rs.n_slots, "realised_switch_rate": flips, "attn_early_kv": int(args.attn_early),
                       "l2": f"inputs larger than L2: {np.mean(attn_bytes) / 1e6:.0f} MB of KV per attention launch, distinct per layer",
                       "catchup": "lazy: one wf_switch_round per round (both drafters, masks derived on the device from route), then "
                                  "wf_final_token_full for the sequences that switched to the AR drafter"},
@@ -725,6 +725,11 @@ def run_ours(args):
     torch.cuda.set_device(local)
     from paper_2606_07710_b200 import binding as wf          # raises if libwhiflash.so is missing: no fallback
     ctx = wf.Ctx(local)
+    # the round is reserve -> L x attention -> accept -> switch -> final token: no kernel that precedes an attention launch
+    # writes lengths, old block-table entries or cached rows below the cached length (the promise of wf_ctx_set_attn_early_kv)
+    ctx.set_attn_early_kv(args.attn_early)
+    if args.attn_cluster != -1:
+        ctx.set_attn_cluster(args.attn_cluster)
     rec = measure(ctx, wf, args.workload, args, rank, world, local, main=True)
     per_config = {}
     for key in [k for k in args.sub_workloads.split(",") if k and k != args.workload]:
@@ -763,6 +768,9 @@ def main():
     ap.add_argument("--sub-e2e-steps", type=int, default=10)
     ap.add_argument("--slots", type=int, default=16, help="round slots of the cyclic schedule (distinct inputs and plans)")
     ap.add_argument("--e2e-steps", type=int, default=30)
+    ap.add_argument("--attn-early", type=int, default=1, choices=[0, 1],
+                    help="wf_ctx_set_attn_early_kv: attention launches stream the cached K/V ahead of the dependency wait")
+    ap.add_argument("--attn-cluster", type=int, default=-1, help="wf_ctx_set_attn_cluster (tuning hook; -1 = automatic)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-tree", action="store_true", help="skip the tree-verification leg (SURVEY.md §8(f) f2)")
     ap.add_argument("--cpu-sample-seqs", type=int, default=8)

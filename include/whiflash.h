@@ -104,6 +104,18 @@ size_t wf_verify_attn_workspace_bytes(const wf_kv_shape* shape, int B, int n_q_h
  * 0: never use clusters.  1..16: force that many CTAs per pair whenever the pairs fit (else stream-K); 1 = one CTA per pair,
  * no merge at all (what the automatic mode picks for an HBM-paced launch whose pairs cover at least 80 % of the SMs). */
 int wf_ctx_set_attn_cluster(wf_ctx* ctx, int cluster_size);
+/* Early K/V (off by default).  Every kernel of this library is launched with programmatic dependent launch and waits for
+ * the previous kernel of the stream before it touches anything that kernel may have written.  With on = 1 the caller
+ * PROMISES, for every later wf_verify_attn / wf_verify_attn_tree / wf_final_token_full through this context, that the
+ * kernel launched immediately before it on the same stream writes none of: q_indptr, the cache's seq_len, its block-table
+ * entries for pages below seq_len[b], and its K/V rows at positions below seq_len[b] (in a decoding loop these are the
+ * previous rounds' data: the preceding kernel is the layer's QKV projection, which writes Q and the block's own rows at
+ * positions >= seq_len[b], or wf_kv_reserve, which only appends block-table entries), and that this preceding kernel, if
+ * it uses programmatic launch completion itself, signals it only after its own dependency wait (this library's kernels do).
+ * The attention launch then reads lengths and page ids and streams the K/V tiles that lie wholly below seq_len[b] while
+ * the previous kernel is still running; only Q, the tree masks and the tiles holding the block's own rows wait for it.
+ * Results are identical; a broken promise is a data race.  PAPER.md:133 (batch 1: the round is a chain of short launches). */
+int wf_ctx_set_attn_early_kv(wf_ctx* ctx, int on);
 /* Reproducible attention bits.  A (sequence, kv head) pair whose keys are split over several CTAs is merged from partial
  * (max, sum, O) triples.  on = 0 (default): in the stream-K shape the CTA that arrives last folds the others' partials into
  * its own, so the order of the floating-point merges (not the tolerance) depends on timing.  on = 1: every merge folds

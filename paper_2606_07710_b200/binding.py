@@ -35,6 +35,7 @@ EXPORTS = [
     "wf_tree_masks", "wf_verify_attn_tree", "wf_accept_tree_entropy_route", "wf_kv_compact_path",
     "wf_accept_sample_entropy_route", "wf_switch_round",
     "wf_drafter_set_full_layer", "wf_final_token_workspace_bytes", "wf_final_token_full", "wf_ctx_set_attn_cluster", "wf_ctx_set_deterministic",
+    "wf_ctx_set_attn_early_kv",
 ]
 
 
@@ -75,6 +76,7 @@ _SIG = {
     "wf_final_token_workspace_bytes": (_sz, [_vp, _i]),
     "wf_ctx_set_attn_cluster": (_i, [_vp, _i]),
     "wf_ctx_set_deterministic": (_i, [_vp, _i]),
+    "wf_ctx_set_attn_early_kv": (_i, [_vp, _i]),
     "wf_final_token_full": (_i, [_vp, _vp, _vp, _vp, _vp, _vp, _i, _i, _vp, _vp, _sz, _vp]),
     "wf_neural_route_workspace_bytes": (_sz, [_i, _i]),
     "wf_neural_route": (_i, [_vp, _vp, _vp, _vp, _i, _i, _i, _vp, _vp, _vp, _vp, _vp, _i, _vp, _vp, _vp, _sz, _vp]),
@@ -134,6 +136,11 @@ class Ctx:
     def set_deterministic(self, on):
         """Attention merges fold a pair's partials in key-range order (bit-reproducible) instead of last-arriver order."""
         self.check(lib.wf_ctx_set_deterministic(self.h, 1 if on else 0))
+
+    def set_attn_early_kv(self, on):
+        """Attention launches read lengths, page ids and the K/V below the cached length ahead of the dependency wait
+        (the caller promises the preceding kernel of the stream writes none of them; see whiflash.h)."""
+        self.check(lib.wf_ctx_set_attn_early_kv(self.h, 1 if on else 0))
 
     def set_attn_cluster(self, cluster_size):
         """Launch shape of wf_verify_attn: -1 automatic, 0 never clusters, 2..16 force that cluster size."""

@@ -59,8 +59,8 @@ wf_accept_kernel(const float* __restrict__ logits, int V, int n_chunks, const in
                  int* __restrict__ status) {
   // parent == nullptr: chain block (C6).  Else tree block (T1-T4): greedy walk over parent pointers, the accepted
   // node indices go to path[b][0..a] (-1 beyond), and the cache length is left to wf_kv_compact_path.
-  wf_pdl_trigger();
   wf_pdl_wait();
+  wf_pdl_trigger();
   const int b = blockIdx.z, i = blockIdx.y, chunk = blockIdx.x;
   const int r0 = q_indptr[b];
   const size_t prow0 = (size_t)b * gridDim.y;             // partials are indexed by (sequence, row): in bounds whatever q_indptr says

@@ -62,6 +62,9 @@ struct AttnParams {
   int layer, B, n_q_heads, group;
   int cl;                              // > 0: cluster mode (launched with clusters of `cl` CTAs, one cluster per (b, g) pair)
   int deterministic;                   // stream-K merges fold the partials of a pair in range order, whoever arrives last
+  int early;                           // wf_ctx_set_attn_early_kv: lengths, page ids and the K/V tiles below the cached length are
+                                       // read AHEAD of the dependency wait (only Q, the tree masks and the tiles that hold the
+                                       // block's own rows wait for the previous kernel of the stream)
   int ctx_adj;                         // added to seq_len: 0 for verification (the block sits behind the cache length, C10);
                                        // -1 for the final-token path (wf_final.cu: the token is the last cached one, F1)
   float scale_log2;                    // sm_scale * log2(e)
@@ -219,18 +222,25 @@ __device__ __forceinline__ void attn_loader(const AttnParams& p, AttnShared<TREE
   constexpr int PP = AT_BN / 16;                              // pages per tile
   const void* tmap = kv.tmaps + which;
   const uint32_t ring_s = smem_u32(ring);
+  // Early mode: tiles that lie wholly below the cached length (rows and block-table entries of earlier rounds) are fetched
+  // ahead of the dependency wait; the wait comes before the first page id of a tile that reaches the block's own rows
+  // (page ids are fetched one tile ahead, hence the look-ahead of one tile).
+  bool waited = !p.early;
   while (walk.next(sg)) {
+    if (!waited && sg.k0 + AT_BN > sg.ctx) { wf_pdl_wait(); waited = true; }
     const int32_t* bt = kv.block_table + (size_t)sg.b * kv.max_pages_per_seq + (sg.k0 >> 4);
     const int pages_seg = (sg.k1 - sg.k0 + 15) >> 4;           // pages of this segment, tile t takes [8t, 8t+8)
     // The page ids of tile t+1 are fetched while tile t is issued: the block-table latency is off the ring's
-    // critical path.  Lane q holds page q of the tile.
-    int page_next = lane < min(PP, pages_seg) ? __ldg(bt + lane) : 0;
+    // critical path.  Lane q holds page q of the tile.  (L2 loads: in early mode a line fetched ahead of the wait may
+    // hold entries the previous kernel writes later.)
+    int page_next = lane < min(PP, pages_seg) ? __ldcg(bt + lane) : 0;
     for (int t = 0; t < sg.n_tiles; ++t, ++gt) {
       const int n_st = which ? sh.n_stv : sh.n_stk;
       const int st = gt % n_st;
       const int npages = min(PP, pages_seg - t * PP);
       const int row = (((p.layer * kv.num_pages + page_next) * kv.n_kv_heads) + sg.g) * 16;
-      if ((t + 1) * PP + lane < pages_seg && lane < PP) page_next = __ldg(bt + (t + 1) * PP + lane);
+      if (!waited && sg.k0 + (t + 2) * AT_BN > sg.ctx) { wf_pdl_wait(); waited = true; }
+      if ((t + 1) * PP + lane < pages_seg && lane < PP) page_next = __ldcg(bt + (t + 1) * PP + lane);
       int rows[PP];
 #pragma unroll
       for (int q = 0; q < PP; ++q) rows[q] = __shfl_sync(0xffffffffu, row, q);
@@ -472,6 +482,7 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared<fal
   SegWalker<false> walk(sh, p.kv.n_kv_heads, blockIdx.x, lean);
   Segment sg;
   uint32_t gt0 = 0;                                            // global tile counter at the start of the segment
+  bool waited = !p.early;
   if (sh.cl > 1) {
     // cluster mode: the row-dealing tables of the merge, by threads that would otherwise idle through the Q load's
     // integer work: group 1 builds them, everybody reads them behind the named barriers of the group merge
@@ -506,6 +517,12 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared<fal
     }
     // ---- Q tile -> smem (K-major, 128-byte swizzle) by both groups; rows >= R are zero.  Every MMA of the
     //      previous segment has retired (both groups waited for their last pv_done). ----
+    if (!waited) {                                             // early mode: Q is what the previous kernel produces
+      wf_pdl_wait();
+      if (grp == 0 && stid == 0) wf_pdl_trigger();
+      waited = true;
+      WF_PROBE_AT(15, warp == 0 && lane == 0);
+    }
     {
       // all loads first, then the stores: one round trip instead of one per chunk
       constexpr int NQ = AT_ROWS * (D / 8) / 256;
@@ -900,6 +917,7 @@ __device__ __forceinline__ void attn_softmax_tree(const AttnParams& p, AttnShare
   SegWalker<true> walk(sh, p.kv.n_kv_heads, blockIdx.x, nullptr);
   Segment sg;
   uint32_t gt0 = 0;                                            // global tile counter at the start of the segment
+  bool waited = !p.early;
   while (walk.next(sg)) {
     const int n_mine = max(0, min(sg.q_b - grp * npt, npt));   // nodes of this group's sub-block
     const int R = n_mine * p.group;                            // its live rows
@@ -919,6 +937,11 @@ __device__ __forceinline__ void attn_softmax_tree(const AttnParams& p, AttnShare
     }
     // ---- Q tile -> smem: 128 rows (K-major, 128-byte swizzle) by both groups; padding rows are zero.  Every MMA of the
     //      previous segment has retired (both groups waited for the last pv_done). ----
+    if (!waited) {                                             // early mode: Q and the masks are the previous kernels' outputs
+      wf_pdl_wait();
+      if (grp == 0 && stid == 0) wf_pdl_trigger();
+      waited = true;
+    }
     {
       constexpr int NQ = 128 * (D / 8) / 256;
       uint4 qv[NQ];
@@ -1162,7 +1185,6 @@ __global__ void __launch_bounds__(AT_THREADS, 1) wf_verify_attn_kernel(const Att
   // barrier init and TMEM allocation touch no global memory: they run before the dependency wait and overlap the
   // tail of the previous kernel of the stream (programmatic dependent launch)
   WF_PROBE_AT(0, tid == 0);
-  wf_pdl_trigger();
   if (tid == 0) {
     for (int i = 0; i < AT_MAX_STAGES; ++i) {
       mbar_init(smem_u32(&sh.k_full[i]), 1); mbar_init(smem_u32(&sh.k_empty[i]), 1);
@@ -1197,7 +1219,9 @@ __global__ void __launch_bounds__(AT_THREADS, 1) wf_verify_attn_kernel(const Att
   }
   if (tid == 32 * 8 || tid == 32 * 10)                         // the K / V tensor maps are constants: fetch them ahead of the wait
     asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(p.kv.tmaps + (tid == 32 * 10 ? 1 : 0))) : "memory");
-  wf_pdl_wait();
+  // The successor may be scheduled once this launch has passed ITS dependency wait (wf_internal.cuh).  Early mode: the roles
+  // wait where they first need the previous kernel's output (loaders: the tiles with the block's own rows; softmax warps: Q).
+  if (!p.early) { wf_pdl_wait(); wf_pdl_trigger(); }
   WF_PROBE_AT(1, tid == 0);
   // Cluster mode: a CTA serves ONE (b, g) pair.  Every thread loads that sequence's three lengths itself (one global round
   // trip, the same for all) and derives the CTA's one segment in registers: no table, no barrier behind the dependency wait
@@ -1334,6 +1358,7 @@ __global__ void __launch_bounds__(AT_THREADS, 1) wf_verify_attn_kernel(const Att
   const bool run = lean ? lean_nt > 0 : (sh.total_tiles > 0 && (int)blockIdx.x < sh.g_eff);
   const Segment* lp = lean ? &lean_sg : nullptr;
   WF_PROBE_AT(2, tid == 0);
+  if (p.early && !run && tid == 0) { wf_pdl_wait(); wf_pdl_trigger(); }   // an idle CTA must not hold back the successor's launch
   if (run) {
     if (warp < 8) {
       asm volatile("setmaxnreg.inc.sync.aligned.u32 216;");
@@ -1441,8 +1466,8 @@ int launch_attn(wf_ctx* ctx, AttnParams& p, int* h_hint, cudaStream_t st) {
 __global__ void __launch_bounds__(64) wf_tree_masks_kernel(const int32_t* parent, const int32_t* q_indptr,
                                                            unsigned long long* mask, int* status) {
   __shared__ int par[64];
-  wf_pdl_trigger();
   wf_pdl_wait();
+  wf_pdl_trigger();
   const int b = blockIdx.x, i = threadIdx.x;
   const int r0 = q_indptr[b], n = min(q_indptr[b + 1] - r0, 64);
   if (i < n) par[i] = parent[r0 + i];
@@ -1498,6 +1523,7 @@ int wf_attn_launch_chain(wf_ctx* ctx, const wf_paged_kv* kv, int layer, const vo
   p.layer = layer; p.B = B; p.n_q_heads = n_q_heads; p.group = group;
   p.ctx_adj = ctx_adj;
   p.deterministic = ctx->deterministic;
+  p.early = ctx->attn_early;
   p.scale_log2 = sm_scale * LOG2E;
   p.ws_o = (float4*)workspace;
   p.ws_ml = (float4*)((char*)workspace + items * r_pad * kv->s.head_dim * sizeof(float));
@@ -1562,6 +1588,7 @@ extern "C" int wf_verify_attn_tree(wf_ctx* ctx, const wf_paged_kv* kv, int layer
   p.layer = layer; p.B = B; p.n_q_heads = n_q_heads; p.group = group;
   p.ctx_adj = 0;
   p.deterministic = ctx->deterministic;
+  p.early = ctx->attn_early;
   p.scale_log2 = sm_scale * LOG2E;
   p.ws_o = (float4*)workspace;
   p.ws_ml = (float4*)((char*)workspace + items * AT_ROWS * kv->s.head_dim * sizeof(float));
@@ -1579,6 +1606,12 @@ extern "C" int wf_ctx_set_attn_cluster(wf_ctx* ctx, int cluster_size) {
   WF_REQUIRE(ctx, cluster_size >= -1 && cluster_size <= 16, WF_ERR_INVALID_ARG,
              "wf_ctx_set_attn_cluster: cluster_size must be -1 (automatic), 0 (never) or 1..16");
   ctx->attn_cluster_override = cluster_size;
+  return WF_OK;
+}
+
+extern "C" int wf_ctx_set_attn_early_kv(wf_ctx* ctx, int on) {
+  if (!ctx) return WF_ERR_INVALID_ARG;
+  ctx->attn_early = on ? 1 : 0;
   return WF_OK;
 }
 

@@ -67,6 +67,7 @@ extern "C" int wf_ctx_create(wf_ctx** out, int device_ordinal) {
   c->launches = 0;
   c->func_configured = 0;
   c->deterministic = 0;
+  c->attn_early = 0;
   memset(c->attn_max_clusters, 0, sizeof(c->attn_max_clusters));
   c->attn_cluster_override = -1;
   c->err[0] = 0;
@@ -188,8 +189,8 @@ extern "C" const int32_t* wf_kv_pages_held(const wf_paged_kv* kv) { return kv ? 
 
 __global__ void __launch_bounds__(1024) wf_kv_reserve_kernel(KvView kv, const int32_t* __restrict__ add_tokens,
                                                              int B, int* status) {
-  wf_pdl_trigger();
   wf_pdl_wait();
+  wf_pdl_trigger();
   kv_reserve_block(kv, B, [&](int b) { return add_tokens[b]; }, [](int b) { return b; }, status);
 }
 
@@ -204,8 +205,8 @@ extern "C" int wf_kv_reserve(wf_paged_kv* kv, const int32_t* add_tokens, int B, 
 
 __global__ void wf_kv_release_kernel(KvView kv, int seq) {
   // pages return to the ring tail in block-table order
-  wf_pdl_trigger();
   wf_pdl_wait();
+  wf_pdl_trigger();
   const int held = kv.pages_held[seq];
   const int head = kv.ring_state[0], count = kv.ring_state[1];
   int32_t* row = kv.block_table + (size_t)seq * kv.max_pages_per_seq;
@@ -241,8 +242,8 @@ __global__ void __launch_bounds__(256) wf_kv_compact_path_kernel(KvView kv, cons
                                                                  int path_stride, const int32_t* __restrict__ n_commit,
                                                                  int* status) {
   __shared__ int s_src[64], s_dst[64];                      // row index in the pool's [page][head][slot] order, head 0
-  wf_pdl_trigger();
   wf_pdl_wait();
+  wf_pdl_trigger();
   const int b = blockIdx.x, layer = blockIdx.y;
   const int nc = min(n_commit[b], 64);
   if (nc <= 1) return;                                      // the root is in place
@@ -279,8 +280,8 @@ __global__ void __launch_bounds__(256) wf_kv_compact_path_kernel(KvView kv, cons
 }
 
 __global__ void wf_kv_advance_kernel(int32_t* __restrict__ seq_len, const int32_t* __restrict__ n_commit, int B) {
-  wf_pdl_trigger();
   wf_pdl_wait();
+  wf_pdl_trigger();
   const int b = blockIdx.x * blockDim.x + threadIdx.x;
   if (b < B) seq_len[b] += n_commit[b];
 }

@@ -67,8 +67,8 @@ __global__ void __launch_bounds__(FT_PLAN_THREADS) wf_final_plan_kernel(const Ft
   __shared__ int s_b[FT_MAX_TOK];
   __shared__ int s_total;
   const int tid = threadIdx.x, lane = tid & 31;
-  wf_pdl_trigger();
   wf_pdl_wait();
+  wf_pdl_trigger();
   if (tid < 32) {                                             // every CTA derives the same compaction (ascending b)
     int run = 0;
     for (int base = 0; base < p.B; base += 32) {
@@ -162,7 +162,6 @@ __global__ void __launch_bounds__(FT_THREADS, 1) wf_final_gemm_kernel(const __gr
   __shared__ uint32_t s_tmem;
   __shared__ int s_last;
 
-  wf_pdl_trigger();
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int tile = (int)blockIdx.x / p.n_split, split = (int)blockIdx.x % p.n_split;
   const int tiles_n = p.N / FT_TILE;
@@ -193,6 +192,7 @@ __global__ void __launch_bounds__(FT_THREADS, 1) wf_final_gemm_kernel(const __gr
   }
   __syncwarp();
   wf_pdl_wait();
+  wf_pdl_trigger();
   const int M = min(*p.m_total, p.m_cap);
   if (M == 0) {
     // nobody switched: let the prefetched stages land (shared memory must outlive the copies), return the TMEM columns

@@ -22,6 +22,7 @@ struct wf_ctx {
   int deterministic;           // wf_ctx_set_deterministic: fixed-order split merges
   int attn_max_clusters[2][17]; // [D == 64][cluster size]: co-resident clusters of the chain attention kernel (0 = not queried)
   int attn_cluster_override;   // test / tuning hook: -1 = automatic, 0 = never, n > 0 = force cluster size n
+  int attn_early;              // wf_ctx_set_attn_early_kv
   char err[256];
 };
 
@@ -127,10 +128,14 @@ int wf_check_launch(wf_ctx* ctx, const char* what);   // cudaGetLastError -> WF_
 // ---------------------------------------------------------------------------------------------
 // Programmatic dependent launch.  Every kernel of the library is launched with programmatic stream
 // serialisation: it may be scheduled while the previous kernel of the stream is still running.  A
-// kernel calls wf_pdl_trigger() first (its successor may start launching) and wf_pdl_wait() before
-// its first access to global memory (blocks until the previous grid has completed and its writes
-// are visible); since every kernel waits before it finishes, completion is transitive.  What runs
-// before the wait (barrier init, TMEM allocation, launch latency) overlaps the predecessor's tail.
+// kernel calls wf_pdl_wait() before its first access to global memory that another kernel may have
+// written (blocks until the previous grid has completed and its writes are visible) and
+// wf_pdl_trigger() right AFTER it (its successor may then be scheduled).  Order matters: a successor
+// that starts only once this kernel has passed its wait knows that everything up to this kernel's
+// PREDECESSOR is complete, so it may read, ahead of its own wait, whatever this kernel does not
+// write (constants such as weights; in the attention kernel's early mode also the lengths, page ids
+// and K/V rows of earlier rounds).  What runs before the wait (barrier init, TMEM allocation,
+// prefetches, launch latency) overlaps the predecessor.
 // ---------------------------------------------------------------------------------------------
 #ifdef __CUDACC__
 __device__ __forceinline__ void wf_pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }

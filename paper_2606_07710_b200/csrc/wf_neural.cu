@@ -48,8 +48,8 @@ __global__ void __launch_bounds__(NR_THREADS) wf_neural_route_kernel(const Neura
   extern __shared__ __align__(16) uint8_t smem[];          // [NR_TILE_B][d] bf16
   __shared__ float s_term[NR_WARPS][NR_TILE_B];
   __shared__ int s_last;
-  wf_pdl_trigger();
   wf_pdl_wait();
+  wf_pdl_trigger();
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int chunks = p.d / 8;                               // 16-byte chunks per row
   const int j = blockIdx.x * NR_WARPS + warp;               // this warp's hidden unit

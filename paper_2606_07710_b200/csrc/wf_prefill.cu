@@ -92,8 +92,8 @@ __global__ void __launch_bounds__(PP_THREADS) wf_plan_pack_kernel(const __grid_c
   __shared__ int s_carry;
   __shared__ int s_n[PP_MAX_B], s_nb[PP_MAX_B], s_off[PP_MAX_B + 1], s_eb[PP_MAX_B], s_nl[PP_MAX_B];
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5, nw = PP_THREADS >> 5;
-  wf_pdl_trigger();
   wf_pdl_wait();
+  wf_pdl_trigger();
   const int jb = (int)blockIdx.x >= pp.ctas_job0 ? 1 : 0;
   const PlanJob& p = pp.job[jb];
   const int c = (int)blockIdx.x - (jb ? pp.ctas_job0 : 0);
@@ -307,7 +307,6 @@ __global__ void __launch_bounds__(PF_THREADS, 1) wf_prefill_gemm_kernel(const __
   __shared__ int s_last;
   constexpr int W_PRE = PF_W_PRE_BYTES / W_BYTES;          // W slots valid under every layout
 
-  wf_pdl_trigger();
   const int jb = (int)blockIdx.x >= gp.ctas_job0 ? 1 : 0;
   const GemmJob& p = gp.job[jb];
   const int cta = (int)blockIdx.x - (jb ? gp.ctas_job0 : 0);
@@ -345,6 +344,7 @@ __global__ void __launch_bounds__(PF_THREADS, 1) wf_prefill_gemm_kernel(const __
   }
   __syncwarp();
   wf_pdl_wait();
+  wf_pdl_trigger();
   const int M = *p.m_total;
 
   // Enqueue and commit ride on this kernel (kernel 1 has packed the projection's operand, backlog rows included, so

@@ -41,6 +41,9 @@ def wf():
     assert torch.cuda.is_available(), "gpu tests need a CUDA device"
     from paper_2606_07710_b200 import binding
     ctx = binding.Ctx(0)
+    # the launch mode bench.py times: rounds.py keeps the promise of wf_ctx_set_attn_early_kv (no kernel that precedes an
+    # attention launch writes lengths, old block-table entries or rows below the cached length)
+    ctx.set_attn_early_kv(1)
     yield binding, ctx
     ctx.close()
 
@@ -208,6 +211,50 @@ def test_cfg5_whole_rounds(wf):
     r = _round_parity(wf, 4, 3, lambda B: [0, 21, 42, 63], [2, 13, 27], sample_rows=[0, 3, 7, 15])
     assert r["routes"] == {0, 1} and r["flushes"] > 0 and r["n_final"] > 0, r
     print("cfg5", r)
+
+
+@pytest.mark.parametrize("index,layers,n_rounds", [(1, 36, 12), (2, 3, 6), (4, 2, 5)])
+def test_early_kv_rounds_bit_identical_to_waiting_rounds(index, layers, n_rounds):
+    """wf_ctx_set_attn_early_kv changes WHEN an attention launch reads the cache (ahead of its dependency wait), never what
+    it computes: whole rounds launched back to back without a host synchronisation (every launch overlaps the tail of the
+    previous one: reserve -> layers x attention -> accept -> switch -> final token -> reserve ...) leave the same bits in
+    every output as the same rounds with the mode off.  Both contexts fold split pairs in a fixed order (deterministic mode)
+    so that equality of bits is the expectation.  cfg2 takes the cluster shape at full depth, cfg3 / cfg5 stream-K ranges."""
+    import torch
+    from paper_2606_07710_b200 import binding
+    from paper_2606_07710_b200.rounds import RoundState
+    wl = synth.WORKLOADS[index]
+    runs = []
+    for early in (0, 1):
+        ctx = binding.Ctx(0)
+        ctx.set_deterministic(1)
+        ctx.set_attn_early_kv(early)
+        rs = RoundState(ctx, wl, n_slots=n_rounds, n_rounds_max=n_rounds + 2, layers=layers)
+        outs = []
+        for _ in range(n_rounds):
+            s = rs.run_round()
+            outs.append((s.attn_out.clone(), {k: v.clone() for k, v in rs.out.items()}, rs.ft.h_out.clone()))
+        torch.cuda.synchronize()
+        assert ctx.poll_status() == 0
+        runs.append((ctx, rs, outs))
+    (ctx0, rs0, outs0), (ctx1, rs1, outs1) = runs
+    try:
+        assert torch.equal(rs0.seq_len, rs1.seq_len)
+        for rnd, ((a0, o0, h0), (a1, o1, h1)) in enumerate(zip(outs0, outs1)):
+            diff = int((a0.view(torch.int16) != a1.view(torch.int16)).sum())
+            assert diff == 0, (wl.name, rnd, "attention output bits", diff)
+            for k in o0:
+                assert torch.equal(o0[k], o1[k]), (wl.name, rnd, k)
+            assert torch.equal(h0.view(torch.int16), h1.view(torch.int16)), (wl.name, rnd, "final-token state bits")
+        for n in rs0.drafters:
+            d0, d1 = rs0.drafters[n], rs1.drafters[n]
+            assert torch.equal(d0.seq_len, d1.seq_len) and torch.equal(d0.backlog_len, d1.backlog_len), (wl.name, n)
+            assert torch.equal(d0.k_pool.view(torch.int16), d1.k_pool.view(torch.int16)), (wl.name, n, "K pool")
+            assert torch.equal(d0.v_pool.view(torch.int16), d1.v_pool.view(torch.int16)), (wl.name, n, "V pool")
+    finally:
+        for ctx, rs, _ in runs:
+            rs.close()
+            ctx.close()
 
 
 def test_cfg4_flush_of_64_deferred_tokens_bit_identical_to_eager(wf):

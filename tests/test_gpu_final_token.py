@@ -16,12 +16,16 @@ pytestmark = pytest.mark.gpu
 H_REL_L2 = 5e-3
 
 
-@pytest.fixture(scope="module")
-def wf():
+@pytest.fixture(scope="module", params=[0, 1], ids=["wait", "early_kv"])
+def wf(request):
+    """Every test runs twice: attention launches wait for the previous kernel before anything else (default), or stream the
+    cached K/V ahead of that wait (wf_ctx_set_attn_early_kv; in these tests the caches and lengths are set up by uploads and by
+    library calls that are followed by other work before the attention launch, which is the promise that mode asks for)."""
     import torch
     assert torch.cuda.is_available(), "gpu tests need a CUDA device"
     from paper_2606_07710_b200 import binding
     ctx = binding.Ctx(0)
+    ctx.set_attn_early_kv(request.param)
     yield binding, ctx
     ctx.close()
 
