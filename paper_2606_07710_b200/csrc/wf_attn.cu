@@ -571,7 +571,36 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared<fal
     bool pending = false;                                      // a PV of this group is in flight and not folded yet
     uint32_t g_prev = 0;
     const int t_first = ((gt0 & 1) == (uint32_t)grp) ? 0 : 1;
-    for (int t = t_first; t < sg.n_tiles; t += 2) {
+    // A warp whose 16 rows are all padding (rows >= R: a gamma = 7 block with 4 query heads per kv head fills 32 of the 64
+    // rows) walks the tiles through the barrier protocol alone: it never reads S, its P rows keep whatever the buffer held
+    // (a P row only feeds its own O row, which nobody reads) and its (m, l, O) stay (-inf, 0, 0).  A loop of its own,
+    // so that the live warps' code is untouched.
+    const bool live = qw * 16 < R;
+    for (int t = t_first; !live && t < sg.n_tiles; t += 2) {
+      const uint32_t g2 = gt0 + t;
+      const int tk0 = sg.k0 + t * AT_BN;
+      mbar_wait(smem_u32(&sh.s_full[grp]), (g2 >> 1) & 1);
+      mbar_arrive(smem_u32(&sh.s_empty[grp]));
+      if (tk0 + AT_BN > sg.k1) {                               // its share of the stale V rows of the last tile (see below)
+        if (pending) mbar_wait(smem_u32(&sh.pv_done[grp]), (g_prev >> 1) & 1);
+        mbar_wait(smem_u32(&sh.v_full[g2 % sh.n_stv]), (g2 / sh.n_stv) & 1);
+        const int key = (sg.k1 - tk0) + stid;
+        if (key < AT_BN) {
+          uint8_t* vrow = v_s + (size_t)(g2 % sh.n_stv) * C::K_BYTES + key * 128;
+#pragma unroll
+          for (int h = 0; h < C::NH; ++h)
+#pragma unroll
+            for (int c = 0; c < 8; ++c) *reinterpret_cast<uint4*>(vrow + h * C::KV_HALF + c * 16) = make_uint4(0, 0, 0, 0);
+        }
+      }
+      if (pending) mbar_wait(smem_u32(&sh.pv_done[grp]), (g_prev >> 1) & 1);
+      fence_proxy_async();
+      mbar_arrive(smem_u32(&sh.p_full[grp]));
+      if (pending) mbar_arrive(smem_u32(&sh.o_empty[grp]));
+      pending = true;
+      g_prev = g2;
+    }
+    for (int t = t_first; live && t < sg.n_tiles; t += 2) {
       const uint32_t g2 = gt0 + t;
       const int tk0 = sg.k0 + t * AT_BN;
       mbar_wait(smem_u32(&sh.s_full[grp]), (g2 >> 1) & 1);
@@ -655,7 +684,10 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared<fal
       pending = true;
       g_prev = g2;
     }
-    if (pending) {
+    if (pending && !live) {
+      mbar_wait(smem_u32(&sh.pv_done[grp]), (g_prev >> 1) & 1);
+      mbar_arrive(smem_u32(&sh.o_empty[grp]));
+    } else if (pending) {
       mbar_wait(smem_u32(&sh.pv_done[grp]), (g_prev >> 1) & 1);
       WF_PROBE_AT(24, warp == 4 && lane == 0);
       tc_fence_after();
