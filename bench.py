@@ -528,15 +528,25 @@ def measure(ctx, wf, key, args, rank, world, local, main):
             t1.record()
             torch.cuda.synchronize()
             us = 1e3 * t0.elapsed_time(t1) / 20
-            ft_rec[tag] = {"tokens": n_tok, "us_per_call": us, "weight_gbs": rs.ft.weight_bytes / (us * 1e-6) / 1e9 if n_tok else None}
+            # algorithmic bytes of a call: the layer's four matrices once + the drafter-cache K/V of the selected sequences
+            # (one query row each over its whole cached context, every drafter layer)
+            dA = rs.drafters["A"]
+            lens = dA.seq_len.cpu().numpy().astype(np.int64)
+            picked = lens if sel is None else lens[s.masks["A"].flush_host.astype(bool)]
+            kv_bytes = int(picked.sum()) * sh.n_kv_heads * sh.head_dim * 2 * 2 * dA.n_layers
+            tot = rs.ft.weight_bytes + kv_bytes
+            ft_rec[tag] = {"tokens": n_tok, "us_per_call": us, "kv_bytes": kv_bytes,
+                           "weight_gbs": rs.ft.weight_bytes / (us * 1e-6) / 1e9 if n_tok else None,
+                           "hbm_gbs": tot / (us * 1e-6) / 1e9 if n_tok else None}
 
     peak, peak_src = measured_peaks()
     if ft_rec:
         for tag in ("switching", "whole_batch"):
-            g_ = ft_rec[tag]["weight_gbs"]
+            g_ = ft_rec[tag]["hbm_gbs"]
             ft_rec[tag]["frac_of_hbm_peak"] = g_ / peak if g_ else None
         ft_rec["note"] = ("wf_final_token_full for the AR drafter (one transformer layer, PAPER.md:231): Q/O/up/down weight streams "
-                          "(bytes = weight_bytes) + one-row attention over the drafter cache; 'switching' = the sequences the "
+                          "(weight_bytes) + one-row attention over the drafter cache (kv_bytes of the selected sequences); hbm_gbs and "
+                          "frac_of_hbm_peak count both; 'switching' = the sequences the "
                           "last timed slot switches to the AR drafter, 'whole_batch' = every sequence; back-to-back calls")
     avg_launch_ms = attn_ms / (K * L)
     achieved = float(np.mean(attn_bytes)) / (avg_launch_ms * 1e-3) / 1e9

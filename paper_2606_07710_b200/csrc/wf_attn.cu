@@ -565,7 +565,11 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared<fal
       tc_fence_before();
       mbar_arrive(smem_u32(&sh.o_empty[grp]));
 #pragma unroll
-      for (int c = 0; c < NO; ++c) o[c] = fmaf(o[c], alpha_prev[(c >> 1) & 1], __uint_as_float(v[c]));
+      for (int c = 0; c < NO; c += 2) {
+        const float a = alpha_prev[(c >> 1) & 1];
+        const float2 r = ffma2(make_float2(o[c], o[c + 1]), make_float2(a, a), make_float2(__uint_as_float(v[c]), __uint_as_float(v[c + 1])));
+        o[c] = r.x; o[c + 1] = r.y;
+      }
     };
 
     bool pending = false;                                      // a PV of this group is in flight and not folded yet
@@ -636,13 +640,18 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared<fal
       }
       uint32_t pk[32];
 #pragma unroll
+      float2 rs2[2] = {make_float2(0.f, 0.f), make_float2(0.f, 0.f)};
+      const float2 sc2 = make_float2(p.scale_log2, p.scale_log2);
+#pragma unroll
       for (int c = 0; c < 64; c += 2) {
         const int h = (c >> 1) & 1;
-        const float p0 = fast_exp2(fmaf(__uint_as_float(sv[c]), p.scale_log2, -m_use[h]));
-        const float p1 = fast_exp2(fmaf(__uint_as_float(sv[c + 1]), p.scale_log2, -m_use[h]));
-        rs[h] += p0 + p1;
+        const float2 x = ffma2(make_float2(__uint_as_float(sv[c]), __uint_as_float(sv[c + 1])), sc2, make_float2(-m_use[h], -m_use[h]));
+        const float p0 = fast_exp2(x.x), p1 = fast_exp2(x.y);
+        rs2[h] = fadd2(rs2[h], make_float2(p0, p1));
         pk[c >> 1] = pack_bf16(p0, p1);
       }
+      rs[0] = rs2[0].x + rs2[0].y;
+      rs[1] = rs2[1].x + rs2[1].y;
       l_run[0] = l_run[0] * alpha[0] + rs[0];
       l_run[1] = l_run[1] * alpha[1] + rs[1];
       WF_PROBE_AT(21 + 6 * pti, warp == 4 && lane == 0 && pti < 2);
@@ -1015,7 +1024,11 @@ __device__ __forceinline__ void attn_softmax_tree(const AttnParams& p, AttnShare
       tc_fence_before();
       mbar_arrive(smem_u32(&sh.o_empty[gprev & 1]));
 #pragma unroll
-      for (int c = 0; c < NO; ++c) o[c] = fmaf(o[c], alpha_prev[(c >> 1) & 1], __uint_as_float(v[c]));
+      for (int c = 0; c < NO; c += 2) {
+        const float a = alpha_prev[(c >> 1) & 1];
+        const float2 r = ffma2(make_float2(o[c], o[c + 1]), make_float2(a, a), make_float2(__uint_as_float(v[c]), __uint_as_float(v[c + 1])));
+        o[c] = r.x; o[c + 1] = r.y;
+      }
     };
 
     for (int t = 0; t < sg.n_tiles; ++t) {
@@ -1053,18 +1066,22 @@ __device__ __forceinline__ void attn_softmax_tree(const AttnParams& p, AttnShare
         m_run[h] = m_new;
       }
       uint32_t pk[32];
+      float2 rs2[2] = {make_float2(0.f, 0.f), make_float2(0.f, 0.f)};
+      const float2 sc2 = make_float2(p.scale_log2, p.scale_log2);
 #pragma unroll
       for (int c = 0; c < 64; c += 2) {
         // Both groups run this phase at the same time and the four MUFUs of a sub-partition are its bottleneck (64 ex2
         // per thread and tile): every fourth pair is evaluated on the FMA pipe instead, which balances the two pipes.
         const int h = (c >> 1) & 1;
-        const float x0 = fmaf(__uint_as_float(sv[c]), p.scale_log2, -m_use[h]);
-        const float x1 = fmaf(__uint_as_float(sv[c + 1]), p.scale_log2, -m_use[h]);
-        const float p0 = (c & 6) == 0 ? poly_exp2(x0) : fast_exp2(x0);
-        const float p1 = (c & 6) == 0 ? poly_exp2(x1) : fast_exp2(x1);
-        rs[h] += p0 + p1;
-        pk[c >> 1] = pack_bf16(p0, p1);
+        const float2 x = ffma2(make_float2(__uint_as_float(sv[c]), __uint_as_float(sv[c + 1])), sc2, make_float2(-m_use[h], -m_use[h]));
+        float2 e;
+        if ((c & 6) == 0) e = poly_exp2_2(x);
+        else e = make_float2(fast_exp2(x.x), fast_exp2(x.y));
+        rs2[h] = fadd2(rs2[h], e);
+        pk[c >> 1] = pack_bf16(e.x, e.y);
       }
+      rs[0] = rs2[0].x + rs2[0].y;
+      rs[1] = rs2[1].x + rs2[1].y;
       l_run[0] = l_run[0] * alpha[0] + rs[0];
       l_run[1] = l_run[1] * alpha[1] + rs[1];
 

@@ -115,6 +115,36 @@ __device__ __forceinline__ uint32_t umma_idesc_mn_k(int M, int N) {
 __device__ __forceinline__ uint32_t umma_idesc_kk(int M, int N) {
   return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
 }
+// Packed fp32 pairs (sm_100: FFMA2 / FADD2 / FMUL2, one issue slot for two lanes' worth of results).  The softmax loops are
+// bound by their instruction stream, and their fragments come in (column, column + 1) pairs of the same row.
+__device__ __forceinline__ float2 ffma2(float2 a, float2 b, float2 c) {
+  float2 d;
+  asm("{\n\t.reg .b64 ra, rb, rc, rd;\n\tmov.b64 ra, {%2, %3};\n\tmov.b64 rb, {%4, %5};\n\tmov.b64 rc, {%6, %7};\n\t"
+      "fma.rn.f32x2 rd, ra, rb, rc;\n\tmov.b64 {%0, %1}, rd;\n\t}"
+      : "=f"(d.x), "=f"(d.y) : "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y), "f"(c.x), "f"(c.y));
+  return d;
+}
+__device__ __forceinline__ float2 fadd2(float2 a, float2 b) {
+  float2 d;
+  asm("{\n\t.reg .b64 ra, rb, rd;\n\tmov.b64 ra, {%2, %3};\n\tmov.b64 rb, {%4, %5};\n\tadd.rn.f32x2 rd, ra, rb;\n\tmov.b64 {%0, %1}, rd;\n\t}"
+      : "=f"(d.x), "=f"(d.y) : "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y));
+  return d;
+}
+// 2^x on the FMA pipe for a pair: poly_exp2 below with the additions and the polynomial packed
+__device__ __forceinline__ float2 poly_exp2_2(float2 x) {
+  x.x = fmaxf(x.x, -127.f);
+  x.y = fmaxf(x.y, -127.f);
+  const float2 big = make_float2(12582912.f, 12582912.f), nbig = make_float2(-12582912.f, -12582912.f);
+  const float2 t = fadd2(x, big);
+  const float2 n = fadd2(t, nbig);
+  const float2 f = fadd2(x, make_float2(-n.x, -n.y));
+  float2 q = ffma2(f, make_float2(0.0096181291f, 0.0096181291f), make_float2(0.0555041087f, 0.0555041087f));
+  q = ffma2(q, f, make_float2(0.2402265070f, 0.2402265070f));
+  q = ffma2(q, f, make_float2(0.6931471806f, 0.6931471806f));
+  q = ffma2(q, f, make_float2(1.0f, 1.0f));
+  return make_float2(__int_as_float(__float_as_int(q.x) + (__float_as_int(t.x) << 23)),
+                     __int_as_float(__float_as_int(q.y) + (__float_as_int(t.y) << 23)));
+}
 // 2^x on the FMA pipe (no MUFU): round-to-nearest split x = n + f, |f| <= 0.5, degree-4 Taylor polynomial of 2^f
 // (relative error < 5e-5, far below the bf16 rounding of P), exponent added as an integer.  x <= 0 expected.  The clamp
 // makes a masked key (x = -inf) exactly +0: n = -127, f = 0, p = 1.0f, and 0x3F800000 - (127 << 23) = 0.
