@@ -163,6 +163,16 @@ __global__ void __launch_bounds__(FT_THREADS, 1) wf_final_gemm_kernel(const __gr
   __shared__ int s_last;
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  if constexpr (EPI != EPI_Q) {
+    // O / up / down: the token count was written by the plan kernel, at least two launches back, and every kernel in
+    // between triggered its successor only after its own dependency wait: the count is final when this CTA starts.  A call
+    // in which nobody switched leaves before it has prefetched a byte of weights or allocated TMEM.
+    if (*reinterpret_cast<const volatile int32_t*>(p.m_total) == 0) {
+      wf_pdl_wait();
+      wf_pdl_trigger();
+      return;
+    }
+  }
   const int tile = (int)blockIdx.x / p.n_split, split = (int)blockIdx.x % p.n_split;
   const int tiles_n = p.N / FT_TILE;
   const int layer = tile / tiles_n, nt = tile % tiles_n;
