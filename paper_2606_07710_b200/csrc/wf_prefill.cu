@@ -22,6 +22,7 @@
 #include <math.h>
 
 #include <new>
+#include <type_traits>
 #include <vector>
 
 #include "wf_internal.cuh"
@@ -392,9 +393,15 @@ __global__ void __launch_bounds__(PF_THREADS, 1) wf_prefill_gemm_kernel(const __
   // its start, the few surplus rows feed accumulator columns nobody reads.  Layout: W ring (n_sw stages) | X ring (n_sx).
   const int m_first = min(M, N_MAX);
   const int x_sub = ((m_first + 7) / 8) * 1024;          // one 64-wide k-block of the X operand
-  const int x_stage = PF_KSUB * x_sub;
-  const int n_sw = (PF_SMEM_BUDGET - PF_W_PRE_BYTES - W_BYTES) >= 2 * x_stage ? W_PRE + 1 : W_PRE;
-  const int n_sx = max(1, min(PF_MAX_STAGES, (PF_SMEM_BUDGET - n_sw * W_BYTES) / x_stage));
+  // The X ring is cut into single 64-wide k-blocks (a W stage spans PF_KSUB of them): at 256 rows a k-block is 32 KB and the
+  // 72 KB beside the four prefetched W stages hold two of them, so the load of one overlaps the MMAs of the other (with
+  // whole stages as ring units a call of >= 128 rows had ONE X stage: load and MMA took turns, 0.23 us per row).
+  // Small calls keep whole stages as ring units (xg = PF_KSUB k-blocks per slot): every hand-off costs the one-thread loops a
+  // barrier round trip, and there is room for many slots anyway.
+  const int n_sw = (PF_SMEM_BUDGET - PF_W_PRE_BYTES - W_BYTES) >= 2 * PF_KSUB * x_sub ? W_PRE + 1 : W_PRE;
+  const int xg = (PF_SMEM_BUDGET - n_sw * W_BYTES) >= 2 * PF_KSUB * x_sub ? PF_KSUB : 1;   // k-blocks per X ring slot
+  const int x_slot = xg * x_sub;
+  const int n_sx = max(PF_KSUB / xg, min(PF_MAX_STAGES, (PF_SMEM_BUDGET - n_sw * W_BYTES) / x_slot));
   uint8_t* w_base = smem;
   uint8_t* x_base = smem + (size_t)n_sw * W_BYTES;         // 1024-aligned: W_BYTES is a multiple of 1024
 
@@ -410,6 +417,8 @@ __global__ void __launch_bounds__(PF_THREADS, 1) wf_prefill_gemm_kernel(const __
       const uint32_t x0 = smem_u32(x_base), w0 = smem_u32(w_base);
       int sw = 0, sx = 0, kw = 0;                        // W slot, X slot, W stages issued so far (the first n_pre are in flight)
       uint32_t phw = 1, phx = 1;                         // parities to wait for on the empty barriers: the rings start empty
+      auto produce = [&](auto xg_c) {
+      constexpr int XG = decltype(xg_c)::value;              // compile-time copy of xg: the one-thread loop stays straight-line
       for (int pass = 0; pass < n_pass; ++pass) {
         const int rows_here = min(M - pass * N_MAX, N_MAX);
         const uint32_t x_bytes = (uint32_t)((rows_here + 7) / 8) * 1024;
@@ -425,19 +434,25 @@ __global__ void __launch_bounds__(PF_THREADS, 1) wf_prefill_gemm_kernel(const __
               bulk_load(w0 + sw * W_BYTES, w_kb, W_BYTES, wf0 + 8 * sw);
             }
           }
-          mbar_wait(xe0 + 8 * sx, phx);
-          if (elect_one()) {
-            mbar_arrive_expect_tx(xf0 + 8 * sx, PF_KSUB * x_bytes);
 #pragma unroll
-            for (int u = 0; u < PF_KSUB; ++u) bulk_load(x0 + sx * x_stage + u * x_sub, x_src + u * x_kb_stride, x_bytes, xf0 + 8 * sx);
+          for (int u = 0; u < PF_KSUB; u += XG) {
+            mbar_wait(xe0 + 8 * sx, phx);
+            if (elect_one()) {
+              mbar_arrive_expect_tx(xf0 + 8 * sx, XG * x_bytes);
+#pragma unroll
+              for (int uu = 0; uu < XG; ++uu)
+                bulk_load(x0 + sx * x_slot + uu * x_sub, x_src + (u + uu) * x_kb_stride, x_bytes, xf0 + 8 * sx);
+            }
+            __syncwarp();
+            if (++sx == n_sx) { sx = 0; phx ^= 1; }
           }
-          __syncwarp();
           w_kb += W_BYTES;
           x_src += PF_KSUB * x_kb_stride;
           if (++sw == n_sw) { sw = 0; phw ^= 1; }
-          if (++sx == n_sx) { sx = 0; phx ^= 1; }
         }
       }
+      };
+      if (xg == 1) produce(std::integral_constant<int, 1>{}); else produce(std::integral_constant<int, PF_KSUB>{});
     }
   } else if (warp == 1) {
     // ===== MMA issuer: one thread drives the tensor core for the CTA.  Descriptors are built once and advanced by
@@ -446,36 +461,47 @@ __global__ void __launch_bounds__(PF_THREADS, 1) wf_prefill_gemm_kernel(const __
       const uint64_t dw0 = umma_desc(smem_u32(w_base), 8192, 1024);        // MN-major: 64-column halves 8 KB apart
       const uint64_t dx0 = umma_desc(smem_u32(x_base), 16, 1024);          // K-major
       const uint32_t wf0 = smem_u32(&w_full[0]), we0 = smem_u32(&w_empty[0]), xf0 = smem_u32(&x_full[0]), xe0 = smem_u32(&x_empty[0]);
-      const uint64_t dw_step = (uint64_t)(W_BYTES >> 4), dx_step = (uint64_t)(x_stage >> 4);
+      const uint64_t dw_step = (uint64_t)(W_BYTES >> 4), dx_step = (uint64_t)(x_slot >> 4);
       int sw = 0, sx = 0;
       uint32_t phw = 0, phx = 0;
       uint64_t dw = dw0, dx = dx0;
+      auto issue = [&](auto xg_c) {
+      constexpr int XG = decltype(xg_c)::value;
       for (int pass = 0; pass < n_pass; ++pass) {
         const int rows_here = min(M - pass * N_MAX, N_MAX);
         const uint32_t idesc = umma_idesc_mn_k(128, (rows_here + 15) & ~15);
         if (pass > 0) { mbar_wait(smem_u32(&s_acc_empty), (pass - 1) & 1); tc_fence_after(); }
         for (int kb = 0; kb < n_kb; ++kb) {
           mbar_wait(wf0 + 8 * sw, phw);
-          mbar_wait(xf0 + 8 * sx, phx);
-          tc_fence_after();
-          if (elect_one()) {
-          // k16 step j of the stage: W k-block j/4 (W_SUB apart), 16 k-rows = 2 KB per step; X k-block j/4 (x_sub apart),
-          // 32 bytes per step
+          // k-block u of the stage: W k-block u (W_SUB apart), its own X ring slot; k16 step j: 16 k-rows = 2 KB of W,
+          // 32 bytes of X
 #pragma unroll
-          for (int k16 = 0; k16 < PF_KSUB * PF_BLOCK_K / 16; ++k16)
-            umma_bf16(tmem_base, dw + (uint64_t)(((k16 >> 2) * W_SUB + (k16 & 3) * 2048) >> 4),
-                      dx + (uint64_t)(((k16 >> 2) * x_sub + (k16 & 3) * 32) >> 4), idesc, (kb | k16) != 0);
-          umma_commit(we0 + 8 * sw);                     // frees the stages when these MMAs retire
-          umma_commit(xe0 + 8 * sx);
+          for (int u = 0; u < PF_KSUB; u += XG) {
+            mbar_wait(xf0 + 8 * sx, phx);
+            tc_fence_after();
+            if (elect_one()) {
+#pragma unroll
+              for (int uu = 0; uu < XG; ++uu) {
+#pragma unroll
+                for (int k16 = 0; k16 < PF_BLOCK_K / 16; ++k16)
+                  umma_bf16(tmem_base, dw + (uint64_t)(((u + uu) * W_SUB + k16 * 2048) >> 4),
+                            dx + (uint64_t)((uu * x_sub + k16 * 32) >> 4), idesc, (kb | u | uu | k16) != 0);
+              }
+              umma_commit(xe0 + 8 * sx);                 // frees the X slot when these MMAs retire
+              if (u + XG == PF_KSUB) umma_commit(we0 + 8 * sw);
+            }
+            __syncwarp();
+            dx += dx_step;
+            if (++sx == n_sx) { sx = 0; phx ^= 1; dx = dx0; }
           }
-          __syncwarp();
-          dw += dw_step; dx += dx_step;
+          dw += dw_step;
           if (++sw == n_sw) { sw = 0; phw ^= 1; dw = dw0; }
-          if (++sx == n_sx) { sx = 0; phx ^= 1; dx = dx0; }
         }
         if (elect_one()) umma_commit(smem_u32(&s_acc_full));
         __syncwarp();
       }
+      };
+      if (xg == 1) issue(std::integral_constant<int, 1>{}); else issue(std::integral_constant<int, PF_KSUB>{});
     }
   } else {
     // ===== warps 2-5: epilogue.  TMEM lane = output column d of the head, TMEM column = token.  The accumulator is
@@ -562,9 +588,14 @@ __global__ void __launch_bounds__(PF_THREADS, 1) wf_prefill_gemm_kernel(const __
           named_bar_sync(1, 128);
         }
       }
+      // (read-only loads and an unroll of 4: the row entry -> RoPE entry -> store chains of four iterations overlap; one at a
+      // time they cost about 1.5k cycles each, 16 of them per 256-row pass)
+#pragma unroll 4
       for (int idx = et; finish && idx < rows_here * PC; idx += 128) {
         const int t = idx / PC, pc = idx % PC;
-        const RowEntry e = p.rows[m_base + t];
+        const int2 e2 = __ldg(reinterpret_cast<const int2*>(p.rows + m_base + t));
+        RowEntry e;
+        e.pos = e2.x; e.page_slot = e2.y;
         const float* lo = tr + t * D + pc * 8;
         const float4 a0 = *reinterpret_cast<const float4*>(lo), a1 = *reinterpret_cast<const float4*>(lo + 4);
         const float4 b0 = *reinterpret_cast<const float4*>(lo + D / 2), b1 = *reinterpret_cast<const float4*>(lo + D / 2 + 4);
