@@ -143,7 +143,7 @@ class Ctx:
         self.check(lib.wf_ctx_set_attn_early_kv(self.h, 1 if on else 0))
 
     def set_attn_cluster(self, cluster_size):
-        """Launch shape of wf_verify_attn: -1 automatic, 0 never clusters, 2..16 force that cluster size."""
+        """Launch shape of wf_verify_attn: -1 automatic, 0 never clusters, 1..16 force that many CTAs per pair (1 = no merge)."""
         self.check(lib.wf_ctx_set_attn_cluster(self.h, int(cluster_size)))
 
     def close(self):

@@ -11,7 +11,11 @@
 // keeps its partial in registers and folds in the partials the others published (fragment-order float4,
 // coalesced; more than two are staged through the idle shared memory with cp.async); nobody re-reads
 // its own partial.  Launched with programmatic dependent launch: barrier init and TMEM allocation run
-// before griddepcontrol.wait.  Warp roles:
+// before griddepcontrol.wait; in the early-KV mode (wf_ctx_set_attn_early_kv) so do the length table, the page ids and the
+// TMA loads of every tile below the cached length: only Q, the tree masks and the tiles that hold the block's own rows wait.
+// Other launch shapes (launch_attn): one thread-block cluster per (b, g) pair with the merge through distributed shared memory
+// (few pairs: batch 1-4), or one CTA per pair with no merge at all (HBM-paced launches whose pairs cover >= 80 % of the SMs).
+// Warp roles:
 //   warps 8,10: TMA producers (K ring, V ring).  One elected lane issues the 16 page boxes of a tile
 //               (cp.async.bulk.tensor.2d, 128-byte swizzle) in straight-line code; the page ids of the
 //               next tile are prefetched; a K tile is released when its QK^T retires.

@@ -17,7 +17,8 @@
 //                          shared memory, RoPE (fp32, host-built fp64 table) on K tiles, bf16 RNE, 16-byte
 //                          stores straight into the paged pool.
 // A row's bits do not depend on M, on its position in the call or on the call that carries it: one code
-// path, a fixed K order, no split-K; an accumulator column depends only on its own X row.
+// path, a fixed K order, a split-K factor fixed per drafter (partials summed in split order by the last CTA to
+// arrive); an accumulator column depends only on its own X row.
 #include <cuda.h>
 #include <math.h>
 
