@@ -32,9 +32,10 @@ WORKLOADS = {"cfg1": 0, "cfg2": 1, "cfg3": 2, "cfg4": 3, "cfg5": 4}
 # dram__bytes_read.sum + dram__bytes_write.sum per attention launch, from the committed `ncu --set full` capture named
 # beside each figure (a profiler cannot run inside the timed region); workloads without a capture report null
 NCU_TRAFFIC = {   # dram__bytes_read.sum + dram__bytes_write.sum per attention launch, from the committed ncu --set full captures
-    "cfg5": (1059.1e6, "profiles/r2_ncu_kernels.md (ncu --set full of this workload, round 2)"),
-    "cfg2": (17.15e6, "profiles/r2_ncu_kernels.md (ncu --set full of this workload, cluster launch shape, round 2)"),
-    "cfg3": (552.5e6, "profiles/r1g_final.md (ncu --set full, chain kernel in the stream-K shape, round 1 commit abe3062)"),
+    "cfg5": (1059.9e6, "profiles/r2_final.md section 5 (ncu --set full of this workload, stream-K over 148 SMs, final round-2 library)"),
+    "cfg2": (17.14e6, "profiles/r2_final.md section 5 (ncu --set full of this workload, 8 clusters of 10, final round-2 library)"),
+    "cfg3": (548.2e6, "profiles/r2_final.md section 5 (ncu --set full of this workload, one CTA per pair, final round-2 library)"),
+    "cfg4": (545.9e6, "profiles/r2_final.md section 5 (ncu --set full of this workload, 32 clusters of 4, final round-2 library)"),
 }
 METRIC = "verify_rounds_per_s"
 UNIT = "rounds/s"
