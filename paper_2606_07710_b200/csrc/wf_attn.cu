@@ -243,8 +243,10 @@ __device__ __forceinline__ void attn_loader(const AttnParams& p, AttnShared<TREE
       const int st = gt % n_st;
       const int npages = min(PP, pages_seg - t * PP);
       const int row = (((p.layer * kv.num_pages + page_next) * kv.n_kv_heads) + sg.g) * 16;
-      if (!waited && sg.k0 + (t + 2) * AT_BN > sg.ctx) { wf_pdl_wait(); waited = true; }
-      if ((t + 1) * PP + lane < pages_seg && lane < PP) page_next = __ldcg(bt + (t + 1) * PP + lane);
+      // early mode: when the NEXT tile reaches the block's own rows, its page ids are fetched behind the wait, after this
+      // tile (still wholly below the cached length) has been issued
+      const bool defer_next = !waited && sg.k0 + (t + 2) * AT_BN > sg.ctx;
+      if (!defer_next && (t + 1) * PP + lane < pages_seg && lane < PP) page_next = __ldcg(bt + (t + 1) * PP + lane);
       int rows[PP];
 #pragma unroll
       for (int q = 0; q < PP; ++q) rows[q] = __shfl_sync(0xffffffffu, row, q);
@@ -275,6 +277,11 @@ __device__ __forceinline__ void attn_loader(const AttnParams& p, AttnShared<TREE
           }
       }
       __syncwarp();
+      if (defer_next) {
+        wf_pdl_wait();
+        waited = true;
+        if ((t + 1) * PP + lane < pages_seg && lane < PP) page_next = __ldcg(bt + (t + 1) * PP + lane);
+      }
     }
   }
 }
@@ -1293,7 +1300,10 @@ __global__ void __launch_bounds__(AT_THREADS, 1) wf_verify_attn_kernel(const Att
     // cluster `pair` = (b, g) over ALL sequences of the call (an empty one idles its cluster); CTA rank r of the cluster owns
     // tiles [r * nt / cl, (r + 1) * nt / cl) of the pair: pair-aligned, equal shares, one segment
     lean_sg.b = b; lean_sg.pb = 0; lean_sg.nt = nt; lean_sg.g = pair % p.kv.n_kv_heads;
-    lean_sg.t_lo = rank * nt / p.cl; lean_sg.t_hi = (rank + 1) * nt / p.cl;
+    // The pair's LAST tile holds the block's own rows: it is never fetched ahead of the dependency wait, it is ragged (stale V
+    // rows to clear, causal mask) and the rank that owns it was the cluster's straggler (profiles/r2_final.md: its push landed
+    // 2.5k cycles after everybody else's).  It counts as two tiles in the split: the ranks share nt + 1 units.
+    lean_sg.t_lo = min(rank * (nt + 1) / p.cl, nt); lean_sg.t_hi = min((rank + 1) * (nt + 1) / p.cl, nt);
     lean_sg.flat0 = 0; lean_sg.r0 = r0; lean_sg.ctx = ctx; lean_sg.q_b = r1 - r0;
     lean_sg.k0 = lean_sg.t_lo * AT_BN; lean_sg.k1 = min(ctx + lean_sg.q_b, lean_sg.t_hi * AT_BN);
     lean_sg.n_tiles = lean_sg.t_hi - lean_sg.t_lo; lean_sg.partial = p.cl > 1; lean_sg.slot = 0;   // one CTA per pair: no merge at all
