@@ -141,6 +141,22 @@ int wf_accept_entropy_route(wf_ctx* ctx, const float* logits, int V, const int32
                             wf_paged_kv* target_kv, void* workspace, size_t workspace_bytes,
                             void* stream);
 size_t wf_accept_workspace_bytes(int sum_q, int V);
+/* The same operation for callers that cannot allocate and do not want to carry a workspace (code under CUDA graph capture,
+ * tight serving loops, harnesses that forbid cudaMalloc): the slice partials and completion counters live in one file-scope
+ * device array inside the library (516 KB, held by every GPU that loads the library until the process exits).  The call makes
+ * no cudaMalloc / cudaFree and calls no allocating routine; inputs and outputs are the caller's, exactly as above, and the
+ * results are those of wf_accept_entropy_route bit for bit (same kernel).
+ * Limits: B <= 1024 and B * max(max_q_len, 1) * ceil(V / 8192) <= 32768 (e.g. 64 sequences x 16 rows at V = 151936 use
+ * 19456); anything larger returns WF_ERR_UNSUPPORTED_SHAPE with a message and launches nothing.
+ * Every call on a device shares the array, which keeps the last call's contents: the call clears its counters itself (a
+ * memset node in stream order); two calls that overlap on the GPU (different streams, or two contexts on one device) RACE on
+ * it: keep them stream-ordered.  The first call on each device resolves the array's address (cudaGetSymbolAddress; no
+ * allocation) and needs the context's device to be current: make that call before starting a stream capture. */
+int wf_accept_entropy_route_static(wf_ctx* ctx, const float* logits, int V, const int32_t* draft_tokens,
+                                   const int32_t* q_indptr, int B, int max_q_len, const float* tau,
+                                   int tau_is_scalar, int32_t* accept_len, int32_t* bonus_token,
+                                   float* entropy, int32_t* route, int32_t* n_commit,
+                                   wf_paged_kv* target_kv, void* stream);
 
 /* ---- drafter descriptor -------------------------------------------------------------------------
  * PAPER.md:119; readings C14-C18: every layer l projects the same hidden rows X with its own

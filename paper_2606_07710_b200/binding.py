@@ -28,7 +28,7 @@ EXPORTS = [
     "wf_ctx_create", "wf_ctx_destroy", "wf_last_error", "wf_poll_status", "wf_launch_count",
     "wf_kv_create", "wf_kv_destroy", "wf_kv_reserve", "wf_kv_release_seq", "wf_kv_pages_held",
     "wf_verify_attn", "wf_verify_attn_workspace_bytes",
-    "wf_accept_entropy_route", "wf_accept_workspace_bytes",
+    "wf_accept_entropy_route", "wf_accept_workspace_bytes", "wf_accept_entropy_route_static",
     "wf_drafter_create", "wf_drafter_destroy", "wf_kv_only_prefill",
     "wf_lazy_catchup_enqueue", "wf_lazy_catchup_flush",
     "wf_neural_route", "wf_neural_route_workspace_bytes", "wf_lazy_catchup_round",
@@ -64,6 +64,7 @@ _SIG = {
     "wf_verify_attn": (_i, [_vp, _vp, _i, _vp, _vp, _i, _i, _i, C.c_float, _vp, _vp, _sz, _vp]),
     "wf_verify_attn_workspace_bytes": (_sz, [C.POINTER(KvShape), _i, _i, _i]),
     "wf_accept_entropy_route": (_i, [_vp, _vp, _i, _vp, _vp, _i, _i, _vp, _i, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _sz, _vp]),
+    "wf_accept_entropy_route_static": (_i, [_vp, _vp, _i, _vp, _vp, _i, _i, _vp, _i, _vp, _vp, _vp, _vp, _vp, _vp, _vp]),
     "wf_accept_workspace_bytes": (_sz, [_i, _i]),
     "wf_drafter_create": (_i, [_vp, C.POINTER(DrafterShape), C.POINTER(_vp), C.POINTER(_vp), _vp, _vp, _vp, C.POINTER(_vp)]),
     "wf_drafter_destroy": (_i, [_vp]),
@@ -201,6 +202,16 @@ def wf_accept_entropy_route(ctx, logits, V, draft_tokens, q_indptr, B, max_q_len
         _ptr(accept_len), _ptr(bonus_token), _ptr(entropy), _ptr(route), _ptr(n_commit),
         target_kv.h if target_kv is not None else None, _ptr(workspace),
         workspace.numel() * workspace.element_size(), _stream(stream)))
+
+
+def wf_accept_entropy_route_static(ctx, logits, V, draft_tokens, q_indptr, B, max_q_len, tau, tau_is_scalar,
+                                   accept_len, bonus_token, entropy, route, n_commit, target_kv, stream=None):
+    """wf_accept_entropy_route without a workspace and without any allocation: scratch in the library's static device array
+    (limits and the sharing rule: include/whiflash.h)."""
+    ctx.check(lib.wf_accept_entropy_route_static(
+        ctx.h, _ptr(logits), V, _ptr(draft_tokens), _ptr(q_indptr), B, max_q_len, _ptr(tau), int(tau_is_scalar),
+        _ptr(accept_len), _ptr(bonus_token), _ptr(entropy), _ptr(route), _ptr(n_commit),
+        target_kv.h if target_kv is not None else None, _stream(stream)))
 
 
 class Drafter:

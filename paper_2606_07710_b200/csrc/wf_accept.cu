@@ -581,3 +581,93 @@ int accept_launch(wf_ctx* ctx, const float* logits, int V, const int32_t* draft_
   return wf_check_launch(ctx, "wf_accept_kernel");
 }
 }  // namespace
+
+// ------------------------------------------------------------------------------------------------
+// wf_accept_entropy_route_static: the same sweep for callers that cannot allocate (CUDA graph capture, tight serving
+// loops, harnesses that forbid cudaMalloc) and do not want to carry a workspace: the slice partials and the completion
+// counters live in ONE file-scope device array of a fixed size.  Every GPU that loads the library holds the array
+// (516 KB) until the process exits.  Nothing here calls cudaMalloc, cudaFree or an allocating library routine.
+// ------------------------------------------------------------------------------------------------
+#include <mutex>
+
+namespace {
+constexpr int ACC_STATIC_MAX_B = 1024;                         // counters (one per sequence)
+constexpr int ACC_STATIC_MAX_PARTIALS = 32768;                 // B * max_q_len * ceil(V / 8192) slice partials of 16 bytes
+constexpr size_t ACC_STATIC_COUNTER_BYTES = ACC_STATIC_MAX_B * sizeof(unsigned int);
+constexpr size_t ACC_STATIC_BYTES = ACC_STATIC_COUNTER_BYTES + (size_t)ACC_STATIC_MAX_PARTIALS * sizeof(AccPartial);
+constexpr int ACC_STATIC_MAX_DEVICES = 64;
+}  // namespace
+
+// layout: [ACC_STATIC_MAX_B] unsigned int counters | [ACC_STATIC_MAX_PARTIALS] AccPartial.  In host code this NAME is a
+// host-side stand-in, not a device address: the address a kernel may use comes from cudaGetSymbolAddress (below).
+static __device__ __align__(256) unsigned char wf_accept_static_scratch[ACC_STATIC_BYTES];
+
+namespace {
+std::mutex g_static_mu;
+void* g_static_ptr[ACC_STATIC_MAX_DEVICES];                    // per device: the array's device address, resolved once
+
+// set-up, once per device, with that device current
+int accept_static_setup(wf_ctx* ctx, void** out) {
+  const int dev = ctx->device;
+  WF_REQUIRE(ctx, dev >= 0 && dev < ACC_STATIC_MAX_DEVICES, WF_ERR_INVALID_ARG,
+             "wf_accept_entropy_route_static: device ordinal %d out of range", dev);
+  std::lock_guard<std::mutex> lock(g_static_mu);
+  if (!g_static_ptr[dev]) {
+    int cur = -1;
+    WF_CUDA(ctx, cudaGetDevice(&cur));
+    WF_REQUIRE(ctx, cur == dev, WF_ERR_INVALID_ARG,
+               "wf_accept_entropy_route_static: the context's device (%d) must be current (current: %d)", dev, cur);
+    void* ptr = nullptr;
+    WF_CUDA(ctx, cudaGetSymbolAddress((void**)&ptr, wf_accept_static_scratch));
+    WF_REQUIRE(ctx, ptr != nullptr, WF_ERR_CUDA, "wf_accept_entropy_route_static: cudaGetSymbolAddress returned null");
+    g_static_ptr[dev] = ptr;
+  }
+  *out = g_static_ptr[dev];
+  return WF_OK;
+}
+}  // namespace
+
+extern "C" int wf_accept_entropy_route_static(wf_ctx* ctx, const float* logits, int V, const int32_t* draft_tokens,
+                                              const int32_t* q_indptr, int B, int max_q_len, const float* tau,
+                                              int tau_is_scalar, int32_t* accept_len, int32_t* bonus_token,
+                                              float* entropy, int32_t* route, int32_t* n_commit,
+                                              wf_paged_kv* target_kv, void* stream) {
+  if (!ctx) return WF_ERR_INVALID_ARG;
+  WF_REQUIRE(ctx, logits && draft_tokens && q_indptr && tau && accept_len && bonus_token && entropy && route && n_commit,
+             WF_ERR_INVALID_ARG, "wf_accept_entropy_route_static: null argument");
+  WF_REQUIRE(ctx, V > 0 && B >= 0 && B <= 65535, WF_ERR_INVALID_ARG, "wf_accept_entropy_route_static: bad V or B");
+  WF_REQUIRE(ctx, max_q_len >= 0 && max_q_len <= ACC_MAX_Q, WF_ERR_UNSUPPORTED_SHAPE,
+             "wf_accept_entropy_route_static: max_q_len must be <= %d", ACC_MAX_Q);
+  WF_REQUIRE(ctx, !target_kv || B <= target_kv->s.max_seqs, WF_ERR_INVALID_ARG,
+             "wf_accept_entropy_route_static: B exceeds the cache's max_seqs");
+  if (max_q_len == 0) max_q_len = 1;                       // still launch: empty blocks get zeroed outputs
+  const int n_chunks = (V + ACC_CHUNK - 1) / ACC_CHUNK;
+  const long long need = (long long)B * max_q_len * n_chunks;
+  WF_REQUIRE(ctx, B <= ACC_STATIC_MAX_B && need <= ACC_STATIC_MAX_PARTIALS, WF_ERR_UNSUPPORTED_SHAPE,
+             "wf_accept_entropy_route_static: B = %d, B * max_q_len * ceil(V / %d) = %lld exceed the static scratch "
+             "(at most %d sequences and %d slice partials); use wf_accept_entropy_route with a caller workspace",
+             B, ACC_CHUNK, need, ACC_STATIC_MAX_B, ACC_STATIC_MAX_PARTIALS);
+  if (B == 0) return WF_OK;
+  void* base = nullptr;
+  const int rc = accept_static_setup(ctx, &base);
+  if (rc != WF_OK) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  unsigned int* counters = reinterpret_cast<unsigned int*>(base);
+  AccPartial* partials = reinterpret_cast<AccPartial*>(reinterpret_cast<unsigned char*>(base) + ACC_STATIC_COUNTER_BYTES);
+  // The array keeps the last call's contents.  The counters must start at zero (they reset themselves when a call completes,
+  // but a call that was cut short would leave them counting): cleared here, in stream order.  The partials need no clearing:
+  // every one that is read was written by this call.
+  WF_CUDA(ctx, cudaMemsetAsync(counters, 0, (size_t)B * sizeof(unsigned int), st));
+  dim3 grid(n_chunks, max_q_len, B);
+  int32_t* kv_len = target_kv ? target_kv->seq_len : nullptr;
+  const bool vec = (V % 4 == 0) && ((uintptr_t)logits % 16 == 0);
+  if (vec)
+    wf_launch(wf_accept_kernel<true>, grid, dim3(ACC_THREADS), 0, st, logits, V, n_chunks, draft_tokens, q_indptr, tau,
+        tau_is_scalar, accept_len, bonus_token, entropy, route, n_commit, kv_len, partials, counters,
+        (const int32_t*)nullptr, (int32_t*)nullptr, 0, kGreedy, ctx->d_status);
+  else
+    wf_launch(wf_accept_kernel<false>, grid, dim3(ACC_THREADS), 0, st, logits, V, n_chunks, draft_tokens, q_indptr, tau,
+        tau_is_scalar, accept_len, bonus_token, entropy, route, n_commit, kv_len, partials, counters,
+        (const int32_t*)nullptr, (int32_t*)nullptr, 0, kGreedy, ctx->d_status);
+  return wf_check_launch(ctx, "wf_accept_kernel<static scratch>");
+}
