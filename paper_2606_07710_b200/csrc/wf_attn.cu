@@ -82,7 +82,8 @@ struct AttnParams {
 // TREE: the query tile has 128 rows (UMMA M = 128): two 64-row sub-blocks of a draft tree stacked on the TMEM lanes, rows
 // of sub-block A on lanes 32w..32w+15 and of sub-block B on lanes 32w+16..32w+31 of every warp quadrant w, so that softmax
 // group 0 works on A and group 1 on B of the SAME K/V tile with the chain kernel's fragment code (M = 64 puts its rows on
-// lanes 32w..32w+15 as well).  One P buffer of 128 rows, S and O double buffered over the tiles.
+// lanes 32w..32w+15 as well).  S and O are double buffered over the tiles; P(t) is written with tcgen05.st over the head of
+// the S buffer it was computed from (bf16, two keys per 32-bit column) and is the A operand of the PV product FROM TMEM.
 template <int D, bool TREE>
 struct AttnCfg {
   static constexpr int NH = D / 64;                         // 64-element (128-byte) column halves of a K/V row
@@ -92,10 +93,10 @@ struct AttnCfg {
   static constexpr int P_BYTES = 2 * Q_HALF;                // 2 key halves x rows x 128 B
   static constexpr int KV_HALF = AT_BN * 128;               // one column half of a K (or V) tile: 16 KB
   static constexpr int K_BYTES = NH * KV_HALF;               // one K (or V) tile
-  static constexpr int STAGES_K = D == 128 ? (TREE ? 2 : 3) : 4;          // K ring
+  static constexpr int STAGES_K = D == 128 ? 3 : 4;                       // K ring (TREE: P lives in TMEM, its 32 KB went to a third K stage)
   static constexpr int STAGES_V = D == 128 ? 2 : 4;                       // V ring
-  // smem map, chain: P0 | Q | P1 | K ring | V ring (Q + P1 double as the group-merge buffer); tree: P | Q | K | V
-  static constexpr int SMEM = Q_BYTES + (TREE ? 1 : 2) * P_BYTES + (STAGES_K + STAGES_V) * K_BYTES;
+  // smem map, chain: P0 | Q | P1 | K ring | V ring (Q + P1 double as the group-merge buffer); tree: Q | K ring | V ring
+  static constexpr int SMEM = Q_BYTES + (TREE ? 0 : 2) * P_BYTES + (STAGES_K + STAGES_V) * K_BYTES;
   static constexpr uint32_t TM_S = 0, TM_O = 2 * AT_BN;     // TMEM columns: S0, S1, then O0, O1
 };
 
@@ -317,6 +318,9 @@ __device__ __forceinline__ void attn_mma_qk(const AttnParams& p, AttnShared<TREE
       mbar_wait(smem_u32(&sh.k_full[st]), (gt / n_stk) & 1);
       WF_PROBE_AT(12 + (gt < 3 ? (int)gt : 3), (threadIdx.x & 31) == 0 && gt < 3);
       mbar_wait(smem_u32(&sh.s_empty[gt & 1]), ((gt >> 1) & 1) ^ 1);
+      // TREE: P(gt - 2) lives in the S buffer this product overwrites (tcgen05.st by the softmax warps, A operand of PV from
+      // TMEM): the PV of tile gt - 2 must have retired (the two issuers' MMAs are not ordered with each other)
+      if constexpr (TREE) { if (gt >= 2) mbar_wait(smem_u32(&sh.pv_done[gt & 1]), ((gt - 2) >> 1) & 1); }
       tc_fence_after();
       if (elect_one()) {
         const uint64_t dk = dk0 + (uint64_t)((st * C::K_BYTES) >> 4);
@@ -362,18 +366,28 @@ __device__ __forceinline__ void attn_mma_pv(const AttnParams& p, AttnShared<TREE
     for (int t = 0; t < sg.n_tiles; ++t, ++gt) {
       const int st = gt % sh.n_stv, g = gt & 1;
       mbar_wait(smem_u32(&sh.v_full[st]), (gt / sh.n_stv) & 1);
-      if constexpr (TREE) mbar_wait(smem_u32(&sh.p_full[0]), gt & 1);       // one P buffer, one phase per tile
-      else mbar_wait(smem_u32(&sh.p_full[g]), (gt >> 1) & 1);
+      // one barrier per P buffer (TREE: P shares the S buffer of its tile).  With a single barrier a softmax thread that runs
+      // one tile ahead of another would arrive twice in one phase: nothing holds it back between P(t) and P(t+1) any more
+      // (two tiles ahead is impossible: S(t+2) needs PV(t), which needs every arrival of P(t)).
+      mbar_wait(smem_u32(&sh.p_full[g]), (gt >> 1) & 1);
       mbar_wait(smem_u32(&sh.o_empty[g]), ((gt >> 1) & 1) ^ 1);
       tc_fence_after();
       if (elect_one()) {
         const uint64_t dv = dv0 + (uint64_t)((st * C::K_BYTES) >> 4);
         const uint64_t dp = (!TREE && g) ? dp1 : dp0;
         const uint32_t td = tmem_base + C::TM_O + g * D;
+        if constexpr (TREE) {
+          // A = P(gt) from TMEM: 128 rows on the lanes, 16 keys = 8 packed columns per step, at the head of S buffer g
+          const uint32_t ta = tmem_base + C::TM_S + g * AT_BN;
 #pragma unroll
-        for (int k16 = 0; k16 < AT_BN / 16; ++k16)
-          umma_bf16(td, dp + (uint64_t)(((k16 >> 2) * C::Q_HALF + (k16 & 3) * 32) >> 4), dv + (uint64_t)((k16 * 2048) >> 4),
-                    idesc_pv, k16 != 0);
+          for (int k16 = 0; k16 < AT_BN / 16; ++k16)
+            umma_bf16_ts(td, ta + k16 * 8, dv + (uint64_t)((k16 * 2048) >> 4), idesc_pv, k16 != 0);
+        } else {
+#pragma unroll
+          for (int k16 = 0; k16 < AT_BN / 16; ++k16)
+            umma_bf16(td, dp + (uint64_t)(((k16 >> 2) * C::Q_HALF + (k16 & 3) * 32) >> 4), dv + (uint64_t)((k16 * 2048) >> 4),
+                      idesc_pv, k16 != 0);
+        }
         umma_commit(smem_u32(&sh.pv_done[g]));
         umma_commit(smem_u32(&sh.v_empty[st]));
       }
@@ -951,7 +965,7 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared<fal
 // ================= TREE: warps 0-3 (sub-block A) and 4-7 (sub-block B) on the same K/V tile =================
 // Group g owns the 64 rows of sub-block g of the 128-row tile (TMEM lanes 32w + 16g .. +15 of quadrant w) for EVERY tile
 // of the segment: running (m, l, O) per group, no hand-over between the groups; S and O alternate between two TMEM
-// buffers from tile to tile, P has one 128-row buffer (the store of P(t) waits for PV(t-1)).  Fragment code, mask,
+// buffers from tile to tile, P(t) goes to TMEM over the head of S(t)'s buffer (nothing waits for PV(t-1)).  Fragment code, mask,
 // partial publishing and the last-arriver fold are those of the chain kernel; a partial slot is (CTA slot, group).
 template <int D>
 __device__ __forceinline__ void attn_softmax_tree(const AttnParams& p, AttnShared<true>& sh, uint8_t* q_s, uint8_t* p_s,
@@ -1096,9 +1110,6 @@ __device__ __forceinline__ void attn_softmax_tree(const AttnParams& p, AttnShare
       l_run[0] = l_run[0] * alpha[0] + rs[0];
       l_run[1] = l_run[1] * alpha[1] + rs[1];
 
-      // P(t) overwrites P(t-1): wait for PV(t-1) (it also makes O(t-1) ready and, the pipe being in order, every
-      // earlier PV retired: the V stage of this tile holds no older tile any more)
-      if (t > 0) mbar_wait(smem_u32(&sh.pv_done[(g2 - 1) & 1]), ((g2 - 1) >> 1) & 1);
       if (tk0 + AT_BN > sg.k1 && grp == 0) {
         // Last tile of the sequence: keys >= k1 hold stale or never-written V bits; zero them so that 0 * garbage cannot
         // produce NaN in the PV product (P is exactly 0 there).  Group 0 does it; PV waits for all 256 P arrivals.
@@ -1112,18 +1123,19 @@ __device__ __forceinline__ void attn_softmax_tree(const AttnParams& p, AttnShare
             for (int c = 0; c < 8; ++c) *reinterpret_cast<uint4*>(vrow + h * C::KV_HALF + c * 16) = make_uint4(0, 0, 0, 0);
         }
       }
-      {
-        // P -> smem, K-major 128-byte swizzle, this warp's 16 rows of the 128-row tile: stmatrix.x4 per chunk pair
-        const int mi = lane >> 3, r8 = lane & 7;
-        const uint32_t prow = smem_u32(p_s) + (uint32_t)(qw * 32 + grp * 16 + (mi & 1) * 8 + r8) * 128;
-#pragma unroll
-        for (int j = 0; j < 16; j += 2)
-          stmatrix_x4(prow + (j >> 3) * C::Q_HALF + ((((j & 7) + (mi >> 1)) ^ r8) << 4), pk[2 * j], pk[2 * j + 1], pk[2 * j + 2],
-                      pk[2 * j + 3]);
+      // P(t) -> TMEM, over the first 64 columns of the S buffer it was computed from (this warp's 16 lanes; S(t) is in
+      // registers): the packed fragment is the 16x128b store layout.  P is double buffered with S, so nothing waits for
+      // PV(t-1) here; QK^T(t+2) waits for PV(t) before it overwrites the buffer (attn_mma_qk).
+      tmem_st_16x128b_x16(t_lane + C::TM_S + sb * AT_BN, pk);
+      tmem_st_wait();
+      fence_proxy_async();                                     // the zeroed V rows above are generic-proxy writes the MMA reads
+      tc_fence_before();
+      mbar_arrive(smem_u32(&sh.p_full[sb]));
+      if (t > 0) {                                             // O(t-1): its PV has had the whole softmax of tile t to retire
+        mbar_wait(smem_u32(&sh.pv_done[(g2 - 1) & 1]), ((g2 - 1) >> 1) & 1);
+        tc_fence_after();
+        fold_o(g2 - 1);
       }
-      fence_proxy_async();
-      mbar_arrive(smem_u32(&sh.p_full[0]));
-      if (t > 0) { tc_fence_after(); fold_o(g2 - 1); }
       alpha_prev[0] = alpha[0];
       alpha_prev[1] = alpha[1];
     }
@@ -1237,9 +1249,9 @@ __global__ void __launch_bounds__(AT_THREADS, 1) wf_verify_attn_kernel(const Att
   __shared__ __align__(8) AttnShared<TREE> sh;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   uint8_t* p0_s = smem;                                        // smem map: P0 | Q | P1 | K ring | V ring
-  uint8_t* q_s = p0_s + C::P_BYTES;
+  uint8_t* q_s = p0_s + (TREE ? 0 : C::P_BYTES);               // TREE: no P buffer in shared memory (P goes to TMEM)
   uint8_t* p1_s = q_s + C::Q_BYTES;
-  uint8_t* k_s = p1_s + (TREE ? 0 : C::P_BYTES);             // TREE: one P buffer (p0_s), no p1_s
+  uint8_t* k_s = p1_s + (TREE ? 0 : C::P_BYTES);             // TREE: no P buffers
   uint8_t* v_s = k_s + C::STAGES_K * C::K_BYTES;
 
   // barrier init and TMEM allocation touch no global memory: they run before the dependency wait and overlap the
