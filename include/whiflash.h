@@ -91,8 +91,11 @@ const int32_t* wf_kv_pages_held(const wf_paged_kv* kv);
  *     O[i,h,:] = sum_j softmax(s)_j V[b,j,g,:]                          (fp32 accumulate, C13)
  * The block's own K/V must already be in the cache at positions ctx_b .. ctx_b+q_b-1 (C10).
  * q, out: bf16 [sum_q][n_q_heads][head_dim].  workspace: >= wf_verify_attn_workspace_bytes.
- * Supported: head_dim 64 or 128; page_size 16; q_b * group <= 64 (group = n_q_heads/n_kv_heads; rows beyond that
- * are not computed and the sticky status becomes WF_ERR_INVALID_ARG). */
+ * Supported: head_dim 64 or 128; page_size 16; max_q_len <= 64 and group = n_q_heads/n_kv_heads <= 64 (rows of a block
+ * beyond max_q_len are not computed and the sticky status becomes WF_ERR_INVALID_ARG).  Blocks of up to 64 rows per kv head
+ * (max_q_len * group <= 64: every config of BASELINE.json) run on the chain kernel; longer ones (e.g. gamma = 15 at a group of
+ * 8) are run as degenerate trees on the tree kernel's 128-row tiles (one extra tiny launch writes their masks into the
+ * workspace), subject to wf_verify_attn_tree's limit B * ceil(max_q_len * group / 128) <= 1024. */
 int wf_verify_attn(wf_ctx* ctx, const wf_paged_kv* target_kv, int layer,
                    const void* q, const int32_t* q_indptr, int B, int n_q_heads, int max_q_len,
                    float sm_scale, void* out, void* workspace, size_t workspace_bytes, void* stream);

@@ -1560,13 +1560,26 @@ __global__ void __launch_bounds__(64) wf_tree_masks_kernel(const int32_t* parent
   mask[r0 + i] = m;
 }
 
+// ancestor masks of a CHAIN block (parent[i] = i - 1): row i sees block rows 0..i.  For blocks of more than 64 / group rows,
+// which wf_verify_attn runs on the tree kernel's 128-row tiles.
+__global__ void __launch_bounds__(64) wf_chain_masks_kernel(const int32_t* q_indptr, unsigned long long* mask) {
+  wf_pdl_wait();
+  wf_pdl_trigger();
+  const int b = blockIdx.x, i = threadIdx.x;
+  const int r0 = q_indptr[b], n = min(q_indptr[b + 1] - r0, 64);
+  if (i < n) mask[r0 + i] = i == 63 ? ~0ull : (2ull << i) - 1ull;
+}
+
 }  // namespace
 
 extern "C" size_t wf_verify_attn_workspace_bytes(const wf_kv_shape* s, int B, int n_q_heads, int max_q_len) {
   if (!s || B <= 0 || n_q_heads <= 0 || s->n_kv_heads <= 0) return 16;
   const size_t items = 4 * (size_t)AT_MAX_CTAS;            // a CTA writes at most a head and a tail partial (tree: per group)
   const size_t r_pad = AT_ROWS;
-  return items * (r_pad * (size_t)s->head_dim * sizeof(float) + 128 * sizeof(float4));
+  const size_t base = items * (r_pad * (size_t)s->head_dim * sizeof(float) + 128 * sizeof(float4));
+  // a chain block of more than 64 rows per kv head runs on the tree kernel: its chain masks live behind the partials
+  const bool wide = max_q_len > 0 && (long long)max_q_len * (n_q_heads / s->n_kv_heads) > AT_ROWS;
+  return base + (wide ? (((size_t)B * (size_t)max_q_len * sizeof(unsigned long long) + 15) & ~(size_t)15) : 0);
 }
 
 // shared by wf_verify_attn (ctx_adj = 0) and the final-token path of wf_final.cu (ctx_adj = -1, one query row per
@@ -1581,13 +1594,25 @@ int wf_attn_launch_chain(wf_ctx* ctx, const wf_paged_kv* kv, int layer, const vo
   WF_REQUIRE(ctx, n_q_heads > 0 && n_q_heads % kv->s.n_kv_heads == 0, WF_ERR_INVALID_ARG,
              "%s: n_q_heads must be a multiple of n_kv_heads", who);
   const int group = n_q_heads / kv->s.n_kv_heads;
-  WF_REQUIRE(ctx, max_q_len >= 1 && max_q_len * group <= 64, WF_ERR_UNSUPPORTED_SHAPE,
-             "%s: max_q_len * group must be in [1, 64]", who);
+  WF_REQUIRE(ctx, max_q_len >= 1 && max_q_len <= 64 && group <= 64, WF_ERR_UNSUPPORTED_SHAPE,
+             "%s: max_q_len must be in [1, 64] and the GQA group <= 64", who);
   WF_REQUIRE(ctx, workspace_bytes >= wf_verify_attn_workspace_bytes(&kv->s, B, n_q_heads, max_q_len),
              WF_ERR_INVALID_ARG, "%s: workspace too small", who);
   WF_REQUIRE(ctx, ((uintptr_t)q % 16 == 0) && ((uintptr_t)out % 16 == 0) && ((uintptr_t)workspace % 16 == 0),
              WF_ERR_INVALID_ARG, "%s: q/out/workspace must be 16-byte aligned", who);
   if (B == 0) return WF_OK;
+  if (max_q_len * group > AT_ROWS) {
+    // More than 64 rows per kv head (e.g. gamma = 15 at a GQA group of 8): the block is a degenerate tree (parent[i] = i - 1)
+    // and runs on the tree kernel's 128-row tiles; its masks are written into the tail of the workspace first.
+    WF_REQUIRE(ctx, ctx_adj == 0, WF_ERR_UNSUPPORTED_SHAPE, "%s: more than 64 rows per kv head", who);
+    const size_t base = wf_verify_attn_workspace_bytes(&kv->s, B, n_q_heads, 1);
+    unsigned long long* masks = reinterpret_cast<unsigned long long*>((char*)workspace + base);
+    wf_launch(wf_chain_masks_kernel, dim3(B), dim3(64), 0, (cudaStream_t)stream, q_indptr, masks);
+    const int rc = wf_check_launch(ctx, "wf_chain_masks_kernel");
+    if (rc != WF_OK) return rc;
+    return wf_verify_attn_tree(ctx, kv, layer, q, q_indptr, (const uint64_t*)masks, B, n_q_heads, max_q_len, sm_scale, out,
+                               workspace, workspace_bytes, stream);
+  }
   const int r_pad = AT_ROWS;
   const size_t items = 4 * (size_t)AT_MAX_CTAS;
   AttnParams p;

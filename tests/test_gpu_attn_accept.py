@@ -261,6 +261,17 @@ def test_attn_group_shapes(wf):
         assert max_abs <= ATTN_MAX_ABS and rel <= ATTN_REL_L2, (Hq, Hkv, D, max_abs, rel)
 
 
+def test_attn_blocks_wider_than_64_rows_per_kv_head(wf):
+    """max_q_len * group > 64 (gamma = 15 at a GQA group of 8 or 16; blocks of up to 64 tokens at group 4): wf_verify_attn
+    runs these as degenerate trees on the tree kernel's 128-row tiles; same definition, same tolerance.  Ragged tails, an
+    empty block, a block of one token, zero context, several 128-row tiles per block, NaN beyond the visible range."""
+    for (Hq, Hkv, D, q_lens, ctx, poison) in [(64, 8, 128, [16, 9, 16, 0, 1], [700, 129, 2050, 33, 5], True),
+                                              (8, 2, 64, [64, 33, 17], [300, 0, 1000], False),
+                                              (16, 1, 128, [16, 5, 12], [515, 64, 4100], True)]:
+        max_abs, rel = _attn_case(wf, ctx, q_lens, Hq, Hkv, D, seed=61 + Hq, poison=poison)
+        assert max_abs <= ATTN_MAX_ABS and rel <= ATTN_REL_L2, (Hq, Hkv, D, max_abs, rel)
+
+
 def test_attn_many_short_sequences_with_empty_blocks(wf):
     """200 sequences with contexts 0..40 and blocks of 0, 1, 8 or 16 rows: far more (sequence, kv head) pairs than CTAs,
     every range holds many one-tile segments, empty blocks in between (the weighted walker must skip them)."""
