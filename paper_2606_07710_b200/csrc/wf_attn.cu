@@ -54,7 +54,9 @@ constexpr int AT_MAX_B = 1024;
 constexpr int AT_MAX_STAGES = 5;
 constexpr int AT_MAX_CTAS = 160;       // workspace is sized for this many persistent CTAs
 constexpr int AT_MAX_SEG = 32;         // partials merged per (b, g) pair
-constexpr int AT_SEG_COST = 4;         // fixed cost of a segment (Q load, pipeline restart, merge, stores) in tiles
+constexpr int AT_SEG_COST = 5;         // fixed cost of a segment (Q load, pipeline restart, merge, stores) in tiles; measured at cfg5
+                                       // (us per launch): 2: 192.6, 3: 184.8, 4: 178.5, 5: 176.3-177.2, 6: 176.9-178.3, 7: 178.8-179.3,
+                                       // 8: 179.4, 10: 184.8, 14: 190.7
 constexpr float LOG2E = 1.4426950408889634f;
 
 struct AttnParams {
