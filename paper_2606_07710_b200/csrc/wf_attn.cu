@@ -57,6 +57,9 @@ constexpr int AT_MAX_SEG = 32;         // partials merged per (b, g) pair
 constexpr int AT_SEG_COST = 5;         // fixed cost of a segment (Q load, pipeline restart, merge, stores) in tiles; measured at cfg5
                                        // (us per launch): 2: 192.6, 3: 184.8, 4: 178.5, 5: 176.3-177.2, 6: 176.9-178.3, 7: 178.8-179.3,
                                        // 8: 179.4, 10: 184.8, 14: 190.7
+constexpr int AT_SEG_COST_TREE = 8;    // the same for a 128-row tree block (Q tile of 32 KB, merges per sub-block); 60-node trees at cfg5
+                                       // shapes (us per launch): 4: 388, 5: 369, 8: 352, 12: 354, 16: 362
+template <bool TREE> constexpr int seg_cost() { return TREE ? AT_SEG_COST_TREE : AT_SEG_COST; }
 constexpr float LOG2E = 1.4426950408889634f;
 
 struct AttnParams {
@@ -173,12 +176,12 @@ struct SegWalker {
     }
     while (x < hi) {
       while (x >= Hkv * sh.pref[b + 1]) ++b;                   // also skips empty sequences
-      const int wlen = sh.pref[b + 1] - sh.pref[b], nt = wlen - AT_SEG_COST;
+      const int wlen = sh.pref[b + 1] - sh.pref[b], nt = wlen - seg_cost<TREE>();
       const int base = Hkv * sh.pref[b];
       const int g = (x - base) / wlen;
       const int wbase = base + g * wlen;
-      const int t_lo = max(0, x - wbase - AT_SEG_COST);
-      const int t_hi = min(nt, hi - wbase - AT_SEG_COST);
+      const int t_lo = max(0, x - wbase - seg_cost<TREE>());
+      const int t_hi = min(nt, hi - wbase - seg_cost<TREE>());
       x = t_hi >= nt ? wbase + wlen : hi;                      // the pair is finished, or the range is
       if (t_hi <= t_lo) continue;                              // the range ends inside the cost positions
       s.b = b; s.pb = b; s.nt = nt; s.g = g; s.t_lo = t_lo; s.t_hi = t_hi;
@@ -741,8 +744,8 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared<fal
     int c_first = 0, n_seg = 1;
     unsigned int arrive_old = 0;
     if (sg.partial && grp == 0 && sh.cl == 0) {
-      c_first = cta_of_tile(sg.flat0 + AT_SEG_COST, T, G);
-      n_seg = cta_of_tile(sg.flat0 + AT_SEG_COST + sg.nt - 1, T, G) - c_first + 1;
+      c_first = cta_of_tile(sg.flat0 + seg_cost<false>(), T, G);
+      n_seg = cta_of_tile(sg.flat0 + seg_cost<false>() + sg.nt - 1, T, G) - c_first + 1;
       if (stid == 0) arrive_old = atomicAdd(&p.counters[sg.pb * Hkv + sg.g], 1u);
     }
 
@@ -1172,8 +1175,8 @@ __device__ __forceinline__ void attn_softmax_tree(const AttnParams& p, AttnShare
 
     // ---- the pair is shared with other CTAs: last-arriver fold as in the chain kernel, both groups in step ----
     unsigned int* cnt = p.counters + sg.pb * Hkv + sg.g;
-    const int c_first = cta_of_tile(sg.flat0 + AT_SEG_COST, T, G);
-    const int n_seg = cta_of_tile(sg.flat0 + AT_SEG_COST + sg.nt - 1, T, G) - c_first + 1;
+    const int c_first = cta_of_tile(sg.flat0 + seg_cost<true>(), T, G);
+    const int n_seg = cta_of_tile(sg.flat0 + seg_cost<true>() + sg.nt - 1, T, G) - c_first + 1;
     if (grp == 0 && stid == 0) {
       const unsigned int arrive_old = atomicAdd(cnt, 1u);
       sh.last = (arrive_old & 0xffffu) == (unsigned int)n_seg - 1 ? 1 + (int)(arrive_old >> 16) : 0;
@@ -1347,7 +1350,7 @@ __global__ void __launch_bounds__(AT_THREADS, 1) wf_verify_attn_kernel(const Att
       } else {
         sh.r0[b] = r0;
         sh.ctx[b] = ctx;
-        sh.pref[b + 1] = r1 > r0 ? (ctx + (r1 - r0) + AT_BN - 1) / AT_BN + AT_SEG_COST : 0;
+        sh.pref[b + 1] = r1 > r0 ? (ctx + (r1 - r0) + AT_BN - 1) / AT_BN + seg_cost<false>() : 0;
         if (b == p.B - 1) sh.r0[p.B] = r1;
       }
     }
@@ -1377,7 +1380,7 @@ __global__ void __launch_bounds__(AT_THREADS, 1) wf_verify_attn_kernel(const Att
               sh.r0[idx] = t_r0[b] + s0;
               sh.ctx[idx] = ctx;
               sh.meta[idx] = min(npt, q - s0) | (q << 7) | (s0 << 14) | (b << 21);
-              sh.pref[idx + 1] = (ctx + q + AT_BN - 1) / AT_BN + AT_SEG_COST;
+              sh.pref[idx + 1] = (ctx + q + AT_BN - 1) / AT_BN + seg_cost<true>();
             }
             cursor += __popc(bal);
           }
