@@ -791,7 +791,7 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared<fal
       l_run[h] += __shfl_xor_sync(0xffffffffu, l_run[h], 2);
     }
     if (sh.cl > 1) {
-      // Cluster mode: the partial (m, l, unnormalised O) of this CTA goes to its OWN shared memory (K stage 1 is idle: every
+      // Cluster mode: the partial (m, l, unnormalised O) of this CTA goes to its OWN shared memory (the last K stage is idle: every
       // MMA has retired), then warp 0 pushes every owner its rows (attn_cluster_push).  Group 0 only.
       const int Rc = min(R, AT_ROWS);
 #pragma unroll
@@ -1443,7 +1443,16 @@ __global__ void __launch_bounds__(AT_THREADS, 1) wf_verify_attn_kernel(const Att
     if (warp < 8) {
       asm volatile("setmaxnreg.inc.sync.aligned.u32 216;");
       if constexpr (TREE) attn_softmax_tree<D>(p, sh, q_s, p0_s, v_s, tmem_base, warp, lane);
-      else attn_softmax<D>(p, sh, q_s, p0_s, p1_s, v_s, k_s + C::K_BYTES, k_s, tmem_base, warp, lane, lp);
+      else {
+        // Cluster mode buffers inside the (then idle) K ring: the receive buffer at its start (cl slices of this CTA's rows: at
+        // most (64 + cl - 1) rows of D fp32 = 40 KB at D = 128), this CTA's own staged partial in its LAST stage (64 rows of D
+        // fp32 = exactly one stage).  They must not overlap: a peer's slice may land before this CTA has staged or pushed its
+        // own partial.  (Until the end of round 2 the partial sat in stage 1 and the slices of an owner with 7 rows, 35 KB from
+        // 10 senders, reached 3 KB into it: harmless only as long as the last rank was also the last to push, which stopped
+        // being true when its ragged tile was weighted as two; the early / waiting bit-identity test caught it, 1 run in 6.)
+        static_assert((AT_ROWS + 15) * D * 4 <= (C::STAGES_K - 1) * C::K_BYTES && AT_ROWS * D * 4 <= C::K_BYTES, "cluster buffers");
+        attn_softmax<D>(p, sh, q_s, p0_s, p1_s, v_s, k_s + (C::STAGES_K - 1) * C::K_BYTES, k_s, tmem_base, warp, lane, lp);
+      }
     } else {
       asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
       if (warp == 8) attn_loader<D, TREE>(p, sh, k_s, k_s, 0, lane, lp);

@@ -196,3 +196,56 @@ def test_attention_six_hundred_launches_identical_and_finite():
     finally:
         rs.close()
         ctx.close()
+
+
+@pytest.mark.parametrize("workload,early", [(1, 0), (1, 1), (3, 1)])
+def test_attention_cluster_shape_two_thousand_launches_identical(workload, early):
+    """The cluster launch shape (cfg2: 8 clusters of 10; cfg4: 32 clusters of 4) folds a pair's partials in rank order, so its
+    bits never depend on timing: 2000 launches issued back to back over all 36 layer pools in turn (no host synchronisation
+    between them: consecutive launches overlap through programmatic dependent launch, with and without the early-KV mode)
+    must repeat, layer by layer, the bits of the first pass, and those are within tolerance of the stream-K shape's.
+    Regression: until the end of round 2 a CTA's own staged partial overlapped the tail of its receive buffer by 3 KB
+    (7-row owners, 10 senders); a peer's slice that landed before the CTA had pushed its own partial corrupted up to six
+    rows.  It showed as 128-384 differing values in about one run in six of the early / waiting comparison, once the last
+    rank stopped being the last to push."""
+    import torch
+    from paper_2606_07710_b200 import binding as wf
+    from paper_2606_07710_b200.rounds import RoundState
+    wl = synth.WORKLOADS[workload]
+    sh = wl.shapes
+    ctx = wf.Ctx(0)
+    ctx.set_attn_early_kv(early)
+    L = 6
+    rs = RoundState(ctx, wl, n_slots=1, n_rounds_max=8, layers=L, final_token=False)
+    try:
+        s = rs.slots[0]
+        rs.target_kv.reserve(s.add_tokens, rs.B)
+        outs = [torch.zeros_like(s.attn_out) for _ in range(L)]
+        run = lambda l: wf.wf_verify_attn(ctx, rs.target_kv, l, s.q, s.q_indptr, rs.B, sh.n_q_heads, rs.qmax, rs.sm_scale, outs[l],
+                                          rs.attn_ws)
+        ctx.set_attn_cluster(0)                                  # stream-K reference
+        for l in range(L):
+            run(l)
+        torch.cuda.synchronize()
+        ref_sk = [o.float().clone() for o in outs]
+        ctx.set_attn_cluster(-1)                                 # automatic: the cluster shape at these sizes
+        for l in range(L):
+            run(l)
+        torch.cuda.synchronize()
+        ref = [o.view(torch.int16).clone() for o in outs]
+        for l in range(L):
+            d = outs[l].float() - ref_sk[l]
+            assert not torch.isnan(outs[l].float()).any()
+            assert float(d.abs().max()) <= 2e-3 and float((d ** 2).sum().sqrt() / (ref_sk[l] ** 2).sum().sqrt()) <= 3e-3, l
+        bad = torch.zeros((), dtype=torch.int64, device="cuda")
+        for it in range(2000 // L):
+            for l in range(L):
+                run(l)
+            for l in range(L):                                   # compared on the device, in stream order: no host sync
+                bad += (outs[l].view(torch.int16) != ref[l]).sum()
+        torch.cuda.synchronize()
+        assert int(bad) == 0, f"{int(bad)} values differ from the first pass"
+        assert ctx.poll_status() == 0
+    finally:
+        rs.close()
+        ctx.close()
