@@ -414,6 +414,9 @@ __device__ __forceinline__ uint32_t mapa_u32(uint32_t addr, uint32_t rank) {   /
   return r;
 }
 __device__ __forceinline__ void cluster_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
+// the exit barrier of the cluster shape orders no data (it only keeps every CTA's shared memory alive until all pushes have
+// landed, which the receivers have observed through their mbarriers): no release fence
+__device__ __forceinline__ void cluster_arrive_relaxed() { asm volatile("barrier.cluster.arrive.relaxed.aligned;" ::: "memory"); }
 __device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
 // bulk copy own shared memory -> a peer CTA's shared memory, completing (bytes) on the PEER's mbarrier
 __device__ __forceinline__ void bulk_push_dsmem(uint32_t dst_cluster, uint32_t src_cta, uint32_t bytes, uint32_t bar_cluster) {
@@ -959,7 +962,7 @@ __device__ __forceinline__ void attn_softmax(const AttnParams& p, AttnShared<fal
     WF_PROBE_AT(7, warp == 0 && lane == 0);
     mbar_wait(smem_u32(&sh.cl_bar), 0);                        // every slice of this CTA's rows has landed
     WF_PROBE_AT(8, warp == 0 && lane == 0);
-    cluster_arrive();                                          // "what was pushed to me has landed": see the kernel's epilogue
+    cluster_arrive_relaxed();                                  // "what was pushed to me has landed": see the kernel's epilogue
     attn_cluster_reduce<D>(p, sh, recv_s, grp * 128 + stid);
     WF_PROBE_AT(9, warp == 0 && lane == 0);
     cluster_wait();
@@ -1472,7 +1475,7 @@ __global__ void __launch_bounds__(AT_THREADS, 1) wf_verify_attn_kernel(const Att
     }
     // cluster mode: nobody leaves while a copy it pushed may still be reading its shared memory: a CTA arrives once
     // everything pushed TO it has landed (the softmax warps of a running CTA do so inside attn_softmax), and all wait
-    if (sh.cl > 1 && !(run && warp < 8)) { cluster_arrive(); cluster_wait(); }
+    if (sh.cl > 1 && !(run && warp < 8)) { cluster_arrive_relaxed(); cluster_wait(); }
   }
   tc_fence_before();
   __syncthreads();
