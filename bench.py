@@ -776,7 +776,7 @@ def main():
     ap.add_argument("--sub-workloads", default="cfg2,cfg3,cfg4",
                     help="comma-separated workloads reported as compact per_config sub-records of the same line ('' = none)")
     ap.add_argument("--sub-steps", type=int, default=30)
-    ap.add_argument("--sub-e2e-steps", type=int, default=10)
+    ap.add_argument("--sub-e2e-steps", type=int, default=30)
     ap.add_argument("--slots", type=int, default=16, help="round slots of the cyclic schedule (distinct inputs and plans)")
     ap.add_argument("--e2e-steps", type=int, default=30)
     ap.add_argument("--attn-early", type=int, default=1, choices=[0, 1],
