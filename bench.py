@@ -571,6 +571,8 @@ def measure(ctx, wf, key, args, rank, world, local, main):
                     "final_token_us_per_round": final_us, "flush_us_per_round": lazy_us - final_us,
                     "eager_kv_us_per_round": eager_us - 1e3 * eager_final_ms / leg_steps,
                     "switch_us_per_round": lazy_us - active_us, "share_of_round": lazy_us / round_us,
+                    "flush_share_of_round": (lazy_us - final_us) / round_us,
+                    "final_token_share_of_round": final_us / round_us,
                     "switch_share_of_round": (lazy_us - active_us) / round_us, "eager_share_of_round": eager_catch_ms / eager_ms,
                     "eager_rounds_per_s": leg_steps / (eager_ms * 1e-3), "lazy_rounds_per_s": leg_steps / (lazy_leg_ms * 1e-3),
                     "leg_steps": leg_steps,
@@ -578,7 +580,8 @@ def measure(ctx, wf, key, args, rank, world, local, main):
                             "(Lazy Catch-up off, PAPER.md Table 3 baseline); active_append = only the active drafter's own append "
                             "(reading C22: drafting cost, not switching cost); switch = lazy - active_append (derived); "
                             "final_token = wf_final_token_full for the sequences that switched to the AR drafter (PAPER.md:119), "
-                            "inside lazy and eager alike; flush = lazy - final_token is what Lazy Catch-up costs per round and "
+                            "inside lazy and eager alike; flush = lazy - final_token is what Lazy Catch-up costs per round (rows (c) + (d) of "
+                            "north_star: flush_share_of_round is the figure its 7 % bar is about; share_of_round also counts f3) and "
                             "eager_kv = eager - its final token what the naive scheme costs (PAPER.md Table 3)"},
         "roofline": {"bound": "hbm", "kernel": "wf_verify_attn_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
                      "frac": achieved / peak, "peak_source": peak_src, "traffic": traffic, "traffic_source": traffic_src,
