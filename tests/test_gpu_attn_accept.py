@@ -272,6 +272,25 @@ def test_attn_blocks_wider_than_64_rows_per_kv_head(wf):
         assert max_abs <= ATTN_MAX_ABS and rel <= ATTN_REL_L2, (Hq, Hkv, D, max_abs, rel)
 
 
+def test_attn_wide_blocks_and_plain_blocks_in_early_kv_mode():
+    """The same definition with wf_ctx_set_attn_early_kv on (a context of its own): a wide block (its mask kernel is the
+    launch's predecessor), 8B-class ragged shapes with NaN poison, and a cluster-shaped batch-1 call."""
+    import torch
+    from paper_2606_07710_b200 import binding
+    ctx = binding.Ctx(0)
+    ctx.set_attn_early_kv(1)
+    try:
+        for (Hq, Hkv, D, q_lens, ctx_lens) in [(64, 8, 128, [16, 9, 0, 1], [700, 2050, 33, 5]),
+                                               (32, 8, 128, [16, 8, 16, 0, 8], [3000, 17, 1500, 640, 255]),
+                                               (32, 8, 128, [16], [4096])]:
+            max_abs, rel = _attn_case((binding, ctx), ctx_lens, q_lens, Hq, Hkv, D, seed=91 + len(q_lens), poison=True)
+            assert max_abs <= ATTN_MAX_ABS and rel <= ATTN_REL_L2, (Hq, Hkv, D, max_abs, rel)
+        torch.cuda.synchronize()
+        assert ctx.poll_status() == 0
+    finally:
+        ctx.close()
+
+
 def test_attn_many_short_sequences_with_empty_blocks(wf):
     """200 sequences with contexts 0..40 and blocks of 0, 1, 8 or 16 rows: far more (sequence, kv head) pairs than CTAs,
     every range holds many one-tile segments, empty blocks in between (the weighted walker must skip them)."""
