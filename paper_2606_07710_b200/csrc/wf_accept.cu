@@ -173,48 +173,64 @@ wf_accept_kernel(const float* __restrict__ logits, int V, int n_chunks, const in
   // ---- finalise sequence b (one CTA) ----
   __shared__ int s_g[ACC_MAX_Q];
   __shared__ int s_a;
-  for (int r = wid; r < q_b; r += ACC_THREADS / 32) {     // one warp per row: argmax over slices
-    float rm = -INFINITY;
-    int ri = 0x7fffffff;
-    for (int c = lane; c < n_chunks; c += 32) {
-      const AccPartial* pp = &partials[(prow0 + r) * n_chunks + c];
-      const float pm = __ldcg(&pp->m);
-      const int pi = __ldcg(&pp->idx);
-      argmax_merge(rm, ri, pm, pi);
-    }
-#pragma unroll
-    for (int d = 16; d > 0; d >>= 1) {
-      float om = __shfl_xor_sync(0xffffffffu, rm, d);
-      int oi = __shfl_xor_sync(0xffffffffu, ri, d);
-      argmax_merge(rm, ri, om, oi);
-    }
-    if (lane == 0) s_g[r] = ri;
-  }
+  __shared__ float s_M[ACC_MAX_Q];                         // per row: max over the slices, and relative to it ...
+  __shared__ double s_Z[ACC_MAX_Q], s_S[ACC_MAX_Q];        // ... Z = sum e^{z-M} and S = sum e^{z-M}(z-M), combined in fp64
+  __shared__ int s_ok[ACC_MAX_Q];
   __shared__ int s_row;                                    // the row whose logits give the bonus token and the entropy
   __shared__ int s_par[ACC_MAX_Q], s_tok[ACC_MAX_Q];
   if (tid < q_b) { s_par[tid] = parent ? parent[r0 + tid] : tid - 1; s_tok[tid] = draft_tokens[r0 + tid]; }   // one round trip for all
-  __syncthreads();
-  __shared__ float s_M[ACC_MAX_Q];
-  __shared__ double s_Z[ACC_MAX_Q];
-  __shared__ int s_ok[ACC_MAX_Q];
-  if (smp.u_accept) {
-    // ---- speculative sampling (S3): p_{j-1}(x_j) from row j-1's slice partials and one gathered logit ----
-    for (int r = wid; r < q_b; r += ACC_THREADS / 32) {   // one warp per row: (max, Z) over the slices
-      const AccPartial* pr = &partials[(prow0 + r) * n_chunks];
-      float gm = -INFINITY;
-      for (int c = lane; c < n_chunks; c += 32) gm = fmaxf(gm, __ldcg(&pr[c].m));
+  // One pass over the slice partials (16 bytes each, one load), one warp per row and TWO rows of a warp in flight: per row
+  // the argmax g_i AND (M, Z, S), so that neither the acceptance test of the sampling mode nor the entropy of the last
+  // accepted row (whichever row that turns out to be) needs another round trip to L2.  (The finalise used to make three
+  // dependent ones: argmax, then max, then Z and S of row a.)
+  for (int rb = wid; rb < q_b; rb += 2 * (ACC_THREADS / 32)) {
+    const int rows[2] = {rb, rb + ACC_THREADS / 32};
+    float4 first[2];
 #pragma unroll
-      for (int d = 16; d > 0; d >>= 1) gm = fmaxf(gm, __shfl_xor_sync(0xffffffffu, gm, d));
-      double Zd = 0.0;
-      for (int c = lane; c < n_chunks; c += 32) {
-        const float pm = __ldcg(&pr[c].m);
-        if (pm > -INFINITY) Zd += (double)__ldcg(&pr[c].Z) * exp((double)pm - (double)gm);
+    for (int u = 0; u < 2; ++u) {
+      first[u] = make_float4(-INFINITY, __int_as_float(0x7fffffff), 0.f, 0.f);
+      if (rows[u] < q_b && lane < n_chunks)
+        first[u] = __ldcg(reinterpret_cast<const float4*>(&partials[(prow0 + rows[u]) * n_chunks + lane]));
+    }
+#pragma unroll
+    for (int u = 0; u < 2; ++u) {
+      const int r = rows[u];
+      if (r >= q_b) continue;                              // whole warp together
+      const AccPartial* pr = &partials[(prow0 + r) * n_chunks];
+      float rm = first[u].x;
+      int ri = __float_as_int(first[u].y);
+      for (int c = lane + 32; c < n_chunks; c += 32) {      // vocabularies of more than 32 slices
+        const float4 x = __ldcg(reinterpret_cast<const float4*>(&pr[c]));
+        argmax_merge(rm, ri, x.x, __float_as_int(x.y));
       }
 #pragma unroll
-      for (int d = 16; d > 0; d >>= 1) Zd += __shfl_xor_sync(0xffffffffu, Zd, d);
-      if (lane == 0) { s_M[r] = gm; s_Z[r] = Zd; }
+      for (int d = 16; d > 0; d >>= 1) {
+        float om = __shfl_xor_sync(0xffffffffu, rm, d);
+        int oi = __shfl_xor_sync(0xffffffffu, ri, d);
+        argmax_merge(rm, ri, om, oi);
+      }
+      const float gm = rm;                                 // the row maximum (every lane)
+      double Zd = 0.0, Sd = 0.0;
+      for (int c = lane; c < n_chunks; c += 32) {
+        const float4 x = c == lane ? first[u] : __ldcg(reinterpret_cast<const float4*>(&pr[c]));
+        if (x.x > -INFINITY) {
+          const double dm = (double)x.x - (double)gm;
+          const double w = exp(dm);
+          Zd += (double)x.z * w;
+          Sd += w * ((double)x.w + dm * (double)x.z);
+        }
+      }
+#pragma unroll
+      for (int d = 16; d > 0; d >>= 1) {
+        Zd += __shfl_xor_sync(0xffffffffu, Zd, d);
+        Sd += __shfl_xor_sync(0xffffffffu, Sd, d);
+      }
+      if (lane == 0) { s_g[r] = ri; s_M[r] = gm; s_Z[r] = Zd; s_S[r] = Sd; }
     }
-    __syncthreads();
+  }
+  __syncthreads();
+  if (smp.u_accept) {
+    // ---- speculative sampling (S3): p_{j-1}(x_j) from row j-1's (M, Z) (the pass above) and one gathered logit ----
     if (tid >= 1 && tid < q_b) {                           // draft j = tid against row j - 1
       const int x = draft_tokens[r0 + tid];
       if (x < 0 || x >= V) {                               // not a token: rejected, never gathered
@@ -265,30 +281,10 @@ wf_accept_kernel(const float* __restrict__ logits, int V, int n_chunks, const in
     if (lane == 0) { s_a = a; s_row = cur; }
   }
   __syncthreads();
-  if (wid == 0) {                                          // entropy of the last accepted row, fp64 combine (C3, C4, T4)
+  if (tid == 0) {                                          // entropy of the last accepted row from its fp64 (Z, S) (C3, C4, T4)
     const int a = s_a, row_a = s_row;
-    const AccPartial* pr = &partials[(prow0 + row_a) * n_chunks];
-    float gm = -INFINITY;
-    for (int c = lane; c < n_chunks; c += 32) gm = fmaxf(gm, __ldcg(&pr[c].m));
-#pragma unroll
-    for (int d = 16; d > 0; d >>= 1) gm = fmaxf(gm, __shfl_xor_sync(0xffffffffu, gm, d));
-    double Zd = 0.0, Sd = 0.0;
-    for (int c = lane; c < n_chunks; c += 32) {
-      const float pm = __ldcg(&pr[c].m);
-      if (pm > -INFINITY) {
-        const double dm = (double)pm - (double)gm;
-        const double w = exp(dm);
-        const double Zc = (double)__ldcg(&pr[c].Z), Sc = (double)__ldcg(&pr[c].S);
-        Zd += Zc * w;
-        Sd += w * (Sc + dm * Zc);
-      }
-    }
-#pragma unroll
-    for (int d = 16; d > 0; d >>= 1) {
-      Zd += __shfl_xor_sync(0xffffffffu, Zd, d);
-      Sd += __shfl_xor_sync(0xffffffffu, Sd, d);
-    }
-    if (lane == 0) {
+    {
+      const double Zd = s_Z[row_a], Sd = s_S[row_a];
       const float H = (float)(log(Zd) - Sd / Zd);
       const float t = tau_is_scalar ? tau[0] : tau[b];
       accept_len[b] = a;
